@@ -1,0 +1,121 @@
+/*
+ * vog.h -- C ABI of libvog: the B200 (sm_100a) hot path of the 1Dx1D semi-Lagrangian
+ * Vlasov-Poisson solver of "Vlasov on GPU (VOG project)", arXiv 1301.5892.
+ * Citations "P:n" are line n of the paper text; "Qn" are the readings listed
+ * in DESIGN.md.
+ *
+ * Data layout.  The phase-space array f is fp32, row-major [Nv][Nx]: f[j*Nx + i] is the
+ * value at (x_i, v_j), x_i = i*L/Nx, v_j = vmin + j*(vmax-vmin)/Nv (Q2).  Both
+ * directions are periodic.  In delta-f mode (feq.n > 0) the array holds
+ * delta f = f - f_eq(v_j); in full-f mode (feq.n == 0) it holds f.
+ *
+ * Conventions.  Every entry point returns a status (VOG_OK == 0, negative on error),
+ * never throws, and never synchronises the host unless stated: work is enqueued on the
+ * plan's CUDA stream.  Argument errors are detected before anything is enqueued.
+ * Pointers named *_dev are caller-owned DEVICE memory (16-byte aligned); pointers named
+ * *_host are caller-owned HOST memory.  The library never frees caller memory.  Plan-owned
+ * scratch is O(Nx + Nv): no N^2 work array exists (contrast P:307, 326).  A plan is not
+ * thread-safe; distinct plans are independent.  There is no CPU fallback anywhere: every
+ * step of the path runs in the library's CUDA kernels.
+ */
+#ifndef VOG_H
+#define VOG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vog_plan_s* vog_plan_t; /* opaque, library-owned */
+
+enum { VOG_OK = 0, VOG_EINVAL = -1, VOG_ENOMEM = -2, VOG_ECUDA = -3, VOG_EUNSUPPORTED = -4 };
+enum { VOG_LAGRANGE = 0, VOG_BSPLINE = 1 }; /* order = polynomial degree: Lagrange odd 1..17, B-spline 3 (Q6) */
+enum { VOG_SPLIT_XVX = 0, VOG_SPLIT_VXV = 1 };
+
+/* f_eq(v) = sum_{g<n} amp[g] * exp(-c[g] * (v - mu[g])^2); n == 0 selects full-f storage.
+ * The paper's f_eq is n=1, amp=1/sqrt(2 pi), mu=0, c=1/2. */
+typedef struct {
+    int n;
+    double amp[4], mu[4], c[4];
+} vog_feq_t;
+
+typedef struct {
+    int Nx, Nv;          /* powers of two in [64, 16384]                         */
+    double L;            /* x in [0, L), periodic; L > 0                          */
+    double vmin, vmax;   /* v in [vmin, vmax), periodic; vmax > vmin              */
+    int kind, order;     /* VOG_LAGRANGE with odd order <= min(17, N-1), or VOG_BSPLINE with order 3 */
+    vog_feq_t feq;       /* delta-f equilibrium                       */
+    int split;           /* VOG_SPLIT_XVX (default, binds BASELINE.json's configs) or VOG_SPLIT_VXV; Q1 */
+} vog_params_t;
+
+/* Create a plan: validates p, allocates the O(Nx+Nv) device scratch (roots of unity, rho, E,
+ * per-line shift records) on the current CUDA device and binds the plan to `cuda_stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream).  Synchronises once.
+ * Errors: VOG_EINVAL (NULL pointer, sizes, L, v-range, feq.n outside [0,4], c[g] <= 0),
+ * VOG_EUNSUPPORTED (kind/order), VOG_ENOMEM, VOG_ECUDA.  *out is set only on VOG_OK. */
+int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_stream);
+
+/* Destroy a plan and free its scratch.  Synchronises the plan's stream.  NULL is VOG_EINVAL. */
+int vog_destroy(vog_plan_t plan);
+
+/* Transport in x over dt: for every velocity row j, the periodic line f[j][:] is
+ * multiplied by the circulant interpolation matrix A of eq (4) for the normalised
+ * displacement beta_j = -v_j*dt/dx, computed as FFT -> symbol -> inverse FFT
+ * inside one fused kernel.  In place; f_dev holds Nx*Nv floats.  dt may be < 0. */
+int vog_advect_x(vog_plan_t plan, float* f_dev, double dt);
+
+/* Transport in v over dt: for every space column i, the periodic line
+ * f[:][i] is shifted by beta_i = -E_i*dt/dv; E_dev holds Nx floats (the total advecting
+ * field).  In delta-f mode the source f_eq(v_j - dt*E_i) - f_eq(v_j) is added, an
+ * evaluation, not an interpolation.  In place. */
+int vog_advect_v(vog_plan_t plan, float* f_dev, const float* E_dev, double dt);
+
+/* Self-consistent field: rho_i = dv * sum_j f[j][i] (of delta f in
+ * delta-f mode, Q11), made zero-mean, then the Fourier solve E^_m = rho^_m / (i k_m),
+ * k_m = 2 pi m / L, with modes 0 and Nx/2 set to 0 (Q12).  E_dev receives Nx floats
+ * with zero mean.  f_dev is not modified. */
+int vog_field(vog_plan_t plan, const float* f_dev, float* E_dev);
+
+/* One Strang step of size dt, in place (Q1).  E_ext_dev (Nx floats, or NULL) is added
+ * to the self-consistent field before every v-advection of the step (for the KEEN drive pass
+ * -E_app).
+ *   VOG_SPLIT_XVX: x(dt/2); E = field(f); v(dt, E + E_ext); x(dt/2).
+ *   VOG_SPLIT_VXV: v(dt/2, E_prev + E_ext); x(dt); E = field(f); v(dt/2, E + E_ext), where
+ *                  E_prev is the field of the previous step (solved from f on the first step).
+ * The self-consistent E solved inside the step stays in the plan: see vog_get_field. */
+int vog_step(vog_plan_t plan, float* f_dev, double dt, const float* E_ext_dev);
+
+/* Copy the self-consistent field of the last vog_step / vog_field of this plan (Nx floats)
+ * into E_dev (device to device, asynchronous).  VOG_EINVAL if none was computed yet. */
+int vog_get_field(vog_plan_t plan, float* E_dev);
+
+/* Lower level (BASELINE.json config 4: "per-line shifts uniform in [-8,8] cells"): apply the
+ * circulant interpolation matrix with an explicit normalised displacement beta (in cells,
+ * fp64, device memory) per line: row j of f is shifted by beta_cells_dev[j] (Nv values) /
+ * column i by beta_cells_dev[i] (Nx values).  No delta-f source.  In place. */
+int vog_shift_x(vog_plan_t plan, float* f_dev, const double* beta_cells_dev);
+int vog_shift_v(vog_plan_t plan, float* f_dev, const double* beta_cells_dev);
+
+/* End-to-end convenience with HOST buffers: copies f_host (Nx*Nv floats) and E_ext_host (Nx
+ * floats or NULL) into a device buffer that the plan allocates on the first call and keeps (the
+ * only O(Nx*Nv) allocation of the library, made only if this call is used), runs `nsteps`
+ * Strang steps with the same E_ext, copies f back into f_host and the last self-consistent E
+ * into E_host (Nx floats, may be NULL), and SYNCHRONISES the stream before returning.
+ * Pinned host memory gives full-rate copies; pageable memory also works. */
+int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
+                 const float* E_ext_host, float* E_host);
+
+/* Tile-shape override for measurements; not needed for normal use.
+ * which: 0 = log2(complex lines per CTA) of the x-kernel, 1 = threads per CTA of the x-kernel,
+ * 2, 3 = the same for the v-kernel.  VOG_EINVAL if the shape does not fit (shared memory, grid). */
+int vog_plan_tune(vog_plan_t plan, int which, int value);
+
+/* Number of kernels the library launched on this plan since creation (for accounting). */
+long long vog_launch_count(vog_plan_t plan);
+
+/* Static description of a status code.  Never NULL. */
+const char* vog_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VOG_H */

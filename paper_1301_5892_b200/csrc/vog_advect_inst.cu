@@ -1,0 +1,46 @@
+// vog_advect_inst.cu -- instantiates the fused advection kernel for ONE line length
+// (compile with -DVOG_N=<64..16384>; the build compiles this file once per length).
+#include "vog_advect.cuh"
+
+#ifndef VOG_N
+#error "compile with -DVOG_N=<line length>"
+#endif
+#define VOG_CAT2(a, b) a##b
+#define VOG_CAT(a, b) VOG_CAT2(a, b)
+
+namespace vog {
+
+template <int N, int SYM, bool VDIR>
+static cudaError_t launch_one(const AdvectArgs& a, int n_tiles, int threads, size_t smem, cudaStream_t st)
+{
+    auto kern = advect_kernel<N, SYM, VDIR>;
+    static size_t smem_set = 0;
+    if (smem > 48 * 1024 && smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    kern<<<n_tiles, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <int N, bool VDIR>
+static cudaError_t launch_sym(const AdvectArgs& a, int sym, int n_tiles, int threads, size_t smem, cudaStream_t st)
+{
+    switch (sym) {
+        case SYM_LAG_D1:  return launch_one<N, SYM_LAG_D1, VDIR>(a, n_tiles, threads, smem, st);
+        case SYM_LAG_D4:  return launch_one<N, SYM_LAG_D4, VDIR>(a, n_tiles, threads, smem, st);
+        case SYM_LAG_D8:  return launch_one<N, SYM_LAG_D8, VDIR>(a, n_tiles, threads, smem, st);
+        case SYM_SPLINE3: return launch_one<N, SYM_SPLINE3, VDIR>(a, n_tiles, threads, smem, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t VOG_CAT(advect_launch_, VOG_N)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,
+                                           size_t smem, cudaStream_t st)
+{
+    return vdir ? launch_sym<VOG_N, true>(a, sym, n_tiles, threads, smem, st)
+                : launch_sym<VOG_N, false>(a, sym, n_tiles, threads, smem, st);
+}
+
+}  // namespace vog

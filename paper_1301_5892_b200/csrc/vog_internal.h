@@ -1,0 +1,41 @@
+// vog_internal.h -- structures shared by the translation units of libvog (product code only).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace vog {
+
+// symbol variants compiled into the advection kernel
+enum { SYM_LAG_D1 = 0, SYM_LAG_D4 = 1, SYM_LAG_D8 = 2, SYM_SPLINE3 = 3, SYM_COUNT = 4 };
+
+// Per-line shift record, REC_WORDS floats, written by the shift-setup kernel (step S1):
+//   [0]      b mod N as int bits                      (integer part of beta)
+//   [1..9]   Lagrange: a_k(1-b*)/(2N), k=0..8         (Everett-form polynomial in s = 2-2cos(theta))
+//            spline:   [1..4] = 3/(2N) * (B(b*+1), B(b*), B(b*-1), B(b*-2))
+//   [10..18] Lagrange: a_k(b*)/(2N)
+//   [19]     v-direction: s_i = E_i * dt (fp32) for the delta-f source; else 0
+constexpr int REC_WORDS = 20;
+
+struct AdvectArgs {
+    float* f;              // [Nv][Nx]
+    int Nx, Nv;
+    const float2* tw;      // N roots e^{-2 pi i k/N} of the advected direction
+    const float* rec;      // [n_lines][REC_WORDS]
+    int lognl;             // log2(complex lines per CTA)
+    int ng;                // number of Gaussians of f_eq (v-direction source), 0 = none
+    const float* feq_tab;  // [ng][Nv]  amp_g exp(-c_g (v_j-mu_g)^2)
+    const float* vmu_tab;  // [ng][Nv]  v_j - mu_g
+    float cg[4];
+};
+
+// launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
+typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,
+                                        size_t smem, cudaStream_t st);
+advect_launch_fn advect_launcher(int N);
+size_t advect_smem_bytes(int N, int lognl);
+
+#define VOG_DECL_LAUNCH(NN) cudaError_t advect_launch_##NN(const AdvectArgs&, int, bool, int, int, size_t, cudaStream_t);
+VOG_DECL_LAUNCH(64) VOG_DECL_LAUNCH(128) VOG_DECL_LAUNCH(256) VOG_DECL_LAUNCH(512) VOG_DECL_LAUNCH(1024)
+VOG_DECL_LAUNCH(2048) VOG_DECL_LAUNCH(4096) VOG_DECL_LAUNCH(8192) VOG_DECL_LAUNCH(16384)
+#undef VOG_DECL_LAUNCH
+
+}  // namespace vog

@@ -1,0 +1,572 @@
+// vog_lib.cu -- C ABI of libvog (include/vog.h): plan, shift-setup kernel (S1), density (S8) and
+// Poisson (S9) kernels, and the Strang driver (S10).  The fused advection kernels (S2-S7) live in
+// vog_advect.cuh.  Product code: no CPU fallback, nothing shared with oracle/.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/vog.h"
+#include "vog_fft.cuh"
+#include "vog_internal.h"
+
+namespace vog {
+
+advect_launch_fn advect_launcher(int N)
+{
+    switch (N) {
+        case 64: return advect_launch_64;
+        case 128: return advect_launch_128;
+        case 256: return advect_launch_256;
+        case 512: return advect_launch_512;
+        case 1024: return advect_launch_1024;
+        case 2048: return advect_launch_2048;
+        case 4096: return advect_launch_4096;
+        case 8192: return advect_launch_8192;
+        case 16384: return advect_launch_16384;
+    }
+    return nullptr;
+}
+
+size_t advect_smem_bytes(int N, int lognl)
+{
+    const size_t NL = (size_t)1 << lognl;
+    return NL * padded_len(N) * sizeof(float2) + 2 * NL * REC_WORDS * sizeof(float);
+}
+
+// ------------------------------------------------------------------------------------------
+// S1: per-line shift records.  beta = -c dt / Delta in fp64; b = floor(beta), b* = beta - b.
+struct SetupArgs {
+    int n_lines, N, mode;      // mode 0: c = v_l (x-advection); 1: c = E_l (+E_ext_l); 2: explicit beta
+    int spline, d;             // interpolation: spline3 or Lagrange degree 2d+1
+    double dt, delta, vmin, dv;
+    const float* E;
+    const float* Eext;
+    const double* beta;
+    float* rec;
+};
+
+__global__ void shift_setup_kernel(const SetupArgs s)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= s.n_lines) return;
+    double beta;
+    float sshift = 0.0f;
+    if (s.mode == 0) {
+        const double v = s.vmin + (double)l * s.dv;
+        beta = -v * s.dt / s.delta;
+    } else if (s.mode == 1) {
+        double e = (double)s.E[l];
+        if (s.Eext) e += (double)s.Eext[l];
+        beta = -e * s.dt / s.delta;
+        sshift = (float)(s.dt * e);
+    } else {
+        beta = s.beta[l];
+    }
+    const double fl = floor(beta);
+    const double t = beta - fl;
+    double bm = fmod(fl, (double)s.N);
+    if (bm < 0.0) bm += (double)s.N;
+    int b = (int)bm;
+    if (b >= s.N) b = 0;
+    float* r = s.rec + (size_t)l * REC_WORDS;
+    const double sc = 1.0 / (2.0 * (double)s.N);
+    r[0] = __int_as_float(b);
+    if (s.spline) {
+        // cardinal cubic B-spline at b*+1, b*, b*-1, b*-2 (= B_0^3(x_{j+b*}), j = 3..0), times 3/(2N)
+        const double u = 1.0 - t;
+        r[1] = (float)(3.0 * sc * (u * u * u / 6.0));
+        r[2] = (float)(3.0 * sc * ((4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0));
+        r[3] = (float)(3.0 * sc * ((1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0));
+        r[4] = (float)(3.0 * sc * (t * t * t / 6.0));
+        for (int k = 5; k < 19; ++k) r[k] = 0.0f;
+    } else {
+        // a_k(t) = (-1)^k C(t+k, 2k+1): a_0 = t, a_k = a_{k-1} (k^2 - t^2) / (2k (2k+1))
+        for (int half = 0; half < 2; ++half) {
+            const double tt = half == 0 ? 1.0 - t : t;
+            double a = tt;
+            float* o = r + 1 + 9 * half;
+            o[0] = (float)(a * sc);
+            for (int k = 1; k <= 8; ++k) {
+                a = (k <= s.d) ? a * ((double)(k * k) - tt * tt) / (double)(2 * k * (2 * k + 1)) : 0.0;
+                o[k] = (float)(a * sc);
+            }
+        }
+    }
+    r[19] = sshift;
+}
+
+// ------------------------------------------------------------------------------------------
+// S8: rho partial sums.  grid (Nx/32, NBY), 256 threads: a warp covers 4 rows x 32 columns
+// (8 lanes x float4 = one 128 B line per row); the 4 row-lanes are folded by warp shuffles,
+// the 8 warps through shared memory; fp64 accumulation, fixed order => deterministic.
+__global__ void __launch_bounds__(256) density_partial_kernel(const float* __restrict__ f, int Nx, int Nv,
+                                                              int rows_per_block, double* __restrict__ part)
+{
+    __shared__ double red[8][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int xl = lane & 7, rl = lane >> 3;
+    const int col = blockIdx.x * 32 + xl * 4;
+    const int j0 = blockIdx.y * rows_per_block;
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    const float* p = f + (size_t)(j0 + warp * 4 + rl) * Nx + col;
+#pragma unroll 4
+    for (int j = warp * 4 + rl; j < rows_per_block; j += 32) {
+        const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+        s0 += (double)v.x; s1 += (double)v.y; s2 += (double)v.z; s3 += (double)v.w;
+        p += (size_t)32 * Nx;
+    }
+#pragma unroll
+    for (int o = 8; o <= 16; o <<= 1) {
+        s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        s3 += __shfl_xor_sync(0xffffffffu, s3, o);
+    }
+    if (rl == 0) { red[warp][xl * 4 + 0] = s0; red[warp][xl * 4 + 1] = s1; red[warp][xl * 4 + 2] = s2; red[warp][xl * 4 + 3] = s3; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double s = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
+        part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
+    }
+}
+
+// S9: single-CTA Poisson solve.  rho_i = dv * sum of partials (fp64), zero mean in fp64
+// (P:205-211), radix-2 DIF FFT in shared memory (fp32), E^_m = rho^_m / (i k_m) with modes 0 and
+// Nx/2 dropped, DIT inverse, E written to E_a (and E_b if non-NULL).
+__global__ void __launch_bounds__(1024) poisson_kernel(const double* __restrict__ part, int nby, int Nx, int logNx,
+                                                       double dv, double L, const float2* __restrict__ tw,
+                                                       double* __restrict__ rho, float* __restrict__ E_a,
+                                                       float* __restrict__ E_b)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* z = reinterpret_cast<float2*>(smem_raw);
+    __shared__ double wsum[32];
+    __shared__ double mean_s;
+    const int tid = threadIdx.x, T = blockDim.x;
+    double local = 0.0;
+    for (int i = tid; i < Nx; i += T) {
+        double s = 0.0;
+        for (int y = 0; y < nby; ++y) s += part[(size_t)y * Nx + i];
+        s *= dv;
+        rho[i] = s;
+        local += s;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) local += __shfl_xor_sync(0xffffffffu, local, o);
+    if ((tid & 31) == 0) wsum[tid >> 5] = local;
+    __syncthreads();
+    if (tid == 0) {
+        double s = 0.0;
+        for (int w = 0; w < (T >> 5); ++w) s += wsum[w];
+        mean_s = s / (double)Nx;
+    }
+    __syncthreads();
+    const double mean = mean_s;
+    for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rho[i] - mean), 0.0f);
+    __syncthreads();
+    // forward, decimation in frequency: X[m] lands at position bitrev(m)
+    for (int s = Nx >> 1, sh = logNx - 1; s >= 1; s >>= 1, --sh) {
+        const int mul = Nx / (2 * s);
+        for (int idx = tid; idx < (Nx >> 1); idx += T) {
+            const int t = idx & (s - 1);
+            const int i0 = ((idx >> sh) << (sh + 1)) + t;
+            const float2 a = z[i0], b = z[i0 + s];
+            z[i0] = cadd(a, b);
+            z[i0 + s] = cmul(csub(a, b), __ldg(tw + t * mul));
+        }
+        __syncthreads();
+    }
+    for (int p = tid; p < Nx; p += T) {
+        const int m = (int)(__brev((unsigned)p) >> (32 - logNx));
+        float2 v = z[p];
+        if (m == 0 || 2 * m == Nx) v = make_float2(0.0f, 0.0f);
+        else {
+            const int ms = (m <= Nx / 2) ? m : m - Nx;
+            const float ik = (float)(L / (2.0 * 3.14159265358979323846 * (double)ms * (double)Nx));
+            v = make_float2(v.y * ik, -v.x * ik);      // (zr + i zi) / (i k)
+        }
+        z[p] = v;
+    }
+    __syncthreads();
+    for (int s = 1, sh = 0; s <= (Nx >> 1); s <<= 1, ++sh) {
+        const int mul = Nx / (2 * s);
+        for (int idx = tid; idx < (Nx >> 1); idx += T) {
+            const int t = idx & (s - 1);
+            const int i0 = ((idx >> sh) << (sh + 1)) + t;
+            const float2 a = z[i0], b = cmulc(z[i0 + s], __ldg(tw + t * mul));
+            z[i0] = cadd(a, b);
+            z[i0 + s] = csub(a, b);
+        }
+        __syncthreads();
+    }
+    for (int i = tid; i < Nx; i += T) {
+        const float e = z[i].x;
+        E_a[i] = e;
+        if (E_b) E_b[i] = e;
+    }
+}
+
+}  // namespace vog
+
+// ==========================================================================================
+struct vog_plan_s {
+    vog_params_t p;
+    cudaStream_t st;
+    int sym, d;                 // symbol variant and Lagrange half-width
+    float2 *tw_x, *tw_v;        // roots of unity of order Nx / Nv
+    float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
+    double* part;               // density partials [nby][Nx]
+    double* rho;                // [Nx]
+    float* E_self;              // [Nx] last self-consistent field
+    float *feq_tab, *vmu_tab;   // [ng][Nv]
+    int nby;
+    int lognl_x, lognl_v, thr_x, thr_v;
+    bool E_valid;
+    bool recx_valid; double recx_dt;
+    long long launches;
+    float* f_buf;               // only for vog_run_host
+    float* ext_buf;
+};
+
+using namespace vog;
+
+static int ilog2i(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+static bool pow2_in_range(int n) { return n >= 64 && n <= 16384 && (n & (n - 1)) == 0; }
+
+static void fill_roots(std::vector<float2>& h, int N)
+{
+    h.resize(N);
+    for (int k = 0; k < N; ++k) {
+        // e^{-2 pi i k / N}, exact on the axes, long double elsewhere, rounded once
+        float c, s;
+        if ((4 * k) % N == 0) {
+            const int q = (4 * k) / N;
+            c = q == 0 ? 1.f : (q == 2 ? -1.f : 0.f);
+            s = q == 1 ? 1.f : (q == 3 ? -1.f : 0.f);
+        } else {
+            const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)N;
+            c = (float)cosl(a);
+            s = (float)sinl(a);
+        }
+        h[k] = make_float2(c, -s);
+    }
+}
+
+// default tile shape: NL complex lines per CTA and threads per CTA (kernel section)
+static void default_tile(int N, int n_lines, bool vdir, int* lognl, int* threads)
+{
+    const int pairs = n_lines / 2;
+    int nl;
+    if (N >= 16384) { *lognl = 0; *threads = 512; return; }
+    if (vdir) {
+        nl = N <= 2048 ? 4 : (N <= 4096 ? 2 : 1);
+    } else {
+        nl = 8192 / N;
+        if (nl < 1) nl = 1;
+        if (nl > 16) nl = 16;
+    }
+    while (nl > 1 && pairs / nl < 592) nl >>= 1;
+    if (nl > pairs) nl = pairs;
+    int t = nl * (N / 32);
+    if (t < 64) t = 64;
+    if (t > 256) t = 256;
+    *lognl = ilog2i(nl);
+    *threads = t;
+}
+
+extern "C" const char* vog_strerror(int status)
+{
+    switch (status) {
+        case VOG_OK: return "ok";
+        case VOG_EINVAL: return "invalid argument";
+        case VOG_ENOMEM: return "out of device memory";
+        case VOG_ECUDA: return "CUDA error";
+        case VOG_EUNSUPPORTED: return "unsupported interpolation kind/order";
+    }
+    return "unknown status";
+}
+
+static void free_plan(vog_plan_s* P)
+{
+    if (!P) return;
+    cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
+    cudaFree(P->part); cudaFree(P->rho); cudaFree(P->E_self);
+    cudaFree(P->feq_tab); cudaFree(P->vmu_tab); cudaFree(P->f_buf); cudaFree(P->ext_buf);
+    delete P;
+}
+
+extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_stream)
+{
+    if (!out || !p) return VOG_EINVAL;
+    if (!pow2_in_range(p->Nx) || !pow2_in_range(p->Nv)) return VOG_EINVAL;
+    if (!(p->L > 0.0) || !(p->vmax > p->vmin) || !std::isfinite(p->L) || !std::isfinite(p->vmin) || !std::isfinite(p->vmax))
+        return VOG_EINVAL;
+    if (p->feq.n < 0 || p->feq.n > 4) return VOG_EINVAL;
+    for (int g = 0; g < p->feq.n; ++g)
+        if (!(p->feq.c[g] > 0.0) || !std::isfinite(p->feq.amp[g]) || !std::isfinite(p->feq.mu[g])) return VOG_EINVAL;
+    if (p->split != VOG_SPLIT_XVX && p->split != VOG_SPLIT_VXV) return VOG_EINVAL;
+    int sym, d = 0;
+    const int nmin = p->Nx < p->Nv ? p->Nx : p->Nv;
+    if (p->kind == VOG_LAGRANGE) {
+        if (p->order < 1 || p->order > 17 || (p->order & 1) == 0 || p->order > nmin - 1) return VOG_EUNSUPPORTED;
+        d = (p->order - 1) / 2;
+        sym = d <= 1 ? SYM_LAG_D1 : (d <= 4 ? SYM_LAG_D4 : SYM_LAG_D8);
+    } else if (p->kind == VOG_BSPLINE) {
+        if (p->order != 3) return VOG_EUNSUPPORTED;
+        sym = SYM_SPLINE3;
+    } else {
+        return VOG_EUNSUPPORTED;
+    }
+    vog_plan_s* P = new (std::nothrow) vog_plan_s();
+    if (!P) return VOG_ENOMEM;
+    std::memset(P, 0, sizeof(*P));
+    P->p = *p;
+    P->st = (cudaStream_t)cuda_stream;
+    P->sym = sym;
+    P->d = d;
+    const int Nx = p->Nx, Nv = p->Nv, ng = p->feq.n;
+    // density partial rows: enough blocks to fill the chip, at least 32 rows per block
+    int nby = 1;
+    while ((Nx / 32) * nby < 592 && Nv / (nby * 2) >= 32) nby *= 2;
+    P->nby = nby;
+    default_tile(Nx, Nv, false, &P->lognl_x, &P->thr_x);
+    default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
+    cudaError_t e = cudaSuccess;
+    auto alloc = [&](void** ptr, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(ptr, bytes ? bytes : 16); };
+    alloc((void**)&P->tw_x, sizeof(float2) * Nx);
+    alloc((void**)&P->tw_v, sizeof(float2) * Nv);
+    alloc((void**)&P->rec_x, sizeof(float) * REC_WORDS * Nv);
+    alloc((void**)&P->rec_v, sizeof(float) * REC_WORDS * Nx);
+    alloc((void**)&P->part, sizeof(double) * nby * Nx);
+    alloc((void**)&P->rho, sizeof(double) * Nx);
+    alloc((void**)&P->E_self, sizeof(float) * Nx);
+    alloc((void**)&P->feq_tab, sizeof(float) * (ng ? ng : 1) * Nv);
+    alloc((void**)&P->vmu_tab, sizeof(float) * (ng ? ng : 1) * Nv);
+    if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
+    std::vector<float2> h;
+    fill_roots(h, Nx);
+    e = cudaMemcpyAsync(P->tw_x, h.data(), sizeof(float2) * Nx, cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
+    fill_roots(h, Nv);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->tw_v, h.data(), sizeof(float2) * Nv, cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
+    if (ng > 0 && e == cudaSuccess) {
+        std::vector<float> ft((size_t)ng * Nv), vt((size_t)ng * Nv);
+        const double dv = (p->vmax - p->vmin) / (double)Nv;
+        for (int g = 0; g < ng; ++g)
+            for (int j = 0; j < Nv; ++j) {
+                const double v = p->vmin + (double)j * dv;
+                const double u = v - p->feq.mu[g];
+                ft[(size_t)g * Nv + j] = (float)(p->feq.amp[g] * std::exp(-p->feq.c[g] * u * u));
+                vt[(size_t)g * Nv + j] = (float)u;
+            }
+        e = cudaMemcpyAsync(P->feq_tab, ft.data(), sizeof(float) * ft.size(), cudaMemcpyHostToDevice, P->st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(P->vmu_tab, vt.data(), sizeof(float) * vt.size(), cudaMemcpyHostToDevice, P->st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
+    }
+    if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return VOG_ECUDA; }
+    *out = P;
+    return VOG_OK;
+}
+
+extern "C" int vog_destroy(vog_plan_t P)
+{
+    if (!P) return VOG_EINVAL;
+    cudaStreamSynchronize(P->st);
+    free_plan(P);
+    return VOG_OK;
+}
+
+// internal tuning hook (documented in DESIGN.md; not part of the paper-facing API):
+// which: 0 = log2(NL) x, 1 = threads x, 2 = log2(NL) v, 3 = threads v, 4 = density row blocks
+extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
+{
+    if (!P) return VOG_EINVAL;
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    switch (which) {
+        case 0: if (value < 0 || (2 << value) > Nv || advect_smem_bytes(Nx, value) > 227 * 1024) return VOG_EINVAL; P->lognl_x = value; break;
+        case 1: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_x = value; break;
+        case 2: if (value < 0 || (2 << value) > Nx || advect_smem_bytes(Nv, value) > 227 * 1024) return VOG_EINVAL; P->lognl_v = value; break;
+        case 3: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_v = value; break;
+        default: return VOG_EINVAL;
+    }
+    return VOG_OK;
+}
+
+static int cuda_status(cudaError_t e) { return e == cudaSuccess ? VOG_OK : VOG_ECUDA; }
+
+static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, const float* E, const float* Eext,
+                             const double* beta)
+{
+    SetupArgs s;
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    s.n_lines = vdir ? Nx : Nv;
+    s.N = vdir ? Nv : Nx;
+    s.mode = mode;
+    s.spline = P->sym == SYM_SPLINE3;
+    s.d = P->d;
+    s.dt = dt;
+    s.dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    s.delta = vdir ? s.dv : P->p.L / (double)Nx;
+    s.vmin = P->p.vmin;
+    s.E = E; s.Eext = Eext; s.beta = beta;
+    s.rec = vdir ? P->rec_v : P->rec_x;
+    shift_setup_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
+    P->launches++;
+    return cudaGetLastError();
+}
+
+static cudaError_t run_advect(vog_plan_s* P, float* f, bool vdir, bool source)
+{
+    AdvectArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    const int N = vdir ? Nv : Nx, n_lines = vdir ? Nx : Nv;
+    const int lognl = vdir ? P->lognl_v : P->lognl_x;
+    a.f = f; a.Nx = Nx; a.Nv = Nv;
+    a.tw = vdir ? P->tw_v : P->tw_x;
+    a.rec = vdir ? P->rec_v : P->rec_x;
+    a.lognl = lognl;
+    a.ng = (vdir && source) ? P->p.feq.n : 0;
+    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab;
+    for (int g = 0; g < 4; ++g) a.cg[g] = g < P->p.feq.n ? (float)P->p.feq.c[g] : 0.0f;
+    const int n_tiles = n_lines / (2 << lognl);
+    advect_launch_fn fn = advect_launcher(N);
+    if (!fn) return cudaErrorInvalidValue;
+    P->launches++;
+    return fn(a, P->sym, vdir, n_tiles, vdir ? P->thr_v : P->thr_x, advect_smem_bytes(N, lognl), P->st);
+}
+
+static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
+{
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    dim3 grid(Nx / 32, P->nby);
+    density_partial_kernel<<<grid, 256, 0, P->st>>>(f, Nx, Nv, Nv / P->nby, P->part);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const size_t smem = sizeof(float2) * Nx;
+    static bool attr = false;
+    if (!attr) {
+        e = cudaFuncSetAttribute(poisson_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * (int)sizeof(float2));
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    const int T = Nx >= 2048 ? 1024 : Nx / 2;
+    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    poisson_kernel<<<1, T, smem, P->st>>>(P->part, P->nby, Nx, ilog2i(Nx), dv, P->p.L, P->tw_x, P->rho, P->E_self, E_out);
+    P->launches += 2;
+    P->E_valid = true;
+    return cudaGetLastError();
+}
+
+static cudaError_t ensure_recx(vog_plan_s* P, double dt)
+{
+    if (P->recx_valid && P->recx_dt == dt) return cudaSuccess;
+    cudaError_t e = run_setup(P, false, 0, dt, nullptr, nullptr, nullptr);
+    P->recx_valid = (e == cudaSuccess);
+    P->recx_dt = dt;
+    return e;
+}
+
+extern "C" int vog_advect_x(vog_plan_t P, float* f_dev, double dt)
+{
+    if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
+    cudaError_t e = ensure_recx(P, dt);
+    if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+    return cuda_status(e);
+}
+
+extern "C" int vog_advect_v(vog_plan_t P, float* f_dev, const float* E_dev, double dt)
+{
+    if (!P || !f_dev || !E_dev || !std::isfinite(dt)) return VOG_EINVAL;
+    cudaError_t e = run_setup(P, true, 1, dt, E_dev, nullptr, nullptr);
+    if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+    return cuda_status(e);
+}
+
+extern "C" int vog_shift_x(vog_plan_t P, float* f_dev, const double* beta)
+{
+    if (!P || !f_dev || !beta) return VOG_EINVAL;
+    P->recx_valid = false;
+    cudaError_t e = run_setup(P, false, 2, 0.0, nullptr, nullptr, beta);
+    if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+    return cuda_status(e);
+}
+
+extern "C" int vog_shift_v(vog_plan_t P, float* f_dev, const double* beta)
+{
+    if (!P || !f_dev || !beta) return VOG_EINVAL;
+    cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
+    if (e == cudaSuccess) e = run_advect(P, f_dev, true, false);
+    return cuda_status(e);
+}
+
+extern "C" int vog_field(vog_plan_t P, const float* f_dev, float* E_dev)
+{
+    if (!P || !f_dev || !E_dev) return VOG_EINVAL;
+    return cuda_status(run_field(P, f_dev, E_dev));
+}
+
+extern "C" int vog_get_field(vog_plan_t P, float* E_dev)
+{
+    if (!P || !E_dev || !P->E_valid) return VOG_EINVAL;
+    return cuda_status(cudaMemcpyAsync(E_dev, P->E_self, sizeof(float) * P->p.Nx, cudaMemcpyDeviceToDevice, P->st));
+}
+
+extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ext_dev)
+{
+    if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
+    cudaError_t e;
+    if (P->p.split == VOG_SPLIT_XVX) {
+        e = ensure_recx(P, 0.5 * dt);
+        if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+        if (e == cudaSuccess) e = run_field(P, f_dev, nullptr);
+        if (e == cudaSuccess) e = run_setup(P, true, 1, dt, P->E_self, E_ext_dev, nullptr);
+        if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+        if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+    } else {
+        e = cudaSuccess;
+        if (!P->E_valid) e = run_field(P, f_dev, nullptr);
+        if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
+        if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+        if (e == cudaSuccess) e = ensure_recx(P, dt);
+        if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+        if (e == cudaSuccess) e = run_field(P, f_dev, nullptr);
+        if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
+        if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+    }
+    return cuda_status(e);
+}
+
+extern "C" int vog_run_host(vog_plan_t P, float* f_host, double dt, int nsteps, const float* E_ext_host, float* E_host)
+{
+    if (!P || !f_host || nsteps < 0 || !std::isfinite(dt)) return VOG_EINVAL;
+    const size_t nf = (size_t)P->p.Nx * P->p.Nv;
+    cudaError_t e = cudaSuccess;
+    if (!P->f_buf) {
+        e = cudaMalloc((void**)&P->f_buf, sizeof(float) * nf);
+        if (e != cudaSuccess) { cudaGetLastError(); return VOG_ENOMEM; }
+        e = cudaMalloc((void**)&P->ext_buf, sizeof(float) * P->p.Nx);
+        if (e != cudaSuccess) { cudaGetLastError(); return VOG_ENOMEM; }
+    }
+    e = cudaMemcpyAsync(P->f_buf, f_host, sizeof(float) * nf, cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess && E_ext_host)
+        e = cudaMemcpyAsync(P->ext_buf, E_ext_host, sizeof(float) * P->p.Nx, cudaMemcpyHostToDevice, P->st);
+    if (e != cudaSuccess) return VOG_ECUDA;
+    for (int s = 0; s < nsteps; ++s) {
+        int rc = vog_step(P, P->f_buf, dt, E_ext_host ? P->ext_buf : nullptr);
+        if (rc != VOG_OK) return rc;
+    }
+    e = cudaMemcpyAsync(f_host, P->f_buf, sizeof(float) * nf, cudaMemcpyDeviceToHost, P->st);
+    if (e == cudaSuccess && E_host && P->E_valid)
+        e = cudaMemcpyAsync(E_host, P->E_self, sizeof(float) * P->p.Nx, cudaMemcpyDeviceToHost, P->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
+    return cuda_status(e);
+}
+
+extern "C" long long vog_launch_count(vog_plan_t P) { return P ? P->launches : -1; }

@@ -1,0 +1,311 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the oracle,
+element by element on the same seeded inputs.  Run with `-m gpu` on the B200 box.
+
+Tolerance (BASELINE.json north_star): per advection, max|f_gpu - f_oracle| <= 2e-6 * max|f|
+where f is the stored array handed in.  The oracle always receives the GPU's
+own fp32 inputs promoted to double.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1301_5892_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+LAG, SPL = 0, 1
+TOL = 2e-6
+ALL_KINDS = [(LAG, 1), (LAG, 3), (LAG, 5), (LAG, 9), (LAG, 13), (LAG, 17), (SPL, 3)]
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return t
+
+
+@pytest.fixture(scope="module")
+def vog():
+    from paper_1301_5892_b200 import vog as v
+    v.lib()      # fails loudly if the extension is missing
+    return v
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _shifts(n, seed):
+    beta = inputs.uniform_shifts(n, seed)
+    # salt in the degenerate cases: integer, zero, negative fraction, huge, just-below-integer
+    special = [0.0, 3.0, -5.0, -0.25, 0.999999, 1e-9, -1e-9, 123456.75, -98765.5, 7.5]
+    beta[: len(special)] = special
+    return beta
+
+
+def _check(out, ref, scale, tol=TOL):
+    err = np.abs(out.astype(np.float64) - ref).max()
+    assert err <= tol * scale, "max err %.3e > %.1e * %.3e" % (err, tol, scale)
+    return err
+
+
+# ------------------------------------------------------------------ per-advection parity (config 4 recipe)
+@pytest.mark.parametrize("kind,order", ALL_KINDS)
+@pytest.mark.parametrize("Nx,Nv", [(64, 64), (128, 256), (512, 512), (1024, 128), (256, 2048)])
+def test_shift_parity_both_directions(torch, vog, oracle, Nx, Nv, kind, order):
+    f = inputs.uniform_grid(Nx, Nv)
+    plan = vog.Plan(Nx, Nv, 4 * math.pi, -6.0, 6.0, kind, order)
+    bx, bv = _shifts(Nv, 11), _shifts(Nx, 12)
+    fd = _dev(torch, f)
+    plan.shift_x(fd, _dev(torch, bx))
+    torch.cuda.synchronize()
+    _check(fd.cpu().numpy(), oracle.shift_x(f, bx, kind, order), np.abs(f).max())
+    fd = _dev(torch, f)
+    plan.shift_v(fd, _dev(torch, bv))
+    torch.cuda.synchronize()
+    _check(fd.cpu().numpy(), oracle.shift_v(f, bv, kind, order), np.abs(f).max())
+    plan.destroy()
+
+
+@pytest.mark.parametrize("N", [4096, 8192, 16384])
+@pytest.mark.parametrize("kind,order", [(LAG, 17), (SPL, 3), (LAG, 3)])
+def test_shift_parity_large_lines_sampled(torch, vog, oracle, N, kind, order):
+    """Line lengths up to the maximum (16384) on a thin grid; every line compared."""
+    for Nx, Nv in ((N, 64), (64, N)):
+        f = inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + N)
+        plan = vog.Plan(Nx, Nv, 10.0, -5.0, 5.0, kind, order)
+        bx, bv = _shifts(Nv, 21), _shifts(Nx, 22)
+        fd = _dev(torch, f)
+        plan.shift_x(fd, _dev(torch, bx))
+        _check(fd.cpu().numpy(), oracle.shift_x(f, bx, kind, order), 1.0)
+        fd = _dev(torch, f)
+        plan.shift_v(fd, _dev(torch, bv))
+        _check(fd.cpu().numpy(), oracle.shift_v(f, bv, kind, order), 1.0)
+        plan.destroy()
+
+
+def test_integer_shift_and_zero_dt(torch, vog):
+    """b* = 0: an exact roll up to FFT rounding; dt = 0: identity up to rounding."""
+    Nx = Nv = 256
+    f = inputs.uniform_grid(Nx, Nv)
+    plan = vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, LAG, 17)
+    fd = _dev(torch, f)
+    plan.shift_x(fd, _dev(torch, np.full(Nv, 5.0)))
+    _check(fd.cpu().numpy(), np.roll(f, -5, axis=1).astype(np.float64), 1.0)
+    fd = _dev(torch, f)
+    plan.shift_v(fd, _dev(torch, np.full(Nx, -3.0)))
+    _check(fd.cpu().numpy(), np.roll(f, 3, axis=0).astype(np.float64), 1.0)
+    fd = _dev(torch, f)
+    plan.advect_x(fd, 0.0)
+    _check(fd.cpu().numpy(), f.astype(np.float64), 1.0)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ physics calls
+@pytest.mark.parametrize("idx,over", [(0, {}), (1, {}), (1, dict(kind=SPL, order=3)),
+                                      (2, dict(Nx=256, Nv=512)), (3, dict(Nx=128, Nv=1024))])
+def test_advect_x_v_field_parity_on_config_shapes(torch, vog, oracle, idx, over):
+    cfg = inputs.config(idx, **over)
+    f = inputs.initial_f(cfg)
+    if np.abs(f).max() == 0:     # KEEN starts from delta f = 0: use a smooth synthetic delta f instead
+        f = 1e-3 * inputs.smooth_grid(cfg.Nx, cfg.Nv)
+    scale = np.abs(f).max()
+    plan = vog.Plan.from_config(cfg)
+    feq = oracle.Feq.make(cfg.feq)
+    # x
+    fd = _dev(torch, f)
+    plan.advect_x(fd, cfg.dt)
+    _check(fd.cpu().numpy(), oracle.advect_x(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order), scale)
+    # field
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    plan.field(_dev(torch, f), Ed)
+    E = Ed.cpu().numpy()
+    Eo = oracle.field(f, cfg.L, cfg.vmin, cfg.vmax)
+    assert np.abs(E - Eo).max() <= 2e-6 * max(np.abs(Eo).max(), 1e-30) + 1e-9 * scale
+    assert abs(E.astype(np.float64).mean()) <= 1e-6 * max(np.abs(Eo).max(), 1e-30)
+    # v, with a field large enough to move several cells, plus the delta-f source
+    rng = np.random.default_rng(5)
+    Ebig = (0.6 * np.sin(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx + 0.3) + 0.05 * rng.normal(size=cfg.Nx)).astype(np.float32)
+    fd = _dev(torch, f)
+    plan.advect_v(fd, _dev(torch, Ebig), cfg.dt)
+    ref = oracle.advect_v(f, Ebig, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq)
+    _check(fd.cpu().numpy(), ref, max(scale, np.abs(ref).max()))
+    plan.destroy()
+
+
+@pytest.mark.parametrize("split", [0, 1])
+@pytest.mark.parametrize("idx", [0, 1])
+def test_one_step_parity(torch, vog, oracle, idx, split):
+    cfg = inputs.config(idx, split=split)
+    f = inputs.initial_f(cfg)
+    plan = vog.Plan.from_config(cfg)
+    feq = oracle.Feq.make(cfg.feq)
+    ext = (0.01 * np.cos(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx)).astype(np.float32)
+    fd = _dev(torch, f)
+    for _ in range(2):
+        plan.step(fd, cfg.dt, _dev(torch, ext))
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    plan.get_field(Ed)
+    fo = f.astype(np.float64)
+    Eo = None
+    for _ in range(2):
+        fo, Eo = oracle.step(fo, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, split, ext, Eo)
+    _check(fd.cpu().numpy(), fo, np.abs(f).max(), tol=3 * TOL * 2)   # 3 advections x 2 steps
+    assert np.abs(Ed.cpu().numpy() - Eo).max() <= 1e-4 * np.abs(Eo).max()
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ full runs: energy history, configs 0-1
+def _gpu_history(torch, vog, cfg, steps):
+    plan = vog.Plan.from_config(cfg)
+    fd = _dev(torch, inputs.initial_f(cfg))
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    hist = np.zeros(steps)
+    for n in range(steps):
+        plan.step(fd, cfg.dt)
+        plan.field(fd, Ed)
+        E = Ed.cpu().numpy().astype(np.float64)
+        hist[n] = 0.5 * cfg.dx * (E ** 2).sum()
+    plan.destroy()
+    return hist, fd.cpu().numpy()
+
+
+def _oracle_history(oracle, cfg, steps):
+    f = inputs.initial_f(cfg).astype(np.float64)
+    feq = oracle.Feq.make(cfg.feq)
+    hist = np.zeros(steps)
+    for n in range(steps):
+        f, _E = oracle.step(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, cfg.split)
+        hist[n] = oracle.electric_energy(oracle.field(f, cfg.L, cfg.vmin, cfg.vmax), cfg.L)
+    return hist, f
+
+
+def test_config0_energy_history_and_landau_rate(torch, vog, oracle):
+    cfg = inputs.config(0)
+    hg, _ = _gpu_history(torch, vog, cfg, cfg.steps)
+    ho, _ = _oracle_history(oracle, cfg, cfg.steps)
+    # "1e-4 relative" = max_n |EE_gpu - EE_oracle| / max_n EE_oracle (reading Q13)
+    assert np.abs(hg - ho).max() / ho.max() <= 1e-4
+    t = cfg.dt * np.arange(1, cfg.steps + 1)
+    pk = [i for i in range(1, cfg.steps - 1) if hg[i] > hg[i - 1] and hg[i] > hg[i + 1]]
+    slope = np.polyfit(t[pk], np.log(hg[pk]), 1)[0]
+    assert abs(0.5 * slope + 0.1533) < 0.004
+
+
+@pytest.mark.parametrize("kind,order", [(LAG, 17), (SPL, 3)])
+def test_config1_energy_history(torch, vog, oracle, kind, order):
+    cfg = inputs.config(1, kind=kind, order=order)
+    hg, fg = _gpu_history(torch, vog, cfg, cfg.steps)
+    ho, fo = _oracle_history(oracle, cfg, cfg.steps)
+    assert np.abs(hg - ho).max() / ho.max() <= 1e-4
+
+
+# ------------------------------------------------------------------ invariants at full size (configs 2-3) and sampled parity
+@pytest.mark.parametrize("idx", [2, 3])
+def test_full_size_sampled_step_parity_and_invariants(torch, vog, oracle, idx):
+    cfg = inputs.config(idx)
+    f0 = inputs.initial_f(cfg)
+    plan = vog.Plan.from_config(cfg)
+    fd = _dev(torch, f0)
+    t = 0.0
+    for n in range(20):
+        ext = _dev(torch, inputs.keen_E_ext(cfg, t + 0.5 * cfg.dt)) if cfg.keen else None
+        plan.step(fd, cfg.dt, ext)
+        t += cfg.dt
+    f = fd.cpu().numpy()
+    assert np.isfinite(f).all()
+    # mass of delta f stays ~0 relative to the mass of f_eq
+    feq_mass = inputs.gaussians(cfg.v(), cfg.feq).sum() * cfg.Nx
+    assert abs(f.astype(np.float64).sum() - f0.astype(np.float64).sum()) / feq_mass < 1e-6
+    # one more x- and v-advection, compared with the oracle on sampled lines
+    scale = max(np.abs(f).max(), 1e-30)
+    rows = np.array([0, 1, cfg.Nv // 2 - 1, cfg.Nv // 2, cfg.Nv - 2, cfg.Nv - 1, 777 % cfg.Nv])
+    cols = np.array([0, 1, cfg.Nx // 2, cfg.Nx - 1, 333 % cfg.Nx, 334 % cfg.Nx])
+    gx = fd.clone()
+    plan.advect_x(gx, cfg.dt)
+    gx = gx.cpu().numpy()
+    v = cfg.v()
+    for j in rows:
+        ref = oracle.advect_line(f[j].astype(np.float64), -v[j] * cfg.dt / cfg.dx, cfg.kind, cfg.order)
+        _check(gx[j], ref, scale)
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    plan.field(fd, Ed)
+    E = Ed.cpu().numpy()
+    gv = fd.clone()
+    plan.advect_v(gv, Ed, cfg.dt)
+    gv = gv.cpu().numpy()
+    feq = oracle.Feq.make(cfg.feq)
+    for i in cols:
+        s = float(E[i]) * cfg.dt
+        ref = oracle.advect_line(f[:, i].astype(np.float64), -float(E[i]) * cfg.dt / cfg.dv, cfg.kind, cfg.order)
+        ref = ref + np.array([oracle.feq_eval(feq, vj - s) - oracle.feq_eval(feq, vj) for vj in v])
+        _check(gv[:, i], ref, scale)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("N", [8192, 16384])
+def test_sweep_shape_sampled_parity(torch, vog, oracle, N):
+    """Config 4 at full size, in the launch configuration bench.py times; sampled lines."""
+    f = inputs.uniform_grid(N, N)
+    plan = vog.Plan(N, N, 1.0, -1.0, 1.0, LAG, 17)
+    bx, bv = inputs.uniform_shifts(N, 31), inputs.uniform_shifts(N, 32)
+    fd = _dev(torch, f)
+    plan.shift_x(fd, _dev(torch, bx))
+    gx = fd.cpu().numpy()
+    del fd
+    for j in (0, 1, 2, N // 2 + 1, N - 1, 4321 % N):
+        _check(gx[j], oracle.advect_line(f[j].astype(np.float64), bx[j], LAG, 17), 1.0)
+    del gx
+    fd = _dev(torch, f)
+    plan.shift_v(fd, _dev(torch, bv))
+    gv = fd.cpu().numpy()
+    del fd
+    for i in (0, 1, 2, 3, N // 2, N - 1, 1234 % N):
+        _check(gv[:, i], oracle.advect_line(np.ascontiguousarray(f[:, i]).astype(np.float64), bv[i], LAG, 17), 1.0)
+    plan.destroy()
+
+
+# ------------------------------------------------------------------ error behaviour and host path
+def test_argument_errors(torch, vog):
+    with pytest.raises(vog.VogError) as e:
+        vog.Plan(100, 64, 1.0, -1, 1)
+    assert e.value.status == vog.EINVAL
+    with pytest.raises(vog.VogError) as e:
+        vog.Plan(64, 64, 1.0, -1, 1, LAG, 4)
+    assert e.value.status == vog.EUNSUPPORTED
+    with pytest.raises(vog.VogError) as e:
+        vog.Plan(64, 64, 1.0, -1, 1, SPL, 5)
+    assert e.value.status == vog.EUNSUPPORTED
+    with pytest.raises(vog.VogError):
+        vog.Plan(64, 64, -1.0, -1, 1)
+    with pytest.raises(vog.VogError):
+        vog.Plan(64, 64, 1.0, 1, 1)
+    plan = vog.Plan(64, 64, 1.0, -1, 1)
+    with pytest.raises(vog.VogError):
+        plan.advect_x(None, 0.1)
+    with pytest.raises(vog.VogError):
+        plan.get_field(torch.empty(64, device="cuda"))
+    assert vog.lib().vog_destroy(None) == vog.EINVAL
+    plan.destroy()
+
+
+def test_run_host_matches_device_steps(torch, vog):
+    cfg = inputs.config(1)
+    f = inputs.initial_f(cfg)
+    plan = vog.Plan.from_config(cfg)
+    fd = _dev(torch, f)
+    for _ in range(3):
+        plan.step(fd, cfg.dt)
+    fh = torch.from_numpy(f.copy()).pin_memory()
+    Eh = torch.empty(cfg.Nx, dtype=torch.float32).pin_memory()
+    n0 = plan.launch_count()
+    plan.run_host(fh, cfg.dt, 3, None, Eh)
+    assert plan.launch_count() > n0
+    assert torch.equal(fh, fd.cpu())
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    plan.get_field(Ed)
+    assert torch.equal(Eh, Ed.cpu())
+    plan.destroy()
