@@ -126,6 +126,9 @@ def main():
     ap.add_argument("--impl", default="vog")
     ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 advection sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sweep-only", action="store_true", help="only the config-4 advection sweep (for profiling)")
+    ap.add_argument("--sizes", default="2048,8192", help="sweep grid sizes N (Nx=Nv=N)")
+    ap.add_argument("--kinds", default="lag17,lag3,spline", help="sweep interpolators: lagN or spline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -148,9 +151,14 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     vog.lib()
 
+    sizes = tuple(int(x) for x in args.sizes.split(","))
+    kinds = tuple((1, 3) if k == "spline" else (0, int(k[3:])) for k in args.kinds.split(","))
+    stream = torch.cuda.Stream()
+    if args.sweep_only:
+        print(json.dumps({"sweep": sweep(torch, vog, stream, _peaks()[0], sizes, kinds)}))
+        return
     cfg = inputs.metric_config()
     cells = cfg.Nx * cfg.Nv
-    stream = torch.cuda.Stream()
     plan = vog.Plan.from_config(cfg, stream=stream)
     f0 = torch.from_numpy(inputs.initial_f(cfg))
     with torch.cuda.stream(stream):
@@ -251,7 +259,7 @@ def main():
 
     # ---- config-4 sweep at the north-star size (8192^2), one x- and one v-advection
     if rank == 0 and not args.no_sweep:
-        out["sweep"] = sweep(torch, vog, stream, peak)
+        out["sweep"] = sweep(torch, vog, stream, peak, sizes, kinds)
     # ---- oracle on the host cores (rank 0, N=1 only)
     if rank == 0 and world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(cfg)
