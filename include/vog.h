@@ -105,8 +105,10 @@ int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
                  const float* E_ext_host, float* E_host);
 
 /* Tile-shape override for measurements; not needed for normal use.
- * which: 0 = log2(complex lines per CTA) of the x-kernel, 1 = threads per CTA of the x-kernel,
- * 2, 3 = the same for the v-kernel.  VOG_EINVAL if the shape does not fit (shared memory, grid). */
+ * which: 2 = log2(complex lines per CTA) of the v-kernel, 3 = threads per CTA of the v-kernel,
+ * 5 = log2(lines per iteration) of the persistent x-kernel, 6 = its threads per CTA (32..128),
+ * 7 = its CTAs per SM (0 = as many as fit).  (0, 1 are accepted and ignored: the round-0 x-kernel.)
+ * VOG_EINVAL if the shape does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 
 /* Number of kernels the library launched on this plan since creation (for accounting). */

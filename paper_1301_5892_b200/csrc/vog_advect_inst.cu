@@ -1,6 +1,7 @@
 // vog_advect_inst.cu -- instantiates the fused advection kernel for ONE line length
 // (compile with -DVOG_N=<64..16384>; the build compiles this file once per length).
 #include "vog_advect.cuh"
+#include "vog_advect_x.cuh"
 
 #ifndef VOG_N
 #error "compile with -DVOG_N=<line length>"
@@ -41,6 +42,61 @@ cudaError_t VOG_CAT(advect_launch_, VOG_N)(const AdvectArgs& a, int sym, bool vd
 {
     return vdir ? launch_sym<VOG_N, true>(a, sym, n_tiles, threads, smem, st)
                 : launch_sym<VOG_N, false>(a, sym, n_tiles, threads, smem, st);
+}
+
+// ---- contiguous-line (x) kernel
+template <int N, int SYM>
+static cudaError_t launch_x_one(const AdvectXArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    auto kern = advect_x_kernel<N, SYM>;
+    static size_t smem_set = 0;
+    if (smem > 48 * 1024 && smem > smem_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        smem_set = smem;
+    }
+    kern<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <int N, int SYM>
+static int occ_x_one(int threads, size_t smem)
+{
+    auto kern = advect_x_kernel<N, SYM>;
+    if (smem > 48 * 1024 &&
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return nb;
+}
+
+cudaError_t VOG_CAT(advect_x_launch_, VOG_N)(const AdvectXArgs& a, int sym, int grid, int threads, size_t smem,
+                                             cudaStream_t st)
+{
+    switch (sym) {
+        case SYM_LAG_D1:  return launch_x_one<VOG_N, SYM_LAG_D1>(a, grid, threads, smem, st);
+        case SYM_LAG_D4:  return launch_x_one<VOG_N, SYM_LAG_D4>(a, grid, threads, smem, st);
+        case SYM_LAG_D8:  return launch_x_one<VOG_N, SYM_LAG_D8>(a, grid, threads, smem, st);
+        case SYM_SPLINE3: return launch_x_one<VOG_N, SYM_SPLINE3>(a, grid, threads, smem, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+int VOG_CAT(advect_x_occ_, VOG_N)(int sym, int threads, size_t smem)
+{
+    switch (sym) {
+        case SYM_LAG_D1:  return occ_x_one<VOG_N, SYM_LAG_D1>(threads, smem);
+        case SYM_LAG_D4:  return occ_x_one<VOG_N, SYM_LAG_D4>(threads, smem);
+        case SYM_LAG_D8:  return occ_x_one<VOG_N, SYM_LAG_D8>(threads, smem);
+        case SYM_SPLINE3: return occ_x_one<VOG_N, SYM_SPLINE3>(threads, smem);
+    }
+    return 0;
 }
 
 }  // namespace vog

@@ -27,13 +27,39 @@ struct AdvectArgs {
     float cg[4];
 };
 
+// Per-line record of the contiguous-line (x) kernel, XREC_WORDS floats (96 B = 6 cp.async chunks):
+//   [0]      b mod N as int bits (integer part of beta)
+//   [1]      1/N                       (mode 0: lambda_0 = 1 exactly)
+//   [2]      lambda_{N/2} / N          (Nyquist mode of the line, real)
+//   [4..12]  Lagrange: a_k(1-b*)/(2N), k = 0..8;   spline: [4..7] = 3/(2N) (B(b*+1), B(b*), B(b*-1), B(b*-2))
+//   [13..21] Lagrange: a_k(b*)/(2N)
+constexpr int XREC_WORDS = 24;
+
+struct AdvectXArgs {
+    float* f;             // [n_lines][N], lines contiguous
+    int n_groups;         // n_lines >> lpi_log
+    int lpi_log;          // log2(lines per iteration)
+    const float2* twA;    // [R1-1][S1]   e^{-2 pi i t q / M}
+    const float2* twB;    // [15][16]     e^{-2 pi i t q / 256}
+    const float2* cs;     // [N/2+1]      (cos, sin)(2 pi k / N)
+    const float* rec;     // [n_lines][XREC_WORDS]
+    float2 root32[32];    // e^{+2 pi i j / 32}
+};
+
+typedef cudaError_t (*advect_x_launch_fn)(const AdvectXArgs& a, int sym, int grid, int threads, size_t smem,
+                                          cudaStream_t st);
+advect_x_launch_fn advect_x_launcher(int N);
+int advect_x_occupancy(int N, int sym, int threads, size_t smem);
+
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
 typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,
                                         size_t smem, cudaStream_t st);
 advect_launch_fn advect_launcher(int N);
 size_t advect_smem_bytes(int N, int lognl);
 
-#define VOG_DECL_LAUNCH(NN) cudaError_t advect_launch_##NN(const AdvectArgs&, int, bool, int, int, size_t, cudaStream_t);
+#define VOG_DECL_LAUNCH(NN) cudaError_t advect_launch_##NN(const AdvectArgs&, int, bool, int, int, size_t, cudaStream_t); \
+    cudaError_t advect_x_launch_##NN(const AdvectXArgs&, int, int, int, size_t, cudaStream_t); \
+    int advect_x_occ_##NN(int, int, size_t);
 VOG_DECL_LAUNCH(64) VOG_DECL_LAUNCH(128) VOG_DECL_LAUNCH(256) VOG_DECL_LAUNCH(512) VOG_DECL_LAUNCH(1024)
 VOG_DECL_LAUNCH(2048) VOG_DECL_LAUNCH(4096) VOG_DECL_LAUNCH(8192) VOG_DECL_LAUNCH(16384)
 #undef VOG_DECL_LAUNCH

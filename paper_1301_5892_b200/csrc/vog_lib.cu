@@ -30,6 +30,43 @@ advect_launch_fn advect_launcher(int N)
     return nullptr;
 }
 
+advect_x_launch_fn advect_x_launcher(int N)
+{
+    switch (N) {
+        case 64: return advect_x_launch_64;
+        case 128: return advect_x_launch_128;
+        case 256: return advect_x_launch_256;
+        case 512: return advect_x_launch_512;
+        case 1024: return advect_x_launch_1024;
+        case 2048: return advect_x_launch_2048;
+        case 4096: return advect_x_launch_4096;
+        case 8192: return advect_x_launch_8192;
+        case 16384: return advect_x_launch_16384;
+    }
+    return nullptr;
+}
+
+int advect_x_occupancy(int N, int sym, int threads, size_t smem)
+{
+    switch (N) {
+        case 64: return advect_x_occ_64(sym, threads, smem);
+        case 128: return advect_x_occ_128(sym, threads, smem);
+        case 256: return advect_x_occ_256(sym, threads, smem);
+        case 512: return advect_x_occ_512(sym, threads, smem);
+        case 1024: return advect_x_occ_1024(sym, threads, smem);
+        case 2048: return advect_x_occ_2048(sym, threads, smem);
+        case 4096: return advect_x_occ_4096(sym, threads, smem);
+        case 8192: return advect_x_occ_8192(sym, threads, smem);
+        case 16384: return advect_x_occ_16384(sym, threads, smem);
+    }
+    return 0;
+}
+
+size_t advect_x_smem_bytes(int N, int lpi_log)
+{
+    return ((size_t)2 << lpi_log) * ((size_t)N * sizeof(float) + XREC_WORDS * sizeof(float));
+}
+
 size_t advect_smem_bytes(int N, int lognl)
 {
     const size_t NL = (size_t)1 << lognl;
@@ -96,6 +133,53 @@ __global__ void shift_setup_kernel(const SetupArgs s)
         }
     }
     r[19] = sshift;
+}
+
+// S1 for the contiguous-line kernel: records of XREC_WORDS floats (layout in vog_internal.h).
+__global__ void shift_setup_x_kernel(const SetupArgs s)
+{
+    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= s.n_lines) return;
+    double beta;
+    if (s.mode == 0) beta = -(s.vmin + (double)l * s.dv) * s.dt / s.delta;
+    else beta = s.beta[l];
+    const double fl = floor(beta);
+    const double t = beta - fl;
+    double bm = fmod(fl, (double)s.N);
+    if (bm < 0.0) bm += (double)s.N;
+    int b = (int)bm;
+    if (b >= s.N) b = 0;
+    float* r = s.rec + (size_t)l * XREC_WORDS;
+    const double sc = 1.0 / (2.0 * (double)s.N);
+    const double sgn = (b & 1) ? -1.0 : 1.0;
+    for (int k = 0; k < XREC_WORDS; ++k) r[k] = 0.0f;
+    r[0] = __int_as_float(b);
+    r[1] = (float)(1.0 / (double)s.N);
+    double nyq;
+    if (s.spline) {
+        const double u = 1.0 - t;
+        const double Bm1 = u * u * u / 6.0, B0 = (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0;
+        const double B1 = (1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0, B2 = t * t * t / 6.0;
+        r[4] = (float)(3.0 * sc * Bm1); r[5] = (float)(3.0 * sc * B0);
+        r[6] = (float)(3.0 * sc * B1);  r[7] = (float)(3.0 * sc * B2);
+        nyq = 3.0 * (B0 + B2 - Bm1 - B1);           // theta = pi: c = -1, s = 0, 3/(2+c) = 3
+    } else {
+        double p[2];
+        for (int half = 0; half < 2; ++half) {
+            const double tt = half == 0 ? 1.0 - t : t;
+            double a = tt, pw = 1.0, acc = 0.0;
+            float* o = r + 4 + 9 * half;
+            for (int k = 0; k <= 8; ++k) {
+                if (k > 0) a = (k <= s.d) ? a * ((double)(k * k) - tt * tt) / (double)(2 * k * (2 * k + 1)) : 0.0;
+                o[k] = (float)(a * sc);
+                acc += a * pw;
+                pw *= 4.0;                           // s = 2 - 2 cos(pi) = 4
+            }
+            p[half] = acc;
+        }
+        nyq = p[0] - p[1];                           // P(4;1-b*) + e^{i pi} P(4;b*)
+    }
+    r[2] = (float)(sgn * nyq / (double)s.N);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -219,6 +303,9 @@ struct vog_plan_s {
     cudaStream_t st;
     int sym, d;                 // symbol variant and Lagrange half-width
     float2 *tw_x, *tw_v;        // roots of unity of order Nx / Nv
+    float2 *xtwA, *xtwB, *xcs;  // x kernel: pass-A twiddles [R1-1][S1], pass-B twiddles [15][16], (cos,sin)(2 pi k/Nx)
+    float* xrec;                // x kernel shift records [Nv][XREC_WORDS]
+    int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
     float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
     double* part;               // density partials [nby][Nx]
     double* rho;                // [Nx]
@@ -226,6 +313,7 @@ struct vog_plan_s {
     float *feq_tab, *vmu_tab;   // [ng][Nv]
     int nby;
     int lognl_x, lognl_v, thr_x, thr_v;
+    int n_sm;
     bool E_valid;
     bool recx_valid; double recx_dt;
     long long launches;
@@ -255,6 +343,67 @@ static void fill_roots(std::vector<float2>& h, int N)
         }
         h[k] = make_float2(c, -s);
     }
+}
+
+// e^{-2 pi i k / n}, exact on the axes and diagonals' signs, long double elsewhere, rounded once
+static float2 unit_root_neg(long long k, long long n)
+{
+    k %= n;
+    if (k < 0) k += n;
+    if ((4 * k) % n == 0) {
+        const int q = (int)((4 * k) / n);
+        return make_float2(q == 0 ? 1.f : (q == 2 ? -1.f : 0.f), q == 1 ? -1.f : (q == 3 ? 1.f : 0.f));
+    }
+    const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)n;
+    return make_float2((float)cosl(a), -(float)sinl(a));
+}
+
+static void x_radix(int N, int* R1, int* R2)
+{
+    switch (N) {
+        case 64: *R1 = 2; *R2 = 1; break;
+        case 128: *R1 = 4; *R2 = 1; break;
+        case 256: *R1 = 8; *R2 = 1; break;
+        case 512: *R1 = 16; *R2 = 1; break;
+        case 1024: *R1 = 32; *R2 = 1; break;
+        case 2048: *R1 = 4; *R2 = 16; break;
+        case 4096: *R1 = 8; *R2 = 16; break;
+        case 8192: *R1 = 16; *R2 = 16; break;
+        default: *R1 = 32; *R2 = 16; break;
+    }
+}
+
+// twiddle tables of the contiguous-line kernel for line length N (complex length M = N/2)
+static void fill_x_tables(int N, std::vector<float2>& twA, std::vector<float2>& twB, std::vector<float2>& cs)
+{
+    int R1, R2;
+    x_radix(N, &R1, &R2);
+    const int M = N / 2, S1 = M / R1;
+    twA.assign((size_t)(R1 - 1) * S1, make_float2(1.f, 0.f));
+    for (int q = 1; q < R1; ++q)
+        for (int t = 0; t < S1; ++t) twA[(size_t)(q - 1) * S1 + t] = unit_root_neg((long long)t * q, M);
+    twB.assign(15 * 16, make_float2(1.f, 0.f));
+    for (int q = 1; q < 16; ++q)
+        for (int t = 0; t < 16; ++t) twB[(q - 1) * 16 + t] = unit_root_neg(t * q, 256);
+    cs.resize(M + 1);
+    for (int k = 0; k <= M; ++k) {
+        const float2 w = unit_root_neg(k, N);
+        cs[k] = make_float2(w.x, -w.y);          // (cos, sin)(2 pi k / N)
+    }
+}
+
+static void default_x_tile(int N, int n_lines, int* lpi_log, int* threads)
+{
+    int lpi = 8192 / N;
+    if (lpi < 1) lpi = 1;
+    if (lpi > 16) lpi = 16;
+    while (lpi > 1 && n_lines / lpi < 148 * 4) lpi >>= 1;
+    while (lpi > n_lines) lpi >>= 1;
+    int t = lpi * (N / 64);
+    if (t < 32) t = 32;
+    if (t > 128) t = 128;
+    *lpi_log = ilog2i(lpi);
+    *threads = t;
 }
 
 // default tile shape: NL complex lines per CTA and threads per CTA (kernel section)
@@ -294,6 +443,7 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
+    cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
     cudaFree(P->part); cudaFree(P->rho); cudaFree(P->E_self);
     cudaFree(P->feq_tab); cudaFree(P->vmu_tab); cudaFree(P->f_buf); cudaFree(P->ext_buf);
@@ -334,13 +484,25 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     int nby = 1;
     while ((Nx / 32) * nby < 592 && Nv / (nby * 2) >= 32) nby *= 2;
     P->nby = nby;
+    {
+        int dev = 0, nsm = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        P->n_sm = nsm > 0 ? nsm : 148;
+    }
     default_tile(Nx, Nv, false, &P->lognl_x, &P->thr_x);
+    default_x_tile(Nx, Nv, &P->x_lpi_log, &P->x_thr);
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void** ptr, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(ptr, bytes ? bytes : 16); };
     alloc((void**)&P->tw_x, sizeof(float2) * Nx);
     alloc((void**)&P->tw_v, sizeof(float2) * Nv);
     alloc((void**)&P->rec_x, sizeof(float) * REC_WORDS * Nv);
+    alloc((void**)&P->xrec, sizeof(float) * XREC_WORDS * Nv);
+    std::vector<float2> xa, xb, xc;
+    fill_x_tables(Nx, xa, xb, xc);
+    alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
+    alloc((void**)&P->xtwB, sizeof(float2) * xb.size());
+    alloc((void**)&P->xcs, sizeof(float2) * xc.size());
     alloc((void**)&P->rec_v, sizeof(float) * REC_WORDS * Nx);
     alloc((void**)&P->part, sizeof(double) * nby * Nx);
     alloc((void**)&P->rho, sizeof(double) * Nx);
@@ -348,9 +510,13 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->feq_tab, sizeof(float) * (ng ? ng : 1) * Nv);
     alloc((void**)&P->vmu_tab, sizeof(float) * (ng ? ng : 1) * Nv);
     if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
+    e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwB, xb.data(), sizeof(float2) * xb.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->xcs, xc.data(), sizeof(float2) * xc.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
     std::vector<float2> h;
     fill_roots(h, Nx);
-    e = cudaMemcpyAsync(P->tw_x, h.data(), sizeof(float2) * Nx, cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->tw_x, h.data(), sizeof(float2) * Nx, cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
     fill_roots(h, Nv);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->tw_v, h.data(), sizeof(float2) * Nv, cudaMemcpyHostToDevice, P->st);
@@ -393,6 +559,9 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 1: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_x = value; break;
         case 2: if (value < 0 || (2 << value) > Nx || advect_smem_bytes(Nv, value) > 227 * 1024) return VOG_EINVAL; P->lognl_v = value; break;
         case 3: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_v = value; break;
+        case 5: if (value < 0 || (1 << value) > Nv || advect_x_smem_bytes(Nx, value) > 227 * 1024) return VOG_EINVAL; P->x_lpi_log = value; P->x_occ = 0; break;
+        case 6: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->x_thr = value; P->x_occ = 0; break;
+        case 7: if (value < 0 || value > 32) return VOG_EINVAL; P->x_cps = value; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -415,14 +584,42 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
     s.delta = vdir ? s.dv : P->p.L / (double)Nx;
     s.vmin = P->p.vmin;
     s.E = E; s.Eext = Eext; s.beta = beta;
-    s.rec = vdir ? P->rec_v : P->rec_x;
-    shift_setup_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
+    s.rec = vdir ? P->rec_v : P->xrec;
+    if (vdir) shift_setup_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
+    else shift_setup_x_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
     P->launches++;
     return cudaGetLastError();
 }
 
+static cudaError_t run_advect_x(vog_plan_s* P, float* f)
+{
+    AdvectXArgs a;
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.f = f;
+    a.lpi_log = P->x_lpi_log;
+    a.n_groups = Nv >> a.lpi_log;
+    a.twA = P->xtwA; a.twB = P->xtwB; a.cs = P->xcs; a.rec = P->xrec;
+    for (int j = 0; j < 32; ++j) {
+        const float2 w = unit_root_neg(j, 32);
+        a.root32[j] = make_float2(w.x, -w.y);
+    }
+    const size_t smem = advect_x_smem_bytes(Nx, a.lpi_log);
+    if (P->x_occ == 0) {
+        P->x_occ = advect_x_occupancy(Nx, P->sym, P->x_thr, smem);
+        if (P->x_occ <= 0) return cudaErrorInvalidConfiguration;
+    }
+    const int cps = (P->x_cps > 0 && P->x_cps < P->x_occ) ? P->x_cps : P->x_occ;
+    int grid = cps * P->n_sm;
+    if (grid > a.n_groups) grid = a.n_groups;
+    advect_x_launch_fn fn = advect_x_launcher(Nx);
+    if (!fn) return cudaErrorInvalidValue;
+    P->launches++;
+    return fn(a, P->sym, grid, P->x_thr, smem, P->st);
+}
+
 static cudaError_t run_advect(vog_plan_s* P, float* f, bool vdir, bool source)
 {
+    if (!vdir) return run_advect_x(P, f);
     AdvectArgs a;
     std::memset(&a, 0, sizeof(a));
     const int Nx = P->p.Nx, Nv = P->p.Nv;
