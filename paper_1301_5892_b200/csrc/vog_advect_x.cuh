@@ -293,11 +293,18 @@ __device__ __forceinline__ float2 unit_root(const float2* __restrict__ cs, int j
     return make_float2(v.x, up ? -v.y : v.y);
 }
 
-// Fused middle stage on one item = two radix-16 groups gA, gB whose modes mirror each other.
-template <int N, int SYM, bool SPECIAL>
+// Fused middle stage on one item = two radix-16 groups gA, gB whose modes mirror each other:
+// pair slot q holds (Z_k, Z_{M-k}) in (XA[brev q], XB[brev(15-q)]), k = klowA + ML q.
+// The one "special" item per line (gA = group 0, gB = the self-mirrored group) is brought to the
+// same form by a register permutation (executed by that thread's warp only):
+//   slots 0..7  : group B pairs  (q, 15-q),      k = ML/2 + ML q
+//   slots 8..14 : group A pairs  (q', 16-q'),    k = ML q',  q' = slot - 7
+//   slot  15    : k = M/2, its own mirror;   k = 0 (with k = M, the line's Nyquist mode) apart.
+template <int N, int SYM>
 __device__ __forceinline__ void symbol_item_x(float4* __restrict__ buf, const int cline, const int gA,
-                                              const int gB, const int klowA, float* __restrict__ rec,
-                                              const float2* __restrict__ cs, const float2* ROOT32)
+                                              const int gB, const int klowA, const bool special,
+                                              float* __restrict__ rec, const float2* __restrict__ cs,
+                                              const float2* ROOT32)
 {
     constexpr int M = N / 2, ML = M / 16;
     float2 XA[16], XB[16];
@@ -311,38 +318,50 @@ __device__ __forceinline__ void symbol_item_x(float4* __restrict__ buf, const in
     }
     dft_dif<16, 1>(XA);
     dft_dif<16, 1>(XB);
+    float2 z0 = XA[0];
+    if (special) {
+        float2 TA[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) TA[i] = XA[i];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) XA[brev(q, 16)] = XB[brev(q, 16)];
+#pragma unroll
+        for (int q = 8; q < 15; ++q) { XA[brev(q, 16)] = TA[brev(q - 7, 16)]; XB[brev(15 - q, 16)] = TA[brev(23 - q, 16)]; }
+        XA[brev(15, 16)] = TA[brev(8, 16)];
+        XB[brev(0, 16)] = TA[brev(8, 16)];
+    }
     SymCoef<SYM> K;
     sym_load<SYM>(K, rec);
     const int b = __float_as_int(rec[0]);
     const float sgn = (b & 1) ? -1.0f : 1.0f;
-    if constexpr (!SPECIAL) {
-        const float2 base = unit_root<N>(cs, b * klowA);
+    const int klo = special ? ML / 2 : klowA;            // slots 0..7
+    const int khi = special ? ML / 2 - 15 * ML / 2 : klowA;   // slots 8..15: k = khi + ML q
+    const float2 base_lo = unit_root<N>(cs, b * klo);
+    const float2 base_hi = unit_root<N>(cs, b * khi);
 #pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const float2 rot = cmul(base, ROOT32[(b * q) & 31]);
-            pair_op<SYM>(XA[brev(q, 16)], XB[brev(15 - q, 16)], __ldg(cs + klowA + ML * q), rot, sgn, K);
-        }
-    } else {
-        // group B is its own mirror: modes ML/2 + ML q  <->  ML/2 + ML (15 - q)
-        const float2 base = unit_root<N>(cs, b * (ML / 2));
+    for (int q = 0; q < 16; ++q) {
+        const float2 rot = cmul(q < 8 ? base_lo : base_hi, ROOT32[(b * q) & 31]);
+        pair_op<SYM>(XA[brev(q, 16)], XB[brev(15 - q, 16)], __ldg(cs + (q < 8 ? klo : khi) + ML * q), rot, sgn, K);
+    }
+    if (special) {
+        // back to group order: XA[brev i] = Z'_{ML i}, XB[brev i] = Z'_{ML/2 + ML i}
+        float2 TA[16], TB[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            const float2 rot = cmul(base, ROOT32[(b * q) & 31]);
-            pair_op<SYM>(XB[brev(q, 16)], XB[brev(15 - q, 16)], __ldg(cs + ML / 2 + ML * q), rot, sgn, K);
-        }
-        // group A holds modes ML q: q <-> 16 - q, q = 8 (k = M/2) mirrors itself, q = 0 is special
+        for (int i = 0; i < 16; ++i) TA[i] = XA[i];
 #pragma unroll
-        for (int q = 1; q < 8; ++q)
-            pair_op<SYM>(XA[brev(q, 16)], XA[brev(16 - q, 16)], __ldg(cs + ML * q), ROOT32[(b * q) & 31], sgn, K);
-        {
-            float2 dup = XA[brev(8, 16)];
-            pair_op<SYM>(XA[brev(8, 16)], dup, __ldg(cs + ML * 8), ROOT32[(b * 8) & 31], sgn, K);
+        for (int j = 1; j < 8; ++j) TB[j] = XB[brev(j, 16)];                  // Q'_{15-j} = Z'_{ML (8+j)}
+#pragma unroll
+        for (int q = 0; q < 8; ++q) XB[brev(q, 16)] = TA[brev(q, 16)];        // P'_q = Z'_{ML/2 + ML q}
+#pragma unroll
+        for (int i = 1; i < 8; ++i) {
+            XA[brev(i, 16)] = TA[brev(i + 7, 16)];                            // P'_{i+7} = Z'_{ML i}
+            XA[brev(16 - i, 16)] = TB[8 - i];                                 // Q'_{i+7} = Z'_{ML (16-i)}
         }
-        // k = 0 and k = M (line modes 0 and N/2): U_0 = x + y, U_M = x - y, lambda_0 = 1 exactly
-        const float x = XA[0].x, y = XA[0].y;
-        // the line mean A0 by-passes the inverse transform (added back in the last pass): the
-        // intermediate sums then stay at fluctuation level, one rounding at the level of the mean
-        const float A0 = rec[1] * (x + y), Bn = rec[2] * (x - y);
+        XA[brev(8, 16)] = TA[brev(15, 16)];                                   // P'_15 = Z'_{M/2}
+        // k = 0 and k = M: U_0 = x + y, U_M = x - y, lambda_0 = 1 exactly.  The line mean A0 by-passes
+        // the inverse transform (added back in the last pass): the intermediate sums then stay at
+        // fluctuation level, with one rounding at the level of the mean.
+        const float A0 = rec[1] * (z0.x + z0.y), Bn = rec[2] * (z0.x - z0.y);
         XA[0] = make_float2(Bn, -Bn);
         rec[3] = A0;
     }
@@ -393,8 +412,9 @@ __global__ void __launch_bounds__(128, 4) advect_x_kernel(const AdvectXArgs a)
 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const int lpi = 1 << a.lpi_log;
-    float4* const bufs = reinterpret_cast<float4*>(smem_raw);                     // 2 x lpi x CH chunks
-    float4* const recs4 = bufs + 2 * lpi * CH;                                    // 2 x lpi x RCH chunks
+    const int nbuf = a.nbuf;                                                      // 1 or 2 line buffers
+    float4* const bufs = reinterpret_cast<float4*>(smem_raw);                     // nbuf x lpi x CH chunks
+    float4* const recs4 = bufs + nbuf * lpi * CH;                                 // nbuf x lpi x RCH chunks
     const int tid = threadIdx.x, T = blockDim.x;
 
     auto prefetch = [&](int g, int sel) {
@@ -410,15 +430,23 @@ __global__ void __launch_bounds__(128, 4) advect_x_kernel(const AdvectXArgs a)
     if (g < a.n_groups) prefetch(g, 0);
     cp_async_commit();
     for (int it = 0; g < a.n_groups; g += gridDim.x, ++it) {
-        const int sel = it & 1;
+        const int sel = nbuf == 2 ? (it & 1) : 0;
+        if (nbuf == 1 && it > 0) {                 // single buffer: reload after everybody left iteration it-1
+            __syncthreads();
+            prefetch(g, 0);
+            cp_async_commit();
+        }
         cp_async_wait_all();
         __syncthreads();                           // group g landed; everybody left iteration it-1
-        if (g + (int)gridDim.x < a.n_groups) prefetch(g + gridDim.x, sel ^ 1);
-        cp_async_commit();
+        if (nbuf == 2) {
+            if (g + (int)gridDim.x < a.n_groups) prefetch(g + gridDim.x, sel ^ 1);
+            cp_async_commit();
+        }
         float4* const buf = bufs + sel * lpi * CH;
         float* const recs = reinterpret_cast<float*>(recs4 + sel * lpi * RCH);
 
         // ---- forward pass A
+#pragma unroll 1
         for (int w = tid; w < lpi * ITEMS_A; w += T) {
             const int l = w / ITEMS_A, t = w & (ITEMS_A - 1);
             if constexpr (PAIR_A) fwd_pair_pass<R1, S1>(buf, l * CH + t, t, a.twA);
@@ -427,6 +455,7 @@ __global__ void __launch_bounds__(128, 4) advect_x_kernel(const AdvectXArgs a)
         __syncthreads();
         // ---- forward pass B
         if constexpr (R2 == 16) {
+#pragma unroll 1
             for (int w = tid; w < lpi * ITEMS_C; w += T) {
                 const int l = w / ITEMS_C, i = w & (ITEMS_C - 1);
                 mid_pass<false>(buf, l * CH + (i >> 3) * 128, i & 7, a.twB);
@@ -434,18 +463,19 @@ __global__ void __launch_bounds__(128, 4) advect_x_kernel(const AdvectXArgs a)
             __syncthreads();
         }
         // ---- symbol stage
+#pragma unroll 1
         for (int w = tid; w < lpi * ITEMS_C; w += T) {
             const int l = w / ITEMS_C, u = w & (ITEMS_C - 1);
             int gA, gB, klowA;
             bool special;
             item_groups<R1, R2>(u, gA, gB, klowA, special);
             float* rec = recs + l * XREC_WORDS;
-            if (special) symbol_item_x<N, SYM, true>(buf, l * CH, gA, gB, klowA, rec, a.cs, a.root32);
-            else         symbol_item_x<N, SYM, false>(buf, l * CH, gA, gB, klowA, rec, a.cs, a.root32);
+            symbol_item_x<N, SYM>(buf, l * CH, gA, gB, klowA, special, rec, a.cs, a.root32);
         }
         __syncthreads();
         // ---- inverse pass B
         if constexpr (R2 == 16) {
+#pragma unroll 1
             for (int w = tid; w < lpi * ITEMS_C; w += T) {
                 const int l = w / ITEMS_C, i = w & (ITEMS_C - 1);
                 mid_pass<true>(buf, l * CH + (i >> 3) * 128, i & 7, a.twB);
@@ -454,6 +484,7 @@ __global__ void __launch_bounds__(128, 4) advect_x_kernel(const AdvectXArgs a)
         }
         // ---- inverse pass A: shared -> registers -> global
         float4* const gout = reinterpret_cast<float4*>(a.f) + (size_t)g * lpi * CH;
+#pragma unroll 1
         for (int w = tid; w < lpi * ITEMS_A; w += T) {
             const int l = w / ITEMS_A, t = w & (ITEMS_A - 1);
             const float dc = recs[l * XREC_WORDS + 3];

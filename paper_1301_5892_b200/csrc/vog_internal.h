@@ -39,6 +39,7 @@ struct AdvectXArgs {
     float* f;             // [n_lines][N], lines contiguous
     int n_groups;         // n_lines >> lpi_log
     int lpi_log;          // log2(lines per iteration)
+    int nbuf;             // line buffers per CTA: 2 = prefetch the next group during the transform, 1 = none
     const float2* twA;    // [R1-1][S1]   e^{-2 pi i t q / M}
     const float2* twB;    // [15][16]     e^{-2 pi i t q / 256}
     const float2* cs;     // [N/2+1]      (cos, sin)(2 pi k / N)

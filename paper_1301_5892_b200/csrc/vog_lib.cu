@@ -62,9 +62,9 @@ int advect_x_occupancy(int N, int sym, int threads, size_t smem)
     return 0;
 }
 
-size_t advect_x_smem_bytes(int N, int lpi_log)
+size_t advect_x_smem_bytes(int N, int lpi_log, int nbuf)
 {
-    return ((size_t)2 << lpi_log) * ((size_t)N * sizeof(float) + XREC_WORDS * sizeof(float));
+    return ((size_t)nbuf << lpi_log) * ((size_t)N * sizeof(float) + XREC_WORDS * sizeof(float));
 }
 
 size_t advect_smem_bytes(int N, int lognl)
@@ -305,6 +305,7 @@ struct vog_plan_s {
     float2 *tw_x, *tw_v;        // roots of unity of order Nx / Nv
     float2 *xtwA, *xtwB, *xcs;  // x kernel: pass-A twiddles [R1-1][S1], pass-B twiddles [15][16], (cos,sin)(2 pi k/Nx)
     float* xrec;                // x kernel shift records [Nv][XREC_WORDS]
+    int x_nbuf;
     int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
     float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
     double* part;               // density partials [nby][Nx]
@@ -491,6 +492,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     }
     default_tile(Nx, Nv, false, &P->lognl_x, &P->thr_x);
     default_x_tile(Nx, Nv, &P->x_lpi_log, &P->x_thr);
+    P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void** ptr, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(ptr, bytes ? bytes : 16); };
@@ -559,9 +561,10 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 1: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_x = value; break;
         case 2: if (value < 0 || (2 << value) > Nx || advect_smem_bytes(Nv, value) > 227 * 1024) return VOG_EINVAL; P->lognl_v = value; break;
         case 3: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_v = value; break;
-        case 5: if (value < 0 || (1 << value) > Nv || advect_x_smem_bytes(Nx, value) > 227 * 1024) return VOG_EINVAL; P->x_lpi_log = value; P->x_occ = 0; break;
+        case 5: if (value < 0 || (1 << value) > Nv || advect_x_smem_bytes(Nx, value, P->x_nbuf) > 227 * 1024) return VOG_EINVAL; P->x_lpi_log = value; P->x_occ = 0; break;
         case 6: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->x_thr = value; P->x_occ = 0; break;
         case 7: if (value < 0 || value > 32) return VOG_EINVAL; P->x_cps = value; break;
+        case 8: if (value < 1 || value > 2 || advect_x_smem_bytes(Nx, P->x_lpi_log, value) > 227 * 1024) return VOG_EINVAL; P->x_nbuf = value; P->x_occ = 0; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -597,13 +600,14 @@ static cudaError_t run_advect_x(vog_plan_s* P, float* f)
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     a.f = f;
     a.lpi_log = P->x_lpi_log;
+    a.nbuf = P->x_nbuf;
     a.n_groups = Nv >> a.lpi_log;
     a.twA = P->xtwA; a.twB = P->xtwB; a.cs = P->xcs; a.rec = P->xrec;
     for (int j = 0; j < 32; ++j) {
         const float2 w = unit_root_neg(j, 32);
         a.root32[j] = make_float2(w.x, -w.y);
     }
-    const size_t smem = advect_x_smem_bytes(Nx, a.lpi_log);
+    const size_t smem = advect_x_smem_bytes(Nx, a.lpi_log, a.nbuf);
     if (P->x_occ == 0) {
         P->x_occ = advect_x_occupancy(Nx, P->sym, P->x_thr, smem);
         if (P->x_occ <= 0) return cudaErrorInvalidConfiguration;
