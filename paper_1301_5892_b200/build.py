@@ -50,7 +50,8 @@ def build(force=False, verbose=False):
     if not force and not _stale(LIB, deps):
         return LIB
     os.makedirs(OBJ, exist_ok=True)
-    jobs = [(os.path.join(CSRC, "vog_lib.cu"), os.path.join(OBJ, "vog_lib.o"), [])]
+    jobs = [(os.path.join(CSRC, "vog_lib.cu"), os.path.join(OBJ, "vog_lib.o"), []),
+            (os.path.join(CSRC, "vog_os.cu"), os.path.join(OBJ, "vog_os.o"), [])]
     for n in SIZES:
         jobs.append((os.path.join(CSRC, "vog_advect_inst.cu"), os.path.join(OBJ, "vog_advect_%d.o" % n),
                      ["-DVOG_N=%d" % n]))

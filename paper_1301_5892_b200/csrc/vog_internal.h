@@ -52,6 +52,47 @@ typedef cudaError_t (*advect_x_launch_fn)(const AdvectXArgs& a, int sym, int gri
 advect_x_launch_fn advect_x_launcher(int N);
 int advect_x_occupancy(int N, int sym, int threads, size_t smem);
 
+// ---- overlap-save kernels (vog_os.cuh), line length >= 1024
+constexpr int OS_LB = 256;     // block length (reals)
+constexpr int OS_V = 224;      // valid outputs per block
+constexpr int OS_H = 16;       // discarded samples on either side
+// Per-line symbol table, OS_LAMW float2 (1040 B): [k] = lambda(2 pi k/OS_LB) / (2 OS_LB), k = 0..128
+// (x: times e^{i theta_k (b mod 4)}); [129] = (integer shift as int bits: x: b >> 2 in 16-byte chunks,
+// v: b in rows;  v: s = E dt of the delta-f source).
+constexpr int OS_LAMW = 130;
+
+struct OsArgs {
+    const float* src;      // [Nv][Nx]
+    float* dst;            // x: may equal src; v: must differ
+    int Nx, Nv;
+    int N;                 // line length (x: Nx, v: Nv)
+    int nb;                // blocks per line = ceil(N / OS_V)
+    const float2* lam;     // [n_lines][OS_LAMW]
+    const float2* tw;      // x: [7][16] e^{-2 pi i t q/128};  v: [15][16] e^{-2 pi i t q/256}
+    const float2* cs;      // [129] (cos, sin)(2 pi k/256)   (x only)
+    int lpi, n_groups;     // x: lines per iteration, n_lines / lpi
+    int np_log, rb, gpc;   // v: log2(column pairs per strip), row blocks per group, groups per CTA
+    int ng;                // v: Gaussians of f_eq (0 = no source)
+    const float* feq_tab;  // [ng][Nv]
+    const float* vmu_tab;  // [ng][Nv]
+    float cg[4];
+};
+
+struct OsSetupArgs {
+    int n_lines, N, mode;      // mode 0: c = v_l; 1: c = E_l (+E_ext_l); 2: explicit beta
+    int spline, d, vdir;
+    double dt, delta, vmin, dv;
+    const float* E;
+    const float* Eext;
+    const double* beta;
+    float2* lam;
+};
+
+cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st);
+cudaError_t osx_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
+int osx_occupancy(int threads, size_t smem);
+
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
 typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,
                                         size_t smem, cudaStream_t st);

@@ -306,6 +306,13 @@ struct vog_plan_s {
     float2 *xtwA, *xtwB, *xcs;  // x kernel: pass-A twiddles [R1-1][S1], pass-B twiddles [15][16], (cos,sin)(2 pi k/Nx)
     float* xrec;                // x kernel shift records [Nv][XREC_WORDS]
     int x_nbuf;
+    // overlap-save path (line length >= 1024)
+    bool os_x, os_v;
+    float2 *os_lam_x, *os_lam_v;   // symbol tables [Nv][OS_LAMW], [Nx][OS_LAMW]
+    float2 *os_twx, *os_twv, *os_cs;
+    float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
+    int osx_lpi, osx_thr, osx_cps, osx_occ;
+    int osv_np_log, osv_thr, osv_rb, osv_gpc;
     int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
     float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
     double* part;               // density partials [nby][Nx]
@@ -444,6 +451,8 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
+    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs);
+    cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
     cudaFree(P->part); cudaFree(P->rho); cudaFree(P->E_self);
@@ -492,6 +501,16 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     }
     default_tile(Nx, Nv, false, &P->lognl_x, &P->thr_x);
     default_x_tile(Nx, Nv, &P->x_lpi_log, &P->x_thr);
+    P->os_x = Nx >= 1024;
+    P->os_v = Nv >= 1024;
+    {
+        const int nbx = (Nx + OS_V - 1) / OS_V;
+        int lpi = 1;
+        while (lpi * 2 * nbx <= 40 && lpi * 2 <= Nv) lpi *= 2;
+        while (lpi > 1 && Nv / lpi < P->n_sm * 3) lpi >>= 1;
+        P->osx_lpi = lpi; P->osx_thr = 160; P->osx_cps = 0; P->osx_occ = 0;
+        P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 2; P->osv_gpc = 0;
+    }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
     cudaError_t e = cudaSuccess;
@@ -502,6 +521,17 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->xrec, sizeof(float) * XREC_WORDS * Nv);
     std::vector<float2> xa, xb, xc;
     fill_x_tables(Nx, xa, xb, xc);
+    std::vector<float2> otx(112), otv(240), ocs(130, make_float2(0.f, 0.f));
+    for (int q = 1; q < 8; ++q)
+        for (int t = 0; t < 16; ++t) otx[(q - 1) * 16 + t] = unit_root_neg(t * q, 128);
+    for (int q = 1; q < 16; ++q)
+        for (int t = 0; t < 16; ++t) otv[(q - 1) * 16 + t] = unit_root_neg(t * q, 256);
+    for (int k = 0; k <= 128; ++k) { const float2 w = unit_root_neg(k, 256); ocs[k] = make_float2(w.x, -w.y); }
+    alloc((void**)&P->os_twx, sizeof(float2) * otx.size());
+    alloc((void**)&P->os_twv, sizeof(float2) * otv.size());
+    alloc((void**)&P->os_cs, sizeof(float2) * ocs.size());
+    alloc((void**)&P->os_lam_x, sizeof(float2) * OS_LAMW * (P->os_x ? Nv : 1));
+    alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx : 1));
     alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
     alloc((void**)&P->xtwB, sizeof(float2) * xb.size());
     alloc((void**)&P->xcs, sizeof(float2) * xc.size());
@@ -512,7 +542,10 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->feq_tab, sizeof(float) * (ng ? ng : 1) * Nv);
     alloc((void**)&P->vmu_tab, sizeof(float) * (ng ? ng : 1) * Nv);
     if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
-    e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
+    e = cudaMemcpyAsync(P->os_twx, otx.data(), sizeof(float2) * otx.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs, ocs.data(), sizeof(float2) * ocs.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwB, xb.data(), sizeof(float2) * xb.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xcs, xc.data(), sizeof(float2) * xc.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
@@ -550,6 +583,9 @@ extern "C" int vog_destroy(vog_plan_t P)
     return VOG_OK;
 }
 
+static size_t osx_smem_bytes(int lpi, int nb);
+static size_t osv_smem_bytes(int np_log, int rb);
+
 // internal tuning hook (documented in DESIGN.md; not part of the paper-facing API):
 // which: 0 = log2(NL) x, 1 = threads x, 2 = log2(NL) v, 3 = threads v, 4 = density row blocks
 extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
@@ -565,6 +601,13 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 6: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->x_thr = value; P->x_occ = 0; break;
         case 7: if (value < 0 || value > 32) return VOG_EINVAL; P->x_cps = value; break;
         case 8: if (value < 1 || value > 2 || advect_x_smem_bytes(Nx, P->x_lpi_log, value) > 227 * 1024) return VOG_EINVAL; P->x_nbuf = value; P->x_occ = 0; break;
+        case 10: if (value < 1 || Nv % value || osx_smem_bytes(value, (Nx + OS_V - 1) / OS_V) > 227 * 1024) return VOG_EINVAL; P->osx_lpi = value; P->osx_occ = 0; break;
+        case 11: if (value < 32 || value > 160 || value % 32) return VOG_EINVAL; P->osx_thr = value; P->osx_occ = 0; break;
+        case 12: if (value < 0 || value > 32) return VOG_EINVAL; P->osx_cps = value; break;
+        case 13: if (value < 0 || (2 << value) > Nx || osv_smem_bytes(value, P->osv_rb) > 227 * 1024) return VOG_EINVAL; P->osv_np_log = value; break;
+        case 14: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->osv_thr = value; break;
+        case 15: if (value < 1 || osv_smem_bytes(P->osv_np_log, value) > 227 * 1024) return VOG_EINVAL; P->osv_rb = value; break;
+        case 16: if (value < 0) return VOG_EINVAL; P->osv_gpc = value; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -575,23 +618,99 @@ static int cuda_status(cudaError_t e) { return e == cudaSuccess ? VOG_OK : VOG_E
 static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, const float* E, const float* Eext,
                              const double* beta)
 {
-    SetupArgs s;
     const int Nx = P->p.Nx, Nv = P->p.Nv;
+    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    P->launches++;
+    if (vdir ? P->os_v : P->os_x) {
+        OsSetupArgs s;
+        s.n_lines = vdir ? Nx : Nv;
+        s.N = vdir ? Nv : Nx;
+        s.mode = mode;
+        s.spline = P->sym == SYM_SPLINE3;
+        s.d = P->d;
+        s.vdir = vdir ? 1 : 0;
+        s.dt = dt; s.dv = dv;
+        s.delta = vdir ? dv : P->p.L / (double)Nx;
+        s.vmin = P->p.vmin;
+        s.E = E; s.Eext = Eext; s.beta = beta;
+        s.lam = vdir ? P->os_lam_v : P->os_lam_x;
+        return os_setup_launch(s, P->st);
+    }
+    SetupArgs s;
     s.n_lines = vdir ? Nx : Nv;
     s.N = vdir ? Nv : Nx;
     s.mode = mode;
     s.spline = P->sym == SYM_SPLINE3;
     s.d = P->d;
     s.dt = dt;
-    s.dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    s.dv = dv;
     s.delta = vdir ? s.dv : P->p.L / (double)Nx;
     s.vmin = P->p.vmin;
     s.E = E; s.Eext = Eext; s.beta = beta;
     s.rec = vdir ? P->rec_v : P->xrec;
     if (vdir) shift_setup_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
     else shift_setup_x_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
-    P->launches++;
     return cudaGetLastError();
+}
+
+// ---- overlap-save launches (line length >= 1024)
+static size_t osx_smem_bytes(int lpi, int nb)
+{
+    return (size_t)lpi * nb * 1024 + (size_t)lpi * OS_LAMW * 8 + 130 * 8 + 112 * 8 + (size_t)lpi * nb * 4 + 16;
+}
+
+static cudaError_t run_osx(vog_plan_s* P, const float* src, float* dst)
+{
+    OsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nx;
+    a.nb = (Nx + OS_V - 1) / OS_V;
+    a.lam = P->os_lam_x; a.tw = P->os_twx; a.cs = P->os_cs;
+    a.lpi = P->osx_lpi;
+    a.n_groups = Nv / a.lpi;
+    const size_t smem = osx_smem_bytes(a.lpi, a.nb);
+    if (P->osx_occ == 0) {
+        P->osx_occ = osx_occupancy(P->osx_thr, smem);
+        if (P->osx_occ <= 0) return cudaErrorInvalidConfiguration;
+    }
+    const int cps = (P->osx_cps > 0 && P->osx_cps < P->osx_occ) ? P->osx_cps : P->osx_occ;
+    int grid = cps * P->n_sm;
+    if (grid > a.n_groups) grid = a.n_groups;
+    P->launches++;
+    return osx_launch(a, grid, P->osx_thr, smem, P->st);
+}
+
+static size_t osv_smem_bytes(int np_log, int rb)
+{
+    const size_t np = (size_t)1 << np_log;
+    return (size_t)rb * 272 * np * 8 + 2 * np * 131 * 8 + 240 * 8 + 16;
+}
+
+static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool source)
+{
+    OsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
+    a.nb = (Nv + OS_V - 1) / OS_V;
+    a.lam = P->os_lam_v; a.tw = P->os_twv; a.cs = P->os_cs;
+    a.np_log = P->osv_np_log; a.rb = P->osv_rb;
+    a.ng = source ? P->p.feq.n : 0;
+    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab;
+    for (int g = 0; g < 4; ++g) a.cg[g] = g < P->p.feq.n ? (float)P->p.feq.c[g] : 0.0f;
+    const int strips = Nx >> (a.np_log + 1);
+    const int ngroups = (a.nb + a.rb - 1) / a.rb;
+    int gpc = P->osv_gpc;
+    if (gpc <= 0) {                       // enough CTAs to fill the chip 8 deep, else one group per CTA
+        gpc = (int)(((long long)strips * ngroups) / ((long long)P->n_sm * 8));
+        if (gpc < 1) gpc = 1;
+    }
+    if (gpc > ngroups) gpc = ngroups;
+    a.gpc = gpc;
+    dim3 grid(strips, (ngroups + gpc - 1) / gpc);
+    P->launches++;
+    return osv_launch(a, grid, P->osv_thr, osv_smem_bytes(a.np_log, a.rb), P->st);
 }
 
 static cudaError_t run_advect_x(vog_plan_s* P, float* f)
@@ -621,7 +740,7 @@ static cudaError_t run_advect_x(vog_plan_s* P, float* f)
     return fn(a, P->sym, grid, P->x_thr, smem, P->st);
 }
 
-static cudaError_t run_advect(vog_plan_s* P, float* f, bool vdir, bool source)
+static cudaError_t run_advect_line(vog_plan_s* P, float* f, bool vdir, bool source)
 {
     if (!vdir) return run_advect_x(P, f);
     AdvectArgs a;
@@ -641,6 +760,47 @@ static cudaError_t run_advect(vog_plan_s* P, float* f, bool vdir, bool source)
     if (!fn) return cudaErrorInvalidValue;
     P->launches++;
     return fn(a, P->sym, vdir, n_tiles, vdir ? P->thr_v : P->thr_x, advect_smem_bytes(N, lognl), P->st);
+}
+
+static cudaError_t ensure_gbuf(vog_plan_s* P)
+{
+    if (P->g_buf) return cudaSuccess;
+    return cudaMalloc((void**)&P->g_buf, sizeof(float) * (size_t)P->p.Nx * P->p.Nv);
+}
+
+static cudaError_t copy_grid(vog_plan_s* P, float* dst, const float* src)
+{
+    return cudaMemcpyAsync(dst, src, sizeof(float) * (size_t)P->p.Nx * P->p.Nv, cudaMemcpyDeviceToDevice, P->st);
+}
+
+// x-advection src -> dst (dst may equal src); the shift records/tables must be current
+static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
+{
+    if (P->os_x) return run_osx(P, src, dst);
+    cudaError_t e = cudaSuccess;
+    if (src != dst) e = copy_grid(P, dst, src);
+    if (e == cudaSuccess) e = run_advect_line(P, dst, false, false);
+    return e;
+}
+
+// v-advection src -> dst; the overlap-save kernel needs dst != src, the whole-line kernel works in place
+static cudaError_t advect_v(vog_plan_s* P, const float* src, float* dst, bool source)
+{
+    if (P->os_v) return src == dst ? cudaErrorInvalidValue : run_osv(P, src, dst, source);
+    cudaError_t e = cudaSuccess;
+    if (src != dst) e = copy_grid(P, dst, src);
+    if (e == cudaSuccess) e = run_advect_line(P, dst, true, source);
+    return e;
+}
+
+// in-place v-advection through the plan's second grid buffer when the kernel is out of place
+static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
+{
+    if (!P->os_v) return run_advect_line(P, f, true, source);
+    cudaError_t e = ensure_gbuf(P);
+    if (e == cudaSuccess) e = run_osv(P, f, P->g_buf, source);
+    if (e == cudaSuccess) e = copy_grid(P, f, P->g_buf);
+    return e;
 }
 
 static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
@@ -678,7 +838,7 @@ extern "C" int vog_advect_x(vog_plan_t P, float* f_dev, double dt)
 {
     if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
     cudaError_t e = ensure_recx(P, dt);
-    if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+    if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
     return cuda_status(e);
 }
 
@@ -686,7 +846,7 @@ extern "C" int vog_advect_v(vog_plan_t P, float* f_dev, const float* E_dev, doub
 {
     if (!P || !f_dev || !E_dev || !std::isfinite(dt)) return VOG_EINVAL;
     cudaError_t e = run_setup(P, true, 1, dt, E_dev, nullptr, nullptr);
-    if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+    if (e == cudaSuccess) e = advect_v_inplace(P, f_dev, true);
     return cuda_status(e);
 }
 
@@ -695,7 +855,7 @@ extern "C" int vog_shift_x(vog_plan_t P, float* f_dev, const double* beta)
     if (!P || !f_dev || !beta) return VOG_EINVAL;
     P->recx_valid = false;
     cudaError_t e = run_setup(P, false, 2, 0.0, nullptr, nullptr, beta);
-    if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+    if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
     return cuda_status(e);
 }
 
@@ -703,7 +863,7 @@ extern "C" int vog_shift_v(vog_plan_t P, float* f_dev, const double* beta)
 {
     if (!P || !f_dev || !beta) return VOG_EINVAL;
     cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
-    if (e == cudaSuccess) e = run_advect(P, f_dev, true, false);
+    if (e == cudaSuccess) e = advect_v_inplace(P, f_dev, false);
     return cuda_status(e);
 }
 
@@ -722,24 +882,31 @@ extern "C" int vog_get_field(vog_plan_t P, float* E_dev)
 extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ext_dev)
 {
     if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
-    cudaError_t e;
+    cudaError_t e = cudaSuccess;
+    // The overlap-save v kernel is out of place: it writes the plan's second grid g, and the x-advection
+    // that follows reads g and writes f, so a step moves no extra bytes.
+    float* g = f_dev;
+    if (P->os_v) {
+        e = ensure_gbuf(P);
+        if (e != cudaSuccess) { cudaGetLastError(); return VOG_ENOMEM; }
+        g = P->g_buf;
+    }
     if (P->p.split == VOG_SPLIT_XVX) {
         e = ensure_recx(P, 0.5 * dt);
-        if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+        if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
         if (e == cudaSuccess) e = run_field(P, f_dev, nullptr);
         if (e == cudaSuccess) e = run_setup(P, true, 1, dt, P->E_self, E_ext_dev, nullptr);
-        if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
-        if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
+        if (e == cudaSuccess) e = advect_v(P, f_dev, g, true);
+        if (e == cudaSuccess) e = advect_x(P, g, f_dev);
     } else {
-        e = cudaSuccess;
         if (!P->E_valid) e = run_field(P, f_dev, nullptr);
         if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
-        if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+        if (e == cudaSuccess) e = advect_v(P, f_dev, g, true);
         if (e == cudaSuccess) e = ensure_recx(P, dt);
-        if (e == cudaSuccess) e = run_advect(P, f_dev, false, false);
-        if (e == cudaSuccess) e = run_field(P, f_dev, nullptr);
+        if (e == cudaSuccess) e = advect_x(P, g, g);
+        if (e == cudaSuccess) e = run_field(P, g, nullptr);
         if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
-        if (e == cudaSuccess) e = run_advect(P, f_dev, true, true);
+        if (e == cudaSuccess) e = advect_v(P, g, f_dev, true);
     }
     return cuda_status(e);
 }

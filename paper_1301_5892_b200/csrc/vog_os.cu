@@ -1,0 +1,123 @@
+// vog_os.cu -- overlap-save advection kernels: instantiation, launchers and the fp64 setup kernel that
+// tabulates the symbol lambda(theta_k) per line (S1 + the closed form of S4).  Product code.
+#include "vog_os.cuh"
+
+namespace vog {
+
+// One CTA per line, thread k = 0..129.  beta = -c dt / Delta in fp64; b = floor(beta), b* = beta - b.
+//   Lagrange 2d+1, Everett form: lambda = P(s;1-b*) + e^{i theta} P(s;b*), s = 2 - 2 cos(theta),
+//     P(s;t) = sum_k a_k(t) s^k, a_0 = t, a_k = a_{k-1} (k^2 - t^2) / (2k (2k+1));
+//   cubic spline: [B(b*+1) e^{-i theta} + B(b*) + B(b*-1) e^{i theta} + B(b*-2) e^{2 i theta}] 3/(2 + cos(theta)).
+__global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
+{
+    const int l = blockIdx.x, k = threadIdx.x;
+    if (l >= s.n_lines || k >= OS_LAMW) return;
+    double beta;
+    float sshift = 0.0f;
+    if (s.mode == 0) {
+        beta = -(s.vmin + (double)l * s.dv) * s.dt / s.delta;
+    } else if (s.mode == 1) {
+        double e = (double)s.E[l];
+        if (s.Eext) e += (double)s.Eext[l];
+        beta = -e * s.dt / s.delta;
+        sshift = (float)(s.dt * e);
+    } else {
+        beta = s.beta[l];
+    }
+    const double fl = floor(beta);
+    const double t = beta - fl;
+    double bm = fmod(fl, (double)s.N);
+    if (bm < 0.0) bm += (double)s.N;
+    int b = (int)bm;
+    if (b >= s.N) b = 0;
+    const int br = s.vdir ? 0 : (b & 3);
+    float2* out = s.lam + (size_t)l * OS_LAMW;
+    if (k == 129) {
+        out[129] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift);
+        return;
+    }
+    const double sc = 1.0 / (2.0 * (double)OS_LB);
+    if (k == 0) { out[0] = make_float2((float)sc, 0.0f); return; }   // lambda_0 = sum of the weights = 1
+    double c, sn;
+    sincospi((double)k / (double)(OS_LB / 2), &sn, &c);
+    double lr, li;
+    if (s.spline) {
+        const double u = 1.0 - t;
+        const double Bm1 = u * u * u / 6.0, B0 = (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0;
+        const double B1 = (1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0, B2 = t * t * t / 6.0;
+        const double c2 = 2.0 * c * c - 1.0, s2 = 2.0 * sn * c;
+        const double g = 3.0 / (2.0 + c);
+        lr = (B0 + (Bm1 + B1) * c + B2 * c2) * g;
+        li = ((B1 - Bm1) * sn + B2 * s2) * g;
+    } else {
+        const double sv = 2.0 - 2.0 * c;
+        double p[2];
+        for (int half = 0; half < 2; ++half) {
+            const double tt = half == 0 ? 1.0 - t : t;
+            double a = tt, pw = 1.0, acc = 0.0;
+            for (int j = 0; j <= s.d; ++j) {
+                if (j > 0) a = a * ((double)(j * j) - tt * tt) / (double)(2 * j * (2 * j + 1));
+                acc += a * pw;
+                pw *= sv;
+            }
+            p[half] = acc;
+        }
+        lr = p[0] + c * p[1];
+        li = sn * p[1];
+    }
+    if (br) {
+        double rc, rs;
+        sincospi((double)(k * br) / (double)(OS_LB / 2), &rs, &rc);
+        const double xr = lr * rc - li * rs, xi = lr * rs + li * rc;
+        lr = xr; li = xi;
+    }
+    out[k] = make_float2((float)(lr * sc), (float)(li * sc));
+}
+
+cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
+{
+    os_setup_kernel<<<s.n_lines, 160, 0, st>>>(s);
+    return cudaGetLastError();
+}
+
+static cudaError_t set_smem(const void* fn, size_t smem, size_t* cur)
+{
+    if (smem > 48 * 1024 && smem > *cur) {
+        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        *cur = smem;
+    }
+    return cudaSuccess;
+}
+
+cudaError_t osx_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    cudaError_t e = set_smem((const void*)osx_kernel, smem, &cur);
+    if (e != cudaSuccess) return e;
+    osx_kernel<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    cudaError_t e = set_smem((const void*)osv_kernel, smem, &cur);
+    if (e != cudaSuccess) return e;
+    osv_kernel<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+int osx_occupancy(int threads, size_t smem)
+{
+    static size_t cur = 0;
+    if (set_smem((const void*)osx_kernel, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx_kernel, threads, smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return nb;
+}
+
+}  // namespace vog

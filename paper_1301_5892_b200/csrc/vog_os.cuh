@@ -1,0 +1,427 @@
+// vog_os.cuh -- overlap-save advection kernels (line length N >= 1024).
+// Product code; shares nothing with oracle/.
+//
+// The circulant interpolation matrix A of P:98-100 has a SHORT first row: 2d+2 non-zeros for Lagrange
+// 2d+1, and an exponentially decaying one for the cubic spline (|a_j| ~ 0.268^|j|,
+// P:117-129).  u' = A u is therefore a short cyclic convolution, and the Fourier-space product of
+// P:131-149 can be taken block-wise (overlap-save): every block of LB = 256 samples of the rolled line
+// r_i = u_{i+b} is transformed, multiplied by the symbol lambda(theta_k), theta_k = 2 pi k / LB, and
+// transformed back; the V = 224 samples in the middle of the block are exactly (Lagrange) or to
+// 0.268^17 ~ 2e-10 (spline, far below fp32 rounding) the samples of A u, the H = 16 on either side are
+// discarded.  Compared with one length-N transform per line:
+//   * 8 instead of log2(N) butterfly levels, two passes instead of three, no big twiddle table;
+//   * the symbol is a per-line table lam[k], k = 0..128, computed in fp64 by the setup kernel and shared
+//     by all blocks of the line -- no polynomial evaluation in the hot loop;
+//   * the integer part b of the shift is folded into the load address ("integer roll by
+//     index"): no rotation factor at all (x keeps a residual b mod 4 in the table to stay 128-bit aligned);
+//   * the working set of a block is 1-2 KB, so the strided (v) direction can use tiles 16-32 columns
+//     wide at ANY Nv: full 32-byte sectors, no shared-memory capacity limit.
+// x-direction: even/odd packing (a block is 128 complex), CTA owns whole lines, in place.
+// v-direction: two-for-one over adjacent columns (a block is 256 complex per column pair), OUT of place
+//   (src != dst): a block reads rows that other blocks write, so in-place would race.
+#pragma once
+#include "vog_fft.cuh"
+#include "vog_internal.h"
+
+namespace vog {
+
+__device__ __forceinline__ void os_cp_async16(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void os_cp_async_commit_wait()
+{
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
+}
+
+// scratch swizzle for the x kernel: chunk C (16 B = 2 complex) of the block-major scratch; key mixes the
+// radix-16 group (C >> 3) & 7 and the parity of the block (C >> 6) & 1 so that the 8 lanes of a
+// quarter-warp (4 items x 2 blocks) hit 8 distinct 16-byte bank groups in the middle stage.
+__device__ __forceinline__ int os_swz(int C) { return C ^ (((C >> 3) ^ ((C >> 4) & 4)) & 7); }
+
+// One mirror pair (k, M-k) of the half-length spectrum of an even/odd packed real block:
+// untangle, multiply by the tabulated symbol, re-tangle.  P = Z_k, Qm = Z_{M-k}; cs = (cos, sin)(2 pi k/LB);
+// a = lambda_k/(2 LB), cc = conj(lambda_{M-k})/(2 LB).
+__device__ __forceinline__ void os_pair_x(float2& P, float2& Qm, const float2 cs, const float2 a, const float2 cc)
+{
+    const float c = cs.x, s = cs.y;
+    const float2 E2 = make_float2(P.x + Qm.x, P.y - Qm.y);
+    const float2 D2 = make_float2(P.x - Qm.x, P.y + Qm.y);
+    const float2 T2 = make_float2(fmaf(c, D2.y, -s * D2.x), -fmaf(c, D2.x, s * D2.y));
+    const float2 Up = cadd(E2, T2), Um = csub(E2, T2);
+    const float2 Vp = cmul(a, Up), Vm = cmul(cc, Um);
+    const float2 Ep = cadd(Vp, Vm), Dp = csub(Vp, Vm);
+    const float2 Op = make_float2(fmaf(c, Dp.x, -s * Dp.y), fmaf(c, Dp.y, s * Dp.x));
+    P = make_float2(Ep.x - Op.y, Ep.y + Op.x);
+    Qm = make_float2(Ep.x + Op.y, Op.x - Ep.y);
+}
+
+// Two-for-one pair (m, LB-m) of the spectrum of z = uA + i uB: P = Z_m, Q = Z_{LB-m};
+// la, lb = lambda_m/(2 LB) of line A and line B.
+__device__ __forceinline__ void os_pair_v(float2& P, float2& Q, const float2 la, const float2 lb)
+{
+    const float2 ua = make_float2(P.x + Q.x, P.y - Q.y);      // 2 U_A = P + conj Q
+    const float2 ub = make_float2(P.y + Q.y, Q.x - P.x);      // 2 U_B = (P - conj Q)/i
+    const float2 wa = cmul(la, ua), wb = cmul(lb, ub);
+    P = make_float2(wa.x - wb.y, wa.y + wb.x);                // W_A + i W_B
+    Q = make_float2(wa.x + wb.y, wb.x - wa.y);                // conj(W_A) + i conj(W_B)
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// x-direction.  Block of LB = 256 reals = 128 complex = radix 8 (stride 16) x radix 16.
+// Scratch: 64 chunks (1 KB) per block, chunk index = group*8 + (position in group)/2, swizzled.
+namespace osx {
+constexpr int MB = OS_LB / 2;      // complex length of a block
+constexpr int CPB = MB / 2;        // chunks per block (64)
+constexpr int VC = OS_V / 4;       // valid chunks per block (56)
+constexpr int HC = OS_H / 4;       // halo chunks (4)
+}
+
+// forward pass A of one item: two adjacent radix-8 butterflies (positions 2tp, 2tp+1 + 16k)
+__device__ __forceinline__ void osx_fwd(const float4* __restrict__ gline, const int nchunk_mask, const int wc0,
+                                        float4* __restrict__ scr, const int cb, const int tp,
+                                        const float2* __restrict__ twS)
+{
+    float2 x0[8], x1[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const float4 v = __ldg(gline + ((wc0 + tp + 8 * k) & nchunk_mask));
+        x0[k] = make_float2(v.x, v.y);
+        x1[k] = make_float2(v.z, v.w);
+    }
+    dft_dif<8, 1>(x0);
+    dft_dif<8, 1>(x1);
+    const int par = (cb >> 4) & 4;
+    scr[cb + (tp ^ par)] = make_float4(x0[0].x, x0[0].y, x1[0].x, x1[0].y);
+    const float4* __restrict__ tw4 = reinterpret_cast<const float4*>(twS) + tp;
+#pragma unroll
+    for (int q = 1; q < 8; ++q) {
+        const float4 w = tw4[(q - 1) * 8];
+        const float2 y0 = cmul(x0[brev(q, 8)], make_float2(w.x, w.y));
+        const float2 y1 = cmul(x1[brev(q, 8)], make_float2(w.z, w.w));
+        scr[cb + q * 8 + (tp ^ ((q ^ par) & 7))] = make_float4(y0.x, y0.y, y1.x, y1.y);
+    }
+}
+
+// inverse pass A of one item; stores the valid chunks of the block (+ the block mean dc)
+__device__ __forceinline__ void osx_inv(float4* __restrict__ gline, const int nchunk, const int oc0,
+                                        const float4* __restrict__ scr, const int cb, const int tp,
+                                        const float2* __restrict__ twS, const float dc)
+{
+    float2 x0[8], x1[8];
+    const int par = (cb >> 4) & 4;
+    {
+        const float4 v = scr[cb + (tp ^ par)];
+        x0[0] = make_float2(v.x, v.y);
+        x1[0] = make_float2(v.z, v.w);
+    }
+    const float4* __restrict__ tw4 = reinterpret_cast<const float4*>(twS) + tp;
+#pragma unroll
+    for (int q = 1; q < 8; ++q) {
+        const float4 v = scr[cb + q * 8 + (tp ^ ((q ^ par) & 7))];
+        const float4 w = tw4[(q - 1) * 8];
+        x0[brev(q, 8)] = cmulc(make_float2(v.x, v.y), make_float2(w.x, w.y));
+        x1[brev(q, 8)] = cmulc(make_float2(v.z, v.w), make_float2(w.z, w.w));
+    }
+    idft_dit<8, 1>(x0);
+    idft_dit<8, 1>(x1);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int c = tp + 8 * k;                    // chunk inside the window
+        const int oc = oc0 + c - osx::HC;            // chunk of the line
+        if (c >= osx::HC && c < osx::HC + osx::VC && oc < nchunk)
+            __stcs(gline + oc, make_float4(x0[k].x + dc, x0[k].y + dc, x1[k].x + dc, x1[k].y + dc));
+    }
+}
+
+// middle stage of one item (two mirror groups of 16 complex): radix 16, untangle, symbol, re-tangle,
+// inverse radix 16.  Same slot layout and "special item" permutation as symbol_item_x (vog_advect_x.cuh).
+__device__ __forceinline__ void osx_mid(float4* __restrict__ scr, const int cb, const int u,
+                                        const float2* __restrict__ lamS, const float2* __restrict__ csS,
+                                        float* __restrict__ dc)
+{
+    constexpr int M = osx::MB, ML = M / 16;          // 128, 8
+    const bool special = (u == 0);
+    const int gA = u, gB = special ? 4 : 8 - u;
+    const int par = (cb >> 4) & 4;
+    const int pa = cb + gA * 8, pb = cb + gB * 8;
+    const int xa = (gA ^ par) & 7, xb = (gB ^ par) & 7;
+    float2 XA[16], XB[16];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const float4 va = scr[pa + (j ^ xa)], vb = scr[pb + (j ^ xb)];
+        XA[2 * j] = make_float2(va.x, va.y); XA[2 * j + 1] = make_float2(va.z, va.w);
+        XB[2 * j] = make_float2(vb.x, vb.y); XB[2 * j + 1] = make_float2(vb.z, vb.w);
+    }
+    dft_dif<16, 1>(XA);
+    dft_dif<16, 1>(XB);
+    const float2 z0 = XA[0];
+    if (special) {
+        float2 TA[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) TA[i] = XA[i];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) XA[brev(q, 16)] = XB[brev(q, 16)];
+#pragma unroll
+        for (int q = 8; q < 15; ++q) { XA[brev(q, 16)] = TA[brev(q - 7, 16)]; XB[brev(15 - q, 16)] = TA[brev(23 - q, 16)]; }
+        XA[brev(15, 16)] = TA[brev(8, 16)];
+        XB[brev(0, 16)] = TA[brev(8, 16)];
+    }
+    const int klo = special ? ML / 2 : u;            // slots 0..7:  k = klo + ML q
+    const int khi = special ? -7 * ML : u;           // slots 8..15: k = khi + ML q
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int k = (q < 8 ? klo : khi) + ML * q;
+        const float2 a = lamS[k], lm = lamS[M - k];
+        os_pair_x(XA[brev(q, 16)], XB[brev(15 - q, 16)], csS[k], a, make_float2(lm.x, -lm.y));
+    }
+    if (special) {
+        float2 TA[16], TB[8];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) TA[i] = XA[i];
+#pragma unroll
+        for (int j = 1; j < 8; ++j) TB[j] = XB[brev(j, 16)];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) XB[brev(q, 16)] = TA[brev(q, 16)];
+#pragma unroll
+        for (int i = 1; i < 8; ++i) {
+            XA[brev(i, 16)] = TA[brev(i + 7, 16)];
+            XA[brev(16 - i, 16)] = TB[8 - i];
+        }
+        XA[brev(8, 16)] = TA[brev(15, 16)];
+        // block modes 0 and LB/2: U_0 = x + y, U_M = x - y; lambda_0 = 1 exactly (lam[0] = (1/(2 LB), 0)).
+        // The block mean A0 by-passes the inverse transform and is added back in the last pass.
+        const float A0 = 2.0f * lamS[0].x * (z0.x + z0.y), Bn = 2.0f * lamS[M].x * (z0.x - z0.y);
+        XA[0] = make_float2(Bn, -Bn);
+        *dc = A0;
+    }
+    idft_dit<16, 1>(XA);
+    idft_dit<16, 1>(XB);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        scr[pa + (j ^ xa)] = make_float4(XA[2 * j].x, XA[2 * j].y, XA[2 * j + 1].x, XA[2 * j + 1].y);
+        scr[pb + (j ^ xb)] = make_float4(XB[2 * j].x, XB[2 * j].y, XB[2 * j + 1].x, XB[2 * j + 1].y);
+    }
+}
+
+// Persistent kernel: one iteration = lpi whole lines (a CTA owns whole lines, so src may equal dst: all
+// loads of a line happen before the barrier that precedes its first store).
+__global__ void __launch_bounds__(160, 3) osx_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lpi = a.lpi, nb = a.nb;
+    float4* const scr = reinterpret_cast<float4*>(smem_raw);                        // lpi*nb*64 chunks
+    float2* const lamS = reinterpret_cast<float2*>(scr + lpi * nb * osx::CPB);      // lpi*OS_LAMW
+    float2* const csS = lamS + lpi * OS_LAMW;                                       // 130
+    float2* const twS = csS + 130;                                                  // 7*16
+    float* const dcS = reinterpret_cast<float*>(twS + 112);                         // lpi*nb
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int nchunk = a.N >> 2;
+
+    for (int i = tid; i < 129; i += T) csS[i] = __ldg(a.cs + i);
+    for (int i = tid; i < 112; i += T) twS[i] = __ldg(a.tw + i);
+
+    for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
+        const int line0 = g * lpi;
+        __syncthreads();                           // previous iteration done with scratch and tables
+        {
+            const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
+            float4* dst4 = reinterpret_cast<float4*>(lamS);
+            for (int i = tid; i < lpi * (OS_LAMW / 2); i += T) os_cp_async16(dst4 + i, src4 + i);
+        }
+        // ---- pass A: global -> registers -> scratch
+#pragma unroll 1
+        for (int w = tid; w < lpi * nb * 8; w += T) {
+            const int lb = w >> 3, tp = w & 7;      // (line, block) flattened, item in block
+            const int l = lb / nb, blk = lb - l * nb;
+            const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
+            const int wc0 = (osx::VC * blk - osx::HC + b4) & (nchunk - 1);
+            const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
+            osx_fwd(gline, nchunk - 1, wc0, scr, lb * osx::CPB, tp, twS);
+        }
+        os_cp_async_commit_wait();
+        __syncthreads();
+        // ---- middle stage
+#pragma unroll 1
+        for (int w = tid; w < lpi * nb * 4; w += T) {
+            const int lb = w >> 2, u = w & 3;
+            const int l = lb / nb;
+            osx_mid(scr, lb * osx::CPB, u, lamS + l * OS_LAMW, csS, dcS + lb);
+        }
+        __syncthreads();
+        // ---- inverse pass A: scratch -> registers -> global
+#pragma unroll 1
+        for (int w = tid; w < lpi * nb * 8; w += T) {
+            const int lb = w >> 3, tp = w & 7;
+            const int l = lb / nb, blk = lb - l * nb;
+            float4* gline = reinterpret_cast<float4*>(a.dst) + (size_t)(line0 + l) * nchunk;
+            osx_inv(gline, nchunk, osx::VC * blk, scr, lb * osx::CPB, tp, twS, dcS[lb]);
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// v-direction.  Strip of NP column pairs; a block is LB = 256 rows of one pair = 256 complex =
+// radix 16 (stride 16) x radix 16.  Scratch per block: [padded position][pair] float2, one position of
+// padding per 16 (conflict-free 64-bit accesses in both passes).  Lanes run over the pairs first, so a
+// row segment of 8 NP bytes is contiguous in global memory.
+namespace osv {
+constexpr int PADLEN = OS_LB + OS_LB / 16;     // 272 padded positions
+constexpr int LS = 131;                        // shared-memory stride (float2) of one column's symbol table
+}
+
+__global__ void __launch_bounds__(128, 4) osv_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int npl = a.np_log, np = 1 << npl, rb = a.rb, nb = a.nb;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // rb * PADLEN * np
+    float2* const lamS = scr + rb * osv::PADLEN * np;                         // 2 np * LS
+    float2* const twS = lamS + 2 * np * osv::LS;                              // 15 * 16
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int Nx = a.Nx, Nv = a.Nv;
+    const int c0 = blockIdx.x * 2 * np;
+
+    for (int i = tid; i < 2 * np * OS_LAMW; i += T) {
+        const int col = i / OS_LAMW, k = i - col * OS_LAMW;
+        lamS[col * osv::LS + k] = __ldg(a.lam + (size_t)(c0 + col) * OS_LAMW + k);
+    }
+    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
+    __syncthreads();
+
+    const int ngroups = (nb + rb - 1) / rb;
+    const int g1 = min(ngroups, ((int)blockIdx.y + 1) * a.gpc);
+    for (int gi = blockIdx.y * a.gpc; gi < g1; ++gi) {
+        // ---- pass A: global -> registers -> scratch (radix 16 over rows t + 16 k)
+#pragma unroll 1
+        for (int w = tid; w < rb * 16 * np; w += T) {
+            const int p = w & (np - 1), t = (w >> npl) & 15, bl = w >> (npl + 4);
+            const int blk = gi * rb + bl;
+            if (blk >= nb) continue;
+            const int bA = __float_as_int(lamS[(2 * p) * osv::LS + 129].x);
+            const int bB = __float_as_int(lamS[(2 * p + 1) * osv::LS + 129].x);
+            const int r0 = blk * OS_V - OS_H + t;
+            const float* colA = a.src + c0 + 2 * p;
+            float2 x[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const int rA = (r0 + 16 * k + bA) & (Nv - 1), rB = (r0 + 16 * k + bB) & (Nv - 1);
+                x[k] = make_float2(__ldg(colA + (size_t)rA * Nx), __ldg(colA + (size_t)rB * Nx + 1));
+            }
+            dft_dif<16, 1>(x);
+            float2* o = scr + (bl * osv::PADLEN + t) * np + p;
+            o[0] = x[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) o[q * 17 * np] = cmul(x[brev(q, 16)], twS[(q - 1) * 16 + t]);
+        }
+        __syncthreads();
+        // ---- middle stage: radix 16, two-for-one separation, symbols, recombination, inverse radix 16
+#pragma unroll 1
+        for (int w = tid; w < rb * 8 * np; w += T) {
+            const int p = w & (np - 1), u = (w >> npl) & 7, bl = w >> (npl + 3);
+            if (gi * rb + bl >= nb) continue;
+            const bool special = (u == 0);
+            const int gA = u, gB = special ? 8 : 16 - u;
+            float2* const sa = scr + (bl * osv::PADLEN + gA * 17) * np + p;
+            float2* const sb = scr + (bl * osv::PADLEN + gB * 17) * np + p;
+            float2 XA[16], XB[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) { XA[j] = sa[j * np]; XB[j] = sb[j * np]; }
+            dft_dif<16, 1>(XA);
+            dft_dif<16, 1>(XB);
+            const float2 z0 = XA[0];
+            if (special) {
+                float2 TA[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) TA[i] = XA[i];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) XA[brev(q, 16)] = XB[brev(q, 16)];
+#pragma unroll
+                for (int q = 8; q < 15; ++q) { XA[brev(q, 16)] = TA[brev(q - 7, 16)]; XB[brev(15 - q, 16)] = TA[brev(23 - q, 16)]; }
+                XA[brev(15, 16)] = TA[brev(8, 16)];
+                XB[brev(0, 16)] = TA[brev(8, 16)];
+            }
+            // slot q: P = Z_m in XA[brev q], Q = Z_{LB-m} in XB[brev(15-q)];
+            //   q < 8 : m = mlo + 16 q              (<= 127)
+            //   q >= 8: special: m = 16 (q - 7);  else m = u + 16 q > 128: lambda_m = conj(lambda_{LB-m})
+            const int mlo = special ? 8 : u;
+            const int mh0 = special ? -112 : OS_LB - u, mh1 = special ? 16 : -16;
+            const float sgh = special ? 1.0f : -1.0f;
+            const float2* const lA = lamS + (2 * p) * osv::LS;
+            const float2* const lB = lA + osv::LS;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const int m = q < 8 ? mlo + 16 * q : mh0 + mh1 * q;
+                float2 la = lA[m], lb = lB[m];
+                if (q >= 8) { la.y *= sgh; lb.y *= sgh; }
+                os_pair_v(XA[brev(q, 16)], XB[brev(15 - q, 16)], la, lb);
+            }
+            if (special) {
+                float2 TA[16], TB[8];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) TA[i] = XA[i];
+#pragma unroll
+                for (int j = 1; j < 8; ++j) TB[j] = XB[brev(j, 16)];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) XB[brev(q, 16)] = TA[brev(q, 16)];
+#pragma unroll
+                for (int i = 1; i < 8; ++i) {
+                    XA[brev(i, 16)] = TA[brev(i + 7, 16)];
+                    XA[brev(16 - i, 16)] = TB[8 - i];
+                }
+                XA[brev(8, 16)] = TA[brev(15, 16)];
+                // mode 0 of both lines: lambda_0 = 1 exactly, Y_0 = Z_0 / LB
+                const float s0 = 2.0f * lA[0].x;
+                XA[0] = make_float2(z0.x * s0, z0.y * s0);
+            }
+            idft_dit<16, 1>(XA);
+            idft_dit<16, 1>(XB);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) { sa[j * np] = XA[j]; sb[j * np] = XB[j]; }
+        }
+        __syncthreads();
+        // ---- inverse pass A: scratch -> registers -> global (+ delta-f source); rows k = 1..14 are valid
+#pragma unroll 1
+        for (int w = tid; w < rb * 16 * np; w += T) {
+            const int p = w & (np - 1), t = (w >> npl) & 15, bl = w >> (npl + 4);
+            const int blk = gi * rb + bl;
+            if (blk >= nb) continue;
+            const float2* o = scr + (bl * osv::PADLEN + t) * np + p;
+            float2 x[16];
+            x[0] = o[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(o[q * 17 * np], twS[(q - 1) * 16 + t]);
+            idft_dit<16, 1>(x);
+            const int row0 = blk * OS_V + t - OS_H;           // + 16 k
+            if (a.ng > 0) {
+                const float sA = lamS[(2 * p) * osv::LS + 129].y, sB = lamS[(2 * p + 1) * osv::LS + 129].y;
+                for (int g = 0; g < a.ng; ++g) {
+                    const float cg = a.cg[g];
+                    const float* __restrict__ ft = a.feq_tab + (size_t)g * Nv;
+                    const float* __restrict__ vt = a.vmu_tab + (size_t)g * Nv;
+#pragma unroll
+                    for (int k = 1; k < 15; ++k) {
+                        const int j = row0 + 16 * k;
+                        if (j < Nv) {
+                            const float fe = __ldg(ft + j), vm2 = 2.0f * __ldg(vt + j);
+                            // f_eq,g(v - s) - f_eq,g(v) = f_eq,g(v) expm1(c s (2 (v - mu) - s))
+                            x[k].x = fmaf(fe, expm1f(cg * sA * (vm2 - sA)), x[k].x);
+                            x[k].y = fmaf(fe, expm1f(cg * sB * (vm2 - sB)), x[k].y);
+                        }
+                    }
+                }
+            }
+            float* colA = a.dst + c0 + 2 * p;
+#pragma unroll
+            for (int k = 1; k < 15; ++k) {
+                const int j = row0 + 16 * k;
+                if (j < Nv) __stcs(reinterpret_cast<float2*>(colA + (size_t)j * Nx), x[k]);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace vog
