@@ -33,16 +33,23 @@ __host__ __device__ constexpr int brev(int q, int R)
 }
 __host__ __device__ constexpr int ilog2(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Complex arithmetic on packed fp32 pairs (sm_100 FADD2/FMUL2/FFMA2: the same 128 fp32 lanes/cycle/SM as
+// the scalar forms but half the issue slots; operand swap / negate / broadcast are instruction modifiers,
+// so conj() and multiplication by +-i cost nothing).  Results are bit-identical to the scalar forms.
+__device__ __forceinline__ float fneg(float x) { return __int_as_float(__float_as_int(x) ^ 0x80000000); }  // ALU pipe
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+// a * b = a.x (b.x, b.y) + a.y (-b.y, b.x)
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 {
-    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+    const float2 t = __fmul2_rn(make_float2(a.y, a.y), make_float2(fneg(b.y), b.x));
+    return __ffma2_rn(make_float2(a.x, a.x), b, t);
 }
-// a * conj(b)
+// a * conj(b) = a.x (b.x, -b.y) + a.y (b.y, b.x)
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b)
 {
-    return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y));
+    const float2 t = __fmul2_rn(make_float2(a.y, a.y), make_float2(b.y, b.x));
+    return __ffma2_rn(make_float2(a.x, a.x), make_float2(b.x, fneg(b.y)), t);
 }
 
 // multiply by the compile-time root e^{-/+ 2 pi i K / R} (forward: minus; INV: plus)
@@ -57,7 +64,9 @@ __device__ __forceinline__ float2 mul_root(float2 d)
     else {
         constexpr float c = (float)cos32(k32);
         constexpr float s = INV ? (float)sin32(k32) : -(float)sin32(k32);
-        return make_float2(fmaf(d.x, c, -d.y * s), fmaf(d.x, s, d.y * c));
+        // (d.x c - d.y s, d.x s + d.y c)
+        const float2 t = __fmul2_rn(make_float2(d.y, d.y), make_float2(-s, c));
+        return __ffma2_rn(make_float2(d.x, d.x), make_float2(c, s), t);
     }
 }
 

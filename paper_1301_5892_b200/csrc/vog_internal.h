@@ -71,6 +71,7 @@ struct OsArgs {
     const float2* tw;      // x: [7][16] e^{-2 pi i t q/128};  v: [15][16] e^{-2 pi i t q/256}
     const float2* cs;      // [129] (cos, sin)(2 pi k/256)   (x only)
     int lpi, n_groups;     // x: lines per iteration, n_lines / lpi
+    unsigned inv_nb;       // x: ceil(2^16 / nb)
     int np_log, rb, gpc;   // v: log2(column pairs per strip), row blocks per group, groups per CTA
     int ng;                // v: Gaussians of f_eq (0 = no source)
     const float* feq_tab;  // [ng][Nv]
@@ -85,6 +86,7 @@ struct OsSetupArgs {
     const float* E;
     const float* Eext;
     const double* beta;
+    const double2* cs64;       // [OS_LB] (cos, sin)(2 pi j / OS_LB) in fp64
     float2* lam;
 };
 

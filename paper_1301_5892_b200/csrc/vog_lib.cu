@@ -310,6 +310,7 @@ struct vog_plan_s {
     bool os_x, os_v;
     float2 *os_lam_x, *os_lam_v;   // symbol tables [Nv][OS_LAMW], [Nx][OS_LAMW]
     float2 *os_twx, *os_twv, *os_cs;
+    double2* os_cs64;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int osx_lpi, osx_thr, osx_cps, osx_occ;
     int osv_np_log, osv_thr, osv_rb, osv_gpc;
@@ -451,7 +452,7 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
-    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs);
+    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64);
     cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
@@ -508,7 +509,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         int lpi = 1;
         while (lpi * 2 * nbx <= 40 && lpi * 2 <= Nv) lpi *= 2;
         while (lpi > 1 && Nv / lpi < P->n_sm * 3) lpi >>= 1;
-        P->osx_lpi = lpi; P->osx_thr = 160; P->osx_cps = 0; P->osx_occ = 0;
+        P->osx_lpi = lpi; P->osx_thr = 128; P->osx_cps = 0; P->osx_occ = 0;
         P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 2; P->osv_gpc = 0;
     }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
@@ -530,6 +531,16 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->os_twx, sizeof(float2) * otx.size());
     alloc((void**)&P->os_twv, sizeof(float2) * otv.size());
     alloc((void**)&P->os_cs, sizeof(float2) * ocs.size());
+    std::vector<double2> ocs64(OS_LB);
+    for (int j = 0; j < OS_LB; ++j) {
+        const int q4 = (4 * j) / OS_LB;
+        if ((4 * j) % OS_LB == 0) ocs64[j] = make_double2(q4 == 0 ? 1.0 : (q4 == 2 ? -1.0 : 0.0), q4 == 1 ? 1.0 : (q4 == 3 ? -1.0 : 0.0));
+        else {
+            const long double a = 2.0L * 3.14159265358979323846264338327950288L * (long double)j / (long double)OS_LB;
+            ocs64[j] = make_double2((double)cosl(a), (double)sinl(a));
+        }
+    }
+    alloc((void**)&P->os_cs64, sizeof(double2) * ocs64.size());
     alloc((void**)&P->os_lam_x, sizeof(float2) * OS_LAMW * (P->os_x ? Nv : 1));
     alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx : 1));
     alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
@@ -545,6 +556,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     e = cudaMemcpyAsync(P->os_twx, otx.data(), sizeof(float2) * otx.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs, ocs.data(), sizeof(float2) * ocs.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs64, ocs64.data(), sizeof(double2) * ocs64.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwB, xb.data(), sizeof(float2) * xb.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xcs, xc.data(), sizeof(float2) * xc.size(), cudaMemcpyHostToDevice, P->st);
@@ -633,6 +645,7 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
         s.delta = vdir ? dv : P->p.L / (double)Nx;
         s.vmin = P->p.vmin;
         s.E = E; s.Eext = Eext; s.beta = beta;
+        s.cs64 = P->os_cs64;
         s.lam = vdir ? P->os_lam_v : P->os_lam_x;
         return os_setup_launch(s, P->st);
     }
@@ -668,6 +681,7 @@ static cudaError_t run_osx(vog_plan_s* P, const float* src, float* dst)
     a.nb = (Nx + OS_V - 1) / OS_V;
     a.lam = P->os_lam_x; a.tw = P->os_twx; a.cs = P->os_cs;
     a.lpi = P->osx_lpi;
+    a.inv_nb = (65536u + (unsigned)a.nb - 1u) / (unsigned)a.nb;
     a.n_groups = Nv / a.lpi;
     const size_t smem = osx_smem_bytes(a.lpi, a.nb);
     if (P->osx_occ == 0) {

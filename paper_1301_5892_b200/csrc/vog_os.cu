@@ -38,8 +38,8 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
     }
     const double sc = 1.0 / (2.0 * (double)OS_LB);
     if (k == 0) { out[0] = make_float2((float)sc, 0.0f); return; }   // lambda_0 = sum of the weights = 1
-    double c, sn;
-    sincospi((double)k / (double)(OS_LB / 2), &sn, &c);
+    const double2 cs = s.cs64[k];                      // (cos, sin)(2 pi k / OS_LB), fp64 table
+    const double c = cs.x, sn = cs.y;
     double lr, li;
     if (s.spline) {
         const double u = 1.0 - t;
@@ -55,8 +55,10 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
         for (int half = 0; half < 2; ++half) {
             const double tt = half == 0 ? 1.0 - t : t;
             double a = tt, pw = 1.0, acc = 0.0;
-            for (int j = 0; j <= s.d; ++j) {
-                if (j > 0) a = a * ((double)(j * j) - tt * tt) / (double)(2 * j * (2 * j + 1));
+#pragma unroll
+            for (int j = 0; j <= 8; ++j) {
+                if (j > s.d) break;
+                if (j > 0) a = a * ((double)(j * j) - tt * tt) * (1.0 / (double)(2 * j * (2 * j + 1)));
                 acc += a * pw;
                 pw *= sv;
             }
@@ -66,8 +68,8 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
         li = sn * p[1];
     }
     if (br) {
-        double rc, rs;
-        sincospi((double)(k * br) / (double)(OS_LB / 2), &rs, &rc);
+        const double2 r = s.cs64[(k * br) & (OS_LB - 1)];
+        const double rc = r.x, rs = r.y;
         const double xr = lr * rc - li * rs, xi = lr * rs + li * rc;
         lr = xr; li = xi;
     }

@@ -45,33 +45,40 @@ __device__ __forceinline__ int os_swz(int C) { return C ^ (((C >> 3) ^ ((C >> 4)
 // a = lambda_k/(2 LB), cc = conj(lambda_{M-k})/(2 LB).
 __device__ __forceinline__ void os_pair_x(float2& P, float2& Qm, const float2 cs, const float2 a, const float2 cc)
 {
-    const float c = cs.x, s = cs.y;
-    const float2 E2 = make_float2(P.x + Qm.x, P.y - Qm.y);
-    const float2 D2 = make_float2(P.x - Qm.x, P.y + Qm.y);
-    const float2 T2 = make_float2(fmaf(c, D2.y, -s * D2.x), -fmaf(c, D2.x, s * D2.y));
+    const float2 Qc = make_float2(Qm.x, -Qm.y);                     // conj(Z_{M-k})
+    const float2 E2 = cadd(P, Qc), D2 = csub(P, Qc);
+    // T2 = W_N^k (-i D2), W_N^k = (c, -s):  (-i D2) conj((c, s))
+    const float2 T2 = cmulc(make_float2(D2.y, -D2.x), cs);
     const float2 Up = cadd(E2, T2), Um = csub(E2, T2);
-    const float2 Vp = cmul(a, Up), Vm = cmul(cc, Um);
+    const float2 Vp = cmul(Up, a), Vm = cmul(Um, cc);
     const float2 Ep = cadd(Vp, Vm), Dp = csub(Vp, Vm);
-    const float2 Op = make_float2(fmaf(c, Dp.x, -s * Dp.y), fmaf(c, Dp.y, s * Dp.x));
-    P = make_float2(Ep.x - Op.y, Ep.y + Op.x);
-    Qm = make_float2(Ep.x + Op.y, Op.x - Ep.y);
+    const float2 Op = cmul(Dp, cs);                                 // conj(W) Dp
+    P = cadd(Ep, make_float2(-Op.y, Op.x));                         // E' + i O'
+    const float2 R = csub(Ep, make_float2(-Op.y, Op.x));            // E' - i O'
+    Qm = make_float2(R.x, -R.y);
 }
 
 // Two-for-one pair (m, LB-m) of the spectrum of z = uA + i uB: P = Z_m, Q = Z_{LB-m};
 // la, lb = lambda_m/(2 LB) of line A and line B.
 __device__ __forceinline__ void os_pair_v(float2& P, float2& Q, const float2 la, const float2 lb)
 {
-    const float2 ua = make_float2(P.x + Q.x, P.y - Q.y);      // 2 U_A = P + conj Q
-    const float2 ub = make_float2(P.y + Q.y, Q.x - P.x);      // 2 U_B = (P - conj Q)/i
-    const float2 wa = cmul(la, ua), wb = cmul(lb, ub);
-    P = make_float2(wa.x - wb.y, wa.y + wb.x);                // W_A + i W_B
-    Q = make_float2(wa.x + wb.y, wb.x - wa.y);                // conj(W_A) + i conj(W_B)
+    const float2 ua = cadd(P, make_float2(Q.x, -Q.y));              // 2 U_A = P + conj Q
+    const float2 ub = cadd(make_float2(P.y, -P.x), make_float2(Q.y, Q.x));   // 2 U_B = (P - conj Q)/i
+    const float2 wa = cmul(ua, la), wb = cmul(ub, lb);
+    const float2 iwb = make_float2(-wb.y, wb.x);
+    P = cadd(wa, iwb);                                              // W_A + i W_B
+    const float2 R = csub(wa, iwb);                                 // W_A - i W_B
+    Q = make_float2(R.x, -R.y);                                     // conj(W_A) + i conj(W_B)
 }
 
 
 // ---------------------------------------------------------------------------------------------
 // x-direction.  Block of LB = 256 reals = 128 complex = radix 8 (stride 16) x radix 16.
-// Scratch: 64 chunks (1 KB) per block, chunk index = group*8 + (position in group)/2, swizzled.
+// Scratch: 64 chunks (1 KB) per block; logical chunk = group*8 + j (group = radix-8 output index,
+// j = pair of positions inside the group); physical chunk = group*8 + (j ^ key(block, group)).
+// key: groups 0 and 4 (the "special" middle-stage item of a block): block & 7; groups g and 8-g,
+// g = 1..3 (item u = g): (3 block + g - 1) & 7.  With the item orders used below, the 8 lanes of every
+// quarter-warp hit 8 distinct 16-byte bank groups in all three phases.
 namespace osx {
 constexpr int MB = OS_LB / 2;      // complex length of a block
 constexpr int CPB = MB / 2;        // chunks per block (64)
@@ -79,120 +86,130 @@ constexpr int VC = OS_V / 4;       // valid chunks per block (56)
 constexpr int HC = OS_H / 4;       // halo chunks (4)
 }
 
+// slots of one pass-A item: sl[c] = (block base + (tp ^ key_c)), c = 0: groups 0,4; c = 1..3: groups c, 8-c
+struct OsxSlots { int s[4]; };
+__device__ __forceinline__ OsxSlots osx_slots(const int lb, const int tp)
+{
+    OsxSlots r;
+    const int cb = lb * osx::CPB, k3 = 3 * lb;
+    r.s[0] = cb + (tp ^ (lb & 7));
+    r.s[1] = cb + (tp ^ (k3 & 7));
+    r.s[2] = cb + (tp ^ ((k3 + 1) & 7));
+    r.s[3] = cb + (tp ^ ((k3 + 2) & 7));
+    return r;
+}
+__host__ __device__ constexpr int osx_cls(int g) { return (g & 3) == 0 ? 0 : (g < 4 ? g : 8 - g); }
+
+__device__ __forceinline__ void osx_load(float4 (&v)[8], const float4* __restrict__ gline, const int mask,
+                                         const int wc)
+{
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = __ldg(gline + ((wc + 8 * k) & mask));
+}
+
 // forward pass A of one item: two adjacent radix-8 butterflies (positions 2tp, 2tp+1 + 16k)
-__device__ __forceinline__ void osx_fwd(const float4* __restrict__ gline, const int nchunk_mask, const int wc0,
-                                        float4* __restrict__ scr, const int cb, const int tp,
-                                        const float2* __restrict__ twS)
+__device__ __forceinline__ void osx_fwd(const float4 (&v)[8], float4* __restrict__ scr, const OsxSlots sl,
+                                        const int tp, const float2* __restrict__ twS)
 {
     float2 x0[8], x1[8];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
-        const float4 v = __ldg(gline + ((wc0 + tp + 8 * k) & nchunk_mask));
-        x0[k] = make_float2(v.x, v.y);
-        x1[k] = make_float2(v.z, v.w);
-    }
+    for (int k = 0; k < 8; ++k) { x0[k] = make_float2(v[k].x, v[k].y); x1[k] = make_float2(v[k].z, v[k].w); }
     dft_dif<8, 1>(x0);
     dft_dif<8, 1>(x1);
-    const int par = (cb >> 4) & 4;
-    scr[cb + (tp ^ par)] = make_float4(x0[0].x, x0[0].y, x1[0].x, x1[0].y);
+    scr[sl.s[0]] = make_float4(x0[0].x, x0[0].y, x1[0].x, x1[0].y);
     const float4* __restrict__ tw4 = reinterpret_cast<const float4*>(twS) + tp;
 #pragma unroll
     for (int q = 1; q < 8; ++q) {
         const float4 w = tw4[(q - 1) * 8];
         const float2 y0 = cmul(x0[brev(q, 8)], make_float2(w.x, w.y));
         const float2 y1 = cmul(x1[brev(q, 8)], make_float2(w.z, w.w));
-        scr[cb + q * 8 + (tp ^ ((q ^ par) & 7))] = make_float4(y0.x, y0.y, y1.x, y1.y);
+        scr[sl.s[osx_cls(q)] + q * 8] = make_float4(y0.x, y0.y, y1.x, y1.y);
     }
 }
 
 // inverse pass A of one item; stores the valid chunks of the block (+ the block mean dc)
 __device__ __forceinline__ void osx_inv(float4* __restrict__ gline, const int nchunk, const int oc0,
-                                        const float4* __restrict__ scr, const int cb, const int tp,
+                                        const float4* __restrict__ scr, const OsxSlots sl, const int tp,
                                         const float2* __restrict__ twS, const float dc)
 {
     float2 x0[8], x1[8];
-    const int par = (cb >> 4) & 4;
     {
-        const float4 v = scr[cb + (tp ^ par)];
+        const float4 v = scr[sl.s[0]];
         x0[0] = make_float2(v.x, v.y);
         x1[0] = make_float2(v.z, v.w);
     }
     const float4* __restrict__ tw4 = reinterpret_cast<const float4*>(twS) + tp;
 #pragma unroll
     for (int q = 1; q < 8; ++q) {
-        const float4 v = scr[cb + q * 8 + (tp ^ ((q ^ par) & 7))];
+        const float4 v = scr[sl.s[osx_cls(q)] + q * 8];
         const float4 w = tw4[(q - 1) * 8];
         x0[brev(q, 8)] = cmulc(make_float2(v.x, v.y), make_float2(w.x, w.y));
         x1[brev(q, 8)] = cmulc(make_float2(v.z, v.w), make_float2(w.z, w.w));
     }
     idft_dit<8, 1>(x0);
     idft_dit<8, 1>(x1);
+    const float2 d2 = make_float2(dc, dc);
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         const int c = tp + 8 * k;                    // chunk inside the window
         const int oc = oc0 + c - osx::HC;            // chunk of the line
-        if (c >= osx::HC && c < osx::HC + osx::VC && oc < nchunk)
-            __stcs(gline + oc, make_float4(x0[k].x + dc, x0[k].y + dc, x1[k].x + dc, x1[k].y + dc));
+        if (c >= osx::HC && c < osx::HC + osx::VC && oc < nchunk) {
+            const float2 a = cadd(x0[k], d2), b = cadd(x1[k], d2);
+            __stcs(gline + oc, make_float4(a.x, a.y, b.x, b.y));
+        }
     }
 }
-
-// middle stage of one item (two mirror groups of 16 complex): radix 16, untangle, symbol, re-tangle,
-// inverse radix 16.  Same slot layout and "special item" permutation as symbol_item_x (vog_advect_x.cuh).
-__device__ __forceinline__ void osx_mid(float4* __restrict__ scr, const int cb, const int u,
+// middle stage of one item (two mirror groups gA, gB of 16 complex): radix 16, untangle, symbol,
+// re-tangle, inverse radix 16.  XA[brev q] = Z_{kA + 8 q}, XB[brev q] = Z_{kB + 8 q}.
+//   normal item u = 1..3: gA = u, gB = 8 - u; pairs (XA[brev q], XB[brev(15-q)]), k = u + 8 q.
+//   SPECIAL item: gA = 0, gB = 4 (its own mirror): pairs (XB[brev q], XB[brev(15-q)]), k = 4 + 8 q, q < 8;
+//     (XA[brev q], XA[brev(16-q)]), k = 8 q, q = 1..7; k = 64 mirrors itself; k = 0 (with k = 128) apart.
+template <bool SPECIAL>
+__device__ __forceinline__ void osx_mid(float4* __restrict__ scr, const int cb, const int key, const int u,
                                         const float2* __restrict__ lamS, const float2* __restrict__ csS,
                                         float* __restrict__ dc)
 {
     constexpr int M = osx::MB, ML = M / 16;          // 128, 8
-    const bool special = (u == 0);
-    const int gA = u, gB = special ? 4 : 8 - u;
-    const int par = (cb >> 4) & 4;
-    const int pa = cb + gA * 8, pb = cb + gB * 8;
-    const int xa = (gA ^ par) & 7, xb = (gB ^ par) & 7;
+    const int gA = SPECIAL ? 0 : u, gB = SPECIAL ? 4 : 8 - u;
+    float4* const pa = scr + cb + gA * 8;
+    float4* const pb = scr + cb + gB * 8;
     float2 XA[16], XB[16];
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-        const float4 va = scr[pa + (j ^ xa)], vb = scr[pb + (j ^ xb)];
+        const float4 va = pa[j ^ key], vb = pb[j ^ key];
         XA[2 * j] = make_float2(va.x, va.y); XA[2 * j + 1] = make_float2(va.z, va.w);
         XB[2 * j] = make_float2(vb.x, vb.y); XB[2 * j + 1] = make_float2(vb.z, vb.w);
     }
     dft_dif<16, 1>(XA);
     dft_dif<16, 1>(XB);
-    const float2 z0 = XA[0];
-    if (special) {
-        float2 TA[16];
+    if constexpr (!SPECIAL) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) TA[i] = XA[i];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) XA[brev(q, 16)] = XB[brev(q, 16)];
-#pragma unroll
-        for (int q = 8; q < 15; ++q) { XA[brev(q, 16)] = TA[brev(q - 7, 16)]; XB[brev(15 - q, 16)] = TA[brev(23 - q, 16)]; }
-        XA[brev(15, 16)] = TA[brev(8, 16)];
-        XB[brev(0, 16)] = TA[brev(8, 16)];
-    }
-    const int klo = special ? ML / 2 : u;            // slots 0..7:  k = klo + ML q
-    const int khi = special ? -7 * ML : u;           // slots 8..15: k = khi + ML q
-#pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        const int k = (q < 8 ? klo : khi) + ML * q;
-        const float2 a = lamS[k], lm = lamS[M - k];
-        os_pair_x(XA[brev(q, 16)], XB[brev(15 - q, 16)], csS[k], a, make_float2(lm.x, -lm.y));
-    }
-    if (special) {
-        float2 TA[16], TB[8];
-#pragma unroll
-        for (int i = 0; i < 16; ++i) TA[i] = XA[i];
-#pragma unroll
-        for (int j = 1; j < 8; ++j) TB[j] = XB[brev(j, 16)];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) XB[brev(q, 16)] = TA[brev(q, 16)];
-#pragma unroll
-        for (int i = 1; i < 8; ++i) {
-            XA[brev(i, 16)] = TA[brev(i + 7, 16)];
-            XA[brev(16 - i, 16)] = TB[8 - i];
+        for (int q = 0; q < 16; ++q) {
+            const int k = u + ML * q;
+            const float2 lm = lamS[M - k];
+            os_pair_x(XA[brev(q, 16)], XB[brev(15 - q, 16)], csS[k], lamS[k], make_float2(lm.x, -lm.y));
         }
-        XA[brev(8, 16)] = TA[brev(15, 16)];
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int k = ML / 2 + ML * q;
+            const float2 lm = lamS[M - k];
+            os_pair_x(XB[brev(q, 16)], XB[brev(15 - q, 16)], csS[k], lamS[k], make_float2(lm.x, -lm.y));
+        }
+#pragma unroll
+        for (int q = 1; q < 8; ++q) {
+            const int k = ML * q;
+            const float2 lm = lamS[M - k];
+            os_pair_x(XA[brev(q, 16)], XA[brev(16 - q, 16)], csS[k], lamS[k], make_float2(lm.x, -lm.y));
+        }
+        {
+            const float2 lm = lamS[M / 2];
+            float2 dup = XA[brev(8, 16)];
+            os_pair_x(XA[brev(8, 16)], dup, csS[M / 2], lm, make_float2(lm.x, -lm.y));
+        }
         // block modes 0 and LB/2: U_0 = x + y, U_M = x - y; lambda_0 = 1 exactly (lam[0] = (1/(2 LB), 0)).
         // The block mean A0 by-passes the inverse transform and is added back in the last pass.
+        const float2 z0 = XA[0];
         const float A0 = 2.0f * lamS[0].x * (z0.x + z0.y), Bn = 2.0f * lamS[M].x * (z0.x - z0.y);
         XA[0] = make_float2(Bn, -Bn);
         *dc = A0;
@@ -201,8 +218,8 @@ __device__ __forceinline__ void osx_mid(float4* __restrict__ scr, const int cb, 
     idft_dit<16, 1>(XB);
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-        scr[pa + (j ^ xa)] = make_float4(XA[2 * j].x, XA[2 * j].y, XA[2 * j + 1].x, XA[2 * j + 1].y);
-        scr[pb + (j ^ xb)] = make_float4(XB[2 * j].x, XB[2 * j].y, XB[2 * j + 1].x, XB[2 * j + 1].y);
+        pa[j ^ key] = make_float4(XA[2 * j].x, XA[2 * j].y, XA[2 * j + 1].x, XA[2 * j + 1].y);
+        pb[j ^ key] = make_float4(XB[2 * j].x, XB[2 * j].y, XB[2 * j + 1].x, XB[2 * j + 1].y);
     }
 }
 
@@ -211,14 +228,15 @@ __device__ __forceinline__ void osx_mid(float4* __restrict__ scr, const int cb, 
 __global__ void __launch_bounds__(160, 3) osx_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lpi = a.lpi, nb = a.nb;
-    float4* const scr = reinterpret_cast<float4*>(smem_raw);                        // lpi*nb*64 chunks
-    float2* const lamS = reinterpret_cast<float2*>(scr + lpi * nb * osx::CPB);      // lpi*OS_LAMW
+    const int lpi = a.lpi, nb = a.nb, nblk = lpi * nb;
+    float4* const scr = reinterpret_cast<float4*>(smem_raw);                        // nblk*64 chunks
+    float2* const lamS = reinterpret_cast<float2*>(scr + nblk * osx::CPB);          // lpi*OS_LAMW
     float2* const csS = lamS + lpi * OS_LAMW;                                       // 130
     float2* const twS = csS + 130;                                                  // 7*16
-    float* const dcS = reinterpret_cast<float*>(twS + 112);                         // lpi*nb
+    float* const dcS = reinterpret_cast<float*>(twS + 112);                         // nblk
     const int tid = threadIdx.x, T = blockDim.x;
     const int nchunk = a.N >> 2;
+    const unsigned inv_nb = a.inv_nb;      // ceil(2^16 / nb): lb / nb == (lb * inv_nb) >> 16 for lb < 2^12
 
     for (int i = tid; i < 129; i += T) csS[i] = __ldg(a.cs + i);
     for (int i = tid; i < 112; i += T) twS[i] = __ldg(a.tw + i);
@@ -231,37 +249,56 @@ __global__ void __launch_bounds__(160, 3) osx_kernel(const OsArgs a)
             float4* dst4 = reinterpret_cast<float4*>(lamS);
             for (int i = tid; i < lpi * (OS_LAMW / 2); i += T) os_cp_async16(dst4 + i, src4 + i);
         }
-        // ---- pass A: global -> registers -> scratch
+        // ---- pass A: global -> registers -> scratch; the loads of two rounds are in flight together
+        const int nA = nblk * 8;
 #pragma unroll 1
-        for (int w = tid; w < lpi * nb * 8; w += T) {
-            const int lb = w >> 3, tp = w & 7;      // (line, block) flattened, item in block
-            const int l = lb / nb, blk = lb - l * nb;
-            const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
-            const int wc0 = (osx::VC * blk - osx::HC + b4) & (nchunk - 1);
-            const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
-            osx_fwd(gline, nchunk - 1, wc0, scr, lb * osx::CPB, tp, twS);
+        for (int w = tid; w < nA; w += 2 * T) {
+            const int w2 = w + T;
+            const bool has2 = w2 < nA;
+            float4 v0[8], v1[8];
+            const int lb = w >> 3, tp = w & 7;
+            const int lb2 = w2 >> 3, tp2 = w2 & 7;
+            {
+                const int l = (int)(((unsigned)lb * inv_nb) >> 16), blk = lb - l * nb;
+                const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
+                const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
+                osx_load(v0, gline, nchunk - 1, osx::VC * blk - osx::HC + b4 + tp);
+            }
+            if (has2) {
+                const int l = (int)(((unsigned)lb2 * inv_nb) >> 16), blk = lb2 - l * nb;
+                const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
+                const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
+                osx_load(v1, gline, nchunk - 1, osx::VC * blk - osx::HC + b4 + tp2);
+            }
+            osx_fwd(v0, scr, osx_slots(lb, tp), tp, twS);
+            if (has2) osx_fwd(v1, scr, osx_slots(lb2, tp2), tp2, twS);
         }
         os_cp_async_commit_wait();
         __syncthreads();
-        // ---- middle stage
+        // ---- middle stage: items [0, nblk) are the special items of the blocks, then 3 per block
 #pragma unroll 1
-        for (int w = tid; w < lpi * nb * 4; w += T) {
-            const int lb = w >> 2, u = w & 3;
-            const int l = lb / nb;
-            osx_mid(scr, lb * osx::CPB, u, lamS + l * OS_LAMW, csS, dcS + lb);
+        for (int w = tid; w < nblk * 4; w += T) {
+            if (w < nblk) {
+                const int l = (int)(((unsigned)w * inv_nb) >> 16);
+                osx_mid<true>(scr, w * osx::CPB, w & 7, 0, lamS + l * OS_LAMW, csS, dcS + w);
+            } else {
+                const int wp = w - nblk;
+                const int lb = (int)(((unsigned)wp * 43691u) >> 17), u = wp - 3 * lb + 1;   // wp / 3 (wp < 2^15)
+                const int l = (int)(((unsigned)lb * inv_nb) >> 16);
+                osx_mid<false>(scr, lb * osx::CPB, wp & 7, u, lamS + l * OS_LAMW, csS, nullptr);
+            }
         }
         __syncthreads();
         // ---- inverse pass A: scratch -> registers -> global
 #pragma unroll 1
-        for (int w = tid; w < lpi * nb * 8; w += T) {
+        for (int w = tid; w < nA; w += T) {
             const int lb = w >> 3, tp = w & 7;
-            const int l = lb / nb, blk = lb - l * nb;
+            const int l = (int)(((unsigned)lb * inv_nb) >> 16), blk = lb - l * nb;
             float4* gline = reinterpret_cast<float4*>(a.dst) + (size_t)(line0 + l) * nchunk;
-            osx_inv(gline, nchunk, osx::VC * blk, scr, lb * osx::CPB, tp, twS, dcS[lb]);
+            osx_inv(gline, nchunk, osx::VC * blk, scr, osx_slots(lb, tp), tp, twS, dcS[lb]);
         }
     }
 }
-
 
 // ---------------------------------------------------------------------------------------------
 // v-direction.  Strip of NP column pairs; a block is LB = 256 rows of one pair = 256 complex =
