@@ -220,24 +220,80 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
 }
 
 // S9: single-CTA Poisson solve.  rho_i = dv * sum of partials (fp64), zero mean in fp64
-// (P:205-211), radix-2 DIF FFT in shared memory (fp32), E^_m = rho^_m / (i k_m) with modes 0 and
-// Nx/2 dropped, DIT inverse, E written to E_a (and E_b if non-NULL).
-__global__ void __launch_bounds__(1024) poisson_kernel(const double* __restrict__ part, int nby, int Nx, int logNx,
-                                                       double dv, double L, const float2* __restrict__ tw,
+// (P:205-211), mixed-radix (4/8/16, in registers) DIF FFT in shared memory (fp32), E^_m = rho^_m / (i k_m)
+// with modes 0 and Nx/2 dropped, DIT inverse, E written to E_a (and E_b if non-NULL).
+struct PoissonRadix { int np; int r[4]; };
+
+template <int R, bool INV>
+__device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int Nx, const int B,
+                                             const float2* __restrict__ tw, const int tid, const int T)
+{
+    const int S = B / R, mul = Nx / B;
+    for (int g = tid; g < Nx / R; g += T) {
+        const int t = g % S, base = (g / S) * B + t, tm = t * mul;
+        float2 x[R];
+        if constexpr (!INV) {
+#pragma unroll
+            for (int k = 0; k < R; ++k) x[k] = z[base + k * S];
+            dft_dif<R, 1>(x);
+            z[base] = x[0];
+#pragma unroll
+            for (int q = 1; q < R; ++q) z[base + q * S] = cmul(x[brev(q, R)], tw[tm * q]);
+        } else {
+            x[0] = z[base];
+#pragma unroll
+            for (int q = 1; q < R; ++q) x[brev(q, R)] = cmulc(z[base + q * S], tw[tm * q]);
+            idft_dit<R, 1>(x);
+#pragma unroll
+            for (int k = 0; k < R; ++k) z[base + k * S] = x[k];
+        }
+    }
+}
+
+template <bool INV>
+__device__ __forceinline__ void poisson_pass_r(const int R, float2* z, const int Nx, const int B, const float2* tw,
+                                               const int tid, const int T)
+{
+    if (R == 16) poisson_pass<16, INV>(z, Nx, B, tw, tid, T);
+    else if (R == 8) poisson_pass<8, INV>(z, Nx, B, tw, tid, T);
+    else poisson_pass<4, INV>(z, Nx, B, tw, tid, T);
+}
+
+__global__ void __launch_bounds__(1024) poisson_kernel(const double* __restrict__ part, int nby, int Nx,
+                                                       const PoissonRadix rx, double dv, int tw_in_smem,
+                                                       const float2* __restrict__ tw_g, const float* __restrict__ ikt,
                                                        double* __restrict__ rho, float* __restrict__ E_a,
                                                        float* __restrict__ E_b)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* z = reinterpret_cast<float2*>(smem_raw);
+    float* iks = reinterpret_cast<float*>(z + Nx);      // 1/(i k) factors, staged with the first loads
+    float2* tws = reinterpret_cast<float2*>(iks + Nx);
+    double* rs = reinterpret_cast<double*>(z);          // rho in fp64 shares the storage of z (8 B per point)
     __shared__ double wsum[32];
     __shared__ double mean_s;
     const int tid = threadIdx.x, T = blockDim.x;
+    for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);
+    if (tw_in_smem)
+        for (int i = tid; i < Nx; i += T) tws[i] = __ldg(tw_g + i);
+    const float2* __restrict__ tw = tw_in_smem ? tws : tw_g;
     double local = 0.0;
     for (int i = tid; i < Nx; i += T) {
-        double s = 0.0;
-        for (int y = 0; y < nby; ++y) s += part[(size_t)y * Nx + i];
-        s *= dv;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;       // nby is a power of two >= 1
+        if (nby >= 4) {
+#pragma unroll 2
+            for (int y = 0; y < nby; y += 4) {
+                s0 += part[(size_t)y * Nx + i];
+                s1 += part[(size_t)(y + 1) * Nx + i];
+                s2 += part[(size_t)(y + 2) * Nx + i];
+                s3 += part[(size_t)(y + 3) * Nx + i];
+            }
+        } else {
+            for (int y = 0; y < nby; ++y) s0 += part[(size_t)y * Nx + i];
+        }
+        const double s = ((s0 + s1) + (s2 + s3)) * dv;
         rho[i] = s;
+        rs[i] = s;
         local += s;
     }
 #pragma unroll
@@ -246,46 +302,30 @@ __global__ void __launch_bounds__(1024) poisson_kernel(const double* __restrict_
     __syncthreads();
     if (tid == 0) {
         double s = 0.0;
-        for (int w = 0; w < (T >> 5); ++w) s += wsum[w];
+        for (int w = 0; w < ((T + 31) >> 5); ++w) s += wsum[w];
         mean_s = s / (double)Nx;
     }
     __syncthreads();
     const double mean = mean_s;
-    for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rho[i] - mean), 0.0f);
+    for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rs[i] - mean), 0.0f);   // same thread, same slot
     __syncthreads();
-    // forward, decimation in frequency: X[m] lands at position bitrev(m)
-    for (int s = Nx >> 1, sh = logNx - 1; s >= 1; s >>= 1, --sh) {
-        const int mul = Nx / (2 * s);
-        for (int idx = tid; idx < (Nx >> 1); idx += T) {
-            const int t = idx & (s - 1);
-            const int i0 = ((idx >> sh) << (sh + 1)) + t;
-            const float2 a = z[i0], b = z[i0 + s];
-            z[i0] = cadd(a, b);
-            z[i0 + s] = cmul(csub(a, b), __ldg(tw + t * mul));
-        }
+    // forward, decimation in frequency: after passes r0, r1, .. position ((q0 r1 + q1) r2 + q2).. holds
+    // mode q0 + r0 (q1 + r1 (q2 + ..)); ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
+    int B = Nx;
+    for (int p = 0; p < rx.np; ++p) {
+        poisson_pass_r<false>(rx.r[p], z, Nx, B, tw, tid, T);
+        B /= rx.r[p];
         __syncthreads();
     }
-    for (int p = tid; p < Nx; p += T) {
-        const int m = (int)(__brev((unsigned)p) >> (32 - logNx));
-        float2 v = z[p];
-        if (m == 0 || 2 * m == Nx) v = make_float2(0.0f, 0.0f);
-        else {
-            const int ms = (m <= Nx / 2) ? m : m - Nx;
-            const float ik = (float)(L / (2.0 * 3.14159265358979323846 * (double)ms * (double)Nx));
-            v = make_float2(v.y * ik, -v.x * ik);      // (zr + i zi) / (i k)
-        }
-        z[p] = v;
+    for (int pos = tid; pos < Nx; pos += T) {
+        const float2 v = z[pos];
+        const float ik = iks[pos];
+        z[pos] = make_float2(v.y * ik, -v.x * ik);         // (zr + i zi) / (i k), times 1/Nx
     }
     __syncthreads();
-    for (int s = 1, sh = 0; s <= (Nx >> 1); s <<= 1, ++sh) {
-        const int mul = Nx / (2 * s);
-        for (int idx = tid; idx < (Nx >> 1); idx += T) {
-            const int t = idx & (s - 1);
-            const int i0 = ((idx >> sh) << (sh + 1)) + t;
-            const float2 a = z[i0], b = cmulc(z[i0 + s], __ldg(tw + t * mul));
-            z[i0] = cadd(a, b);
-            z[i0 + s] = csub(a, b);
-        }
+    for (int p = rx.np - 1; p >= 0; --p) {
+        B *= rx.r[p];
+        poisson_pass_r<true>(rx.r[p], z, Nx, B, tw, tid, T);
         __syncthreads();
     }
     for (int i = tid; i < Nx; i += T) {
@@ -311,6 +351,8 @@ struct vog_plan_s {
     float2 *os_lam_x, *os_lam_v;   // symbol tables [Nv][OS_LAMW], [Nx][OS_LAMW]
     float2 *os_twx, *os_twv, *os_cs;
     double2* os_cs64;
+    float* ikt;                    // Poisson: 1/(i k) factor per digit-reversed position
+    vog::PoissonRadix prx;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int osx_lpi, osx_thr, osx_cps, osx_occ;
     int osv_np_log, osv_thr, osv_rb, osv_gpc;
@@ -452,7 +494,7 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
-    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64);
+    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64); cudaFree(P->ikt);
     cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
@@ -541,6 +583,29 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         }
     }
     alloc((void**)&P->os_cs64, sizeof(double2) * ocs64.size());
+    std::vector<float> ikt(Nx);
+    {
+        static const int parts[9][4] = {{3, 3, 0, 0}, {4, 3, 0, 0}, {4, 4, 0, 0}, {3, 3, 3, 0}, {4, 3, 3, 0},
+                                        {4, 4, 3, 0}, {4, 4, 4, 0}, {4, 3, 3, 3}, {4, 4, 3, 3}};
+        const int* pp = parts[ilog2i(Nx) - 6];
+        P->prx.np = 0;
+        for (int i = 0; i < 4; ++i) { P->prx.r[i] = pp[i] ? 1 << pp[i] : 1; if (pp[i]) P->prx.np++; }
+        for (int pos = 0; pos < Nx; ++pos) {
+            int rem = pos, m = 0, wgt = Nx;
+            for (int q = P->prx.np - 1; q >= 0; --q) {     // digits from the last pass outwards
+                const int dgt = rem % P->prx.r[q];
+                rem /= P->prx.r[q];
+                wgt /= P->prx.r[q];
+                m += dgt * wgt;
+            }
+            if (m == 0 || 2 * m == Nx) ikt[pos] = 0.0f;
+            else {
+                const int ms = (m <= Nx / 2) ? m : m - Nx;
+                ikt[pos] = (float)(p->L / (2.0 * 3.14159265358979323846 * (double)ms * (double)Nx));
+            }
+        }
+    }
+    alloc((void**)&P->ikt, sizeof(float) * Nx);
     alloc((void**)&P->os_lam_x, sizeof(float2) * OS_LAMW * (P->os_x ? Nv : 1));
     alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx : 1));
     alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
@@ -556,6 +621,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     e = cudaMemcpyAsync(P->os_twx, otx.data(), sizeof(float2) * otx.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs, ocs.data(), sizeof(float2) * ocs.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->ikt, ikt.data(), sizeof(float) * Nx, cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs64, ocs64.data(), sizeof(double2) * ocs64.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwB, xb.data(), sizeof(float2) * xb.size(), cudaMemcpyHostToDevice, P->st);
@@ -824,16 +890,19 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
     density_partial_kernel<<<grid, 256, 0, P->st>>>(f, Nx, Nv, Nv / P->nby, P->part);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const size_t smem = sizeof(float2) * Nx;
     static bool attr = false;
     if (!attr) {
-        e = cudaFuncSetAttribute(poisson_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * (int)sizeof(float2));
+        e = cudaFuncSetAttribute(poisson_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * (int)(sizeof(float2) + sizeof(float)));
         if (e != cudaSuccess) return e;
         attr = true;
     }
-    const int T = Nx >= 2048 ? 1024 : Nx / 2;
+    int T = Nx / 2;
+    if (T > 1024) T = 1024;
+    const int tw_in_smem = Nx <= 8192;
+    const size_t psmem = sizeof(float2) * Nx * (tw_in_smem ? 2 : 1) + sizeof(float) * Nx;
     const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
-    poisson_kernel<<<1, T, smem, P->st>>>(P->part, P->nby, Nx, ilog2i(Nx), dv, P->p.L, P->tw_x, P->rho, P->E_self, E_out);
+    poisson_kernel<<<1, T, psmem, P->st>>>(P->part, P->nby, Nx, P->prx, dv, tw_in_smem, P->tw_x, P->ikt, P->rho,
+                                            P->E_self, E_out);
     P->launches += 2;
     P->E_valid = true;
     return cudaGetLastError();

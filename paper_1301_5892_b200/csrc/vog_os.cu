@@ -11,7 +11,7 @@ namespace vog {
 __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
 {
     const int l = blockIdx.x, k = threadIdx.x;
-    if (l >= s.n_lines || k >= OS_LAMW) return;
+    __shared__ double acoef[2][9];
     double beta;
     float sshift = 0.0f;
     if (s.mode == 0) {
@@ -32,6 +32,15 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
     if (b >= s.N) b = 0;
     const int br = s.vdir ? 0 : (b & 3);
     float2* out = s.lam + (size_t)l * OS_LAMW;
+    if (k < 18) {                                    // a_j(t) = t prod_{m=1..j} (m^2 - t^2) / (2m (2m+1))
+        const int half = k / 9, j = k - 9 * half;
+        const double tt = half == 0 ? 1.0 - t : t;
+        double a = tt;
+        for (int m = 1; m <= j; ++m) a = a * ((double)(m * m) - tt * tt) * (1.0 / (double)(2 * m * (2 * m + 1)));
+        acoef[half][j] = j <= s.d ? a : 0.0;
+    }
+    __syncthreads();
+    if (k >= OS_LAMW) return;
     if (k == 129) {
         out[129] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift);
         return;
@@ -51,21 +60,14 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
         li = ((B1 - Bm1) * sn + B2 * s2) * g;
     } else {
         const double sv = 2.0 - 2.0 * c;
-        double p[2];
-        for (int half = 0; half < 2; ++half) {
-            const double tt = half == 0 ? 1.0 - t : t;
-            double a = tt, pw = 1.0, acc = 0.0;
+        double p0 = 0.0, p1 = 0.0;
 #pragma unroll
-            for (int j = 0; j <= 8; ++j) {
-                if (j > s.d) break;
-                if (j > 0) a = a * ((double)(j * j) - tt * tt) * (1.0 / (double)(2 * j * (2 * j + 1)));
-                acc += a * pw;
-                pw *= sv;
-            }
-            p[half] = acc;
+        for (int j = 8; j >= 0; --j) {               // coefficients beyond the degree are zero
+            p0 = p0 * sv + acoef[0][j];
+            p1 = p1 * sv + acoef[1][j];
         }
-        lr = p[0] + c * p[1];
-        li = sn * p[1];
+        lr = p0 + c * p1;
+        li = sn * p1;
     }
     if (br) {
         const double2 r = s.cs64[(k * br) & (OS_LB - 1)];
