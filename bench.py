@@ -140,15 +140,13 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
-    from paper_1301_5892_b200 import vog
+    from paper_1301_5892_b200 import multi, vog
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local)
     if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        multi.init("nccl", device_id=torch.device("cuda", local))
     vog.lib()
 
     sizes = tuple(int(x) for x in args.sizes.split(","))
@@ -168,7 +166,7 @@ def main():
     def sync_all():
         torch.cuda.synchronize()
         if world > 1:
-            dist.barrier()
+            multi.barrier()
             torch.cuda.synchronize()
 
     def bench_step():
@@ -191,11 +189,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     launches = plan.launch_count() - n0
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * BATCH * cells * args.steps / (ms * 1e-3)
+    ms = multi.max_over_ranks(ms, device="cuda")
+    value = multi.aggregate_throughput(BATCH * cells * args.steps, world, ms)
 
     # ---- per-kernel timing of the same step on the same stream (roofline of the dominant kernel)
     Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
@@ -236,10 +231,7 @@ def main():
         plan.run_host(fh, cfg.dt, 1, None, Eh)      # synchronises before returning
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = multi.max_over_ranks(e2e_s, device="cuda")
     e2e = {"value": world * cells * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 4 * cells,
            "d2h_bytes_per_step": 4 * cells + 4 * cfg.Nx, "steps": e2e_steps,
            "note": "vog_run_host: pinned host f -> device, 1 Strang step, f and E back to host, per step"}
@@ -267,8 +259,7 @@ def main():
     if rank == 0:
         print(json.dumps(out))
     if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
+        multi.finalize()
 
 
 def sweep(torch, vog, stream, peak, sizes=(2048, 8192), kinds=((0, 17), (0, 3), (1, 3))):

@@ -77,6 +77,7 @@ struct OsArgs {
     const float* feq_tab;  // [ng][Nv]
     const float* vmu_tab;  // [ng][Nv]
     float cg[4];
+    const float* cg4;      // the same four constants in device memory (dynamic indexing)
 };
 
 struct OsSetupArgs {

@@ -351,6 +351,7 @@ struct vog_plan_s {
     float2 *os_lam_x, *os_lam_v;   // symbol tables [Nv][OS_LAMW], [Nx][OS_LAMW]
     float2 *os_twx, *os_twv, *os_cs;
     double2* os_cs64;
+    float* cg4;                    // f_eq exponents c_g as floats
     float* ikt;                    // Poisson: 1/(i k) factor per digit-reversed position
     vog::PoissonRadix prx;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
@@ -494,7 +495,7 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
-    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64); cudaFree(P->ikt);
+    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->cg4);
     cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
@@ -606,6 +607,9 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         }
     }
     alloc((void**)&P->ikt, sizeof(float) * Nx);
+    alloc((void**)&P->cg4, sizeof(float) * 4);
+    float cg4h[4];
+    for (int g = 0; g < 4; ++g) cg4h[g] = g < ng ? (float)p->feq.c[g] : 0.0f;
     alloc((void**)&P->os_lam_x, sizeof(float2) * OS_LAMW * (P->os_x ? Nv : 1));
     alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx : 1));
     alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
@@ -621,6 +625,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     e = cudaMemcpyAsync(P->os_twx, otx.data(), sizeof(float2) * otx.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs, ocs.data(), sizeof(float2) * ocs.size(), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->cg4, cg4h, sizeof(cg4h), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->ikt, ikt.data(), sizeof(float) * Nx, cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs64, ocs64.data(), sizeof(double2) * ocs64.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
@@ -684,7 +689,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 12: if (value < 0 || value > 32) return VOG_EINVAL; P->osx_cps = value; break;
         case 13: if (value < 0 || (2 << value) > Nx || osv_smem_bytes(value, P->osv_rb) > 227 * 1024) return VOG_EINVAL; P->osv_np_log = value; break;
         case 14: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->osv_thr = value; break;
-        case 15: if (value < 1 || osv_smem_bytes(P->osv_np_log, value) > 227 * 1024) return VOG_EINVAL; P->osv_rb = value; break;
+        case 15: if (value < 1 || value > 2) return VOG_EINVAL; P->osv_rb = value; break;
         case 16: if (value < 0) return VOG_EINVAL; P->osv_gpc = value; break;
         default: return VOG_EINVAL;
     }
@@ -763,8 +768,8 @@ static cudaError_t run_osx(vog_plan_s* P, const float* src, float* dst)
 
 static size_t osv_smem_bytes(int np_log, int rb)
 {
-    const size_t np = (size_t)1 << np_log;
-    return (size_t)rb * 272 * np * 8 + 2 * np * 131 * 8 + 240 * 8 + 16;
+    (void)np_log;
+    return (size_t)rb * 128 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 130 * 8 + 112 * 8 + (size_t)rb * 32 * 4 + 16;
 }
 
 static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool source)
@@ -774,23 +779,23 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
     a.nb = (Nv + OS_V - 1) / OS_V;
-    a.lam = P->os_lam_v; a.tw = P->os_twv; a.cs = P->os_cs;
-    a.np_log = P->osv_np_log; a.rb = P->osv_rb;
+    a.lam = P->os_lam_v; a.tw = P->os_twx; a.cs = P->os_cs;
+    a.rb = P->osv_rb;
     a.ng = source ? P->p.feq.n : 0;
-    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab;
+    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
     for (int g = 0; g < 4; ++g) a.cg[g] = g < P->p.feq.n ? (float)P->p.feq.c[g] : 0.0f;
-    const int strips = Nx >> (a.np_log + 1);
+    const int strips = Nx / 32;
     const int ngroups = (a.nb + a.rb - 1) / a.rb;
     int gpc = P->osv_gpc;
-    if (gpc <= 0) {                       // enough CTAs to fill the chip 8 deep, else one group per CTA
-        gpc = (int)(((long long)strips * ngroups) / ((long long)P->n_sm * 8));
+    if (gpc <= 0) {                       // about 6 CTAs per SM in total, else one group per CTA
+        gpc = (int)(((long long)strips * ngroups) / ((long long)P->n_sm * 6));
         if (gpc < 1) gpc = 1;
     }
     if (gpc > ngroups) gpc = ngroups;
     a.gpc = gpc;
     dim3 grid(strips, (ngroups + gpc - 1) / gpc);
     P->launches++;
-    return osv_launch(a, grid, P->osv_thr, osv_smem_bytes(a.np_log, a.rb), P->st);
+    return osv_launch(a, grid, 128 * a.rb, osv_smem_bytes(0, a.rb), P->st);
 }
 
 static cudaError_t run_advect_x(vog_plan_s* P, float* f)

@@ -31,7 +31,9 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
     int b = (int)bm;
     if (b >= s.N) b = 0;
     const int br = s.vdir ? 0 : (b & 3);
-    float2* out = s.lam + (size_t)l * OS_LAMW;
+    // x: [line][k]; v: transposed [k][line] so that a strip of 32 columns reads 256-byte rows
+    float2* out = s.vdir ? s.lam + l : s.lam + (size_t)l * OS_LAMW;
+    const size_t ks = s.vdir ? (size_t)s.n_lines : 1;
     if (k < 18) {                                    // a_j(t) = t prod_{m=1..j} (m^2 - t^2) / (2m (2m+1))
         const int half = k / 9, j = k - 9 * half;
         const double tt = half == 0 ? 1.0 - t : t;
@@ -42,7 +44,7 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
     __syncthreads();
     if (k >= OS_LAMW) return;
     if (k == 129) {
-        out[129] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift);
+        out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift);
         return;
     }
     const double sc = 1.0 / (2.0 * (double)OS_LB);
@@ -75,7 +77,7 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
         const double xr = lr * rc - li * rs, xi = lr * rs + li * rc;
         lr = xr; li = xi;
     }
-    out[k] = make_float2((float)(lr * sc), (float)(li * sc));
+    out[k * ks] = make_float2((float)(lr * sc), (float)(li * sc));
 }
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)

@@ -225,7 +225,7 @@ __device__ __forceinline__ void osx_mid(float4* __restrict__ scr, const int cb, 
 
 // Persistent kernel: one iteration = lpi whole lines (a CTA owns whole lines, so src may equal dst: all
 // loads of a line happen before the barrier that precedes its first store).
-__global__ void __launch_bounds__(160, 3) osx_kernel(const OsArgs a)
+__global__ void __launch_bounds__(128, 4) osx_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lpi = a.lpi, nb = a.nb, nblk = lpi * nb;
@@ -301,160 +301,201 @@ __global__ void __launch_bounds__(160, 3) osx_kernel(const OsArgs a)
 }
 
 // ---------------------------------------------------------------------------------------------
-// v-direction.  Strip of NP column pairs; a block is LB = 256 rows of one pair = 256 complex =
-// radix 16 (stride 16) x radix 16.  Scratch per block: [padded position][pair] float2, one position of
-// padding per 16 (conflict-free 64-bit accesses in both passes).  Lanes run over the pairs first, so a
-// row segment of 8 NP bytes is contiguous in global memory.
+// v-direction.  A strip is 32 adjacent columns = the 32 lanes of a warp; every lane advects ITS column with
+// even/odd packing along v (z_n = f[2n][c] + i f[2n+1][c], the same 128-complex block transform as in x).
+//   * a row of the strip is one 128-byte line: every global load and store is fully coalesced, and a
+//     lane applies its own integer shift b_c by addressing (rows r + b_c);
+//   * scratch is [position][lane] float2: all shared accesses are conflict-free without padding;
+//   * an item type (radix-8 butterfly t, middle-stage item u) is uniform across a warp: no divergence
+//     between the "special" and the normal middle-stage items;
+//   * the symbol tables arrive transposed ([k][column], written that way by the setup kernel).
+// Out of place (src != dst): a block reads rows that other blocks write.
 namespace osv {
-constexpr int PADLEN = OS_LB + OS_LB / 16;     // 272 padded positions
-constexpr int LS = 131;                        // shared-memory stride (float2) of one column's symbol table
+constexpr int MB = OS_LB / 2;          // complex per block and column (128)
+constexpr int W = 32;                  // columns per strip
+constexpr int HN = OS_H / 2;           // halo in complex samples (8)
+constexpr int VN = OS_V / 2;           // valid complex samples per block (112)
 }
 
-__global__ void __launch_bounds__(128, 4) osv_kernel(const OsArgs a)
+template <bool SPECIAL>
+__device__ __forceinline__ void osv_mid(float2* __restrict__ scr, const int u, const float2* __restrict__ lamS,
+                                        const float2* __restrict__ csS, float* __restrict__ dc)
+{
+    constexpr int M = osv::MB, ML = M / 16, W = osv::W;     // 128, 8
+    const int gA = SPECIAL ? 0 : u, gB = SPECIAL ? 4 : 8 - u;
+    float2* const pa = scr + gA * 16 * W;
+    float2* const pb = scr + gB * 16 * W;
+    float2 XA[16], XB[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) { XA[j] = pa[j * W]; XB[j] = pb[j * W]; }
+    dft_dif<16, 1>(XA);
+    dft_dif<16, 1>(XB);
+    if constexpr (!SPECIAL) {
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int k = u + ML * q;
+            const float2 lm = lamS[(M - k) * W];
+            os_pair_x(XA[brev(q, 16)], XB[brev(15 - q, 16)], csS[k], lamS[k * W], make_float2(lm.x, -lm.y));
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            constexpr int k0 = ML / 2;
+            const int k = k0 + ML * q;
+            const float2 lm = lamS[(M - k) * W];
+            os_pair_x(XB[brev(q, 16)], XB[brev(15 - q, 16)], csS[k], lamS[k * W], make_float2(lm.x, -lm.y));
+        }
+#pragma unroll
+        for (int q = 1; q < 8; ++q) {
+            const int k = ML * q;
+            const float2 lm = lamS[(M - k) * W];
+            os_pair_x(XA[brev(q, 16)], XA[brev(16 - q, 16)], csS[k], lamS[k * W], make_float2(lm.x, -lm.y));
+        }
+        {
+            const float2 lm = lamS[(M / 2) * W];
+            float2 dup = XA[brev(8, 16)];
+            os_pair_x(XA[brev(8, 16)], dup, csS[M / 2], lm, make_float2(lm.x, -lm.y));
+        }
+        const float2 z0 = XA[0];
+        const float A0 = 2.0f * lamS[0].x * (z0.x + z0.y), Bn = 2.0f * lamS[M * W].x * (z0.x - z0.y);
+        XA[0] = make_float2(Bn, -Bn);
+        *dc = A0;                                   // block mean of this column, added back in the last pass
+    }
+    idft_dit<16, 1>(XA);
+    idft_dit<16, 1>(XB);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) { pa[j * W] = XA[j]; pb[j * W] = XB[j]; }
+}
+
+__device__ __forceinline__ void osv_load(float2 (&x)[8], const float* __restrict__ col, const int Nx, const int vmask,
+                                         const int r0)
+{
+    const int rr = r0 & vmask;
+    if (rr + OS_LB <= vmask) {                      // the window does not wrap: constant row stride
+        const float* p = col + rr * Nx;
+        const int s32 = 32 * Nx;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            x[k] = make_float2(__ldg(p), __ldg(p + Nx));
+            p += s32;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int ra = (r0 + 32 * k) & vmask, rb = (r0 + 32 * k + 1) & vmask;
+            x[k] = make_float2(__ldg(col + ra * Nx), __ldg(col + rb * Nx));
+        }
+    }
+}
+
+__device__ __forceinline__ void osv_fwd(float2 (&x)[8], float2* __restrict__ o, const float2* __restrict__ tw)
+{
+    constexpr int W = osv::W;
+    dft_dif<8, 1>(x);
+    o[0] = x[0];
+#pragma unroll
+    for (int q = 1; q < 8; ++q) o[q * 16 * W] = cmul(x[brev(q, 8)], tw[(q - 1) * 16]);
+}
+
+// T = 128 rb threads: warp w handles butterflies t = w, w + nw, .. of the rb blocks of a group
+__global__ void __launch_bounds__(256, 2) osv_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int npl = a.np_log, np = 1 << npl, rb = a.rb, nb = a.nb;
-    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // rb * PADLEN * np
-    float2* const lamS = scr + rb * osv::PADLEN * np;                         // 2 np * LS
-    float2* const twS = lamS + 2 * np * osv::LS;                              // 15 * 16
-    const int tid = threadIdx.x, T = blockDim.x;
-    const int Nx = a.Nx, Nv = a.Nv;
-    const int c0 = blockIdx.x * 2 * np;
+    constexpr int W = osv::W, MB = osv::MB;
+    const int rb = a.rb, nb = a.nb;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // rb * 128 * 32
+    float2* const lamS = scr + rb * MB * W;                                   // 130 * 32, [k][lane]
+    float2* const csS = lamS + OS_LAMW * W;                                   // 130
+    float2* const twS = csS + 130;                                            // 7 * 16
+    float* const dcS = reinterpret_cast<float*>(twS + 112);                   // rb * 32
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5, nw = T >> 5;
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
+    const int c0 = blockIdx.x * W;
 
-    for (int i = tid; i < 2 * np * OS_LAMW; i += T) {
-        const int col = i / OS_LAMW, k = i - col * OS_LAMW;
-        lamS[col * osv::LS + k] = __ldg(a.lam + (size_t)(c0 + col) * OS_LAMW + k);
+    {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
+        const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
+        float4* dst4 = reinterpret_cast<float4*>(lamS);
+        for (int i = tid; i < OS_LAMW * 16; i += T)
+            os_cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
     }
-    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
+    for (int i = tid; i < 129; i += T) csS[i] = __ldg(a.cs + i);
+    for (int i = tid; i < 112; i += T) twS[i] = __ldg(a.tw + i);
+    os_cp_async_commit_wait();
     __syncthreads();
+    const int b = __float_as_int(lamS[129 * W + lane].x);
+    const float ssh = lamS[129 * W + lane].y;
+    const float* const col = a.src + c0 + lane;
+    float* const ocol = a.dst + c0 + lane;
 
     const int ngroups = (nb + rb - 1) / rb;
     const int g1 = min(ngroups, ((int)blockIdx.y + 1) * a.gpc);
     for (int gi = blockIdx.y * a.gpc; gi < g1; ++gi) {
-        // ---- pass A: global -> registers -> scratch (radix 16 over rows t + 16 k)
+        // ---- pass A: global -> registers -> scratch (two butterflies' loads in flight)
 #pragma unroll 1
-        for (int w = tid; w < rb * 16 * np; w += T) {
-            const int p = w & (np - 1), t = (w >> npl) & 15, bl = w >> (npl + 4);
-            const int blk = gi * rb + bl;
-            if (blk >= nb) continue;
-            const int bA = __float_as_int(lamS[(2 * p) * osv::LS + 129].x);
-            const int bB = __float_as_int(lamS[(2 * p + 1) * osv::LS + 129].x);
-            const int r0 = blk * OS_V - OS_H + t;
-            const float* colA = a.src + c0 + 2 * p;
-            float2 x[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                const int rA = (r0 + 16 * k + bA) & (Nv - 1), rB = (r0 + 16 * k + bB) & (Nv - 1);
-                x[k] = make_float2(__ldg(colA + (size_t)rA * Nx), __ldg(colA + (size_t)rB * Nx + 1));
-            }
-            dft_dif<16, 1>(x);
-            float2* o = scr + (bl * osv::PADLEN + t) * np + p;
-            o[0] = x[0];
-#pragma unroll
-            for (int q = 1; q < 16; ++q) o[q * 17 * np] = cmul(x[brev(q, 16)], twS[(q - 1) * 16 + t]);
+        for (int w = wid; w < rb * 16; w += 2 * nw) {
+            const int w2 = w + nw;
+            const int bl = w >> 4, t = w & 15, bl2 = w2 >> 4, t2 = w2 & 15;
+            const int blk = gi * rb + bl, blk2 = gi * rb + bl2;
+            const bool ok = blk < nb, ok2 = (w2 < rb * 16) && (blk2 < nb);
+            float2 x0[8], x1[8];
+            if (ok) osv_load(x0, col, Nx, vmask, blk * OS_V - OS_H + b + 2 * t);
+            if (ok2) osv_load(x1, col, Nx, vmask, blk2 * OS_V - OS_H + b + 2 * t2);
+            if (ok) osv_fwd(x0, scr + (bl * MB + t) * W + lane, twS + t);
+            if (ok2) osv_fwd(x1, scr + (bl2 * MB + t2) * W + lane, twS + t2);
         }
         __syncthreads();
-        // ---- middle stage: radix 16, two-for-one separation, symbols, recombination, inverse radix 16
+        // ---- middle stage: item u of block bl, all 32 columns of the warp alike
 #pragma unroll 1
-        for (int w = tid; w < rb * 8 * np; w += T) {
-            const int p = w & (np - 1), u = (w >> npl) & 7, bl = w >> (npl + 3);
+        for (int w = wid; w < rb * 4; w += nw) {
+            const int bl = w >> 2, u = w & 3;
             if (gi * rb + bl >= nb) continue;
-            const bool special = (u == 0);
-            const int gA = u, gB = special ? 8 : 16 - u;
-            float2* const sa = scr + (bl * osv::PADLEN + gA * 17) * np + p;
-            float2* const sb = scr + (bl * osv::PADLEN + gB * 17) * np + p;
-            float2 XA[16], XB[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) { XA[j] = sa[j * np]; XB[j] = sb[j * np]; }
-            dft_dif<16, 1>(XA);
-            dft_dif<16, 1>(XB);
-            const float2 z0 = XA[0];
-            if (special) {
-                float2 TA[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) TA[i] = XA[i];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) XA[brev(q, 16)] = XB[brev(q, 16)];
-#pragma unroll
-                for (int q = 8; q < 15; ++q) { XA[brev(q, 16)] = TA[brev(q - 7, 16)]; XB[brev(15 - q, 16)] = TA[brev(23 - q, 16)]; }
-                XA[brev(15, 16)] = TA[brev(8, 16)];
-                XB[brev(0, 16)] = TA[brev(8, 16)];
-            }
-            // slot q: P = Z_m in XA[brev q], Q = Z_{LB-m} in XB[brev(15-q)];
-            //   q < 8 : m = mlo + 16 q              (<= 127)
-            //   q >= 8: special: m = 16 (q - 7);  else m = u + 16 q > 128: lambda_m = conj(lambda_{LB-m})
-            const int mlo = special ? 8 : u;
-            const int mh0 = special ? -112 : OS_LB - u, mh1 = special ? 16 : -16;
-            const float sgh = special ? 1.0f : -1.0f;
-            const float2* const lA = lamS + (2 * p) * osv::LS;
-            const float2* const lB = lA + osv::LS;
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const int m = q < 8 ? mlo + 16 * q : mh0 + mh1 * q;
-                float2 la = lA[m], lb = lB[m];
-                if (q >= 8) { la.y *= sgh; lb.y *= sgh; }
-                os_pair_v(XA[brev(q, 16)], XB[brev(15 - q, 16)], la, lb);
-            }
-            if (special) {
-                float2 TA[16], TB[8];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) TA[i] = XA[i];
-#pragma unroll
-                for (int j = 1; j < 8; ++j) TB[j] = XB[brev(j, 16)];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) XB[brev(q, 16)] = TA[brev(q, 16)];
-#pragma unroll
-                for (int i = 1; i < 8; ++i) {
-                    XA[brev(i, 16)] = TA[brev(i + 7, 16)];
-                    XA[brev(16 - i, 16)] = TB[8 - i];
-                }
-                XA[brev(8, 16)] = TA[brev(15, 16)];
-                // mode 0 of both lines: lambda_0 = 1 exactly, Y_0 = Z_0 / LB
-                const float s0 = 2.0f * lA[0].x;
-                XA[0] = make_float2(z0.x * s0, z0.y * s0);
-            }
-            idft_dit<16, 1>(XA);
-            idft_dit<16, 1>(XB);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) { sa[j * np] = XA[j]; sb[j * np] = XB[j]; }
+            float2* const sb = scr + bl * MB * W + lane;
+            if (u == 0) osv_mid<true>(sb, 0, lamS + lane, csS, dcS + bl * W + lane);
+            else osv_mid<false>(sb, u, lamS + lane, csS, nullptr);
         }
         __syncthreads();
-        // ---- inverse pass A: scratch -> registers -> global (+ delta-f source); rows k = 1..14 are valid
+        // ---- inverse pass A: scratch -> registers -> global (+ delta-f source)
 #pragma unroll 1
-        for (int w = tid; w < rb * 16 * np; w += T) {
-            const int p = w & (np - 1), t = (w >> npl) & 15, bl = w >> (npl + 4);
+        for (int w = wid; w < rb * 16; w += nw) {
+            const int bl = w >> 4, t = w & 15;
             const int blk = gi * rb + bl;
             if (blk >= nb) continue;
-            const float2* o = scr + (bl * osv::PADLEN + t) * np + p;
-            float2 x[16];
+            const float2* o = scr + (bl * MB + t) * W + lane;
+            float2 x[8];
             x[0] = o[0];
 #pragma unroll
-            for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(o[q * 17 * np], twS[(q - 1) * 16 + t]);
-            idft_dit<16, 1>(x);
-            const int row0 = blk * OS_V + t - OS_H;           // + 16 k
-            if (a.ng > 0) {
-                const float sA = lamS[(2 * p) * osv::LS + 129].y, sB = lamS[(2 * p + 1) * osv::LS + 129].y;
-                for (int g = 0; g < a.ng; ++g) {
-                    const float cg = a.cg[g];
-                    const float* __restrict__ ft = a.feq_tab + (size_t)g * Nv;
-                    const float* __restrict__ vt = a.vmu_tab + (size_t)g * Nv;
+            for (int q = 1; q < 8; ++q) x[brev(q, 8)] = cmulc(o[q * 16 * W], twS[(q - 1) * 16 + t]);
+            idft_dit<8, 1>(x);
+            const float dc = dcS[bl * W + lane];
+            const int row0 = blk * OS_V - OS_H + 2 * t;           // + 32 k, two rows per complex sample
+            const float2 d2 = make_float2(dc, dc);
 #pragma unroll
-                    for (int k = 1; k < 15; ++k) {
-                        const int j = row0 + 16 * k;
-                        if (j < Nv) {
-                            const float fe = __ldg(ft + j), vm2 = 2.0f * __ldg(vt + j);
-                            // f_eq,g(v - s) - f_eq,g(v) = f_eq,g(v) expm1(c s (2 (v - mu) - s))
-                            x[k].x = fmaf(fe, expm1f(cg * sA * (vm2 - sA)), x[k].x);
-                            x[k].y = fmaf(fe, expm1f(cg * sB * (vm2 - sB)), x[k].y);
-                        }
+            for (int k = 0; k < 8; ++k) x[k] = cadd(x[k], d2);
+            if (a.ng > 0) {                                       // delta-f source
+#pragma unroll 1
+                for (int g = 0; g < a.ng; ++g) {
+                    const float cgs = a.cg4[g] * ssh;
+                    const float* __restrict__ ft = a.feq_tab + g * Nv;
+                    const float* __restrict__ vt = a.vmu_tab + g * Nv;
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const int j = min(max(row0 + 32 * k, 0), Nv - 2);     // rows outside are never stored
+                        // f_eq,g(v - s) - f_eq,g(v) = f_eq,g(v) expm1(c s (2 (v - mu) - s))
+                        x[k].x = fmaf(__ldg(ft + j), expm1f(cgs * (2.0f * __ldg(vt + j) - ssh)), x[k].x);
+                        x[k].y = fmaf(__ldg(ft + j + 1), expm1f(cgs * (2.0f * __ldg(vt + j + 1) - ssh)), x[k].y);
                     }
                 }
             }
-            float* colA = a.dst + c0 + 2 * p;
+            float* po = ocol + row0 * Nx;
+            const int s32 = 32 * Nx;
 #pragma unroll
-            for (int k = 1; k < 15; ++k) {
-                const int j = row0 + 16 * k;
-                if (j < Nv) __stcs(reinterpret_cast<float2*>(colA + (size_t)j * Nx), x[k]);
+            for (int k = 0; k < 8; ++k) {
+                const int n = t + 16 * k;
+                if (n >= osv::HN && n < osv::HN + osv::VN && row0 + 32 * k < Nv) {
+                    __stcs(po, x[k].x);
+                    __stcs(po + Nx, x[k].y);
+                }
+                po += s32;
             }
         }
         __syncthreads();
