@@ -104,11 +104,15 @@ int vog_shift_v(vog_plan_t plan, float* f_dev, const double* beta_cells_dev);
 int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
                  const float* E_ext_host, float* E_host);
 
-/* Tile-shape override for measurements; not needed for normal use.
- * which: 2 = log2(complex lines per CTA) of the v-kernel, 3 = threads per CTA of the v-kernel,
- * 5 = log2(lines per iteration) of the persistent x-kernel, 6 = its threads per CTA (32..128),
- * 7 = its CTAs per SM (0 = as many as fit).  (0, 1 are accepted and ignored: the round-0 x-kernel.)
- * VOG_EINVAL if the shape does not fit (shared memory, grid). */
+/* Launch-shape override for measurements; never needed for normal use and never
+ * changes results beyond rounding.  which:
+ *   2, 3   whole-line v kernel (Nv <= 512): log2(complex lines per CTA), threads per CTA;
+ *   5..8   whole-line x kernel (Nx <= 512): log2(lines per iteration), threads (32..128), CTAs per SM
+ *          (0 = as many as fit), line buffers (1 or 2);
+ *   10..12 overlap-save x kernel (Nx >= 1024): lines per iteration, threads (32..160), CTAs per SM;
+ *   15, 16 overlap-save v kernel (Nv >= 1024): row blocks per group (1 or 2; threads = 128 x that),
+ *          groups per CTA (0 = automatic).
+ * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 
 /* Number of kernels the library launched on this plan since creation (for accounting). */

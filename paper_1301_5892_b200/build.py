@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libvog.so")
-SIZES = (64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384)
+SIZES = (64, 128, 256, 512)   # whole-line kernels; longer lines use the overlap-save kernels (vog_os.cu)
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "--use_fast_math=false"]

@@ -105,8 +105,8 @@ size_t advect_smem_bytes(int N, int lognl);
 #define VOG_DECL_LAUNCH(NN) cudaError_t advect_launch_##NN(const AdvectArgs&, int, bool, int, int, size_t, cudaStream_t); \
     cudaError_t advect_x_launch_##NN(const AdvectXArgs&, int, int, int, size_t, cudaStream_t); \
     int advect_x_occ_##NN(int, int, size_t);
-VOG_DECL_LAUNCH(64) VOG_DECL_LAUNCH(128) VOG_DECL_LAUNCH(256) VOG_DECL_LAUNCH(512) VOG_DECL_LAUNCH(1024)
-VOG_DECL_LAUNCH(2048) VOG_DECL_LAUNCH(4096) VOG_DECL_LAUNCH(8192) VOG_DECL_LAUNCH(16384)
+// whole-line kernels serve line lengths <= 512; longer lines use the overlap-save kernels
+VOG_DECL_LAUNCH(64) VOG_DECL_LAUNCH(128) VOG_DECL_LAUNCH(256) VOG_DECL_LAUNCH(512)
 #undef VOG_DECL_LAUNCH
 
 }  // namespace vog

@@ -21,11 +21,6 @@ advect_launch_fn advect_launcher(int N)
         case 128: return advect_launch_128;
         case 256: return advect_launch_256;
         case 512: return advect_launch_512;
-        case 1024: return advect_launch_1024;
-        case 2048: return advect_launch_2048;
-        case 4096: return advect_launch_4096;
-        case 8192: return advect_launch_8192;
-        case 16384: return advect_launch_16384;
     }
     return nullptr;
 }
@@ -37,11 +32,6 @@ advect_x_launch_fn advect_x_launcher(int N)
         case 128: return advect_x_launch_128;
         case 256: return advect_x_launch_256;
         case 512: return advect_x_launch_512;
-        case 1024: return advect_x_launch_1024;
-        case 2048: return advect_x_launch_2048;
-        case 4096: return advect_x_launch_4096;
-        case 8192: return advect_x_launch_8192;
-        case 16384: return advect_x_launch_16384;
     }
     return nullptr;
 }
@@ -53,11 +43,6 @@ int advect_x_occupancy(int N, int sym, int threads, size_t smem)
         case 128: return advect_x_occ_128(sym, threads, smem);
         case 256: return advect_x_occ_256(sym, threads, smem);
         case 512: return advect_x_occ_512(sym, threads, smem);
-        case 1024: return advect_x_occ_1024(sym, threads, smem);
-        case 2048: return advect_x_occ_2048(sym, threads, smem);
-        case 4096: return advect_x_occ_4096(sym, threads, smem);
-        case 8192: return advect_x_occ_8192(sym, threads, smem);
-        case 16384: return advect_x_occ_16384(sym, threads, smem);
     }
     return 0;
 }

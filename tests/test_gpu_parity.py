@@ -158,6 +158,59 @@ def test_one_step_parity(torch, vog, oracle, idx, split):
     plan.destroy()
 
 
+@pytest.mark.parametrize("split", [0, 1])
+@pytest.mark.parametrize("Nx,Nv", [(1024, 128), (128, 1024), (1024, 1024)])
+def test_one_step_parity_mixed_kernel_dispatch(torch, vog, oracle, Nx, Nv, split):
+    """Lines >= 1024 use the overlap-save kernels (v out of place through the plan's second grid), shorter
+    lines the whole-line kernels: a step must chain them correctly in both split orders."""
+    cfg = inputs.config(1, Nx=Nx, Nv=Nv, split=split)
+    f = inputs.initial_f(cfg)
+    plan = vog.Plan.from_config(cfg)
+    feq = oracle.Feq.make(cfg.feq)
+    ext = (0.02 * np.sin(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx)).astype(np.float32)
+    fd = _dev(torch, f)
+    for _ in range(2):
+        plan.step(fd, cfg.dt, _dev(torch, ext))
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    plan.get_field(Ed)
+    fo = f.astype(np.float64)
+    Eo = None
+    for _ in range(2):
+        fo, Eo = oracle.step(fo, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, split, ext, Eo)
+    _check(fd.cpu().numpy(), fo, np.abs(f).max(), tol=3 * TOL * 2)
+    assert np.abs(Ed.cpu().numpy() - Eo).max() <= 1e-4 * np.abs(Eo).max()
+    plan.destroy()
+
+
+def test_tile_shape_overrides_keep_parity(torch, vog, oracle):
+    """vog_plan_tune changes launch shapes only: results must not move beyond rounding."""
+    N = 2048
+    f = inputs.uniform_grid(N, 64)
+    bx = _shifts(64, 51)
+    ref = oracle.shift_x(f, bx, LAG, 17)
+    for which, value in ((10, 1), (10, 2), (11, 96), (12, 2)):
+        plan = vog.Plan(N, 64, 1.0, -1.0, 1.0, LAG, 17)
+        plan.tune(which, value)
+        fd = _dev(torch, f)
+        plan.shift_x(fd, _dev(torch, bx))
+        _check(fd.cpu().numpy(), ref, 1.0)
+        plan.destroy()
+    f = inputs.uniform_grid(64, N)
+    bv = _shifts(64, 52)
+    ref = oracle.shift_v(f, bv, LAG, 17)
+    for which, value in ((15, 1), (15, 2), (16, 1), (16, 3)):
+        plan = vog.Plan(64, N, 1.0, -1.0, 1.0, LAG, 17)
+        plan.tune(which, value)
+        fd = _dev(torch, f)
+        plan.shift_v(fd, _dev(torch, bv))
+        _check(fd.cpu().numpy(), ref, 1.0)
+        plan.destroy()
+    plan = vog.Plan(64, 64, 1.0, -1.0, 1.0)
+    with pytest.raises(vog.VogError):
+        plan.tune(99, 0)
+    plan.destroy()
+
+
 # ------------------------------------------------------------------ full runs: energy history, configs 0-1
 def _gpu_history(torch, vog, cfg, steps):
     plan = vog.Plan.from_config(cfg)
