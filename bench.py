@@ -31,6 +31,15 @@ UNIT = "cell-updates/s"
 BATCH = 16
 
 
+def _traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), else None."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    try:
+        return float(json.load(open(path))["osx_kernel_bench_dram_bytes_per_launch"])
+    except Exception:
+        return None
+
+
 def _peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -127,8 +136,8 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 advection sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--sweep-only", action="store_true", help="only the config-4 advection sweep (for profiling)")
-    ap.add_argument("--sizes", default="2048,8192", help="sweep grid sizes N (Nx=Nv=N)")
-    ap.add_argument("--kinds", default="lag17,lag3,spline", help="sweep interpolators: lagN or spline")
+    ap.add_argument("--sizes", default="512,2048,8192,16384", help="sweep grid sizes N (Nx=Nv=N), BASELINE.json config 4")
+    ap.add_argument("--kinds", default="lag3,lag9,lag17,spline", help="sweep interpolators: lagN or spline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -214,10 +223,13 @@ def main():
     alg_bytes = 8.0 * cells                      # one read + one write of f per advection
     ach = alg_bytes / (ms_x * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "osx_kernel (overlap-save x-advection, 2048-cell lines)", "achieved": ach, "peak": peak,
-                "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                "unit": "GB/s", "frac": ach / peak, "traffic": _traffic(), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_x,
                 "other_kernels_ms": {"advect_v(+delta-f source)": ms_v, "density+poisson": ms_f},
-                "note": "2048^2 replica is L2-cold on entry (batch 256 MiB > L2) but 16 MiB fits L2 within a step"}
+                "note": "2048^2 replica is L2-cold on entry (batch 256 MiB > L2) but 16 MiB fits L2 within a step; "
+                        "advect_v here is the standalone in-place call (table setup + kernel + copy back from the "
+                        "plan's second grid); inside vog_step the v kernel writes the second grid and the next "
+                        "x-advection reads it, so no copy is made; HBM-roofline fractions at 8192^2/16384^2 are in sweep"}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     fh = f0.clone().pin_memory()
@@ -283,6 +295,7 @@ def sweep(torch, vog, stream, peak, sizes=(2048, 8192), kinds=((0, 17), (0, 3), 
                 gbs = 8.0 * N * N / (med * 1e-3) / 1e9
                 row[name] = {"ms_median": med, "ms_best": min(times), "GBps": gbs, "frac_hbm_measured": gbs / peak,
                              "frac_hbm_8TBps": gbs / 8000.0}
+            row["note"] = "vog_shift_x/v calls: fp64 table setup + kernel (+ copy back for v, whose kernel is out of place)"
             res.append(row)
             plan.destroy()
         del f

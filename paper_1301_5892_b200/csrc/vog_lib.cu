@@ -172,7 +172,8 @@ __global__ void shift_setup_x_kernel(const SetupArgs s)
 // (8 lanes x float4 = one 128 B line per row); the 4 row-lanes are folded by warp shuffles,
 // the 8 warps through shared memory; fp64 accumulation, fixed order => deterministic.
 __global__ void __launch_bounds__(256) density_partial_kernel(const float* __restrict__ f, int Nx, int Nv,
-                                                              int rows_per_block, double* __restrict__ part)
+                                                              int rows_per_block, double* __restrict__ part,
+                                                              double dv, double* __restrict__ rho, unsigned* __restrict__ cnt)
 {
     __shared__ double red[8][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -202,104 +203,120 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
         for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
         part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
     }
+    // The last of the gridDim.y blocks of this column group to finish adds the partial rows in a FIXED
+    // order (y = 0, 1, ..): deterministic, and the reduction is spread over the SMs instead of being
+    // pulled through the single SM that solves the Poisson equation.
+    __shared__ unsigned ticket;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) ticket = atomicAdd(cnt + blockIdx.x, 1u);
+    __syncthreads();
+    if (ticket == gridDim.y - 1) {
+        __threadfence();
+        if (threadIdx.x < 32) {
+            const int i = blockIdx.x * 32 + threadIdx.x;
+            double s = 0.0;
+            for (int y0 = 0; y0 < (int)gridDim.y; y0 += 16) {      // 16 loads in flight, fixed order
+                double v[16];
+#pragma unroll
+                for (int y = 0; y < 16; ++y) v[y] = y0 + y < (int)gridDim.y ? __ldcg(part + (size_t)(y0 + y) * Nx + i) : 0.0;
+#pragma unroll
+                for (int y = 0; y < 16; ++y) s += v[y];
+            }
+            rho[i] = s * dv;
+        }
+        if (threadIdx.x == 0) cnt[blockIdx.x] = 0u;
+    }
 }
+
 
 // S9: single-CTA Poisson solve.  rho_i = dv * sum of partials (fp64), zero mean in fp64
 // (P:205-211), mixed-radix (4/8/16, in registers) DIF FFT in shared memory (fp32), E^_m = rho^_m / (i k_m)
 // with modes 0 and Nx/2 dropped, DIT inverse, E written to E_a (and E_b if non-NULL).
-struct PoissonRadix { int np; int r[4]; };
+struct PoissonRadix { int np; int lr[8]; int off[8]; };   // log2 radix and twiddle-table offset of each pass
 
+// One pass over sub-blocks of length B = 1 << lB, radix R, stride S = B / R.  tw = the pass's compact table
+// [(q-1) S + t] = e^{-2 pi i t q / B}: lanes read consecutive entries (no bank conflicts).
 template <int R, bool INV>
-__device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int Nx, const int B,
+__device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int Nx, const int lB,
                                              const float2* __restrict__ tw, const int tid, const int T)
 {
-    const int S = B / R, mul = Nx / B;
-    for (int g = tid; g < Nx / R; g += T) {
-        const int t = g % S, base = (g / S) * B + t, tm = t * mul;
+    constexpr int LR = ilog2(R);
+    const int lS = lB - LR, S = 1 << lS;
+    for (int g = tid; g < (Nx >> LR); g += T) {
+        const int t = g & (S - 1), base = ((g >> lS) << lB) + t;
         float2 x[R];
         if constexpr (!INV) {
 #pragma unroll
-            for (int k = 0; k < R; ++k) x[k] = z[base + k * S];
+            for (int k = 0; k < R; ++k) x[k] = z[base + (k << lS)];
             dft_dif<R, 1>(x);
             z[base] = x[0];
 #pragma unroll
-            for (int q = 1; q < R; ++q) z[base + q * S] = cmul(x[brev(q, R)], tw[tm * q]);
+            for (int q = 1; q < R; ++q) z[base + (q << lS)] = cmul(x[brev(q, R)], tw[((q - 1) << lS) + t]);
         } else {
             x[0] = z[base];
 #pragma unroll
-            for (int q = 1; q < R; ++q) x[brev(q, R)] = cmulc(z[base + q * S], tw[tm * q]);
+            for (int q = 1; q < R; ++q) x[brev(q, R)] = cmulc(z[base + (q << lS)], tw[((q - 1) << lS) + t]);
             idft_dit<R, 1>(x);
 #pragma unroll
-            for (int k = 0; k < R; ++k) z[base + k * S] = x[k];
+            for (int k = 0; k < R; ++k) z[base + (k << lS)] = x[k];
         }
     }
 }
 
-template <bool INV>
-__device__ __forceinline__ void poisson_pass_r(const int R, float2* z, const int Nx, const int B, const float2* tw,
-                                               const int tid, const int T)
-{
-    if (R == 16) poisson_pass<16, INV>(z, Nx, B, tw, tid, T);
-    else if (R == 8) poisson_pass<8, INV>(z, Nx, B, tw, tid, T);
-    else poisson_pass<4, INV>(z, Nx, B, tw, tid, T);
-}
-
-__global__ void __launch_bounds__(1024) poisson_kernel(const double* __restrict__ part, int nby, int Nx,
-                                                       const PoissonRadix rx, double dv, int tw_in_smem,
+// S9: single-CTA Poisson solve.  rho (fp64, from the density kernel) is made zero-mean in fp64
+// (P:205-211); radix-4 (one radix-8 pass for odd log2 Nx) DIF FFT in shared memory (fp32) with all threads
+// busy in every pass; E^_m = rho^_m / (i k_m) with modes 0 and Nx/2 dropped; DIT inverse; E to E_a (and E_b).
+__global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadix rx, int tw_len, int tw_in_smem,
                                                        const float2* __restrict__ tw_g, const float* __restrict__ ikt,
-                                                       double* __restrict__ rho, float* __restrict__ E_a,
+                                                       const double* __restrict__ rho, float* __restrict__ E_a,
                                                        float* __restrict__ E_b)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* z = reinterpret_cast<float2*>(smem_raw);
-    float* iks = reinterpret_cast<float*>(z + Nx);      // 1/(i k) factors, staged with the first loads
-    float2* tws = reinterpret_cast<float2*>(iks + Nx);
-    double* rs = reinterpret_cast<double*>(z);          // rho in fp64 shares the storage of z (8 B per point)
+    float* iks = reinterpret_cast<float*>(z + Nx);      // 1/(i k) factors
+    float2* twsm = reinterpret_cast<float2*>(iks + Nx); // compact twiddle tables of all passes (if they fit)
+    const float2* __restrict__ tws = tw_in_smem ? twsm : tw_g;
     __shared__ double wsum[32];
     __shared__ double mean_s;
     const int tid = threadIdx.x, T = blockDim.x;
+    double r0[16];                                       // Nx / T <= 16 values per thread
+    double local = 0.0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const int i = tid + k * T;
+        r0[k] = i < Nx ? rho[i] : 0.0;
+    }
     for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);
     if (tw_in_smem)
-        for (int i = tid; i < Nx; i += T) tws[i] = __ldg(tw_g + i);
-    const float2* __restrict__ tw = tw_in_smem ? tws : tw_g;
-    double local = 0.0;
-    for (int i = tid; i < Nx; i += T) {
-        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;       // nby is a power of two >= 1
-        if (nby >= 4) {
-#pragma unroll 2
-            for (int y = 0; y < nby; y += 4) {
-                s0 += part[(size_t)y * Nx + i];
-                s1 += part[(size_t)(y + 1) * Nx + i];
-                s2 += part[(size_t)(y + 2) * Nx + i];
-                s3 += part[(size_t)(y + 3) * Nx + i];
-            }
-        } else {
-            for (int y = 0; y < nby; ++y) s0 += part[(size_t)y * Nx + i];
-        }
-        const double s = ((s0 + s1) + (s2 + s3)) * dv;
-        rho[i] = s;
-        rs[i] = s;
-        local += s;
-    }
+        for (int i = tid; i < tw_len; i += T) twsm[i] = __ldg(tw_g + i);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) local += r0[k];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) local += __shfl_xor_sync(0xffffffffu, local, o);
     if ((tid & 31) == 0) wsum[tid >> 5] = local;
     __syncthreads();
-    if (tid == 0) {
-        double s = 0.0;
-        for (int w = 0; w < ((T + 31) >> 5); ++w) s += wsum[w];
-        mean_s = s / (double)Nx;
+    if (tid < 32) {
+        double s = tid < ((T + 31) >> 5) ? wsum[tid] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (tid == 0) mean_s = s / (double)Nx;
     }
     __syncthreads();
     const double mean = mean_s;
-    for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rs[i] - mean), 0.0f);   // same thread, same slot
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const int i = tid + k * T;
+        if (i < Nx) z[i] = make_float2((float)(r0[k] - mean), 0.0f);
+    }
     __syncthreads();
-    // forward, decimation in frequency: after passes r0, r1, .. position ((q0 r1 + q1) r2 + q2).. holds
-    // mode q0 + r0 (q1 + r1 (q2 + ..)); ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
-    int B = Nx;
+    // forward, decimation in frequency: position ((q0 r1 + q1) r2 + q2).. holds mode q0 + r0 (q1 + r1 (q2 + ..));
+    // ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
+    int lB = ilog2(Nx);
     for (int p = 0; p < rx.np; ++p) {
-        poisson_pass_r<false>(rx.r[p], z, Nx, B, tw, tid, T);
-        B /= rx.r[p];
+        if (rx.lr[p] == 3) poisson_pass<8, false>(z, Nx, lB, tws + rx.off[p], tid, T);
+        else poisson_pass<4, false>(z, Nx, lB, tws + rx.off[p], tid, T);
+        lB -= rx.lr[p];
         __syncthreads();
     }
     for (int pos = tid; pos < Nx; pos += T) {
@@ -309,8 +326,9 @@ __global__ void __launch_bounds__(1024) poisson_kernel(const double* __restrict_
     }
     __syncthreads();
     for (int p = rx.np - 1; p >= 0; --p) {
-        B *= rx.r[p];
-        poisson_pass_r<true>(rx.r[p], z, Nx, B, tw, tid, T);
+        lB += rx.lr[p];
+        if (rx.lr[p] == 3) poisson_pass<8, true>(z, Nx, lB, tws + rx.off[p], tid, T);
+        else poisson_pass<4, true>(z, Nx, lB, tws + rx.off[p], tid, T);
         __syncthreads();
     }
     for (int i = tid; i < Nx; i += T) {
@@ -338,6 +356,9 @@ struct vog_plan_s {
     double2* os_cs64;
     float* cg4;                    // f_eq exponents c_g as floats
     float* ikt;                    // Poisson: 1/(i k) factor per digit-reversed position
+    float2* ptw;                   // Poisson: compact per-pass twiddle tables
+    int ptw_len;
+    unsigned* dcnt;                // density: per column-group ticket counters
     vog::PoissonRadix prx;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int osx_lpi, osx_thr, osx_cps, osx_occ;
@@ -480,7 +501,7 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
-    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->cg4);
+    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->ptw); cudaFree(P->dcnt); cudaFree(P->cg4);
     cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
@@ -538,7 +559,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         while (lpi * 2 * nbx <= 40 && lpi * 2 <= Nv) lpi *= 2;
         while (lpi > 1 && Nv / lpi < P->n_sm * 3) lpi >>= 1;
         P->osx_lpi = lpi; P->osx_thr = 128; P->osx_cps = 0; P->osx_occ = 0;
-        P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 2; P->osv_gpc = 0;
+        P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 0; P->osv_gpc = 0;
     }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
@@ -570,18 +591,28 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     }
     alloc((void**)&P->os_cs64, sizeof(double2) * ocs64.size());
     std::vector<float> ikt(Nx);
+    std::vector<float2> ptw;
     {
-        static const int parts[9][4] = {{3, 3, 0, 0}, {4, 3, 0, 0}, {4, 4, 0, 0}, {3, 3, 3, 0}, {4, 3, 3, 0},
-                                        {4, 4, 3, 0}, {4, 4, 4, 0}, {4, 3, 3, 3}, {4, 4, 3, 3}};
-        const int* pp = parts[ilog2i(Nx) - 6];
+        int lg = ilog2i(Nx);
         P->prx.np = 0;
-        for (int i = 0; i < 4; ++i) { P->prx.r[i] = pp[i] ? 1 << pp[i] : 1; if (pp[i]) P->prx.np++; }
+        for (int i = 0; i < 8; ++i) { P->prx.lr[i] = 0; P->prx.off[i] = 0; }
+        if (lg & 1) { P->prx.lr[P->prx.np++] = 3; lg -= 3; }
+        while (lg > 0) { P->prx.lr[P->prx.np++] = 2; lg -= 2; }
+        int Bp = Nx;
+        for (int q = 0; q < P->prx.np; ++q) {             // compact twiddles [(j-1) S + t] = e^{-2 pi i t j / B}
+            const int R = 1 << P->prx.lr[q], S = Bp / R;
+            P->prx.off[q] = (int)ptw.size();
+            for (int j = 1; j < R; ++j)
+                for (int t = 0; t < S; ++t) ptw.push_back(unit_root_neg((long long)t * j, Bp));
+            Bp = S;
+        }
         for (int pos = 0; pos < Nx; ++pos) {
             int rem = pos, m = 0, wgt = Nx;
             for (int q = P->prx.np - 1; q >= 0; --q) {     // digits from the last pass outwards
-                const int dgt = rem % P->prx.r[q];
-                rem /= P->prx.r[q];
-                wgt /= P->prx.r[q];
+                const int rq = 1 << P->prx.lr[q];
+                const int dgt = rem % rq;
+                rem /= rq;
+                wgt /= rq;
                 m += dgt * wgt;
             }
             if (m == 0 || 2 * m == Nx) ikt[pos] = 0.0f;
@@ -592,6 +623,10 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         }
     }
     alloc((void**)&P->ikt, sizeof(float) * Nx);
+    alloc((void**)&P->ptw, sizeof(float2) * ptw.size());
+    P->ptw_len = (int)ptw.size();
+    alloc((void**)&P->dcnt, sizeof(unsigned) * (Nx / 32));
+    if (e == cudaSuccess) e = cudaMemsetAsync(P->dcnt, 0, sizeof(unsigned) * (Nx / 32), P->st);
     alloc((void**)&P->cg4, sizeof(float) * 4);
     float cg4h[4];
     for (int g = 0; g < 4; ++g) cg4h[g] = g < ng ? (float)p->feq.c[g] : 0.0f;
@@ -611,6 +646,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs, ocs.data(), sizeof(float2) * ocs.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->cg4, cg4h, sizeof(cg4h), cudaMemcpyHostToDevice, P->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(P->ptw, ptw.data(), sizeof(float2) * ptw.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->ikt, ikt.data(), sizeof(float) * Nx, cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs64, ocs64.data(), sizeof(double2) * ocs64.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->xtwA, xa.data(), sizeof(float2) * xa.size(), cudaMemcpyHostToDevice, P->st);
@@ -674,7 +710,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 12: if (value < 0 || value > 32) return VOG_EINVAL; P->osx_cps = value; break;
         case 13: if (value < 0 || (2 << value) > Nx || osv_smem_bytes(value, P->osv_rb) > 227 * 1024) return VOG_EINVAL; P->osv_np_log = value; break;
         case 14: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->osv_thr = value; break;
-        case 15: if (value < 1 || value > 2) return VOG_EINVAL; P->osv_rb = value; break;
+        case 15: if (value < 0 || value > 2) return VOG_EINVAL; P->osv_rb = value; break;
         case 16: if (value < 0) return VOG_EINVAL; P->osv_gpc = value; break;
         default: return VOG_EINVAL;
     }
@@ -765,17 +801,32 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
     a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
     a.nb = (Nv + OS_V - 1) / OS_V;
     a.lam = P->os_lam_v; a.tw = P->os_twx; a.cs = P->os_cs;
-    a.rb = P->osv_rb;
     a.ng = source ? P->p.feq.n : 0;
     a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
     for (int g = 0; g < 4; ++g) a.cg[g] = g < P->p.feq.n ? (float)P->p.feq.c[g] : 0.0f;
     const int strips = Nx / 32;
-    const int ngroups = (a.nb + a.rb - 1) / a.rb;
-    int gpc = P->osv_gpc;
-    if (gpc <= 0) {                       // about 6 CTAs per SM in total, else one group per CTA
-        gpc = (int)(((long long)strips * ngroups) / ((long long)P->n_sm * 6));
-        if (gpc < 1) gpc = 1;
+    // Launch shape: rb row blocks per group (128 rb threads, 3 or 2 CTAs per SM), gpc groups per CTA.  The
+    // kernel is latency-bound, so the time is ~ waves x (row blocks per CTA); ties go to the larger CTA
+    // (fewer reloads of the strip's symbol tables).
+    int rb = P->osv_rb, gpc = P->osv_gpc;
+    if (rb <= 0 || gpc <= 0) {
+        long long best = -1;
+        int brb = 1, bgpc = 1;
+        for (int r = 1; r <= 2; ++r) {
+            if (P->osv_rb > 0 && r != P->osv_rb) continue;
+            const int ng_r = (a.nb + r - 1) / r;
+            const long long slots = (long long)P->n_sm * (r == 1 ? 3 : 2);
+            for (int gp = 1; gp <= ng_r; ++gp) {
+                if (P->osv_gpc > 0 && gp != P->osv_gpc) continue;
+                const long long ctas = (long long)strips * ((ng_r + gp - 1) / gp);
+                const long long cost = ((ctas + slots - 1) / slots) * gp * r * 16 + 1;   // +1: table reload
+                if (best < 0 || cost < best || (cost == best && gp * r > bgpc * brb)) { best = cost; brb = r; bgpc = gp; }
+            }
+        }
+        rb = brb; gpc = bgpc;
     }
+    a.rb = rb;
+    const int ngroups = (a.nb + a.rb - 1) / a.rb;
     if (gpc > ngroups) gpc = ngroups;
     a.gpc = gpc;
     dim3 grid(strips, (ngroups + gpc - 1) / gpc);
@@ -876,23 +927,23 @@ static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
 static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
 {
     const int Nx = P->p.Nx, Nv = P->p.Nv;
+    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
     dim3 grid(Nx / 32, P->nby);
-    density_partial_kernel<<<grid, 256, 0, P->st>>>(f, Nx, Nv, Nv / P->nby, P->part);
+    density_partial_kernel<<<grid, 256, 0, P->st>>>(f, Nx, Nv, Nv / P->nby, P->part, dv, P->rho, P->dcnt);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     static bool attr = false;
     if (!attr) {
-        e = cudaFuncSetAttribute(poisson_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * (int)(sizeof(float2) + sizeof(float)));
+        e = cudaFuncSetAttribute(poisson_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 12 + 1024);
         if (e != cudaSuccess) return e;
         attr = true;
     }
-    int T = Nx / 2;
+    int T = Nx / 4;
     if (T > 1024) T = 1024;
+    if (T < 32) T = 32;
     const int tw_in_smem = Nx <= 8192;
-    const size_t psmem = sizeof(float2) * Nx * (tw_in_smem ? 2 : 1) + sizeof(float) * Nx;
-    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
-    poisson_kernel<<<1, T, psmem, P->st>>>(P->part, P->nby, Nx, P->prx, dv, tw_in_smem, P->tw_x, P->ikt, P->rho,
-                                            P->E_self, E_out);
+    const size_t psmem = (sizeof(float2) + sizeof(float)) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
+    poisson_kernel<<<1, T, psmem, P->st>>>(Nx, P->prx, P->ptw_len, tw_in_smem, P->ptw, P->ikt, P->rho, P->E_self, E_out);
     P->launches += 2;
     P->E_valid = true;
     return cudaGetLastError();
