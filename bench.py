@@ -33,11 +33,15 @@ BATCH = 16
 
 def _traffic():
     """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), else None."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
     try:
-        return float(json.load(open(path))["osx_kernel_bench_dram_bytes_per_launch"])
+        for line in open(path):
+            key, _, val = line.strip().partition(",")
+            if key == "osx_kernel_bench_dram_bytes_per_launch":
+                return float(val)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def _peaks():

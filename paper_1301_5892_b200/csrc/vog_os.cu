@@ -4,13 +4,13 @@
 
 namespace vog {
 
-// One CTA per line, thread k = 0..129.  beta = -c dt / Delta in fp64; b = floor(beta), b* = beta - b.
+// One CTA of 128 threads per line, thread k writes entry k (threads 0, 1 also entries 128, 129).  beta = -c dt / Delta in fp64; b = floor(beta), b* = beta - b.
 //   Lagrange 2d+1, Everett form: lambda = P(s;1-b*) + e^{i theta} P(s;b*), s = 2 - 2 cos(theta),
 //     P(s;t) = sum_k a_k(t) s^k, a_0 = t, a_k = a_{k-1} (k^2 - t^2) / (2k (2k+1));
 //   cubic spline: [B(b*+1) e^{-i theta} + B(b*) + B(b*-1) e^{i theta} + B(b*-2) e^{2 i theta}] 3/(2 + cos(theta)).
-__global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
+__global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
 {
-    const int l = blockIdx.x, k = threadIdx.x;
+    const int l = blockIdx.x;
     __shared__ double acoef[2][9];
     double beta;
     float sshift = 0.0f;
@@ -26,63 +26,66 @@ __global__ void __launch_bounds__(160) os_setup_kernel(const OsSetupArgs s)
     }
     const double fl = floor(beta);
     const double t = beta - fl;
-    double bm = fmod(fl, (double)s.N);
-    if (bm < 0.0) bm += (double)s.N;
-    int b = (int)bm;
-    if (b >= s.N) b = 0;
+    int b;
+    if (fabs(fl) < 9.0e18) {                         // N is a power of two: mathematical mod by masking
+        b = (int)(__double2ll_rn(fl) & (long long)(s.N - 1));
+    } else {
+        double bm = fmod(fl, (double)s.N);
+        if (bm < 0.0) bm += (double)s.N;
+        b = (int)bm;
+        if (b >= s.N) b = 0;
+    }
     const int br = s.vdir ? 0 : (b & 3);
     // x: [line][k]; v: transposed [k][line] so that a strip of 32 columns reads 256-byte rows
     float2* out = s.vdir ? s.lam + l : s.lam + (size_t)l * OS_LAMW;
     const size_t ks = s.vdir ? (size_t)s.n_lines : 1;
-    if (k < 18) {                                    // a_j(t) = t prod_{m=1..j} (m^2 - t^2) / (2m (2m+1))
-        const int half = k / 9, j = k - 9 * half;
+    if (threadIdx.x < 18 && !s.spline) {             // a_j(t) = t prod_{m=1..j} (m^2 - t^2) / (2m (2m+1))
+        const int half = threadIdx.x / 9, j = threadIdx.x - 9 * half;
         const double tt = half == 0 ? 1.0 - t : t;
         double a = tt;
         for (int m = 1; m <= j; ++m) a = a * ((double)(m * m) - tt * tt) * (1.0 / (double)(2 * m * (2 * m + 1)));
         acoef[half][j] = j <= s.d ? a : 0.0;
     }
     __syncthreads();
-    if (k >= OS_LAMW) return;
-    if (k == 129) {
-        out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift);
-        return;
-    }
     const double sc = 1.0 / (2.0 * (double)OS_LB);
-    if (k == 0) { out[0] = make_float2((float)sc, 0.0f); return; }   // lambda_0 = sum of the weights = 1
-    const double2 cs = s.cs64[k];                      // (cos, sin)(2 pi k / OS_LB), fp64 table
-    const double c = cs.x, sn = cs.y;
-    double lr, li;
-    if (s.spline) {
-        const double u = 1.0 - t;
-        const double Bm1 = u * u * u / 6.0, B0 = (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0;
-        const double B1 = (1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0, B2 = t * t * t / 6.0;
-        const double c2 = 2.0 * c * c - 1.0, s2 = 2.0 * sn * c;
-        const double g = 3.0 / (2.0 + c);
-        lr = (B0 + (Bm1 + B1) * c + B2 * c2) * g;
-        li = ((B1 - Bm1) * sn + B2 * s2) * g;
-    } else {
-        const double sv = 2.0 - 2.0 * c;
-        double p0 = 0.0, p1 = 0.0;
+    // 128 threads: k = threadIdx.x, and threads 0 and 1 also write entries 128 and 129 (16 CTAs per SM)
+    for (int k = threadIdx.x; k < OS_LAMW; k += 128) {
+        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift); continue; }
+        if (k == 0) { out[0] = make_float2((float)sc, 0.0f); continue; }   // lambda_0 = sum of the weights = 1
+        const double2 cs = s.cs64[k];                  // (cos, sin)(2 pi k / OS_LB), fp64 table
+        const double c = cs.x, sn = cs.y;
+        double lr, li;
+        if (s.spline) {
+            const double u = 1.0 - t;
+            const double Bm1 = u * u * u / 6.0, B0 = (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0;
+            const double B1 = (1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0, B2 = t * t * t / 6.0;
+            const double c2 = 2.0 * c * c - 1.0, s2 = 2.0 * sn * c;
+            const double g = 3.0 / (2.0 + c);
+            lr = (B0 + (Bm1 + B1) * c + B2 * c2) * g;
+            li = ((B1 - Bm1) * sn + B2 * s2) * g;
+        } else {
+            const double sv = 2.0 - 2.0 * c;
+            double p0 = 0.0, p1 = 0.0;
 #pragma unroll
-        for (int j = 8; j >= 0; --j) {               // coefficients beyond the degree are zero
-            p0 = p0 * sv + acoef[0][j];
-            p1 = p1 * sv + acoef[1][j];
+            for (int j = 8; j >= 0; --j) {             // coefficients beyond the degree are zero
+                p0 = p0 * sv + acoef[0][j];
+                p1 = p1 * sv + acoef[1][j];
+            }
+            lr = p0 + c * p1;
+            li = sn * p1;
         }
-        lr = p0 + c * p1;
-        li = sn * p1;
+        if (br) {
+            const double2 r = s.cs64[(k * br) & (OS_LB - 1)];
+            const double xr = lr * r.x - li * r.y, xi = lr * r.y + li * r.x;
+            lr = xr; li = xi;
+        }
+        out[k * ks] = make_float2((float)(lr * sc), (float)(li * sc));
     }
-    if (br) {
-        const double2 r = s.cs64[(k * br) & (OS_LB - 1)];
-        const double rc = r.x, rs = r.y;
-        const double xr = lr * rc - li * rs, xi = lr * rs + li * rc;
-        lr = xr; li = xi;
-    }
-    out[k * ks] = make_float2((float)(lr * sc), (float)(li * sc));
 }
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
 {
-    os_setup_kernel<<<s.n_lines, 160, 0, st>>>(s);
+    os_setup_kernel<<<s.n_lines, 128, 0, st>>>(s);
     return cudaGetLastError();
 }
 
