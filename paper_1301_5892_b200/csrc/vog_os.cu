@@ -35,7 +35,10 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
         b = (int)bm;
         if (b >= s.N) b = 0;
     }
-    const int br = s.vdir ? 0 : (b & 3);
+    // x keeps 16-byte aligned loads: b = 4 b4 + br with br in {-2,..,1} (centred, so that the stencil shifted by
+    // br has the same room, >= 14 cells, on both sides of the kept samples); br goes into the table as e^{i theta br}
+    const int b4 = ((b + 2) >> 2) & ((s.N >> 2) - 1);
+    const int br = s.vdir ? 0 : b - 4 * ((b + 2) >> 2);
     // x: [line][k]; v: transposed [k][line] so that a strip of 32 columns reads 256-byte rows
     float2* out = s.vdir ? s.lam + l : s.lam + (size_t)l * OS_LAMW;
     const size_t ks = s.vdir ? (size_t)s.n_lines : 1;
@@ -50,7 +53,7 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
     const double sc = 1.0 / (2.0 * (double)OS_LB);
     // 128 threads: k = threadIdx.x, and threads 0 and 1 also write entries 128 and 129 (16 CTAs per SM)
     for (int k = threadIdx.x; k < OS_LAMW; k += 128) {
-        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : (b >> 2)), sshift); continue; }
+        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : b4), sshift); continue; }
         if (k == 0) { out[0] = make_float2((float)sc, 0.0f); continue; }   // lambda_0 = sum of the weights = 1
         const double2 cs = s.cs64[k];                  // (cos, sin)(2 pi k / OS_LB), fp64 table
         const double c = cs.x, sn = cs.y;

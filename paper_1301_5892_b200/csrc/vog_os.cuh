@@ -7,13 +7,13 @@
 // P:131-149 can be taken block-wise (overlap-save): every block of LB = 256 samples of the rolled line
 // r_i = u_{i+b} is transformed, multiplied by the symbol lambda(theta_k), theta_k = 2 pi k / LB, and
 // transformed back; the V = 224 samples in the middle of the block are exactly (Lagrange) or to
-// 0.268^17 ~ 2e-10 (spline, far below fp32 rounding) the samples of A u, the H = 16 on either side are
-// discarded.  Compared with one length-N transform per line:
+// <= 2e-9 max|u| (spline: the neglected tail of the row, far below fp32 rounding) the samples
+// of A u, the H = 16 on either side are discarded.  Compared with one length-N transform per line:
 //   * 8 instead of log2(N) butterfly levels, two passes instead of three, no big twiddle table;
 //   * the symbol is a per-line table lam[k], k = 0..128, computed in fp64 by the setup kernel and shared
 //     by all blocks of the line -- no polynomial evaluation in the hot loop;
 //   * the integer part b of the shift is folded into the load address ("integer roll by
-//     index"): no rotation factor at all (x keeps a residual b mod 4 in the table to stay 128-bit aligned);
+//     index"): no rotation factor at all (x keeps a residual br in {-2..1} in the table to stay 128-bit aligned);
 //   * the working set of a block is 1-2 KB, so the strided (v) direction can use tiles 16-32 columns
 //     wide at ANY Nv: full 32-byte sectors, no shared-memory capacity limit.
 // x-direction: even/odd packing (a block is 128 complex), CTA owns whole lines, in place.
