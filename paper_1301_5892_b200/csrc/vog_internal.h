@@ -78,6 +78,7 @@ struct OsArgs {
     const float* vmu_tab;  // [ng][Nv]
     float cg[4];
     const float* cg4;      // the same four constants in device memory (dynamic indexing)
+    float dvf;             // v: dv as float (row stride of the delta-f source recurrence)
 };
 
 struct OsSetupArgs {

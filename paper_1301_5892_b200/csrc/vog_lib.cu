@@ -803,6 +803,7 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
     a.lam = P->os_lam_v; a.tw = P->os_twx; a.cs = P->os_cs;
     a.ng = source ? P->p.feq.n : 0;
     a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
+    a.dvf = (float)((P->p.vmax - P->p.vmin) / (double)Nv);
     for (int g = 0; g < 4; ++g) a.cg[g] = g < P->p.feq.n ? (float)P->p.feq.c[g] : 0.0f;
     const int strips = Nx / 32;
     // Launch shape: rb row blocks per group (128 rb threads, 3 or 2 CTAs per SM), gpc groups per CTA.  The

@@ -472,17 +472,27 @@ __global__ void __launch_bounds__(256, 2) osv_kernel(const OsArgs a)
 #pragma unroll
             for (int k = 0; k < 8; ++k) x[k] = cadd(x[k], d2);
             if (a.ng > 0) {                                       // delta-f source
+                // f_eq,g(v - s) - f_eq,g(v) = f_eq,g(v) expm1(x_j),  x_j = c s (2 (v_j - mu) - s).  x_j is affine
+                // in the row j, so along the rows of this thread expm1 obeys e' = e R + (R - 1): one expm1 per
+                // item and two constants per row stride instead of one expm1 per cell (7 recurrence steps:
+                // a few ulp of the source term).
 #pragma unroll 1
                 for (int g = 0; g < a.ng; ++g) {
                     const float cgs = a.cg4[g] * ssh;
                     const float* __restrict__ ft = a.feq_tab + g * Nv;
-                    const float* __restrict__ vt = a.vmu_tab + g * Nv;
+                    const float u0 = __ldg(a.vmu_tab + g * Nv);                // v_0 - mu_g
+                    const float h1 = 2.0f * cgs * a.dvf, h32 = 32.0f * h1;
+                    const float r1 = expm1f(h1);
+                    const float R32 = expf(h32), r32 = expm1f(h32);
+                    float ea = expm1f(cgs * (2.0f * fmaf((float)row0, a.dvf, u0) - ssh));
+                    float eb = fmaf(ea, expf(h1), r1);
 #pragma unroll
                     for (int k = 0; k < 8; ++k) {
                         const int j = min(max(row0 + 32 * k, 0), Nv - 2);     // rows outside are never stored
-                        // f_eq,g(v - s) - f_eq,g(v) = f_eq,g(v) expm1(c s (2 (v - mu) - s))
-                        x[k].x = fmaf(__ldg(ft + j), expm1f(cgs * (2.0f * __ldg(vt + j) - ssh)), x[k].x);
-                        x[k].y = fmaf(__ldg(ft + j + 1), expm1f(cgs * (2.0f * __ldg(vt + j + 1) - ssh)), x[k].y);
+                        x[k].x = fmaf(__ldg(ft + j), ea, x[k].x);
+                        x[k].y = fmaf(__ldg(ft + j + 1), eb, x[k].y);
+                        ea = fmaf(ea, R32, r32);
+                        eb = fmaf(eb, R32, r32);
                     }
                 }
             }
