@@ -30,6 +30,11 @@ __device__ __forceinline__ void os_cp_async16(void* smem, const void* gmem)
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
 }
+__device__ __forceinline__ void os_cp_async16_cg(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
 __device__ __forceinline__ void os_cp_async_commit_wait()
 {
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
@@ -100,20 +105,28 @@ __device__ __forceinline__ OsxSlots osx_slots(const int lb, const int tp)
 }
 __host__ __device__ constexpr int osx_cls(int g) { return (g & 3) == 0 ? 0 : (g < 4 ? g : 8 - g); }
 
-__device__ __forceinline__ void osx_load(float4 (&v)[8], const float4* __restrict__ gline, const int mask,
-                                         const int wc)
+// asynchronous landing of one item's 8 window chunks in the scratch slots the SAME thread transforms in
+// pass A and reads again in the inverse pass (window chunk tp + 8k <-> slot of (group k, tp)): no other
+// thread touches these slots between the inverse pass of one line group and pass A of the next.
+__device__ __forceinline__ void osx_land(float4* __restrict__ scr, const OsxSlots sl, const float4* __restrict__ gline,
+                                         const int mask, const int wc)
 {
 #pragma unroll
-    for (int k = 0; k < 8; ++k) v[k] = __ldg(gline + ((wc + 8 * k) & mask));
+    for (int k = 0; k < 8; ++k)
+        os_cp_async16_cg(scr + sl.s[osx_cls(k)] + k * 8, gline + ((wc + 8 * k) & mask));
 }
 
-// forward pass A of one item: two adjacent radix-8 butterflies (positions 2tp, 2tp+1 + 16k)
-__device__ __forceinline__ void osx_fwd(const float4 (&v)[8], float4* __restrict__ scr, const OsxSlots sl,
+// forward pass A of one item: two adjacent radix-8 butterflies (positions 2tp, 2tp+1 + 16k), in place
+__device__ __forceinline__ void osx_fwd(float4* __restrict__ scr, const OsxSlots sl,
                                         const int tp, const float2* __restrict__ twS)
 {
     float2 x0[8], x1[8];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) { x0[k] = make_float2(v[k].x, v[k].y); x1[k] = make_float2(v[k].z, v[k].w); }
+    for (int k = 0; k < 8; ++k) {
+        const float4 v = scr[sl.s[osx_cls(k)] + k * 8];
+        x0[k] = make_float2(v.x, v.y);
+        x1[k] = make_float2(v.z, v.w);
+    }
     dft_dif<8, 1>(x0);
     dft_dif<8, 1>(x1);
     scr[sl.s[0]] = make_float4(x0[0].x, x0[0].y, x1[0].x, x1[0].y);
@@ -241,39 +254,29 @@ __global__ void __launch_bounds__(128, 4) osx_kernel(const OsArgs a)
     for (int i = tid; i < 129; i += T) csS[i] = __ldg(a.cs + i);
     for (int i = tid; i < 112; i += T) twS[i] = __ldg(a.tw + i);
 
+    const int nA = nblk * 8;
+    // window chunk of item w of the line group starting at line0, and the landing of all of a thread's items
+    auto land = [&](const int w, const int line0) {
+        const int lb = w >> 3, tp = w & 7;
+        const int l = (int)(((unsigned)lb * inv_nb) >> 16), blk = lb - l * nb;
+        const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
+        const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
+        osx_land(scr, osx_slots(lb, tp), gline, nchunk - 1, osx::VC * blk - osx::HC + b4 + tp);
+    };
+    if ((int)blockIdx.x < a.n_groups)
+        for (int w = tid; w < nA; w += T) land(w, blockIdx.x * lpi);
     for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
         const int line0 = g * lpi;
-        __syncthreads();                           // previous iteration done with scratch and tables
+        __syncthreads();                           // previous iteration done with the symbol tables
         {
             const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
             float4* dst4 = reinterpret_cast<float4*>(lamS);
             for (int i = tid; i < lpi * (OS_LAMW / 2); i += T) os_cp_async16(dst4 + i, src4 + i);
         }
-        // ---- pass A: global -> registers -> scratch; the loads of two rounds are in flight together
-        const int nA = nblk * 8;
+        os_cp_async_commit_wait();                 // this thread's window chunks (and table rows) have landed
+        // ---- pass A: scratch -> registers -> scratch, every thread on the slots it landed itself
 #pragma unroll 1
-        for (int w = tid; w < nA; w += 2 * T) {
-            const int w2 = w + T;
-            const bool has2 = w2 < nA;
-            float4 v0[8], v1[8];
-            const int lb = w >> 3, tp = w & 7;
-            const int lb2 = w2 >> 3, tp2 = w2 & 7;
-            {
-                const int l = (int)(((unsigned)lb * inv_nb) >> 16), blk = lb - l * nb;
-                const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
-                const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
-                osx_load(v0, gline, nchunk - 1, osx::VC * blk - osx::HC + b4 + tp);
-            }
-            if (has2) {
-                const int l = (int)(((unsigned)lb2 * inv_nb) >> 16), blk = lb2 - l * nb;
-                const int b4 = __float_as_int(__ldg(&a.lam[(size_t)(line0 + l) * OS_LAMW + 129].x));
-                const float4* gline = reinterpret_cast<const float4*>(a.src) + (size_t)(line0 + l) * nchunk;
-                osx_load(v1, gline, nchunk - 1, osx::VC * blk - osx::HC + b4 + tp2);
-            }
-            osx_fwd(v0, scr, osx_slots(lb, tp), tp, twS);
-            if (has2) osx_fwd(v1, scr, osx_slots(lb2, tp2), tp2, twS);
-        }
-        os_cp_async_commit_wait();
+        for (int w = tid; w < nA; w += T) osx_fwd(scr, osx_slots(w >> 3, w & 7), w & 7, twS);
         __syncthreads();
         // ---- middle stage: items [0, nblk) are the special items of the blocks, then 3 per block
 #pragma unroll 1
@@ -289,13 +292,18 @@ __global__ void __launch_bounds__(128, 4) osx_kernel(const OsArgs a)
             }
         }
         __syncthreads();
-        // ---- inverse pass A: scratch -> registers -> global
+        // ---- inverse pass A: scratch -> registers -> global; as soon as an item's slots are read, the
+        // same item of the NEXT line group starts landing in them (hidden behind the rest of this pass).
+        // In place this is safe: every load of THIS group completed before the barrier after pass A, and
+        // the next group is other lines.
+        const int gn = g + gridDim.x;
 #pragma unroll 1
         for (int w = tid; w < nA; w += T) {
             const int lb = w >> 3, tp = w & 7;
             const int l = (int)(((unsigned)lb * inv_nb) >> 16), blk = lb - l * nb;
             float4* gline = reinterpret_cast<float4*>(a.dst) + (size_t)(line0 + l) * nchunk;
             osx_inv(gline, nchunk, osx::VC * blk, scr, osx_slots(lb, tp), tp, twS, dcS[lb]);
+            if (gn < a.n_groups) land(w, gn * lpi);
         }
     }
 }
