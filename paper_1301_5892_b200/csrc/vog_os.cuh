@@ -14,11 +14,13 @@
 //     by all blocks of the line -- no polynomial evaluation in the hot loop;
 //   * the integer part b of the shift is folded into the load address ("integer roll by
 //     index"): no rotation factor at all (x keeps a residual br in {-2..1} in the table to stay 128-bit aligned);
-//   * the working set of a block is 1-2 KB, so the strided (v) direction can use tiles 16-32 columns
-//     wide at ANY Nv: full 32-byte sectors, no shared-memory capacity limit.
+//   * the working set of a block is 1 KB per line, so the strided (v) direction can use strips 32 columns
+//     wide at ANY Nv: full 128-byte lines, no shared-memory capacity limit.
 // x-direction: even/odd packing (a block is 128 complex), CTA owns whole lines, in place.
-// v-direction: two-for-one over adjacent columns (a block is 256 complex per column pair), OUT of place
-//   (src != dst): a block reads rows that other blocks write, so in-place would race.
+// v-direction: 32 adjacent columns = the 32 lanes of a warp, the same even/odd block transform per column;
+//   OUT of place (src != dst): a block reads rows that other blocks write, so in-place would race.
+// Both kernels land their input asynchronously (cp.async) in the scratch slots that the landing thread
+// itself transforms, and start landing the next work unit as soon as those slots have been read back.
 #pragma once
 #include "vog_fft.cuh"
 #include "vog_internal.h"
@@ -265,9 +267,11 @@ __global__ void __launch_bounds__(128, 4) osx_kernel(const OsArgs a)
     };
     if ((int)blockIdx.x < a.n_groups)
         for (int w = tid; w < nA; w += T) land(w, blockIdx.x * lpi);
+    __syncthreads();                               // csS, twS visible
     for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
         const int line0 = g * lpi;
-        __syncthreads();                           // previous iteration done with the symbol tables
+        // (the symbol tables and dcS of the previous group were last read before / are rewritten after a
+        // barrier of this iteration, so no barrier is needed here)
         {
             const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
             float4* dst4 = reinterpret_cast<float4*>(lamS);
@@ -375,30 +379,45 @@ __device__ __forceinline__ void osv_mid(float2* __restrict__ scr, const int u, c
     for (int j = 0; j < 16; ++j) { pa[j * W] = XA[j]; pb[j * W] = XB[j]; }
 }
 
-__device__ __forceinline__ void osv_load(float2 (&x)[8], const float* __restrict__ col, const int Nx, const int vmask,
-                                         const int r0)
+__device__ __forceinline__ void os_cp_async4(void* smem, const void* gmem)
 {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+
+// asynchronous landing of one item (butterfly t of a block, this lane's column): sample n = t + 16 k is rows
+// r0 + 32 k and r0 + 32 k + 1 of the column and lands in the slot o[k 16 W] that the same thread transforms
+// in pass A and reads again in the inverse pass.
+__device__ __forceinline__ void osv_land(float2* __restrict__ o, const float* __restrict__ col, const int Nx,
+                                         const int vmask, const int r0)
+{
+    constexpr int W = osv::W;
     const int rr = r0 & vmask;
     if (rr + OS_LB <= vmask) {                      // the window does not wrap: constant row stride
         const float* p = col + rr * Nx;
         const int s32 = 32 * Nx;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            x[k] = make_float2(__ldg(p), __ldg(p + Nx));
+            os_cp_async4(&o[k * 16 * W].x, p);
+            os_cp_async4(&o[k * 16 * W].y, p + Nx);
             p += s32;
         }
     } else {
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
             const int ra = (r0 + 32 * k) & vmask, rb = (r0 + 32 * k + 1) & vmask;
-            x[k] = make_float2(__ldg(col + ra * Nx), __ldg(col + rb * Nx));
+            os_cp_async4(&o[k * 16 * W].x, col + ra * Nx);
+            os_cp_async4(&o[k * 16 * W].y, col + rb * Nx);
         }
     }
 }
 
-__device__ __forceinline__ void osv_fwd(float2 (&x)[8], float2* __restrict__ o, const float2* __restrict__ tw)
+__device__ __forceinline__ void osv_fwd(float2* __restrict__ o, const float2* __restrict__ tw)
 {
     constexpr int W = osv::W;
+    float2 x[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) x[k] = o[k * 16 * W];
     dft_dif<8, 1>(x);
     o[0] = x[0];
 #pragma unroll
@@ -436,20 +455,20 @@ __global__ void __launch_bounds__(256, 2) osv_kernel(const OsArgs a)
     float* const ocol = a.dst + c0 + lane;
 
     const int ngroups = (nb + rb - 1) / rb;
-    const int g1 = min(ngroups, ((int)blockIdx.y + 1) * a.gpc);
-    for (int gi = blockIdx.y * a.gpc; gi < g1; ++gi) {
-        // ---- pass A: global -> registers -> scratch (two butterflies' loads in flight)
+    const int g0 = blockIdx.y * a.gpc, g1 = min(ngroups, g0 + a.gpc);
+    auto land = [&](const int w, const int gi) {
+        const int bl = w >> 4, t = w & 15, blk = gi * rb + bl;
+        if (blk < nb) osv_land(scr + (bl * MB + t) * W + lane, col, Nx, vmask, blk * OS_V - OS_H + b + 2 * t);
+    };
+    if (g0 < g1)
+        for (int w = wid; w < rb * 16; w += nw) land(w, g0);
+    for (int gi = g0; gi < g1; ++gi) {
+        os_cp_async_commit_wait();                 // this thread's samples have landed
+        // ---- pass A: scratch -> registers -> scratch, every thread on the slots it landed itself
 #pragma unroll 1
-        for (int w = wid; w < rb * 16; w += 2 * nw) {
-            const int w2 = w + nw;
-            const int bl = w >> 4, t = w & 15, bl2 = w2 >> 4, t2 = w2 & 15;
-            const int blk = gi * rb + bl, blk2 = gi * rb + bl2;
-            const bool ok = blk < nb, ok2 = (w2 < rb * 16) && (blk2 < nb);
-            float2 x0[8], x1[8];
-            if (ok) osv_load(x0, col, Nx, vmask, blk * OS_V - OS_H + b + 2 * t);
-            if (ok2) osv_load(x1, col, Nx, vmask, blk2 * OS_V - OS_H + b + 2 * t2);
-            if (ok) osv_fwd(x0, scr + (bl * MB + t) * W + lane, twS + t);
-            if (ok2) osv_fwd(x1, scr + (bl2 * MB + t2) * W + lane, twS + t2);
+        for (int w = wid; w < rb * 16; w += nw) {
+            const int bl = w >> 4, t = w & 15;
+            if (gi * rb + bl < nb) osv_fwd(scr + (bl * MB + t) * W + lane, twS + t);
         }
         __syncthreads();
         // ---- middle stage: item u of block bl, all 32 columns of the warp alike
@@ -515,8 +534,10 @@ __global__ void __launch_bounds__(256, 2) osv_kernel(const OsArgs a)
                 }
                 po += s32;
             }
+            if (gi + 1 < g1) land(w, gi + 1);      // the next group's item lands in the slots just read
         }
-        __syncthreads();
+        // no barrier here: pass A touches only a thread's own slots, and dcS is rewritten only after the
+        // barrier that follows the next pass A
     }
 }
 
