@@ -46,7 +46,11 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
         const int half = threadIdx.x / 9, j = threadIdx.x - 9 * half;
         const double tt = half == 0 ? 1.0 - t : t;
         double a = tt;
-        for (int m = 1; m <= j; ++m) a = a * ((double)(m * m) - tt * tt) * (1.0 / (double)(2 * m * (2 * m + 1)));
+        constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
+                                   1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
+#pragma unroll
+        for (int m = 1; m <= 8; ++m)
+            if (m <= j) a = a * ((double)(m * m) - tt * tt) * rcp[m];
         acoef[half][j] = j <= s.d ? a : 0.0;
     }
     __syncthreads();
