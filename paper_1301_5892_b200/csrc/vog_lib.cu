@@ -264,8 +264,8 @@ __device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int N
     }
 }
 
-// S9: single-CTA Poisson solve.  rho (fp64, from the density kernel) is made zero-mean in fp64
-// (P:205-211); radix-4 (one radix-8 pass for odd log2 Nx) DIF FFT in shared memory (fp32) with all threads
+// S9: single-CTA Poisson solve.  rho (fp64, from the density kernel) minus a reference value in fp64
+// (zero mean, = mode 0 dropped); radix-4 (one radix-8 pass for odd log2 Nx) DIF FFT in shared memory (fp32) with all threads
 // busy in every pass; E^_m = rho^_m / (i k_m) with modes 0 and Nx/2 dropped; DIT inverse; E to E_a (and E_b).
 __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadix rx, int tw_len, int tw_in_smem,
                                                        const float2* __restrict__ tw_g, const float* __restrict__ ikt,
@@ -277,38 +277,15 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     float* iks = reinterpret_cast<float*>(z + Nx);      // 1/(i k) factors
     float2* twsm = reinterpret_cast<float2*>(iks + Nx); // compact twiddle tables of all passes (if they fit)
     const float2* __restrict__ tws = tw_in_smem ? twsm : tw_g;
-    __shared__ double wsum[32];
-    __shared__ double mean_s;
     const int tid = threadIdx.x, T = blockDim.x;
-    double r0[16];                                       // Nx / T <= 16 values per thread
-    double local = 0.0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        const int i = tid + k * T;
-        r0[k] = i < Nx ? rho[i] : 0.0;
-    }
+    // Zero mean = mode 0 dropped below.  Before the conversion to fp32 a constant of the size of
+    // the mean must still be removed in fp64 (in full-f mode rho ~ 1 carries a 1e-3 perturbation): rho[0]
+    // serves as well as the mean (any constant only changes mode 0) and needs no reduction.
+    const double ref = rho[0];
     for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);
     if (tw_in_smem)
         for (int i = tid; i < tw_len; i += T) twsm[i] = __ldg(tw_g + i);
-#pragma unroll
-    for (int k = 0; k < 16; ++k) local += r0[k];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) local += __shfl_xor_sync(0xffffffffu, local, o);
-    if ((tid & 31) == 0) wsum[tid >> 5] = local;
-    __syncthreads();
-    if (tid < 32) {
-        double s = tid < ((T + 31) >> 5) ? wsum[tid] : 0.0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (tid == 0) mean_s = s / (double)Nx;
-    }
-    __syncthreads();
-    const double mean = mean_s;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        const int i = tid + k * T;
-        if (i < Nx) z[i] = make_float2((float)(r0[k] - mean), 0.0f);
-    }
+    for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rho[i] - ref), 0.0f);
     __syncthreads();
     // forward, decimation in frequency: position ((q0 r1 + q1) r2 + q2).. holds mode q0 + r0 (q1 + r1 (q2 + ..));
     // ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
