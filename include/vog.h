@@ -14,7 +14,9 @@
  * plan's CUDA stream.  Argument errors are detected before anything is enqueued.
  * Pointers named *_dev are caller-owned DEVICE memory (16-byte aligned); pointers named
  * *_host are caller-owned HOST memory.  The library never frees caller memory.  Plan-owned
- * scratch is O(Nx + Nv): no N^2 work array exists (contrast P:307, 326).  A plan is not
+ * scratch is O(Nx + Nv) tables, plus -- only when Nv >= 1024 -- ONE second grid of Nx*Nv floats that the
+ * out-of-place v kernel writes and the following x-advection reads back (contrast the
+ * paper's transposed copies).  It is allocated on the first v-advection.  A plan is not
  * thread-safe; distinct plans are independent.  There is no CPU fallback anywhere: every
  * step of the path runs in the library's CUDA kernels.
  */
@@ -66,7 +68,9 @@ int vog_advect_x(vog_plan_t plan, float* f_dev, double dt);
 /* Transport in v over dt: for every space column i, the periodic line
  * f[:][i] is shifted by beta_i = -E_i*dt/dv; E_dev holds Nx floats (the total advecting
  * field).  In delta-f mode the source f_eq(v_j - dt*E_i) - f_eq(v_j) is added, an
- * evaluation, not an interpolation.  In place. */
+ * evaluation, not an interpolation.  In place for the caller; for Nv >= 1024 the kernel writes
+ * the plan's second grid and the result is copied back (vog_step avoids that copy).  VOG_ENOMEM if the
+ * second grid cannot be allocated. */
 int vog_advect_v(vog_plan_t plan, float* f_dev, const float* E_dev, double dt);
 
 /* Self-consistent field: rho_i = dv * sum_j f[j][i] (of delta f in

@@ -40,8 +40,9 @@ static cudaError_t launch_sym(const AdvectArgs& a, int sym, int n_tiles, int thr
 cudaError_t VOG_CAT(advect_launch_, VOG_N)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,
                                            size_t smem, cudaStream_t st)
 {
-    return vdir ? launch_sym<VOG_N, true>(a, sym, n_tiles, threads, smem, st)
-                : launch_sym<VOG_N, false>(a, sym, n_tiles, threads, smem, st);
+    // the contiguous direction is served by advect_x_kernel (vog_advect_x.cuh); only the column-tile
+    // instantiation of this kernel is built
+    return vdir ? launch_sym<VOG_N, true>(a, sym, n_tiles, threads, smem, st) : cudaErrorInvalidValue;
 }
 
 // ---- contiguous-line (x) kernel

@@ -42,11 +42,6 @@ __device__ __forceinline__ void os_cp_async_commit_wait()
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
 }
 
-// scratch swizzle for the x kernel: chunk C (16 B = 2 complex) of the block-major scratch; key mixes the
-// radix-16 group (C >> 3) & 7 and the parity of the block (C >> 6) & 1 so that the 8 lanes of a
-// quarter-warp (4 items x 2 blocks) hit 8 distinct 16-byte bank groups in the middle stage.
-__device__ __forceinline__ int os_swz(int C) { return C ^ (((C >> 3) ^ ((C >> 4) & 4)) & 7); }
-
 // One mirror pair (k, M-k) of the half-length spectrum of an even/odd packed real block:
 // untangle, multiply by the tabulated symbol, re-tangle.  P = Z_k, Qm = Z_{M-k}; cs = (cos, sin)(2 pi k/LB);
 // a = lambda_k/(2 LB), cc = conj(lambda_{M-k})/(2 LB).
@@ -63,19 +58,6 @@ __device__ __forceinline__ void os_pair_x(float2& P, float2& Qm, const float2 cs
     P = cadd(Ep, make_float2(-Op.y, Op.x));                         // E' + i O'
     const float2 R = csub(Ep, make_float2(-Op.y, Op.x));            // E' - i O'
     Qm = make_float2(R.x, -R.y);
-}
-
-// Two-for-one pair (m, LB-m) of the spectrum of z = uA + i uB: P = Z_m, Q = Z_{LB-m};
-// la, lb = lambda_m/(2 LB) of line A and line B.
-__device__ __forceinline__ void os_pair_v(float2& P, float2& Q, const float2 la, const float2 lb)
-{
-    const float2 ua = cadd(P, make_float2(Q.x, -Q.y));              // 2 U_A = P + conj Q
-    const float2 ub = cadd(make_float2(P.y, -P.x), make_float2(Q.y, Q.x));   // 2 U_B = (P - conj Q)/i
-    const float2 wa = cmul(ua, la), wb = cmul(ub, lb);
-    const float2 iwb = make_float2(-wb.y, wb.x);
-    P = cadd(wa, iwb);                                              // W_A + i W_B
-    const float2 R = csub(wa, iwb);                                 // W_A - i W_B
-    Q = make_float2(R.x, -R.y);                                     // conj(W_A) + i conj(W_B)
 }
 
 
