@@ -368,9 +368,11 @@ __device__ __forceinline__ void os_cp_async4(void* smem, const void* gmem)
 }
 
 // asynchronous landing of one item (butterfly t of a block, this lane's column): sample n = t + 16 k is rows
-// r0 + 32 k and r0 + 32 k + 1 of the column and lands in the slot o[k 16 W] that the same thread transforms
-// in pass A and reads again in the inverse pass.
-__device__ __forceinline__ void osv_land(float2* __restrict__ o, const float* __restrict__ col, const int Nx,
+// r0 + 32 k and r0 + 32 k + 1 of the column.  It lands in the 256 bytes of position n that this WARP (32
+// columns, same t) transforms in pass A and reads again in the inverse pass -- planar (32 real parts, then 32
+// imaginary parts) so that the 4-byte copies of a warp are bank-conflict free; pass A reads the planar
+// words and writes the position back as interleaved float2 (all reads of a warp precede its writes).
+__device__ __forceinline__ void osv_land(float* __restrict__ pw, const float* __restrict__ col, const int Nx,
                                          const int vmask, const int r0)
 {
     constexpr int W = osv::W;
@@ -380,26 +382,29 @@ __device__ __forceinline__ void osv_land(float2* __restrict__ o, const float* __
         const int s32 = 32 * Nx;
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            os_cp_async4(&o[k * 16 * W].x, p);
-            os_cp_async4(&o[k * 16 * W].y, p + Nx);
+            os_cp_async4(pw + k * 16 * W * 2, p);
+            os_cp_async4(pw + k * 16 * W * 2 + W, p + Nx);
             p += s32;
         }
     } else {
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
             const int ra = (r0 + 32 * k) & vmask, rb = (r0 + 32 * k + 1) & vmask;
-            os_cp_async4(&o[k * 16 * W].x, col + ra * Nx);
-            os_cp_async4(&o[k * 16 * W].y, col + rb * Nx);
+            os_cp_async4(pw + k * 16 * W * 2, col + ra * Nx);
+            os_cp_async4(pw + k * 16 * W * 2 + W, col + rb * Nx);
         }
     }
 }
 
-__device__ __forceinline__ void osv_fwd(float2* __restrict__ o, const float2* __restrict__ tw)
+// pw = planar words of position t for this lane (float index (pos * 32) * 2 + lane); o = the same position as
+// interleaved float2 for this lane
+__device__ __forceinline__ void osv_fwd(const float* __restrict__ pw, float2* __restrict__ o,
+                                        const float2* __restrict__ tw)
 {
     constexpr int W = osv::W;
     float2 x[8];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) x[k] = o[k * 16 * W];
+    for (int k = 0; k < 8; ++k) x[k] = make_float2(pw[k * 16 * W * 2], pw[k * 16 * W * 2 + W]);
     dft_dif<8, 1>(x);
     o[0] = x[0];
 #pragma unroll
@@ -440,7 +445,9 @@ __global__ void __launch_bounds__(256, 2) osv_kernel(const OsArgs a)
     const int g0 = blockIdx.y * a.gpc, g1 = min(ngroups, g0 + a.gpc);
     auto land = [&](const int w, const int gi) {
         const int bl = w >> 4, t = w & 15, blk = gi * rb + bl;
-        if (blk < nb) osv_land(scr + (bl * MB + t) * W + lane, col, Nx, vmask, blk * OS_V - OS_H + b + 2 * t);
+        if (blk < nb)
+            osv_land(reinterpret_cast<float*>(scr + (bl * MB + t) * W) + lane, col, Nx, vmask,
+                     blk * OS_V - OS_H + b + 2 * t);
     };
     if (g0 < g1)
         for (int w = wid; w < rb * 16; w += nw) land(w, g0);
@@ -450,7 +457,9 @@ __global__ void __launch_bounds__(256, 2) osv_kernel(const OsArgs a)
 #pragma unroll 1
         for (int w = wid; w < rb * 16; w += nw) {
             const int bl = w >> 4, t = w & 15;
-            if (gi * rb + bl < nb) osv_fwd(scr + (bl * MB + t) * W + lane, twS + t);
+            if (gi * rb + bl < nb)
+                osv_fwd(reinterpret_cast<const float*>(scr + (bl * MB + t) * W) + lane, scr + (bl * MB + t) * W + lane,
+                        twS + t);
         }
         __syncthreads();
         // ---- middle stage: item u of block bl, all 32 columns of the warp alike
