@@ -1,4 +1,4 @@
-// vog_os.cu -- overlap-save advection kernels: instantiation, launchers and the fp64 setup kernel that
+// vog_os.cu -- overlap-save advection kernels: instantiation, launchers and the setup kernel that
 // tabulates the symbol lambda(theta_k) per line (S1 + the closed form of S4).  Product code.
 #include "vog_os.cuh"
 
@@ -11,7 +11,6 @@ namespace vog {
 __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
 {
     const int l = blockIdx.x;
-    __shared__ double acoef[2][9];
     double beta;
     float sshift = 0.0f;
     if (s.mode == 0) {
@@ -42,51 +41,63 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
     // x: [line][k]; v: transposed [k][line] so that a strip of 32 columns reads 256-byte rows
     float2* out = s.vdir ? s.lam + l : s.lam + (size_t)l * OS_LAMW;
     const size_t ks = s.vdir ? (size_t)s.n_lines : 1;
-    if (threadIdx.x < 18 && !s.spline) {             // a_j(t) = t prod_{m=1..j} (m^2 - t^2) / (2m (2m+1))
-        const int half = threadIdx.x / 9, j = threadIdx.x - 9 * half;
-        const double tt = half == 0 ? 1.0 - t : t;
-        double a = tt;
-        constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
-                                   1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
+    // fp64 for everything that is per line (beta, b, b*, the Everett / B-spline coefficients); the 129 table
+    // entries are then evaluated in fp32 from those coefficients (rounded once) and from (cos, sin, 2 - 2 cos)
+    // rounded from the fp64 table: ~1e-7 relative, the same as the whole-line kernels' in-kernel symbol.
+    __shared__ float af[2][9];
+    __shared__ float bs[4];
+    if (!s.spline) {
+        if (threadIdx.x < 18) {                      // a_j(t) = t prod_{m=1..j} (m^2 - t^2) / (2m (2m+1))
+            const int half = threadIdx.x / 9, j = threadIdx.x - 9 * half;
+            const double tt = half == 0 ? 1.0 - t : t;
+            double a = tt;
+            constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
+                                       1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
 #pragma unroll
-        for (int m = 1; m <= 8; ++m)
-            if (m <= j) a = a * ((double)(m * m) - tt * tt) * rcp[m];
-        acoef[half][j] = j <= s.d ? a : 0.0;
+            for (int m = 1; m <= 8; ++m)
+                if (m <= j) a = a * ((double)(m * m) - tt * tt) * rcp[m];
+            af[half][j] = j <= s.d ? (float)a : 0.0f;
+        }
+    } else if (threadIdx.x == 0) {
+        const double u = 1.0 - t;
+        bs[0] = (float)(u * u * u / 6.0);
+        bs[1] = (float)((4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0);
+        bs[2] = (float)((1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0);
+        bs[3] = (float)(t * t * t / 6.0);
     }
     __syncthreads();
-    const double sc = 1.0 / (2.0 * (double)OS_LB);
+    const float sc = 1.0f / (2.0f * (float)OS_LB);   // a power of two: exact
     // 128 threads: k = threadIdx.x, and threads 0 and 1 also write entries 128 and 129 (16 CTAs per SM)
     for (int k = threadIdx.x; k < OS_LAMW; k += 128) {
         if (k == 129) { out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : b4), sshift); continue; }
-        if (k == 0) { out[0] = make_float2((float)sc, 0.0f); continue; }   // lambda_0 = sum of the weights = 1
+        if (k == 0) { out[0] = make_float2(sc, 0.0f); continue; }   // lambda_0 = sum of the weights = 1
         const double2 cs = s.cs64[k];                  // (cos, sin)(2 pi k / OS_LB), fp64 table
-        const double c = cs.x, sn = cs.y;
-        double lr, li;
+        const float c = (float)cs.x, sn = (float)cs.y;
+        float lr, li;
         if (s.spline) {
-            const double u = 1.0 - t;
-            const double Bm1 = u * u * u / 6.0, B0 = (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0;
-            const double B1 = (1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0, B2 = t * t * t / 6.0;
-            const double c2 = 2.0 * c * c - 1.0, s2 = 2.0 * sn * c;
-            const double g = 3.0 / (2.0 + c);
-            lr = (B0 + (Bm1 + B1) * c + B2 * c2) * g;
-            li = ((B1 - Bm1) * sn + B2 * s2) * g;
+            const float Bm1 = bs[0], B0 = bs[1], B1 = bs[2], B2 = bs[3];
+            const float c2 = (float)(2.0 * cs.x * cs.x - 1.0), s2 = (float)(2.0 * cs.y * cs.x);
+            const float g = 3.0f / (2.0f + c);
+            lr = fmaf(B2, c2, fmaf(Bm1 + B1, c, B0)) * g;
+            li = fmaf(B2, s2, (B1 - Bm1) * sn) * g;
         } else {
-            const double sv = 2.0 - 2.0 * c;
-            double p0 = 0.0, p1 = 0.0;
+            const float sv = (float)(2.0 - 2.0 * cs.x);
+            float p0 = 0.0f, p1 = 0.0f;
 #pragma unroll
             for (int j = 8; j >= 0; --j) {             // coefficients beyond the degree are zero
-                p0 = p0 * sv + acoef[0][j];
-                p1 = p1 * sv + acoef[1][j];
+                p0 = fmaf(p0, sv, af[0][j]);
+                p1 = fmaf(p1, sv, af[1][j]);
             }
-            lr = p0 + c * p1;
+            lr = fmaf(c, p1, p0);
             li = sn * p1;
         }
         if (br) {
             const double2 r = s.cs64[(k * br) & (OS_LB - 1)];
-            const double xr = lr * r.x - li * r.y, xi = lr * r.y + li * r.x;
+            const float rx = (float)r.x, ry = (float)r.y;
+            const float xr = fmaf(lr, rx, -li * ry), xi = fmaf(lr, ry, li * rx);
             lr = xr; li = xi;
         }
-        out[k * ks] = make_float2((float)(lr * sc), (float)(li * sc));
+        out[k * ks] = make_float2(lr * sc, li * sc);
     }
 }
 

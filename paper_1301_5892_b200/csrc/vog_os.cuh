@@ -10,8 +10,9 @@
 // <= 2e-9 max|u| (spline: the neglected tail of the row, far below fp32 rounding) the samples
 // of A u, the H = 16 on either side are discarded.  Compared with one length-N transform per line:
 //   * 8 instead of log2(N) butterfly levels, two passes instead of three, no big twiddle table;
-//   * the symbol is a per-line table lam[k], k = 0..128, computed in fp64 by the setup kernel and shared
-//     by all blocks of the line -- no polynomial evaluation in the hot loop;
+//   * the symbol is a per-line table lam[k], k = 0..128, written by the setup kernel (shift split and
+//     interpolation coefficients in fp64, the 129 entries in fp32) and shared by all blocks of the line --
+//     no polynomial evaluation in the hot loop;
 //   * the integer part b of the shift is folded into the load address ("integer roll by
 //     index"): no rotation factor at all (x keeps a residual br in {-2..1} in the table to stay 128-bit aligned);
 //   * the working set of a block is 1 KB per line, so the strided (v) direction can use strips 32 columns
