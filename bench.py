@@ -304,7 +304,30 @@ def sweep(torch, vog, stream, peak, sizes=(2048, 8192), kinds=((0, 17), (0, 3), 
                 gbs = 8.0 * N * N / (med * 1e-3) / 1e9
                 row[name] = {"ms_median": med, "ms_best": min(times), "GBps": gbs, "frac_hbm_measured": gbs / peak,
                              "frac_hbm_8TBps": gbs / 8000.0}
-            row["note"] = "vog_shift_x/v calls: fp64 table setup + kernel (+ copy back for v, whose kernel is out of place)"
+            row["note"] = "vog_shift_x/v calls: table setup + kernel (+ copy back for v, whose kernel is out of place)"
+            # the x kernel alone (vog_advect_x caches its tables per dt) and a whole Strang step (in which the
+            # v kernel writes the plan's second grid and no copy is made), on the same grid
+            for _ in range(3):
+                plan.advect_x(f, 0.01)
+            times = []
+            for _ in range(10):
+                e0.record(stream); plan.advect_x(f, 0.01); e1.record(stream)
+                stream.synchronize()
+                times.append(e0.elapsed_time(e1))
+            med = float(np.median(times))
+            gbs = 8.0 * N * N / (med * 1e-3) / 1e9
+            row["x_kernel_only"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak}
+            for _ in range(2):
+                plan.step(f, 1e-3)
+            times = []
+            for _ in range(5):
+                e0.record(stream); plan.step(f, 1e-3); e1.record(stream)
+                stream.synchronize()
+                times.append(e0.elapsed_time(e1))
+            med = float(np.median(times))
+            gbs = 28.0 * N * N / (med * 1e-3) / 1e9     # 3 advections x 8 B + 4 B density read per cell
+            row["strang_step"] = {"ms_median": med, "cell_updates_per_s": N * N / (med * 1e-3), "GBps_28B_per_cell": gbs,
+                                  "frac_hbm_measured": gbs / peak}
             res.append(row)
             plan.destroy()
         del f
