@@ -39,17 +39,18 @@ __host__ __device__ constexpr int ilog2(int n) { int l = 0; while ((1 << l) < n)
 __device__ __forceinline__ float fneg(float x) { return __int_as_float(__float_as_int(x) ^ 0x80000000); }  // ALU pipe
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
-// a * b = a.x (b.x, b.y) + a.y (-b.y, b.x)
+// a * b = a b.x + i (a b.y):  FMUL2 by the broadcast scalar b.y, then FFMA2 by the broadcast scalar b.x with the
+// product swapped and half-negated as an operand modifier (-R.F32x2.LO_HI.NP): two instructions, no moves.
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 {
-    const float2 t = __fmul2_rn(make_float2(a.y, a.y), make_float2(fneg(b.y), b.x));
-    return __ffma2_rn(make_float2(a.x, a.x), b, t);
+    const float2 t = __fmul2_rn(a, make_float2(b.y, b.y));
+    return __ffma2_rn(a, make_float2(b.x, b.x), make_float2(-t.y, t.x));
 }
-// a * conj(b) = a.x (b.x, -b.y) + a.y (b.y, b.x)
+// a * conj(b) = a b.x - i (a b.y)
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b)
 {
-    const float2 t = __fmul2_rn(make_float2(a.y, a.y), make_float2(b.y, b.x));
-    return __ffma2_rn(make_float2(a.x, a.x), make_float2(b.x, fneg(b.y)), t);
+    const float2 t = __fmul2_rn(a, make_float2(b.y, b.y));
+    return __ffma2_rn(a, make_float2(b.x, b.x), make_float2(t.y, -t.x));
 }
 
 // multiply by the compile-time root e^{-/+ 2 pi i K / R} (forward: minus; INV: plus)
@@ -64,9 +65,10 @@ __device__ __forceinline__ float2 mul_root(float2 d)
     else {
         constexpr float c = (float)cos32(k32);
         constexpr float s = INV ? (float)sin32(k32) : -(float)sin32(k32);
-        // (d.x c - d.y s, d.x s + d.y c)
-        const float2 t = __fmul2_rn(make_float2(d.y, d.y), make_float2(-s, c));
-        return __ffma2_rn(make_float2(d.x, d.x), make_float2(c, s), t);
+        // d (c + i s) = d c + i (d s): both constants are broadcast immediates, the swap and the half negation
+        // of the first product are operand modifiers of the FFMA2 -- two instructions, no constant pairs to build
+        const float2 t = __fmul2_rn(d, make_float2(s, s));
+        return __ffma2_rn(d, make_float2(c, c), make_float2(-t.y, t.x));
     }
 }
 

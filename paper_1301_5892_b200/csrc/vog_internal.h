@@ -79,11 +79,15 @@ struct OsArgs {
     float cg[4];
     const float* cg4;      // the same four constants in device memory (dynamic indexing)
     float dvf;             // v: dv as float (row stride of the delta-f source recurrence)
+    int np;                // second-generation kernels (vog_os2.cuh): pairs of blocks per line = ceil(nb / 2)
+    unsigned inv_np;       // x: ceil(2^16 / np)
+    int n_lines;           // x: number of lines (the last line group may be ragged)
 };
 
 struct OsSetupArgs {
     int n_lines, N, mode;      // mode 0: c = v_l; 1: c = E_l (+E_ext_l); 2: explicit beta
     int spline, d, vdir;
+    int gen2;                  // tables for vog_os2.cuh: scale 1/OS_LB, full integer shift b in entry 129 (no residue)
     double dt, delta, vmin, dv;
     const float* E;
     const float* Eext;
@@ -96,6 +100,12 @@ cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st);
 cudaError_t osx_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
 int osx_occupancy(int threads, size_t smem);
+cudaError_t osx2_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
+int osx2_occupancy(int threads, size_t smem);
+cudaError_t osx3_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
+int osx3_occupancy(int threads, size_t smem);
+cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
 
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
 typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,

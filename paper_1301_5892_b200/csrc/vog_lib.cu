@@ -340,6 +340,10 @@ struct vog_plan_s {
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int osx_lpi, osx_thr, osx_cps, osx_occ;
     int osv_np_log, osv_thr, osv_rb, osv_gpc;
+    int os_gen;                            // 2 = pair kernels of vog_os2.cuh (default), 1 = even/odd kernels of vog_os.cuh
+    int os2x_lpi, os2x_thr, os2x_occ, os2v_gpc;
+    int os2v_direct;                       // v: register-landing kernel osv3_kernel (measured slower than osv2_kernel: off)
+    int os2x_direct, os3x_occ;             // x: register-landing kernel (osx3_kernel) when a line group fits one round of 320 threads
     int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
     float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
     double* part;               // density partials [nby][Nx]
@@ -537,6 +541,16 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         while (lpi > 1 && Nv / lpi < P->n_sm * 3) lpi >>= 1;
         P->osx_lpi = lpi; P->osx_thr = 128; P->osx_cps = 0; P->osx_occ = 0;
         P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 0; P->osv_gpc = 0;
+        // pair kernels: 16 items per pair and phase; lines per iteration so that one round of <= 320 threads
+        // covers the items (8192: 19 pairs = 304 items; 2048: 4 lines x 5 pairs = 320)
+        const int npx = (nbx + 1) / 2;
+        int l2 = 320 / (16 * npx);
+        if (l2 < 1) l2 = 1;
+        while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
+        int thr = ((16 * npx * l2 + 31) / 32) * 32;
+        if (thr > 320) thr = 320;
+        P->os2x_direct = 1; P->os3x_occ = 0; P->os2v_direct = 0;
+        P->os_gen = 2; P->os2x_lpi = l2; P->os2x_thr = thr; P->os2x_occ = 0; P->os2v_gpc = 0;
     }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
@@ -616,7 +630,8 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->part, sizeof(double) * nby * Nx);
     alloc((void**)&P->rho, sizeof(double) * Nx);
     alloc((void**)&P->E_self, sizeof(float) * Nx);
-    alloc((void**)&P->feq_tab, sizeof(float) * (ng ? ng : 1) * Nv);
+    alloc((void**)&P->feq_tab, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512));   // + padding read (not used) by osv2_kernel
+    if (e == cudaSuccess) e = cudaMemsetAsync(P->feq_tab, 0, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512), P->st);
     alloc((void**)&P->vmu_tab, sizeof(float) * (ng ? ng : 1) * Nv);
     if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
     e = cudaMemcpyAsync(P->os_twx, otx.data(), sizeof(float2) * otx.size(), cudaMemcpyHostToDevice, P->st);
@@ -666,6 +681,7 @@ extern "C" int vog_destroy(vog_plan_t P)
 
 static size_t osx_smem_bytes(int lpi, int nb);
 static size_t osv_smem_bytes(int np_log, int rb);
+static size_t osx2_smem_bytes(int lpi, int np);
 
 // internal tuning hook (documented in DESIGN.md; not part of the paper-facing API):
 // which: 0 = log2(NL) x, 1 = threads x, 2 = log2(NL) v, 3 = threads v, 4 = density row blocks
@@ -689,6 +705,13 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 14: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->osv_thr = value; break;
         case 15: if (value < 0 || value > 2) return VOG_EINVAL; P->osv_rb = value; break;
         case 16: if (value < 0) return VOG_EINVAL; P->osv_gpc = value; break;
+        case 17: if (value < 1 || value > 2) return VOG_EINVAL; P->os_gen = value; P->recx_valid = false; break;
+        case 18: if (value < 1 || value > Nv || osx2_smem_bytes(value, ((Nx + OS_V - 1) / OS_V + 1) / 2) > 227 * 1024) return VOG_EINVAL;
+                 P->os2x_lpi = value; P->os2x_occ = 0; P->os3x_occ = 0; break;
+        case 19: if (value < 32 || value > 320 || value % 32) return VOG_EINVAL; P->os2x_thr = value; P->os2x_occ = 0; break;
+        case 20: if (value < 0) return VOG_EINVAL; P->os2v_gpc = value; break;
+        case 21: if (value < 0 || value > 1) return VOG_EINVAL; P->os2x_direct = value; break;
+        case 22: if (value < 0 || value > 1) return VOG_EINVAL; P->os2v_direct = value; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -710,6 +733,7 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
         s.spline = P->sym == SYM_SPLINE3;
         s.d = P->d;
         s.vdir = vdir ? 1 : 0;
+        s.gen2 = P->os_gen == 2 ? 1 : 0;
         s.dt = dt; s.dv = dv;
         s.delta = vdir ? dv : P->p.L / (double)Nx;
         s.vmin = P->p.vmin;
@@ -762,6 +786,80 @@ static cudaError_t run_osx(vog_plan_s* P, const float* src, float* dst)
     if (grid > a.n_groups) grid = a.n_groups;
     P->launches++;
     return osx_launch(a, grid, P->osx_thr, smem, P->st);
+}
+
+// ---- pair kernels (vog_os2.cuh)
+static size_t osx2_smem_bytes(int lpi, int np)
+{
+    return (size_t)lpi * np * (16 * 17 * 8) + (size_t)lpi * OS_LAMW * 8 + 240 * 8;
+}
+
+static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
+{
+    OsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nx;
+    a.nb = (Nx + OS_V - 1) / OS_V;
+    a.np = (a.nb + 1) / 2;
+    a.inv_np = (65536u + (unsigned)a.np - 1u) / (unsigned)a.np;
+    a.lam = P->os_lam_x; a.tw = P->os_twv;
+    a.lpi = P->os2x_lpi;
+    a.n_lines = Nv;
+    a.n_groups = (Nv + a.lpi - 1) / a.lpi;
+    const size_t smem = osx2_smem_bytes(a.lpi, a.np);
+    if (P->os2x_direct && 16 * a.np * a.lpi <= 320) {
+        const int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
+        if (P->os3x_occ == 0) {
+            P->os3x_occ = osx3_occupancy(thr, smem);
+            if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
+        }
+        int grid = P->os3x_occ * P->n_sm;
+        if (grid > a.n_groups) grid = a.n_groups;
+        P->launches++;
+        return osx3_launch(a, grid, thr, smem, P->st);
+    }
+    if (P->os2x_occ == 0) {
+        P->os2x_occ = osx2_occupancy(P->os2x_thr, smem);
+        if (P->os2x_occ <= 0) return cudaErrorInvalidConfiguration;
+    }
+    int grid = P->os2x_occ * P->n_sm;
+    if (grid > a.n_groups) grid = a.n_groups;
+    P->launches++;
+    return osx2_launch(a, grid, P->os2x_thr, smem, P->st);
+}
+
+static cudaError_t run_osv2(vog_plan_s* P, const float* src, float* dst, bool source)
+{
+    OsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
+    a.nb = (Nv + OS_V - 1) / OS_V;
+    a.np = (a.nb + 1) / 2;
+    a.lam = P->os_lam_v; a.tw = P->os_twv;
+    a.ng = source ? P->p.feq.n : 0;
+    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
+    a.dvf = (float)((P->p.vmax - P->p.vmin) / (double)Nv);
+    const int strips = Nx / 32;
+    // pairs per CTA: minimise waves x pairs per CTA (2 CTAs of 512 threads per SM); ties go to the longer loop
+    // (fewer reloads of the strip's symbol tables)
+    int gpc = P->os2v_gpc;
+    if (gpc <= 0) {
+        long long best = -1;
+        const long long slots = (long long)P->n_sm * 2;
+        for (int gp = 1; gp <= a.np; ++gp) {
+            const long long ctas = (long long)strips * ((a.np + gp - 1) / gp);
+            const long long cost = ((ctas + slots - 1) / slots) * (gp * 8 + 1);      // +1: table load
+            if (best < 0 || cost <= best) { best = cost; gpc = gp; }
+        }
+    }
+    if (gpc > a.np) gpc = a.np;
+    a.gpc = gpc;
+    dim3 grid(strips, (a.np + gpc - 1) / gpc);
+    P->launches++;
+    if (P->os2v_direct) return osv3_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 4 * 32 * 16, P->st);
+    return osv2_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
 }
 
 static size_t osv_smem_bytes(int np_log, int rb)
@@ -875,7 +973,7 @@ static cudaError_t copy_grid(vog_plan_s* P, float* dst, const float* src)
 // x-advection src -> dst (dst may equal src); the shift records/tables must be current
 static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
 {
-    if (P->os_x) return run_osx(P, src, dst);
+    if (P->os_x) return P->os_gen == 2 ? run_osx2(P, src, dst) : run_osx(P, src, dst);
     cudaError_t e = cudaSuccess;
     if (src != dst) e = copy_grid(P, dst, src);
     if (e == cudaSuccess) e = run_advect_line(P, dst, false, false);
@@ -885,7 +983,7 @@ static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
 // v-advection src -> dst; the overlap-save kernel needs dst != src, the whole-line kernel works in place
 static cudaError_t advect_v(vog_plan_s* P, const float* src, float* dst, bool source)
 {
-    if (P->os_v) return src == dst ? cudaErrorInvalidValue : run_osv(P, src, dst, source);
+    if (P->os_v) return src == dst ? cudaErrorInvalidValue : (P->os_gen == 2 ? run_osv2(P, src, dst, source) : run_osv(P, src, dst, source));
     cudaError_t e = cudaSuccess;
     if (src != dst) e = copy_grid(P, dst, src);
     if (e == cudaSuccess) e = run_advect_line(P, dst, true, source);
@@ -897,7 +995,7 @@ static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
 {
     if (!P->os_v) return run_advect_line(P, f, true, source);
     cudaError_t e = ensure_gbuf(P);
-    if (e == cudaSuccess) e = run_osv(P, f, P->g_buf, source);
+    if (e == cudaSuccess) e = P->os_gen == 2 ? run_osv2(P, f, P->g_buf, source) : run_osv(P, f, P->g_buf, source);
     if (e == cudaSuccess) e = copy_grid(P, f, P->g_buf);
     return e;
 }

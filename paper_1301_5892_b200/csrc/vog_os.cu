@@ -1,6 +1,7 @@
 // vog_os.cu -- overlap-save advection kernels: instantiation, launchers and the setup kernel that
 // tabulates the symbol lambda(theta_k) per line (S1 + the closed form of S4).  Product code.
 #include "vog_os.cuh"
+#include "vog_os2.cuh"
 
 namespace vog {
 
@@ -36,8 +37,9 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
     }
     // x keeps 16-byte aligned loads: b = 4 b4 + br with br in {-2,..,1} (centred, so that the stencil shifted by
     // br has the same room, >= 14 cells, on both sides of the kept samples); br goes into the table as e^{i theta br}
+    const bool whole_b = s.vdir || s.gen2;       // the integer shift goes entirely into the load address
     const int b4 = ((b + 2) >> 2) & ((s.N >> 2) - 1);
-    const int br = s.vdir ? 0 : b - 4 * ((b + 2) >> 2);
+    const int br = whole_b ? 0 : b - 4 * ((b + 2) >> 2);
     // x: [line][k]; v: transposed [k][line] so that a strip of 32 columns reads 256-byte rows
     float2* out = s.vdir ? s.lam + l : s.lam + (size_t)l * OS_LAMW;
     const size_t ks = s.vdir ? (size_t)s.n_lines : 1;
@@ -66,10 +68,11 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
         bs[3] = (float)(t * t * t / 6.0);
     }
     __syncthreads();
-    const float sc = 1.0f / (2.0f * (float)OS_LB);   // a power of two: exact
+    // a power of two: exact.  Even/odd packing (vog_os.cuh) carries a factor 2 from the untangle stage.
+    const float sc = s.gen2 ? 1.0f / (float)OS_LB : 1.0f / (2.0f * (float)OS_LB);
     // 128 threads: k = threadIdx.x, and threads 0 and 1 also write entries 128 and 129 (16 CTAs per SM)
     for (int k = threadIdx.x; k < OS_LAMW; k += 128) {
-        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(s.vdir ? b : b4), sshift); continue; }
+        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(whole_b ? b : b4), sshift); continue; }
         if (k == 0) { out[0] = make_float2(sc, 0.0f); continue; }   // lambda_0 = sum of the weights = 1
         const double2 cs = s.cs64[k];                  // (cos, sin)(2 pi k / OS_LB), fp64 table
         const float c = (float)cs.x, sn = (float)cs.y;
@@ -133,6 +136,77 @@ cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cud
     if (e != cudaSuccess) return e;
     osv_kernel<<<grid, threads, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+cudaError_t osx2_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    static size_t cur2 = 0;
+    if (threads <= 160) {
+        cudaError_t e = set_smem((const void*)osx2_kernel<160, 5>, smem, &cur);
+        if (e != cudaSuccess) return e;
+        osx2_kernel<160, 5><<<grid, threads, smem, st>>>(a);
+    } else {
+        cudaError_t e = set_smem((const void*)osx2_kernel<320, 3>, smem, &cur2);
+        if (e != cudaSuccess) return e;
+        osx2_kernel<320, 3><<<grid, threads, smem, st>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    cudaError_t e = set_smem((const void*)osv2_kernel, smem, &cur);
+    if (e != cudaSuccess) return e;
+    osv2_kernel<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    cudaError_t e = set_smem((const void*)osv3_kernel, smem, &cur);
+    if (e != cudaSuccess) return e;
+    osv3_kernel<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t osx3_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    cudaError_t e = set_smem((const void*)osx3_kernel, smem, &cur);
+    if (e != cudaSuccess) return e;
+    osx3_kernel<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+int osx3_occupancy(int threads, size_t smem)
+{
+    static size_t cur = 0;
+    if (set_smem((const void*)osx3_kernel, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx3_kernel, threads, smem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return nb;
+}
+
+int osx2_occupancy(int threads, size_t smem)
+{
+    static size_t cur = 0, cur2 = 0;
+    const void* fn = threads <= 160 ? (const void*)osx2_kernel<160, 5> : (const void*)osx2_kernel<320, 3>;
+    if (set_smem(fn, smem, threads <= 160 ? &cur : &cur2) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int nb = 0;
+    const cudaError_t eo = threads <= 160
+        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx2_kernel<160, 5>, threads, smem)
+        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx2_kernel<320, 3>, threads, smem);
+    if (eo != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return nb;
 }
 
 int osx_occupancy(int threads, size_t smem)

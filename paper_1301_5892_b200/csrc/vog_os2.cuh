@@ -1,0 +1,642 @@
+// vog_os2.cuh -- overlap-save advection kernels, second generation (line length N >= 1024;
+// SURVEY.md 8(a) S2-S7).  Product code; shares nothing with oracle/.
+//
+// Same method as vog_os.cuh (the circulant product of P:98-100 taken block-wise in Fourier space, P:131-149:
+// blocks of LB = 256 samples of the rolled line, V = 224 kept, H = 16 discarded on either side), but the
+// real-data trick is different.  The interpolation matrix is REAL, so two blocks A, B of the SAME line share
+// the symbol lambda and can ride one complex transform:  z_n = A_n + i B_n,  Z = FFT_256(z),
+// Z_k *= lambda_k (lambda_{256-k} = conj lambda_k),  z' = IFFT(Z)  =>  A' = Re z', B' = Im z'.
+// Compared with the even/odd packing of vog_os.cuh there is no untangle / re-tangle stage, no "special"
+// mirror item, no divergence, and a work item is ONE radix-16 butterfly (16 complex = 32 registers) in every
+// phase, so the kernels fit 64 registers and run at twice the occupancy:
+//   pass A   : item (pair, t):  n = t + 16 k  -> radix 16 over k, times W_256^{t k1}, stored at [k1][t]
+//   middle   : item (pair, g = k1): radix 16 over t -> Z_{g + 16 k2}; times lambda; inverse radix 16
+//   inverse A: item (pair, j): times conj W, inverse radix 16 over k1 -> z'_{j + 16 m}; m = 1..14 are the
+//              kept samples of both blocks (uniform over the threads), stored straight to global memory.
+// Every phase has 16 items per pair, every item touches only its own 16 scratch slots, and a thread lands
+// (cp.async, 4 bytes: the full integer shift b of P:107 is applied by addressing, no alignment residue) exactly
+// the samples that it transforms in pass A.
+#pragma once
+#include "vog_fft.cuh"
+#include "vog_internal.h"
+
+namespace vog {
+
+namespace os2 {
+constexpr int PW = 2 * OS_V;           // cells advanced by one pair of blocks (448)
+
+__device__ __forceinline__ void cp_async4(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
+}
+
+// middle stage on 16 registers: x[j] = Y[g][j] -> Z_{g+16 q} at x[brev q] -> times lambda -> inverse over q.
+// lam(k) returns lambda_k / 256 for k = 0..128 (the tabulated half); LS = stride of the table in float2.
+template <int LS>
+__device__ __forceinline__ void mid16(float2* x, const float2* __restrict__ lam, const int g)
+{
+    dft_dif<16, 1>(x);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) x[brev(q, 16)] = cmul(x[brev(q, 16)], lam[(g + 16 * q) * LS]);
+#pragma unroll
+    for (int q = 8; q < 16; ++q) x[brev(q, 16)] = cmulc(x[brev(q, 16)], lam[(256 - 16 * q - g) * LS]);
+    idft_dit<16, 1>(x);
+}
+}  // namespace os2
+
+// ---------------------------------------------------------------------------------------------
+// x-direction.  Scratch: 16 rows of 17 float2 per pair (2176 B): position p = 16 g + j sits at 17 g + j.
+// All shared accesses are 8 bytes wide; passes A (16 lanes = 16 adjacent j of one row) and the middle stage
+// (16 lanes = 16 rows, same j: bank pairs 2 g + 2 j mod 32) are bank-conflict free, and every address is
+// "item base + compile-time constant" (no swizzle arithmetic, nothing to keep in registers).
+// Persistent CTAs own whole lines (in place: all loads of a line group complete before the barrier that
+// precedes its first store).
+namespace os2 {
+constexpr int XROW = 17;               // float2 per scratch row
+constexpr int XPAIR = 16 * XROW;       // float2 per pair
+}
+
+__device__ __forceinline__ void osx2_land(float2* __restrict__ s, const float* __restrict__ gl, const int c0,
+                                          const int mask)
+{
+    float* const sf = reinterpret_cast<float*>(s);
+    if (c0 + OS_V + 241 <= mask + 1) {                 // the two windows do not wrap
+        const float* p = gl + c0;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            os2::cp_async4(sf + 2 * os2::XROW * k, p + 16 * k);
+            os2::cp_async4(sf + 2 * os2::XROW * k + 1, p + 16 * k + OS_V);
+        }
+    } else {
+#pragma unroll 2
+        for (int k = 0; k < 16; ++k) {
+            os2::cp_async4(sf + 2 * os2::XROW * k, gl + ((c0 + 16 * k) & mask));
+            os2::cp_async4(sf + 2 * os2::XROW * k + 1, gl + ((c0 + 16 * k + OS_V) & mask));
+        }
+    }
+}
+
+// s = pair base + t; tw = table + t
+__device__ __forceinline__ void osx2_fwd(float2* __restrict__ s, const float2* __restrict__ tw)
+{
+    float2 x[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) x[k] = s[os2::XROW * k];
+    dft_dif<16, 1>(x);
+    s[0] = x[0];
+#pragma unroll
+    for (int q = 1; q < 16; ++q) s[os2::XROW * q] = cmul(x[brev(q, 16)], tw[(q - 1) * 16]);
+}
+
+// s = pair base + 17 g
+__device__ __forceinline__ void osx2_mid(float2* __restrict__ s, const int g, const float2* __restrict__ lam)
+{
+    float2 x[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) x[j] = s[j];
+    os2::mid16<1>(x, lam, g);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) s[j] = x[j];
+}
+
+// inverse pass A of item (pair, j): kept samples m = 1..14 of block A (real parts) and block B (imaginary
+// parts) go to cells o0 + 16 (m - 1) and o0 + OS_V + 16 (m - 1) of the line; cells >= N do not exist.
+// s = pair base + j; tw = table + j
+__device__ __forceinline__ void osx2_inv(float* __restrict__ gl, const int o0, const bool full, const int N,
+                                         const float2* __restrict__ s, const float2* __restrict__ tw)
+{
+    float2 x[16];
+    x[0] = s[0];
+#pragma unroll
+    for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(s[os2::XROW * q], tw[(q - 1) * 16]);
+    idft_dit<16, 1>(x);
+    float* const o = gl + o0;
+    if (full) {
+#pragma unroll
+        for (int m = 1; m < 15; ++m) {
+            __stcs(o + 16 * (m - 1), x[m].x);
+            __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
+        }
+    } else {
+#pragma unroll
+        for (int m = 1; m < 15; ++m) {
+            if (o0 + 16 * (m - 1) < N) __stcs(o + 16 * (m - 1), x[m].x);
+            if (o0 + 16 * (m - 1) + OS_V < N) __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
+        }
+    }
+}
+
+// One iteration = lpi whole lines = lpi * np pairs = 16 lpi np items per phase; blockDim.x is a multiple of 16,
+// so the position index t = tid & 15 of a thread is the same for all its items.
+template <int TMAX, int MINB>
+__global__ void __launch_bounds__(TMAX, MINB) osx2_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
+    float2* const lamS = scr + ptot * os2::XPAIR;                       // lpi rows of the symbol table
+    float2* const twS = lamS + lpi * OS_LAMW;                           // 15 * 16
+    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
+    const int N = a.N, mask = N - 1;
+    const unsigned inv_np = a.inv_np;       // ceil(2^16 / np): pr / np == (pr * inv_np) >> 16 for pr < 2^12
+
+    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
+
+    // landing of item w of the line group that starts at line0, and of the group's table rows
+    auto land = [&](const int w, const int line0) {
+        const int pr = w >> 4;
+        const int l = (int)(((unsigned)pr * inv_np) >> 16), pp = pr - l * np;
+        const int line = line0 + l;
+        if (line >= a.n_lines) return;
+        const int b = __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x));
+        osx2_land(scr + pr * os2::XPAIR + t, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+    };
+    auto land_tab = [&](const int line0) {
+        const int nl = min(lpi, a.n_lines - line0);
+        const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
+        float4* dst4 = reinterpret_cast<float4*>(lamS);
+        for (int i = tid; i < nl * (OS_LAMW / 2); i += T) os2::cp_async16(dst4 + i, src4 + i);
+    };
+    if ((int)blockIdx.x < a.n_groups) {
+        for (int w = tid; w < nitem; w += T) land(w, blockIdx.x * lpi);
+        land_tab(blockIdx.x * lpi);
+    }
+    __syncthreads();                               // twS visible
+    for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
+        const int line0 = g * lpi;
+        os2::cp_async_wait_all();                  // this thread's samples (and table chunks) have landed
+        // ---- pass A: every thread on the slots it landed itself
+#pragma unroll 1
+        for (int w = tid; w < nitem; w += T) {
+            int tt = t;
+            asm volatile("" : "+r"(tt));           // keep the 15 twiddle loads inside the loop (30 registers)
+            osx2_fwd(scr + (w >> 4) * os2::XPAIR + t, twS + tt);
+        }
+        __syncthreads();
+        // ---- middle stage
+#pragma unroll 1
+        for (int w = tid; w < nitem; w += T) {
+            const int pr = w >> 4;
+            const int l = (int)(((unsigned)pr * inv_np) >> 16);
+            osx2_mid(scr + pr * os2::XPAIR + os2::XROW * t, t, lamS + l * OS_LAMW);
+        }
+        __syncthreads();
+        // ---- inverse pass A: scratch -> registers -> global; the same item of the NEXT line group lands in
+        // the slots just read.  In place this is safe: every load of THIS group completed before the
+        // barrier after pass A, and the next group is other lines (owned by this CTA).
+        const int gn = g + gridDim.x;
+        if (gn < a.n_groups) land_tab(gn * lpi);   // lamS was last read before the barrier above
+#pragma unroll 1
+        for (int w = tid; w < nitem; w += T) {
+            const int pr = w >> 4;
+            const int l = (int)(((unsigned)pr * inv_np) >> 16), pp = pr - l * np;
+            int tt = t;
+            asm volatile("" : "+r"(tt));
+            const float2* twp = twS + tt;
+            if (line0 + l < a.n_lines)
+                osx2_inv(a.dst + (size_t)(line0 + l) * N, pp * os2::PW + t, (pp + 1) * os2::PW <= N, N,
+                         scr + pr * os2::XPAIR + t, twp);
+            if (gn < a.n_groups) land(w, gn * lpi);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// x-direction, register-landing variant (lines with at most 20 pairs, i.e. N <= 8192): one item per thread and
+// phase (16 lpi np <= blockDim.x).  The 32 samples of a thread's pass-A item are loaded straight into the
+// butterfly registers (coalesced 4-byte loads, 64-byte runs per half-warp) at the END of the previous
+// iteration, so the scratch is only the exchange buffer between the phases (4 instead of 6 shared accesses
+// per sample), and the 15 twiddles W^{t q} of a thread (t is fixed) are products of 4 register-resident
+// powers W^t, W^2t, W^4t, W^8t instead of 15 shared loads per pass.
+struct Tw4 { float2 b1, b2, b4, b8; };
+
+// Calls f(q, W^{t q}) for q = 1..15 (q a compile-time constant of each call), building the powers from the four
+// binary ones (at most 3 chained roundings) in an order that keeps at most two temporaries alive.
+template <int Q> struct QC { static constexpr int value = Q; };
+template <class F>
+__device__ __forceinline__ void os2_tw_each(const Tw4& w, F&& f)
+{
+    f(QC<1>(), w.b1); f(QC<2>(), w.b2); f(QC<4>(), w.b4); f(QC<8>(), w.b8);
+    {
+        const float2 y3 = cmul(w.b1, w.b2);
+        f(QC<3>(), y3);
+        f(QC<11>(), cmul(y3, w.b8));
+        const float2 y7 = cmul(y3, w.b4);
+        f(QC<7>(), y7);
+        f(QC<15>(), cmul(y7, w.b8));
+    }
+    {
+        const float2 y5 = cmul(w.b1, w.b4);
+        f(QC<5>(), y5);
+        f(QC<13>(), cmul(y5, w.b8));
+    }
+    {
+        const float2 y6 = cmul(w.b2, w.b4);
+        f(QC<6>(), y6);
+        f(QC<14>(), cmul(y6, w.b8));
+    }
+    f(QC<9>(), cmul(w.b1, w.b8));
+    f(QC<10>(), cmul(w.b2, w.b8));
+    f(QC<12>(), cmul(w.b4, w.b8));
+}
+
+__device__ __forceinline__ void osx3_load(float2* x, const float* __restrict__ gl, const int c0, const int mask)
+{
+    if (c0 + OS_V + 241 <= mask + 1) {                 // the two windows do not wrap
+        const float* p = gl + c0;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) x[k] = make_float2(__ldg(p + 16 * k), __ldg(p + 16 * k + OS_V));
+    } else {
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+            x[k] = make_float2(__ldg(gl + ((c0 + 16 * k) & mask)), __ldg(gl + ((c0 + 16 * k + OS_V) & mask)));
+    }
+}
+
+__global__ void __launch_bounds__(320, 3) osx3_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
+    float2* const lamS = scr + ptot * os2::XPAIR;                       // lpi rows of the symbol table
+    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
+    const int N = a.N, mask = N - 1;
+    const bool active = tid < nitem;
+    const int pr = tid >> 4;
+    const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
+    Tw4 w;
+    w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
+    w.b2 = __ldg(a.tw + 16 + t);
+    w.b4 = __ldg(a.tw + 3 * 16 + t);
+    w.b8 = __ldg(a.tw + 7 * 16 + t);
+    float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
+    float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
+    const float2* const lamL = lamS + l * OS_LAMW;
+    const int o0 = pp * os2::PW + t;
+    const bool full = (pp + 1) * os2::PW <= N;
+
+    auto land_tab = [&](const int line0) {
+        const int nl = min(lpi, a.n_lines - line0);
+        const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
+        float4* dst4 = reinterpret_cast<float4*>(lamS);
+        for (int i = tid; i < nl * (OS_LAMW / 2); i += T) os2::cp_async16(dst4 + i, src4 + i);
+    };
+    if ((int)blockIdx.x < a.n_groups) land_tab(blockIdx.x * lpi);
+    for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
+        const int line = min(g * lpi + l, a.n_lines - 1);      // (a ragged last group recomputes the last line)
+        // ---- pass A straight from global memory
+        if (active) {
+            float2 x[16];
+            const int b = __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x));
+            osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+            dft_dif<16, 1>(x);
+            sA[0] = x[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
+            });
+        }
+        os2::cp_async_wait_all();                  // table chunks
+        __syncthreads();
+        // ---- middle stage
+        if (active) osx2_mid(sM, t, lamL);
+        __syncthreads();
+        // ---- inverse pass A: scratch -> registers -> global, then the loads of the next line group.  In place
+        // this is safe: every load of THIS group was consumed before the first barrier, and the next group is
+        // other lines (owned by this CTA).
+        const int gn = g + gridDim.x;
+        if (gn < a.n_groups) land_tab(gn * lpi);   // lamS was last read before the barrier above
+        if (active) {
+            float2 x[16];
+            x[0] = sA[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
+            });
+            idft_dit<16, 1>(x);
+            if (g * lpi + l < a.n_lines) {
+                float* const o = a.dst + (size_t)line * N + o0;
+                if (full) {
+#pragma unroll
+                    for (int m = 1; m < 15; ++m) {
+                        __stcs(o + 16 * (m - 1), x[m].x);
+                        __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
+                    }
+                } else {
+#pragma unroll
+                    for (int m = 1; m < 15; ++m) {
+                        if (o0 + 16 * (m - 1) < N) __stcs(o + 16 * (m - 1), x[m].x);
+                        if (o0 + 16 * (m - 1) + OS_V < N) __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// v-direction.  A strip is 32 adjacent columns = the 32 lanes of a warp; every lane advects ITS column, the
+// pair = two consecutive row blocks of that column.  A row of the strip is one 128-byte line: loads and
+// stores are fully coalesced, and a lane applies its own integer shift b_c by addressing.  Scratch is
+// [position][lane] float2 (64 KB per pair): conflict-free with no padding; an item (t, g or j) is one WARP, so
+// a CTA of 16 warps does each phase of a pair in one round.  The symbol tables arrive transposed
+// ([k][column]) and are staged once per CTA; CTAs loop over gpc pairs.  Out of place (src != dst).
+// Landing is planar inside the 256 bytes of a position (32 real parts = block A, then 32 imaginary parts =
+// block B) so that the 4-byte copies of a warp are bank-conflict free; pass A reads the planar words and
+// writes the position back as interleaved float2 (all reads of the warp precede its writes).
+__device__ __forceinline__ void osv2_land(float* __restrict__ pw, const float* __restrict__ col, const int Nx,
+                                          const int vmask, const int r0)
+{
+    constexpr int PS = 16 * 32 * 2;                 // floats between positions t + 16 k and t + 16 (k + 1)
+    const int rr = r0 & vmask;
+    if (rr + OS_V + 241 <= vmask + 1) {             // the two windows do not wrap: constant row stride
+        const float* p = col + (size_t)rr * Nx;
+        const float* q = p + (size_t)OS_V * Nx;
+        const size_t s16 = (size_t)16 * Nx;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            os2::cp_async4(pw + k * PS, p);
+            os2::cp_async4(pw + k * PS + 32, q);
+            p += s16;
+            q += s16;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const int ra = (r0 + 16 * k) & vmask, rb = (r0 + 16 * k + OS_V) & vmask;
+            os2::cp_async4(pw + k * PS, col + (size_t)ra * Nx);
+            os2::cp_async4(pw + k * PS + 32, col + (size_t)rb * Nx);
+        }
+    }
+}
+
+// delta-f source on the kept samples of one item: x[m].x += f_eq,g(v_j)(e^{X_j} - 1) at rows
+// j = row0 + 16 (m - 1), x[m].y the same at rows j + OS_V, with X_j = c s (2 (v_j - mu) - s) affine in j.  Along rows
+// 16 apart expm1 obeys e' = e R + r (R = e^h, r = expm1(h), h = 32 c s dv); the recurrence starts in the
+// middle (m = 8) and runs both ways (RS[g] = (R, r, 1/R, expm1(-h)) per lane), so at most 7 steps accumulate.
+// The f_eq table has 512 floats of padding: rows >= Nv are read but never stored.
+__device__ __forceinline__ void osv2_source(float2* x, const OsArgs& a, const float4* __restrict__ RS, const int lane,
+                                            const int row0, const float ssh)
+{
+#pragma unroll 1
+    for (int g = 0; g < a.ng; ++g) {
+        const float cgs = a.cg4[g] * ssh;
+        const float* __restrict__ fa = a.feq_tab + g * a.Nv + row0;
+        const float u0 = __ldg(a.vmu_tab + g * a.Nv);                          // v_0 - mu_g
+        const float4 Rr = RS[g * 32 + lane];
+        const float ea8 = expm1f(cgs * (2.0f * fmaf((float)(row0 + 112), a.dvf, u0) - ssh));
+        const float eb8 = expm1f(cgs * (2.0f * fmaf((float)(row0 + 112 + OS_V), a.dvf, u0) - ssh));
+        float ea = ea8, eb = eb8;
+#pragma unroll
+        for (int m = 8; m < 15; ++m) {
+            x[m].x = fmaf(__ldg(fa + 16 * (m - 1)), ea, x[m].x);
+            x[m].y = fmaf(__ldg(fa + 16 * (m - 1) + OS_V), eb, x[m].y);
+            ea = fmaf(ea, Rr.x, Rr.y);
+            eb = fmaf(eb, Rr.x, Rr.y);
+        }
+        ea = ea8; eb = eb8;
+#pragma unroll
+        for (int m = 7; m >= 1; --m) {
+            ea = fmaf(ea, Rr.z, Rr.w);
+            eb = fmaf(eb, Rr.z, Rr.w);
+            x[m].x = fmaf(__ldg(fa + 16 * (m - 1)), ea, x[m].x);
+            x[m].y = fmaf(__ldg(fa + 16 * (m - 1) + OS_V), eb, x[m].y);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(512, 2) osv2_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int W = 32;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // 256 * 32
+    float2* const lamS = scr + 256 * W;                                       // 130 * 32, [k][lane]
+    float2* const twS = lamS + OS_LAMW * W;                                   // 15 * 16
+    float4* const RS = reinterpret_cast<float4*>(twS + 240);                  // [4][32] source recurrence constants
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5;   // wid = item index (t, g, j)
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
+    const int c0 = blockIdx.x * W;
+
+    {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
+        const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
+        float4* dst4 = reinterpret_cast<float4*>(lamS);
+        for (int i = tid; i < OS_LAMW * 16; i += T)
+            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
+    }
+    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
+    os2::cp_async_wait_all();
+    __syncthreads();
+    const int b = __float_as_int(lamS[129 * W + lane].x);
+    const float ssh = lamS[129 * W + lane].y;
+    if (a.ng > 0 && tid < 4 * W) {
+        // delta-f source: x_j = c s (2 (v_j - mu) - s) is affine in the row j, so along rows 16 apart
+        // expm1 obeys e' = e R + r with R = exp(h), r = expm1(h), h = 32 c s dv
+        const int g = tid >> 5;
+        const float h = 32.0f * (g < a.ng ? a.cg4[g] : 0.0f) * ssh * a.dvf;
+        RS[g * W + lane] = make_float4(expf(h), expm1f(h), expf(-h), expm1f(-h));
+    }
+    const float* const col = a.src + c0 + lane;
+    float* const ocol = a.dst + c0 + lane;
+    const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
+    float* const pw = reinterpret_cast<float*>(scr + wid * W) + lane;        // planar words of position t = wid
+    float2* const own = scr + wid * W + lane;                                 // the same position, interleaved
+    constexpr int PS2 = 16 * W;                                               // float2 between positions 16 apart
+
+    if (p0 < p1) osv2_land(pw, col, Nx, vmask, p0 * os2::PW - OS_H + b + wid);
+    __syncthreads();                               // RS visible (twS, lamS already are)
+    for (int p = p0; p < p1; ++p) {
+        int wt = wid;
+        asm volatile("" : "+r"(wt));               // keep the twiddle loads inside the loop (30 registers)
+        const float2* const twp = twS + wt;
+        os2::cp_async_wait_all();                  // this thread's samples have landed
+        // ---- pass A (item t = wid)
+        {
+            float2 x[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) x[k] = make_float2(pw[k * PS2 * 2], pw[k * PS2 * 2 + W]);
+            __syncwarp();                          // planar words all read before the interleaved writes
+            dft_dif<16, 1>(x);
+            own[0] = x[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) own[q * PS2] = cmul(x[brev(q, 16)], twp[(q - 1) * 16]);
+        }
+        __syncthreads();
+        // ---- middle stage (item g = wid): positions 16 g + j
+        {
+            float2* const s = scr + wid * 16 * W + lane;
+            float2 x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = s[j * W];
+            os2::mid16<W>(x, lamS + lane, wid);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) s[j * W] = x[j];
+        }
+        __syncthreads();
+        // ---- inverse pass A (item j = wid): kept samples m = 1..14 -> rows p PW + j + 16 (m - 1) (+ OS_V)
+        {
+            float2 x[16];
+            x[0] = own[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(own[q * PS2], twp[(q - 1) * 16]);
+            __syncwarp();                          // interleaved words all read before the next planar landing
+            if (p + 1 < p1) osv2_land(pw, col, Nx, vmask, (p + 1) * os2::PW - OS_H + b + wid);
+            idft_dit<16, 1>(x);
+            const int row0 = p * os2::PW + wid;    // row of m = 1, block A
+            if (a.ng > 0) osv2_source(x, a, RS, lane, row0, ssh);
+            float* po = ocol + (size_t)row0 * Nx;
+            const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
+            if (p * os2::PW + os2::PW <= Nv) {
+#pragma unroll
+                for (int m = 1; m < 15; ++m) {
+                    __stcs(po, x[m].x);
+                    __stcs(po + sV, x[m].y);
+                    po += s16;
+                }
+            } else {
+#pragma unroll
+                for (int m = 1; m < 15; ++m) {
+                    if (row0 + 16 * (m - 1) < Nv) __stcs(po, x[m].x);
+                    if (row0 + 16 * (m - 1) + OS_V < Nv) __stcs(po + sV, x[m].y);
+                    po += s16;
+                }
+            }
+        }
+        // no barrier here: pass A touches only the warp's own positions
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// v-direction, register-landing variant: as osv2_kernel, but the 32 samples of a warp's pass-A item go
+// straight from global memory into the butterfly registers (each load instruction of a warp is one
+// 128-byte row segment per distinct shift), and the twiddles are products of four register-resident powers
+// (t = warp index is fixed).  The scratch is only the exchange buffer between the phases.
+__device__ __forceinline__ void osv3_load(float2* x, const float* __restrict__ col, const int Nx, const int vmask,
+                                          const int r0)
+{
+    const int rr = r0 & vmask;
+    if (rr + OS_V + 241 <= vmask + 1) {             // the two windows do not wrap: constant row stride
+        const float* p = col + (size_t)rr * Nx;
+        const float* q = p + (size_t)OS_V * Nx;
+        const size_t s16 = (size_t)16 * Nx;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            x[k] = make_float2(__ldg(p), __ldg(q));
+            p += s16;
+            q += s16;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const int ra = (r0 + 16 * k) & vmask, rb = (r0 + 16 * k + OS_V) & vmask;
+            x[k] = make_float2(__ldg(col + (size_t)ra * Nx), __ldg(col + (size_t)rb * Nx));
+        }
+    }
+}
+
+__global__ void __launch_bounds__(512, 2) osv3_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int W = 32;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // 256 * 32
+    float2* const lamS = scr + 256 * W;                                       // 130 * 32, [k][lane]
+    float4* const RS = reinterpret_cast<float4*>(lamS + OS_LAMW * W);         // [4][32] source recurrence constants
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5;   // wid = item index (t, g, j)
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
+    const int c0 = blockIdx.x * W;
+
+    {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
+        const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
+        float4* dst4 = reinterpret_cast<float4*>(lamS);
+        for (int i = tid; i < OS_LAMW * 16; i += T)
+            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
+    }
+    Tw4 w;
+    w.b1 = __ldg(a.tw + wid);
+    w.b2 = __ldg(a.tw + 16 + wid);
+    w.b4 = __ldg(a.tw + 3 * 16 + wid);
+    w.b8 = __ldg(a.tw + 7 * 16 + wid);
+    // integer shift and source shift of this lane's column straight from the table in global memory, so that
+    // the first loads do not wait for the staged copy
+    const float2 e129 = __ldg(a.lam + (size_t)129 * Nx + c0 + lane);
+    const int b = __float_as_int(e129.x);
+    const float ssh = e129.y;
+    if (a.ng > 0 && tid < 4 * W) {
+        const int g = tid >> 5;
+        const float h = 32.0f * (g < a.ng ? a.cg4[g] : 0.0f) * ssh * a.dvf;
+        RS[g * W + lane] = make_float4(expf(h), expm1f(h), expf(-h), expm1f(-h));
+    }
+    const float* const col = a.src + c0 + lane;
+    float* const ocol = a.dst + c0 + lane;
+    const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
+    float2* const own = scr + wid * W + lane;                                 // position t = wid
+    constexpr int PS2 = 16 * W;                                               // float2 between positions 16 apart
+
+    for (int p = p0; p < p1; ++p) {
+        // ---- pass A (item t = wid) straight from global memory
+        {
+            float2 x[16];
+            osv3_load(x, col, Nx, vmask, p * os2::PW - OS_H + b + wid);
+            dft_dif<16, 1>(x);
+            own[0] = x[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                own[q * PS2] = cmul(x[brev(q, 16)], y);
+            });
+        }
+        if (p == p0) os2::cp_async_wait_all();     // symbol tables
+        __syncthreads();
+        // ---- middle stage (item g = wid): positions 16 g + j
+        {
+            float2* const s = scr + wid * 16 * W + lane;
+            float2 x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = s[j * W];
+            os2::mid16<W>(x, lamS + lane, wid);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) s[j * W] = x[j];
+        }
+        __syncthreads();
+        // ---- inverse pass A (item j = wid): kept samples m = 1..14 -> rows p PW + j + 16 (m - 1) (+ OS_V)
+        {
+            float2 x[16];
+            x[0] = own[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                x[brev(q, 16)] = cmulc(own[q * PS2], y);
+            });
+            idft_dit<16, 1>(x);
+            const int row0 = p * os2::PW + wid;    // row of m = 1, block A
+            if (a.ng > 0) osv2_source(x, a, RS, lane, row0, ssh);
+            float* po = ocol + (size_t)row0 * Nx;
+            const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
+            if (p * os2::PW + os2::PW <= Nv) {
+#pragma unroll
+                for (int m = 1; m < 15; ++m) {
+                    __stcs(po, x[m].x);
+                    __stcs(po + sV, x[m].y);
+                    po += s16;
+                }
+            } else {
+#pragma unroll
+                for (int m = 1; m < 15; ++m) {
+                    if (row0 + 16 * (m - 1) < Nv) __stcs(po, x[m].x);
+                    if (row0 + 16 * (m - 1) + OS_V < Nv) __stcs(po + sV, x[m].y);
+                    po += s16;
+                }
+            }
+        }
+        // no barrier here: the next pass A writes only the warp's own positions, which it has just read
+    }
+}
+
+}  // namespace vog
