@@ -103,8 +103,10 @@ int osx_occupancy(int threads, size_t smem);
 cudaError_t osx2_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
 int osx2_occupancy(int threads, size_t smem);
-cudaError_t osx3_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
-int osx3_occupancy(int threads, size_t smem);
+cudaError_t osx3_launch(const OsArgs& a, int mode, int grid, int threads, size_t smem, cudaStream_t st);
+int osx3_occupancy(int mode, int threads, size_t smem);
+cudaError_t osx5_launch(const OsArgs& a, bool inplace, int grid, int threads, size_t smem, cudaStream_t st);
+int osx5_occupancy(int threads, size_t smem);
 cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
 
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)

@@ -549,7 +549,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         int thr = ((16 * npx * l2 + 31) / 32) * 32;
         if (thr > 320) thr = 320;
-        P->os2x_direct = 1; P->os3x_occ = 0; P->os2v_direct = 0;
+        P->os2x_direct = 3; P->os3x_occ = 0; P->os2v_direct = 0;
         P->os_gen = 2; P->os2x_lpi = l2; P->os2x_thr = thr; P->os2x_occ = 0; P->os2v_gpc = 0;
     }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
@@ -710,7 +710,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
                  P->os2x_lpi = value; P->os2x_occ = 0; P->os3x_occ = 0; break;
         case 19: if (value < 32 || value > 320 || value % 32) return VOG_EINVAL; P->os2x_thr = value; P->os2x_occ = 0; break;
         case 20: if (value < 0) return VOG_EINVAL; P->os2v_gpc = value; break;
-        case 21: if (value < 0 || value > 1) return VOG_EINVAL; P->os2x_direct = value; break;
+        case 21: if (value < 0 || value > 3) return VOG_EINVAL; P->os2x_direct = value; P->os3x_occ = 0; break;
         case 22: if (value < 0 || value > 1) return VOG_EINVAL; P->os2v_direct = value; break;
         default: return VOG_EINVAL;
     }
@@ -810,14 +810,26 @@ static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
     const size_t smem = osx2_smem_bytes(a.lpi, a.np);
     if (P->os2x_direct && 16 * a.np * a.lpi <= 320) {
         const int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
+        if (P->os2x_direct == 3) {                 // warp-private kernel
+            const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8 + OS_LAMW * 8) + 16;
+            if (P->os3x_occ == 0) {
+                P->os3x_occ = osx5_occupancy(thr, sm5);
+                if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
+            }
+            int grid = P->os3x_occ * P->n_sm;
+            if (grid > a.n_groups) grid = a.n_groups;
+            P->launches++;
+            return osx5_launch(a, src == dst, grid, thr, sm5, P->st);
+        }
+        const size_t smem = osx2_smem_bytes(a.lpi, a.np) - 240 * 8 + (P->os2x_direct == 2 ? (size_t)a.lpi * Nx * 4 : 0);
         if (P->os3x_occ == 0) {
-            P->os3x_occ = osx3_occupancy(thr, smem);
+            P->os3x_occ = osx3_occupancy(P->os2x_direct == 2, thr, smem);
             if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
         }
         int grid = P->os3x_occ * P->n_sm;
         if (grid > a.n_groups) grid = a.n_groups;
         P->launches++;
-        return osx3_launch(a, grid, thr, smem, P->st);
+        return osx3_launch(a, P->os2x_direct == 2, grid, thr, smem, P->st);
     }
     if (P->os2x_occ == 0) {
         P->os2x_occ = osx2_occupancy(P->os2x_thr, smem);

@@ -172,21 +172,48 @@ cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cu
     return cudaGetLastError();
 }
 
-cudaError_t osx3_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+// mode 1: raw-line landing of the next line group (needs lpi N floats more shared memory); mode 0: direct loads
+cudaError_t osx3_launch(const OsArgs& a, int mode, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    static size_t cur = 0;
-    cudaError_t e = set_smem((const void*)osx3_kernel, smem, &cur);
+    static size_t cur[2] = {0, 0};
+    const void* fn = mode ? (const void*)osx3_kernel<true> : (const void*)osx3_kernel<false>;
+    cudaError_t e = set_smem(fn, smem, &cur[mode ? 1 : 0]);
     if (e != cudaSuccess) return e;
-    osx3_kernel<<<grid, threads, smem, st>>>(a);
+    if (mode) osx3_kernel<true><<<grid, threads, smem, st>>>(a);
+    else osx3_kernel<false><<<grid, threads, smem, st>>>(a);
     return cudaGetLastError();
 }
 
-int osx3_occupancy(int threads, size_t smem)
+int osx3_occupancy(int mode, int threads, size_t smem)
+{
+    static size_t cur[2] = {0, 0};
+    const void* fn = mode ? (const void*)osx3_kernel<true> : (const void*)osx3_kernel<false>;
+    if (set_smem(fn, smem, &cur[mode ? 1 : 0]) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int nb = 0;
+    const cudaError_t e = mode ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx3_kernel<true>, threads, smem)
+                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx3_kernel<false>, threads, smem);
+    if (e != cudaSuccess) { cudaGetLastError(); return 0; }
+    return nb;
+}
+
+// warp-private x kernel; inplace selects the split-mbarrier variant (src may equal dst)
+cudaError_t osx5_launch(const OsArgs& a, bool inplace, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur[2] = {0, 0};
+    const void* fn = inplace ? (const void*)osx5_kernel<true> : (const void*)osx5_kernel<false>;
+    cudaError_t e = set_smem(fn, smem, &cur[inplace ? 1 : 0]);
+    if (e != cudaSuccess) return e;
+    if (inplace) osx5_kernel<true><<<grid, threads, smem, st>>>(a);
+    else osx5_kernel<false><<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+int osx5_occupancy(int threads, size_t smem)
 {
     static size_t cur = 0;
-    if (set_smem((const void*)osx3_kernel, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (set_smem((const void*)osx5_kernel<true>, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx3_kernel, threads, smem) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx5_kernel<true>, threads, smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }

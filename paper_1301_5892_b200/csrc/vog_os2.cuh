@@ -263,12 +263,21 @@ __device__ __forceinline__ void osx3_load(float2* x, const float* __restrict__ g
     }
 }
 
+// RAW = false: the loads of a group are issued and consumed at the top of its own iteration (nothing is in
+// flight while a CTA computes; the other CTAs of the SM cover for it).
+// RAW = true: the lines of the NEXT group are copied as they are (cp.async, 16 bytes, no shift) into a raw line
+// buffer right after pass A of the current group has emptied it, so they have the middle stage and the inverse
+// pass to arrive (~2/3 of the time, 32 KB per CTA in flight); pass A then reads its samples from the raw
+// buffer with the shift applied by addressing (4-byte shared loads, any alignment).  One more barrier per
+// iteration (the raw lines are landed by all threads).
+template <bool RAW>
 __global__ void __launch_bounds__(320, 3) osx3_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
     float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
     float2* const lamS = scr + ptot * os2::XPAIR;                       // lpi rows of the symbol table
+    float* const raw = reinterpret_cast<float*>(lamS + lpi * OS_LAMW);  // RAW: lpi lines of N floats
     const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
     const int N = a.N, mask = N - 1;
     const bool active = tid < nitem;
@@ -284,21 +293,49 @@ __global__ void __launch_bounds__(320, 3) osx3_kernel(const OsArgs a)
     const float2* const lamL = lamS + l * OS_LAMW;
     const int o0 = pp * os2::PW + t;
     const bool full = (pp + 1) * os2::PW <= N;
+    const int G = gridDim.x;
 
-    auto land_tab = [&](const int line0) {
-        const int nl = min(lpi, a.n_lines - line0);
+    // the group's table rows and (RAW) its lines; a ragged last group has fewer lines
+    auto land = [&](const int g) {
+        const int line0 = g * lpi, nl = min(lpi, a.n_lines - line0);
         const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
         float4* dst4 = reinterpret_cast<float4*>(lamS);
         for (int i = tid; i < nl * (OS_LAMW / 2); i += T) os2::cp_async16(dst4 + i, src4 + i);
+        if constexpr (RAW) {
+            const float4* s4 = reinterpret_cast<const float4*>(a.src + (size_t)line0 * N);
+            float4* d4 = reinterpret_cast<float4*>(raw);
+            const int n4 = nl * (N >> 2);
+#pragma unroll 4
+            for (int i = tid; i < n4; i += T) os2::cp_async16(d4 + i, s4 + i);
+        }
     };
-    if ((int)blockIdx.x < a.n_groups) land_tab(blockIdx.x * lpi);
-    for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
+    if ((int)blockIdx.x < a.n_groups) land(blockIdx.x);
+    for (int g = blockIdx.x; g < a.n_groups; g += G) {
+        const int gn = g + G;
         const int line = min(g * lpi + l, a.n_lines - 1);      // (a ragged last group recomputes the last line)
-        // ---- pass A straight from global memory
+        if constexpr (RAW) {
+            os2::cp_async_wait_all();              // this thread's chunks of the raw lines and table rows
+            __syncthreads();
+        }
+        // ---- pass A
         if (active) {
             float2 x[16];
-            const int b = __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x));
-            osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+            if constexpr (RAW) {
+                const int b = __float_as_int(lamL[129].x);
+                const float* const rl = raw + l * N;
+                const int c0 = (pp * os2::PW - OS_H + b + t) & mask;
+                if (c0 + OS_V + 241 <= N) {
+#pragma unroll
+                    for (int k = 0; k < 16; ++k) x[k] = make_float2(rl[c0 + 16 * k], rl[c0 + 16 * k + OS_V]);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 16; ++k)
+                        x[k] = make_float2(rl[(c0 + 16 * k) & mask], rl[(c0 + 16 * k + OS_V) & mask]);
+                }
+            } else {
+                const int b = __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x));
+                osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+            }
             dft_dif<16, 1>(x);
             sA[0] = x[0];
             os2_tw_each(w, [&](auto qc, const float2 y) {
@@ -306,16 +343,16 @@ __global__ void __launch_bounds__(320, 3) osx3_kernel(const OsArgs a)
                 sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
             });
         }
-        os2::cp_async_wait_all();                  // table chunks
+        if constexpr (!RAW) os2::cp_async_wait_all();          // table rows
         __syncthreads();
         // ---- middle stage
         if (active) osx2_mid(sM, t, lamL);
         __syncthreads();
-        // ---- inverse pass A: scratch -> registers -> global, then the loads of the next line group.  In place
-        // this is safe: every load of THIS group was consumed before the first barrier, and the next group is
-        // other lines (owned by this CTA).
-        const int gn = g + gridDim.x;
-        if (gn < a.n_groups) land_tab(gn * lpi);   // lamS was last read before the barrier above
+        // the raw buffer was emptied before the first barrier, the table rows were last read before the second:
+        // the next group starts landing now and has the whole inverse pass (and the other CTAs' phases) to arrive
+        if (gn < a.n_groups) land(gn);
+        // ---- inverse pass A: scratch -> registers -> global.  In place this is safe: every load of THIS group
+        // completed before the first barrier, and the other groups are other lines (owned by this CTA).
         if (active) {
             float2 x[16];
             x[0] = sA[0];
@@ -325,7 +362,136 @@ __global__ void __launch_bounds__(320, 3) osx3_kernel(const OsArgs a)
             });
             idft_dit<16, 1>(x);
             if (g * lpi + l < a.n_lines) {
-                float* const o = a.dst + (size_t)line * N + o0;
+                float* const o = a.dst + (size_t)(g * lpi + l) * N + o0;
+                if (full) {
+#pragma unroll
+                    for (int m = 1; m < 15; ++m) {
+                        __stcs(o + 16 * (m - 1), x[m].x);
+                        __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
+                    }
+                } else {
+#pragma unroll
+                    for (int m = 1; m < 15; ++m) {
+                        if (o0 + 16 * (m - 1) < N) __stcs(o + 16 * (m - 1), x[m].x);
+                        if (o0 + 16 * (m - 1) + OS_V < N) __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// x-direction, warp-private variant.  The 16 items of a pair are 16 consecutive threads in EVERY phase (pass A
+// item t, middle item g, inverse item j), so a warp owns its two pairs from the first load to the last store
+// and the phases are separated by __syncwarp() only: the warps of a CTA drift apart freely and their load,
+// compute and store phases overlap.  The symbol is read straight from the per-line table in global memory
+// (a 1 KB row shared by all warps of the line: L1 hits), so nothing is staged CTA-wide.
+// The only CTA-wide dependency left is the in-place hazard (every load of a line must complete before its
+// first store): a split mbarrier -- each warp ARRIVES once its samples are in registers and WAITS just before
+// its first store, with the middle stage and the inverse transform in between.  With INPLACE = false
+// (src != dst) there is no synchronisation between warps at all.
+namespace os2 {
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, const unsigned count)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(s), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(s) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, const unsigned parity)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n.reg .pred p;\nWAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n}\n" ::"r"(s), "r"(parity) : "memory");
+}
+}  // namespace os2
+
+template <bool INPLACE>
+__global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
+    float2* const lamP = scr + ptot * os2::XPAIR;                       // one table row per pair (half-warp private)
+    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(lamP + ptot * OS_LAMW);
+    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
+    const int N = a.N, mask = N - 1;
+    const bool active = tid < nitem;
+    const int pr = tid >> 4;
+    const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
+    Tw4 w;
+    w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
+    w.b2 = __ldg(a.tw + 16 + t);
+    w.b4 = __ldg(a.tw + 3 * 16 + t);
+    w.b8 = __ldg(a.tw + 7 * 16 + t);
+    float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
+    float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
+    const int o0 = pp * os2::PW + t;
+    const bool full = (pp + 1) * os2::PW <= N;
+    if constexpr (INPLACE) {
+        if (tid == 0) os2::mbar_init(bar, T >> 5);
+        __syncthreads();
+    }
+    unsigned parity = 0;
+    for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
+        const int line = min(g * lpi + l, a.n_lines - 1);      // (a ragged last group recomputes the last line)
+        const float2* __restrict__ lamG = a.lam + (size_t)line * OS_LAMW;
+        const float2* const lamL = lamP + pr * OS_LAMW;
+        // ---- pass A straight from global memory
+        if (active) {
+            // the pair's copy of the line's symbol table lands behind pass A (its previous contents were last read
+            // by these 16 threads before the __syncwarp() that closed the previous middle stage)
+            for (int i = t; i < OS_LAMW / 2; i += 16)
+                os2::cp_async16(reinterpret_cast<float4*>(lamP + pr * OS_LAMW) + i, reinterpret_cast<const float4*>(lamG) + i);
+            float2 x[16];
+            const int b = __float_as_int(__ldg(&lamG[129].x));
+            osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+            dft_dif<16, 1>(x);
+            sA[0] = x[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
+            });
+        }
+        os2::cp_async_wait_all();
+        __syncwarp();
+        // (the stores above needed every loaded value, and a warp issues in order: its loads have completed)
+        if constexpr (INPLACE) { if ((tid & 31) == 0) os2::mbar_arrive(bar); }
+        // ---- middle stage
+        if (active) {
+            float2 x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = sM[j];
+            dft_dif<16, 1>(x);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) x[brev(q, 16)] = cmul(x[brev(q, 16)], lamL[t + 16 * q]);
+#pragma unroll
+            for (int q = 8; q < 16; ++q) x[brev(q, 16)] = cmulc(x[brev(q, 16)], lamL[256 - 16 * q - t]);
+            idft_dit<16, 1>(x);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) sM[j] = x[j];
+        }
+        __syncwarp();
+        // ---- inverse pass A: scratch -> registers -> global
+        if constexpr (INPLACE) { os2::mbar_wait(bar, parity); parity ^= 1u; }
+        {
+            float2 x[16];
+            if (active) {
+                x[0] = sA[0];
+                os2_tw_each(w, [&](auto qc, const float2 y) {
+                    constexpr int q = decltype(qc)::value;
+                    x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
+                });
+                idft_dit<16, 1>(x);
+            }
+            if (active && g * lpi + l < a.n_lines) {
+                float* const o = a.dst + (size_t)(g * lpi + l) * N + o0;
                 if (full) {
 #pragma unroll
                     for (int m = 1; m < 15; ++m) {

@@ -211,6 +211,50 @@ def test_tile_shape_overrides_keep_parity(torch, vog, oracle):
     plan.destroy()
 
 
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
+def test_x_pair_kernel_variants_in_place_with_large_shifts(torch, vog, oracle, mode):
+    """Every variant of the pair x kernel (landing through shared memory, direct register loads, raw-line
+    landing, warp-private with the split barrier) advects IN PLACE with shifts of thousands of cells: a store
+    that overtook a load of the same line would show up as an error of order one.  512 lines > one wave of
+    CTAs, so the persistent loop and the barrier phase flip are exercised too."""
+    Nx, Nv = 8192, 512
+    f = inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + 77)
+    bx = inputs.uniform_shifts(Nv, inputs.SEED + 78, lo=-4000.0, hi=4000.0)
+    ref = oracle.shift_x(f, bx, LAG, 17)
+    plan = vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, LAG, 17)
+    plan.tune(21, mode)
+    fd = _dev(torch, f)
+    plan.shift_x(fd, _dev(torch, bx))
+    _check(fd.cpu().numpy(), ref, 1.0)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("which,value", [(17, 1), (22, 1), (20, 1), (20, 3), (18, 2), (19, 160)])
+def test_kernel_generation_and_shape_overrides_keep_parity(torch, vog, oracle, which, value):
+    """The even/odd kernels (generation 1), the register-landing v kernel and other launch shapes of the pair
+    kernels compute the same advection, delta-f source included."""
+    cfg = inputs.config(3, Nx=128, Nv=2048)
+    f = 1e-3 * inputs.smooth_grid(cfg.Nx, cfg.Nv)
+    feq = oracle.Feq.make(cfg.feq)
+    rng = np.random.default_rng(9)
+    Ebig = (0.6 * np.sin(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx + 0.3) + 0.05 * rng.normal(size=cfg.Nx)).astype(np.float32)
+    ref = oracle.advect_v(f, Ebig, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq)
+    plan = vog.Plan.from_config(cfg)
+    plan.tune(which, value)
+    fd = _dev(torch, f)
+    plan.advect_v(fd, _dev(torch, Ebig), cfg.dt)
+    _check(fd.cpu().numpy(), ref, max(np.abs(f).max(), np.abs(ref).max()))
+    plan.destroy()
+    g = inputs.uniform_grid(2048, 64, seed=inputs.SEED + 5)
+    bx = _shifts(64, 53)
+    plan = vog.Plan(2048, 64, 1.0, -1.0, 1.0, SPL, 3)
+    plan.tune(which, value)
+    gd = _dev(torch, g)
+    plan.shift_x(gd, _dev(torch, bx))
+    _check(gd.cpu().numpy(), oracle.shift_x(g, bx, SPL, 3), 1.0)
+    plan.destroy()
+
+
 # ------------------------------------------------------------------ full runs: energy history, configs 0-1
 def _gpu_history(torch, vog, cfg, steps):
     plan = vog.Plan.from_config(cfg)
