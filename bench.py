@@ -37,7 +37,7 @@ def _traffic():
     try:
         for line in open(path):
             key, _, val = line.strip().partition(",")
-            if key == "osx_kernel_bench_dram_bytes_per_launch":
+            if key == "x_kernel_bench_dram_bytes_per_launch":
                 return float(val)
     except Exception:
         pass
@@ -231,7 +231,7 @@ def main():
     peak, peak_src = _peaks()
     alg_bytes = 8.0 * cells                      # one read + one write of f per advection
     ach = alg_bytes / (ms_x * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "osx_kernel (overlap-save x-advection, 2048-cell lines)", "achieved": ach, "peak": peak,
+    roofline = {"bound": "hbm", "kernel": "osx5_kernel (overlap-save x-advection, block pairs, warp-private; 2048-cell lines)", "achieved": ach, "peak": peak,
                 "unit": "GB/s", "frac": ach / peak, "traffic": _traffic(), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_x,
                 "other_kernels_ms": {"advect_v(+delta-f source)": ms_v, "density+poisson": ms_f},

@@ -808,19 +808,22 @@ static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
     a.n_lines = Nv;
     a.n_groups = (Nv + a.lpi - 1) / a.lpi;
     const size_t smem = osx2_smem_bytes(a.lpi, a.np);
+    if (P->os2x_direct == 3) {                     // warp-private kernel: any group size (rounds of thr items)
+        int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
+        if (thr > 320) thr = ((((16 * a.np * a.lpi + 1) / 2) + 31) / 32) * 32;      // two rounds
+        if (thr > 320) thr = 320;
+        const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8) + (size_t)(thr / 16) * OS_LAMW * 8 + 16;
+        if (P->os3x_occ == 0) {
+            P->os3x_occ = osx5_occupancy(thr, sm5);
+            if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
+        }
+        int grid = P->os3x_occ * P->n_sm;
+        if (grid > a.n_groups) grid = a.n_groups;
+        P->launches++;
+        return osx5_launch(a, src == dst, grid, thr, sm5, P->st);
+    }
     if (P->os2x_direct && 16 * a.np * a.lpi <= 320) {
         const int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
-        if (P->os2x_direct == 3) {                 // warp-private kernel
-            const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8 + OS_LAMW * 8) + 16;
-            if (P->os3x_occ == 0) {
-                P->os3x_occ = osx5_occupancy(thr, sm5);
-                if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
-            }
-            int grid = P->os3x_occ * P->n_sm;
-            if (grid > a.n_groups) grid = a.n_groups;
-            P->launches++;
-            return osx5_launch(a, src == dst, grid, thr, sm5, P->st);
-        }
         const size_t smem = osx2_smem_bytes(a.lpi, a.np) - 240 * 8 + (P->os2x_direct == 2 ? (size_t)a.lpi * Nx * 4 : 0);
         if (P->os3x_occ == 0) {
             P->os3x_occ = osx3_occupancy(P->os2x_direct == 2, thr, smem);
@@ -856,7 +859,7 @@ static cudaError_t run_osv2(vog_plan_s* P, const float* src, float* dst, bool so
     const int strips = Nx / 32;
     // pairs per CTA: minimise waves x pairs per CTA (2 CTAs of 512 threads per SM); ties go to the longer loop
     // (fewer reloads of the strip's symbol tables)
-    int gpc = P->os2v_gpc;
+    int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : 1;   // measured: one pair per CTA is fastest at 2048..8192 (profiles/)
     if (gpc <= 0) {
         long long best = -1;
         const long long slots = (long long)P->n_sm * 2;

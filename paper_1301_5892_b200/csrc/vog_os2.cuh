@@ -417,82 +417,90 @@ __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
+    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15, hw = tid >> 4;
     float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
-    float2* const lamP = scr + ptot * os2::XPAIR;                       // one table row per pair (half-warp private)
-    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(lamP + ptot * OS_LAMW);
-    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
+    float2* const lamP = scr + ptot * os2::XPAIR;                       // one table row per half-warp (private)
+    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(lamP + (T >> 4) * OS_LAMW);
     const int N = a.N, mask = N - 1;
-    const bool active = tid < nitem;
-    const int pr = tid >> 4;
-    const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
     Tw4 w;
     w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
     w.b2 = __ldg(a.tw + 16 + t);
     w.b4 = __ldg(a.tw + 3 * 16 + t);
     w.b8 = __ldg(a.tw + 7 * 16 + t);
-    float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
-    float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
-    const int o0 = pp * os2::PW + t;
-    const bool full = (pp + 1) * os2::PW <= N;
+    float2* const lamL = lamP + hw * OS_LAMW;
     if constexpr (INPLACE) {
         if (tid == 0) os2::mbar_init(bar, T >> 5);
         __syncthreads();
     }
     unsigned parity = 0;
+    // A line group has nitem items; thread tid takes items tid, tid + T, .. ("rounds"; one round when the group
+    // fits the CTA, two for 16384-cell lines).  Per round: load, pass A, middle stage -- the pair's spectrum
+    // stays in its scratch; then, once every load of the group has completed, per round: inverse pass and stores.
     for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
-        const int line = min(g * lpi + l, a.n_lines - 1);      // (a ragged last group recomputes the last line)
-        const float2* __restrict__ lamG = a.lam + (size_t)line * OS_LAMW;
-        const float2* const lamL = lamP + pr * OS_LAMW;
-        // ---- pass A straight from global memory
-        if (active) {
-            // the pair's copy of the line's symbol table lands behind pass A (its previous contents were last read
-            // by these 16 threads before the __syncwarp() that closed the previous middle stage)
-            for (int i = t; i < OS_LAMW / 2; i += 16)
-                os2::cp_async16(reinterpret_cast<float4*>(lamP + pr * OS_LAMW) + i, reinterpret_cast<const float4*>(lamG) + i);
-            float2 x[16];
-            const int b = __float_as_int(__ldg(&lamG[129].x));
-            osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
-            dft_dif<16, 1>(x);
-            sA[0] = x[0];
-            os2_tw_each(w, [&](auto qc, const float2 y) {
-                constexpr int q = decltype(qc)::value;
-                sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
-            });
-        }
-        os2::cp_async_wait_all();
-        __syncwarp();
-        // (the stores above needed every loaded value, and a warp issues in order: its loads have completed)
-        if constexpr (INPLACE) { if ((tid & 31) == 0) os2::mbar_arrive(bar); }
-        // ---- middle stage
-        if (active) {
-            float2 x[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) x[j] = sM[j];
-            dft_dif<16, 1>(x);
-#pragma unroll
-            for (int q = 0; q < 8; ++q) x[brev(q, 16)] = cmul(x[brev(q, 16)], lamL[t + 16 * q]);
-#pragma unroll
-            for (int q = 8; q < 16; ++q) x[brev(q, 16)] = cmulc(x[brev(q, 16)], lamL[256 - 16 * q - t]);
-            idft_dit<16, 1>(x);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) sM[j] = x[j];
-        }
-        __syncwarp();
-        // ---- inverse pass A: scratch -> registers -> global
-        if constexpr (INPLACE) { os2::mbar_wait(bar, parity); parity ^= 1u; }
-        {
-            float2 x[16];
+#pragma unroll 1
+        for (int it = tid; it - (tid & 31) < nitem; it += T) {          // (trip count uniform over the warp)
+            const int pr = it >> 4;
+            const bool active = it < nitem;
+            const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
+            const int line = min(g * lpi + l, a.n_lines - 1);  // (a ragged last group recomputes the last line)
+            const float2* __restrict__ lamG = a.lam + (size_t)line * OS_LAMW;
+            float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
+            float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
+            // ---- pass A straight from global memory
             if (active) {
-                x[0] = sA[0];
+                // the half-warp's copy of the line's symbol table lands behind pass A (its previous contents
+                // were last read by these 16 threads before the __syncwarp() that closed their last middle stage)
+                for (int i = t; i < OS_LAMW / 2; i += 16)
+                    os2::cp_async16(reinterpret_cast<float4*>(lamL) + i, reinterpret_cast<const float4*>(lamG) + i);
+                float2 x[16];
+                const int b = __float_as_int(__ldg(&lamG[129].x));
+                osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+                dft_dif<16, 1>(x);
+                sA[0] = x[0];
                 os2_tw_each(w, [&](auto qc, const float2 y) {
                     constexpr int q = decltype(qc)::value;
-                    x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
+                    sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
                 });
-                idft_dit<16, 1>(x);
             }
-            if (active && g * lpi + l < a.n_lines) {
+            os2::cp_async_wait_all();
+            __syncwarp();
+            // (the shared stores of pass A needed every loaded value, and a warp issues in order: once its last
+            // round is here, all loads of this warp have completed)
+            if constexpr (INPLACE) {
+                if (it - (tid & 31) + T >= nitem && (tid & 31) == 0) os2::mbar_arrive(bar);
+            }
+            // ---- middle stage
+            if (active) {
+                float2 x[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) x[j] = sM[j];
+                os2::mid16<1>(x, lamL, t);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) sM[j] = x[j];
+            }
+            __syncwarp();
+        }
+        if constexpr (INPLACE) {                   // every load of the group has completed, in every warp
+            os2::mbar_wait(bar, parity);
+            parity ^= 1u;
+        }
+        // ---- inverse pass A: scratch -> registers -> global
+#pragma unroll 1
+        for (int it = tid; it < nitem; it += T) {
+            const int pr = it >> 4;
+            const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;
+            const float2* const sA = scr + pr * os2::XPAIR + t;
+            const int o0 = pp * os2::PW + t;
+            float2 x[16];
+            x[0] = sA[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
+            });
+            idft_dit<16, 1>(x);
+            if (g * lpi + l < a.n_lines) {
                 float* const o = a.dst + (size_t)(g * lpi + l) * N + o0;
-                if (full) {
+                if ((pp + 1) * os2::PW <= N) {
 #pragma unroll
                     for (int m = 1; m < 15; ++m) {
                         __stcs(o + 16 * (m - 1), x[m].x);
