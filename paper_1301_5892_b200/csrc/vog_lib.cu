@@ -342,7 +342,7 @@ struct vog_plan_s {
     int osv_np_log, osv_thr, osv_rb, osv_gpc;
     int os_gen;                            // 2 = pair kernels of vog_os2.cuh (default), 1 = even/odd kernels of vog_os.cuh
     int os2x_lpi, os2x_thr, os2x_occ, os2v_gpc;
-    int os2v_direct;                       // v: register-landing kernel osv3_kernel (measured slower than osv2_kernel: off)
+    int os2v_direct;                       // v kernel: 2 = coalesced raw-row landing (osv4_kernel, default), 1 = register landing (osv3), 0 = per-lane landing (osv2)
     int os2x_direct, os3x_occ;             // x: register-landing kernel (osx3_kernel) when a line group fits one round of 320 threads
     int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
     float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
@@ -549,7 +549,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         int thr = ((16 * npx * l2 + 31) / 32) * 32;
         if (thr > 320) thr = 320;
-        P->os2x_direct = 3; P->os3x_occ = 0; P->os2v_direct = 0;
+        P->os2x_direct = 3; P->os3x_occ = 0; P->os2v_direct = 2;
         P->os_gen = 2; P->os2x_lpi = l2; P->os2x_thr = thr; P->os2x_occ = 0; P->os2v_gpc = 0;
     }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
@@ -711,7 +711,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 19: if (value < 32 || value > 320 || value % 32) return VOG_EINVAL; P->os2x_thr = value; P->os2x_occ = 0; break;
         case 20: if (value < 0) return VOG_EINVAL; P->os2v_gpc = value; break;
         case 21: if (value < 0 || value > 3) return VOG_EINVAL; P->os2x_direct = value; P->os3x_occ = 0; break;
-        case 22: if (value < 0 || value > 1) return VOG_EINVAL; P->os2v_direct = value; break;
+        case 22: if (value < 0 || value > 2) return VOG_EINVAL; P->os2v_direct = value; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -873,6 +873,8 @@ static cudaError_t run_osv2(vog_plan_s* P, const float* src, float* dst, bool so
     a.gpc = gpc;
     dim3 grid(strips, (a.np + gpc - 1) / gpc);
     P->launches++;
+    if (P->os2v_direct == 2)
+        return osv4_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
     if (P->os2v_direct) return osv3_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 4 * 32 * 16, P->st);
     return osv2_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
 }

@@ -163,6 +163,15 @@ cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cu
     return cudaGetLastError();
 }
 
+cudaError_t osv4_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur = 0;
+    cudaError_t e = set_smem((const void*)osv4_kernel, smem, &cur);
+    if (e != cudaSuccess) return e;
+    osv4_kernel<<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
 cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
 {
     static size_t cur = 0;

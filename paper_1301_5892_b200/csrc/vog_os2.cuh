@@ -813,4 +813,137 @@ __global__ void __launch_bounds__(512, 2) osv3_kernel(const OsArgs a)
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// v-direction, coalesced-landing variant.  osv2_kernel lets every lane fetch its own shifted rows, which is a
+// gather of up to 32 rows per load instruction when neighbouring columns have different integer shifts (the
+// sweep's random shifts).  Here the CTA first copies the UNION of the rows its 32 columns need -- unshifted,
+// 16 bytes per lane, whole 128-byte row segments -- into shared memory, raw[row][column], and a lane applies its
+// own shift when it reads its samples from there: in this layout a lane only ever touches its own bank, so
+// any per-lane row offset is conflict-free.  The raw rows (480 + R, R = spread of the shifts in the strip,
+// <= 32) share the 64 KB of the exchange buffer, so two more barriers separate "raw read" from "exchange
+// written".  Strips whose shifts spread over more than 32 rows fall back to the per-lane fetch (same layout).
+namespace os2 {
+constexpr int RMAX = 32;
+}
+
+__global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int W = 32;
+    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // 256 * 32 float2 = raw[512][32] floats
+    float* const raw = reinterpret_cast<float*>(smem_raw);
+    float2* const lamS = scr + 256 * W;                                       // 130 * 32, [k][lane]
+    float2* const twS = lamS + OS_LAMW * W;                                   // 15 * 16
+    float4* const RS = reinterpret_cast<float4*>(twS + 240);                  // [4][32] source recurrence constants
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5;   // wid = item index (t, g, j)
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
+    const int c0 = blockIdx.x * W;
+
+    {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
+        const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
+        float4* dst4 = reinterpret_cast<float4*>(lamS);
+        for (int i = tid; i < OS_LAMW * 16; i += T)
+            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
+    }
+    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
+    // integer shift (rows) and source shift of this lane's column
+    const float2 e129 = __ldg(a.lam + (size_t)129 * Nx + c0 + lane);
+    const int b = __float_as_int(e129.x);
+    const float ssh = e129.y;
+    // spread of the shifts over the strip, as signed distances from column 0's (shifts live mod Nv)
+    const int b0 = __shfl_sync(0xffffffffu, b, 0);
+    int d = (((b - b0) + (Nv >> 1)) & vmask) - (Nv >> 1);
+    int dmin = d, dmax = d;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dmin = min(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+        dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+    }
+    const int R = dmax - dmin;
+    const bool gather = R > os2::RMAX;             // uniform over the CTA (every warp sees the same 32 columns)
+    const int db = gather ? 0 : d - dmin;          // this lane's row offset inside the raw window
+    const int base = gather ? b : b0 + dmin;       // first raw row = pair start - OS_H + base
+    if (a.ng > 0 && tid < 4 * W) {
+        const int g = tid >> 5;
+        const float h = 32.0f * (g < a.ng ? a.cg4[g] : 0.0f) * ssh * a.dvf;
+        RS[g * W + lane] = make_float4(expf(h), expm1f(h), expf(-h), expm1f(-h));
+    }
+    const float* const col = a.src + c0 + lane;
+    float* const ocol = a.dst + c0 + lane;
+    const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
+    float2* const own = scr + wid * W + lane;                                 // position t = wid, interleaved
+    constexpr int PS2 = 16 * W;                                               // float2 between positions 16 apart
+    const int nrows = OS_V + OS_LB + (gather ? 0 : R);                        // 480 + R
+
+    for (int p = p0; p < p1; ++p) {
+        // ---- landing: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
+        const int rs = p * os2::PW - OS_H + base;
+        if (!gather) {
+            const float* const src = a.src + c0;
+            for (int c = tid; c < nrows * 8; c += T) {
+                const int r = c >> 3, q4 = (c & 7) * 4;
+                os2::cp_async16(raw + r * W + q4, src + (size_t)((rs + r) & vmask) * Nx + q4);
+            }
+        } else {
+            for (int r = wid; r < nrows; r += 16) os2::cp_async4(raw + r * W + lane, col + (size_t)((rs + r) & vmask) * Nx);
+        }
+        os2::cp_async_wait_all();
+        __syncthreads();
+        // ---- pass A (item t = wid): samples from the raw rows with this lane's offset
+        {
+            float2 x[16];
+            const float* const rp = raw + (wid + db) * W + lane;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + OS_V) * W]);
+            __syncthreads();                       // raw rows all read before the exchange buffer is written
+            const float2* const twp = twS + wid;
+            dft_dif<16, 1>(x);
+            own[0] = x[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) own[q * PS2] = cmul(x[brev(q, 16)], twp[(q - 1) * 16]);
+        }
+        __syncthreads();
+        // ---- middle stage (item g = wid): positions 16 g + j
+        {
+            float2* const s = scr + wid * 16 * W + lane;
+            float2 x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = s[j * W];
+            os2::mid16<W>(x, lamS + lane, wid);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) s[j * W] = x[j];
+        }
+        __syncthreads();
+        // ---- inverse pass A (item j = wid): kept samples m = 1..14 -> rows p PW + j + 16 (m - 1) (+ OS_V)
+        {
+            float2 x[16];
+            const float2* const twp = twS + wid;
+            x[0] = own[0];
+#pragma unroll
+            for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(own[q * PS2], twp[(q - 1) * 16]);
+            idft_dit<16, 1>(x);
+            const int row0 = p * os2::PW + wid;    // row of m = 1, block A
+            if (a.ng > 0) osv2_source(x, a, RS, lane, row0, ssh);
+            float* po = ocol + (size_t)row0 * Nx;
+            const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
+            if (p * os2::PW + os2::PW <= Nv) {
+#pragma unroll
+                for (int m = 1; m < 15; ++m) {
+                    __stcs(po, x[m].x);
+                    __stcs(po + sV, x[m].y);
+                    po += s16;
+                }
+            } else {
+#pragma unroll
+                for (int m = 1; m < 15; ++m) {
+                    if (row0 + 16 * (m - 1) < Nv) __stcs(po, x[m].x);
+                    if (row0 + 16 * (m - 1) + OS_V < Nv) __stcs(po + sV, x[m].y);
+                    po += s16;
+                }
+            }
+        }
+        if (p + 1 < p1) __syncthreads();           // the exchange buffer is read before the next raw rows land
+    }
+}
+
 }  // namespace vog

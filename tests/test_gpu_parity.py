@@ -229,7 +229,7 @@ def test_x_pair_kernel_variants_in_place_with_large_shifts(torch, vog, oracle, m
     plan.destroy()
 
 
-@pytest.mark.parametrize("which,value", [(17, 1), (22, 1), (20, 1), (20, 3), (18, 2), (19, 160)])
+@pytest.mark.parametrize("which,value", [(17, 1), (22, 0), (22, 1), (20, 2), (20, 3), (18, 2), (19, 160)])
 def test_kernel_generation_and_shape_overrides_keep_parity(torch, vog, oracle, which, value):
     """The even/odd kernels (generation 1), the register-landing v kernel and other launch shapes of the pair
     kernels compute the same advection, delta-f source included."""
@@ -253,6 +253,22 @@ def test_kernel_generation_and_shape_overrides_keep_parity(torch, vog, oracle, w
     plan.shift_x(gd, _dev(torch, bx))
     _check(gd.cpu().numpy(), oracle.shift_x(g, bx, SPL, 3), 1.0)
     plan.destroy()
+
+
+@pytest.mark.parametrize("lo,hi", [(-8.0, 8.0), (-20.0, 12.0), (-900.0, 900.0)])
+def test_v_coalesced_landing_any_shift_spread(torch, vog, oracle, lo, hi):
+    """The default v kernel lands the union of the rows of a 32-column strip unshifted and applies each column's
+    integer shift when reading shared memory; strips whose shifts spread over more than 32 rows (last case) take the
+    per-lane fallback inside the same kernel.  Nv = 2048 has a ragged last pair of blocks."""
+    Nx, Nv = 64, 2048
+    f = inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + 91)
+    bv = inputs.uniform_shifts(Nx, inputs.SEED + 92, lo=lo, hi=hi)
+    for kind, order in ((LAG, 17), (SPL, 3)):
+        plan = vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, kind, order)
+        fd = _dev(torch, f)
+        plan.shift_v(fd, _dev(torch, bv))
+        _check(fd.cpu().numpy(), oracle.shift_v(f, bv, kind, order), 1.0)
+        plan.destroy()
 
 
 # ------------------------------------------------------------------ full runs: energy history, configs 0-1
