@@ -317,6 +317,21 @@ def sweep(torch, vog, stream, peak, sizes=(2048, 8192), kinds=((0, 17), (0, 3), 
             med = float(np.median(times))
             gbs = 8.0 * N * N / (med * 1e-3) / 1e9
             row["x_kernel_only"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak}
+            # the v kernel out of place (table setup + kernel, no copy back): what vog_step runs
+            if N * N * 4 * 3 < 160e9:
+                g = torch.empty_like(f)
+                for _ in range(3):
+                    plan.shift_v_to(f, g, bx)
+                times = []
+                for _ in range(10):
+                    e0.record(stream); plan.shift_v_to(f, g, bx); e1.record(stream)
+                    stream.synchronize()
+                    times.append(e0.elapsed_time(e1))
+                med = float(np.median(times))
+                gbs = 8.0 * N * N / (med * 1e-3) / 1e9
+                row["v_out_of_place"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak,
+                                         "note": "vog_shift_v_to: table setup + kernel, src -> dst"}
+                del g
             for _ in range(2):
                 plan.step(f, 1e-3)
             times = []

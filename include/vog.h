@@ -99,6 +99,13 @@ int vog_get_field(vog_plan_t plan, float* E_dev);
 int vog_shift_x(vog_plan_t plan, float* f_dev, const double* beta_cells_dev);
 int vog_shift_v(vog_plan_t plan, float* f_dev, const double* beta_cells_dev);
 
+/* Out-of-place form of vog_shift_v: reads src_dev, writes dst_dev (both Nx*Nv floats, caller-owned device
+ * memory, dst_dev != src_dev and not overlapping).  For Nv >= 1024 the v kernel is out of place by
+ * construction (a block reads rows that other blocks write), so the in-place calls vog_shift_v / vog_advect_v
+ * go through the plan's second grid and copy back; this call is the kernel alone (it is what vog_step uses
+ * internally, ping-ponging between f and the second grid).  VOG_EINVAL if dst_dev == src_dev. */
+int vog_shift_v_to(vog_plan_t plan, const float* src_dev, float* dst_dev, const double* beta_cells_dev);
+
 /* End-to-end convenience with HOST buffers: copies f_host (Nx*Nv floats) and E_ext_host (Nx
  * floats or NULL) into a device buffer that the plan allocates on the first call and keeps (the
  * only O(Nx*Nv) allocation of the library, made only if this call is used), runs `nsteps`
@@ -113,9 +120,15 @@ int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   2, 3   whole-line v kernel (Nv <= 512): log2(complex lines per CTA), threads per CTA;
  *   5..8   whole-line x kernel (Nx <= 512): log2(lines per iteration), threads (32..128), CTAs per SM
  *          (0 = as many as fit), line buffers (1 or 2);
- *   10..12 overlap-save x kernel (Nx >= 1024): lines per iteration, threads (32..160), CTAs per SM;
- *   15, 16 overlap-save v kernel (Nv >= 1024): row blocks per group (1 or 2; threads = 128 x that),
- *          groups per CTA (0 = automatic).
+ *   10..12 first-generation overlap-save x kernel (Nx >= 1024): lines per iteration, threads (32..160), CTAs per SM;
+ *   15, 16 first-generation overlap-save v kernel (Nv >= 1024): row blocks per group (1 or 2; threads = 128 x
+ *          that), groups per CTA (0 = automatic);
+ *   17     overlap-save kernel generation: 2 = block-pair kernels (default), 1 = even/odd kernels;
+ *   18..20 block-pair kernels: x lines per iteration; x threads of the shared-memory-landing variant (32..320);
+ *          v pairs per CTA (0 = default: 1);
+ *   21     x variant: 0 = landing through shared memory, 1 = direct register loads with CTA barriers, 2 = raw-line
+ *          landing of the next line group, 3 = warp-private with the split barrier (default);
+ *   22     v variant: 0 = per-lane landing, 1 = direct register loads, 2 = coalesced landing of the strip's rows (default).
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

@@ -1084,6 +1084,14 @@ extern "C" int vog_shift_v(vog_plan_t P, float* f_dev, const double* beta)
     return cuda_status(e);
 }
 
+extern "C" int vog_shift_v_to(vog_plan_t P, const float* src_dev, float* dst_dev, const double* beta)
+{
+    if (!P || !src_dev || !dst_dev || !beta || src_dev == dst_dev) return VOG_EINVAL;
+    cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
+    if (e == cudaSuccess) e = advect_v(P, src_dev, dst_dev, false);
+    return cuda_status(e);
+}
+
 extern "C" int vog_field(vog_plan_t P, const float* f_dev, float* E_dev)
 {
     if (!P || !f_dev || !E_dev) return VOG_EINVAL;

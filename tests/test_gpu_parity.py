@@ -271,6 +271,23 @@ def test_v_coalesced_landing_any_shift_spread(torch, vog, oracle, lo, hi):
         plan.destroy()
 
 
+def test_shift_v_out_of_place_entry(torch, vog, oracle):
+    """vog_shift_v_to (the v kernel alone, src -> dst) equals the in-place call; src stays untouched; and it
+    refuses src == dst.  Also on a grid served by the whole-line kernels (copy + in-place kernel)."""
+    for Nx, Nv in ((64, 2048), (128, 256)):
+        f = inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + 93)
+        bv = _shifts(Nx, 94)
+        plan = vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, LAG, 17)
+        src, dst = _dev(torch, f), torch.zeros((Nv, Nx), device="cuda", dtype=torch.float32)
+        plan.shift_v_to(src, dst, _dev(torch, bv))
+        torch.cuda.synchronize()
+        _check(dst.cpu().numpy(), oracle.shift_v(f, bv, LAG, 17), 1.0)
+        assert np.array_equal(src.cpu().numpy(), f)
+        with pytest.raises(vog.VogError):
+            plan.shift_v_to(src, src, _dev(torch, bv))
+        plan.destroy()
+
+
 # ------------------------------------------------------------------ full runs: energy history, configs 0-1
 def _gpu_history(torch, vog, cfg, steps):
     plan = vog.Plan.from_config(cfg)
