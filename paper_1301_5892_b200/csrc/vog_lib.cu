@@ -201,8 +201,10 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
         double s = 0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
-        part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
+        if (gridDim.y == 1) rho[blockIdx.x * 32 + threadIdx.x] = s * dv;      // the block owns its columns: done
+        else part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
     }
+    if (gridDim.y == 1) return;
     // The last of the gridDim.y blocks of this column group to finish adds the partial rows in a FIXED
     // order (y = 0, 1, ..): deterministic, and the reduction is spread over the SMs instead of being
     // pulled through the single SM that solves the Poisson equation.
@@ -350,7 +352,7 @@ struct vog_plan_s {
     double* rho;                // [Nx]
     float* E_self;              // [Nx] last self-consistent field
     float *feq_tab, *vmu_tab;   // [ng][Nv]
-    int nby;
+    int nby, nby_max;           // density: row slabs per column group (tunable up to the allocated nby_max)
     int lognl_x, lognl_v, thr_x, thr_v;
     int n_sm;
     bool E_valid;
@@ -521,10 +523,11 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     P->sym = sym;
     P->d = d;
     const int Nx = p->Nx, Nv = p->Nv, ng = p->feq.n;
-    // density partial rows: enough blocks to fill the chip, at least 32 rows per block
+    // density row slabs per column group: up to 512 blocks of at least 128 rows (measured on 1024^2 .. 8192^2:
+    // more blocks cost more in the ticket reduction than they gain in parallelism; _work sweep, profiles/)
     int nby = 1;
-    while ((Nx / 32) * nby < 592 && Nv / (nby * 2) >= 32) nby *= 2;
-    P->nby = nby;
+    while ((Nx / 32) * nby * 2 <= 512 && Nv / (nby * 2) >= 128) nby *= 2;
+    P->nby = nby; P->nby_max = 16;
     {
         int dev = 0, nsm = 148;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -627,7 +630,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->xtwB, sizeof(float2) * xb.size());
     alloc((void**)&P->xcs, sizeof(float2) * xc.size());
     alloc((void**)&P->rec_v, sizeof(float) * REC_WORDS * Nx);
-    alloc((void**)&P->part, sizeof(double) * nby * Nx);
+    alloc((void**)&P->part, sizeof(double) * 16 * Nx);
     alloc((void**)&P->rho, sizeof(double) * Nx);
     alloc((void**)&P->E_self, sizeof(float) * Nx);
     alloc((void**)&P->feq_tab, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512));   // + padding read (not used) by osv2_kernel
@@ -710,6 +713,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
                  P->os2x_lpi = value; P->os2x_occ = 0; P->os3x_occ = 0; break;
         case 19: if (value < 32 || value > 320 || value % 32) return VOG_EINVAL; P->os2x_thr = value; P->os2x_occ = 0; break;
         case 20: if (value < 0) return VOG_EINVAL; P->os2v_gpc = value; break;
+        case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
         case 21: if (value < 0 || value > 3) return VOG_EINVAL; P->os2x_direct = value; P->os3x_occ = 0; break;
         case 22: if (value < 0 || value > 2) return VOG_EINVAL; P->os2v_direct = value; break;
         default: return VOG_EINVAL;
