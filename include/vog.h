@@ -129,7 +129,9 @@ int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   21     x variant: 0 = landing through shared memory, 1 = direct register loads with CTA barriers, 2 = raw-line
  *          landing of the next line group, 3 = warp-private with the split barrier (default);
  *   22     v variant: 0 = per-lane landing, 1 = direct register loads, 2 = coalesced landing of the strip's rows (default);
- *   24     density kernel: row slabs per column group (power of two, 1..16, at least 32 rows each).
+ *   24     density kernel: row slabs per column group (power of two, 1..16, at least 32 rows each);
+ *   25     block geometry of the default overlap-save kernels: 1 = 232 kept samples, 8 + 16 discarded (Lagrange
+ *          plans only, their default), 0 = 224 kept, 16 + 16 discarded (the cubic spline's).
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

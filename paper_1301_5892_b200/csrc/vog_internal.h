@@ -105,10 +105,10 @@ cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cu
 int osx2_occupancy(int threads, size_t smem);
 cudaError_t osx3_launch(const OsArgs& a, int mode, int grid, int threads, size_t smem, cudaStream_t st);
 int osx3_occupancy(int mode, int threads, size_t smem);
-cudaError_t osx5_launch(const OsArgs& a, bool inplace, int grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t osx5_launch(const OsArgs& a, bool inplace, int geom, int grid, int threads, size_t smem, cudaStream_t st);
 int osx5_occupancy(int threads, size_t smem);
 cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
-cudaError_t osv4_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
+cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st);
 
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
 typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,

@@ -344,6 +344,7 @@ struct vog_plan_s {
     int osv_np_log, osv_thr, osv_rb, osv_gpc;
     int os_gen;                            // 2 = pair kernels of vog_os2.cuh (default), 1 = even/odd kernels of vog_os.cuh
     int os2x_lpi, os2x_thr, os2x_occ, os2v_gpc;
+    int os_geom;                           // block geometry of the default kernels: 1 = Lagrange (232 kept, 8 + 16 discarded), 0 = spline (224, 16 + 16)
     int os2v_direct;                       // v kernel: 2 = coalesced raw-row landing (osv4_kernel, default), 1 = register landing (osv3), 0 = per-lane landing (osv2)
     int os2x_direct, os3x_occ;             // x: register-landing kernel (osx3_kernel) when a line group fits one round of 320 threads
     int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
@@ -546,13 +547,15 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 0; P->osv_gpc = 0;
         // pair kernels: 16 items per pair and phase; lines per iteration so that one round of <= 320 threads
         // covers the items (8192: 19 pairs = 304 items; 2048: 4 lines x 5 pairs = 320)
-        const int npx = (nbx + 1) / 2;
+        const int Vx = p->kind == VOG_LAGRANGE ? 232 : OS_V;
+        const int npx = ((Nx + Vx - 1) / Vx + 1) / 2;
         int l2 = 320 / (16 * npx);
         if (l2 < 1) l2 = 1;
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         int thr = ((16 * npx * l2 + 31) / 32) * 32;
         if (thr > 320) thr = 320;
         P->os2x_direct = 3; P->os3x_occ = 0; P->os2v_direct = 2;
+        P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
         P->os_gen = 2; P->os2x_lpi = l2; P->os2x_thr = thr; P->os2x_occ = 0; P->os2v_gpc = 0;
     }
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
@@ -713,6 +716,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
                  P->os2x_lpi = value; P->os2x_occ = 0; P->os3x_occ = 0; break;
         case 19: if (value < 32 || value > 320 || value % 32) return VOG_EINVAL; P->os2x_thr = value; P->os2x_occ = 0; break;
         case 20: if (value < 0) return VOG_EINVAL; P->os2v_gpc = value; break;
+        case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
         case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
         case 21: if (value < 0 || value > 3) return VOG_EINVAL; P->os2x_direct = value; P->os3x_occ = 0; break;
         case 22: if (value < 0 || value > 2) return VOG_EINVAL; P->os2v_direct = value; break;
@@ -804,7 +808,9 @@ static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
     std::memset(&a, 0, sizeof(a));
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nx;
-    a.nb = (Nx + OS_V - 1) / OS_V;
+    const int geom = P->os2x_direct == 3 ? P->os_geom : 0;        // (the other variants use the spline geometry)
+    const int V = geom ? 232 : OS_V;
+    a.nb = (Nx + V - 1) / V;
     a.np = (a.nb + 1) / 2;
     a.inv_np = (65536u + (unsigned)a.np - 1u) / (unsigned)a.np;
     a.lam = P->os_lam_x; a.tw = P->os_twv;
@@ -824,7 +830,7 @@ static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
         int grid = P->os3x_occ * P->n_sm;
         if (grid > a.n_groups) grid = a.n_groups;
         P->launches++;
-        return osx5_launch(a, src == dst, grid, thr, sm5, P->st);
+        return osx5_launch(a, src == dst, geom, grid, thr, sm5, P->st);
     }
     if (P->os2x_direct && 16 * a.np * a.lpi <= 320) {
         const int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
@@ -854,7 +860,9 @@ static cudaError_t run_osv2(vog_plan_s* P, const float* src, float* dst, bool so
     std::memset(&a, 0, sizeof(a));
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
-    a.nb = (Nv + OS_V - 1) / OS_V;
+    const int geom = P->os2v_direct == 2 ? P->os_geom : 0;
+    const int V = geom ? 232 : OS_V;
+    a.nb = (Nv + V - 1) / V;
     a.np = (a.nb + 1) / 2;
     a.lam = P->os_lam_v; a.tw = P->os_twv;
     a.ng = source ? P->p.feq.n : 0;
@@ -878,7 +886,7 @@ static cudaError_t run_osv2(vog_plan_s* P, const float* src, float* dst, bool so
     dim3 grid(strips, (a.np + gpc - 1) / gpc);
     P->launches++;
     if (P->os2v_direct == 2)
-        return osv4_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
+        return osv4_launch(a, geom, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
     if (P->os2v_direct) return osv3_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 4 * 32 * 16, P->st);
     return osv2_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
 }

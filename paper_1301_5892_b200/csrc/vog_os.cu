@@ -163,12 +163,18 @@ cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cu
     return cudaGetLastError();
 }
 
-cudaError_t osv4_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
+cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st)
 {
-    static size_t cur = 0;
-    cudaError_t e = set_smem((const void*)osv4_kernel, smem, &cur);
-    if (e != cudaSuccess) return e;
-    osv4_kernel<<<grid, threads, smem, st>>>(a);
+    static size_t cur[2] = {0, 0};
+    if (geom) {
+        cudaError_t e = set_smem((const void*)osv4_kernel<232, 8>, smem, &cur[1]);
+        if (e != cudaSuccess) return e;
+        osv4_kernel<232, 8><<<grid, threads, smem, st>>>(a);
+    } else {
+        cudaError_t e = set_smem((const void*)osv4_kernel<OS_V, OS_H>, smem, &cur[0]);
+        if (e != cudaSuccess) return e;
+        osv4_kernel<OS_V, OS_H><<<grid, threads, smem, st>>>(a);
+    }
     return cudaGetLastError();
 }
 
@@ -205,24 +211,32 @@ int osx3_occupancy(int mode, int threads, size_t smem)
     return nb;
 }
 
-// warp-private x kernel; inplace selects the split-mbarrier variant (src may equal dst)
-cudaError_t osx5_launch(const OsArgs& a, bool inplace, int grid, int threads, size_t smem, cudaStream_t st)
+// warp-private x kernel; inplace selects the split-mbarrier variant (src may equal dst); geom 1 = the Lagrange
+// block geometry (232 kept, 8 + 16 discarded), 0 = the spline's (224, 16 + 16)
+template <bool INPLACE, int V, int HLO>
+static cudaError_t osx5_launch_t(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st, size_t* cur)
 {
-    static size_t cur[2] = {0, 0};
-    const void* fn = inplace ? (const void*)osx5_kernel<true> : (const void*)osx5_kernel<false>;
-    cudaError_t e = set_smem(fn, smem, &cur[inplace ? 1 : 0]);
+    cudaError_t e = set_smem((const void*)osx5_kernel<INPLACE, V, HLO>, smem, cur);
     if (e != cudaSuccess) return e;
-    if (inplace) osx5_kernel<true><<<grid, threads, smem, st>>>(a);
-    else osx5_kernel<false><<<grid, threads, smem, st>>>(a);
+    osx5_kernel<INPLACE, V, HLO><<<grid, threads, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+cudaError_t osx5_launch(const OsArgs& a, bool inplace, int geom, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    static size_t cur[4] = {0, 0, 0, 0};
+    if (geom) return inplace ? osx5_launch_t<true, 232, 8>(a, grid, threads, smem, st, &cur[0])
+                             : osx5_launch_t<false, 232, 8>(a, grid, threads, smem, st, &cur[1]);
+    return inplace ? osx5_launch_t<true, OS_V, OS_H>(a, grid, threads, smem, st, &cur[2])
+                   : osx5_launch_t<false, OS_V, OS_H>(a, grid, threads, smem, st, &cur[3]);
 }
 
 int osx5_occupancy(int threads, size_t smem)
 {
     static size_t cur = 0;
-    if (set_smem((const void*)osx5_kernel<true>, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (set_smem((const void*)osx5_kernel<true, OS_V, OS_H>, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx5_kernel<true>, threads, smem) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx5_kernel<true, OS_V, OS_H>, threads, smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }

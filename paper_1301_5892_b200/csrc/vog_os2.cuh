@@ -218,6 +218,54 @@ __global__ void __launch_bounds__(TMAX, MINB) osx2_kernel(const OsArgs a)
 // iteration, so the scratch is only the exchange buffer between the phases (4 instead of 6 shared accesses
 // per sample), and the 15 twiddles W^{t q} of a thread (t is fixed) are products of 4 register-resident
 // powers W^t, W^2t, W^4t, W^8t instead of 15 shared loads per pass.
+// ---------------------------------------------------------------------------------------------
+// Block geometry of the default kernels (osx5_kernel, osv4_kernel) as template parameters: V kept samples per
+// block, HLO discarded on the left, 256 - V - HLO on the right.  The cubic spline needs 16 + 16 (its circulant
+// row decays like 0.268^|j|: section 6.1 of DESIGN.md), i.e. (224, 16); a Lagrange stencil of degree <= 17
+// reaches 8 cells to the left and 9 to the right, so (232, 8) is exact for it and needs 5 % fewer
+// blocks at 8192 (36 instead of 37) and 10 % fewer at 4096.
+// Thread t of an inverse-pass item holds samples n = t + 16 m, m = 0..15; sample n is kept iff HLO <= n < HLO + V.
+template <int V, int HLO, int M>
+struct KeptM {
+    static constexpr int lo = HLO - 16 * M, hi = HLO + V - 16 * M;     // kept iff lo <= t < hi
+    static constexpr bool none = hi <= 0 || lo >= 16;
+    static constexpr bool all = lo <= 0 && hi >= 16;
+    static __device__ __forceinline__ bool kept(const int t) { return all || (!none && t >= lo && t < hi); }
+};
+
+// x: store the kept samples of both blocks of a pair.  o = line + (first cell of block A) + t - HLO, i.e. the cell
+// of sample n = t; c = that cell index; cells >= N do not exist (checked only when !full).
+template <int V, int HLO, int M = 0>
+__device__ __forceinline__ void os2_store_x(float* __restrict__ o, const int c, const int N, const int t,
+                                            const bool full, const float2* x)
+{
+    if constexpr (M < 16) {
+        using K = KeptM<V, HLO, M>;
+        if constexpr (!K::none) {
+            const bool k = K::kept(t);
+            if (k && (full || c + 16 * M < N)) __stcs(o + 16 * M, x[M].x);
+            if (k && (full || c + 16 * M + V < N)) __stcs(o + 16 * M + V, x[M].y);
+        }
+        os2_store_x<V, HLO, M + 1>(o, c, N, t, full, x);
+    }
+}
+
+// v: the same along rows (row stride Nx); po = column + (row of sample n = t) * Nx, r = that row.
+template <int V, int HLO, int M = 0>
+__device__ __forceinline__ void os2_store_v(float* __restrict__ po, const size_t Nx, const int r, const int Nv,
+                                            const int t, const bool full, const float2* x)
+{
+    if constexpr (M < 16) {
+        using K = KeptM<V, HLO, M>;
+        if constexpr (!K::none) {
+            const bool k = K::kept(t);
+            if (k && (full || r + 16 * M < Nv)) __stcs(po + (size_t)(16 * M) * Nx, x[M].x);
+            if (k && (full || r + 16 * M + V < Nv)) __stcs(po + (size_t)(16 * M + V) * Nx, x[M].y);
+        }
+        os2_store_v<V, HLO, M + 1>(po, Nx, r, Nv, t, full, x);
+    }
+}
+
 struct Tw4 { float2 b1, b2, b4, b8; };
 
 // Calls f(q, W^{t q}) for q = 1..15 (q a compile-time constant of each call), building the powers from the four
@@ -250,16 +298,17 @@ __device__ __forceinline__ void os2_tw_each(const Tw4& w, F&& f)
     f(QC<12>(), cmul(w.b4, w.b8));
 }
 
+template <int V = OS_V>
 __device__ __forceinline__ void osx3_load(float2* x, const float* __restrict__ gl, const int c0, const int mask)
 {
-    if (c0 + OS_V + 241 <= mask + 1) {                 // the two windows do not wrap
+    if (c0 + V + 241 <= mask + 1) {                    // the two windows do not wrap
         const float* p = gl + c0;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) x[k] = make_float2(__ldg(p + 16 * k), __ldg(p + 16 * k + OS_V));
+        for (int k = 0; k < 16; ++k) x[k] = make_float2(__ldg(p + 16 * k), __ldg(p + 16 * k + V));
     } else {
 #pragma unroll
         for (int k = 0; k < 16; ++k)
-            x[k] = make_float2(__ldg(gl + ((c0 + 16 * k) & mask)), __ldg(gl + ((c0 + 16 * k + OS_V) & mask)));
+            x[k] = make_float2(__ldg(gl + ((c0 + 16 * k) & mask)), __ldg(gl + ((c0 + 16 * k + V) & mask)));
     }
 }
 
@@ -414,7 +463,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, const unsigne
 }
 }  // namespace os2
 
-template <bool INPLACE>
+template <bool INPLACE, int V, int HLO>
 __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -456,7 +505,7 @@ __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
                     os2::cp_async16(reinterpret_cast<float4*>(lamL) + i, reinterpret_cast<const float4*>(lamG) + i);
                 float2 x[16];
                 const int b = __float_as_int(__ldg(&lamG[129].x));
-                osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
+                osx3_load<V>(x, a.src + (size_t)line * N, (pp * (2 * V) - HLO + b + t) & mask, mask);
                 dft_dif<16, 1>(x);
                 sA[0] = x[0];
                 os2_tw_each(w, [&](auto qc, const float2 y) {
@@ -492,7 +541,6 @@ __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
             const int pr = it >> 4;
             const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;
             const float2* const sA = scr + pr * os2::XPAIR + t;
-            const int o0 = pp * os2::PW + t;
             float2 x[16];
             x[0] = sA[0];
             os2_tw_each(w, [&](auto qc, const float2 y) {
@@ -501,20 +549,8 @@ __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
             });
             idft_dit<16, 1>(x);
             if (g * lpi + l < a.n_lines) {
-                float* const o = a.dst + (size_t)(g * lpi + l) * N + o0;
-                if ((pp + 1) * os2::PW <= N) {
-#pragma unroll
-                    for (int m = 1; m < 15; ++m) {
-                        __stcs(o + 16 * (m - 1), x[m].x);
-                        __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
-                    }
-                } else {
-#pragma unroll
-                    for (int m = 1; m < 15; ++m) {
-                        if (o0 + 16 * (m - 1) < N) __stcs(o + 16 * (m - 1), x[m].x);
-                        if (o0 + 16 * (m - 1) + OS_V < N) __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
-                    }
-                }
+                const int c = pp * (2 * V) + t - HLO;          // cell of sample n = t of block A
+                os2_store_x<V, HLO>(a.dst + (size_t)(g * lpi + l) * N + c, c, N, t, (pp + 1) * (2 * V) <= N, x);
             }
         }
     }
@@ -556,37 +592,41 @@ __device__ __forceinline__ void osv2_land(float* __restrict__ pw, const float* _
     }
 }
 
-// delta-f source on the kept samples of one item: x[m].x += f_eq,g(v_j)(e^{X_j} - 1) at rows
-// j = row0 + 16 (m - 1), x[m].y the same at rows j + OS_V, with X_j = c s (2 (v_j - mu) - s) affine in j.  Along rows
-// 16 apart expm1 obeys e' = e R + r (R = e^h, r = expm1(h), h = 32 c s dv); the recurrence starts in the
-// middle (m = 8) and runs both ways (RS[g] = (R, r, 1/R, expm1(-h)) per lane), so at most 7 steps accumulate.
-// The f_eq table has 512 floats of padding: rows >= Nv are read but never stored.
+// delta-f source on the samples of one item: x[m].x += f_eq,g(v_j)(e^{X_j} - 1) at rows j = r0 + 16 m
+// (r0 = row of sample n = t of block A), x[m].y the same at rows j + V, with X_j = c s (2 (v_j - mu) - s) affine in j.
+// Along rows 16 apart expm1 obeys e' = e R + r (R = e^h, r = expm1(h), h = 32 c s dv); the recurrence starts in
+// the middle (m = 8) and runs both ways (RS[g] = (R, r, 1/R, expm1(-h)) per lane), so at most 8 steps accumulate.
+// Samples that are not kept (m = 15, and m = 0 unless HLO < 16) are skipped or harmlessly updated.  The f_eq table
+// has 512 floats of padding: rows >= Nv are read but never stored; rows < 0 (m = 0 of the first pair) are clamped.
+template <int V, int HLO>
 __device__ __forceinline__ void osv2_source(float2* x, const OsArgs& a, const float4* __restrict__ RS, const int lane,
-                                            const int row0, const float ssh)
+                                            const int r0, const float ssh)
 {
+    constexpr int M0 = HLO < 16 ? 0 : 1;
 #pragma unroll 1
     for (int g = 0; g < a.ng; ++g) {
         const float cgs = a.cg4[g] * ssh;
-        const float* __restrict__ fa = a.feq_tab + g * a.Nv + row0;
+        const float* __restrict__ fa = a.feq_tab + g * a.Nv + r0;
         const float u0 = __ldg(a.vmu_tab + g * a.Nv);                          // v_0 - mu_g
         const float4 Rr = RS[g * 32 + lane];
-        const float ea8 = expm1f(cgs * (2.0f * fmaf((float)(row0 + 112), a.dvf, u0) - ssh));
-        const float eb8 = expm1f(cgs * (2.0f * fmaf((float)(row0 + 112 + OS_V), a.dvf, u0) - ssh));
+        const float ea8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128), a.dvf, u0) - ssh));
+        const float eb8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128 + V), a.dvf, u0) - ssh));
         float ea = ea8, eb = eb8;
 #pragma unroll
         for (int m = 8; m < 15; ++m) {
-            x[m].x = fmaf(__ldg(fa + 16 * (m - 1)), ea, x[m].x);
-            x[m].y = fmaf(__ldg(fa + 16 * (m - 1) + OS_V), eb, x[m].y);
+            x[m].x = fmaf(__ldg(fa + 16 * m), ea, x[m].x);
+            x[m].y = fmaf(__ldg(fa + 16 * m + V), eb, x[m].y);
             ea = fmaf(ea, Rr.x, Rr.y);
             eb = fmaf(eb, Rr.x, Rr.y);
         }
         ea = ea8; eb = eb8;
 #pragma unroll
-        for (int m = 7; m >= 1; --m) {
+        for (int m = 7; m >= M0; --m) {
             ea = fmaf(ea, Rr.z, Rr.w);
             eb = fmaf(eb, Rr.z, Rr.w);
-            x[m].x = fmaf(__ldg(fa + 16 * (m - 1)), ea, x[m].x);
-            x[m].y = fmaf(__ldg(fa + 16 * (m - 1) + OS_V), eb, x[m].y);
+            const int ia = (m == 0) ? max(-r0, 0) : 16 * m;      // (row r0 < 0 exists only as a discarded sample)
+            x[m].x = fmaf(__ldg(fa + ia), ea, x[m].x);
+            x[m].y = fmaf(__ldg(fa + 16 * m + V), eb, x[m].y);
         }
     }
 }
@@ -668,7 +708,7 @@ __global__ void __launch_bounds__(512, 2) osv2_kernel(const OsArgs a)
             if (p + 1 < p1) osv2_land(pw, col, Nx, vmask, (p + 1) * os2::PW - OS_H + b + wid);
             idft_dit<16, 1>(x);
             const int row0 = p * os2::PW + wid;    // row of m = 1, block A
-            if (a.ng > 0) osv2_source(x, a, RS, lane, row0, ssh);
+            if (a.ng > 0) osv2_source<OS_V, OS_H>(x, a, RS, lane, row0 - 16, ssh);
             float* po = ocol + (size_t)row0 * Nx;
             const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
             if (p * os2::PW + os2::PW <= Nv) {
@@ -792,7 +832,7 @@ __global__ void __launch_bounds__(512, 2) osv3_kernel(const OsArgs a)
             });
             idft_dit<16, 1>(x);
             const int row0 = p * os2::PW + wid;    // row of m = 1, block A
-            if (a.ng > 0) osv2_source(x, a, RS, lane, row0, ssh);
+            if (a.ng > 0) osv2_source<OS_V, OS_H>(x, a, RS, lane, row0 - 16, ssh);
             float* po = ocol + (size_t)row0 * Nx;
             const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
             if (p * os2::PW + os2::PW <= Nv) {
@@ -824,10 +864,7 @@ __global__ void __launch_bounds__(512, 2) osv3_kernel(const OsArgs a)
 // any per-lane row offset is conflict-free.  The raw rows (480 + R, R = spread of the shifts in the strip,
 // <= 32) share the 64 KB of the exchange buffer, so two more barriers separate "raw read" from "exchange
 // written".  Strips whose shifts spread over more than 32 rows fall back to the per-lane fetch (same layout).
-namespace os2 {
-constexpr int RMAX = 32;
-}
-
+template <int V, int HLO>
 __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -862,9 +899,10 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
         dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
     }
     const int R = dmax - dmin;
-    const bool gather = R > os2::RMAX;             // uniform over the CTA (every warp sees the same 32 columns)
+    constexpr int RMAX = 512 - OS_LB - V;          // the raw rows (V + 256 + R) share the 512 rows of the exchange buffer
+    const bool gather = R > RMAX;             // uniform over the CTA (every warp sees the same 32 columns)
     const int db = gather ? 0 : d - dmin;          // this lane's row offset inside the raw window
-    const int base = gather ? b : b0 + dmin;       // first raw row = pair start - OS_H + base
+    const int base = gather ? b : b0 + dmin;       // first raw row = pair start - HLO + base
     if (a.ng > 0 && tid < 4 * W) {
         const int g = tid >> 5;
         const float h = 32.0f * (g < a.ng ? a.cg4[g] : 0.0f) * ssh * a.dvf;
@@ -875,11 +913,11 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
     const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
     float2* const own = scr + wid * W + lane;                                 // position t = wid, interleaved
     constexpr int PS2 = 16 * W;                                               // float2 between positions 16 apart
-    const int nrows = OS_V + OS_LB + (gather ? 0 : R);                        // 480 + R
+    const int nrows = V + OS_LB + (gather ? 0 : R);
 
     for (int p = p0; p < p1; ++p) {
         // ---- landing: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
-        const int rs = p * os2::PW - OS_H + base;
+        const int rs = p * (2 * V) - HLO + base;
         if (!gather) {
             const float* const src = a.src + c0;
             for (int c = tid; c < nrows * 8; c += T) {
@@ -896,7 +934,7 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
             float2 x[16];
             const float* const rp = raw + (wid + db) * W + lane;
 #pragma unroll
-            for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + OS_V) * W]);
+            for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + V) * W]);
             __syncthreads();                       // raw rows all read before the exchange buffer is written
             const float2* const twp = twS + wid;
             dft_dif<16, 1>(x);
@@ -924,25 +962,9 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
 #pragma unroll
             for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(own[q * PS2], twp[(q - 1) * 16]);
             idft_dit<16, 1>(x);
-            const int row0 = p * os2::PW + wid;    // row of m = 1, block A
-            if (a.ng > 0) osv2_source(x, a, RS, lane, row0, ssh);
-            float* po = ocol + (size_t)row0 * Nx;
-            const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
-            if (p * os2::PW + os2::PW <= Nv) {
-#pragma unroll
-                for (int m = 1; m < 15; ++m) {
-                    __stcs(po, x[m].x);
-                    __stcs(po + sV, x[m].y);
-                    po += s16;
-                }
-            } else {
-#pragma unroll
-                for (int m = 1; m < 15; ++m) {
-                    if (row0 + 16 * (m - 1) < Nv) __stcs(po, x[m].x);
-                    if (row0 + 16 * (m - 1) + OS_V < Nv) __stcs(po + sV, x[m].y);
-                    po += s16;
-                }
-            }
+            const int r0 = p * (2 * V) + wid - HLO;        // row of sample n = t = wid of block A
+            if (a.ng > 0) osv2_source<V, HLO>(x, a, RS, lane, r0, ssh);
+            os2_store_v<V, HLO>(ocol + (ptrdiff_t)r0 * Nx, (size_t)Nx, r0, Nv, wid, (p + 1) * (2 * V) <= Nv, x);
         }
         if (p + 1 < p1) __syncthreads();           // the exchange buffer is read before the next raw rows land
     }

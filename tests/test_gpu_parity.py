@@ -229,7 +229,7 @@ def test_x_pair_kernel_variants_in_place_with_large_shifts(torch, vog, oracle, m
     plan.destroy()
 
 
-@pytest.mark.parametrize("which,value", [(17, 1), (22, 0), (22, 1), (20, 2), (20, 3), (18, 2), (19, 160)])
+@pytest.mark.parametrize("which,value", [(17, 1), (22, 0), (22, 1), (20, 2), (20, 3), (18, 2), (19, 160), (25, 0), (24, 2)])
 def test_kernel_generation_and_shape_overrides_keep_parity(torch, vog, oracle, which, value):
     """The even/odd kernels (generation 1), the register-landing v kernel and other launch shapes of the pair
     kernels compute the same advection, delta-f source included."""
@@ -247,12 +247,14 @@ def test_kernel_generation_and_shape_overrides_keep_parity(torch, vog, oracle, w
     plan.destroy()
     g = inputs.uniform_grid(2048, 64, seed=inputs.SEED + 5)
     bx = _shifts(64, 53)
-    plan = vog.Plan(2048, 64, 1.0, -1.0, 1.0, SPL, 3)
-    plan.tune(which, value)
-    gd = _dev(torch, g)
-    plan.shift_x(gd, _dev(torch, bx))
-    _check(gd.cpu().numpy(), oracle.shift_x(g, bx, SPL, 3), 1.0)
-    plan.destroy()
+    for kind, order in ((SPL, 3), (LAG, 17)):
+        plan = vog.Plan(2048, 64, 1.0, -1.0, 1.0, kind, order)
+        if not (which == 25 and kind == SPL):       # (the spline has one block geometry only)
+            plan.tune(which, value)
+        gd = _dev(torch, g)
+        plan.shift_x(gd, _dev(torch, bx))
+        _check(gd.cpu().numpy(), oracle.shift_x(g, bx, kind, order), 1.0)
+        plan.destroy()
 
 
 @pytest.mark.parametrize("lo,hi", [(-8.0, 8.0), (-20.0, 12.0), (-900.0, 900.0)])
