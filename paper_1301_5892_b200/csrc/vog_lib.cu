@@ -822,7 +822,7 @@ static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
         int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
         if (thr > 320) thr = ((((16 * a.np * a.lpi + 1) / 2) + 31) / 32) * 32;      // two rounds
         if (thr > 320) thr = 320;
-        const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8) + (size_t)(thr / 16) * OS_LAMW * 8 + 16;
+        const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8) + (size_t)(a.lpi == 1 ? thr / 32 : thr / 16) * OS_LAMW * 8 + 16;
         if (P->os3x_occ == 0) {
             P->os3x_occ = osx5_occupancy(thr, sm5);
             if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;

@@ -470,15 +470,19 @@ __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
     const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
     const int tid = threadIdx.x, T = blockDim.x, t = tid & 15, hw = tid >> 4;
     float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
-    float2* const lamP = scr + ptot * os2::XPAIR;                       // one table row per half-warp (private)
-    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(lamP + (T >> 4) * OS_LAMW);
+    // one private copy of the line's table row per half-warp, or per warp when a group is one line (then both
+    // pairs of a warp read the same copy: broadcast, and half the shared memory)
+    const bool one_line = lpi == 1;
+    float2* const lamP = scr + ptot * os2::XPAIR;
+    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(lamP + (one_line ? (T >> 5) : (T >> 4)) * OS_LAMW);
     const int N = a.N, mask = N - 1;
     Tw4 w;
     w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
     w.b2 = __ldg(a.tw + 16 + t);
     w.b4 = __ldg(a.tw + 3 * 16 + t);
     w.b8 = __ldg(a.tw + 7 * 16 + t);
-    float2* const lamL = lamP + hw * OS_LAMW;
+    float2* const lamL = lamP + (one_line ? (hw >> 1) : hw) * OS_LAMW;
+    const int cp0 = one_line ? (tid & 31) : t, cps = one_line ? 32 : 16;      // this thread's chunks of the copy
     if constexpr (INPLACE) {
         if (tid == 0) os2::mbar_init(bar, T >> 5);
         __syncthreads();
@@ -498,11 +502,15 @@ __global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
             float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
             float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
             // ---- pass A straight from global memory
+            // the (half-)warp's copy of the line's symbol table lands behind pass A (its previous contents were
+            // last read by these threads before the __syncwarp() that closed their last middle stage); with one
+            // line per group all 32 lanes copy, the inactive ones of the last warp included
+            if (active || one_line) {
+                const float2* __restrict__ lamC = one_line ? a.lam + (size_t)min(g, a.n_lines - 1) * OS_LAMW : lamG;
+                for (int i = cp0; i < OS_LAMW / 2; i += cps)
+                    os2::cp_async16(reinterpret_cast<float4*>(lamL) + i, reinterpret_cast<const float4*>(lamC) + i);
+            }
             if (active) {
-                // the half-warp's copy of the line's symbol table lands behind pass A (its previous contents
-                // were last read by these 16 threads before the __syncwarp() that closed their last middle stage)
-                for (int i = t; i < OS_LAMW / 2; i += 16)
-                    os2::cp_async16(reinterpret_cast<float4*>(lamL) + i, reinterpret_cast<const float4*>(lamG) + i);
                 float2 x[16];
                 const int b = __float_as_int(__ldg(&lamG[129].x));
                 osx3_load<V>(x, a.src + (size_t)line * N, (pp * (2 * V) - HLO + b + t) & mask, mask);
