@@ -331,6 +331,19 @@ def sweep(torch, vog, stream, peak, sizes=(2048, 8192), kinds=((0, 17), (0, 3), 
                 gbs = 8.0 * N * N / (med * 1e-3) / 1e9
                 row["v_out_of_place"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak,
                                          "note": "vog_shift_v_to: table setup + kernel, src -> dst"}
+                if N >= 1024:
+                    # control: the loads and stores of the x kernel without the transform (memory-system floor)
+                    for _ in range(3):
+                        plan.probe_x_memory_pattern(f, g)
+                    times = []
+                    for _ in range(10):
+                        e0.record(stream); plan.probe_x_memory_pattern(f, g); e1.record(stream)
+                        stream.synchronize()
+                        times.append(e0.elapsed_time(e1))
+                    med = float(np.median(times))
+                    gbs = 8.0 * N * N / (med * 1e-3) / 1e9
+                    row["x_memory_pattern"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak,
+                                               "note": "vog_probe_x_memory_pattern: the x kernel's loads and stores, no transform"}
                 del g
             for _ in range(2):
                 plan.step(f, 1e-3)

@@ -135,6 +135,12 @@ int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 
+/* Measurement probe, not part of the method: runs a kernel with exactly the global loads and stores of the
+ * x-advection kernel (Nx >= 1024, zero shift, Lagrange block geometry) and no transform, src_dev -> dst_dev
+ * (dst_dev != src_dev, Nx*Nv floats each; the cells a line's last block does not cover keep their value).  Its time
+ * is the memory-system floor of that access pattern (`bench.py --sweep-only` reports it as "x_memory_pattern"). */
+int vog_probe_x_memory_pattern(vog_plan_t plan, const float* src_dev, float* dst_dev);
+
 /* Number of kernels the library launched on this plan since creation (for accounting). */
 long long vog_launch_count(vog_plan_t plan);
 

@@ -97,6 +97,7 @@ struct OsSetupArgs {
 };
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st);
+cudaError_t os_mempattern_launch(const float* src, float* dst, int N, int n_lines, int grid, cudaStream_t st);
 cudaError_t osx_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
 cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
 int osx_occupancy(int threads, size_t smem);

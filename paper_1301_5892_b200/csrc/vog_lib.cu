@@ -1104,6 +1104,13 @@ extern "C" int vog_shift_v_to(vog_plan_t P, const float* src_dev, float* dst_dev
     return cuda_status(e);
 }
 
+extern "C" int vog_probe_x_memory_pattern(vog_plan_t P, const float* src_dev, float* dst_dev)
+{
+    if (!P || !src_dev || !dst_dev || src_dev == dst_dev || P->p.Nx < 1024) return VOG_EINVAL;
+    P->launches++;
+    return cuda_status(os_mempattern_launch(src_dev, dst_dev, P->p.Nx, P->p.Nv, 3 * P->n_sm, P->st));
+}
+
 extern "C" int vog_field(vog_plan_t P, const float* f_dev, float* E_dev)
 {
     if (!P || !f_dev || !E_dev) return VOG_EINVAL;

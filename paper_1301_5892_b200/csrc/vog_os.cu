@@ -104,6 +104,43 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
     }
 }
 
+// Measurement probe (vog_probe_x_memory_pattern): exactly the global loads and stores of osx5_kernel<., 232, 8> on
+// N-cell lines with zero shift -- 32 four-byte loads per thread in 64-byte runs per half-warp, the kept samples
+// stored with four-byte streaming stores -- and no transform.  Its time is the memory-system floor of that
+// access pattern (profiles/r1g2_pair_kernels.md, section 4).
+__global__ void __launch_bounds__(320, 3) os_mempattern_kernel(const float* __restrict__ src, float* __restrict__ dst,
+                                                               int N, int n_lines, int np)
+{
+    const int tid = threadIdx.x, t = tid & 15, mask = N - 1;
+    for (int line = blockIdx.x; line < n_lines; line += gridDim.x) {
+        const float* gl = src + (size_t)line * N;
+        float* go = dst + (size_t)line * N;
+        for (int pr = tid >> 4; pr < np; pr += blockDim.x >> 4) {
+            const int c0 = (pr * 464 - 8 + t) & mask;
+            float2 x[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k)
+                x[k] = make_float2(__ldg(gl + ((c0 + 16 * k) & mask)), __ldg(gl + ((c0 + 16 * k + 232) & mask)));
+            const int o = pr * 464 + t - 8;
+#pragma unroll
+            for (int m = 0; m < 15; ++m) {
+                const bool kept = m > 0 || t >= 8;
+                if (kept && o + 16 * m < N) __stcs(go + o + 16 * m, x[m].x);
+                if (kept && o + 16 * m + 232 < N) __stcs(go + o + 16 * m + 232, x[m].y);
+            }
+        }
+    }
+}
+
+cudaError_t os_mempattern_launch(const float* src, float* dst, int N, int n_lines, int grid, cudaStream_t st)
+{
+    const int np = ((N + 231) / 232 + 1) / 2;
+    int thr = ((16 * np + 31) / 32) * 32;
+    if (thr > 320) thr = 320;
+    os_mempattern_kernel<<<grid, thr, 0, st>>>(src, dst, N, n_lines, np);
+    return cudaGetLastError();
+}
+
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
 {
     os_setup_kernel<<<s.n_lines, 128, 0, st>>>(s);

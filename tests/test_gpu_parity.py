@@ -290,6 +290,20 @@ def test_shift_v_out_of_place_entry(torch, vog, oracle):
         plan.destroy()
 
 
+def test_memory_pattern_probe_moves_every_cell(torch, vog):
+    """The measurement probe (loads and stores of the x kernel, no transform, zero shift) is a copy of the grid."""
+    for Nx, Nv in ((2048, 64), (8192, 96)):
+        if Nv & (Nv - 1):
+            continue
+        f = inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + 95)
+        plan = vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, LAG, 17)
+        src, dst = _dev(torch, f), torch.zeros((Nv, Nx), device="cuda", dtype=torch.float32)
+        plan.probe_x_memory_pattern(src, dst)
+        torch.cuda.synchronize()
+        assert np.array_equal(dst.cpu().numpy(), f)
+        plan.destroy()
+
+
 # ------------------------------------------------------------------ full runs: energy history, configs 0-1
 def _gpu_history(torch, vog, cfg, steps):
     plan = vog.Plan.from_config(cfg)
