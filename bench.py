@@ -139,6 +139,7 @@ def main():
     ap.add_argument("--impl", default="vog")
     ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 advection sweep")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-concurrent", action="store_true", help="skip the 4-stream variant of the timed batch")
     ap.add_argument("--sweep-only", action="store_true", help="only the config-4 advection sweep (for profiling)")
     ap.add_argument("--sizes", default="512,2048,8192,16384", help="sweep grid sizes N (Nx=Nv=N), BASELINE.json config 4")
     ap.add_argument("--kinds", default="lag3,lag9,lag17,spline", help="sweep interpolators: lagN or spline")
@@ -205,6 +206,42 @@ def main():
     ms = multi.max_over_ranks(ms, device="cuda")
     value = multi.aggregate_throughput(BATCH * cells * args.steps, world, ms)
 
+    # ---- the same batch with the replicas spread over 4 plans on 4 streams (independent problems overlap: the
+    # single-CTA Poisson solve and the tails of one replica's kernels run under another replica's advections).
+    # Reported next to `value`, which stays the one-stream figure.
+    concurrent = None
+    if not args.no_concurrent:
+        NS = 4
+        streams = [torch.cuda.Stream() for _ in range(NS)]
+        plans = [vog.Plan.from_config(cfg, stream=st) for st in streams]
+        main = torch.cuda.current_stream()
+
+        def conc_step():
+            for i, fb in enumerate(batch):
+                plans[i % NS].step(fb, cfg.dt)
+
+        for _ in range(args.warmup):
+            conc_step()
+        sync_all()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(main)
+        for st in streams:
+            st.wait_event(c0)
+        for _ in range(args.steps):
+            conc_step()
+        for st in streams:
+            e = torch.cuda.Event()
+            e.record(st)
+            main.wait_event(e)
+        c1.record(main)
+        sync_all()
+        cms = multi.max_over_ranks(c0.elapsed_time(c1), device="cuda")
+        concurrent = {"streams": NS, "value": multi.aggregate_throughput(BATCH * cells * args.steps, world, cms),
+                      "unit": UNIT, "ms_per_step": cms / args.steps,
+                      "note": "same batch and steps, replicas round-robin over 4 plans/streams"}
+        for pl in plans:
+            pl.destroy()
+
     # ---- per-kernel timing of the same step on the same stream (roofline of the dominant kernel)
     # Each kernel type is launched back to back on all replicas of the batch between two events (no host
     # synchronisation inside), so the figure is the average launch duration in steady state.
@@ -264,7 +301,7 @@ def main():
         "config": {"workload": "strang_step_deltaf_2048x2048_lag17", "Nx": cfg.Nx, "Nv": cfg.Nv, "batch": BATCH,
                    "split": "x/2-field-v-x/2", "interp": "LAG17", "parallelism": "replicas x%d" % world,
                    "l2": "inputs larger than L2: batch of %d replicas = %d MiB, visited round-robin" % (BATCH, BATCH * 4 * cells >> 20)},
-        "gpu_launches": launches, "e2e": e2e, "roofline": roofline,
+        "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "concurrent": concurrent,
         "MA_paper_unit": 3.0 * value / 1e6,
     }
     if rank == 0:
