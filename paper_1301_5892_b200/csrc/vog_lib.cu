@@ -292,11 +292,16 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     // forward, decimation in frequency: position ((q0 r1 + q1) r2 + q2).. holds mode q0 + r0 (q1 + r1 (q2 + ..));
     // ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
     int lB = ilog2(Nx);
-    for (int p = 0; p < rx.np; ++p) {
-        if (rx.lr[p] == 3) poisson_pass<8, false>(z, Nx, lB, tws + rx.off[p], tid, T);
-        else poisson_pass<4, false>(z, Nx, lB, tws + rx.off[p], tid, T);
-        lB -= rx.lr[p];
-        __syncthreads();
+    // (the pass loops are unrolled so that rx.lr[p], rx.off[p] are read from the parameter bank; a run-time index
+    // made the compiler copy the struct to local memory: two dependent local loads at the head of every pass)
+#pragma unroll
+    for (int p = 0; p < 8; ++p) {
+        if (p < rx.np) {
+            if (rx.lr[p] == 3) poisson_pass<8, false>(z, Nx, lB, tws + rx.off[p], tid, T);
+            else poisson_pass<4, false>(z, Nx, lB, tws + rx.off[p], tid, T);
+            lB -= rx.lr[p];
+            __syncthreads();
+        }
     }
     for (int pos = tid; pos < Nx; pos += T) {
         const float2 v = z[pos];
@@ -304,11 +309,14 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
         z[pos] = make_float2(v.y * ik, -v.x * ik);         // (zr + i zi) / (i k), times 1/Nx
     }
     __syncthreads();
-    for (int p = rx.np - 1; p >= 0; --p) {
-        lB += rx.lr[p];
-        if (rx.lr[p] == 3) poisson_pass<8, true>(z, Nx, lB, tws + rx.off[p], tid, T);
-        else poisson_pass<4, true>(z, Nx, lB, tws + rx.off[p], tid, T);
-        __syncthreads();
+#pragma unroll
+    for (int p = 7; p >= 0; --p) {
+        if (p < rx.np) {
+            lB += rx.lr[p];
+            if (rx.lr[p] == 3) poisson_pass<8, true>(z, Nx, lB, tws + rx.off[p], tid, T);
+            else poisson_pass<4, true>(z, Nx, lB, tws + rx.off[p], tid, T);
+            __syncthreads();
+        }
     }
     for (int i = tid; i < Nx; i += T) {
         const float e = z[i].x;
