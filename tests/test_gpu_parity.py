@@ -304,6 +304,29 @@ def test_memory_pattern_probe_moves_every_cell(torch, vog):
         plan.destroy()
 
 
+def test_repeat_runs_are_bit_identical(torch, vog):
+    """No atomics on floats, fixed reduction orders, warp-private exchanges: the same call on the same input gives
+    the same bits every time (a race between a load and a store of an in-place line, or between the phases of a warp,
+    would show up here as run-to-run differences on this multi-wave grid with shifts of thousands of cells)."""
+    Nx, Nv = 8192, 1024
+    f0 = _dev(torch, inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + 97))
+    bx = _dev(torch, inputs.uniform_shifts(Nv, inputs.SEED + 98, lo=-3000.0, hi=3000.0))
+    bv = _dev(torch, inputs.uniform_shifts(Nx, inputs.SEED + 99, lo=-30.0, hi=30.0))
+    plan = vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, LAG, 17)
+    ref = {}
+    for it in range(4):
+        for name, fn in (("x", lambda f: plan.shift_x(f, bx)), ("v", lambda f: plan.shift_v(f, bv)),
+                         ("step", lambda f: plan.step(f, 1e-3))):
+            f = f0.clone()
+            fn(f)
+            torch.cuda.synchronize()
+            if it == 0:
+                ref[name] = f
+            else:
+                assert torch.equal(f, ref[name]), name
+    plan.destroy()
+
+
 # ------------------------------------------------------------------ full runs: energy history, configs 0-1
 def _gpu_history(torch, vog, cfg, steps):
     plan = vog.Plan.from_config(cfg)
