@@ -557,7 +557,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         // covers the items (8192: 19 pairs = 304 items; 2048: 4 lines x 5 pairs = 320)
         const int Vx = p->kind == VOG_LAGRANGE ? 232 : OS_V;
         const int npx = ((Nx + Vx - 1) / Vx + 1) / 2;
-        int l2 = 320 / (16 * npx);
+        int l2 = (p->kind == VOG_LAGRANGE ? 288 : 320) / (16 * npx);
         if (l2 < 1) l2 = 1;
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         int thr = ((16 * npx * l2 + 31) / 32) * 32;
@@ -827,9 +827,10 @@ static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
     a.n_groups = (Nv + a.lpi - 1) / a.lpi;
     const size_t smem = osx2_smem_bytes(a.lpi, a.np);
     if (P->os2x_direct == 3) {                     // warp-private kernel: any group size (rounds of thr items)
+        const int tmax = geom ? 288 : 320;         // (launch bounds of the two geometries: 72 / 64 registers)
         int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
-        if (thr > 320) thr = ((((16 * a.np * a.lpi + 1) / 2) + 31) / 32) * 32;      // two rounds
-        if (thr > 320) thr = 320;
+        if (thr > tmax) thr = ((((16 * a.np * a.lpi + 1) / 2) + 31) / 32) * 32;     // two rounds
+        if (thr > tmax) thr = tmax;
         const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8) + (size_t)(a.lpi == 1 ? thr / 32 : thr / 16) * OS_LAMW * 8 + 16;
         if (P->os3x_occ == 0) {
             P->os3x_occ = osx5_occupancy(thr, sm5);

@@ -464,7 +464,7 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, const unsigne
 }  // namespace os2
 
 template <bool INPLACE, int V, int HLO>
-__global__ void __launch_bounds__(320, 3) osx5_kernel(const OsArgs a)
+__global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
