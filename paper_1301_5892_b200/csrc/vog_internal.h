@@ -2,7 +2,38 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <utility>
+
 namespace vog {
+
+// ---- Programmatic dependent launch.  The kernels of a Strang step (S1-S9) run back to back on one stream and at
+// 2048^2 each lasts 7-23 us, so the drain / launch / ramp-up between two of them is a visible share of the step.
+// A kernel launched with launch_pdl() may become resident while its predecessor in the stream is still running;
+// it MUST call pdl_wait() before its first access to anything the predecessor reads or writes (the wait returns
+// when the predecessor grid has completed and its memory is visible), and calls pdl_launch_dependents() so
+// that its own successor may be staged early.  Work placed before pdl_wait() may only touch memory that is constant
+// for the life of the plan (twiddle tables).
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
+#endif
 
 // symbol variants compiled into the advection kernel
 enum { SYM_LAG_D1 = 0, SYM_LAG_D4 = 1, SYM_LAG_D8 = 2, SYM_SPLINE3 = 3, SYM_COUNT = 4 };

@@ -180,6 +180,8 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
     const int xl = lane & 7, rl = lane >> 3;
     const int col = blockIdx.x * 32 + xl * 4;
     const int j0 = blockIdx.y * rows_per_block;
+    pdl_wait();                                   // f comes from the advection before; part/rho/cnt are still in use
+    pdl_launch_dependents();
     double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
     const float* p = f + (size_t)(j0 + warp * 4 + rl) * Nx + col;
 #pragma unroll 4
@@ -283,10 +285,12 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     // Zero mean = mode 0 dropped below.  Before the conversion to fp32 a constant of the size of
     // the mean must still be removed in fp64 (in full-f mode rho ~ 1 carries a 1e-3 perturbation): rho[0]
     // serves as well as the mean (any constant only changes mode 0) and needs no reduction.
-    const double ref = rho[0];
-    for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);
+    for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);               // (plan constants: before the wait)
     if (tw_in_smem)
         for (int i = tid; i < tw_len; i += T) twsm[i] = __ldg(tw_g + i);
+    pdl_wait();                                   // rho comes from the density kernel
+    pdl_launch_dependents();
+    const double ref = rho[0];
     for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rho[i] - ref), 0.0f);
     __syncthreads();
     // forward, decimation in frequency: position ((q0 r1 + q1) r2 + q2).. holds mode q0 + r0 (q1 + r1 (q2 + ..));
@@ -1043,8 +1047,8 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
     dim3 grid(Nx / 32, P->nby);
-    density_partial_kernel<<<grid, 256, 0, P->st>>>(f, Nx, Nv, Nv / P->nby, P->part, dv, P->rho, P->dcnt);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = launch_pdl(density_partial_kernel, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part, dv,
+                               P->rho, P->dcnt);
     if (e != cudaSuccess) return e;
     static bool attr = false;
     if (!attr) {
@@ -1057,10 +1061,10 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
     if (T < 32) T = 32;
     const int tw_in_smem = Nx <= 8192;
     const size_t psmem = (sizeof(float2) + sizeof(float)) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
-    poisson_kernel<<<1, T, psmem, P->st>>>(Nx, P->prx, P->ptw_len, tw_in_smem, P->ptw, P->ikt, P->rho, P->E_self, E_out);
     P->launches += 2;
     P->E_valid = true;
-    return cudaGetLastError();
+    return launch_pdl(poisson_kernel, dim3(1), dim3(T), psmem, P->st, Nx, P->prx, P->ptw_len, tw_in_smem,
+                      (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->rho, P->E_self, E_out);
 }
 
 static cudaError_t ensure_recx(vog_plan_s* P, double dt)

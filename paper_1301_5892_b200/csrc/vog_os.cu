@@ -12,6 +12,8 @@ namespace vog {
 __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
 {
     const int l = blockIdx.x;
+    pdl_wait();                                   // E comes from the Poisson kernel; the tables may still be read
+    pdl_launch_dependents();
     double beta;
     float sshift = 0.0f;
     if (s.mode == 0) {
@@ -143,8 +145,7 @@ cudaError_t os_mempattern_launch(const float* src, float* dst, int N, int n_line
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
 {
-    os_setup_kernel<<<s.n_lines, 128, 0, st>>>(s);
-    return cudaGetLastError();
+    return launch_pdl(os_setup_kernel, dim3(s.n_lines), dim3(128), 0, st, s);
 }
 
 static cudaError_t set_smem(const void* fn, size_t smem, size_t* cur)
@@ -206,11 +207,11 @@ cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_
     if (geom) {
         cudaError_t e = set_smem((const void*)osv4_kernel<232, 8>, smem, &cur[1]);
         if (e != cudaSuccess) return e;
-        osv4_kernel<232, 8><<<grid, threads, smem, st>>>(a);
+        return launch_pdl(osv4_kernel<232, 8>, grid, dim3(threads), smem, st, a);
     } else {
         cudaError_t e = set_smem((const void*)osv4_kernel<OS_V, OS_H>, smem, &cur[0]);
         if (e != cudaSuccess) return e;
-        osv4_kernel<OS_V, OS_H><<<grid, threads, smem, st>>>(a);
+        return launch_pdl(osv4_kernel<OS_V, OS_H>, grid, dim3(threads), smem, st, a);
     }
     return cudaGetLastError();
 }
@@ -255,8 +256,7 @@ static cudaError_t osx5_launch_t(const OsArgs& a, int grid, int threads, size_t 
 {
     cudaError_t e = set_smem((const void*)osx5_kernel<INPLACE, V, HLO>, smem, cur);
     if (e != cudaSuccess) return e;
-    osx5_kernel<INPLACE, V, HLO><<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(osx5_kernel<INPLACE, V, HLO>, dim3(grid), dim3(threads), smem, st, a);
 }
 
 cudaError_t osx5_launch(const OsArgs& a, bool inplace, int geom, int grid, int threads, size_t smem, cudaStream_t st)

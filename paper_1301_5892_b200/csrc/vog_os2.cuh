@@ -487,6 +487,8 @@ __global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsA
         if (tid == 0) os2::mbar_init(bar, T >> 5);
         __syncthreads();
     }
+    pdl_wait();                                   // (the twiddles above are plan constants; tables and grid are not)
+    pdl_launch_dependents();
     unsigned parity = 0;
     // A line group has nitem items; thread tid takes items tid, tid + T, .. ("rounds"; one round when the group
     // fits the CTA, two for 16384-cell lines).  Per round: load, pass A, middle stage -- the pair's spectrum
@@ -886,13 +888,15 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
     const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
     const int c0 = blockIdx.x * W;
 
+    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);             // (plan constant: before the wait)
+    pdl_wait();                                   // the symbol tables and the source grid come from earlier kernels
+    pdl_launch_dependents();
     {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
         const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
         float4* dst4 = reinterpret_cast<float4*>(lamS);
         for (int i = tid; i < OS_LAMW * 16; i += T)
             os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
     }
-    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
     // integer shift (rows) and source shift of this lane's column
     const float2 e129 = __ldg(a.lam + (size_t)129 * Nx + c0 + lane);
     const int b = __float_as_int(e129.x);
