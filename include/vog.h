@@ -132,6 +132,9 @@ int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   24     density kernel: row slabs per column group (power of two, 1..16, at least 32 rows each);
  *   25     block geometry of the default overlap-save kernels: 1 = 232 kept samples, 8 + 16 discarded (Lagrange
  *          plans only, their default), 0 = 224 kept, 16 + 16 discarded (the cubic spline's).
+ *   26 = programmatic dependent launch of the plan's kernels: 1 = each kernel may be staged on the SMs while its
+ *        predecessor in the stream drains and waits for it on the device (default up to 8192 x 8192), 0 = plain
+ *        stream order.  Results are bit-identical either way.
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

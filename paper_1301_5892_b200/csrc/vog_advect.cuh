@@ -201,6 +201,8 @@ __global__ void __launch_bounds__(512) advect_kernel(const AdvectArgs a)
     const int Nx = a.Nx;
     const float2* __restrict__ tw = a.tw;
 
+    pdl_wait();                                   // shift records and grid come from the kernels before
+    pdl_launch_dependents();
     for (int i = tid; i < 2 * NL * REC_WORDS; i += T) recs[i] = a.rec[(size_t)line0 * REC_WORDS + i];
 
     // ---- forward pass 1: global -> registers -> shared

@@ -21,8 +21,7 @@ static cudaError_t launch_one(const AdvectArgs& a, int n_tiles, int threads, siz
         if (e != cudaSuccess) return e;
         smem_set = smem;
     }
-    kern<<<n_tiles, threads, smem, st>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(kern, dim3(n_tiles), dim3(threads), smem, st, a);
 }
 
 template <int N, bool VDIR>
@@ -56,8 +55,7 @@ static cudaError_t launch_x_one(const AdvectXArgs& a, int grid, int threads, siz
         if (e != cudaSuccess) return e;
         smem_set = smem;
     }
-    kern<<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(kern, dim3(grid), dim3(threads), smem, st, a);
 }
 
 template <int N, int SYM>

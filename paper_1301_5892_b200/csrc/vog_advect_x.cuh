@@ -426,6 +426,8 @@ __global__ void __launch_bounds__(128, 4) advect_x_kernel(const AdvectXArgs a)
         for (int i = tid; i < lpi * RCH; i += T) cp_async16(rdst + i, rsrc + i);
     };
 
+    pdl_wait();                                   // shift records and grid come from the kernels before
+    pdl_launch_dependents();
     int g = blockIdx.x;
     if (g < a.n_groups) prefetch(g, 0);
     cp_async_commit();

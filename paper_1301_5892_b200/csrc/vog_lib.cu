@@ -14,6 +14,15 @@
 
 namespace vog {
 
+// Programmatic dependent launch is a per-plan choice (vog_plan_tune(26, .)); the entry points of the C ABI set it
+// for the calling thread before they launch anything.
+static thread_local bool t_pdl = true;
+bool pdl_enabled()
+{
+    static const bool on = [] { const char* e = std::getenv("VOG_NO_PDL"); return !(e && e[0] == '1'); }();
+    return on && t_pdl;
+}
+
 advect_launch_fn advect_launcher(int N)
 {
     switch (N) {
@@ -73,6 +82,8 @@ struct SetupArgs {
 __global__ void shift_setup_kernel(const SetupArgs s)
 {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_wait();                                   // E comes from the Poisson kernel; the records may still be read
+    pdl_launch_dependents();
     if (l >= s.n_lines) return;
     double beta;
     float sshift = 0.0f;
@@ -124,6 +135,8 @@ __global__ void shift_setup_kernel(const SetupArgs s)
 __global__ void shift_setup_x_kernel(const SetupArgs s)
 {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_wait();
+    pdl_launch_dependents();
     if (l >= s.n_lines) return;
     double beta;
     if (s.mode == 0) beta = -(s.vmin + (double)l * s.dv) * s.dt / s.delta;
@@ -356,6 +369,7 @@ struct vog_plan_s {
     int osv_np_log, osv_thr, osv_rb, osv_gpc;
     int os_gen;                            // 2 = pair kernels of vog_os2.cuh (default), 1 = even/odd kernels of vog_os.cuh
     int os2x_lpi, os2x_thr, os2x_occ, os2v_gpc;
+    int pdl;                               // programmatic dependent launch of the step's kernels (default: grids up to 8192^2)
     int os_geom;                           // block geometry of the default kernels: 1 = Lagrange (232 kept, 8 + 16 discarded), 0 = spline (224, 16 + 16)
     int os2v_direct;                       // v kernel: 2 = coalesced raw-row landing (osv4_kernel, default), 1 = register landing (osv3), 0 = per-lane landing (osv2)
     int os2x_direct, os3x_occ;             // x: register-landing kernel (osx3_kernel) when a line group fits one round of 320 threads
@@ -570,6 +584,8 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
         P->os_gen = 2; P->os2x_lpi = l2; P->os2x_thr = thr; P->os2x_occ = 0; P->os2v_gpc = 0;
     }
+    // measured (profiles/r1h_pdl.md): 512^2 step -20 %, 2048^2 -15 %, 8192^2 +-0, 16384^2 +1.3 %
+    P->pdl = (long long)Nx * Nv <= (1ll << 26) ? 1 : 0;
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
     cudaError_t e = cudaSuccess;
@@ -732,6 +748,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
         case 21: if (value < 0 || value > 3) return VOG_EINVAL; P->os2x_direct = value; P->os3x_occ = 0; break;
         case 22: if (value < 0 || value > 2) return VOG_EINVAL; P->os2v_direct = value; break;
+        case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -774,9 +791,8 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
     s.vmin = P->p.vmin;
     s.E = E; s.Eext = Eext; s.beta = beta;
     s.rec = vdir ? P->rec_v : P->xrec;
-    if (vdir) shift_setup_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
-    else shift_setup_x_kernel<<<(s.n_lines + 127) / 128, 128, 0, P->st>>>(s);
-    return cudaGetLastError();
+    if (vdir) return launch_pdl(shift_setup_kernel, dim3((s.n_lines + 127) / 128), dim3(128), 0, P->st, s);
+    return launch_pdl(shift_setup_x_kernel, dim3((s.n_lines + 127) / 128), dim3(128), 0, P->st, s);
 }
 
 // ---- overlap-save launches (line length >= 1024)
@@ -1079,6 +1095,7 @@ static cudaError_t ensure_recx(vog_plan_s* P, double dt)
 extern "C" int vog_advect_x(vog_plan_t P, float* f_dev, double dt)
 {
     if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     cudaError_t e = ensure_recx(P, dt);
     if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
     return cuda_status(e);
@@ -1087,6 +1104,7 @@ extern "C" int vog_advect_x(vog_plan_t P, float* f_dev, double dt)
 extern "C" int vog_advect_v(vog_plan_t P, float* f_dev, const float* E_dev, double dt)
 {
     if (!P || !f_dev || !E_dev || !std::isfinite(dt)) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     cudaError_t e = run_setup(P, true, 1, dt, E_dev, nullptr, nullptr);
     if (e == cudaSuccess) e = advect_v_inplace(P, f_dev, true);
     return cuda_status(e);
@@ -1095,6 +1113,7 @@ extern "C" int vog_advect_v(vog_plan_t P, float* f_dev, const float* E_dev, doub
 extern "C" int vog_shift_x(vog_plan_t P, float* f_dev, const double* beta)
 {
     if (!P || !f_dev || !beta) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     P->recx_valid = false;
     cudaError_t e = run_setup(P, false, 2, 0.0, nullptr, nullptr, beta);
     if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
@@ -1104,6 +1123,7 @@ extern "C" int vog_shift_x(vog_plan_t P, float* f_dev, const double* beta)
 extern "C" int vog_shift_v(vog_plan_t P, float* f_dev, const double* beta)
 {
     if (!P || !f_dev || !beta) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
     if (e == cudaSuccess) e = advect_v_inplace(P, f_dev, false);
     return cuda_status(e);
@@ -1112,6 +1132,7 @@ extern "C" int vog_shift_v(vog_plan_t P, float* f_dev, const double* beta)
 extern "C" int vog_shift_v_to(vog_plan_t P, const float* src_dev, float* dst_dev, const double* beta)
 {
     if (!P || !src_dev || !dst_dev || !beta || src_dev == dst_dev) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
     if (e == cudaSuccess) e = advect_v(P, src_dev, dst_dev, false);
     return cuda_status(e);
@@ -1120,6 +1141,7 @@ extern "C" int vog_shift_v_to(vog_plan_t P, const float* src_dev, float* dst_dev
 extern "C" int vog_probe_x_memory_pattern(vog_plan_t P, const float* src_dev, float* dst_dev)
 {
     if (!P || !src_dev || !dst_dev || src_dev == dst_dev || P->p.Nx < 1024) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     P->launches++;
     return cuda_status(os_mempattern_launch(src_dev, dst_dev, P->p.Nx, P->p.Nv, 3 * P->n_sm, P->st));
 }
@@ -1127,6 +1149,7 @@ extern "C" int vog_probe_x_memory_pattern(vog_plan_t P, const float* src_dev, fl
 extern "C" int vog_field(vog_plan_t P, const float* f_dev, float* E_dev)
 {
     if (!P || !f_dev || !E_dev) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     return cuda_status(run_field(P, f_dev, E_dev));
 }
 
@@ -1139,6 +1162,7 @@ extern "C" int vog_get_field(vog_plan_t P, float* E_dev)
 extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ext_dev)
 {
     if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
     cudaError_t e = cudaSuccess;
     // The overlap-save v kernel is out of place: it writes the plan's second grid g, and the x-advection
     // that follows reads g and writes f, so a step moves no extra bytes.

@@ -478,3 +478,27 @@ def test_run_host_matches_device_steps(torch, vog):
     plan.get_field(Ed)
     assert torch.equal(Eh, Ed.cpu())
     plan.destroy()
+
+
+@pytest.mark.parametrize("idx,over", [(0, {}), (1, {}), (2, {}), (3, dict(Nx=1024, Nv=2048))])
+def test_dependent_launch_on_off_bit_identical(torch, vog, idx, over):
+    """vog_plan_tune(26, .): with programmatic dependent launch a kernel is staged while its predecessor still runs
+    and waits for it on the device; 20 back-to-back steps (a missing wait is a race between consecutive kernels)
+    must give the bits of plain stream order, for the whole-line and the overlap-save kernels, both split orders."""
+    for split in (0, 1):
+        cfg = inputs.config(idx, split=split, **over)
+        f0 = inputs.initial_f(cfg)
+        res = []
+        for pdl in (0, 1):
+            plan = vog.Plan.from_config(cfg)
+            plan.tune(26, pdl)
+            fd = _dev(torch, f0)
+            Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+            for _ in range(20):
+                plan.step(fd, cfg.dt)
+            plan.get_field(Ed)
+            torch.cuda.synchronize()
+            res.append((fd.cpu(), Ed.cpu()))
+            plan.destroy()
+        assert torch.equal(res[0][0], res[1][0])
+        assert torch.equal(res[0][1], res[1][1])
