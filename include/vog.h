@@ -106,6 +106,23 @@ int vog_shift_v(vog_plan_t plan, float* f_dev, const double* beta_cells_dev);
  * internally, ping-ponging between f and the second grid).  VOG_EINVAL if dst_dev == src_dev. */
 int vog_shift_v_to(vog_plan_t plan, const float* src_dev, float* dst_dev, const double* beta_cells_dev);
 
+/* nsteps Strang steps of size dt on the device, in place, asynchronous like vog_step (S10 driver).
+ *   merge = 0: exactly the kernels of nsteps calls of vog_step, bit for bit.
+ *   merge = 1: the half steps that meet between two consecutive steps are taken as one advection over dt, which the
+ *              paper names as the easy way to more speed: 2 advections per step instead of 3.
+ *                VOG_SPLIT_XVX: x(dt/2) [E=field; v(dt,E+E_ext); x(dt)]^(nsteps-1) E=field; v(dt,E+E_ext); x(dt/2)
+ *                VOG_SPLIT_VXV: v(dt/2) [x(dt); E=field; v(dt,E+E_ext)]^(nsteps-1) x(dt); E=field; v(dt/2,E+E_ext)
+ *              (in VXV the two half steps see the same E because rho is invariant under a v-advection, P:205-213;
+ *              the merged result differs from the unmerged one by interpolation error only, not by rounding only).
+ * E_ext_seq_dev: NULL, or one row of Nx floats per v-advection, in the order the v-advections are taken
+ *   (XVX: nsteps rows; VXV: 2*nsteps rows unmerged, nsteps+1 merged).
+ * energy_dev: NULL, or nsteps doubles in device memory; entry s receives the electric energy (1/2) dx sum_i E_i^2
+ *    of the self-consistent field of the s-th field solve of the call (XVX: at the half-advanced density of
+ *   step s; VXV: at t^(s+1)), summed in fp64 in a fixed order.
+ * VOG_EINVAL for NULL plan / f_dev, nsteps < 0, merge outside {0,1}; VOG_ENOMEM if the second grid cannot be had. */
+int vog_run(vog_plan_t plan, float* f_dev, double dt, int nsteps, const float* E_ext_seq_dev, int merge,
+            double* energy_dev);
+
 /* End-to-end convenience with HOST buffers: copies f_host (Nx*Nv floats) and E_ext_host (Nx
  * floats or NULL) into a device buffer that the plan allocates on the first call and keeps (the
  * only O(Nx*Nv) allocation of the library, made only if this call is used), runs `nsteps`

@@ -287,8 +287,10 @@ __device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int N
 __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadix rx, int tw_len, int tw_in_smem,
                                                        const float2* __restrict__ tw_g, const float* __restrict__ ikt,
                                                        const double* __restrict__ rho, float* __restrict__ E_a,
-                                                       float* __restrict__ E_b)
+                                                       float* __restrict__ E_b, double* __restrict__ energy_out,
+                                                       double half_dx)
 {
+    __shared__ double ered[32];
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* z = reinterpret_cast<float2*>(smem_raw);
     float* iks = reinterpret_cast<float*>(z + Nx);      // 1/(i k) factors
@@ -335,10 +337,23 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
             __syncthreads();
         }
     }
+    double e2 = 0.0;
     for (int i = tid; i < Nx; i += T) {
         const float e = z[i].x;
         E_a[i] = e;
         if (E_b) E_b[i] = e;
+        e2 += (double)e * (double)e;
+    }
+    if (energy_out) {   // electric energy (1/2) dx sum_i E_i^2, fp64, fixed summation order
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e2 += __shfl_xor_sync(0xffffffffu, e2, o);
+        if ((tid & 31) == 0) ered[tid >> 5] = e2;
+        __syncthreads();
+        if (tid == 0) {
+            double s = 0.0;
+            for (int w = 0; w < (T >> 5); ++w) s += ered[w];
+            energy_out[0] = half_dx * s;
+        }
     }
 }
 
@@ -1058,7 +1073,7 @@ static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
     return e;
 }
 
-static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
+static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double* energy_out = nullptr)
 {
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
@@ -1080,7 +1095,8 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out)
     P->launches += 2;
     P->E_valid = true;
     return launch_pdl(poisson_kernel, dim3(1), dim3(T), psmem, P->st, Nx, P->prx, P->ptw_len, tw_in_smem,
-                      (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->rho, P->E_self, E_out);
+                      (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->rho, P->E_self, E_out, energy_out,
+                      0.5 * P->p.L / (double)Nx);
 }
 
 static cudaError_t ensure_recx(vog_plan_s* P, double dt)
@@ -1188,6 +1204,67 @@ extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ex
         if (e == cudaSuccess) e = run_field(P, g, nullptr);
         if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
         if (e == cudaSuccess) e = advect_v(P, g, f_dev, true);
+    }
+    return cuda_status(e);
+}
+
+extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const float* E_ext_seq_dev, int merge,
+                       double* energy_dev)
+{
+    if (!P || !f_dev || nsteps < 0 || !std::isfinite(dt) || merge < 0 || merge > 1) return VOG_EINVAL;
+    if (nsteps == 0) return VOG_OK;
+    t_pdl = P->pdl != 0;
+    const int Nx = P->p.Nx;
+    cudaError_t e = cudaSuccess;
+    float* g = f_dev;
+    if (P->os_v) {
+        e = ensure_gbuf(P);
+        if (e != cudaSuccess) { cudaGetLastError(); return VOG_ENOMEM; }
+        g = P->g_buf;
+    }
+    int iv = 0, ie = 0;                                    // v-advections and field solves so far
+    auto ext = [&]() { return E_ext_seq_dev ? E_ext_seq_dev + (size_t)(iv++) * Nx : nullptr; };
+    auto en = [&]() { return energy_dev ? energy_dev + (ie++) : nullptr; };
+    auto ok = [&]() { return e == cudaSuccess; };
+    if (P->p.split == VOG_SPLIT_XVX) {
+        // x(dt/2) [field v(dt) x(dt)]^(n-1) field v(dt) x(dt/2); unmerged: the x(dt) is two x(dt/2)
+        e = ensure_recx(P, 0.5 * dt);
+        if (ok()) e = advect_x(P, f_dev, f_dev);
+        for (int s = 0; s < nsteps && ok(); ++s) {
+            e = run_field(P, f_dev, nullptr, en());
+            if (ok()) e = run_setup(P, true, 1, dt, P->E_self, ext(), nullptr);
+            if (ok()) e = advect_v(P, f_dev, g, true);
+            const bool last = s == nsteps - 1;
+            if (ok()) e = ensure_recx(P, (merge && !last) ? dt : 0.5 * dt);
+            if (ok()) e = advect_x(P, g, f_dev);
+            if (ok() && !merge && !last) e = advect_x(P, f_dev, f_dev);
+        }
+    } else {
+        // v(dt/2) [x(dt) field v(dt)]^(n-1) x(dt) field v(dt/2); the two v(dt/2) around a field solve see the same
+        // E (rho is invariant under the v-advection), so merged they are one v(dt)
+        float *cur = f_dev, *oth = g;                      // (oth == cur for the in-place whole-line kernels)
+        auto vadv = [&](double dts) {
+            e = run_setup(P, true, 1, dts, P->E_self, ext(), nullptr);
+            if (ok()) e = advect_v(P, cur, oth, true);
+            std::swap(cur, oth);
+        };
+        const int nvadv = merge ? nsteps + 1 : 2 * nsteps;
+        bool flip_x = oth != cur && (nvadv & 1);           // odd number of buffer flips: one x-advection goes across
+        if (!P->E_valid) e = run_field(P, f_dev, nullptr, nullptr);
+        if (ok()) vadv(0.5 * dt);
+        if (ok()) e = ensure_recx(P, dt);
+        for (int s = 0; s < nsteps && ok(); ++s) {
+            if (flip_x) { e = advect_x(P, cur, oth); std::swap(cur, oth); flip_x = false; }
+            else e = advect_x(P, cur, cur);
+            if (ok()) e = run_field(P, cur, nullptr, en());
+            const bool last = s == nsteps - 1;
+            if (!ok()) break;
+            if (merge && !last) vadv(dt);
+            else {
+                vadv(0.5 * dt);
+                if (ok() && !last) vadv(0.5 * dt);
+            }
+        }
     }
     return cuda_status(e);
 }

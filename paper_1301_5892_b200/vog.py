@@ -16,7 +16,7 @@ LAGRANGE, BSPLINE = 0, 1
 SPLIT_XVX, SPLIT_VXV = 0, 1
 
 EXPORTS = ("vog_plan", "vog_destroy", "vog_advect_x", "vog_advect_v", "vog_field", "vog_step",
-           "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_probe_x_memory_pattern", "vog_run_host", "vog_launch_count",
+           "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_probe_x_memory_pattern", "vog_run", "vog_run_host", "vog_launch_count",
            "vog_strerror", "vog_plan_tune")
 
 
@@ -60,6 +60,7 @@ def lib():
         L.vog_shift_v.argtypes = [vp, vp, vp]
         L.vog_shift_v_to.argtypes = [vp, vp, vp, vp]
         L.vog_probe_x_memory_pattern.argtypes = [vp, vp, vp]
+        L.vog_run.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, ctypes.c_int, vp]
         L.vog_run_host.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp]
         L.vog_launch_count.argtypes = [vp]
         L.vog_launch_count.restype = ctypes.c_longlong
@@ -150,6 +151,10 @@ class Plan:
 
     def shift_v_to(self, src, dst, beta):
         self._ck(lib().vog_shift_v_to(self._h, _ptr(src), _ptr(dst), _ptr(beta)), "vog_shift_v_to")
+
+    def run(self, f, dt, nsteps, E_ext_seq=None, merge=False, energy=None):
+        self._ck(lib().vog_run(self._h, _ptr(f), float(dt), int(nsteps), _ptr(E_ext_seq), 1 if merge else 0,
+                               _ptr(energy)), "vog_run")
 
     def run_host(self, f_host, dt, nsteps, E_ext_host=None, E_host=None):
         self._ck(lib().vog_run_host(self._h, _ptr(f_host), float(dt), int(nsteps), _ptr(E_ext_host),
