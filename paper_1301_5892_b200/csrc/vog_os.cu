@@ -106,6 +106,96 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
     }
 }
 
+// The same tables for the v direction, one CTA per strip of 32 columns (lane = column): the table is stored
+// transposed, lam[k][column], so with one CTA per column (the kernel above) every entry was an isolated 8-byte
+// store; here a warp writes whole 256-byte rows.  Threads 0..63 do the per-column fp64 work (one Everett chain
+// a_0..a_8 per (column, half); the a_j are prefix products, same operations in the same order as above), then
+// the 8 warps share the 130 rows.  Same arithmetic as os_setup_kernel, entry for entry.
+__global__ void __launch_bounds__(256) os_setup_v_kernel(const OsSetupArgs s)
+{
+    __shared__ float af[18][32];                 // [half * 9 + j][column]; spline: rows 0..3 = B(b*+1), B(b*), B(b*-1), B(b*-2)
+    __shared__ int bsh[32];
+    __shared__ float ssh[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int l0 = blockIdx.x * 32;
+    pdl_wait();                                   // E comes from the Poisson kernel; the tables may still be read
+    pdl_launch_dependents();
+    if (tid < 64) {
+        const int half = tid >> 5, l = l0 + lane;
+        double beta;
+        float sshift = 0.0f;
+        if (s.mode == 0) {
+            beta = -(s.vmin + (double)l * s.dv) * s.dt / s.delta;
+        } else if (s.mode == 1) {
+            double e = (double)s.E[l];
+            if (s.Eext) e += (double)s.Eext[l];
+            beta = -e * s.dt / s.delta;
+            sshift = (float)(s.dt * e);
+        } else {
+            beta = s.beta[l];
+        }
+        const double fl = floor(beta);
+        const double t = beta - fl;
+        int b;
+        if (fabs(fl) < 9.0e18) {
+            b = (int)(__double2ll_rn(fl) & (long long)(s.N - 1));
+        } else {
+            double bm = fmod(fl, (double)s.N);
+            if (bm < 0.0) bm += (double)s.N;
+            b = (int)bm;
+            if (b >= s.N) b = 0;
+        }
+        if (half == 0) { bsh[lane] = b; ssh[lane] = sshift; }
+        if (!s.spline) {
+            const double tt = half == 0 ? 1.0 - t : t;
+            double a = tt;
+            constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
+                                       1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
+            af[half * 9][lane] = (float)a;
+#pragma unroll
+            for (int m = 1; m <= 8; ++m) {
+                a = a * ((double)(m * m) - tt * tt) * rcp[m];
+                af[half * 9 + m][lane] = m <= s.d ? (float)a : 0.0f;
+            }
+        } else if (half == 0) {
+            const double u = 1.0 - t;
+            af[0][lane] = (float)(u * u * u / 6.0);
+            af[1][lane] = (float)((4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0);
+            af[2][lane] = (float)((1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0);
+            af[3][lane] = (float)(t * t * t / 6.0);
+        }
+    }
+    __syncthreads();
+    const float sc = s.gen2 ? 1.0f / (float)OS_LB : 1.0f / (2.0f * (float)OS_LB);
+    float2* const out = s.lam + l0 + lane;
+    const size_t ks = (size_t)s.n_lines;
+    for (int k = wid + 8 * blockIdx.y; k < OS_LAMW; k += 8 * gridDim.y) {      // (the rows are split over gridDim.y CTAs)
+        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(bsh[lane]), ssh[lane]); continue; }
+        if (k == 0) { out[0] = make_float2(sc, 0.0f); continue; }
+        const double2 cs = s.cs64[k];
+        const float c = (float)cs.x, sn = (float)cs.y;
+        float lr, li;
+        if (s.spline) {
+            const float Bm1 = af[0][lane], B0 = af[1][lane], B1 = af[2][lane], B2 = af[3][lane];
+            const float c2 = (float)(2.0 * cs.x * cs.x - 1.0), s2 = (float)(2.0 * cs.y * cs.x);
+            const float g = 3.0f / (2.0f + c);
+            lr = fmaf(B2, c2, fmaf(Bm1 + B1, c, B0)) * g;
+            li = fmaf(B2, s2, (B1 - Bm1) * sn) * g;
+        } else {
+            const float sv = (float)(2.0 - 2.0 * cs.x);
+            float p0 = 0.0f, p1 = 0.0f;
+#pragma unroll
+            for (int j = 8; j >= 0; --j) {
+                p0 = fmaf(p0, sv, af[j][lane]);
+                p1 = fmaf(p1, sv, af[9 + j][lane]);
+            }
+            lr = fmaf(c, p1, p0);
+            li = sn * p1;
+        }
+        out[k * ks] = make_float2(lr * sc, li * sc);
+    }
+}
+
 // Measurement probe (vog_probe_x_memory_pattern): exactly the global loads and stores of osx5_kernel<., 232, 8> on
 // N-cell lines with zero shift -- 32 four-byte loads per thread in 64-byte runs per half-warp, the kept samples
 // stored with four-byte streaming stores -- and no transform.  Its time is the memory-system floor of that
@@ -145,6 +235,11 @@ cudaError_t os_mempattern_launch(const float* src, float* dst, int N, int n_line
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
 {
+    if (s.vdir && s.n_lines % 32 == 0) {
+        // 8 CTAs share the 130 rows of a strip (measured at 2048 columns, step time: 1 -> 62.2, 2 -> 60.0, 4 -> 59.1,
+        // 8 -> 58.8, 17 -> 59.4 us; one CTA per column, the kernel above: 61.0 us)
+        return launch_pdl(os_setup_v_kernel, dim3(s.n_lines / 32, 8), dim3(256), 0, st, s);
+    }
     return launch_pdl(os_setup_kernel, dim3(s.n_lines), dim3(128), 0, st, s);
 }
 
