@@ -599,3 +599,40 @@ def test_run_argument_errors_and_empty_run(torch, vog):
         plan.run(None, 0.1, 1)
     assert vog.lib().vog_run(plan._h, f.data_ptr(), 0.1, 1, None, 2, None) == vog.EINVAL
     plan.destroy()
+
+
+@pytest.mark.parametrize("idx", [2, 3])
+def test_full_length_runs_of_configs_2_and_3_keep_the_invariants(torch, vog, idx):
+    """BASELINE.json configs 2 (bump on tail, 2000 steps) and 3 (KEEN drive, 4000 steps) at their full size and length
+    through vog_run, energies recorded on the device.  Long trajectories are 'parity unpinned' (S:8(c): the paper's own
+    fp32 and fp64 runs separate), so what is checked is what holds for any correct run: everything
+    finite; the mass sum(delta f) dx dv conserved (P5: column sums of A are 1; fp32 storage of |delta f| <= 0.2 against
+    a mass of O(L): 1e-5 relative is 1e3 roundings); the bump-on-tail instability grows out of the 4 % perturbation
+     and saturates; the KEEN response follows the drive's ramp (a(t) rises 0 -> 1 around t = 69)."""
+    cfg = inputs.config(idx)
+    n = cfg.steps
+    f0 = inputs.initial_f(cfg)
+    plan = vog.Plan.from_config(cfg)
+    fd = _dev(torch, f0)
+    ext = None
+    if cfg.keen:
+        ext = _dev(torch, np.stack([inputs.keen_E_ext(cfg, (s + 0.5) * cfg.dt) for s in range(n)]).astype(np.float32))
+    en = torch.zeros(n, device="cuda", dtype=torch.float64)
+    m0 = fd.double().sum().item()
+    plan.run(fd, cfg.dt, n, ext, merge=False, energy=en)
+    torch.cuda.synchronize()
+    e = en.cpu().numpy()
+    m1 = fd.double().sum().item()
+    plan.destroy()
+    assert np.isfinite(e).all() and bool(torch.isfinite(fd).all())
+    mass = inputs.gaussians(cfg.v(), cfg.feq).sum() * cfg.Nx
+    assert abs(m1 - m0) <= 1e-5 * mass
+    assert (e >= 0).all()
+    if idx == 2:
+        assert e.max() >= 5.0 * e[0]                       # instability
+        assert e[-1] <= e.max() and e[n // 2:].max() <= 2.0 * e[: n // 2].max()      # saturated, no blow-up
+    else:
+        t = lambda time: int(round(time / cfg.dt))
+        assert e[0] <= 1e-12                               # Maxwellian start: no self-consistent field yet
+        assert e[t(100.0)] >= 100.0 * e[t(20.0)] > 0.0     # response follows the ramp
+        assert e.max() <= 1.0                              # bounded (drive amplitude 0.052)
