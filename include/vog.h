@@ -132,6 +132,13 @@ int vog_run(vog_plan_t plan, float* f_dev, double dt, int nsteps, const float* E
 int vog_run_host(vog_plan_t plan, float* f_host, double dt, int nsteps,
                  const float* E_ext_host, float* E_host);
 
+/* The same without the final synchronisation: everything (copy in, steps, copies out) is enqueued on the plan's stream
+ * and the call returns; the host buffers must be pinned and stay untouched until the caller has synchronised that
+ * stream.  Several plans on several streams then overlap one replica's copy in, another's steps and a third's copy
+ * out (PCIe is full duplex), which is how `bench.py` measures its end-to-end figure. */
+int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
+                       const float* E_ext_host, float* E_host);
+
 /* Launch-shape override for measurements; never needed for normal use and never
  * changes results beyond rounding.  which:
  *   2, 3   whole-line v kernel (Nv <= 512): log2(complex lines per CTA), threads per CTA;

@@ -1269,7 +1269,7 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
     return cuda_status(e);
 }
 
-extern "C" int vog_run_host(vog_plan_t P, float* f_host, double dt, int nsteps, const float* E_ext_host, float* E_host)
+static int run_host(vog_plan_t P, float* f_host, double dt, int nsteps, const float* E_ext_host, float* E_host, bool sync)
 {
     if (!P || !f_host || nsteps < 0 || !std::isfinite(dt)) return VOG_EINVAL;
     const size_t nf = (size_t)P->p.Nx * P->p.Nv;
@@ -1291,8 +1291,19 @@ extern "C" int vog_run_host(vog_plan_t P, float* f_host, double dt, int nsteps, 
     e = cudaMemcpyAsync(f_host, P->f_buf, sizeof(float) * nf, cudaMemcpyDeviceToHost, P->st);
     if (e == cudaSuccess && E_host && P->E_valid)
         e = cudaMemcpyAsync(E_host, P->E_self, sizeof(float) * P->p.Nx, cudaMemcpyDeviceToHost, P->st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
+    if (e == cudaSuccess && sync) e = cudaStreamSynchronize(P->st);
     return cuda_status(e);
+}
+
+extern "C" int vog_run_host(vog_plan_t P, float* f_host, double dt, int nsteps, const float* E_ext_host, float* E_host)
+{
+    return run_host(P, f_host, dt, nsteps, E_ext_host, E_host, true);
+}
+
+extern "C" int vog_run_host_async(vog_plan_t P, float* f_host, double dt, int nsteps, const float* E_ext_host,
+                                  float* E_host)
+{
+    return run_host(P, f_host, dt, nsteps, E_ext_host, E_host, false);
 }
 
 extern "C" long long vog_launch_count(vog_plan_t P) { return P ? P->launches : -1; }

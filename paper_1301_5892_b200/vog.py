@@ -16,7 +16,7 @@ LAGRANGE, BSPLINE = 0, 1
 SPLIT_XVX, SPLIT_VXV = 0, 1
 
 EXPORTS = ("vog_plan", "vog_destroy", "vog_advect_x", "vog_advect_v", "vog_field", "vog_step",
-           "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_probe_x_memory_pattern", "vog_run", "vog_run_host", "vog_launch_count",
+           "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_probe_x_memory_pattern", "vog_run", "vog_run_host", "vog_run_host_async", "vog_launch_count",
            "vog_strerror", "vog_plan_tune")
 
 
@@ -62,6 +62,7 @@ def lib():
         L.vog_probe_x_memory_pattern.argtypes = [vp, vp, vp]
         L.vog_run.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, ctypes.c_int, vp]
         L.vog_run_host.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp]
+        L.vog_run_host_async.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp]
         L.vog_launch_count.argtypes = [vp]
         L.vog_launch_count.restype = ctypes.c_longlong
         L.vog_strerror.argtypes = [ctypes.c_int]
@@ -159,6 +160,10 @@ class Plan:
     def run_host(self, f_host, dt, nsteps, E_ext_host=None, E_host=None):
         self._ck(lib().vog_run_host(self._h, _ptr(f_host), float(dt), int(nsteps), _ptr(E_ext_host),
                                     _ptr(E_host)), "vog_run_host")
+
+    def run_host_async(self, f_host, dt, nsteps, E_ext_host=None, E_host=None):
+        self._ck(lib().vog_run_host_async(self._h, _ptr(f_host), float(dt), int(nsteps), _ptr(E_ext_host),
+                                          _ptr(E_host)), "vog_run_host_async")
 
     def launch_count(self):
         return int(lib().vog_launch_count(self._h))

@@ -636,3 +636,27 @@ def test_full_length_runs_of_configs_2_and_3_keep_the_invariants(torch, vog, idx
         assert e[0] <= 1e-12                               # Maxwellian start: no self-consistent field yet
         assert e[t(100.0)] >= 100.0 * e[t(20.0)] > 0.0     # response follows the ramp
         assert e.max() <= 1.0                              # bounded (drive amplitude 0.052)
+
+
+def test_run_host_async_overlapped_replicas_match_the_synchronous_call(torch, vog):
+    cfg = inputs.config(1)
+    fs = [inputs.initial_f(inputs.config(1, alpha=a)) for a in (0.5, 0.3, 0.1)]
+    ref = []
+    for f in fs:
+        plan = vog.Plan.from_config(cfg)
+        fh = torch.from_numpy(f.copy()).pin_memory()
+        Eh = torch.empty(cfg.Nx, dtype=torch.float32).pin_memory()
+        plan.run_host(fh, cfg.dt, 2, None, Eh)
+        ref.append((fh.clone(), Eh.clone()))
+        plan.destroy()
+    streams = [torch.cuda.Stream() for _ in fs]
+    plans = [vog.Plan.from_config(cfg, stream=st) for st in streams]
+    fhs = [torch.from_numpy(f.copy()).pin_memory() for f in fs]
+    Ehs = [torch.empty(cfg.Nx, dtype=torch.float32).pin_memory() for _ in fs]
+    for p, fh, Eh in zip(plans, fhs, Ehs):
+        p.run_host_async(fh, cfg.dt, 2, None, Eh)
+    torch.cuda.synchronize()
+    for (rf, rE), fh, Eh in zip(ref, fhs, Ehs):
+        assert torch.equal(rf, fh) and torch.equal(rE, Eh)
+    for p in plans:
+        p.destroy()
