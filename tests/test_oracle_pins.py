@@ -337,3 +337,149 @@ def test_keen_drive_matches_paper_parameters():
     cfg = inputs.config(3, Nx=64, Nv=64)
     e = inputs.keen_E_ext(cfg, 150.0)
     assert abs(np.abs(e).max() - g["Emax"] * g["k"] * inputs.keen_amplitude(150.0)) < 1e-3
+
+
+# ---------------------------------------------------------------- round 2: E_ext in the step, f_eq with mu != 0
+# (VERDICT r1 "What's weak" 2: flipping the sign of E_ext in oracle_step, or (v - mu) -> (v + mu) in oracle_feq,
+# left every pin above green.  The pins below fix both by statements that are independent of the oracle's code:
+# characteristics of the v-transport equation, translation of a profile, a Gaussian integral.)
+_BUMP_FEQ = [(0.9 / math.sqrt(2 * math.pi), 0.0, 0.5), (0.2 / math.sqrt(2 * math.pi), 4.5, 4.0)]   # config 2's f_eq
+
+
+@pytest.mark.parametrize("split", [inputs.SPLIT_XVX, inputs.SPLIT_VXV])
+@pytest.mark.parametrize("kcells", [3, -5])
+def test_step_with_constant_E_ext_is_a_pure_velocity_translation(oracle, split, kcells):
+    """the advecting field is E + E_ext (E_ext = -E_app).  For f independent of x the self-consistent field
+    vanishes and the x half steps act on constant lines, so one Strang step with a constant E_ext = c is the
+    characteristic map f(v) -> f(v - c dt) (d_t f + E d_v f = 0).  With c dt = k dv (XVX; VXV: every half
+    step k/2 cells... chosen even) this is the exact permutation f_new[j] = f[j - k]: c > 0 moves the profile to +v."""
+    Nx, Nv, L, vmin, vmax, dt = 32, 64, 4 * math.pi, -6.0, 6.0, 0.1
+    dv = (vmax - vmin) / Nv
+    k = 2 * kcells                                   # even: the two VXV half steps are whole cells each
+    c = k * dv / dt
+    rng = np.random.default_rng(21)
+    prof = rng.random(Nv)
+    f = np.tile(prof[:, None], (1, Nx))
+    E_ext = np.full(Nx, c)
+    g, E = oracle.step(f, L, vmin, vmax, dt, LAG, 17, None, split, E_ext, np.zeros(Nx))
+    assert np.abs(E).max() < 1e-13                   # rho is constant in x: zero-mean field vanishes
+    expect = np.tile(np.roll(prof, k)[:, None], (1, Nx))     # f_new[j] = f[j - k]
+    assert np.abs(g - expect).max() < 1e-13
+    # and the opposite sign must NOT satisfy it (guards the test itself against a symmetric profile)
+    assert np.abs(g - np.tile(np.roll(prof, -k)[:, None], (1, Nx))).max() > 0.1
+
+
+def test_step_xvx_with_E_ext_cancelling_the_self_field_is_two_x_half_steps(oracle):
+    """P:269 again: with E_ext = -E_self the advecting field is zero, the v-advection is the identity (beta = 0
+    is an exact permutation) and the XVX step is x(dt/2) twice."""
+    cfg = inputs.config(0, Nx=32, Nv=32)
+    f = inputs.initial_f(cfg).astype(np.float64)
+    half = oracle.advect_x(f, cfg.L, cfg.vmin, cfg.vmax, 0.5 * cfg.dt, LAG, 17)
+    E_self = oracle.field(half, cfg.L, cfg.vmin, cfg.vmax)
+    assert np.abs(E_self).max() > 1e-5
+    g, E = oracle.step(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, LAG, 17, None, inputs.SPLIT_XVX, -E_self)
+    expect = oracle.advect_x(half, cfg.L, cfg.vmin, cfg.vmax, 0.5 * cfg.dt, LAG, 17)
+    assert np.array_equal(E, E_self)
+    assert np.abs(g - expect).max() < 1e-15
+    # with +E_self instead the field doubles and the result must differ
+    g2, _ = oracle.step(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, LAG, 17, None, inputs.SPLIT_XVX, E_self)
+    assert np.abs(g2 - expect).max() > 1e-7
+
+
+@pytest.mark.parametrize("split", [inputs.SPLIT_XVX, inputs.SPLIT_VXV])
+def test_step_delta_f_source_sees_E_ext_with_its_sign(oracle, split):
+    """delta-f mode with delta f = 0 and a constant E_ext = c: the step returns f_eq(v - c dt) - f_eq(v), the
+    TRANSLATED equilibrium profile (two-Gaussian f_eq of config 2, mu = 4.5): sampled on an unwrapped extension of
+    the v mesh and shifted by whole cells -- no formula of the oracle is re-evaluated."""
+    Nx, Nv, L, vmin, vmax, dt, k = 32, 256, 20 * math.pi, -9.0, 9.0, 0.05, 6
+    dv = (vmax - vmin) / Nv
+    c = k * dv / dt
+    ext = vmin + dv * np.arange(-16, Nv + 16)                      # unwrapped mesh, 16 cells beyond either end
+    prof = inputs.gaussians(ext, _BUMP_FEQ)
+    expect = prof[16 - k:16 - k + Nv] - prof[16:16 + Nv]           # f_eq(v_j - k dv) - f_eq(v_j)
+    g, _E = oracle.step(np.zeros((Nv, Nx)), L, vmin, vmax, dt, LAG, 17, oracle.Feq.make(_BUMP_FEQ), split,
+                        np.full(Nx, c), np.zeros(Nx))
+    # VXV takes two half steps: source(k/2) shifted by k/2 cells + source(k/2) = the same total, up to the Lagrange
+    # interpolation error of the intermediate (smooth, dv-resolved) profile, ~1e-9 here (LAG17, Nv = 256)
+    tol = 1e-15 if split == inputs.SPLIT_XVX else 1e-12
+    assert np.abs(g - expect[:, None]).max() < tol
+    assert np.abs(g + expect[:, None]).max() > 1e-3                # the mirrored sign fails
+
+
+def test_feq_two_gaussians_off_centre(oracle):
+    """oracle_feq with n = 2, mu != 0 (config 2, B.json): position of the bump, mirror symmetry of each Gaussian
+    about ITS centre, the Gaussian integral sum_g amp_g sqrt(pi / c_g) (closed form; the rectangle rule is
+    spectrally accurate for a Gaussian), and agreement with the profile the workload generator builds f_0 from."""
+    feq = oracle.Feq.make(_BUMP_FEQ)
+    v = -9.0 + (18.0 / 1024) * np.arange(1024)
+    val = np.array([oracle.feq_eval(feq, x) for x in v])
+    assert oracle.feq_eval(feq, 4.5) > 50 * oracle.feq_eval(feq, -4.5)        # the bump sits at +4.5, not -4.5
+    bump_only = oracle.Feq.make(_BUMP_FEQ[1:])
+    for h in (0.1, 0.37, 1.0):
+        assert abs(oracle.feq_eval(bump_only, 4.5 + h) - oracle.feq_eval(bump_only, 4.5 - h)) < 1e-17
+        assert oracle.feq_eval(bump_only, 4.5) > oracle.feq_eval(bump_only, 4.5 + h)
+    closed = sum(a * math.sqrt(math.pi / c) for a, _mu, c in _BUMP_FEQ)        # = 0.9 + 0.2 / sqrt(8)
+    assert abs(closed - (0.9 + 0.2 / math.sqrt(8.0))) < 1e-15
+    assert abs(val.sum() * (18.0 / 1024) - closed) < 1e-12
+    first_moment = sum(a * mu * math.sqrt(math.pi / c) for a, mu, c in _BUMP_FEQ)
+    assert abs((val * v).sum() * (18.0 / 1024) - first_moment) < 1e-12        # odd in the sign of mu
+    assert np.abs(val - inputs.gaussians(v, _BUMP_FEQ)).max() < 1e-16
+
+
+def test_delta_f_source_with_off_centre_feq_is_a_translated_profile(oracle):
+    """P:197 for config 2's f_eq: delta f = 0, E dt = k dv  =>  the update is f_eq sampled k cells lower minus f_eq."""
+    Nx, Nv, vmin, vmax, dt = 4, 512, -9.0, 9.0, 0.05
+    dv = (vmax - vmin) / Nv
+    ks = np.array([7, -3, 0, 12])
+    E = ks * dv / dt
+    ext = vmin + dv * np.arange(-16, Nv + 16)
+    prof = inputs.gaussians(ext, _BUMP_FEQ)
+    g = oracle.advect_v(np.zeros((Nv, Nx)), E, vmin, vmax, dt, LAG, 17, oracle.Feq.make(_BUMP_FEQ))
+    for i, k in enumerate(ks):
+        expect = prof[16 - k:16 - k + Nv] - prof[16:16 + Nv]
+        assert np.abs(g[:, i] - expect).max() < 2e-16
+
+
+def test_delta_f_scheme_matches_full_f_scheme_with_off_centre_feq(oracle):
+    """P:197-199 on a bump-on-tail shaped state: advancing delta f = f - f_eq and adding f_eq back equals advancing f,
+    up to the interpolation error of f_eq itself (LAG17 on a dv-resolved Gaussian: ~1e-9)."""
+    cfg = inputs.config(2, Nx=32, Nv=512)
+    v = cfg.v()[:, None]
+    f_full = (1.0 + cfg.alpha * np.cos(cfg.k * cfg.x()[None, :])) * inputs.gaussians(v, cfg.profile)
+    feq_v = inputs.gaussians(v, cfg.feq)
+    E = 0.6 * np.sin(cfg.k * cfg.x()) + 0.3                                   # |E dt / dv| up to ~1.3 cells
+    a = oracle.advect_v(f_full, E, cfg.vmin, cfg.vmax, cfg.dt, LAG, 17, None)
+    b = oracle.advect_v(f_full - feq_v, E, cfg.vmin, cfg.vmax, cfg.dt, LAG, 17, oracle.Feq.make(cfg.feq))
+    assert np.abs(a - (b + feq_v)).max() < 1e-8
+    # sanity of the bound: the source term itself is 4 orders larger than the tolerance
+    assert np.abs(b - oracle.advect_v(f_full - feq_v, E, cfg.vmin, cfg.vmax, cfg.dt, LAG, 17, None)).max() > 1e-4
+
+
+def test_keen_drive_sign_and_phase(oracle):
+    """the advecting field is E - E_app with E_app = E_max k a(t) sin(kx - w t); the harness passes
+    E_ext = -E_app.  Pins the SIGN and the phase velocity (+w/k) of inputs.keen_E_ext, not only its modulus."""
+    g = _golden("keen_drive.txt")
+    cfg = inputs.config(3, Nx=256, Nv=64)
+    x = cfg.x()
+    for t in (100.0, 150.0, 200.0):
+        e = inputs.keen_E_ext(cfg, t).astype(np.float64)
+        a = inputs.keen_amplitude(t)
+        assert a > 0
+        # projection on sin(kx - wt): -E_max k a(t) (negative: E_ext = -E_app), nothing on the cosine
+        s, c = np.sin(g["k"] * x - g["omega"] * t), np.cos(g["k"] * x - g["omega"] * t)
+        assert abs(2 * (e * s).mean() + g["Emax"] * g["k"] * a) < 1e-8
+        assert abs(2 * (e * c).mean()) < 1e-8
+    # the pattern travels toward +x at w/k: the zero crossing with negative slope of E_ext... follows x = w t / k
+    t0, t1 = 150.0, 150.5
+    ph = lambda t: np.angle(np.fft.fft(inputs.keen_E_ext(cfg, t).astype(np.float64))[1])
+    dphi = (ph(t1) - ph(t0) + math.pi) % (2 * math.pi) - math.pi
+    assert abs(dphi + g["omega"] * (t1 - t0)) < 1e-6          # mode e^{i(kx - wt)}: phase of FFT bin 1 falls at w
+    # driven particles: with f independent of x and NO self field, a step with E_ext(t) moves the column at the
+    # maximum of E_ext toward +v (characteristics dv/dt = E + E_ext)
+    i = int(np.argmax(e))
+    Nv = 64
+    prof = np.exp(-np.linspace(-3, 3, Nv) ** 2)
+    f = np.tile(prof[:, None], (1, 256))
+    dt = 4 * cfg.dv / float(e[i])                               # four cells at the maximum
+    out, _ = oracle.step(f, cfg.L, cfg.vmin, cfg.vmax, dt, LAG, 17, None, inputs.SPLIT_VXV, e, np.zeros(256))
+    assert np.argmax(out[:, i]) == np.argmax(prof) + 4
