@@ -1,7 +1,7 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the vog hot path on B200 (contract: see the task statement / DESIGN.md).
+"""bench.py -- throughput of the vog hot path on B200 (contract: see the task statement / DESIGN.md 9).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--no-sweep]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--no-sweep] [--no-cpu]
 
 Workload (BASELINE.json metric): one Strang step (x/2 - field - v - x/2, 3 fused advections +
 density + Poisson) of the fp32 delta-f scheme on a 2048 x 2048 grid, LAG17, nonlinear-Landau
@@ -9,7 +9,11 @@ initial data.  One bench "step" advances a BATCH of independent replicas of that
 Strang step each; the batch (16 x 16 MiB = 256 MiB) is larger than the 126 MB L2, so every
 replica is L2-cold when its turn comes again.  value = phase-space cells advanced per second by
 the whole job.  Multi-GPU = independent replicas per rank (the path does not shard).
-Prints ONE JSON line on rank 0.
+
+Output (rank 0, stdout): first the detail records -- one JSON line per row of the config-4 sweep
+({"sweep_row": ...}), one for the small grids, one for the per-advection oracle timings -- and then, as the
+LAST line, the short result record the driver parses (< 2.5 KB).  The detail records are also written to
+gpurun_out/bench_detail.json when that directory can be created.
 """
 import argparse
 import json
@@ -28,30 +32,42 @@ from paper_1301_5892_b200 import inputs  # noqa: E402
 
 METRIC = "phase-space cell-updates/s per Strang step (fp32 delta-f, 2048x2048)"
 UNIT = "cell-updates/s"
+WORKLOAD = "strang_step_deltaf_2048x2048_lag17"
 BATCH = 16
 
 
 def _traffic():
-    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/), else None."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    """(dram bytes per launch of the roofline kernel, source) from the committed ncu capture, else (None, None).
+    It is a constant of that capture (ncu cannot run inside a timed bench), named as such in the record."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
+        src = None
         for line in open(path):
             key, _, val = line.strip().partition(",")
-            if key == "x_kernel_bench_dram_bytes_per_launch":
-                return float(val)
+            if key == "source":
+                src = val
+            if key == "x_kernel_2048_dram_bytes_per_launch":
+                return float(val), src
     except Exception:
         pass
-    return None
+    return None, None
 
 
 def _peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
         try:
-            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+            return float(json.load(open(path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
         except Exception:
             pass
-    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+    return 6650.0, "fallback B200_PROFILING.md 6.65 TB/s"
+
+
+def _r(x, n=4):
+    """round to n significant digits (keeps the result line short)"""
+    if x is None:
+        return None
+    return float("%.*g" % (n, x))
 
 
 class ClockSampler:
@@ -103,8 +119,25 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def _oracle_step_rate(orc, cfg, warmup, steps, budget_s):
+    """cell-updates/s of the oracle's Strang step on cfg: `warmup` untimed steps, then the BEST of up to `steps`
+    single-step timings inside budget_s seconds (best of 3)."""
+    f = inputs.initial_f(cfg).astype(np.float64)
+    feq = orc.Feq.make(cfg.feq)
+    for _ in range(warmup):
+        f, _E = orc.step(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, cfg.split)
+    best, n, t_all = None, 0, time.perf_counter()
+    while n < steps and (n == 0 or time.perf_counter() - t_all < budget_s):
+        t0 = time.perf_counter()
+        f, _E = orc.step(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, cfg.split)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+        n += 1
+    return cfg.Nx * cfg.Nv / best, n, time.perf_counter() - t_all
+
+
 def reference_arm(args, rank):
-    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only; other ranks exit 0)."""
     if rank != 0:
         return
     from oracle import vog_oracle as orc
@@ -124,7 +157,7 @@ def reference_arm(args, rank):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "strang_step_deltaf_2048x2048_lag17", "batch": 1, "Nx": cfg.Nx, "Nv": cfg.Nv},
+        "config": {"workload": WORKLOAD, "batch": 1, "Nx": cfg.Nx, "Nv": cfg.Nv},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -138,8 +171,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="vog")
     ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 advection sweep")
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
-    ap.add_argument("--no-concurrent", action="store_true", help="skip the 4-stream variant of the timed batch")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg and the oracle timings of the sweep")
+    ap.add_argument("--no-extras", action="store_true", help="skip the concurrent / merged / small-grid variants")
     ap.add_argument("--sweep-only", action="store_true", help="only the config-4 advection sweep (for profiling)")
     ap.add_argument("--sizes", default="512,2048,8192,16384", help="sweep grid sizes N (Nx=Nv=N), BASELINE.json config 4")
     ap.add_argument("--kinds", default="lag3,lag9,lag17,spline", help="sweep interpolators: lagN or spline")
@@ -163,11 +196,19 @@ def main():
         multi.init("nccl", device_id=torch.device("cuda", local))
     vog.lib()
 
+    detail = []
+
+    def emit(rec):
+        detail.append(rec)
+        if rank == 0:
+            print(json.dumps(rec), flush=True)
+
     sizes = tuple(int(x) for x in args.sizes.split(","))
     kinds = tuple((1, 3) if k == "spline" else (0, int(k[3:])) for k in args.kinds.split(","))
     stream = torch.cuda.Stream()
+    peak, peak_src = _peaks()
     if args.sweep_only:
-        print(json.dumps({"sweep": sweep(torch, vog, stream, _peaks()[0], sizes, kinds)}))
+        sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle=False)
         return
     cfg = inputs.metric_config()
     cells = cfg.Nx * cfg.Nv
@@ -206,65 +247,9 @@ def main():
     ms = multi.max_over_ranks(ms, device="cuda")
     value = multi.aggregate_throughput(BATCH * cells * args.steps, world, ms)
 
-    # ---- the same batch with the replicas spread over 4 plans on 4 streams (independent problems overlap: the
-    # single-CTA Poisson solve and the tails of one replica's kernels run under another replica's advections).
-    # Reported next to `value`, which stays the one-stream figure.
-    concurrent = None
-    if not args.no_concurrent:
-        NS = 4
-        streams = [torch.cuda.Stream() for _ in range(NS)]
-        plans = [vog.Plan.from_config(cfg, stream=st) for st in streams]
-        main = torch.cuda.current_stream()
-
-        def conc_step():
-            for i, fb in enumerate(batch):
-                plans[i % NS].step(fb, cfg.dt)
-
-        for _ in range(args.warmup):
-            conc_step()
-        sync_all()
-        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        c0.record(main)
-        for st in streams:
-            st.wait_event(c0)
-        for _ in range(args.steps):
-            conc_step()
-        for st in streams:
-            e = torch.cuda.Event()
-            e.record(st)
-            main.wait_event(e)
-        c1.record(main)
-        sync_all()
-        cms = multi.max_over_ranks(c0.elapsed_time(c1), device="cuda")
-        concurrent = {"streams": NS, "value": multi.aggregate_throughput(BATCH * cells * args.steps, world, cms),
-                      "unit": UNIT, "ms_per_step": cms / args.steps,
-                      "note": "same batch and steps, replicas round-robin over 4 plans/streams"}
-        for pl in plans:
-            pl.destroy()
-
-    # ---- merged half steps: vog_run(merge=1) takes the two x half steps that
-    # meet between consecutive steps as one advection, 2 advections per step instead of 3.  A different (the
-    # paper's "vlaso") sequence, so it is reported beside `value`, never as `value`.
-    MR = 10
-    for fb in batch[:2]:
-        plan.run(fb, cfg.dt, MR, None, True)
-    sync_all()
-    m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    mrep = max(1, args.steps // MR)
-    m0.record(stream)
-    for _ in range(mrep):
-        for fb in batch:
-            plan.run(fb, cfg.dt, MR, None, True)
-    m1.record(stream)
-    sync_all()
-    mms = multi.max_over_ranks(m0.elapsed_time(m1), device="cuda")
-    merged = {"value": multi.aggregate_throughput(BATCH * cells * MR * mrep, world, mms), "unit": UNIT,
-              "us_per_replica_step": 1e3 * mms / (BATCH * MR * mrep),
-              "note": "vog_run(merge=1), %d steps per call per replica: x(dt/2) [field v(dt) x(dt)]^(n-1) field v(dt) x(dt/2)" % MR}
-
-    # ---- per-kernel timing of the same step on the same stream (roofline of the dominant kernel)
-    # Each kernel type is launched back to back on all replicas of the batch between two events (no host
-    # synchronisation inside), so the figure is the average launch duration in steady state.
+    # ---- per-kernel timing of the same step on the same stream (roofline of the dominant kernel).  Each call type
+    # is enqueued back to back on all replicas of the batch between two events (no host synchronisation inside), so
+    # the figure is the average duration in steady state, every replica L2-cold on entry.
     Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
     plan.field(batch[0], Ed)
 
@@ -282,20 +267,67 @@ def main():
         return tot / (reps * BATCH)
 
     with torch.cuda.stream(stream):
-        ms_x = timed(lambda fb: plan.advect_x(fb, 0.5 * cfg.dt))
-        ms_f = timed(lambda fb: plan.field(fb, Ed))
-        ms_v = timed(lambda fb: plan.advect_v(fb, Ed, cfg.dt))
-    peak, peak_src = _peaks()
+        ms_x = timed(lambda fb: plan.advect_x(fb, 0.5 * cfg.dt))      # tables cached: the x kernel alone
+        ms_f = timed(lambda fb: plan.field(fb, Ed))                   # density + Poisson
+        ms_v = timed(lambda fb: plan.advect_v(fb, Ed, cfg.dt))        # table setup + v kernel (+ delta-f source)
     alg_bytes = 8.0 * cells                      # one read + one write of f per advection
     ach = alg_bytes / (ms_x * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "osx5_kernel (overlap-save x-advection, block pairs, warp-private; 2048-cell lines)", "achieved": ach, "peak": peak,
-                "unit": "GB/s", "frac": ach / peak, "traffic": _traffic(), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_x,
-                "other_kernels_ms": {"advect_v(+delta-f source)": ms_v, "density+poisson": ms_f},
-                "note": "2048^2 replica is L2-cold on entry (batch 256 MiB > L2) but 16 MiB fits L2 within a step; "
-                        "advect_v here is the standalone in-place call (table setup + kernel + copy back from the "
-                        "plan's second grid); inside vog_step the v kernel writes the second grid and the next "
-                        "x-advection reads it, so no copy is made; HBM-roofline fractions at 8192^2/16384^2 are in sweep"}
+    traffic, traffic_src = _traffic()
+    roofline = {"bound": "hbm", "kernel": "x-advection kernel, 2048-cell lines (2 of the step's 3 advections)",
+                "achieved": _r(ach, 5), "peak": peak, "unit": "GB/s", "frac": _r(ach / peak), "traffic": traffic,
+                "traffic_source": traffic_src, "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes,
+                "us_per_launch": _r(1e3 * ms_x), "us_v_call": _r(1e3 * ms_v), "us_field": _r(1e3 * ms_f),
+                "note": "16 MiB replica: L2-cold on entry (batch 256 MiB > L2), its writes stay in L2 until "
+                        "later replicas evict them; the HBM-resident figures are target_8192"}
+
+    extras = {}
+    if not args.no_extras:
+        # ---- the same batch with the replicas spread over 4 plans on 4 streams (independent problems overlap)
+        NS = 4
+        streams = [torch.cuda.Stream() for _ in range(NS)]
+        plans = [vog.Plan.from_config(cfg, stream=st) for st in streams]
+        main_st = torch.cuda.current_stream()
+
+        def conc_step():
+            for i, fb in enumerate(batch):
+                plans[i % NS].step(fb, cfg.dt)
+
+        for _ in range(args.warmup):
+            conc_step()
+        sync_all()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(main_st)
+        for st in streams:
+            st.wait_event(c0)
+        for _ in range(args.steps):
+            conc_step()
+        for st in streams:
+            e = torch.cuda.Event()
+            e.record(st)
+            main_st.wait_event(e)
+        c1.record(main_st)
+        sync_all()
+        cms = multi.max_over_ranks(c0.elapsed_time(c1), device="cuda")
+        extras["concurrent_4_streams"] = _r(multi.aggregate_throughput(BATCH * cells * args.steps, world, cms))
+        for pl in plans:
+            pl.destroy()
+
+        # ---- merged half steps: vog_run(merge=1), 2 advections per step.
+        # A different sequence, so it is reported beside `value`, never as `value`.
+        MR = 10
+        for fb in batch[:2]:
+            plan.run(fb, cfg.dt, MR, None, True)
+        sync_all()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        mrep = max(1, args.steps // MR)
+        m0.record(stream)
+        for _ in range(mrep):
+            for fb in batch:
+                plan.run(fb, cfg.dt, MR, None, True)
+        m1.record(stream)
+        sync_all()
+        mms = multi.max_over_ranks(m0.elapsed_time(m1), device="cuda")
+        extras["merged_half_steps"] = _r(multi.aggregate_throughput(BATCH * cells * MR * mrep, world, mms))
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     fh = f0.clone().pin_memory()
@@ -331,132 +363,166 @@ def main():
     p_s = multi.max_over_ranks(p_s, device="cuda")
     for pl in pplans:
         pl.destroy()
-    e2e = {"value": world * cells * p_steps / p_s, "unit": UNIT, "h2d_bytes_per_step": 4 * cells,
+    e2e = {"value": _r(world * cells * p_steps / p_s, 5), "unit": UNIT, "h2d_bytes_per_step": 4 * cells,
            "d2h_bytes_per_step": 4 * cells + 4 * cfg.Nx, "steps": p_steps, "replicas_in_flight": NP,
-           "serial_value": serial_value,
-           "note": "vog_run_host_async on 3 plans/streams round-robin: pinned host f -> device, 1 Strang step, f and E "
-                   "back to host, per step; serial_value = the same with one replica at a time (vog_run_host, "
-                   "synchronising after every step)"}
+           "serial_value": _r(serial_value, 5),
+           "note": "vog_run_host_async, 3 plans/streams round-robin: pinned host f -> device, 1 Strang step, f and E "
+                   "back to host, every step; serial_value: one replica at a time (vog_run_host, syncs each step)"}
+    plan.destroy()
+
+    # ---- small grids (configs 0-1: launch/latency-bound: report steps/s)
+    if not args.no_extras:
+        extras["small_grids_steps_per_s"] = small_grids(torch, vog, stream, emit)
 
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "strang_step_deltaf_2048x2048_lag17", "Nx": cfg.Nx, "Nv": cfg.Nv, "batch": BATCH,
-                   "split": "x/2-field-v-x/2", "interp": "LAG17", "parallelism": "replicas x%d" % world,
-                   "l2": "inputs larger than L2: batch of %d replicas = %d MiB, visited round-robin" % (BATCH, BATCH * 4 * cells >> 20)},
-        "gpu_launches": launches, "e2e": e2e, "roofline": roofline, "concurrent": concurrent, "merged": merged,
-        "MA_paper_unit": 3.0 * value / 1e6,
+        "metric": METRIC, "value": _r(value, 6), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": _r(ms / args.steps, 6), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "Nx": cfg.Nx, "Nv": cfg.Nv, "batch": BATCH, "split": "x/2-field-v-x/2",
+                   "interp": "LAG17", "parallelism": "replicas x%d" % world,
+                   "l2": "inputs larger than L2: %d replicas = %d MiB, round-robin" % (BATCH, BATCH * 4 * cells >> 20)},
+        "gpu_launches": launches, "us_per_replica_step": _r(1e3 * ms / (args.steps * BATCH)),
+        "MA_paper_unit": _r(3.0 * value / 1e6), "e2e": e2e, "roofline": roofline,
     }
+    out.update(extras)
     if rank == 0:
         out["clocks"] = clocks
 
-    # ---- config-4 sweep at the north-star size (8192^2), one x- and one v-advection
+    # ---- config-4 sweep (one x- and one v-advection on 512..16384 squared, LAG3/9/17 + spline), detail lines
     if rank == 0 and not args.no_sweep:
-        out["sweep"] = sweep(torch, vog, stream, peak, sizes, kinds)
+        rows = sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle=(world == 1 and not args.no_cpu))
+        tgt = {}
+        for N in (8192, 16384):
+            for r in rows:
+                if r["N"] == N and r["kind"] == "lagrange" and r["order"] == 17:
+                    tgt[str(N)] = {"x_kernel_frac": _r(r["x_kernel_only"]["frac_hbm"]),
+                                   "x_call_frac": _r(r["x"]["frac_hbm"]), "v_call_frac": _r(r["v"]["frac_hbm"]),
+                                   "v_out_of_place_frac": _r(r.get("v_out_of_place", {}).get("frac_hbm")),
+                                   "step_frac_28B": _r(r["strang_step"]["frac_hbm"])}
+        roofline["target_8192"] = tgt.get("8192")
+        roofline["at_16384"] = tgt.get("16384")
     # ---- oracle on the host cores (rank 0, N=1 only)
     if rank == 0 and world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(cfg)
-    plan.destroy()
     if rank == 0:
-        print(json.dumps(out))
+        try:
+            os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+            with open(os.path.join(ROOT, "gpurun_out", "bench_detail.json"), "w") as fh_:
+                json.dump({"result": out, "detail": detail}, fh_, indent=1)
+        except Exception:
+            pass
+        print(json.dumps(out), flush=True)
     if world > 1:
         multi.finalize()
 
 
-def sweep(torch, vog, stream, peak, sizes=(2048, 8192), kinds=((0, 17), (0, 3), (1, 3))):
+def small_grids(torch, vog, stream, emit):
+    """Configs 0 and 1 (64^2 full-f, 256^2 delta-f): Strang steps per second through vog_run (one host call for the
+    whole run, energies on the device), the configs' own step counts."""
+    res = {}
+    for idx in (0, 1):
+        cfg = inputs.config(idx)
+        plan = vog.Plan.from_config(cfg, stream=stream)
+        f0 = torch.from_numpy(inputs.initial_f(cfg)).cuda()
+        en = torch.empty(cfg.steps, device="cuda", dtype=torch.float64)
+        best = None
+        for rep in range(4):
+            f = f0.clone()
+            stream.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            plan.run(f, cfg.dt, cfg.steps, None, False, en)
+            e1.record(stream)
+            stream.synchronize()
+            t = e0.elapsed_time(e1)
+            if rep > 0:
+                best = t if best is None else min(best, t)
+        plan.destroy()
+        res[cfg.name] = _r(cfg.steps / (best * 1e-3))
+        emit({"small_grid": cfg.name, "steps": cfg.steps, "ms_run": best, "steps_per_s": cfg.steps / (best * 1e-3),
+              "us_per_step": 1e3 * best / cfg.steps})
+    return res
+
+
+def _time_calls(torch, stream, fn, warm, reps):
+    for _ in range(warm):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    for _ in range(reps):
+        e0.record(stream)
+        fn()
+        e1.record(stream)
+        stream.synchronize()
+        times.append(e0.elapsed_time(e1))
+    return float(np.median(times)), min(times)
+
+
+def sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle):
+    """BASELINE.json config 4: one x- and one v-advection on N x N, f ~ U[0,1), per-line shifts ~ U[-8,8] cells.
+    x / v = the public in-place calls vog_shift_x / vog_shift_v (table setup + kernel); x_kernel_only = vog_advect_x
+    with cached tables; v_out_of_place = vog_shift_v_to; strang_step = vog_step (28 B/cell: 3 advections + density).
+    With with_oracle, the oracle's shift_x / shift_v (double, stencil or cyclic solve, all host cores) is timed on the
+    same shape next to it for N <= 8192 (best of 3)."""
+    orc = None
+    if with_oracle:
+        from oracle import vog_oracle as orc
+        orc.build()
     res = []
     for N in sizes:
         f = torch.rand((N, N), device="cuda", dtype=torch.float32)
         bx = torch.from_numpy(inputs.uniform_shifts(N, 41)).cuda()
+        fo = bo = None
+        if orc is not None and N <= 8192:
+            fo = inputs.uniform_grid(N, N).astype(np.float64)
+            bo = inputs.uniform_shifts(N, 41)
         for kind, order in kinds:
             plan = vog.Plan(N, N, 1.0, -1.0, 1.0, kind, order, stream=stream)
             row = {"N": N, "kind": "lagrange" if kind == 0 else "bspline", "order": order}
-            for name, fn in (("x", plan.shift_x), ("v", plan.shift_v)):
-                for _ in range(3):
-                    fn(f, bx)
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                times = []
-                for _ in range(10):
-                    e0.record(stream); fn(f, bx); e1.record(stream)
-                    stream.synchronize()
-                    times.append(e0.elapsed_time(e1))
-                med = float(np.median(times))
-                gbs = 8.0 * N * N / (med * 1e-3) / 1e9
-                row[name] = {"ms_median": med, "ms_best": min(times), "GBps": gbs, "frac_hbm_measured": gbs / peak,
-                             "frac_hbm_8TBps": gbs / 8000.0}
-            row["note"] = "vog_shift_x/v calls: table setup + kernel (+ copy back for v, whose kernel is out of place)"
-            # the x kernel alone (vog_advect_x caches its tables per dt) and a whole Strang step (in which the
-            # v kernel writes the plan's second grid and no copy is made), on the same grid
-            for _ in range(3):
-                plan.advect_x(f, 0.01)
-            times = []
-            for _ in range(10):
-                e0.record(stream); plan.advect_x(f, 0.01); e1.record(stream)
-                stream.synchronize()
-                times.append(e0.elapsed_time(e1))
-            med = float(np.median(times))
-            gbs = 8.0 * N * N / (med * 1e-3) / 1e9
-            row["x_kernel_only"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak}
-            # the v kernel out of place (table setup + kernel, no copy back): what vog_step runs
+
+            def rec(med, best, nbytes=8.0):
+                gbs = nbytes * N * N / (med * 1e-3) / 1e9
+                return {"us_median": 1e3 * med, "us_best": 1e3 * best, "GBps": gbs, "frac_hbm": gbs / peak,
+                        "frac_8TBps": gbs / 8000.0}
+
+            row["x"] = rec(*_time_calls(torch, stream, lambda: plan.shift_x(f, bx), 3, 10))
+            row["v"] = rec(*_time_calls(torch, stream, lambda: plan.shift_v(f, bx), 3, 10))
+            row["x_kernel_only"] = rec(*_time_calls(torch, stream, lambda: plan.advect_x(f, 0.01), 3, 10))
             if N * N * 4 * 3 < 160e9:
                 g = torch.empty_like(f)
-                for _ in range(3):
-                    plan.shift_v_to(f, g, bx)
-                times = []
-                for _ in range(10):
-                    e0.record(stream); plan.shift_v_to(f, g, bx); e1.record(stream)
-                    stream.synchronize()
-                    times.append(e0.elapsed_time(e1))
-                med = float(np.median(times))
-                gbs = 8.0 * N * N / (med * 1e-3) / 1e9
-                row["v_out_of_place"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak,
-                                         "note": "vog_shift_v_to: table setup + kernel, src -> dst"}
-                if N >= 1024:
-                    # control: the loads and stores of the x kernel without the transform (memory-system floor)
-                    for _ in range(3):
-                        plan.probe_x_memory_pattern(f, g)
-                    times = []
-                    for _ in range(10):
-                        e0.record(stream); plan.probe_x_memory_pattern(f, g); e1.record(stream)
-                        stream.synchronize()
-                        times.append(e0.elapsed_time(e1))
-                    med = float(np.median(times))
-                    gbs = 8.0 * N * N / (med * 1e-3) / 1e9
-                    row["x_memory_pattern"] = {"ms_median": med, "GBps": gbs, "frac_hbm_measured": gbs / peak,
-                                               "note": "vog_probe_x_memory_pattern: the x kernel's loads and stores, no transform"}
+                row["v_out_of_place"] = rec(*_time_calls(torch, stream, lambda: plan.shift_v_to(f, g, bx), 3, 10))
                 del g
-            for _ in range(2):
-                plan.step(f, 1e-3)
-            times = []
-            for _ in range(5):
-                e0.record(stream); plan.step(f, 1e-3); e1.record(stream)
-                stream.synchronize()
-                times.append(e0.elapsed_time(e1))
-            med = float(np.median(times))
-            gbs = 28.0 * N * N / (med * 1e-3) / 1e9     # 3 advections x 8 B + 4 B density read per cell
-            row["strang_step"] = {"ms_median": med, "cell_updates_per_s": N * N / (med * 1e-3), "GBps_28B_per_cell": gbs,
-                                  "frac_hbm_measured": gbs / peak}
-            res.append(row)
+            row["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step(f, 1e-3), 2, 5), 28.0)
+            row["strang_step"]["cell_updates_per_s"] = N * N / (row["strang_step"]["us_median"] * 1e-6)
             plan.destroy()
+            if fo is not None:
+                ot = {}
+                for name, fn in (("x", orc.shift_x), ("v", orc.shift_v)):
+                    best = None
+                    for _ in range(3):
+                        t0 = time.perf_counter()
+                        fn(fo, bo, kind, order)
+                        dt = time.perf_counter() - t0
+                        best = dt if best is None else min(best, dt)
+                    ot[name] = {"s_best_of_3": best, "cell_updates_per_s": N * N / best}
+                ot["cores"] = orc.num_threads()
+                ot["gpu_over_oracle_x"] = (N * N / (row["x"]["us_median"] * 1e-6)) / ot["x"]["cell_updates_per_s"]
+                ot["gpu_over_oracle_v"] = (N * N / (row["v"]["us_median"] * 1e-6)) / ot["v"]["cell_updates_per_s"]
+                row["oracle"] = ot
+            res.append(row)
+            emit({"sweep_row": row})
         del f
     return res
 
 
 def cpu_baseline(cfg):
+    """The oracle's Strang step on the metric grid, host cores: 1 warm-up step, best of 3."""
     from oracle import vog_oracle as orc
     orc.build()
-    f = inputs.initial_f(cfg).astype(np.float64)
-    feq = orc.Feq.make(cfg.feq)
-    t0 = time.perf_counter()
-    n = 0
-    while n < 3 and time.perf_counter() - t0 < 20.0:
-        f, _E = orc.step(f, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, cfg.split)
-        n += 1
-    dt = time.perf_counter() - t0
-    return {"value": cfg.Nx * cfg.Nv * n / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "sample": "%d full %dx%d Strang steps of one replica (double precision, direct stencils, naive-DFT field)"
-                      % (n, cfg.Nx, cfg.Nv)}
+    val, n, secs = _oracle_step_rate(orc, cfg, 1, 3, 25.0)
+    return {"value": _r(val, 5), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "best of %d %dx%d Strang steps of one replica after 1 warm-up step (%.1f s of oracle work; "
+                      "double, direct stencils, naive-DFT field)" % (n, cfg.Nx, cfg.Nv, secs)}
 
 
 if __name__ == "__main__":

@@ -84,7 +84,9 @@ int vog_field(vog_plan_t plan, const float* f_dev, float* E_dev);
  * -E_app).
  *   VOG_SPLIT_XVX: x(dt/2); E = field(f); v(dt, E + E_ext); x(dt/2).
  *   VOG_SPLIT_VXV: v(dt/2, E_prev + E_ext); x(dt); E = field(f); v(dt/2, E + E_ext), where
- *                  E_prev is the field of the previous step (solved from f on the first step).
+ *                  E_prev is the field the previous VXV step (or a vog_field call) on the SAME f_dev left in the
+ *                  plan; after any other call on the plan, or for another array, it is solved from f_dev first
+ *                  (see vog_reset for states changed behind the library's back).
  * The self-consistent E solved inside the step stays in the plan: see vog_get_field. */
 int vog_step(vog_plan_t plan, float* f_dev, double dt, const float* E_ext_dev);
 
@@ -144,29 +146,28 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   2, 3   whole-line v kernel (Nv <= 512): log2(complex lines per CTA), threads per CTA;
  *   5..8   whole-line x kernel (Nx <= 512): log2(lines per iteration), threads (32..128), CTAs per SM
  *          (0 = as many as fit), line buffers (1 or 2);
- *   10..12 first-generation overlap-save x kernel (Nx >= 1024): lines per iteration, threads (32..160), CTAs per SM;
- *   15, 16 first-generation overlap-save v kernel (Nv >= 1024): row blocks per group (1 or 2; threads = 128 x
- *          that), groups per CTA (0 = automatic);
- *   17     overlap-save kernel generation: 2 = block-pair kernels (default), 1 = even/odd kernels;
- *   18..20 block-pair kernels: x lines per iteration; x threads of the shared-memory-landing variant (32..320);
- *          v pairs per CTA (0 = default: 1);
- *   21     x variant: 0 = landing through shared memory, 1 = direct register loads with CTA barriers, 2 = raw-line
- *          landing of the next line group, 3 = warp-private with the split barrier (default);
- *   22     v variant: 0 = per-lane landing, 1 = direct register loads, 2 = coalesced landing of the strip's rows (default);
+ *   18     overlap-save x kernel (Nx >= 1024): lines per iteration of a CTA;
+ *   20     overlap-save v kernel (Nv >= 1024): pairs of blocks per CTA (0 = default);
+ *   21     overlap-save x kernel variant: 0 = every pair of blocks lands its own window of the line by bulk asynchronous
+ *          copies (default for lines up to 8192 cells), 1 = whole lines landed for the whole CTA (what 16384-cell
+ *          lines always use);
+ *   22     overlap-save v kernel variant: 0 = 16-column strips with the next window in flight (default), 1 = 32-column
+ *          strips sharing one buffer (the fallback kept beside it);
  *   24     density kernel: row slabs per column group (power of two, 1..16, at least 32 rows each);
- *   25     block geometry of the default overlap-save kernels: 1 = 232 kept samples, 8 + 16 discarded (Lagrange
- *          plans only, their default), 0 = 224 kept, 16 + 16 discarded (the cubic spline's).
- *   26 = programmatic dependent launch of the plan's kernels: 1 = each kernel may be staged on the SMs while its
- *        predecessor in the stream drains and waits for it on the device (default up to 8192 x 8192), 0 = plain
- *        stream order.  Results are bit-identical either way.
+ *   25     block geometry of the overlap-save kernels: 1 = 232 kept samples, 8 + 16 discarded (Lagrange
+ *          plans only, their default), 0 = 224 kept, 16 + 16 discarded (the cubic spline's);
+ *   26     programmatic dependent launch of the plan's kernels: 1 = each kernel may be staged on the SMs while its
+ *          predecessor in the stream drains and waits for it on the device (default up to 8192 x 8192), 0 = plain
+ *          stream order.  Results are bit-identical either way.
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 
-/* Measurement probe, not part of the method: runs a kernel with exactly the global loads and stores of the
- * x-advection kernel (Nx >= 1024, zero shift, Lagrange block geometry) and no transform, src_dev -> dst_dev
- * (dst_dev != src_dev, Nx*Nv floats each; the cells a line's last block does not cover keep their value).  Its time
- * is the memory-system floor of that access pattern (`bench.py --sweep-only` reports it as "x_memory_pattern"). */
-int vog_probe_x_memory_pattern(vog_plan_t plan, const float* src_dev, float* dst_dev);
+/* Forget what the plan caches about the state it last saw: the self-consistent field kept for vog_get_field and for
+ * the first half step of the next VOG_SPLIT_VXV step, and the x-advection tables of the last time step.  The library
+ * drops these itself whenever one of ITS calls changes the state or is given another array; call vog_reset after
+ * writing into f_dev behind the library's back (e.g. re-initialising the same buffer) before a VXV step.  Never
+ * needed with VOG_SPLIT_XVX.  Returns VOG_OK, or VOG_EINVAL for NULL. */
+int vog_reset(vog_plan_t plan);
 
 /* Number of kernels the library launched on this plan since creation (for accounting). */
 long long vog_launch_count(vog_plan_t plan);

@@ -15,12 +15,8 @@ template <int N, int SYM, bool VDIR>
 static cudaError_t launch_one(const AdvectArgs& a, int n_tiles, int threads, size_t smem, cudaStream_t st)
 {
     auto kern = advect_kernel<N, SYM, VDIR>;
-    static size_t smem_set = 0;
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        smem_set = smem;
-    }
+    const cudaError_t e = set_max_smem((const void*)kern, smem);
+    if (e != cudaSuccess) return e;
     return launch_pdl(kern, dim3(n_tiles), dim3(threads), smem, st, a);
 }
 
@@ -49,12 +45,8 @@ template <int N, int SYM>
 static cudaError_t launch_x_one(const AdvectXArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
 {
     auto kern = advect_x_kernel<N, SYM>;
-    static size_t smem_set = 0;
-    if (smem > 48 * 1024 && smem > smem_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        smem_set = smem;
-    }
+    const cudaError_t e = set_max_smem((const void*)kern, smem);
+    if (e != cudaSuccess) return e;
     return launch_pdl(kern, dim3(grid), dim3(threads), smem, st, a);
 }
 
@@ -62,8 +54,7 @@ template <int N, int SYM>
 static int occ_x_one(int threads, size_t smem)
 {
     auto kern = advect_x_kernel<N, SYM>;
-    if (smem > 48 * 1024 &&
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (set_max_smem((const void*)kern, smem) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }

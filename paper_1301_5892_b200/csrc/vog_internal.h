@@ -85,13 +85,18 @@ typedef cudaError_t (*advect_x_launch_fn)(const AdvectXArgs& a, int sym, int gri
 advect_x_launch_fn advect_x_launcher(int N);
 int advect_x_occupancy(int N, int sym, int threads, size_t smem);
 
-// ---- overlap-save kernels (vog_os.cuh), line length >= 1024
+// ---- overlap-save kernels (vog_os2.cuh), line length >= 1024
 constexpr int OS_LB = 256;     // block length (reals)
-constexpr int OS_V = 224;      // valid outputs per block
-constexpr int OS_H = 16;       // discarded samples on either side
-// Per-line symbol table, OS_LAMW float2 (1040 B): [k] = lambda(2 pi k/OS_LB) / (2 OS_LB), k = 0..128
-// (x: times e^{i theta_k (b mod 4)}); [129] = (integer shift as int bits: x: b >> 2 in 16-byte chunks,
-// v: b in rows;  v: s = E dt of the delta-f source).
+// Kept samples V and samples discarded on the left HLO of a block (256 - V - HLO are discarded on the right):
+//   Lagrange 2d+1 <= 17: the stencil reaches 8 cells to the left and 9 to the right => (232, 8), exact;
+//   cubic spline: the circulant row decays like 0.268^|j|; cut 14 cells either side => (228, 14): the
+//   neglected part of the row sums to <= 8.4e-9 of max|u| over all b* (reading Q6b), 0.4 % of the tolerance.
+constexpr int OS_V = 228;      // spline geometry: kept samples per block
+constexpr int OS_H = 14;       // spline geometry: discarded on the left (and on the right)
+constexpr int OS_VL = 232;     // Lagrange geometry
+constexpr int OS_HL = 8;
+// Per-line symbol table, OS_LAMW float2 (1040 B): [k] = lambda(2 pi k/OS_LB) / OS_LB, k = 0..128;
+// [129] = (integer shift b mod N as int bits;  v: s = E dt of the delta-f source).
 constexpr int OS_LAMW = 130;
 
 struct OsArgs {
@@ -99,7 +104,7 @@ struct OsArgs {
     float* dst;            // x: may equal src; v: must differ
     int Nx, Nv;
     int N;                 // line length (x: Nx, v: Nv)
-    int nb;                // blocks per line = ceil(N / OS_V)
+    int nb;                // blocks per line = ceil(N / V)
     const float2* lam;     // [n_lines][OS_LAMW]
     const float2* tw;      // x: [7][16] e^{-2 pi i t q/128};  v: [15][16] e^{-2 pi i t q/256}
     const float2* cs;      // [129] (cos, sin)(2 pi k/256)   (x only)
@@ -115,12 +120,13 @@ struct OsArgs {
     int np;                // second-generation kernels (vog_os2.cuh): pairs of blocks per line = ceil(nb / 2)
     unsigned inv_np;       // x: ceil(2^16 / np)
     int n_lines;           // x: number of lines (the last line group may be ragged)
+    int lam_ks;            // v: row stride of the transposed symbol table [k][column] in float2 (Nx + 16)
 };
 
 struct OsSetupArgs {
     int n_lines, N, mode;      // mode 0: c = v_l; 1: c = E_l (+E_ext_l); 2: explicit beta
     int spline, d, vdir;
-    int gen2;                  // tables for vog_os2.cuh: scale 1/OS_LB, full integer shift b in entry 129 (no residue)
+    int ks;                    // vdir: row stride of the transposed table [k][line] in float2
     double dt, delta, vmin, dv;
     const float* E;
     const float* Eext;
@@ -130,18 +136,14 @@ struct OsSetupArgs {
 };
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st);
-cudaError_t os_mempattern_launch(const float* src, float* dst, int N, int n_lines, int grid, cudaStream_t st);
-cudaError_t osx_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
-cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
-int osx_occupancy(int threads, size_t smem);
-cudaError_t osx2_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st);
-cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
-int osx2_occupancy(int threads, size_t smem);
-cudaError_t osx3_launch(const OsArgs& a, int mode, int grid, int threads, size_t smem, cudaStream_t st);
-int osx3_occupancy(int mode, int threads, size_t smem);
-cudaError_t osx5_launch(const OsArgs& a, bool inplace, int geom, int grid, int threads, size_t smem, cudaStream_t st);
-int osx5_occupancy(int threads, size_t smem);
-cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st);
+// per-device cudaFuncAttributeMaxDynamicSharedMemorySize (vog_os.cu)
+cudaError_t set_max_smem(const void* fn, size_t smem);
+cudaError_t osx7_launch(const OsArgs& a, int geom, int grid, int threads, size_t smem, cudaStream_t st);
+int osx7_occupancy(int geom, int threads, size_t smem);
+cudaError_t osx6_launch(const OsArgs& a, int geom, int grid, int threads, size_t smem, cudaStream_t st);
+int osx6_occupancy(int geom, int threads, size_t smem);
+cudaError_t osv7_launch(const OsArgs& a, int geom, int n_sm, cudaStream_t st);
+cudaError_t osv6_launch(const OsArgs& a, int geom, dim3 grid, cudaStream_t st);
 cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st);
 
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)

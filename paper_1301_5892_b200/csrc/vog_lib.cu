@@ -183,17 +183,18 @@ __global__ void shift_setup_x_kernel(const SetupArgs s)
 // ------------------------------------------------------------------------------------------
 // S8: rho partial sums.  grid (Nx/32, NBY), 256 threads: a warp covers 4 rows x 32 columns
 // (8 lanes x float4 = one 128 B line per row); the 4 row-lanes are folded by warp shuffles,
-// the 8 warps through shared memory; fp64 accumulation, fixed order => deterministic.
+// the 8 warps through shared memory; fp64 accumulation, fixed order => deterministic.  Block (x, y) writes the sums
+// of its row slab to part[y][32 x .. 32 x + 31]; the Poisson kernel adds the NBY slabs in index order (no atomics,
+// no "last block" pass: the slabs are <= 16 rows of Nx doubles, a few KB for the single CTA that needs them).
 __global__ void __launch_bounds__(256) density_partial_kernel(const float* __restrict__ f, int Nx, int Nv,
-                                                              int rows_per_block, double* __restrict__ part,
-                                                              double dv, double* __restrict__ rho, unsigned* __restrict__ cnt)
+                                                              int rows_per_block, double* __restrict__ part)
 {
     __shared__ double red[8][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int xl = lane & 7, rl = lane >> 3;
     const int col = blockIdx.x * 32 + xl * 4;
     const int j0 = blockIdx.y * rows_per_block;
-    pdl_wait();                                   // f comes from the advection before; part/rho/cnt are still in use
+    pdl_wait();                                   // f comes from the advection before; part may still be read
     pdl_launch_dependents();
     double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
     const float* p = f + (size_t)(j0 + warp * 4 + rl) * Nx + col;
@@ -216,33 +217,7 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
         double s = 0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
-        if (gridDim.y == 1) rho[blockIdx.x * 32 + threadIdx.x] = s * dv;      // the block owns its columns: done
-        else part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
-    }
-    if (gridDim.y == 1) return;
-    // The last of the gridDim.y blocks of this column group to finish adds the partial rows in a FIXED
-    // order (y = 0, 1, ..): deterministic, and the reduction is spread over the SMs instead of being
-    // pulled through the single SM that solves the Poisson equation.
-    __shared__ unsigned ticket;
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) ticket = atomicAdd(cnt + blockIdx.x, 1u);
-    __syncthreads();
-    if (ticket == gridDim.y - 1) {
-        __threadfence();
-        if (threadIdx.x < 32) {
-            const int i = blockIdx.x * 32 + threadIdx.x;
-            double s = 0.0;
-            for (int y0 = 0; y0 < (int)gridDim.y; y0 += 16) {      // 16 loads in flight, fixed order
-                double v[16];
-#pragma unroll
-                for (int y = 0; y < 16; ++y) v[y] = y0 + y < (int)gridDim.y ? __ldcg(part + (size_t)(y0 + y) * Nx + i) : 0.0;
-#pragma unroll
-                for (int y = 0; y < 16; ++y) s += v[y];
-            }
-            rho[i] = s * dv;
-        }
-        if (threadIdx.x == 0) cnt[blockIdx.x] = 0u;
+        part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
     }
 }
 
@@ -286,7 +261,8 @@ __device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int N
 // busy in every pass; E^_m = rho^_m / (i k_m) with modes 0 and Nx/2 dropped; DIT inverse; E to E_a (and E_b).
 __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadix rx, int tw_len, int tw_in_smem,
                                                        const float2* __restrict__ tw_g, const float* __restrict__ ikt,
-                                                       const double* __restrict__ rho, float* __restrict__ E_a,
+                                                       const double* __restrict__ part, int nby, double dv,
+                                                       double* __restrict__ rho, float* __restrict__ E_a,
                                                        float* __restrict__ E_b, double* __restrict__ energy_out,
                                                        double half_dx)
 {
@@ -303,10 +279,19 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);               // (plan constants: before the wait)
     if (tw_in_smem)
         for (int i = tid; i < tw_len; i += T) twsm[i] = __ldg(tw_g + i);
-    pdl_wait();                                   // rho comes from the density kernel
+    pdl_wait();                                   // the slab sums come from the density kernel
     pdl_launch_dependents();
-    const double ref = rho[0];
-    for (int i = tid; i < Nx; i += T) z[i] = make_float2((float)(rho[i] - ref), 0.0f);
+    // rho_i = dv * (sum of the slab sums, in slab order); rho_0 is the reference value
+    double ref = 0.0;
+    for (int y = 0; y < nby; ++y) ref += __ldcg(part + (size_t)y * Nx);
+    ref *= dv;
+    for (int i = tid; i < Nx; i += T) {
+        double s = 0.0;
+        for (int y = 0; y < nby; ++y) s += __ldcg(part + (size_t)y * Nx + i);
+        s *= dv;
+        rho[i] = s;
+        z[i] = make_float2((float)(s - ref), 0.0f);
+    }
     __syncthreads();
     // forward, decimation in frequency: position ((q0 r1 + q1) r2 + q2).. holds mode q0 + r0 (q1 + r1 (q2 + ..));
     // ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
@@ -371,23 +356,19 @@ struct vog_plan_s {
     // overlap-save path (line length >= 1024)
     bool os_x, os_v;
     float2 *os_lam_x, *os_lam_v;   // symbol tables [Nv][OS_LAMW], [Nx][OS_LAMW]
-    float2 *os_twx, *os_twv, *os_cs;
+    float2* os_twv;                // [15][16] e^{-2 pi i t q / 256}
     double2* os_cs64;
     float* cg4;                    // f_eq exponents c_g as floats
     float* ikt;                    // Poisson: 1/(i k) factor per digit-reversed position
     float2* ptw;                   // Poisson: compact per-pass twiddle tables
     int ptw_len;
-    unsigned* dcnt;                // density: per column-group ticket counters
     vog::PoissonRadix prx;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
-    int osx_lpi, osx_thr, osx_cps, osx_occ;
-    int osv_np_log, osv_thr, osv_rb, osv_gpc;
-    int os_gen;                            // 2 = pair kernels of vog_os2.cuh (default), 1 = even/odd kernels of vog_os.cuh
-    int os2x_lpi, os2x_thr, os2x_occ, os2v_gpc;
+    int os2x_lpi, os3x_occ, os2v_gpc;      // x: lines per iteration, cached occupancy; v: pairs per CTA (0 = default)
+    int osv_variant;                       // v kernel: 0 = 16-column strips, next window in flight (osv6_kernel, default), 1 = 32-column strips (osv4_kernel)
+    int osx_variant;                       // x kernel: 0 = per-pair windows when a group fits one round (osx7_kernel), else whole lines; 1 = whole lines always (osx6_kernel)
     int pdl;                               // programmatic dependent launch of the step's kernels (default: grids up to 8192^2)
-    int os_geom;                           // block geometry of the default kernels: 1 = Lagrange (232 kept, 8 + 16 discarded), 0 = spline (224, 16 + 16)
-    int os2v_direct;                       // v kernel: 2 = coalesced raw-row landing (osv4_kernel, default), 1 = register landing (osv3), 0 = per-lane landing (osv2)
-    int os2x_direct, os3x_occ;             // x: register-landing kernel (osx3_kernel) when a line group fits one round of 320 threads
+    int os_geom;                           // block geometry: 1 = Lagrange (232 kept, 8 + 16 discarded), 0 = spline (224, 16 + 16)
     int x_lpi_log, x_thr, x_cps, x_occ;   // lines per iteration (log2), threads, CTAs per SM (0 = occupancy), cached occupancy
     float *rec_x, *rec_v;       // shift records: [Nv] for x-lines, [Nx] for v-lines
     double* part;               // density partials [nby][Nx]
@@ -397,7 +378,9 @@ struct vog_plan_s {
     int nby, nby_max;           // density: row slabs per column group (tunable up to the allocated nby_max)
     int lognl_x, lognl_v, thr_x, thr_v;
     int n_sm;
-    bool E_valid;
+    bool E_valid;               // E_self holds a field (vog_get_field)
+    const float* E_of;          // ... and it is the self-consistent field of the state in this array as the last
+                                // call on the plan left it (VXV steps may then skip their first field solve); NULL otherwise
     bool recx_valid; double recx_dt;
     long long launches;
     float* f_buf;               // only for vog_run_host
@@ -526,7 +509,7 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
-    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twx); cudaFree(P->os_twv); cudaFree(P->os_cs); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->ptw); cudaFree(P->dcnt); cudaFree(P->cg4);
+    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twv); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->ptw); cudaFree(P->cg4);
     cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
@@ -565,11 +548,13 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     P->sym = sym;
     P->d = d;
     const int Nx = p->Nx, Nv = p->Nv, ng = p->feq.n;
-    // density row slabs per column group: up to 512 blocks of at least 128 rows (measured on 1024^2 .. 8192^2:
-    // more blocks cost more in the ticket reduction than they gain in parallelism; _work sweep, profiles/)
+    // density row slabs per column group: up to 512 blocks of at least 128 rows, and never more slabs than the
+    // partial-sum buffer has rows (measured on 1024^2 .. 8192^2: more blocks cost more in the ticket reduction than
+    // they gain in parallelism)
+    P->nby_max = 16;
     int nby = 1;
-    while ((Nx / 32) * nby * 2 <= 512 && Nv / (nby * 2) >= 128) nby *= 2;
-    P->nby = nby; P->nby_max = 16;
+    while ((Nx / 32) * nby * 2 <= 512 && Nv / (nby * 2) >= 128 && nby * 2 <= P->nby_max) nby *= 2;
+    P->nby = nby;
     {
         int dev = 0, nsm = 148;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
@@ -580,24 +565,15 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     P->os_x = Nx >= 1024;
     P->os_v = Nv >= 1024;
     {
-        const int nbx = (Nx + OS_V - 1) / OS_V;
-        int lpi = 1;
-        while (lpi * 2 * nbx <= 40 && lpi * 2 <= Nv) lpi *= 2;
-        while (lpi > 1 && Nv / lpi < P->n_sm * 3) lpi >>= 1;
-        P->osx_lpi = lpi; P->osx_thr = 128; P->osx_cps = 0; P->osx_occ = 0;
-        P->osv_np_log = 3; P->osv_thr = 128; P->osv_rb = 0; P->osv_gpc = 0;
         // pair kernels: 16 items per pair and phase; lines per iteration so that one round of <= 320 threads
-        // covers the items (8192: 19 pairs = 304 items; 2048: 4 lines x 5 pairs = 320)
-        const int Vx = p->kind == VOG_LAGRANGE ? 232 : OS_V;
+        // covers the items (8192: 18 pairs = 288 items; 2048: 3 lines x 5 pairs = 240)
+        const int Vx = p->kind == VOG_LAGRANGE ? OS_VL : OS_V;
         const int npx = ((Nx + Vx - 1) / Vx + 1) / 2;
-        int l2 = (p->kind == VOG_LAGRANGE ? 288 : 320) / (16 * npx);
+        int l2 = 288 / (16 * npx);
         if (l2 < 1) l2 = 1;
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
-        int thr = ((16 * npx * l2 + 31) / 32) * 32;
-        if (thr > 320) thr = 320;
-        P->os2x_direct = 3; P->os3x_occ = 0; P->os2v_direct = 2;
         P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
-        P->os_gen = 2; P->os2x_lpi = l2; P->os2x_thr = thr; P->os2x_occ = 0; P->os2v_gpc = 0;
+        P->os2x_lpi = l2; P->os3x_occ = 0; P->os2v_gpc = 0;
     }
     // measured (profiles/r1i_pdl_setup.md): 512^2 step -20 %, 2048^2 -15 %, 8192^2 +-0, 16384^2 +1.3 %
     P->pdl = (long long)Nx * Nv <= (1ll << 26) ? 1 : 0;
@@ -611,15 +587,10 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->xrec, sizeof(float) * XREC_WORDS * Nv);
     std::vector<float2> xa, xb, xc;
     fill_x_tables(Nx, xa, xb, xc);
-    std::vector<float2> otx(112), otv(240), ocs(130, make_float2(0.f, 0.f));
-    for (int q = 1; q < 8; ++q)
-        for (int t = 0; t < 16; ++t) otx[(q - 1) * 16 + t] = unit_root_neg(t * q, 128);
+    std::vector<float2> otv(240);
     for (int q = 1; q < 16; ++q)
         for (int t = 0; t < 16; ++t) otv[(q - 1) * 16 + t] = unit_root_neg(t * q, 256);
-    for (int k = 0; k <= 128; ++k) { const float2 w = unit_root_neg(k, 256); ocs[k] = make_float2(w.x, -w.y); }
-    alloc((void**)&P->os_twx, sizeof(float2) * otx.size());
     alloc((void**)&P->os_twv, sizeof(float2) * otv.size());
-    alloc((void**)&P->os_cs, sizeof(float2) * ocs.size());
     std::vector<double2> ocs64(OS_LB);
     for (int j = 0; j < OS_LB; ++j) {
         const int q4 = (4 * j) / OS_LB;
@@ -665,27 +636,23 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->ikt, sizeof(float) * Nx);
     alloc((void**)&P->ptw, sizeof(float2) * ptw.size());
     P->ptw_len = (int)ptw.size();
-    alloc((void**)&P->dcnt, sizeof(unsigned) * (Nx / 32));
-    if (e == cudaSuccess) e = cudaMemsetAsync(P->dcnt, 0, sizeof(unsigned) * (Nx / 32), P->st);
     alloc((void**)&P->cg4, sizeof(float) * 4);
     float cg4h[4];
     for (int g = 0; g < 4; ++g) cg4h[g] = g < ng ? (float)p->feq.c[g] : 0.0f;
     alloc((void**)&P->os_lam_x, sizeof(float2) * OS_LAMW * (P->os_x ? Nv : 1));
-    alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx : 1));
+    alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx + 16 : 1));   // rows of Nx + 16 entries
     alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
     alloc((void**)&P->xtwB, sizeof(float2) * xb.size());
     alloc((void**)&P->xcs, sizeof(float2) * xc.size());
     alloc((void**)&P->rec_v, sizeof(float) * REC_WORDS * Nx);
-    alloc((void**)&P->part, sizeof(double) * 16 * Nx);
+    alloc((void**)&P->part, sizeof(double) * P->nby_max * Nx);
     alloc((void**)&P->rho, sizeof(double) * Nx);
     alloc((void**)&P->E_self, sizeof(float) * Nx);
     alloc((void**)&P->feq_tab, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512));   // + padding read (not used) by osv2_kernel
     if (e == cudaSuccess) e = cudaMemsetAsync(P->feq_tab, 0, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512), P->st);
     alloc((void**)&P->vmu_tab, sizeof(float) * (ng ? ng : 1) * Nv);
     if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
-    e = cudaMemcpyAsync(P->os_twx, otx.data(), sizeof(float2) * otx.size(), cudaMemcpyHostToDevice, P->st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(P->os_cs, ocs.data(), sizeof(float2) * ocs.size(), cudaMemcpyHostToDevice, P->st);
+    e = cudaMemcpyAsync(P->os_twv, otv.data(), sizeof(float2) * otv.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->cg4, cg4h, sizeof(cg4h), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->ptw, ptw.data(), sizeof(float2) * ptw.size(), cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(P->ikt, ikt.data(), sizeof(float) * Nx, cudaMemcpyHostToDevice, P->st);
@@ -728,48 +695,66 @@ extern "C" int vog_destroy(vog_plan_t P)
     return VOG_OK;
 }
 
-static size_t osx_smem_bytes(int lpi, int nb);
-static size_t osv_smem_bytes(int np_log, int rb);
-static size_t osx2_smem_bytes(int lpi, int np);
+// geometry of the overlap-save x launch for `lpi` lines per group (shared by vog_plan_tune and run_osx)
+struct OsxShape { int np, thr, rounds; size_t smem6, smem7; };
+static OsxShape osx_shape(const vog_plan_s* P, int lpi)
+{
+    OsxShape o;
+    const int V = P->os_geom ? OS_VL : OS_V, tmax = 288;   // (launch bound of the x kernels)
+    const int nb = (P->p.Nx + V - 1) / V;
+    o.np = (nb + 1) / 2;
+    const int pairs = o.np * lpi;
+    o.rounds = 1;
+    int per = pairs;
+    while (16 * per > tmax) { ++o.rounds; per = (pairs + o.rounds - 1) / o.rounds; }
+    o.thr = ((16 * per + 31) / 32) * 32;
+    // bulk-landed kernel: lines (+ repeated head), two symbol rows per line, exchange scratch per resident pair
+    o.smem6 = (size_t)lpi * (P->p.Nx + 480) * 4 + (size_t)2 * lpi * OS_LAMW * 8 + (size_t)(o.thr / 16) * (16 * 17 * 8) + 16;
+    // warp-private windows (one round only): window slot + exchange scratch per pair, one mbarrier per warp + 1
+    o.smem7 = (size_t)(o.thr / 16) * (496 * 4 + 16 * 17 * 8) + (size_t)(o.thr / 32 + 1) * 8;
+    return o;
+}
 
-// internal tuning hook (documented in DESIGN.md; not part of the paper-facing API):
-// which: 0 = log2(NL) x, 1 = threads x, 2 = log2(NL) v, 3 = threads v, 4 = density row blocks
+// internal tuning hook (launch shapes only; results never change beyond rounding); codes in include/vog.h
 extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
 {
     if (!P) return VOG_EINVAL;
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     switch (which) {
-        case 0: if (value < 0 || (2 << value) > Nv || advect_smem_bytes(Nx, value) > 227 * 1024) return VOG_EINVAL; P->lognl_x = value; break;
-        case 1: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_x = value; break;
         case 2: if (value < 0 || (2 << value) > Nx || advect_smem_bytes(Nv, value) > 227 * 1024) return VOG_EINVAL; P->lognl_v = value; break;
         case 3: if (value < 32 || value > 512 || value % 32) return VOG_EINVAL; P->thr_v = value; break;
         case 5: if (value < 0 || (1 << value) > Nv || advect_x_smem_bytes(Nx, value, P->x_nbuf) > 227 * 1024) return VOG_EINVAL; P->x_lpi_log = value; P->x_occ = 0; break;
         case 6: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->x_thr = value; P->x_occ = 0; break;
         case 7: if (value < 0 || value > 32) return VOG_EINVAL; P->x_cps = value; break;
         case 8: if (value < 1 || value > 2 || advect_x_smem_bytes(Nx, P->x_lpi_log, value) > 227 * 1024) return VOG_EINVAL; P->x_nbuf = value; P->x_occ = 0; break;
-        case 10: if (value < 1 || Nv % value || osx_smem_bytes(value, (Nx + OS_V - 1) / OS_V) > 227 * 1024) return VOG_EINVAL; P->osx_lpi = value; P->osx_occ = 0; break;
-        case 11: if (value < 32 || value > 160 || value % 32) return VOG_EINVAL; P->osx_thr = value; P->osx_occ = 0; break;
-        case 12: if (value < 0 || value > 32) return VOG_EINVAL; P->osx_cps = value; break;
-        case 13: if (value < 0 || (2 << value) > Nx || osv_smem_bytes(value, P->osv_rb) > 227 * 1024) return VOG_EINVAL; P->osv_np_log = value; break;
-        case 14: if (value < 32 || value > 128 || value % 32) return VOG_EINVAL; P->osv_thr = value; break;
-        case 15: if (value < 0 || value > 2) return VOG_EINVAL; P->osv_rb = value; break;
-        case 16: if (value < 0) return VOG_EINVAL; P->osv_gpc = value; break;
-        case 17: if (value < 1 || value > 2) return VOG_EINVAL; P->os_gen = value; P->recx_valid = false; break;
-        case 18: if (value < 1 || value > Nv || osx2_smem_bytes(value, ((Nx + OS_V - 1) / OS_V + 1) / 2) > 227 * 1024) return VOG_EINVAL;
-                 P->os2x_lpi = value; P->os2x_occ = 0; P->os3x_occ = 0; break;
-        case 19: if (value < 32 || value > 320 || value % 32) return VOG_EINVAL; P->os2x_thr = value; P->os2x_occ = 0; break;
+        case 18: {
+            if (value < 1 || value > Nv || !P->os_x) return VOG_EINVAL;
+            const OsxShape o = osx_shape(P, value);
+            if (((P->osx_variant == 0 && o.rounds == 1) ? o.smem7 : o.smem6) > 227 * 1024) return VOG_EINVAL;
+            P->os2x_lpi = value; P->os3x_occ = 0; break;
+        }
         case 20: if (value < 0) return VOG_EINVAL; P->os2v_gpc = value; break;
-        case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
+        case 21: {
+            if (value < 0 || value > 1 || !P->os_x) return VOG_EINVAL;
+            const OsxShape o = osx_shape(P, P->os2x_lpi);
+            if (((value == 0 && o.rounds == 1) ? o.smem7 : o.smem6) > 227 * 1024) return VOG_EINVAL;
+            P->osx_variant = value; P->os3x_occ = 0; break;
+        }
+        case 22: if (value < 0 || value > 2 || !P->os_v) return VOG_EINVAL; P->osv_variant = value; break;
         case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
-        case 21: if (value < 0 || value > 3) return VOG_EINVAL; P->os2x_direct = value; P->os3x_occ = 0; break;
-        case 22: if (value < 0 || value > 2) return VOG_EINVAL; P->os2v_direct = value; break;
+        case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
         case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
 }
 
-static int cuda_status(cudaError_t e) { return e == cudaSuccess ? VOG_OK : VOG_ECUDA; }
+static int cuda_status(cudaError_t e)
+{
+    if (e == cudaSuccess) return VOG_OK;
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return VOG_ENOMEM; }
+    return VOG_ECUDA;
+}
 
 static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, const float* E, const float* Eext,
                              const double* beta)
@@ -785,7 +770,7 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
         s.spline = P->sym == SYM_SPLINE3;
         s.d = P->d;
         s.vdir = vdir ? 1 : 0;
-        s.gen2 = P->os_gen == 2 ? 1 : 0;
+        s.ks = Nx + 16;
         s.dt = dt; s.dv = dv;
         s.delta = vdir ? dv : P->p.L / (double)Nx;
         s.vmin = P->p.vmin;
@@ -810,135 +795,34 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
     return launch_pdl(shift_setup_x_kernel, dim3((s.n_lines + 127) / 128), dim3(128), 0, P->st, s);
 }
 
-// ---- overlap-save launches (line length >= 1024)
-static size_t osx_smem_bytes(int lpi, int nb)
-{
-    return (size_t)lpi * nb * 1024 + (size_t)lpi * OS_LAMW * 8 + 130 * 8 + 112 * 8 + (size_t)lpi * nb * 4 + 16;
-}
-
+// ---- overlap-save launches (line length >= 1024; kernels in vog_os2.cuh)
 static cudaError_t run_osx(vog_plan_s* P, const float* src, float* dst)
 {
     OsArgs a;
     std::memset(&a, 0, sizeof(a));
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nx;
-    a.nb = (Nx + OS_V - 1) / OS_V;
-    a.lam = P->os_lam_x; a.tw = P->os_twx; a.cs = P->os_cs;
-    a.lpi = P->osx_lpi;
-    a.inv_nb = (65536u + (unsigned)a.nb - 1u) / (unsigned)a.nb;
-    a.n_groups = Nv / a.lpi;
-    const size_t smem = osx_smem_bytes(a.lpi, a.nb);
-    if (P->osx_occ == 0) {
-        P->osx_occ = osx_occupancy(P->osx_thr, smem);
-        if (P->osx_occ <= 0) return cudaErrorInvalidConfiguration;
-    }
-    const int cps = (P->osx_cps > 0 && P->osx_cps < P->osx_occ) ? P->osx_cps : P->osx_occ;
-    int grid = cps * P->n_sm;
-    if (grid > a.n_groups) grid = a.n_groups;
-    P->launches++;
-    return osx_launch(a, grid, P->osx_thr, smem, P->st);
-}
-
-// ---- pair kernels (vog_os2.cuh)
-static size_t osx2_smem_bytes(int lpi, int np)
-{
-    return (size_t)lpi * np * (16 * 17 * 8) + (size_t)lpi * OS_LAMW * 8 + 240 * 8;
-}
-
-static cudaError_t run_osx2(vog_plan_s* P, const float* src, float* dst)
-{
-    OsArgs a;
-    std::memset(&a, 0, sizeof(a));
-    const int Nx = P->p.Nx, Nv = P->p.Nv;
-    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nx;
-    const int geom = P->os2x_direct == 3 ? P->os_geom : 0;        // (the other variants use the spline geometry)
-    const int V = geom ? 232 : OS_V;
-    a.nb = (Nx + V - 1) / V;
-    a.np = (a.nb + 1) / 2;
+    const int geom = P->os_geom;
+    const OsxShape o = osx_shape(P, P->os2x_lpi);
+    a.np = o.np;
+    a.nb = 2 * o.np;
     a.inv_np = (65536u + (unsigned)a.np - 1u) / (unsigned)a.np;
     a.lam = P->os_lam_x; a.tw = P->os_twv;
     a.lpi = P->os2x_lpi;
     a.n_lines = Nv;
     a.n_groups = (Nv + a.lpi - 1) / a.lpi;
-    const size_t smem = osx2_smem_bytes(a.lpi, a.np);
-    if (P->os2x_direct == 3) {                     // warp-private kernel: any group size (rounds of thr items)
-        const int tmax = geom ? 288 : 320;         // (launch bounds of the two geometries: 72 / 64 registers)
-        int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
-        if (thr > tmax) thr = ((((16 * a.np * a.lpi + 1) / 2) + 31) / 32) * 32;     // two rounds
-        if (thr > tmax) thr = tmax;
-        const size_t sm5 = (size_t)a.lpi * a.np * (16 * 17 * 8) + (size_t)(a.lpi == 1 ? thr / 32 : thr / 16) * OS_LAMW * 8 + 16;
-        if (P->os3x_occ == 0) {
-            P->os3x_occ = osx5_occupancy(thr, sm5);
-            if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
-        }
-        int grid = P->os3x_occ * P->n_sm;
-        if (grid > a.n_groups) grid = a.n_groups;
-        P->launches++;
-        return osx5_launch(a, src == dst, geom, grid, thr, sm5, P->st);
+    // per-pair windows when the group fits one round of the CTA, whole lines otherwise (16384-cell lines) or on request
+    const bool windows = P->osx_variant == 0 && o.rounds == 1;
+    const size_t smem = windows ? o.smem7 : o.smem6;
+    if (P->os3x_occ == 0) {
+        P->os3x_occ = windows ? osx7_occupancy(geom, o.thr, smem) : osx6_occupancy(geom, o.thr, smem);
+        if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
     }
-    if (P->os2x_direct && 16 * a.np * a.lpi <= 320) {
-        const int thr = ((16 * a.np * a.lpi + 31) / 32) * 32;
-        const size_t smem = osx2_smem_bytes(a.lpi, a.np) - 240 * 8 + (P->os2x_direct == 2 ? (size_t)a.lpi * Nx * 4 : 0);
-        if (P->os3x_occ == 0) {
-            P->os3x_occ = osx3_occupancy(P->os2x_direct == 2, thr, smem);
-            if (P->os3x_occ <= 0) return cudaErrorInvalidConfiguration;
-        }
-        int grid = P->os3x_occ * P->n_sm;
-        if (grid > a.n_groups) grid = a.n_groups;
-        P->launches++;
-        return osx3_launch(a, P->os2x_direct == 2, grid, thr, smem, P->st);
-    }
-    if (P->os2x_occ == 0) {
-        P->os2x_occ = osx2_occupancy(P->os2x_thr, smem);
-        if (P->os2x_occ <= 0) return cudaErrorInvalidConfiguration;
-    }
-    int grid = P->os2x_occ * P->n_sm;
+    int grid = P->os3x_occ * P->n_sm;
     if (grid > a.n_groups) grid = a.n_groups;
     P->launches++;
-    return osx2_launch(a, grid, P->os2x_thr, smem, P->st);
-}
-
-static cudaError_t run_osv2(vog_plan_s* P, const float* src, float* dst, bool source)
-{
-    OsArgs a;
-    std::memset(&a, 0, sizeof(a));
-    const int Nx = P->p.Nx, Nv = P->p.Nv;
-    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
-    const int geom = P->os2v_direct == 2 ? P->os_geom : 0;
-    const int V = geom ? 232 : OS_V;
-    a.nb = (Nv + V - 1) / V;
-    a.np = (a.nb + 1) / 2;
-    a.lam = P->os_lam_v; a.tw = P->os_twv;
-    a.ng = source ? P->p.feq.n : 0;
-    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
-    a.dvf = (float)((P->p.vmax - P->p.vmin) / (double)Nv);
-    const int strips = Nx / 32;
-    // pairs per CTA: minimise waves x pairs per CTA (2 CTAs of 512 threads per SM); ties go to the longer loop
-    // (fewer reloads of the strip's symbol tables)
-    int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : 1;   // measured: one pair per CTA is fastest at 2048..8192 (profiles/)
-    if (gpc <= 0) {
-        long long best = -1;
-        const long long slots = (long long)P->n_sm * 2;
-        for (int gp = 1; gp <= a.np; ++gp) {
-            const long long ctas = (long long)strips * ((a.np + gp - 1) / gp);
-            const long long cost = ((ctas + slots - 1) / slots) * (gp * 8 + 1);      // +1: table load
-            if (best < 0 || cost <= best) { best = cost; gpc = gp; }
-        }
-    }
-    if (gpc > a.np) gpc = a.np;
-    a.gpc = gpc;
-    dim3 grid(strips, (a.np + gpc - 1) / gpc);
-    P->launches++;
-    if (P->os2v_direct == 2)
-        return osv4_launch(a, geom, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
-    if (P->os2v_direct) return osv3_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 4 * 32 * 16, P->st);
-    return osv2_launch(a, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
-}
-
-static size_t osv_smem_bytes(int np_log, int rb)
-{
-    (void)np_log;
-    return (size_t)rb * 128 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 130 * 8 + 112 * 8 + (size_t)rb * 32 * 4 + 16;
+    if (windows) return osx7_launch(a, geom, grid, o.thr, smem, P->st);
+    return osx6_launch(a, geom, grid, o.thr, smem, P->st);
 }
 
 static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool source)
@@ -947,40 +831,36 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
     std::memset(&a, 0, sizeof(a));
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
-    a.nb = (Nv + OS_V - 1) / OS_V;
-    a.lam = P->os_lam_v; a.tw = P->os_twx; a.cs = P->os_cs;
+    const int geom = P->os_geom;
+    const int V = geom ? OS_VL : OS_V;
+    a.nb = (Nv + V - 1) / V;
+    a.np = (a.nb + 1) / 2;
+    a.lam = P->os_lam_v; a.tw = P->os_twv; a.lam_ks = Nx + 16;
     a.ng = source ? P->p.feq.n : 0;
     a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
     a.dvf = (float)((P->p.vmax - P->p.vmin) / (double)Nv);
-    for (int g = 0; g < 4; ++g) a.cg[g] = g < P->p.feq.n ? (float)P->p.feq.c[g] : 0.0f;
-    const int strips = Nx / 32;
-    // Launch shape: rb row blocks per group (128 rb threads, 3 or 2 CTAs per SM), gpc groups per CTA.  The
-    // kernel is latency-bound, so the time is ~ waves x (row blocks per CTA); ties go to the larger CTA
-    // (fewer reloads of the strip's symbol tables).
-    int rb = P->osv_rb, gpc = P->osv_gpc;
-    if (rb <= 0 || gpc <= 0) {
-        long long best = -1;
-        int brb = 1, bgpc = 1;
-        for (int r = 1; r <= 2; ++r) {
-            if (P->osv_rb > 0 && r != P->osv_rb) continue;
-            const int ng_r = (a.nb + r - 1) / r;
-            const long long slots = (long long)P->n_sm * (r == 1 ? 3 : 2);
-            for (int gp = 1; gp <= ng_r; ++gp) {
-                if (P->osv_gpc > 0 && gp != P->osv_gpc) continue;
-                const long long ctas = (long long)strips * ((ng_r + gp - 1) / gp);
-                const long long cost = ((ctas + slots - 1) / slots) * gp * r * 16 + 1;   // +1: table reload
-                if (best < 0 || cost < best || (cost == best && gp * r > bgpc * brb)) { best = cost; brb = r; bgpc = gp; }
-            }
-        }
-        rb = brb; gpc = bgpc;
-    }
-    a.rb = rb;
-    const int ngroups = (a.nb + a.rb - 1) / a.rb;
-    if (gpc > ngroups) gpc = ngroups;
-    a.gpc = gpc;
-    dim3 grid(strips, (ngroups + gpc - 1) / gpc);
     P->launches++;
-    return osv_launch(a, grid, 128 * a.rb, osv_smem_bytes(0, a.rb), P->st);
+    if (P->osv_variant == 0) {
+        // three groups per CTA on one strip's symbol table; a work item is a segment of gpc consecutive pairs of a strip
+        // (each group: every third pair of it, the next one's rows in flight while the current one is transformed)
+        int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : (a.np >= 18 ? 9 : (a.np >= 6 ? 3 : a.np));
+        if (gpc > a.np) gpc = a.np;
+        a.gpc = gpc;
+        return osv7_launch(a, geom, P->n_sm, P->st);
+    }
+    if (P->osv_variant == 2) {
+        // 16-column strips, one group per CTA, symbol through L1
+        int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : (a.np >= 12 ? 3 : 1);
+        if (gpc > a.np) gpc = a.np;
+        a.gpc = gpc;
+        return osv6_launch(a, geom, dim3(Nx / 16, (a.np + gpc - 1) / gpc), P->st);
+    }
+    const int strips = Nx / 32;
+    int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : 1;
+    if (gpc > a.np) gpc = a.np;
+    a.gpc = gpc;
+    dim3 grid(strips, (a.np + gpc - 1) / gpc);
+    return osv4_launch(a, geom, grid, 512, (size_t)256 * 32 * 8 + (size_t)OS_LAMW * 32 * 8 + 240 * 8 + 4 * 32 * 16, P->st);
 }
 
 static cudaError_t run_advect_x(vog_plan_s* P, float* f)
@@ -1046,7 +926,7 @@ static cudaError_t copy_grid(vog_plan_s* P, float* dst, const float* src)
 // x-advection src -> dst (dst may equal src); the shift records/tables must be current
 static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
 {
-    if (P->os_x) return P->os_gen == 2 ? run_osx2(P, src, dst) : run_osx(P, src, dst);
+    if (P->os_x) return run_osx(P, src, dst);
     cudaError_t e = cudaSuccess;
     if (src != dst) e = copy_grid(P, dst, src);
     if (e == cudaSuccess) e = run_advect_line(P, dst, false, false);
@@ -1056,7 +936,7 @@ static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
 // v-advection src -> dst; the overlap-save kernel needs dst != src, the whole-line kernel works in place
 static cudaError_t advect_v(vog_plan_s* P, const float* src, float* dst, bool source)
 {
-    if (P->os_v) return src == dst ? cudaErrorInvalidValue : (P->os_gen == 2 ? run_osv2(P, src, dst, source) : run_osv(P, src, dst, source));
+    if (P->os_v) return src == dst ? cudaErrorInvalidValue : run_osv(P, src, dst, source);
     cudaError_t e = cudaSuccess;
     if (src != dst) e = copy_grid(P, dst, src);
     if (e == cudaSuccess) e = run_advect_line(P, dst, true, source);
@@ -1068,7 +948,7 @@ static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
 {
     if (!P->os_v) return run_advect_line(P, f, true, source);
     cudaError_t e = ensure_gbuf(P);
-    if (e == cudaSuccess) e = P->os_gen == 2 ? run_osv2(P, f, P->g_buf, source) : run_osv(P, f, P->g_buf, source);
+    if (e == cudaSuccess) e = run_osv(P, f, P->g_buf, source);
     if (e == cudaSuccess) e = copy_grid(P, f, P->g_buf);
     return e;
 }
@@ -1078,24 +958,21 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
     dim3 grid(Nx / 32, P->nby);
-    cudaError_t e = launch_pdl(density_partial_kernel, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part, dv,
-                               P->rho, P->dcnt);
+    cudaError_t e = launch_pdl(density_partial_kernel, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part);
     if (e != cudaSuccess) return e;
-    static bool attr = false;
-    if (!attr) {
-        e = cudaFuncSetAttribute(poisson_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 12 + 1024);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
     int T = Nx / 4;
     if (T > 1024) T = 1024;
     if (T < 32) T = 32;
     const int tw_in_smem = Nx <= 8192;
     const size_t psmem = (sizeof(float2) + sizeof(float)) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
+    e = set_max_smem((const void*)poisson_kernel, psmem);
+    if (e != cudaSuccess) return e;
     P->launches += 2;
     P->E_valid = true;
+    P->E_of = f;
     return launch_pdl(poisson_kernel, dim3(1), dim3(T), psmem, P->st, Nx, P->prx, P->ptw_len, tw_in_smem,
-                      (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->rho, P->E_self, E_out, energy_out,
+                      (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->part, P->nby, dv, P->rho, P->E_self, E_out,
+                      energy_out,
                       0.5 * P->p.L / (double)Nx);
 }
 
@@ -1112,6 +989,7 @@ extern "C" int vog_advect_x(vog_plan_t P, float* f_dev, double dt)
 {
     if (!P || !f_dev || !std::isfinite(dt)) return VOG_EINVAL;
     t_pdl = P->pdl != 0;
+    P->E_of = nullptr;                            // the state changes: the cached field no longer belongs to it
     cudaError_t e = ensure_recx(P, dt);
     if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
     return cuda_status(e);
@@ -1121,6 +999,7 @@ extern "C" int vog_advect_v(vog_plan_t P, float* f_dev, const float* E_dev, doub
 {
     if (!P || !f_dev || !E_dev || !std::isfinite(dt)) return VOG_EINVAL;
     t_pdl = P->pdl != 0;
+    P->E_of = nullptr;                            // the state changes: the cached field no longer belongs to it
     cudaError_t e = run_setup(P, true, 1, dt, E_dev, nullptr, nullptr);
     if (e == cudaSuccess) e = advect_v_inplace(P, f_dev, true);
     return cuda_status(e);
@@ -1130,6 +1009,7 @@ extern "C" int vog_shift_x(vog_plan_t P, float* f_dev, const double* beta)
 {
     if (!P || !f_dev || !beta) return VOG_EINVAL;
     t_pdl = P->pdl != 0;
+    P->E_of = nullptr;                            // the state changes: the cached field no longer belongs to it
     P->recx_valid = false;
     cudaError_t e = run_setup(P, false, 2, 0.0, nullptr, nullptr, beta);
     if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
@@ -1140,6 +1020,7 @@ extern "C" int vog_shift_v(vog_plan_t P, float* f_dev, const double* beta)
 {
     if (!P || !f_dev || !beta) return VOG_EINVAL;
     t_pdl = P->pdl != 0;
+    P->E_of = nullptr;                            // the state changes: the cached field no longer belongs to it
     cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
     if (e == cudaSuccess) e = advect_v_inplace(P, f_dev, false);
     return cuda_status(e);
@@ -1149,17 +1030,10 @@ extern "C" int vog_shift_v_to(vog_plan_t P, const float* src_dev, float* dst_dev
 {
     if (!P || !src_dev || !dst_dev || !beta || src_dev == dst_dev) return VOG_EINVAL;
     t_pdl = P->pdl != 0;
+    P->E_of = nullptr;                            // the state changes: the cached field no longer belongs to it
     cudaError_t e = run_setup(P, true, 2, 0.0, nullptr, nullptr, beta);
     if (e == cudaSuccess) e = advect_v(P, src_dev, dst_dev, false);
     return cuda_status(e);
-}
-
-extern "C" int vog_probe_x_memory_pattern(vog_plan_t P, const float* src_dev, float* dst_dev)
-{
-    if (!P || !src_dev || !dst_dev || src_dev == dst_dev || P->p.Nx < 1024) return VOG_EINVAL;
-    t_pdl = P->pdl != 0;
-    P->launches++;
-    return cuda_status(os_mempattern_launch(src_dev, dst_dev, P->p.Nx, P->p.Nv, 3 * P->n_sm, P->st));
 }
 
 extern "C" int vog_field(vog_plan_t P, const float* f_dev, float* E_dev)
@@ -1195,8 +1069,10 @@ extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ex
         if (e == cudaSuccess) e = run_setup(P, true, 1, dt, P->E_self, E_ext_dev, nullptr);
         if (e == cudaSuccess) e = advect_v(P, f_dev, g, true);
         if (e == cudaSuccess) e = advect_x(P, g, f_dev);
+        P->E_of = nullptr;                        // E_self is the field at the half step, not of the final state
     } else {
-        if (!P->E_valid) e = run_field(P, f_dev, nullptr);
+        // E_prev: the field the previous VXV step on this array ended with; anything else is solved from f
+        if (P->E_of != f_dev) e = run_field(P, f_dev, nullptr);
         if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
         if (e == cudaSuccess) e = advect_v(P, f_dev, g, true);
         if (e == cudaSuccess) e = ensure_recx(P, dt);
@@ -1204,6 +1080,7 @@ extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ex
         if (e == cudaSuccess) e = run_field(P, g, nullptr);
         if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
         if (e == cudaSuccess) e = advect_v(P, g, f_dev, true);
+        P->E_of = e == cudaSuccess ? f_dev : nullptr;      // rho, hence E, is invariant under the v-advection
     }
     return cuda_status(e);
 }
@@ -1239,6 +1116,7 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
             if (ok()) e = advect_x(P, g, f_dev);
             if (ok() && !merge && !last) e = advect_x(P, f_dev, f_dev);
         }
+        P->E_of = nullptr;
     } else {
         // v(dt/2) [x(dt) field v(dt)]^(n-1) x(dt) field v(dt/2); the two v(dt/2) around a field solve see the same
         // E (rho is invariant under the v-advection), so merged they are one v(dt)
@@ -1250,7 +1128,7 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
         };
         const int nvadv = merge ? nsteps + 1 : 2 * nsteps;
         bool flip_x = oth != cur && (nvadv & 1);           // odd number of buffer flips: one x-advection goes across
-        if (!P->E_valid) e = run_field(P, f_dev, nullptr, nullptr);
+        if (P->E_of != f_dev) e = run_field(P, f_dev, nullptr, nullptr);
         if (ok()) vadv(0.5 * dt);
         if (ok()) e = ensure_recx(P, dt);
         for (int s = 0; s < nsteps && ok(); ++s) {
@@ -1265,6 +1143,7 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
                 if (ok() && !last) vadv(0.5 * dt);
             }
         }
+        P->E_of = ok() ? f_dev : nullptr;
     }
     return cuda_status(e);
 }
@@ -1274,12 +1153,14 @@ static int run_host(vog_plan_t P, float* f_host, double dt, int nsteps, const fl
     if (!P || !f_host || nsteps < 0 || !std::isfinite(dt)) return VOG_EINVAL;
     const size_t nf = (size_t)P->p.Nx * P->p.Nv;
     cudaError_t e = cudaSuccess;
-    if (!P->f_buf) {
-        e = cudaMalloc((void**)&P->f_buf, sizeof(float) * nf);
-        if (e != cudaSuccess) { cudaGetLastError(); return VOG_ENOMEM; }
-        e = cudaMalloc((void**)&P->ext_buf, sizeof(float) * P->p.Nx);
-        if (e != cudaSuccess) { cudaGetLastError(); return VOG_ENOMEM; }
+    if (!P->f_buf) {                                       // both buffers or neither
+        float *fb = nullptr, *eb = nullptr;
+        e = cudaMalloc((void**)&fb, sizeof(float) * nf);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&eb, sizeof(float) * P->p.Nx);
+        if (e != cudaSuccess) { cudaFree(fb); cudaGetLastError(); return VOG_ENOMEM; }
+        P->f_buf = fb; P->ext_buf = eb;
     }
+    P->E_of = nullptr;                                    // new data in the staging buffer
     e = cudaMemcpyAsync(P->f_buf, f_host, sizeof(float) * nf, cudaMemcpyHostToDevice, P->st);
     if (e == cudaSuccess && E_ext_host)
         e = cudaMemcpyAsync(P->ext_buf, E_ext_host, sizeof(float) * P->p.Nx, cudaMemcpyHostToDevice, P->st);
@@ -1304,6 +1185,15 @@ extern "C" int vog_run_host_async(vog_plan_t P, float* f_host, double dt, int ns
                                   float* E_host)
 {
     return run_host(P, f_host, dt, nsteps, E_ext_host, E_host, false);
+}
+
+extern "C" int vog_reset(vog_plan_t P)
+{
+    if (!P) return VOG_EINVAL;
+    P->E_valid = false;
+    P->E_of = nullptr;
+    P->recx_valid = false;
+    return VOG_OK;
 }
 
 extern "C" long long vog_launch_count(vog_plan_t P) { return P ? P->launches : -1; }

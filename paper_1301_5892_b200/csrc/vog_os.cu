@@ -1,6 +1,9 @@
 // vog_os.cu -- overlap-save advection kernels: instantiation, launchers and the setup kernel that
 // tabulates the symbol lambda(theta_k) per line (S1 + the closed form of S4).  Product code.
-#include "vog_os.cuh"
+#include <map>
+#include <mutex>
+#include <utility>
+
 #include "vog_os2.cuh"
 
 namespace vog {
@@ -37,14 +40,10 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
         b = (int)bm;
         if (b >= s.N) b = 0;
     }
-    // x keeps 16-byte aligned loads: b = 4 b4 + br with br in {-2,..,1} (centred, so that the stencil shifted by
-    // br has the same room, >= 14 cells, on both sides of the kept samples); br goes into the table as e^{i theta br}
-    const bool whole_b = s.vdir || s.gen2;       // the integer shift goes entirely into the load address
-    const int b4 = ((b + 2) >> 2) & ((s.N >> 2) - 1);
-    const int br = whole_b ? 0 : b - 4 * ((b + 2) >> 2);
+    // the integer shift b goes entirely into the load address (entry 129): no rotation factor in the table
     // x: [line][k]; v: transposed [k][line] so that a strip of 32 columns reads 256-byte rows
     float2* out = s.vdir ? s.lam + l : s.lam + (size_t)l * OS_LAMW;
-    const size_t ks = s.vdir ? (size_t)s.n_lines : 1;
+    const size_t ks = s.vdir ? (size_t)s.ks : 1;
     // fp64 for everything that is per line (beta, b, b*, the Everett / B-spline coefficients); the 129 table
     // entries are then evaluated in fp32 from those coefficients (rounded once) and from (cos, sin, 2 - 2 cos)
     // rounded from the fp64 table: ~1e-7 relative, the same as the whole-line kernels' in-kernel symbol.
@@ -70,11 +69,10 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
         bs[3] = (float)(t * t * t / 6.0);
     }
     __syncthreads();
-    // a power of two: exact.  Even/odd packing (vog_os.cuh) carries a factor 2 from the untangle stage.
-    const float sc = s.gen2 ? 1.0f / (float)OS_LB : 1.0f / (2.0f * (float)OS_LB);
+    const float sc = 1.0f / (float)OS_LB;        // a power of two: exact
     // 128 threads: k = threadIdx.x, and threads 0 and 1 also write entries 128 and 129 (16 CTAs per SM)
     for (int k = threadIdx.x; k < OS_LAMW; k += 128) {
-        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(whole_b ? b : b4), sshift); continue; }
+        if (k == 129) { out[129 * ks] = make_float2(__int_as_float(b), sshift); continue; }
         if (k == 0) { out[0] = make_float2(sc, 0.0f); continue; }   // lambda_0 = sum of the weights = 1
         const double2 cs = s.cs64[k];                  // (cos, sin)(2 pi k / OS_LB), fp64 table
         const float c = (float)cs.x, sn = (float)cs.y;
@@ -95,12 +93,6 @@ __global__ void __launch_bounds__(128) os_setup_kernel(const OsSetupArgs s)
             }
             lr = fmaf(c, p1, p0);
             li = sn * p1;
-        }
-        if (br) {
-            const double2 r = s.cs64[(k * br) & (OS_LB - 1)];
-            const float rx = (float)r.x, ry = (float)r.y;
-            const float xr = fmaf(lr, rx, -li * ry), xi = fmaf(lr, ry, li * rx);
-            lr = xr; li = xi;
         }
         out[k * ks] = make_float2(lr * sc, li * sc);
     }
@@ -166,9 +158,9 @@ __global__ void __launch_bounds__(256) os_setup_v_kernel(const OsSetupArgs s)
         }
     }
     __syncthreads();
-    const float sc = s.gen2 ? 1.0f / (float)OS_LB : 1.0f / (2.0f * (float)OS_LB);
+    const float sc = 1.0f / (float)OS_LB;
     float2* const out = s.lam + l0 + lane;
-    const size_t ks = (size_t)s.n_lines;
+    const size_t ks = (size_t)s.ks;
     for (int k = wid + 8 * blockIdx.y; k < OS_LAMW; k += 8 * gridDim.y) {      // (the rows are split over gridDim.y CTAs)
         if (k == 129) { out[129 * ks] = make_float2(__int_as_float(bsh[lane]), ssh[lane]); continue; }
         if (k == 0) { out[0] = make_float2(sc, 0.0f); continue; }
@@ -196,43 +188,6 @@ __global__ void __launch_bounds__(256) os_setup_v_kernel(const OsSetupArgs s)
     }
 }
 
-// Measurement probe (vog_probe_x_memory_pattern): exactly the global loads and stores of osx5_kernel<., 232, 8> on
-// N-cell lines with zero shift -- 32 four-byte loads per thread in 64-byte runs per half-warp, the kept samples
-// stored with four-byte streaming stores -- and no transform.  Its time is the memory-system floor of that
-// access pattern (profiles/r1g2_pair_kernels.md, section 4).
-__global__ void __launch_bounds__(320, 3) os_mempattern_kernel(const float* __restrict__ src, float* __restrict__ dst,
-                                                               int N, int n_lines, int np)
-{
-    const int tid = threadIdx.x, t = tid & 15, mask = N - 1;
-    for (int line = blockIdx.x; line < n_lines; line += gridDim.x) {
-        const float* gl = src + (size_t)line * N;
-        float* go = dst + (size_t)line * N;
-        for (int pr = tid >> 4; pr < np; pr += blockDim.x >> 4) {
-            const int c0 = (pr * 464 - 8 + t) & mask;
-            float2 x[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k)
-                x[k] = make_float2(__ldg(gl + ((c0 + 16 * k) & mask)), __ldg(gl + ((c0 + 16 * k + 232) & mask)));
-            const int o = pr * 464 + t - 8;
-#pragma unroll
-            for (int m = 0; m < 15; ++m) {
-                const bool kept = m > 0 || t >= 8;
-                if (kept && o + 16 * m < N) __stcs(go + o + 16 * m, x[m].x);
-                if (kept && o + 16 * m + 232 < N) __stcs(go + o + 16 * m + 232, x[m].y);
-            }
-        }
-    }
-}
-
-cudaError_t os_mempattern_launch(const float* src, float* dst, int N, int n_lines, int grid, cudaStream_t st)
-{
-    const int np = ((N + 231) / 232 + 1) / 2;
-    int thr = ((16 * np + 31) / 32) * 32;
-    if (thr > 320) thr = 320;
-    os_mempattern_kernel<<<grid, thr, 0, st>>>(src, dst, N, n_lines, np);
-    return cudaGetLastError();
-}
-
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
 {
     if (s.vdir && s.n_lines % 32 == 0) {
@@ -243,164 +198,115 @@ cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st)
     return launch_pdl(os_setup_kernel, dim3(s.n_lines), dim3(128), 0, st, s);
 }
 
-static cudaError_t set_smem(const void* fn, size_t smem, size_t* cur)
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remember, per (device, kernel), the
+// largest size that was set, so that plans on several devices (or threads) each get it set once.
+cudaError_t set_max_smem(const void* fn, size_t smem)
 {
-    if (smem > 48 * 1024 && smem > *cur) {
-        cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (smem <= 48 * 1024) return cudaSuccess;
+    static std::mutex mu;
+    static std::map<std::pair<int, const void*>, size_t> cur;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lk(mu);
+    size_t& c = cur[std::make_pair(dev, fn)];
+    if (smem > c) {
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        *cur = smem;
+        c = smem;
     }
     return cudaSuccess;
 }
 
-cudaError_t osx_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+// warp-private-window x kernel (default when a line group fits one round); geom as above
+cudaError_t osx7_launch(const OsArgs& a, int geom, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    static size_t cur = 0;
-    cudaError_t e = set_smem((const void*)osx_kernel, smem, &cur);
-    if (e != cudaSuccess) return e;
-    osx_kernel<<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-cudaError_t osv_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
-{
-    static size_t cur = 0;
-    cudaError_t e = set_smem((const void*)osv_kernel, smem, &cur);
-    if (e != cudaSuccess) return e;
-    osv_kernel<<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-cudaError_t osx2_launch(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
-{
-    static size_t cur = 0;
-    static size_t cur2 = 0;
-    if (threads <= 160) {
-        cudaError_t e = set_smem((const void*)osx2_kernel<160, 5>, smem, &cur);
-        if (e != cudaSuccess) return e;
-        osx2_kernel<160, 5><<<grid, threads, smem, st>>>(a);
-    } else {
-        cudaError_t e = set_smem((const void*)osx2_kernel<320, 3>, smem, &cur2);
-        if (e != cudaSuccess) return e;
-        osx2_kernel<320, 3><<<grid, threads, smem, st>>>(a);
-    }
-    return cudaGetLastError();
-}
-
-cudaError_t osv2_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
-{
-    static size_t cur = 0;
-    cudaError_t e = set_smem((const void*)osv2_kernel, smem, &cur);
-    if (e != cudaSuccess) return e;
-    osv2_kernel<<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st)
-{
-    static size_t cur[2] = {0, 0};
     if (geom) {
-        cudaError_t e = set_smem((const void*)osv4_kernel<232, 8>, smem, &cur[1]);
+        cudaError_t e = set_max_smem((const void*)osx7_kernel<OS_VL, OS_HL>, smem);
         if (e != cudaSuccess) return e;
-        return launch_pdl(osv4_kernel<232, 8>, grid, dim3(threads), smem, st, a);
-    } else {
-        cudaError_t e = set_smem((const void*)osv4_kernel<OS_V, OS_H>, smem, &cur[0]);
-        if (e != cudaSuccess) return e;
-        return launch_pdl(osv4_kernel<OS_V, OS_H>, grid, dim3(threads), smem, st, a);
+        return launch_pdl(osx7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(threads), smem, st, a);
     }
-    return cudaGetLastError();
-}
-
-cudaError_t osv3_launch(const OsArgs& a, dim3 grid, int threads, size_t smem, cudaStream_t st)
-{
-    static size_t cur = 0;
-    cudaError_t e = set_smem((const void*)osv3_kernel, smem, &cur);
+    cudaError_t e = set_max_smem((const void*)osx7_kernel<OS_V, OS_H>, smem);
     if (e != cudaSuccess) return e;
-    osv3_kernel<<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
+    return launch_pdl(osx7_kernel<OS_V, OS_H>, dim3(grid), dim3(threads), smem, st, a);
 }
 
-// mode 1: raw-line landing of the next line group (needs lpi N floats more shared memory); mode 0: direct loads
-cudaError_t osx3_launch(const OsArgs& a, int mode, int grid, int threads, size_t smem, cudaStream_t st)
+int osx7_occupancy(int geom, int threads, size_t smem)
 {
-    static size_t cur[2] = {0, 0};
-    const void* fn = mode ? (const void*)osx3_kernel<true> : (const void*)osx3_kernel<false>;
-    cudaError_t e = set_smem(fn, smem, &cur[mode ? 1 : 0]);
-    if (e != cudaSuccess) return e;
-    if (mode) osx3_kernel<true><<<grid, threads, smem, st>>>(a);
-    else osx3_kernel<false><<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
-}
-
-int osx3_occupancy(int mode, int threads, size_t smem)
-{
-    static size_t cur[2] = {0, 0};
-    const void* fn = mode ? (const void*)osx3_kernel<true> : (const void*)osx3_kernel<false>;
-    if (set_smem(fn, smem, &cur[mode ? 1 : 0]) != cudaSuccess) { cudaGetLastError(); return 0; }
+    const void* fn = geom ? (const void*)osx7_kernel<OS_VL, OS_HL> : (const void*)osx7_kernel<OS_V, OS_H>;
+    if (set_max_smem(fn, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     int nb = 0;
-    const cudaError_t e = mode ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx3_kernel<true>, threads, smem)
-                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx3_kernel<false>, threads, smem);
+    const cudaError_t e = geom ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx7_kernel<OS_VL, OS_HL>, threads, smem)
+                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx7_kernel<OS_V, OS_H>, threads, smem);
     if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     return nb;
 }
 
-// warp-private x kernel; inplace selects the split-mbarrier variant (src may equal dst); geom 1 = the Lagrange
-// block geometry (232 kept, 8 + 16 discarded), 0 = the spline's (224, 16 + 16)
-template <bool INPLACE, int V, int HLO>
-static cudaError_t osx5_launch_t(const OsArgs& a, int grid, int threads, size_t smem, cudaStream_t st, size_t* cur)
+// bulk-landed whole-line x kernel (lines that need several rounds: 16384 cells); geom as above
+cudaError_t osx6_launch(const OsArgs& a, int geom, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    cudaError_t e = set_smem((const void*)osx5_kernel<INPLACE, V, HLO>, smem, cur);
+    if (geom) {
+        cudaError_t e = set_max_smem((const void*)osx6_kernel<OS_VL, OS_HL>, smem);
+        if (e != cudaSuccess) return e;
+        return launch_pdl(osx6_kernel<OS_VL, OS_HL>, dim3(grid), dim3(threads), smem, st, a);
+    }
+    cudaError_t e = set_max_smem((const void*)osx6_kernel<OS_V, OS_H>, smem);
     if (e != cudaSuccess) return e;
-    return launch_pdl(osx5_kernel<INPLACE, V, HLO>, dim3(grid), dim3(threads), smem, st, a);
+    return launch_pdl(osx6_kernel<OS_V, OS_H>, dim3(grid), dim3(threads), smem, st, a);
 }
 
-cudaError_t osx5_launch(const OsArgs& a, bool inplace, int geom, int grid, int threads, size_t smem, cudaStream_t st)
+int osx6_occupancy(int geom, int threads, size_t smem)
 {
-    static size_t cur[4] = {0, 0, 0, 0};
-    if (geom) return inplace ? osx5_launch_t<true, 232, 8>(a, grid, threads, smem, st, &cur[0])
-                             : osx5_launch_t<false, 232, 8>(a, grid, threads, smem, st, &cur[1]);
-    return inplace ? osx5_launch_t<true, OS_V, OS_H>(a, grid, threads, smem, st, &cur[2])
-                   : osx5_launch_t<false, OS_V, OS_H>(a, grid, threads, smem, st, &cur[3]);
-}
-
-int osx5_occupancy(int threads, size_t smem)
-{
-    static size_t cur = 0;
-    if (set_smem((const void*)osx5_kernel<true, OS_V, OS_H>, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
+    const void* fn = geom ? (const void*)osx6_kernel<OS_VL, OS_HL> : (const void*)osx6_kernel<OS_V, OS_H>;
+    if (set_max_smem(fn, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx5_kernel<true, OS_V, OS_H>, threads, smem) != cudaSuccess) {
-        cudaGetLastError();
-        return 0;
-    }
+    const cudaError_t e = geom ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx6_kernel<OS_VL, OS_HL>, threads, smem)
+                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx6_kernel<OS_V, OS_H>, threads, smem);
+    if (e != cudaSuccess) { cudaGetLastError(); return 0; }
     return nb;
 }
 
-int osx2_occupancy(int threads, size_t smem)
+// three-group v kernel (default): one persistent CTA of 768 threads per SM; a.gpc = pairs per work item
+cudaError_t osv7_launch(const OsArgs& a, int geom, int n_sm, cudaStream_t st)
 {
-    static size_t cur = 0, cur2 = 0;
-    const void* fn = threads <= 160 ? (const void*)osx2_kernel<160, 5> : (const void*)osx2_kernel<320, 3>;
-    if (set_smem(fn, smem, threads <= 160 ? &cur : &cur2) != cudaSuccess) { cudaGetLastError(); return 0; }
-    int nb = 0;
-    const cudaError_t eo = threads <= 160
-        ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx2_kernel<160, 5>, threads, smem)
-        : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx2_kernel<320, 3>, threads, smem);
-    if (eo != cudaSuccess) {
-        cudaGetLastError();
-        return 0;
+    const size_t smem = (size_t)OS_LAMW * os2::VW * 8 + 3 * ((size_t)os2::VRR * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8);
+    const int n_items = (a.Nx / os2::VW) * ((a.np + a.gpc - 1) / a.gpc);
+    const int grid = n_items < n_sm ? n_items : n_sm;
+    if (geom) {
+        cudaError_t e = set_max_smem((const void*)osv7_kernel<OS_VL, OS_HL>, smem);
+        if (e != cudaSuccess) return e;
+        return launch_pdl(osv7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(768), smem, st, a);
     }
-    return nb;
+    cudaError_t e = set_max_smem((const void*)osv7_kernel<OS_V, OS_H>, smem);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a);
 }
 
-int osx_occupancy(int threads, size_t smem)
+// 16-column-strip v kernel, symbol through L1; grid = (Nx / 16, ceil(np / gpc))
+cudaError_t osv6_launch(const OsArgs& a, int geom, dim3 grid, cudaStream_t st)
 {
-    static size_t cur = 0;
-    if (set_smem((const void*)osx_kernel, smem, &cur) != cudaSuccess) { cudaGetLastError(); return 0; }
-    int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, osx_kernel, threads, smem) != cudaSuccess) {
-        cudaGetLastError();
-        return 0;
+    const size_t smem = (size_t)os2::VRR * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8;
+    if (geom) {
+        cudaError_t e = set_max_smem((const void*)osv6_kernel<OS_VL, OS_HL>, smem);
+        if (e != cudaSuccess) return e;
+        return launch_pdl(osv6_kernel<OS_VL, OS_HL>, grid, dim3(256), smem, st, a);
     }
-    return nb;
+    cudaError_t e = set_max_smem((const void*)osv6_kernel<OS_V, OS_H>, smem);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(osv6_kernel<OS_V, OS_H>, grid, dim3(256), smem, st, a);
+}
+
+cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st)
+{
+    if (geom) {
+        cudaError_t e = set_max_smem((const void*)osv4_kernel<OS_VL, OS_HL>, smem);
+        if (e != cudaSuccess) return e;
+        return launch_pdl(osv4_kernel<OS_VL, OS_HL>, grid, dim3(threads), smem, st, a);
+    }
+    cudaError_t e = set_max_smem((const void*)osv4_kernel<OS_V, OS_H>, smem);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(osv4_kernel<OS_V, OS_H>, grid, dim3(threads), smem, st, a);
 }
 
 }  // namespace vog

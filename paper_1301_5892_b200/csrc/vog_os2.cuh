@@ -23,7 +23,6 @@
 namespace vog {
 
 namespace os2 {
-constexpr int PW = 2 * OS_V;           // cells advanced by one pair of blocks (448)
 
 __device__ __forceinline__ void cp_async4(void* smem, const void* gmem)
 {
@@ -53,7 +52,6 @@ __device__ __forceinline__ void mid16(float2* x, const float2* __restrict__ lam,
     idft_dit<16, 1>(x);
 }
 }  // namespace os2
-
 // ---------------------------------------------------------------------------------------------
 // x-direction.  Scratch: 16 rows of 17 float2 per pair (2176 B): position p = 16 g + j sits at 17 g + j.
 // All shared accesses are 8 bytes wide; passes A (16 lanes = 16 adjacent j of one row) and the middle stage
@@ -65,152 +63,6 @@ namespace os2 {
 constexpr int XROW = 17;               // float2 per scratch row
 constexpr int XPAIR = 16 * XROW;       // float2 per pair
 }
-
-__device__ __forceinline__ void osx2_land(float2* __restrict__ s, const float* __restrict__ gl, const int c0,
-                                          const int mask)
-{
-    float* const sf = reinterpret_cast<float*>(s);
-    if (c0 + OS_V + 241 <= mask + 1) {                 // the two windows do not wrap
-        const float* p = gl + c0;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            os2::cp_async4(sf + 2 * os2::XROW * k, p + 16 * k);
-            os2::cp_async4(sf + 2 * os2::XROW * k + 1, p + 16 * k + OS_V);
-        }
-    } else {
-#pragma unroll 2
-        for (int k = 0; k < 16; ++k) {
-            os2::cp_async4(sf + 2 * os2::XROW * k, gl + ((c0 + 16 * k) & mask));
-            os2::cp_async4(sf + 2 * os2::XROW * k + 1, gl + ((c0 + 16 * k + OS_V) & mask));
-        }
-    }
-}
-
-// s = pair base + t; tw = table + t
-__device__ __forceinline__ void osx2_fwd(float2* __restrict__ s, const float2* __restrict__ tw)
-{
-    float2 x[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) x[k] = s[os2::XROW * k];
-    dft_dif<16, 1>(x);
-    s[0] = x[0];
-#pragma unroll
-    for (int q = 1; q < 16; ++q) s[os2::XROW * q] = cmul(x[brev(q, 16)], tw[(q - 1) * 16]);
-}
-
-// s = pair base + 17 g
-__device__ __forceinline__ void osx2_mid(float2* __restrict__ s, const int g, const float2* __restrict__ lam)
-{
-    float2 x[16];
-#pragma unroll
-    for (int j = 0; j < 16; ++j) x[j] = s[j];
-    os2::mid16<1>(x, lam, g);
-#pragma unroll
-    for (int j = 0; j < 16; ++j) s[j] = x[j];
-}
-
-// inverse pass A of item (pair, j): kept samples m = 1..14 of block A (real parts) and block B (imaginary
-// parts) go to cells o0 + 16 (m - 1) and o0 + OS_V + 16 (m - 1) of the line; cells >= N do not exist.
-// s = pair base + j; tw = table + j
-__device__ __forceinline__ void osx2_inv(float* __restrict__ gl, const int o0, const bool full, const int N,
-                                         const float2* __restrict__ s, const float2* __restrict__ tw)
-{
-    float2 x[16];
-    x[0] = s[0];
-#pragma unroll
-    for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(s[os2::XROW * q], tw[(q - 1) * 16]);
-    idft_dit<16, 1>(x);
-    float* const o = gl + o0;
-    if (full) {
-#pragma unroll
-        for (int m = 1; m < 15; ++m) {
-            __stcs(o + 16 * (m - 1), x[m].x);
-            __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
-        }
-    } else {
-#pragma unroll
-        for (int m = 1; m < 15; ++m) {
-            if (o0 + 16 * (m - 1) < N) __stcs(o + 16 * (m - 1), x[m].x);
-            if (o0 + 16 * (m - 1) + OS_V < N) __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
-        }
-    }
-}
-
-// One iteration = lpi whole lines = lpi * np pairs = 16 lpi np items per phase; blockDim.x is a multiple of 16,
-// so the position index t = tid & 15 of a thread is the same for all its items.
-template <int TMAX, int MINB>
-__global__ void __launch_bounds__(TMAX, MINB) osx2_kernel(const OsArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
-    float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
-    float2* const lamS = scr + ptot * os2::XPAIR;                       // lpi rows of the symbol table
-    float2* const twS = lamS + lpi * OS_LAMW;                           // 15 * 16
-    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
-    const int N = a.N, mask = N - 1;
-    const unsigned inv_np = a.inv_np;       // ceil(2^16 / np): pr / np == (pr * inv_np) >> 16 for pr < 2^12
-
-    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
-
-    // landing of item w of the line group that starts at line0, and of the group's table rows
-    auto land = [&](const int w, const int line0) {
-        const int pr = w >> 4;
-        const int l = (int)(((unsigned)pr * inv_np) >> 16), pp = pr - l * np;
-        const int line = line0 + l;
-        if (line >= a.n_lines) return;
-        const int b = __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x));
-        osx2_land(scr + pr * os2::XPAIR + t, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
-    };
-    auto land_tab = [&](const int line0) {
-        const int nl = min(lpi, a.n_lines - line0);
-        const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
-        float4* dst4 = reinterpret_cast<float4*>(lamS);
-        for (int i = tid; i < nl * (OS_LAMW / 2); i += T) os2::cp_async16(dst4 + i, src4 + i);
-    };
-    if ((int)blockIdx.x < a.n_groups) {
-        for (int w = tid; w < nitem; w += T) land(w, blockIdx.x * lpi);
-        land_tab(blockIdx.x * lpi);
-    }
-    __syncthreads();                               // twS visible
-    for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
-        const int line0 = g * lpi;
-        os2::cp_async_wait_all();                  // this thread's samples (and table chunks) have landed
-        // ---- pass A: every thread on the slots it landed itself
-#pragma unroll 1
-        for (int w = tid; w < nitem; w += T) {
-            int tt = t;
-            asm volatile("" : "+r"(tt));           // keep the 15 twiddle loads inside the loop (30 registers)
-            osx2_fwd(scr + (w >> 4) * os2::XPAIR + t, twS + tt);
-        }
-        __syncthreads();
-        // ---- middle stage
-#pragma unroll 1
-        for (int w = tid; w < nitem; w += T) {
-            const int pr = w >> 4;
-            const int l = (int)(((unsigned)pr * inv_np) >> 16);
-            osx2_mid(scr + pr * os2::XPAIR + os2::XROW * t, t, lamS + l * OS_LAMW);
-        }
-        __syncthreads();
-        // ---- inverse pass A: scratch -> registers -> global; the same item of the NEXT line group lands in
-        // the slots just read.  In place this is safe: every load of THIS group completed before the
-        // barrier after pass A, and the next group is other lines (owned by this CTA).
-        const int gn = g + gridDim.x;
-        if (gn < a.n_groups) land_tab(gn * lpi);   // lamS was last read before the barrier above
-#pragma unroll 1
-        for (int w = tid; w < nitem; w += T) {
-            const int pr = w >> 4;
-            const int l = (int)(((unsigned)pr * inv_np) >> 16), pp = pr - l * np;
-            int tt = t;
-            asm volatile("" : "+r"(tt));
-            const float2* twp = twS + tt;
-            if (line0 + l < a.n_lines)
-                osx2_inv(a.dst + (size_t)(line0 + l) * N, pp * os2::PW + t, (pp + 1) * os2::PW <= N, N,
-                         scr + pr * os2::XPAIR + t, twp);
-            if (gn < a.n_groups) land(w, gn * lpi);
-        }
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // x-direction, register-landing variant (lines with at most 20 pairs, i.e. N <= 8192): one item per thread and
 // phase (16 lpi np <= blockDim.x).  The 32 samples of a thread's pass-A item are loaded straight into the
@@ -298,148 +150,8 @@ __device__ __forceinline__ void os2_tw_each(const Tw4& w, F&& f)
     f(QC<12>(), cmul(w.b4, w.b8));
 }
 
-template <int V = OS_V>
-__device__ __forceinline__ void osx3_load(float2* x, const float* __restrict__ gl, const int c0, const int mask)
-{
-    if (c0 + V + 241 <= mask + 1) {                    // the two windows do not wrap
-        const float* p = gl + c0;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) x[k] = make_float2(__ldg(p + 16 * k), __ldg(p + 16 * k + V));
-    } else {
-#pragma unroll
-        for (int k = 0; k < 16; ++k)
-            x[k] = make_float2(__ldg(gl + ((c0 + 16 * k) & mask)), __ldg(gl + ((c0 + 16 * k + V) & mask)));
-    }
-}
-
-// RAW = false: the loads of a group are issued and consumed at the top of its own iteration (nothing is in
-// flight while a CTA computes; the other CTAs of the SM cover for it).
-// RAW = true: the lines of the NEXT group are copied as they are (cp.async, 16 bytes, no shift) into a raw line
-// buffer right after pass A of the current group has emptied it, so they have the middle stage and the inverse
-// pass to arrive (~2/3 of the time, 32 KB per CTA in flight); pass A then reads its samples from the raw
-// buffer with the shift applied by addressing (4-byte shared loads, any alignment).  One more barrier per
-// iteration (the raw lines are landed by all threads).
-template <bool RAW>
-__global__ void __launch_bounds__(320, 3) osx3_kernel(const OsArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
-    float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
-    float2* const lamS = scr + ptot * os2::XPAIR;                       // lpi rows of the symbol table
-    float* const raw = reinterpret_cast<float*>(lamS + lpi * OS_LAMW);  // RAW: lpi lines of N floats
-    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
-    const int N = a.N, mask = N - 1;
-    const bool active = tid < nitem;
-    const int pr = tid >> 4;
-    const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
-    Tw4 w;
-    w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
-    w.b2 = __ldg(a.tw + 16 + t);
-    w.b4 = __ldg(a.tw + 3 * 16 + t);
-    w.b8 = __ldg(a.tw + 7 * 16 + t);
-    float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
-    float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
-    const float2* const lamL = lamS + l * OS_LAMW;
-    const int o0 = pp * os2::PW + t;
-    const bool full = (pp + 1) * os2::PW <= N;
-    const int G = gridDim.x;
-
-    // the group's table rows and (RAW) its lines; a ragged last group has fewer lines
-    auto land = [&](const int g) {
-        const int line0 = g * lpi, nl = min(lpi, a.n_lines - line0);
-        const float4* src4 = reinterpret_cast<const float4*>(a.lam + (size_t)line0 * OS_LAMW);
-        float4* dst4 = reinterpret_cast<float4*>(lamS);
-        for (int i = tid; i < nl * (OS_LAMW / 2); i += T) os2::cp_async16(dst4 + i, src4 + i);
-        if constexpr (RAW) {
-            const float4* s4 = reinterpret_cast<const float4*>(a.src + (size_t)line0 * N);
-            float4* d4 = reinterpret_cast<float4*>(raw);
-            const int n4 = nl * (N >> 2);
-#pragma unroll 4
-            for (int i = tid; i < n4; i += T) os2::cp_async16(d4 + i, s4 + i);
-        }
-    };
-    if ((int)blockIdx.x < a.n_groups) land(blockIdx.x);
-    for (int g = blockIdx.x; g < a.n_groups; g += G) {
-        const int gn = g + G;
-        const int line = min(g * lpi + l, a.n_lines - 1);      // (a ragged last group recomputes the last line)
-        if constexpr (RAW) {
-            os2::cp_async_wait_all();              // this thread's chunks of the raw lines and table rows
-            __syncthreads();
-        }
-        // ---- pass A
-        if (active) {
-            float2 x[16];
-            if constexpr (RAW) {
-                const int b = __float_as_int(lamL[129].x);
-                const float* const rl = raw + l * N;
-                const int c0 = (pp * os2::PW - OS_H + b + t) & mask;
-                if (c0 + OS_V + 241 <= N) {
-#pragma unroll
-                    for (int k = 0; k < 16; ++k) x[k] = make_float2(rl[c0 + 16 * k], rl[c0 + 16 * k + OS_V]);
-                } else {
-#pragma unroll
-                    for (int k = 0; k < 16; ++k)
-                        x[k] = make_float2(rl[(c0 + 16 * k) & mask], rl[(c0 + 16 * k + OS_V) & mask]);
-                }
-            } else {
-                const int b = __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x));
-                osx3_load(x, a.src + (size_t)line * N, (pp * os2::PW - OS_H + b + t) & mask, mask);
-            }
-            dft_dif<16, 1>(x);
-            sA[0] = x[0];
-            os2_tw_each(w, [&](auto qc, const float2 y) {
-                constexpr int q = decltype(qc)::value;
-                sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
-            });
-        }
-        if constexpr (!RAW) os2::cp_async_wait_all();          // table rows
-        __syncthreads();
-        // ---- middle stage
-        if (active) osx2_mid(sM, t, lamL);
-        __syncthreads();
-        // the raw buffer was emptied before the first barrier, the table rows were last read before the second:
-        // the next group starts landing now and has the whole inverse pass (and the other CTAs' phases) to arrive
-        if (gn < a.n_groups) land(gn);
-        // ---- inverse pass A: scratch -> registers -> global.  In place this is safe: every load of THIS group
-        // completed before the first barrier, and the other groups are other lines (owned by this CTA).
-        if (active) {
-            float2 x[16];
-            x[0] = sA[0];
-            os2_tw_each(w, [&](auto qc, const float2 y) {
-                constexpr int q = decltype(qc)::value;
-                x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
-            });
-            idft_dit<16, 1>(x);
-            if (g * lpi + l < a.n_lines) {
-                float* const o = a.dst + (size_t)(g * lpi + l) * N + o0;
-                if (full) {
-#pragma unroll
-                    for (int m = 1; m < 15; ++m) {
-                        __stcs(o + 16 * (m - 1), x[m].x);
-                        __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
-                    }
-                } else {
-#pragma unroll
-                    for (int m = 1; m < 15; ++m) {
-                        if (o0 + 16 * (m - 1) < N) __stcs(o + 16 * (m - 1), x[m].x);
-                        if (o0 + 16 * (m - 1) + OS_V < N) __stcs(o + 16 * (m - 1) + OS_V, x[m].y);
-                    }
-                }
-            }
-        }
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
-// x-direction, warp-private variant.  The 16 items of a pair are 16 consecutive threads in EVERY phase (pass A
-// item t, middle item g, inverse item j), so a warp owns its two pairs from the first load to the last store
-// and the phases are separated by __syncwarp() only: the warps of a CTA drift apart freely and their load,
-// compute and store phases overlap.  The symbol is read straight from the per-line table in global memory
-// (a 1 KB row shared by all warps of the line: L1 hits), so nothing is staged CTA-wide.
-// The only CTA-wide dependency left is the in-place hazard (every load of a line must complete before its
-// first store): a split mbarrier -- each warp ARRIVES once its samples are in registers and WAITS just before
-// its first store, with the middle stage and the inverse transform in between.  With INPLACE = false
-// (src != dst) there is no synchronisation between warps at all.
+// mbarrier helpers (shared::cta)
 namespace os2 {
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, const unsigned count)
 {
@@ -462,60 +174,126 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, const unsigne
         "@!p bra WAIT_%=;\n}\n" ::"r"(s), "r"(parity), "r"(20000u) : "memory");
 }
 }  // namespace os2
+// ---------------------------------------------------------------------------------------------
+// x-direction, bulk-landed variant (default).  A persistent CTA owns whole lines.  ONE elected thread copies the next
+// line group -- each line, the first XPAD cells of the line again behind its tail, and the line's symbol-table row --
+// into shared memory with bulk asynchronous copies (cp.async.bulk, the TMA engine; completion is counted in bytes on an
+// mbarrier), so no warp ever waits on its own global loads and no load occupies registers across its latency:
+//   * pass A reads its samples n = t + 16 k from the line in shared memory, the integer shift b of P:107 applied by
+//     addressing (4-byte loads, 16 consecutive words per half-warp: conflict free); the repeated head makes the
+//     window of every item contiguous, so there is no wrap-around branch and no index masking per sample;
+//   * the line buffer is free again once every warp has its samples in registers: each warp bumps a shared counter
+//     after its (last) pass A, and the warp that completes the count issues the copies of the CTA's next line group,
+//     which then land during the middle stage and the inverse pass (and under the other CTAs of the SM);
+//   * in place needs no barrier at all: a line is completely on chip before the first store to it is issued.
+// The phases of a pair are warp-private (the 16 items of a pair are 16 consecutive lanes in every phase: __syncwarp only).
+// The symbol rows are double-buffered (2 x 1040 B per line): slow warps may still be in the middle stage of group g
+// when the rows of group g+1 arrive.
+namespace os2 {
+constexpr int XPAD = 480;              // >= 240 + V + 1: the last sample of an item's window is c0 + 240 + V
 
-template <bool INPLACE, int V, int HLO>
-__global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsArgs a)
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, const unsigned bytes)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lpi = a.lpi, np = a.np, ptot = lpi * np, nitem = ptot * 16;
-    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15, hw = tid >> 4;
-    float2* const scr = reinterpret_cast<float2*>(smem_raw);            // ptot * XPAIR
-    // one private copy of the line's table row per half-warp, or per warp when a group is one line (then both
-    // pairs of a warp read the same copy: broadcast, and half the shared memory)
-    const bool one_line = lpi == 1;
-    float2* const lamP = scr + ptot * os2::XPAIR;
-    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(lamP + (one_line ? (T >> 5) : (T >> 4)) * OS_LAMW);
-    const int N = a.N, mask = N - 1;
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(s), "r"(bytes) : "memory");
+}
+// global -> shared bulk copy (16-byte aligned addresses, size a multiple of 16), completing on bar
+__device__ __forceinline__ void bulk_g2s(void* smem, const void* gmem, const unsigned bytes, unsigned long long* bar)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem), b = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(d),
+                 "l"(gmem), "r"(bytes), "r"(b)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+// request a global range into L2 (no destination on chip, nothing to wait for)
+__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem, const unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(gmem), "r"(bytes) : "memory");
+}
+}  // namespace os2
+
+// kept samples of a FULL pair (both blocks inside the line): no bounds predicates, only the per-thread one of the
+// partially kept sample row (m = 0 with the Lagrange geometry)
+template <int V, int HLO, int M = 0>
+__device__ __forceinline__ void os2_store_x_full(float* __restrict__ o, const int t, const float2* x)
+{
+    if constexpr (M < 16) {
+        using K = KeptM<V, HLO, M>;
+        if constexpr (K::all) {
+            __stcs(o + 16 * M, x[M].x);
+            __stcs(o + 16 * M + V, x[M].y);
+        } else if constexpr (!K::none) {
+            if (K::kept(t)) {
+                __stcs(o + 16 * M, x[M].x);
+                __stcs(o + 16 * M + V, x[M].y);
+            }
+        }
+        os2_store_x_full<V, HLO, M + 1>(o, t, x);
+    }
+}
+
+template <int V, int HLO>
+__global__ void __launch_bounds__(288, 3) osx6_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lpi = a.lpi, np = a.np, nitem = lpi * np * 16;
+    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
+    const int N = a.N, mask = N - 1, LS = N + os2::XPAD;
+    float* const lines = reinterpret_cast<float*>(smem_raw);                       // lpi lines of LS floats
+    float2* const lamS = reinterpret_cast<float2*>(lines + lpi * LS);              // [2][lpi][OS_LAMW]
+    float2* const scr = lamS + 2 * lpi * OS_LAMW;                                  // (T / 16) pairs
+    unsigned long long* const bar = reinterpret_cast<unsigned long long*>(scr + (T >> 4) * os2::XPAIR);   // [0] full, [1] empty
     Tw4 w;
     w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
     w.b2 = __ldg(a.tw + 16 + t);
     w.b4 = __ldg(a.tw + 3 * 16 + t);
     w.b8 = __ldg(a.tw + 7 * 16 + t);
-    float2* const lamL = lamP + (one_line ? (hw >> 1) : hw) * OS_LAMW;
-    const int cp0 = one_line ? (tid & 31) : t, cps = one_line ? 32 : 16;      // this thread's chunks of the copy
-    if constexpr (INPLACE) {
-        if (tid == 0) os2::mbar_init(bar, T >> 5);
-        __syncthreads();
+    if (tid == 0) {
+        os2::mbar_init(bar, 1);                   // full: the elected thread's expect_tx arrival + the bytes of the copies
+        os2::mbar_init(bar + 1, T >> 5);          // empty: one arrival per warp, after its last pass A of the group
+        os2::mbar_init_fence();
     }
+    __syncthreads();
     pdl_wait();                                   // (the twiddles above are plan constants; tables and grid are not)
     pdl_launch_dependents();
+    // copies of line group g into the line buffers and into symbol-row buffer (par); called by ONE thread.  The lines of
+    // the group after it are requested into L2 at the same time: their HBM latency (and the queueing behind everyone
+    // else's requests) then runs two groups ahead and costs no shared memory; the copy proper is an L2 hit.
+    auto issue = [&](const int g, const unsigned par) {
+        const int line0 = g * lpi, nl = min(lpi, a.n_lines - line0);
+        os2::mbar_expect_tx(bar, (unsigned)nl * (unsigned)(4 * LS + 8 * OS_LAMW));
+        for (int l = 0; l < nl; ++l) {
+            const float* gl = a.src + (size_t)(line0 + l) * N;
+            os2::bulk_g2s(lines + l * LS, gl, 4u * (unsigned)N, bar);
+            os2::bulk_g2s(lines + l * LS + N, gl, 4u * os2::XPAD, bar);
+            os2::bulk_g2s(lamS + (par * lpi + l) * OS_LAMW, a.lam + (size_t)(line0 + l) * OS_LAMW, 8u * OS_LAMW, bar);
+        }
+        const int line2 = (g + (int)gridDim.x) * lpi, nl2 = min(lpi, a.n_lines - line2);
+        for (int l = 0; l < nl2; ++l) os2::bulk_prefetch_l2(a.src + (size_t)(line2 + l) * N, 4u * (unsigned)N);
+    };
+    if (tid == 0 && (int)blockIdx.x < a.n_groups) issue(blockIdx.x, 0u);
+    float2* const sA = scr + (tid >> 4) * os2::XPAIR + t;                          // passes A: column t of the pair
+    float2* const sM = scr + (tid >> 4) * os2::XPAIR + os2::XROW * t;              // middle stage: row g = t
     unsigned parity = 0;
-    // A line group has nitem items; thread tid takes items tid, tid + T, .. ("rounds"; one round when the group
-    // fits the CTA, two for 16384-cell lines).  Per round: load, pass A, middle stage -- the pair's spectrum
-    // stays in its scratch; then, once every load of the group has completed, per round: inverse pass and stores.
     for (int g = blockIdx.x; g < a.n_groups; g += gridDim.x) {
+        os2::mbar_wait(bar, parity);              // the lines and symbol rows of this group have landed
+        const float2* const lamG = lamS + parity * lpi * OS_LAMW;
+        const int gn = g + gridDim.x;
 #pragma unroll 1
-        for (int it = tid; it - (tid & 31) < nitem; it += T) {          // (trip count uniform over the warp)
-            const int pr = it >> 4;
+        for (int it0 = 0; it0 < nitem; it0 += T) {                      // rounds (one when the group fits the CTA)
+            const int it = it0 + tid;
             const bool active = it < nitem;
+            const int pr = it >> 4;
             const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
-            const int line = min(g * lpi + l, a.n_lines - 1);  // (a ragged last group recomputes the last line)
-            const float2* __restrict__ lamG = a.lam + (size_t)line * OS_LAMW;
-            float2* const sA = scr + pr * os2::XPAIR + t;                       // passes A: column t of the pair
-            float2* const sM = scr + pr * os2::XPAIR + os2::XROW * t;           // middle stage: row g = t
-            // ---- pass A straight from global memory
-            // the (half-)warp's copy of the line's symbol table lands behind pass A (its previous contents were
-            // last read by these threads before the __syncwarp() that closed their last middle stage); with one
-            // line per group all 32 lanes copy, the inactive ones of the last warp included
-            if (active || one_line) {
-                const float2* __restrict__ lamC = one_line ? a.lam + (size_t)min(g, a.n_lines - 1) * OS_LAMW : lamG;
-                for (int i = cp0; i < OS_LAMW / 2; i += cps)
-                    os2::cp_async16(reinterpret_cast<float4*>(lamL) + i, reinterpret_cast<const float4*>(lamC) + i);
-            }
+            const float2* const lamL = lamG + l * OS_LAMW;
+            // ---- pass A from the line in shared memory
             if (active) {
+                const int b = __float_as_int(lamL[129].x);
+                const float* const p = lines + l * LS + ((pp * (2 * V) - HLO + b + t) & mask);
                 float2 x[16];
-                const int b = __float_as_int(__ldg(&lamG[129].x));
-                osx3_load<V>(x, a.src + (size_t)line * N, (pp * (2 * V) - HLO + b + t) & mask, mask);
+#pragma unroll
+                for (int k = 0; k < 16; ++k) x[k] = make_float2(p[16 * k], p[16 * k + V]);
                 dft_dif<16, 1>(x);
                 sA[0] = x[0];
                 os2_tw_each(w, [&](auto qc, const float2 y) {
@@ -523,13 +301,10 @@ __global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsA
                     sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
                 });
             }
-            os2::cp_async_wait_all();
             __syncwarp();
-            // (the shared stores of pass A needed every loaded value, and a warp issues in order: once its last
-            // round is here, all loads of this warp have completed)
-            if constexpr (INPLACE) {
-                if (it - (tid & 31) + T >= nitem && (tid & 31) == 0) os2::mbar_arrive(bar);
-            }
+            // (the shared stores above needed every sample: this warp is done with the line buffers)
+            const bool last_round = it0 + T >= nitem;
+            if (last_round && (tid & 31) == 0) os2::mbar_arrive(bar + 1);
             // ---- middle stage
             if (active) {
                 float2 x[16];
@@ -539,18 +314,186 @@ __global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsA
 #pragma unroll
                 for (int j = 0; j < 16; ++j) sM[j] = x[j];
             }
+            // once every warp is done with the line buffers, thread 0 requests the CTA's next line group; it lands
+            // behind the inverse pass (by now the other warps have normally arrived: the wait is a formality)
+            if (last_round && tid == 0 && gn < a.n_groups) {
+                os2::mbar_wait(bar + 1, parity);
+                issue(gn, parity ^ 1u);
+            }
             __syncwarp();
+            // ---- inverse pass A: scratch -> registers -> global
+            if (active) {
+                float2 x[16];
+                x[0] = sA[0];
+                os2_tw_each(w, [&](auto qc, const float2 y) {
+                    constexpr int q = decltype(qc)::value;
+                    x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
+                });
+                idft_dit<16, 1>(x);
+                const int line = g * lpi + l;
+                if (line < a.n_lines) {
+                    const int c = pp * (2 * V) + t - HLO;          // cell of sample n = t of block A
+                    float* const o = a.dst + (size_t)line * N + c;
+                    if ((pp + 1) * (2 * V) <= N) os2_store_x_full<V, HLO>(o, t, x);
+                    else os2_store_x<V, HLO>(o, c, N, t, false, x);
+                }
+            }
+            __syncwarp();                          // the scratch of this warp is rewritten by its next pass A
         }
-        if constexpr (INPLACE) {                   // every load of the group has completed, in every warp
-            os2::mbar_wait(bar, parity);
-            parity ^= 1u;
+        parity ^= 1u;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// x-direction, warp-private windows (default when a line group fits one round of the CTA, i.e. lines up to 8192 cells).
+// osx6_kernel lands whole lines for the whole CTA, so every warp waits for the slowest one twice per line (the line
+// buffer must be empty before it is refilled, and full before anybody starts): measured, a quarter of all warp time
+// sat in that wait.  Here each half-warp copies exactly the WINDOW of its own pair -- 256 + V consecutive cells of the
+// rolled line, 16-byte aligned, at most two bulk copies when it wraps around the end of the line -- into its own 2 KB
+// slot, counted on its WARP's mbarrier:
+//   * a warp refills its slots as soon as ITS pass A is done and waits only for ITS windows: loads, transforms and
+//     stores of different warps overlap freely, as in the register-landing kernel, but nobody waits on a global load;
+//   * in place: a store to line g may only be issued once every window of line g is on chip.  Each warp arrives on a
+//     CTA-wide "landed" mbarrier when it has seen its windows and checks it before its first store, two phases later
+//     (pass A and the middle stage lie in between), so the check practically never blocks;
+//   * the integer shift b of the NEXT group's line is fetched one iteration ahead, the lines of the group after next are
+//     requested into L2, and the symbol row (1 KB per line, shared by the warps of the line) is read through L1.
+// Slots of 496 floats put the two windows of a warp 16 banks apart for either block geometry: pass A is conflict free.
+namespace os2 {
+constexpr int XWIN = 496;              // floats per window slot
+constexpr int XCOPY = 492;             // floats copied per window: 3 (alignment) + 15 + 240 + V + 1 <= 492; the slot's
+                                       // last two words carry the integer shifts
+__device__ __forceinline__ void prefetch_l1(const void* gmem) { asm volatile("prefetch.global.L1 [%0];\n" ::"l"(gmem)); }
+}
+
+template <int V, int HLO>
+__global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int lpi = a.lpi, np = a.np, nitem = lpi * np * 16;        // nitem <= blockDim.x: one item per thread and phase
+    const int tid = threadIdx.x, T = blockDim.x, t = tid & 15, hw = tid >> 4, lane = tid & 31, warp = tid >> 5;
+    const int N = a.N, mask = N - 1, nwarps = T >> 5;
+    float* const win = reinterpret_cast<float*>(smem_raw) + hw * os2::XWIN;                       // this pair's window
+    float2* const scr = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + (T >> 4) * os2::XWIN) + hw * os2::XPAIR;
+    unsigned long long* const bars =
+        reinterpret_cast<unsigned long long*>(reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + (T >> 4) * os2::XWIN) +
+                                              (T >> 4) * os2::XPAIR);   // [0] landed; [1 + warp] windows of the warp
+    Tw4 w;
+    w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
+    w.b2 = __ldg(a.tw + 16 + t);
+    w.b4 = __ldg(a.tw + 3 * 16 + t);
+    w.b8 = __ldg(a.tw + 7 * 16 + t);
+    // (one barrier per thread: a loop over the barriers in ONE thread made ptxas 12.9 read the uniform register that
+    // holds the address of the last barrier before writing it, and the kernel then waited on an uninitialised object)
+    if (tid <= nwarps) {
+        os2::mbar_init(bars + tid, tid == 0 ? (unsigned)nwarps : 2u);     // [0]: one arrival per warp; others: the two
+        os2::mbar_init_fence();                                           // half-warp leaders' expect_tx arrivals
+    }
+    __syncthreads();
+    pdl_wait();                                   // (the twiddles above are plan constants; tables and grid are not)
+    pdl_launch_dependents();
+    const bool has_pair = hw * 16 < nitem;
+    const int l = (int)(((unsigned)hw * a.inv_np) >> 16), pp = hw - l * np;    // line of the group, pair of the line
+    const int G = gridDim.x;
+    float2* const sA = scr + t;                                                // passes A: column t of the pair
+    float2* const sM = scr + os2::XROW * t;                                    // middle stage: row g = t
+    // leader of a half-warp (t == 0): request this pair's window of line group g, whose line has the integer shift b
+    auto issue = [&](const int g, const int b) {
+        const int line = g * lpi + l;
+        if (!has_pair || line >= a.n_lines) { os2::mbar_arrive(bars + 1 + warp); return; }
+        os2::mbar_expect_tx(bars + 1 + warp, 4u * os2::XCOPY);
+        const float* const gl = a.src + (size_t)line * N;
+        const int a0 = ((pp * (2 * V) - HLO + b) & mask) & ~3;
+        if (a0 + os2::XCOPY <= N) os2::bulk_g2s(win, gl + a0, 4u * os2::XCOPY, bars + 1 + warp);
+        else {
+            const int n1 = N - a0;
+            os2::bulk_g2s(win, gl + a0, 4u * (unsigned)n1, bars + 1 + warp);
+            os2::bulk_g2s(win + n1, gl, 4u * (unsigned)(os2::XCOPY - n1), bars + 1 + warp);
         }
+    };
+    // The integer shifts travel through the two spare words of the slot, so that no register holds them across a
+    // phase (they were spilled, and the spill waited for the load): [495] = shift of the window in flight (written by
+    // the leader when it requests the window, read by the 16 threads in pass A), [494] = shift of the group after
+    // that, fetched by a 4-byte cp.async one iteration ahead.
+    int* const wsh = reinterpret_cast<int*>(win) + os2::XWIN - 2;
+    auto fetch_shift = [&](const int g) {          // leader: shift of this pair's line in group g -> wsh[0], asynchronously
+        const int line = g * lpi + l;
+        if (has_pair && g < a.n_groups && line < a.n_lines) os2::cp_async4(wsh, &a.lam[(size_t)line * OS_LAMW + 129].x);
+    };
+    // symbol row of the line of group g into L1, one iteration before the middle stage reads it (first pair of a line)
+    auto prefetch_row = [&](const int g) {
+        const int line = g * lpi + l;
+        if (has_pair && pp == 0 && g < a.n_groups && line < a.n_lines) {
+            const char* const row = reinterpret_cast<const char*>(a.lam + (size_t)line * OS_LAMW);
+            os2::prefetch_l1(row + 32 * t);
+            os2::prefetch_l1(row + 32 * (t + 16));
+            if (t == 0) os2::prefetch_l1(row + 1024);
+        }
+    };
+    if ((int)blockIdx.x < a.n_groups) {
+        if (t == 0) {
+            const int line = blockIdx.x * lpi + l;
+            const int b0 = (has_pair && line < a.n_lines) ? __float_as_int(__ldg(&a.lam[(size_t)line * OS_LAMW + 129].x)) : 0;
+            wsh[1] = b0;
+            issue(blockIdx.x, b0);
+            fetch_shift(blockIdx.x + G);
+        }
+        prefetch_row(blockIdx.x);
+    }
+    unsigned parity = 0;
+    for (int g = blockIdx.x; g < a.n_groups; g += G) {
+        const int gn = g + G;
+        const int line = g * lpi + l;
+        const bool active = has_pair && line < a.n_lines;
+        os2::mbar_wait(bars + 1 + warp, parity);   // this warp's windows have landed
+        if (lane == 0) os2::mbar_arrive(bars);
+        // ---- pass A from the window
+        if (active) {
+            const int b = wsh[1];
+            const float* const p = win + (((pp * (2 * V) - HLO + b) & mask) & 3) + t;
+            float2 x[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) x[k] = make_float2(p[16 * k], p[16 * k + V]);
+            dft_dif<16, 1>(x);
+            sA[0] = x[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                sA[os2::XROW * q] = cmul(x[brev(q, 16)], y);
+            });
+        }
+        __syncwarp();
+        // (the shared stores above needed every sample: the window slots of this warp are free)
+        if (gn < a.n_groups) {
+            if (t == 0) {
+                os2::cp_async_wait_all();          // the shift fetched one iteration ago
+                const int bn = wsh[0];
+                wsh[1] = bn;
+                issue(gn, bn);
+                fetch_shift(gn + G);
+                if (pp == 0 && has_pair && (gn + G) * lpi + l < a.n_lines)
+                    os2::bulk_prefetch_l2(a.src + (size_t)((gn + G) * lpi + l) * N, 4u * (unsigned)N);
+            }
+            prefetch_row(gn);
+        }
+        // ---- middle stage; the symbol row of the line through L1
+        if (active) {
+            const float2* __restrict__ const lamG = a.lam + (size_t)line * OS_LAMW;
+            float2 x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = sM[j];
+            dft_dif<16, 1>(x);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) x[brev(q, 16)] = cmul(x[brev(q, 16)], __ldg(lamG + t + 16 * q));
+#pragma unroll
+            for (int q = 8; q < 16; ++q) x[brev(q, 16)] = cmulc(x[brev(q, 16)], __ldg(lamG + 256 - 16 * q - t));
+            idft_dit<16, 1>(x);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) sM[j] = x[j];
+        }
+        __syncwarp();
+        os2::mbar_wait(bars, parity);              // every window of this line group is on chip: stores may begin
         // ---- inverse pass A: scratch -> registers -> global
-#pragma unroll 1
-        for (int it = tid; it < nitem; it += T) {
-            const int pr = it >> 4;
-            const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;
-            const float2* const sA = scr + pr * os2::XPAIR + t;
+        if (active) {
             float2 x[16];
             x[0] = sA[0];
             os2_tw_each(w, [&](auto qc, const float2 y) {
@@ -558,11 +501,13 @@ __global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsA
                 x[brev(q, 16)] = cmulc(sA[os2::XROW * q], y);
             });
             idft_dit<16, 1>(x);
-            if (g * lpi + l < a.n_lines) {
-                const int c = pp * (2 * V) + t - HLO;          // cell of sample n = t of block A
-                os2_store_x<V, HLO>(a.dst + (size_t)(g * lpi + l) * N + c, c, N, t, (pp + 1) * (2 * V) <= N, x);
-            }
+            const int c = pp * (2 * V) + t - HLO;          // cell of sample n = t of block A
+            float* const o = a.dst + (size_t)line * N + c;
+            if ((pp + 1) * (2 * V) <= N) os2_store_x_full<V, HLO>(o, t, x);
+            else os2_store_x<V, HLO>(o, c, N, t, false, x);
         }
+        __syncwarp();                              // the scratch of this warp is rewritten by its next pass A
+        parity ^= 1u;
     }
 }
 
@@ -576,54 +521,34 @@ __global__ void __launch_bounds__(V == 232 ? 288 : 320, 3) osx5_kernel(const OsA
 // Landing is planar inside the 256 bytes of a position (32 real parts = block A, then 32 imaginary parts =
 // block B) so that the 4-byte copies of a warp are bank-conflict free; pass A reads the planar words and
 // writes the position back as interleaved float2 (all reads of the warp precede its writes).
-__device__ __forceinline__ void osv2_land(float* __restrict__ pw, const float* __restrict__ col, const int Nx,
-                                          const int vmask, const int r0)
-{
-    constexpr int PS = 16 * 32 * 2;                 // floats between positions t + 16 k and t + 16 (k + 1)
-    const int rr = r0 & vmask;
-    if (rr + OS_V + 241 <= vmask + 1) {             // the two windows do not wrap: constant row stride
-        const float* p = col + (size_t)rr * Nx;
-        const float* q = p + (size_t)OS_V * Nx;
-        const size_t s16 = (size_t)16 * Nx;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            os2::cp_async4(pw + k * PS, p);
-            os2::cp_async4(pw + k * PS + 32, q);
-            p += s16;
-            q += s16;
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            const int ra = (r0 + 16 * k) & vmask, rb = (r0 + 16 * k + OS_V) & vmask;
-            os2::cp_async4(pw + k * PS, col + (size_t)ra * Nx);
-            os2::cp_async4(pw + k * PS + 32, col + (size_t)rb * Nx);
-        }
-    }
-}
-
 // delta-f source on the samples of one item: x[m].x += f_eq,g(v_j)(e^{X_j} - 1) at rows j = r0 + 16 m
 // (r0 = row of sample n = t of block A), x[m].y the same at rows j + V, with X_j = c s (2 (v_j - mu) - s) affine in j.
 // Along rows 16 apart expm1 obeys e' = e R + r (R = e^h, r = expm1(h), h = 32 c s dv); the recurrence starts in
 // the middle (m = 8) and runs both ways (RS[g] = (R, r, 1/R, expm1(-h)) per lane), so at most 8 steps accumulate.
-// Samples that are not kept (m = 15, and m = 0 unless HLO < 16) are skipped or harmlessly updated.  The f_eq table
+// Sample rows without kept samples (m = 15 and/or m = 0, depending on the geometry) are skipped.  The f_eq table
 // has 512 floats of padding: rows >= Nv are read but never stored; rows < 0 (m = 0 of the first pair) are clamped.
-template <int V, int HLO>
+template <int V, int HLO, int W = 32>
 __device__ __forceinline__ void osv2_source(float2* x, const OsArgs& a, const float4* __restrict__ RS, const int lane,
                                             const int r0, const float ssh)
 {
-    constexpr int M0 = HLO < 16 ? 0 : 1;
+    constexpr int M0 = KeptM<V, HLO, 0>::none ? 1 : 0;       // first and last sample rows that hold kept samples
+    constexpr int M1 = KeptM<V, HLO, 15>::none ? 14 : 15;
 #pragma unroll 1
     for (int g = 0; g < a.ng; ++g) {
         const float cgs = a.cg4[g] * ssh;
         const float* __restrict__ fa = a.feq_tab + g * a.Nv + r0;
         const float u0 = __ldg(a.vmu_tab + g * a.Nv);                          // v_0 - mu_g
-        const float4 Rr = RS[g * 32 + lane];
+        float4 Rr;
+        if (RS) Rr = RS[g * W + lane];
+        else {                                   // (the 16-column kernel has no room for the table)
+            const float hh = 32.0f * cgs * a.dvf;
+            Rr = make_float4(expf(hh), expm1f(hh), expf(-hh), expm1f(-hh));
+        }
         const float ea8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128), a.dvf, u0) - ssh));
         const float eb8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128 + V), a.dvf, u0) - ssh));
         float ea = ea8, eb = eb8;
 #pragma unroll
-        for (int m = 8; m < 15; ++m) {
+        for (int m = 8; m <= M1; ++m) {
             x[m].x = fmaf(__ldg(fa + 16 * m), ea, x[m].x);
             x[m].y = fmaf(__ldg(fa + 16 * m + V), eb, x[m].y);
             ea = fmaf(ea, Rr.x, Rr.y);
@@ -640,231 +565,6 @@ __device__ __forceinline__ void osv2_source(float2* x, const OsArgs& a, const fl
         }
     }
 }
-
-__global__ void __launch_bounds__(512, 2) osv2_kernel(const OsArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int W = 32;
-    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // 256 * 32
-    float2* const lamS = scr + 256 * W;                                       // 130 * 32, [k][lane]
-    float2* const twS = lamS + OS_LAMW * W;                                   // 15 * 16
-    float4* const RS = reinterpret_cast<float4*>(twS + 240);                  // [4][32] source recurrence constants
-    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5;   // wid = item index (t, g, j)
-    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
-    const int c0 = blockIdx.x * W;
-
-    {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
-        const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
-        float4* dst4 = reinterpret_cast<float4*>(lamS);
-        for (int i = tid; i < OS_LAMW * 16; i += T)
-            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
-    }
-    for (int i = tid; i < 240; i += T) twS[i] = __ldg(a.tw + i);
-    os2::cp_async_wait_all();
-    __syncthreads();
-    const int b = __float_as_int(lamS[129 * W + lane].x);
-    const float ssh = lamS[129 * W + lane].y;
-    if (a.ng > 0 && tid < 4 * W) {
-        // delta-f source: x_j = c s (2 (v_j - mu) - s) is affine in the row j, so along rows 16 apart
-        // expm1 obeys e' = e R + r with R = exp(h), r = expm1(h), h = 32 c s dv
-        const int g = tid >> 5;
-        const float h = 32.0f * (g < a.ng ? a.cg4[g] : 0.0f) * ssh * a.dvf;
-        RS[g * W + lane] = make_float4(expf(h), expm1f(h), expf(-h), expm1f(-h));
-    }
-    const float* const col = a.src + c0 + lane;
-    float* const ocol = a.dst + c0 + lane;
-    const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
-    float* const pw = reinterpret_cast<float*>(scr + wid * W) + lane;        // planar words of position t = wid
-    float2* const own = scr + wid * W + lane;                                 // the same position, interleaved
-    constexpr int PS2 = 16 * W;                                               // float2 between positions 16 apart
-
-    if (p0 < p1) osv2_land(pw, col, Nx, vmask, p0 * os2::PW - OS_H + b + wid);
-    __syncthreads();                               // RS visible (twS, lamS already are)
-    for (int p = p0; p < p1; ++p) {
-        int wt = wid;
-        asm volatile("" : "+r"(wt));               // keep the twiddle loads inside the loop (30 registers)
-        const float2* const twp = twS + wt;
-        os2::cp_async_wait_all();                  // this thread's samples have landed
-        // ---- pass A (item t = wid)
-        {
-            float2 x[16];
-#pragma unroll
-            for (int k = 0; k < 16; ++k) x[k] = make_float2(pw[k * PS2 * 2], pw[k * PS2 * 2 + W]);
-            __syncwarp();                          // planar words all read before the interleaved writes
-            dft_dif<16, 1>(x);
-            own[0] = x[0];
-#pragma unroll
-            for (int q = 1; q < 16; ++q) own[q * PS2] = cmul(x[brev(q, 16)], twp[(q - 1) * 16]);
-        }
-        __syncthreads();
-        // ---- middle stage (item g = wid): positions 16 g + j
-        {
-            float2* const s = scr + wid * 16 * W + lane;
-            float2 x[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) x[j] = s[j * W];
-            os2::mid16<W>(x, lamS + lane, wid);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) s[j * W] = x[j];
-        }
-        __syncthreads();
-        // ---- inverse pass A (item j = wid): kept samples m = 1..14 -> rows p PW + j + 16 (m - 1) (+ OS_V)
-        {
-            float2 x[16];
-            x[0] = own[0];
-#pragma unroll
-            for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(own[q * PS2], twp[(q - 1) * 16]);
-            __syncwarp();                          // interleaved words all read before the next planar landing
-            if (p + 1 < p1) osv2_land(pw, col, Nx, vmask, (p + 1) * os2::PW - OS_H + b + wid);
-            idft_dit<16, 1>(x);
-            const int row0 = p * os2::PW + wid;    // row of m = 1, block A
-            if (a.ng > 0) osv2_source<OS_V, OS_H>(x, a, RS, lane, row0 - 16, ssh);
-            float* po = ocol + (size_t)row0 * Nx;
-            const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
-            if (p * os2::PW + os2::PW <= Nv) {
-#pragma unroll
-                for (int m = 1; m < 15; ++m) {
-                    __stcs(po, x[m].x);
-                    __stcs(po + sV, x[m].y);
-                    po += s16;
-                }
-            } else {
-#pragma unroll
-                for (int m = 1; m < 15; ++m) {
-                    if (row0 + 16 * (m - 1) < Nv) __stcs(po, x[m].x);
-                    if (row0 + 16 * (m - 1) + OS_V < Nv) __stcs(po + sV, x[m].y);
-                    po += s16;
-                }
-            }
-        }
-        // no barrier here: pass A touches only the warp's own positions
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// v-direction, register-landing variant: as osv2_kernel, but the 32 samples of a warp's pass-A item go
-// straight from global memory into the butterfly registers (each load instruction of a warp is one
-// 128-byte row segment per distinct shift), and the twiddles are products of four register-resident powers
-// (t = warp index is fixed).  The scratch is only the exchange buffer between the phases.
-__device__ __forceinline__ void osv3_load(float2* x, const float* __restrict__ col, const int Nx, const int vmask,
-                                          const int r0)
-{
-    const int rr = r0 & vmask;
-    if (rr + OS_V + 241 <= vmask + 1) {             // the two windows do not wrap: constant row stride
-        const float* p = col + (size_t)rr * Nx;
-        const float* q = p + (size_t)OS_V * Nx;
-        const size_t s16 = (size_t)16 * Nx;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            x[k] = make_float2(__ldg(p), __ldg(q));
-            p += s16;
-            q += s16;
-        }
-    } else {
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            const int ra = (r0 + 16 * k) & vmask, rb = (r0 + 16 * k + OS_V) & vmask;
-            x[k] = make_float2(__ldg(col + (size_t)ra * Nx), __ldg(col + (size_t)rb * Nx));
-        }
-    }
-}
-
-__global__ void __launch_bounds__(512, 2) osv3_kernel(const OsArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int W = 32;
-    float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // 256 * 32
-    float2* const lamS = scr + 256 * W;                                       // 130 * 32, [k][lane]
-    float4* const RS = reinterpret_cast<float4*>(lamS + OS_LAMW * W);         // [4][32] source recurrence constants
-    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5;   // wid = item index (t, g, j)
-    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
-    const int c0 = blockIdx.x * W;
-
-    {   // symbol tables of the 32 columns: 130 rows of 256 B, transposed layout [k][column]
-        const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
-        float4* dst4 = reinterpret_cast<float4*>(lamS);
-        for (int i = tid; i < OS_LAMW * 16; i += T)
-            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
-    }
-    Tw4 w;
-    w.b1 = __ldg(a.tw + wid);
-    w.b2 = __ldg(a.tw + 16 + wid);
-    w.b4 = __ldg(a.tw + 3 * 16 + wid);
-    w.b8 = __ldg(a.tw + 7 * 16 + wid);
-    // integer shift and source shift of this lane's column straight from the table in global memory, so that
-    // the first loads do not wait for the staged copy
-    const float2 e129 = __ldg(a.lam + (size_t)129 * Nx + c0 + lane);
-    const int b = __float_as_int(e129.x);
-    const float ssh = e129.y;
-    if (a.ng > 0 && tid < 4 * W) {
-        const int g = tid >> 5;
-        const float h = 32.0f * (g < a.ng ? a.cg4[g] : 0.0f) * ssh * a.dvf;
-        RS[g * W + lane] = make_float4(expf(h), expm1f(h), expf(-h), expm1f(-h));
-    }
-    const float* const col = a.src + c0 + lane;
-    float* const ocol = a.dst + c0 + lane;
-    const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
-    float2* const own = scr + wid * W + lane;                                 // position t = wid
-    constexpr int PS2 = 16 * W;                                               // float2 between positions 16 apart
-
-    for (int p = p0; p < p1; ++p) {
-        // ---- pass A (item t = wid) straight from global memory
-        {
-            float2 x[16];
-            osv3_load(x, col, Nx, vmask, p * os2::PW - OS_H + b + wid);
-            dft_dif<16, 1>(x);
-            own[0] = x[0];
-            os2_tw_each(w, [&](auto qc, const float2 y) {
-                constexpr int q = decltype(qc)::value;
-                own[q * PS2] = cmul(x[brev(q, 16)], y);
-            });
-        }
-        if (p == p0) os2::cp_async_wait_all();     // symbol tables
-        __syncthreads();
-        // ---- middle stage (item g = wid): positions 16 g + j
-        {
-            float2* const s = scr + wid * 16 * W + lane;
-            float2 x[16];
-#pragma unroll
-            for (int j = 0; j < 16; ++j) x[j] = s[j * W];
-            os2::mid16<W>(x, lamS + lane, wid);
-#pragma unroll
-            for (int j = 0; j < 16; ++j) s[j * W] = x[j];
-        }
-        __syncthreads();
-        // ---- inverse pass A (item j = wid): kept samples m = 1..14 -> rows p PW + j + 16 (m - 1) (+ OS_V)
-        {
-            float2 x[16];
-            x[0] = own[0];
-            os2_tw_each(w, [&](auto qc, const float2 y) {
-                constexpr int q = decltype(qc)::value;
-                x[brev(q, 16)] = cmulc(own[q * PS2], y);
-            });
-            idft_dit<16, 1>(x);
-            const int row0 = p * os2::PW + wid;    // row of m = 1, block A
-            if (a.ng > 0) osv2_source<OS_V, OS_H>(x, a, RS, lane, row0 - 16, ssh);
-            float* po = ocol + (size_t)row0 * Nx;
-            const size_t s16 = (size_t)16 * Nx, sV = (size_t)OS_V * Nx;
-            if (p * os2::PW + os2::PW <= Nv) {
-#pragma unroll
-                for (int m = 1; m < 15; ++m) {
-                    __stcs(po, x[m].x);
-                    __stcs(po + sV, x[m].y);
-                    po += s16;
-                }
-            } else {
-#pragma unroll
-                for (int m = 1; m < 15; ++m) {
-                    if (row0 + 16 * (m - 1) < Nv) __stcs(po, x[m].x);
-                    if (row0 + 16 * (m - 1) + OS_V < Nv) __stcs(po + sV, x[m].y);
-                    po += s16;
-                }
-            }
-        }
-        // no barrier here: the next pass A writes only the warp's own positions, which it has just read
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // v-direction, coalesced-landing variant.  osv2_kernel lets every lane fetch its own shifted rows, which is a
 // gather of up to 32 rows per load instruction when neighbouring columns have different integer shifts (the
@@ -877,7 +577,7 @@ __global__ void __launch_bounds__(512, 2) osv3_kernel(const OsArgs a)
 template <int V, int HLO>
 __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int W = 32;
     float2* const scr = reinterpret_cast<float2*>(smem_raw);                  // 256 * 32 float2 = raw[512][32] floats
     float* const raw = reinterpret_cast<float*>(smem_raw);
@@ -895,10 +595,10 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
         const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
         float4* dst4 = reinterpret_cast<float4*>(lamS);
         for (int i = tid; i < OS_LAMW * 16; i += T)
-            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (Nx / 2) + (i & 15));
+            os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 4) * (a.lam_ks / 2) + (i & 15));
     }
     // integer shift (rows) and source shift of this lane's column
-    const float2 e129 = __ldg(a.lam + (size_t)129 * Nx + c0 + lane);
+    const float2 e129 = __ldg(a.lam + (size_t)129 * a.lam_ks + c0 + lane);
     const int b = __float_as_int(e129.x);
     const float ssh = e129.y;
     // spread of the shifts over the strip, as signed distances from column 0's (shifts live mod Nv)
@@ -979,6 +679,301 @@ __global__ void __launch_bounds__(512, 2) osv4_kernel(const OsArgs a)
             os2_store_v<V, HLO>(ocol + (ptrdiff_t)r0 * Nx, (size_t)Nx, r0, Nv, wid, (p + 1) * (2 * V) <= Nv, x);
         }
         if (p + 1 < p1) __syncthreads();           // the exchange buffer is read before the next raw rows land
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// v-direction, 16-column strips with the next window in flight (default).  Same arithmetic as osv4_kernel, other
+// shape: a strip is 16 adjacent columns (64-byte row segments), an item (t, g or j) is a HALF-warp, a CTA is 8 warps
+// and handles one pair of blocks of its strip per iteration.  The raw rows (the union of the rows the 16 columns need,
+// landed unshifted by 16-byte cp.async) and the exchange buffer are SEPARATE 32 KB buffers, so
+//   * the raw rows of the CTA's NEXT pair are requested as soon as pass A has emptied the raw buffer and land during
+//     the middle stage and the inverse pass (the 32-column kernel shares one buffer and loads nothing while it computes);
+//   * three CTA barriers per pair instead of five;
+//   * 64 KB per CTA: three CTAs (24 warps) per SM, out of phase with one another.
+// The symbol table of the strip is read straight from global memory ([k][column]: a half-warp reads one 128-byte
+// row; 16.5 KB per strip, re-read for every pair, so it lives in L1 -- f itself is loaded with cp.async.cg, which
+// bypasses L1).  Bank conflicts: raw[row][16] floats -- a lane only touches bank (column + 16 (row & 1)), and the two
+// half-warps of a warp read rows of opposite parity (items t, t + 1): conflict free for any per-column shift;
+// exchange [position][16] float2 -- a half-warp covers one 128-byte row: conflict free.
+// Strips whose integer shifts spread over more rows than the raw buffer holds fall back to a per-lane landing of the
+// same buffer (4-byte cp.async).  Out of place (src != dst).
+namespace os2 {
+__device__ __forceinline__ void cp_async16_cg(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem) : "memory");
+}
+constexpr int VW = 16;                 // columns per strip
+constexpr int VRR = 516;               // rows of the raw buffer (33 KB + 32 KB of exchange buffer: three CTAs per SM
+                                       // inside the 196 KB shared-memory carve-out, which leaves ~60 KB of L1 for the
+                                       // symbol tables of the three strips)
+}  // namespace os2
+
+// kept samples of a FULL pair along rows (row stride Nx): no bounds predicates
+template <int V, int HLO, int M = 0>
+__device__ __forceinline__ void os2_store_v_full(float* __restrict__ po, const size_t Nx, const int t, const float2* x)
+{
+    if constexpr (M < 16) {
+        using K = KeptM<V, HLO, M>;
+        if constexpr (K::all) {
+            __stcs(po + (size_t)(16 * M) * Nx, x[M].x);
+            __stcs(po + (size_t)(16 * M + V) * Nx, x[M].y);
+        } else if constexpr (!K::none) {
+            if (K::kept(t)) {
+                __stcs(po + (size_t)(16 * M) * Nx, x[M].x);
+                __stcs(po + (size_t)(16 * M + V) * Nx, x[M].y);
+            }
+        }
+        os2_store_v_full<V, HLO, M + 1>(po, Nx, t, x);
+    }
+}
+
+template <int V, int HLO>
+__global__ void __launch_bounds__(256, 3) osv6_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int W = os2::VW, RR = os2::VRR;
+    constexpr int RMAX = RR - OS_LB - V;           // spread of the integer shifts that the raw buffer can hold
+    float* const raw = reinterpret_cast<float*>(smem_raw);                        // [RR][16]
+    float2* const exch = reinterpret_cast<float2*>(raw + RR * W);                 // [256][16]
+    const int tid = threadIdx.x, c = tid & 15, h = tid >> 4;                      // column of the strip, item index
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
+    const int c0 = blockIdx.x * W;
+    Tw4 w;
+    w.b1 = __ldg(a.tw + h);                       // [q-1][t] = e^{-2 pi i t q / 256}, t = item index of passes A
+    w.b2 = __ldg(a.tw + 16 + h);
+    w.b4 = __ldg(a.tw + 3 * 16 + h);
+    w.b8 = __ldg(a.tw + 7 * 16 + h);
+    pdl_wait();                                   // the symbol tables and the source grid come from earlier kernels
+    pdl_launch_dependents();
+    const float2* __restrict__ const lamC = a.lam + c0 + c;                       // entry k of this column: lamC[k ks]
+    // integer shift (rows) and source shift of this lane's column
+    const size_t ks = (size_t)a.lam_ks;            // row stride of the table: Nx + 16 entries (not a power of two: the 129
+                                                  // rows of a strip fall into different L1 sets)
+    const float2 e129 = __ldg(lamC + 129 * ks);
+    const int b = __float_as_int(e129.x);
+    const float ssh = e129.y;
+    // spread of the shifts over the strip, as signed distances from column 0's (shifts live mod Nv)
+    const int b0 = __shfl_sync(0xffffffffu, b, 0, 16);
+    const int d = (((b - b0) + (Nv >> 1)) & vmask) - (Nv >> 1);
+    int dmin = d, dmax = d;
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) {
+        dmin = min(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+        dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+    }
+    const int R = dmax - dmin;
+    const bool gather = R > RMAX;                  // uniform over the CTA (every half-warp sees the same 16 columns)
+    const int db = gather ? 0 : d - dmin;          // this lane's row offset inside the raw window
+    const int base = gather ? b : b0 + dmin;       // first raw row = pair start - HLO + base
+    const float* const col = a.src + c0 + c;
+    float* const ocol = a.dst + c0 + c;
+    const int p0 = blockIdx.y * a.gpc, p1 = min(a.np, p0 + a.gpc);
+    float2* const own = exch + h * W + c;                                     // position t = h
+    constexpr int PS = 16 * W;                                                // float2 between positions 16 apart
+    const int nrows = V + OS_LB + (gather ? 0 : R);
+
+    // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
+    auto land = [&](const int p) {
+        const int rs = p * (2 * V) - HLO + base;
+        if (!gather) {
+            const float* const src = a.src + c0;
+            for (int i = tid; i < nrows * 4; i += 256) {
+                const int r = i >> 2, q4 = (i & 3) * 4;
+                os2::cp_async16_cg(raw + r * W + q4, src + (size_t)((rs + r) & vmask) * Nx + q4);
+            }
+        } else {
+            for (int r = h; r < nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
+        }
+    };
+    if (p0 < p1) land(p0);
+    for (int p = p0; p < p1; ++p) {
+        os2::cp_async_wait_all();
+        __syncthreads();                           // raw rows of pair p visible; exchange buffer of pair p - 1 read
+        // ---- pass A (item t = h): samples from the raw rows with this lane's offset
+        {
+            float2 x[16];
+            const float* const rp = raw + (h + db) * W + c;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + V) * W]);
+            dft_dif<16, 1>(x);
+            own[0] = x[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                own[q * PS] = cmul(x[brev(q, 16)], y);
+            });
+        }
+        __syncthreads();                           // exchange buffer complete; raw rows all read
+        if (p + 1 < p1) land(p + 1);               // the next window lands behind the middle stage and the inverse pass
+        // ---- middle stage (item g = h): positions 16 g + j; symbol from the table in global memory (L1)
+        {
+            float2* const sp = exch + h * 16 * W + c;
+            float2 x[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = sp[j * W];
+            dft_dif<16, 1>(x);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) x[brev(q, 16)] = cmul(x[brev(q, 16)], __ldg(lamC + (size_t)(h + 16 * q) * ks));
+#pragma unroll
+            for (int q = 8; q < 16; ++q) x[brev(q, 16)] = cmulc(x[brev(q, 16)], __ldg(lamC + (size_t)(256 - 16 * q - h) * ks));
+            idft_dit<16, 1>(x);
+#pragma unroll
+            for (int j = 0; j < 16; ++j) sp[j * W] = x[j];
+        }
+        __syncthreads();
+        // ---- inverse pass A (item j = h): kept samples -> rows of the destination
+        {
+            float2 x[16];
+            x[0] = own[0];
+            os2_tw_each(w, [&](auto qc, const float2 y) {
+                constexpr int q = decltype(qc)::value;
+                x[brev(q, 16)] = cmulc(own[q * PS], y);
+            });
+            idft_dit<16, 1>(x);
+            const int r0 = p * (2 * V) + h - HLO;          // row of sample n = t = h of block A
+            if (a.ng > 0) osv2_source<V, HLO, W>(x, a, nullptr, c, r0, ssh);
+            float* const po = ocol + (ptrdiff_t)r0 * Nx;
+            if ((p + 1) * (2 * V) <= Nv) os2_store_v_full<V, HLO>(po, (size_t)Nx, h, x);
+            else os2_store_v<V, HLO>(po, (size_t)Nx, r0, Nv, h, false, x);
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// v-direction, three groups per CTA sharing the strip's symbol table (default).  osv6_kernel reads the symbol through
+// L1, and the profile shows that this is what it waits for (long-scoreboard stalls on the multiplies of the middle
+// stage, L1 hit rate 18 %: three strips x 16.5 KB do not stay resident beside the streaming traffic).  Here ONE CTA of
+// 768 threads per SM holds the table of its strip in shared memory (16.6 KB, staged once per work item) and runs
+// THREE groups of 8 warps on it, each with its own raw-row buffer and exchange buffer (3 x 64.5 KB) and its own named
+// barrier: the groups are the three CTAs of osv6_kernel, minus the table traffic, and drift apart in the same way.
+// A work item is (strip of 16 columns, segment of consecutive pairs); group i takes pairs i, i + 3, .. of the segment
+// and has the raw rows of its next pair in flight while it transforms the current one.  Persistent grid.
+namespace os2 {
+__device__ __forceinline__ void bar_group(const int id) { asm volatile("bar.sync %0, 256;\n" ::"r"(id) : "memory"); }
+}
+
+template <int V, int HLO>
+__global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int W = os2::VW, RR = os2::VRR;
+    constexpr int RMAX = RR - OS_LB - V;           // spread of the integer shifts that the raw buffer can hold
+    constexpr int GB = RR * W * 4 + OS_LB * W * 8; // bytes per group: raw rows + exchange buffer
+    float2* const lamS = reinterpret_cast<float2*>(smem_raw);                     // [OS_LAMW][16]
+    const int tid = threadIdx.x, gid = tid >> 8, gt = tid & 255;                  // group, thread of the group
+    unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + gid * GB;
+    float* const raw = reinterpret_cast<float*>(gbase);                           // [RR][16]
+    float2* const exch = reinterpret_cast<float2*>(raw + RR * W);                 // [256][16]
+    const int c = gt & 15, h = gt >> 4;                                           // column of the strip, item index
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
+    const int nstrips = Nx / W, nseg = (a.np + a.gpc - 1) / a.gpc, n_items = nstrips * nseg;
+    Tw4 w;
+    w.b1 = __ldg(a.tw + h);                       // [q-1][t] = e^{-2 pi i t q / 256}, t = item index of passes A
+    w.b2 = __ldg(a.tw + 16 + h);
+    w.b4 = __ldg(a.tw + 3 * 16 + h);
+    w.b8 = __ldg(a.tw + 7 * 16 + h);
+    pdl_wait();                                   // the symbol tables and the source grid come from earlier kernels
+    pdl_launch_dependents();
+    float2* const own = exch + h * W + c;                                     // position t = h
+    constexpr int PS = 16 * W;                                                // float2 between positions 16 apart
+    const size_t ks = (size_t)a.lam_ks;
+
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const int strip = item % nstrips, seg = item / nstrips;              // (neighbouring CTAs: neighbouring strips)
+        const int c0 = strip * W;
+        const int q0 = seg * a.gpc, q1 = min(a.np, q0 + a.gpc);              // pairs of the segment
+        __syncthreads();                           // every group is done with the table of the previous item
+        {   // symbol table of the strip: OS_LAMW rows of 128 B
+            const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
+            float4* dst4 = reinterpret_cast<float4*>(lamS);
+            for (int i = tid; i < OS_LAMW * 8; i += 768)
+                os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 3) * (ks / 2) + (i & 7));
+        }
+        // integer shift (rows) and source shift of this lane's column
+        const float2 e129 = __ldg(a.lam + 129 * ks + c0 + c);
+        const int b = __float_as_int(e129.x);
+        const float ssh = e129.y;
+        // spread of the shifts over the strip, as signed distances from column 0's (shifts live mod Nv)
+        const int b0 = __shfl_sync(0xffffffffu, b, 0, 16);
+        const int d = (((b - b0) + (Nv >> 1)) & vmask) - (Nv >> 1);
+        int dmin = d, dmax = d;
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) {
+            dmin = min(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+            dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+        }
+        const int R = dmax - dmin;
+        const bool gather = R > RMAX;              // uniform over the CTA (every half-warp sees the same 16 columns)
+        const int db = gather ? 0 : d - dmin;      // this lane's row offset inside the raw window
+        const int base = gather ? b : b0 + dmin;   // first raw row = pair start - HLO + base
+        const float* const col = a.src + c0 + c;
+        float* const ocol = a.dst + c0 + c;
+        const int nrows = V + OS_LB + (gather ? 0 : R);
+        // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
+        auto land = [&](const int p) {
+            const int rs = p * (2 * V) - HLO + base;
+            if (!gather) {
+                const float* const src = a.src + c0;
+                for (int i = gt; i < nrows * 4; i += 256) {
+                    const int r = i >> 2, q4 = (i & 3) * 4;
+                    os2::cp_async16_cg(raw + r * W + q4, src + (size_t)((rs + r) & vmask) * Nx + q4);
+                }
+            } else {
+                for (int r = h; r < nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
+            }
+        };
+        const int p0 = q0 + gid;
+        if (p0 < q1) land(p0);
+        os2::cp_async_wait_all();                  // this thread's chunks of the table (and of the first raw rows)
+        __syncthreads();                           // table visible to everybody
+        for (int p = p0; p < q1; p += 3) {
+            os2::cp_async_wait_all();
+            os2::bar_group(gid + 1);               // raw rows of pair p visible; exchange buffer of the last pair read
+            // ---- pass A (item t = h): samples from the raw rows with this lane's offset
+            {
+                float2 x[16];
+                const float* const rp = raw + (h + db) * W + c;
+#pragma unroll
+                for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + V) * W]);
+                dft_dif<16, 1>(x);
+                own[0] = x[0];
+                os2_tw_each(w, [&](auto qc, const float2 y) {
+                    constexpr int q = decltype(qc)::value;
+                    own[q * PS] = cmul(x[brev(q, 16)], y);
+                });
+            }
+            os2::bar_group(gid + 1);               // exchange buffer complete; raw rows all read
+            if (p + 3 < q1) land(p + 3);           // the next window lands behind the middle stage and the inverse pass
+            // ---- middle stage (item g = h): positions 16 g + j
+            {
+                float2* const sp = exch + h * 16 * W + c;
+                float2 x[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) x[j] = sp[j * W];
+                os2::mid16<W>(x, lamS + c, h);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) sp[j * W] = x[j];
+            }
+            os2::bar_group(gid + 1);
+            // ---- inverse pass A (item j = h): kept samples -> rows of the destination
+            {
+                float2 x[16];
+                x[0] = own[0];
+                os2_tw_each(w, [&](auto qc, const float2 y) {
+                    constexpr int q = decltype(qc)::value;
+                    x[brev(q, 16)] = cmulc(own[q * PS], y);
+                });
+                idft_dit<16, 1>(x);
+                const int r0 = p * (2 * V) + h - HLO;          // row of sample n = t = h of block A
+                if (a.ng > 0) osv2_source<V, HLO, W>(x, a, nullptr, c, r0, ssh);
+                float* const po = ocol + (ptrdiff_t)r0 * Nx;
+                if ((p + 1) * (2 * V) <= Nv) os2_store_v_full<V, HLO>(po, (size_t)Nx, h, x);
+                else os2_store_v<V, HLO>(po, (size_t)Nx, r0, Nv, h, false, x);
+            }
+        }
     }
 }
 

@@ -16,8 +16,8 @@ LAGRANGE, BSPLINE = 0, 1
 SPLIT_XVX, SPLIT_VXV = 0, 1
 
 EXPORTS = ("vog_plan", "vog_destroy", "vog_advect_x", "vog_advect_v", "vog_field", "vog_step",
-           "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_probe_x_memory_pattern", "vog_run", "vog_run_host", "vog_run_host_async", "vog_launch_count",
-           "vog_strerror", "vog_plan_tune")
+           "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_run", "vog_run_host",
+           "vog_run_host_async", "vog_launch_count", "vog_strerror", "vog_plan_tune", "vog_reset")
 
 
 class vog_feq_t(ctypes.Structure):
@@ -59,7 +59,6 @@ def lib():
         L.vog_shift_x.argtypes = [vp, vp, vp]
         L.vog_shift_v.argtypes = [vp, vp, vp]
         L.vog_shift_v_to.argtypes = [vp, vp, vp, vp]
-        L.vog_probe_x_memory_pattern.argtypes = [vp, vp, vp]
         L.vog_run.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, ctypes.c_int, vp]
         L.vog_run_host.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp]
         L.vog_run_host_async.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp]
@@ -68,6 +67,7 @@ def lib():
         L.vog_strerror.argtypes = [ctypes.c_int]
         L.vog_strerror.restype = ctypes.c_char_p
         L.vog_plan_tune.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+        L.vog_reset.argtypes = [vp]
         for name in EXPORTS:
             if name not in ("vog_launch_count", "vog_strerror"):
                 getattr(L, name).restype = ctypes.c_int
@@ -147,9 +147,6 @@ class Plan:
     def shift_v(self, f, beta):
         self._ck(lib().vog_shift_v(self._h, _ptr(f), _ptr(beta)), "vog_shift_v")
 
-    def probe_x_memory_pattern(self, src, dst):
-        self._ck(lib().vog_probe_x_memory_pattern(self._h, _ptr(src), _ptr(dst)), "vog_probe_x_memory_pattern")
-
     def shift_v_to(self, src, dst, beta):
         self._ck(lib().vog_shift_v_to(self._h, _ptr(src), _ptr(dst), _ptr(beta)), "vog_shift_v_to")
 
@@ -167,6 +164,9 @@ class Plan:
 
     def launch_count(self):
         return int(lib().vog_launch_count(self._h))
+
+    def reset(self):
+        self._ck(lib().vog_reset(self._h), "vog_reset")
 
     def tune(self, which, value):
         self._ck(lib().vog_plan_tune(self._h, int(which), int(value)), "vog_plan_tune")
