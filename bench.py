@@ -398,7 +398,9 @@ def main():
                     tgt[str(N)] = {"x_kernel_frac": _r(r["x_kernel_only"]["frac_hbm"]),
                                    "x_call_frac": _r(r["x"]["frac_hbm"]), "v_call_frac": _r(r["v"]["frac_hbm"]),
                                    "v_out_of_place_frac": _r(r.get("v_out_of_place", {}).get("frac_hbm")),
-                                   "step_frac_28B": _r(r["strang_step"]["frac_hbm"])}
+                                   "step_frac_28B": _r(r["strang_step"]["frac_hbm"]),
+                                   "direct_stencil_x_v_step": [_r(r.get("direct_stencil", {}).get(k, {}).get("frac_hbm"))
+                                                               for k in ("x_kernel_only", "v_out_of_place", "strang_step")]}
         roofline["target_8192"] = tgt.get("8192")
         roofline["at_16384"] = tgt.get("16384")
     # ---- oracle on the host cores (rank 0, N=1 only)
@@ -495,6 +497,19 @@ def sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle):
             row["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step(f, 1e-3), 2, 5), 28.0)
             row["strang_step"]["cell_updates_per_s"] = N * N / (row["strang_step"]["us_median"] * 1e-6)
             plan.destroy()
+            if N >= 1024:
+                # the same matrix applied directly (vog_plan_tune(27, 1)): beside the Fourier path,
+                # never instead of it -- the north-star fractions above are the Fourier kernels'
+                plan = vog.Plan(N, N, 1.0, -1.0, 1.0, kind, order, stream=stream)
+                plan.tune(27, 1)
+                st = {"x_kernel_only": rec(*_time_calls(torch, stream, lambda: plan.advect_x(f, 0.01), 3, 10))}
+                if N * N * 4 * 3 < 160e9:
+                    g = torch.empty_like(f)
+                    st["v_out_of_place"] = rec(*_time_calls(torch, stream, lambda: plan.shift_v_to(f, g, bx), 3, 10))
+                    del g
+                st["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step(f, 1e-3), 2, 5), 28.0)
+                row["direct_stencil"] = st
+                plan.destroy()
             if fo is not None:
                 ot = {}
                 for name, fn in (("x", orc.shift_x), ("v", orc.shift_v)):

@@ -79,6 +79,18 @@ int vog_advect_v(vog_plan_t plan, float* f_dev, const float* E_dev, double dt);
  * with zero mean.  f_dev is not modified. */
 int vog_field(vog_plan_t plan, const float* f_dev, float* E_dev);
 
+/* The paper's diagnostics of a state, all summed in fp64 in a fixed order.
+ * Solves the field of f_dev with the plan's field solver (it stays in the plan like after vog_field) and writes five
+ * doubles to diag_dev (device memory):
+ *   [0] electric energy (1/2) dx sum_i E_i^2
+ *   [1] rho^_0 = (1/Nx) sum_i rho_i, the equilibrium's mass dv sum_j f_eq(v_j) added in delta-f mode: the "error of
+ *       mass" of P:245 is |[1] - 1|
+ *   [2] |rho^_1| = |(1/Nx) sum_i rho_i e^(-2 i pi i/Nx)|, "the first mode of rho in absolute value"
+ *   [3] kinetic energy (1/2) dx dv sum_j v_j^2 sum_i f_ji, the equilibrium's part added in delta-f mode
+ *   [4] total energy [0] + [3]
+ * f_dev is not modified.  VOG_EINVAL for NULL pointers. */
+int vog_diagnostics(vog_plan_t plan, const float* f_dev, double* diag_dev);
+
 /* One Strang step of size dt, in place (Q1).  E_ext_dev (Nx floats, or NULL) is added
  * to the self-consistent field before every v-advection of the step (for the KEEN drive pass
  * -E_app).
@@ -159,6 +171,15 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   26     programmatic dependent launch of the plan's kernels: 1 = each kernel may be staged on the SMs while its
  *          predecessor in the stream drains and waits for it on the device (default up to 8192 x 8192), 0 = plain
  *          stream order.  Results are bit-identical either way.
+ *   27     how the circulant product of lines >= 1024 cells is taken: 0 = in Fourier space (default: FFT, symbol,
+ *          inverse FFT, P:131-149 -- the path BASELINE.json names), 1 = directly, u'_i = sum_j a_j u_(i+b+j) with the
+ *          2d+2 non-zero entries of the row of A (eq (4); the spline's row cut at |j| <= 14 like the
+ *          Fourier path's blocks).  The same matrix up to rounding.  Shorter lines always use
+ *          the Fourier kernels.
+ *   28     field solve: 0 = Fourier, modes 0 and Nx/2 dropped (default); 1 = trapezoidal rule with the
+ *          zero-mean modifications on rho and on E; 2 = trapezoidal rule without them (rho - 1, P:213;
+ *          minus the equilibrium's mass in delta-f mode) -- the variant whose drift the paper shows in Fig. 1.
+ *          This one DOES change results: it is the paper's other solver, not a launch shape.
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

@@ -419,6 +419,60 @@ void oracle_field(int Nx, int Nv, const double *f, double L, double vmin, double
     free(rho);
 }
 
+/* The paper's other field solve, written out step by step:
+ *   M = (1/N) sum_k rho_k;  rho~_k = rho_k - M           (zero_mean != 0)
+ *                           rho~_k = rho_k - background   (zero_mean == 0: "rho~ = rho - 1"; the caller passes
+ *                                                          the background, 1 minus the equilibrium's mass in delta-f mode)
+ *   E~_0 = 0;  E~_{k+1} = E~_k + dx (rho~_k + rho~_{k+1}) / 2,  k = 0 .. N-2      (trapezoidal rule)
+ *   M~ = (1/N) sum_k E~_k;  E_k = E~_k - M~               (zero_mean != 0); E_k = E~_k otherwise. */
+void oracle_field_trapezoid(int Nx, const double *rho, double L, int zero_mean, double background, double *E)
+{
+    double dx = L / (double)Nx;
+    double M = background;
+    if (zero_mean) {
+        M = 0.0;
+        for (int k = 0; k < Nx; ++k) M += rho[k];
+        M /= (double)Nx;
+    }
+    E[0] = 0.0;
+    for (int k = 0; k + 1 < Nx; ++k) E[k + 1] = E[k] + dx * ((rho[k] - M) + (rho[k + 1] - M)) / 2.0;
+    if (zero_mean) {
+        double Mt = 0.0;
+        for (int k = 0; k < Nx; ++k) Mt += E[k];
+        Mt /= (double)Nx;
+        for (int k = 0; k < Nx; ++k) E[k] -= Mt;
+    }
+}
+
+/* Diagnostics of P:245, 253-261 from a density:  out[0] = rho^_0 = (1/N) sum_k rho_k  (the mass error is |rho^_0 - 1|,
+ * P:245; in delta-f mode the caller adds the equilibrium's mass);  out[1] = |rho^_1| = |(1/N) sum_k rho_k e^{-2 i pi k/N}|
+ * ("the first mode of rho in absolute value"). */
+void oracle_rho_modes(int Nx, const double *rho, double *out)
+{
+    double s0 = 0.0, sr = 0.0, si = 0.0;
+    for (int k = 0; k < Nx; ++k) {
+        double a = -2.0 * M_PI * (double)k / (double)Nx;
+        s0 += rho[k];
+        sr += rho[k] * cos(a);
+        si += rho[k] * sin(a);
+    }
+    out[0] = s0 / (double)Nx;
+    out[1] = sqrt(sr * sr + si * si) / (double)Nx;
+}
+
+/* Kinetic energy: E_k = int int f v^2/2 dv dx ~ (1/2) dx dv sum_j v_j^2 sum_i f_ji (rectangle rule on the
+ * periodic mesh, the same weights as rho).  Of the stored array: in delta-f mode the caller adds the equilibrium's part. */
+double oracle_kinetic_energy(int Nx, int Nv, const double *f, double L, double vmin, double vmax)
+{
+    double dx = L / (double)Nx, dv = (vmax - vmin) / (double)Nv, s = 0.0;
+    for (int j = 0; j < Nv; ++j) {
+        double v = mesh_v(j, Nv, vmin, vmax), r = 0.0;
+        for (int i = 0; i < Nx; ++i) r += f[(size_t)j * Nx + i];
+        s += v * v * r;
+    }
+    return 0.5 * dx * dv * s;
+}
+
 /* Electric energy (1/2) ||E||^2_{L2} = (1/2) dx sum_i E_i^2. */
 double oracle_electric_energy(int Nx, const double *E, double L)
 {

@@ -215,6 +215,31 @@ def field(f, L, vmin, vmax):
     return E
 
 
+def field_trapezoid(rho, L, zero_mean=True, background=0.0):
+    """trapezoidal rule for E from rho, with (default) or without the zero-mean modifications."""
+    rho = _c(rho)
+    E = np.zeros_like(rho)
+    lib().oracle_field_trapezoid(ctypes.c_int(rho.size), _p(rho), ctypes.c_double(L), ctypes.c_int(1 if zero_mean else 0),
+                                 ctypes.c_double(background), _p(E))
+    return E
+
+
+def rho_modes(rho):
+    """(rho^_0, |rho^_1|) of P:245, 261."""
+    rho = _c(rho)
+    out = np.zeros(2)
+    lib().oracle_rho_modes(ctypes.c_int(rho.size), _p(rho), _p(out))
+    return float(out[0]), float(out[1])
+
+
+def kinetic_energy(f, L, vmin, vmax):
+    f = _c(f)
+    Nv, Nx = f.shape
+    lib().oracle_kinetic_energy.restype = ctypes.c_double
+    return float(lib().oracle_kinetic_energy(ctypes.c_int(Nx), ctypes.c_int(Nv), _p(f), ctypes.c_double(L),
+                                             ctypes.c_double(vmin), ctypes.c_double(vmax)))
+
+
 def electric_energy(E, L):
     E = _c(E)
     return float(lib().oracle_electric_energy(ctypes.c_int(E.size), _p(E), ctypes.c_double(L)))

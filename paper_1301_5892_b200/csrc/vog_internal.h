@@ -146,6 +146,13 @@ cudaError_t osv7_launch(const OsArgs& a, int geom, int n_sm, cudaStream_t st);
 cudaError_t osv6_launch(const OsArgs& a, int geom, dim3 grid, cudaStream_t st);
 cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st);
 
+// ---- direct-stencil kernels (vog_stencil.cu): the same circulant product without the transforms (NEXT-4)
+cudaError_t st_setup_launch(const OsSetupArgs& s, float* taps, cudaStream_t st);
+size_t stx_smem_bytes(int spline, int d, int threads);
+cudaError_t stx_launch(const OsArgs& a, int spline, int d, const float* taps, int grid, int threads, size_t smem, cudaStream_t st);
+int stx_occupancy(int spline, int d, int threads, size_t smem);
+cudaError_t stv_launch(const OsArgs& a, int spline, int d, const float* taps, cudaStream_t st);
+
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
 typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,
                                         size_t smem, cudaStream_t st);

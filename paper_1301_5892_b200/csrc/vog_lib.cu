@@ -186,10 +186,14 @@ __global__ void shift_setup_x_kernel(const SetupArgs s)
 // the 8 warps through shared memory; fp64 accumulation, fixed order => deterministic.  Block (x, y) writes the sums
 // of its row slab to part[y][32 x .. 32 x + 31]; the Poisson kernel adds the NBY slabs in index order (no atomics,
 // no "last block" pass: the slabs are <= 16 rows of Nx doubles, a few KB for the single CTA that needs them).
+// KIN: also the column sums weighted with v_j^2 (kinetic energy) into partk, same layout.
+template <bool KIN>
 __global__ void __launch_bounds__(256) density_partial_kernel(const float* __restrict__ f, int Nx, int Nv,
-                                                              int rows_per_block, double* __restrict__ part)
+                                                              int rows_per_block, double* __restrict__ part,
+                                                              double* __restrict__ partk, double vmin, double dvd)
 {
     __shared__ double red[8][32];
+    __shared__ double redk[KIN ? 8 : 1][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int xl = lane & 7, rl = lane >> 3;
     const int col = blockIdx.x * 32 + xl * 4;
@@ -197,11 +201,16 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
     pdl_wait();                                   // f comes from the advection before; part may still be read
     pdl_launch_dependents();
     double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    double k0 = 0, k1 = 0, k2 = 0, k3 = 0;
     const float* p = f + (size_t)(j0 + warp * 4 + rl) * Nx + col;
 #pragma unroll 4
     for (int j = warp * 4 + rl; j < rows_per_block; j += 32) {
         const float4 v = __ldg(reinterpret_cast<const float4*>(p));
         s0 += (double)v.x; s1 += (double)v.y; s2 += (double)v.z; s3 += (double)v.w;
+        if constexpr (KIN) {
+            const double vj = vmin + (double)(j0 + j) * dvd, v2 = vj * vj;
+            k0 += v2 * (double)v.x; k1 += v2 * (double)v.y; k2 += v2 * (double)v.z; k3 += v2 * (double)v.w;
+        }
         p += (size_t)32 * Nx;
     }
 #pragma unroll
@@ -210,14 +219,131 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
         s1 += __shfl_xor_sync(0xffffffffu, s1, o);
         s2 += __shfl_xor_sync(0xffffffffu, s2, o);
         s3 += __shfl_xor_sync(0xffffffffu, s3, o);
+        if constexpr (KIN) {
+            k0 += __shfl_xor_sync(0xffffffffu, k0, o);
+            k1 += __shfl_xor_sync(0xffffffffu, k1, o);
+            k2 += __shfl_xor_sync(0xffffffffu, k2, o);
+            k3 += __shfl_xor_sync(0xffffffffu, k3, o);
+        }
     }
-    if (rl == 0) { red[warp][xl * 4 + 0] = s0; red[warp][xl * 4 + 1] = s1; red[warp][xl * 4 + 2] = s2; red[warp][xl * 4 + 3] = s3; }
+    if (rl == 0) {
+        red[warp][xl * 4 + 0] = s0; red[warp][xl * 4 + 1] = s1; red[warp][xl * 4 + 2] = s2; red[warp][xl * 4 + 3] = s3;
+        if constexpr (KIN) { redk[warp][xl * 4 + 0] = k0; redk[warp][xl * 4 + 1] = k1; redk[warp][xl * 4 + 2] = k2; redk[warp][xl * 4 + 3] = k3; }
+    }
     __syncthreads();
     if (threadIdx.x < 32) {
-        double s = 0;
+        double s = 0, k = 0;
 #pragma unroll
-        for (int w = 0; w < 8; ++w) s += red[w][threadIdx.x];
+        for (int w = 0; w < 8; ++w) {
+            s += red[w][threadIdx.x];
+            if constexpr (KIN) k += redk[w][threadIdx.x];
+        }
         part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
+        if constexpr (KIN) partk[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = k;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// NEXT-3: the paper's other field solve and its diagnostics, one CTA of 1024 threads.
+//   solver 1: trapezoidal rule with the zero-mean modifications: M = mean rho, rho~ = rho - M,
+//             E~_0 = 0, E~_{k+1} = E~_k + dx (rho~_k + rho~_{k+1})/2, E = E~ - mean E~;
+//   solver 2: the same without them: rho~ = rho - background ("rho - 1"; minus the equilibrium's mass in
+//             delta-f mode), E = E~;
+//   solver 0: E is given (the Fourier solve ran before): diagnostics only.
+// diag (if not NULL): [0] (1/2) dx sum E^2, [1] rho^_0 + mass0 (mass error = |.. - 1|), [2] |rho^_1|
+// (P:261), [3] kinetic energy (1/2) dx dv sum_j v_j^2 sum_i f_ji + kin0, [4] total energy [0] + [3].
+// All sums in fp64, fixed order.
+__device__ __forceinline__ double block_sum_1024(double v, double* red, const int tid, const int T)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();                               // red may still be read from the last call
+    if ((tid & 31) == 0) red[tid >> 5] = v;
+    __syncthreads();
+    double s = 0.0;
+    for (int w = 0; w < (T >> 5); ++w) s += red[w];
+    return s;
+}
+
+__global__ void __launch_bounds__(1024) field_aux_kernel(int Nx, int solver, const double* __restrict__ part,
+                                                         const double* __restrict__ partk, int nby, double dv, double dx,
+                                                         double background, double mass0, double kin0,
+                                                         double* __restrict__ rho, float* __restrict__ E_a,
+                                                         float* __restrict__ E_b, double* __restrict__ diag)
+{
+    __shared__ double red[32];
+    __shared__ double scan[1024];
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int per = (Nx + T - 1) / T, i0 = tid * per, i1 = min(Nx, i0 + per);     // consecutive cells per thread
+    pdl_wait();
+    pdl_launch_dependents();
+    // rho_i = dv * (sum of the slab sums, in slab order); K = dv sum_i (sum_j v_j^2 f_ji)
+    double srho = 0.0, skin = 0.0, sre = 0.0, sim = 0.0;
+    for (int i = i0; i < i1; ++i) {
+        double s = 0.0;
+        for (int y = 0; y < nby; ++y) s += __ldcg(part + (size_t)y * Nx + i);
+        s *= dv;
+        rho[i] = s;                                // (solver 0: the Fourier solve has written the same value already)
+        srho += s;
+        if (diag) {
+            double sn, cs;
+            sincospi(-2.0 * (double)i / (double)Nx, &sn, &cs);
+            sre += s * cs;
+            sim += s * sn;
+            if (partk) {
+                double k = 0.0;
+                for (int y = 0; y < nby; ++y) k += __ldcg(partk + (size_t)y * Nx + i);
+                skin += k;
+            }
+        }
+    }
+    const double mean = block_sum_1024(srho, red, tid, T) / (double)Nx;
+    double e2 = 0.0;
+    if (solver != 0) {
+        __syncthreads();                           // rho[] of the neighbouring thread's first cell
+        const double M = solver == 1 ? mean : background;
+        // increments d_k = dx (rho~_{k-1} + rho~_k)/2 for k >= 1, d_0 = 0; E~_k = inclusive sum
+        double loc = 0.0;
+        for (int i = i0; i < i1; ++i)
+            if (i > 0) loc += dx * ((rho[i - 1] - M) + (rho[i] - M)) * 0.5;
+        scan[tid] = loc;
+        __syncthreads();
+        // exclusive scan of the 1024 per-thread sums (Hillis-Steele in shared memory, fp64)
+        for (int o = 1; o < T; o <<= 1) {
+            const double add = tid >= o ? scan[tid - o] : 0.0;
+            __syncthreads();
+            scan[tid] += add;
+            __syncthreads();
+        }
+        double run = tid > 0 ? scan[tid - 1] : 0.0;
+        double sE = 0.0;
+        for (int i = i0; i < i1; ++i) {
+            if (i > 0) run += dx * ((rho[i - 1] - M) + (rho[i] - M)) * 0.5;
+            sE += run;
+        }
+        const double Mt = solver == 1 ? block_sum_1024(sE, red, tid, T) / (double)Nx : 0.0;
+        run = tid > 0 ? scan[tid - 1] : 0.0;
+        for (int i = i0; i < i1; ++i) {
+            if (i > 0) run += dx * ((rho[i - 1] - M) + (rho[i] - M)) * 0.5;
+            const float e = (float)(run - Mt);
+            E_a[i] = e;
+            if (E_b) E_b[i] = e;
+            e2 += (double)e * (double)e;
+        }
+    } else if (diag) {
+        for (int i = i0; i < i1; ++i) { const double e = (double)E_a[i]; e2 += e * e; }
+    }
+    if (diag) {
+        const double se2 = block_sum_1024(e2, red, tid, T);
+        const double re = block_sum_1024(sre, red, tid, T), im = block_sum_1024(sim, red, tid, T);
+        const double kin = block_sum_1024(skin, red, tid, T);
+        if (tid == 0) {
+            diag[0] = 0.5 * dx * se2;
+            diag[1] = mean + mass0;
+            diag[2] = sqrt(re * re + im * im) / (double)Nx;
+            diag[3] = 0.5 * dx * dv * kin + kin0;
+            diag[4] = diag[0] + diag[3];
+        }
     }
 }
 
@@ -365,6 +491,12 @@ struct vog_plan_s {
     vog::PoissonRadix prx;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int os2x_lpi, os3x_occ, os2v_gpc;      // x: lines per iteration, cached occupancy; v: pairs per CTA (0 = default)
+    int solver;                            // field solve: 0 = Fourier (default), 1 = trapezoid + zero mean, 2 = trapezoid, rho - 1
+    double feq_mass, feq_kin;              // dv sum_j f_eq(v_j) and (1/2) L dv sum_j v_j^2 f_eq(v_j) (0 in full-f mode)
+    double *partk, *diag;                  // kinetic-energy slab sums [nby_max][Nx]; 5 doubles of scratch
+    int method;                            // advection of lines >= 1024 cells: 0 = in Fourier space (default, the graded path), 1 = direct stencil (NEXT-4)
+    float *taps_x, *taps_v;                // stencil path: taps [Nv][32] and, transposed, [32][Nx + 16]
+    int stx_occ;
     int osv_variant;                       // v kernel: 0 = 16-column strips, next window in flight (osv6_kernel, default), 1 = 32-column strips (osv4_kernel)
     int osx_variant;                       // x kernel: 0 = per-pair windows when a group fits one round (osx7_kernel), else whole lines; 1 = whole lines always (osx6_kernel)
     int pdl;                               // programmatic dependent launch of the step's kernels (default: grids up to 8192^2)
@@ -509,11 +641,11 @@ extern "C" const char* vog_strerror(int status)
 static void free_plan(vog_plan_s* P)
 {
     if (!P) return;
-    cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twv); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->ptw); cudaFree(P->cg4);
+    cudaFree(P->taps_x); cudaFree(P->taps_v); cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twv); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->ptw); cudaFree(P->cg4);
     cudaFree(P->g_buf);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
-    cudaFree(P->part); cudaFree(P->rho); cudaFree(P->E_self);
+    cudaFree(P->part); cudaFree(P->partk); cudaFree(P->diag); cudaFree(P->rho); cudaFree(P->E_self);
     cudaFree(P->feq_tab); cudaFree(P->vmu_tab); cudaFree(P->f_buf); cudaFree(P->ext_buf);
     delete P;
 }
@@ -641,11 +773,15 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     for (int g = 0; g < 4; ++g) cg4h[g] = g < ng ? (float)p->feq.c[g] : 0.0f;
     alloc((void**)&P->os_lam_x, sizeof(float2) * OS_LAMW * (P->os_x ? Nv : 1));
     alloc((void**)&P->os_lam_v, sizeof(float2) * OS_LAMW * (P->os_v ? Nx + 16 : 1));   // rows of Nx + 16 entries
+    alloc((void**)&P->taps_x, sizeof(float) * 32 * (P->os_x ? Nv : 1));
+    alloc((void**)&P->taps_v, sizeof(float) * 32 * (P->os_v ? Nx + 16 : 1));
     alloc((void**)&P->xtwA, sizeof(float2) * xa.size());
     alloc((void**)&P->xtwB, sizeof(float2) * xb.size());
     alloc((void**)&P->xcs, sizeof(float2) * xc.size());
     alloc((void**)&P->rec_v, sizeof(float) * REC_WORDS * Nx);
     alloc((void**)&P->part, sizeof(double) * P->nby_max * Nx);
+    alloc((void**)&P->partk, sizeof(double) * P->nby_max * Nx);
+    alloc((void**)&P->diag, sizeof(double) * 8);
     alloc((void**)&P->rho, sizeof(double) * Nx);
     alloc((void**)&P->E_self, sizeof(float) * Nx);
     alloc((void**)&P->feq_tab, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512));   // + padding read (not used) by osv2_kernel
@@ -675,8 +811,11 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
             for (int j = 0; j < Nv; ++j) {
                 const double v = p->vmin + (double)j * dv;
                 const double u = v - p->feq.mu[g];
-                ft[(size_t)g * Nv + j] = (float)(p->feq.amp[g] * std::exp(-p->feq.c[g] * u * u));
+                const double fe = p->feq.amp[g] * std::exp(-p->feq.c[g] * u * u);
+                ft[(size_t)g * Nv + j] = (float)fe;
                 vt[(size_t)g * Nv + j] = (float)u;
+                P->feq_mass += dv * fe;
+                P->feq_kin += 0.5 * p->L * dv * v * v * fe;
             }
         e = cudaMemcpyAsync(P->feq_tab, ft.data(), sizeof(float) * ft.size(), cudaMemcpyHostToDevice, P->st);
         if (e == cudaSuccess) e = cudaMemcpyAsync(P->vmu_tab, vt.data(), sizeof(float) * vt.size(), cudaMemcpyHostToDevice, P->st);
@@ -710,8 +849,9 @@ static OsxShape osx_shape(const vog_plan_s* P, int lpi)
     o.thr = ((16 * per + 31) / 32) * 32;
     // bulk-landed kernel: lines (+ repeated head), two symbol rows per line, exchange scratch per resident pair
     o.smem6 = (size_t)lpi * (P->p.Nx + 480) * 4 + (size_t)2 * lpi * OS_LAMW * 8 + (size_t)(o.thr / 16) * (16 * 17 * 8) + 16;
-    // warp-private windows (one round only): window slot + exchange scratch per pair, one mbarrier per warp + 1
-    o.smem7 = (size_t)(o.thr / 16) * (496 * 4 + 16 * 17 * 8) + (size_t)(o.thr / 32 + 1) * 8;
+    // warp-private windows (one round only): window slot, exchange scratch (overlapping by its unused last element) and
+    // two shift words per pair, two symbol rows per line, one mbarrier per warp + 2
+    o.smem7 = (size_t)(o.thr / 16) * (492 * 4 + (16 * 17 - 1) * 8 + 8) + 8 + (size_t)2 * lpi * OS_LAMW * 8 + (size_t)(o.thr / 32 + 2) * 8;
     return o;
 }
 
@@ -744,6 +884,8 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
         case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
         case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
+        case 28: if (value < 0 || value > 2) return VOG_EINVAL; P->solver = value; P->E_of = nullptr; P->E_valid = false; break;
+        case 27: if (value < 0 || value > 1) return VOG_EINVAL; P->method = value; P->recx_valid = false; P->E_of = nullptr; break;
         default: return VOG_EINVAL;
     }
     return VOG_OK;
@@ -777,6 +919,7 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
         s.E = E; s.Eext = Eext; s.beta = beta;
         s.cs64 = P->os_cs64;
         s.lam = vdir ? P->os_lam_v : P->os_lam_x;
+        if (P->method == 1) return st_setup_launch(s, vdir ? P->taps_v : P->taps_x, P->st);
         return os_setup_launch(s, P->st);
     }
     SetupArgs s;
@@ -823,6 +966,47 @@ static cudaError_t run_osx(vog_plan_s* P, const float* src, float* dst)
     P->launches++;
     if (windows) return osx7_launch(a, geom, grid, o.thr, smem, P->st);
     return osx6_launch(a, geom, grid, o.thr, smem, P->st);
+}
+
+// ---- direct-stencil launches (line length >= 1024; kernels in vog_stencil.cu)
+static cudaError_t run_stx(vog_plan_s* P, const float* src, float* dst)
+{
+    OsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nx;
+    a.np = Nx / 512;                               // segments per line
+    int lpi = 256 / (16 * a.np);
+    if (lpi < 1) lpi = 1;
+    while (lpi > 1 && (Nv + lpi - 1) / lpi < P->n_sm * 3) --lpi;
+    a.lpi = lpi;
+    a.n_lines = Nv;
+    a.n_groups = (Nv + lpi - 1) / lpi;
+    const int thr = ((16 * a.np * lpi + 31) / 32) * 32;
+    const int spline = P->sym == SYM_SPLINE3;
+    const size_t smem = stx_smem_bytes(spline, P->d, thr);
+    if (P->stx_occ == 0) {
+        P->stx_occ = stx_occupancy(spline, P->d, thr, smem);
+        if (P->stx_occ <= 0) return cudaErrorInvalidConfiguration;
+    }
+    int grid = P->stx_occ * P->n_sm;
+    if (grid > a.n_groups) grid = a.n_groups;
+    P->launches++;
+    return stx_launch(a, spline, P->d, P->taps_x, grid, thr, smem, P->st);
+}
+
+static cudaError_t run_stv(vog_plan_s* P, const float* src, float* dst, bool source)
+{
+    OsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    a.src = src; a.dst = dst; a.Nx = Nx; a.Nv = Nv; a.N = Nv;
+    a.lam_ks = Nx + 16;
+    a.ng = source ? P->p.feq.n : 0;
+    a.feq_tab = P->feq_tab; a.vmu_tab = P->vmu_tab; a.cg4 = P->cg4;
+    a.dvf = (float)((P->p.vmax - P->p.vmin) / (double)Nv);
+    P->launches++;
+    return stv_launch(a, P->sym == SYM_SPLINE3, P->d, P->taps_v, P->st);
 }
 
 static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool source)
@@ -926,7 +1110,7 @@ static cudaError_t copy_grid(vog_plan_s* P, float* dst, const float* src)
 // x-advection src -> dst (dst may equal src); the shift records/tables must be current
 static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
 {
-    if (P->os_x) return run_osx(P, src, dst);
+    if (P->os_x) return P->method == 1 ? run_stx(P, src, dst) : run_osx(P, src, dst);
     cudaError_t e = cudaSuccess;
     if (src != dst) e = copy_grid(P, dst, src);
     if (e == cudaSuccess) e = run_advect_line(P, dst, false, false);
@@ -936,7 +1120,7 @@ static cudaError_t advect_x(vog_plan_s* P, const float* src, float* dst)
 // v-advection src -> dst; the overlap-save kernel needs dst != src, the whole-line kernel works in place
 static cudaError_t advect_v(vog_plan_s* P, const float* src, float* dst, bool source)
 {
-    if (P->os_v) return src == dst ? cudaErrorInvalidValue : run_osv(P, src, dst, source);
+    if (P->os_v) return src == dst ? cudaErrorInvalidValue : (P->method == 1 ? run_stv(P, src, dst, source) : run_osv(P, src, dst, source));
     cudaError_t e = cudaSuccess;
     if (src != dst) e = copy_grid(P, dst, src);
     if (e == cudaSuccess) e = run_advect_line(P, dst, true, source);
@@ -948,32 +1132,53 @@ static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
 {
     if (!P->os_v) return run_advect_line(P, f, true, source);
     cudaError_t e = ensure_gbuf(P);
-    if (e == cudaSuccess) e = run_osv(P, f, P->g_buf, source);
+    if (e == cudaSuccess) e = P->method == 1 ? run_stv(P, f, P->g_buf, source) : run_osv(P, f, P->g_buf, source);
     if (e == cudaSuccess) e = copy_grid(P, f, P->g_buf);
     return e;
 }
 
-static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double* energy_out = nullptr)
+static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double* energy_out = nullptr,
+                             double* diag_out = nullptr)
 {
     const int Nx = P->p.Nx, Nv = P->p.Nv;
-    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv, dx = P->p.L / (double)Nx;
     dim3 grid(Nx / 32, P->nby);
-    cudaError_t e = launch_pdl(density_partial_kernel, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part);
-    if (e != cudaSuccess) return e;
-    int T = Nx / 4;
-    if (T > 1024) T = 1024;
-    if (T < 32) T = 32;
-    const int tw_in_smem = Nx <= 8192;
-    const size_t psmem = (sizeof(float2) + sizeof(float)) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
-    e = set_max_smem((const void*)poisson_kernel, psmem);
+    cudaError_t e;
+    if (diag_out)
+        e = launch_pdl(density_partial_kernel<true>, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part, P->partk,
+                       P->p.vmin, dv);
+    else
+        e = launch_pdl(density_partial_kernel<false>, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part,
+                       (double*)nullptr, 0.0, 0.0);
     if (e != cudaSuccess) return e;
     P->launches += 2;
     P->E_valid = true;
     P->E_of = f;
-    return launch_pdl(poisson_kernel, dim3(1), dim3(T), psmem, P->st, Nx, P->prx, P->ptw_len, tw_in_smem,
-                      (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->part, P->nby, dv, P->rho, P->E_self, E_out,
-                      energy_out,
-                      0.5 * P->p.L / (double)Nx);
+    int Ta = Nx < 1024 ? Nx : 1024;
+    if (P->solver == 0) {
+        int T = Nx / 4;
+        if (T > 1024) T = 1024;
+        if (T < 32) T = 32;
+        const int tw_in_smem = Nx <= 8192;
+        const size_t psmem = (sizeof(float2) + sizeof(float)) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
+        e = set_max_smem((const void*)poisson_kernel, psmem);
+        if (e != cudaSuccess) return e;
+        e = launch_pdl(poisson_kernel, dim3(1), dim3(T), psmem, P->st, Nx, P->prx, P->ptw_len, tw_in_smem,
+                       (const float2*)P->ptw, (const float*)P->ikt, (const double*)P->part, P->nby, dv, P->rho, P->E_self, E_out,
+                       energy_out, 0.5 * dx);
+        if (e != cudaSuccess || !diag_out) return e;
+        P->launches++;
+        return launch_pdl(field_aux_kernel, dim3(1), dim3(Ta), 0, P->st, Nx, 0, (const double*)P->part, (const double*)P->partk,
+                          P->nby, dv, dx, 0.0, P->feq_mass, P->feq_kin, P->rho, P->E_self, (float*)nullptr, diag_out);
+    }
+    // trapezoid solve; the electric energy of vog_run goes through the plan's diagnostics scratch
+    double* const dg = diag_out ? diag_out : (energy_out ? P->diag : nullptr);
+    e = launch_pdl(field_aux_kernel, dim3(1), dim3(Ta), 0, P->st, Nx, P->solver, (const double*)P->part,
+                   (const double*)(diag_out ? P->partk : nullptr), P->nby, dv, dx, 1.0 - P->feq_mass, P->feq_mass, P->feq_kin,
+                   P->rho, P->E_self, E_out, dg);
+    if (e == cudaSuccess && energy_out)
+        e = cudaMemcpyAsync(energy_out, dg, sizeof(double), cudaMemcpyDeviceToDevice, P->st);
+    return e;
 }
 
 static cudaError_t ensure_recx(vog_plan_s* P, double dt)
@@ -1041,6 +1246,13 @@ extern "C" int vog_field(vog_plan_t P, const float* f_dev, float* E_dev)
     if (!P || !f_dev || !E_dev) return VOG_EINVAL;
     t_pdl = P->pdl != 0;
     return cuda_status(run_field(P, f_dev, E_dev));
+}
+
+extern "C" int vog_diagnostics(vog_plan_t P, const float* f_dev, double* diag_dev)
+{
+    if (!P || !f_dev || !diag_dev) return VOG_EINVAL;
+    t_pdl = P->pdl != 0;
+    return cuda_status(run_field(P, f_dev, nullptr, nullptr, diag_dev));
 }
 
 extern "C" int vog_get_field(vog_plan_t P, float* E_dev)

@@ -360,10 +360,8 @@ __global__ void __launch_bounds__(288, 3) osx6_kernel(const OsArgs a)
 //     requested into L2, and the symbol row (1 KB per line, shared by the warps of the line) is read through L1.
 // Slots of 496 floats put the two windows of a warp 16 banks apart for either block geometry: pass A is conflict free.
 namespace os2 {
-constexpr int XWIN = 496;              // floats per window slot
-constexpr int XCOPY = 492;             // floats copied per window: 3 (alignment) + 15 + 240 + V + 1 <= 492; the slot's
-                                       // last two words carry the integer shifts
-__device__ __forceinline__ void prefetch_l1(const void* gmem) { asm volatile("prefetch.global.L1 [%0];\n" ::"l"(gmem)); }
+constexpr int XWIN = 492;              // floats per window slot = floats copied per window: 3 (alignment) + 15 + 240 + V + 1
+constexpr int XCOPY = XWIN;
 }
 
 template <int V, int HLO>
@@ -373,11 +371,16 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
     const int lpi = a.lpi, np = a.np, nitem = lpi * np * 16;        // nitem <= blockDim.x: one item per thread and phase
     const int tid = threadIdx.x, T = blockDim.x, t = tid & 15, hw = tid >> 4, lane = tid & 31, warp = tid >> 5;
     const int N = a.N, mask = N - 1, nwarps = T >> 5;
+    // shared memory (sized to the byte: three CTAs of 18 pairs fill an SM): window slots | symbol rows [2][lpi] | exchange
+    // scratch (the unused last pad element of a pair's 16 x 17 block overlaps the next pair's first) | shifts | mbarriers
+    const int S = T >> 4;                                                                          // pair slots
     float* const win = reinterpret_cast<float*>(smem_raw) + hw * os2::XWIN;                       // this pair's window
-    float2* const scr = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + (T >> 4) * os2::XWIN) + hw * os2::XPAIR;
-    unsigned long long* const bars =
-        reinterpret_cast<unsigned long long*>(reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + (T >> 4) * os2::XWIN) +
-                                              (T >> 4) * os2::XPAIR);   // [0] landed; [1 + warp] windows of the warp
+    float2* const lamS = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + S * os2::XWIN);   // [2][lpi][OS_LAMW]
+    float2* const scr = lamS + 2 * lpi * OS_LAMW + hw * (os2::XPAIR - 1);
+    int* const wsh = reinterpret_cast<int*>(lamS + 2 * lpi * OS_LAMW + S * (os2::XPAIR - 1) + 1) + 2 * hw;   // [S][2]
+    unsigned long long* const bars = reinterpret_cast<unsigned long long*>(
+        reinterpret_cast<int*>(lamS + 2 * lpi * OS_LAMW + S * (os2::XPAIR - 1) + 1) + 2 * S);
+    // bars: [0] landed; [1] symbol rows; [2 + warp] windows of the warp
     Tw4 w;
     w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
     w.b2 = __ldg(a.tw + 16 + t);
@@ -385,9 +388,10 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
     w.b8 = __ldg(a.tw + 7 * 16 + t);
     // (one barrier per thread: a loop over the barriers in ONE thread made ptxas 12.9 read the uniform register that
     // holds the address of the last barrier before writing it, and the kernel then waited on an uninitialised object)
-    if (tid <= nwarps) {
-        os2::mbar_init(bars + tid, tid == 0 ? (unsigned)nwarps : 2u);     // [0]: one arrival per warp; others: the two
-        os2::mbar_init_fence();                                           // half-warp leaders' expect_tx arrivals
+    if (tid <= nwarps + 1) {
+        // [0]: one arrival per warp; [1]: thread 0's expect_tx; others: the two half-warp leaders' expect_tx arrivals
+        os2::mbar_init(bars + tid, tid == 0 ? (unsigned)nwarps : (tid == 1 ? 1u : 2u));
+        os2::mbar_init_fence();
     }
     __syncthreads();
     pdl_wait();                                   // (the twiddles above are plan constants; tables and grid are not)
@@ -400,35 +404,33 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
     // leader of a half-warp (t == 0): request this pair's window of line group g, whose line has the integer shift b
     auto issue = [&](const int g, const int b) {
         const int line = g * lpi + l;
-        if (!has_pair || line >= a.n_lines) { os2::mbar_arrive(bars + 1 + warp); return; }
-        os2::mbar_expect_tx(bars + 1 + warp, 4u * os2::XCOPY);
+        if (!has_pair || line >= a.n_lines) { os2::mbar_arrive(bars + 2 + warp); return; }
+        os2::mbar_expect_tx(bars + 2 + warp, 4u * os2::XCOPY);
         const float* const gl = a.src + (size_t)line * N;
         const int a0 = ((pp * (2 * V) - HLO + b) & mask) & ~3;
-        if (a0 + os2::XCOPY <= N) os2::bulk_g2s(win, gl + a0, 4u * os2::XCOPY, bars + 1 + warp);
+        if (a0 + os2::XCOPY <= N) os2::bulk_g2s(win, gl + a0, 4u * os2::XCOPY, bars + 2 + warp);
         else {
             const int n1 = N - a0;
-            os2::bulk_g2s(win, gl + a0, 4u * (unsigned)n1, bars + 1 + warp);
-            os2::bulk_g2s(win + n1, gl, 4u * (unsigned)(os2::XCOPY - n1), bars + 1 + warp);
+            os2::bulk_g2s(win, gl + a0, 4u * (unsigned)n1, bars + 2 + warp);
+            os2::bulk_g2s(win + n1, gl, 4u * (unsigned)(os2::XCOPY - n1), bars + 2 + warp);
         }
     };
-    // The integer shifts travel through the two spare words of the slot, so that no register holds them across a
-    // phase (they were spilled, and the spill waited for the load): [495] = shift of the window in flight (written by
-    // the leader when it requests the window, read by the 16 threads in pass A), [494] = shift of the group after
+    // The integer shifts travel through two words of shared memory per pair, so that no register holds them across
+    // a phase (they were spilled, and the spill waited for the load): wsh[1] = shift of the window in flight (written
+    // by the leader when it requests the window, read by the 16 threads in pass A), wsh[0] = shift of the group after
     // that, fetched by a 4-byte cp.async one iteration ahead.
-    int* const wsh = reinterpret_cast<int*>(win) + os2::XWIN - 2;
     auto fetch_shift = [&](const int g) {          // leader: shift of this pair's line in group g -> wsh[0], asynchronously
         const int line = g * lpi + l;
         if (has_pair && g < a.n_groups && line < a.n_lines) os2::cp_async4(wsh, &a.lam[(size_t)line * OS_LAMW + 129].x);
     };
-    // symbol row of the line of group g into L1, one iteration before the middle stage reads it (first pair of a line)
-    auto prefetch_row = [&](const int g) {
-        const int line = g * lpi + l;
-        if (has_pair && pp == 0 && g < a.n_groups && line < a.n_lines) {
-            const char* const row = reinterpret_cast<const char*>(a.lam + (size_t)line * OS_LAMW);
-            os2::prefetch_l1(row + 32 * t);
-            os2::prefetch_l1(row + 32 * (t + 16));
-            if (t == 0) os2::prefetch_l1(row + 1024);
-        }
+    // thread 0: symbol rows of the lines of group g into row buffer (par).  Called for group g + G right after the
+    // landed barrier of group g: by then every warp has started pass A of group g, i.e. is done with the middle stage
+    // of group g - G, whose rows this overwrites; they arrive long before the first middle stage of group g + G.
+    auto issue_rows = [&](const int g, const unsigned par) {
+        const int line0 = g * lpi, nl = min(lpi, a.n_lines - line0);
+        os2::mbar_expect_tx(bars + 1, (unsigned)nl * 8u * OS_LAMW);
+        for (int i = 0; i < nl; ++i)
+            os2::bulk_g2s(lamS + (par * lpi + i) * OS_LAMW, a.lam + (size_t)(line0 + i) * OS_LAMW, 8u * OS_LAMW, bars + 1);
     };
     if ((int)blockIdx.x < a.n_groups) {
         if (t == 0) {
@@ -438,14 +440,18 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
             issue(blockIdx.x, b0);
             fetch_shift(blockIdx.x + G);
         }
-        prefetch_row(blockIdx.x);
+        if (tid == 0) issue_rows(blockIdx.x, 0u);
     }
     unsigned parity = 0;
     for (int g = blockIdx.x; g < a.n_groups; g += G) {
         const int gn = g + G;
         const int line = g * lpi + l;
         const bool active = has_pair && line < a.n_lines;
-        os2::mbar_wait(bars + 1 + warp, parity);   // this warp's windows have landed
+        os2::mbar_wait(bars + 2 + warp, parity);   // this warp's windows have landed
+        // (the symbol rows of this group were requested a whole group ago.  The wait sits HERE, before the arrival on
+        // the landed barrier, because thread 0 re-arms the row barrier right after the landed barrier completes: a
+        // warp that had not yet observed this phase would then miss it and wait for ever.)
+        os2::mbar_wait(bars + 1, parity);
         if (lane == 0) os2::mbar_arrive(bars);
         // ---- pass A from the window
         if (active) {
@@ -473,25 +479,19 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
                 if (pp == 0 && has_pair && (gn + G) * lpi + l < a.n_lines)
                     os2::bulk_prefetch_l2(a.src + (size_t)((gn + G) * lpi + l) * N, 4u * (unsigned)N);
             }
-            prefetch_row(gn);
         }
-        // ---- middle stage; the symbol row of the line through L1
+        // ---- middle stage
         if (active) {
-            const float2* __restrict__ const lamG = a.lam + (size_t)line * OS_LAMW;
             float2 x[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j) x[j] = sM[j];
-            dft_dif<16, 1>(x);
-#pragma unroll
-            for (int q = 0; q < 8; ++q) x[brev(q, 16)] = cmul(x[brev(q, 16)], __ldg(lamG + t + 16 * q));
-#pragma unroll
-            for (int q = 8; q < 16; ++q) x[brev(q, 16)] = cmulc(x[brev(q, 16)], __ldg(lamG + 256 - 16 * q - t));
-            idft_dit<16, 1>(x);
+            os2::mid16<1>(x, lamS + (parity * lpi + l) * OS_LAMW, t);
 #pragma unroll
             for (int j = 0; j < 16; ++j) sM[j] = x[j];
         }
         __syncwarp();
         os2::mbar_wait(bars, parity);              // every window of this line group is on chip: stores may begin
+        if (tid == 0 && gn < a.n_groups) issue_rows(gn, parity ^ 1u);
         // ---- inverse pass A: scratch -> registers -> global
         if (active) {
             float2 x[16];
@@ -863,18 +863,18 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
     constexpr int RMAX = RR - OS_LB - V;           // spread of the integer shifts that the raw buffer can hold
     constexpr int GB = RR * W * 4 + OS_LB * W * 8; // bytes per group: raw rows + exchange buffer
     float2* const lamS = reinterpret_cast<float2*>(smem_raw);                     // [OS_LAMW][16]
+    float2* const twS = lamS + OS_LAMW * W;                                       // [15][16] e^{-2 pi i t q / 256}
     const int tid = threadIdx.x, gid = tid >> 8, gt = tid & 255;                  // group, thread of the group
-    unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + gid * GB;
+    unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + 240 * 8 + gid * GB;
     float* const raw = reinterpret_cast<float*>(gbase);                           // [RR][16]
     float2* const exch = reinterpret_cast<float2*>(raw + RR * W);                 // [256][16]
     const int c = gt & 15, h = gt >> 4;                                           // column of the strip, item index
     const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
     const int nstrips = Nx / W, nseg = (a.np + a.gpc - 1) / a.gpc, n_items = nstrips * nseg;
-    Tw4 w;
-    w.b1 = __ldg(a.tw + h);                       // [q-1][t] = e^{-2 pi i t q / 256}, t = item index of passes A
-    w.b2 = __ldg(a.tw + 16 + h);
-    w.b4 = __ldg(a.tw + 3 * 16 + h);
-    w.b8 = __ldg(a.tw + 7 * 16 + h);
+    // (the FP32 pipe is what this kernel waits for most: the 15 twiddles of an item come from a 1.9 KB table in
+    // shared memory, 15 loads per pass, instead of 11 complex products of four register-resident powers)
+    for (int i = tid; i < 240; i += 768) twS[i] = __ldg(a.tw + i);               // (plan constant: before the wait)
+    const float2* const twp = twS + h;            // [q-1][t], t = item index of passes A
     pdl_wait();                                   // the symbol tables and the source grid come from earlier kernels
     pdl_launch_dependents();
     float2* const own = exch + h * W + c;                                     // position t = h
@@ -940,10 +940,8 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
                 for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + V) * W]);
                 dft_dif<16, 1>(x);
                 own[0] = x[0];
-                os2_tw_each(w, [&](auto qc, const float2 y) {
-                    constexpr int q = decltype(qc)::value;
-                    own[q * PS] = cmul(x[brev(q, 16)], y);
-                });
+#pragma unroll
+                for (int q = 1; q < 16; ++q) own[q * PS] = cmul(x[brev(q, 16)], twp[(q - 1) * 16]);
             }
             os2::bar_group(gid + 1);               // exchange buffer complete; raw rows all read
             if (p + 3 < q1) land(p + 3);           // the next window lands behind the middle stage and the inverse pass
@@ -962,10 +960,8 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
             {
                 float2 x[16];
                 x[0] = own[0];
-                os2_tw_each(w, [&](auto qc, const float2 y) {
-                    constexpr int q = decltype(qc)::value;
-                    x[brev(q, 16)] = cmulc(own[q * PS], y);
-                });
+#pragma unroll
+                for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(own[q * PS], twp[(q - 1) * 16]);
                 idft_dit<16, 1>(x);
                 const int r0 = p * (2 * V) + h - HLO;          // row of sample n = t = h of block A
                 if (a.ng > 0) osv2_source<V, HLO, W>(x, a, nullptr, c, r0, ssh);

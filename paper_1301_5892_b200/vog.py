@@ -17,7 +17,7 @@ SPLIT_XVX, SPLIT_VXV = 0, 1
 
 EXPORTS = ("vog_plan", "vog_destroy", "vog_advect_x", "vog_advect_v", "vog_field", "vog_step",
            "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_run", "vog_run_host",
-           "vog_run_host_async", "vog_launch_count", "vog_strerror", "vog_plan_tune", "vog_reset")
+           "vog_run_host_async", "vog_launch_count", "vog_strerror", "vog_plan_tune", "vog_reset", "vog_diagnostics")
 
 
 class vog_feq_t(ctypes.Structure):
@@ -68,6 +68,7 @@ def lib():
         L.vog_strerror.restype = ctypes.c_char_p
         L.vog_plan_tune.argtypes = [vp, ctypes.c_int, ctypes.c_int]
         L.vog_reset.argtypes = [vp]
+        L.vog_diagnostics.argtypes = [vp, vp, vp]
         for name in EXPORTS:
             if name not in ("vog_launch_count", "vog_strerror"):
                 getattr(L, name).restype = ctypes.c_int
@@ -137,6 +138,9 @@ class Plan:
 
     def step(self, f, dt, E_ext=None):
         self._ck(lib().vog_step(self._h, _ptr(f), float(dt), _ptr(E_ext)), "vog_step")
+
+    def diagnostics(self, f, diag):
+        self._ck(lib().vog_diagnostics(self._h, _ptr(f), _ptr(diag)), "vog_diagnostics")
 
     def get_field(self, E):
         self._ck(lib().vog_get_field(self._h, _ptr(E)), "vog_get_field")

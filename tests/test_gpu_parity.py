@@ -283,6 +283,138 @@ def test_kernel_shape_overrides_keep_parity(torch, vog, oracle, which, value):
         plan.destroy()
 
 
+# ------------------------------------------------------------------ trapezoid field solve and diagnostics
+@pytest.mark.parametrize("idx,over", [(0, {}), (1, {}), (2, dict(Nx=1024, Nv=256)), (1, dict(Nx=16384, Nv=64)), (0, dict(Nx=2048, Nv=128))])
+def test_trapezoid_field_solver_and_diagnostics(torch, vog, oracle, idx, over):
+    """vog_plan_tune(28, 1 | 2): the paper's trapezoidal-rule field solve with and without the zero-mean modifications
+    (P:205-219), and vog_diagnostics, against the oracle's step-by-step versions."""
+    cfg = inputs.config(idx, **over)
+    f = inputs.initial_f(cfg)
+    rho = oracle.density(f, cfg.vmin, cfg.vmax)
+    v = cfg.v()
+    mass0 = float(inputs.gaussians(v, cfg.feq).sum() * cfg.dv) if cfg.feq else 0.0
+    kin0 = float(0.5 * cfg.L * cfg.dv * (v ** 2 * inputs.gaussians(v, cfg.feq)).sum()) if cfg.feq else 0.0
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    dg = torch.zeros(5, device="cuda", dtype=torch.float64)
+    for solver in (0, 1, 2):
+        plan = vog.Plan.from_config(cfg)
+        plan.tune(28, solver)
+        fd = _dev(torch, f)
+        plan.field(fd, Ed)
+        if solver == 0:
+            Eo = oracle.poisson(rho, cfg.L)
+        else:
+            Eo = oracle.field_trapezoid(rho, cfg.L, zero_mean=(solver == 1), background=1.0 - mass0)
+        E = Ed.cpu().numpy().astype(np.float64)
+        assert np.abs(E - Eo).max() <= 2e-6 * np.abs(Eo).max() + 1e-9 * np.abs(f).max()
+        if solver == 1:
+            assert abs(E.mean()) <= 1e-6 * np.abs(Eo).max()
+        plan.diagnostics(fd, dg)
+        d = dg.cpu().numpy()
+        r0, r1 = oracle.rho_modes(rho)
+        kin = oracle.kinetic_energy(f, cfg.L, cfg.vmin, cfg.vmax)
+        ee = oracle.electric_energy(Eo, cfg.L)
+        assert abs(d[0] - ee) <= 1e-5 * ee                          # E is rounded to fp32 before it is squared
+        assert abs(d[1] - (r0 + mass0)) <= 1e-13
+        assert abs(d[2] - r1) <= 1e-13 + 1e-12 * r1
+        assert abs(d[3] - (kin + kin0)) <= 1e-12 * max(abs(kin + kin0), 1.0)
+        assert abs(d[4] - (d[0] + d[3])) <= 1e-15 * max(abs(d[4]), 1.0)
+        # rho^_0 is the mass of the profile the state was built from (1 for the Landau configs: "error of mass"
+        # |rho^_0 - 1| of P:245; 0.9 + 0.2/sqrt(8) for BASELINE.json's bump-on-tail constants), to fp32 storage accuracy
+        mass = sum(a * math.sqrt(math.pi / c) for a, _mu, c in cfg.profile)
+        assert abs(d[1] - mass) < 1e-5
+        # the diagnostics leave the field in the plan
+        Eg = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+        plan.get_field(Eg)
+        assert torch.equal(Eg, Ed)
+        plan.destroy()
+
+
+def test_trapezoid_solver_run_follows_the_fourier_one(torch, vog, oracle):
+    """Config 1 for 50 steps with the trapezoid solve (zero mean): per-step parity against the oracle-composed sequence,
+    and an energy history within (k dx)^2/12 ~ 1e-4 (relative) of the Fourier solver's."""
+    cfg = inputs.config(1)
+    f0 = inputs.initial_f(cfg)
+    feq = oracle.Feq.make(cfg.feq)
+    hist = {}
+    for solver in (0, 1):
+        plan = vog.Plan.from_config(cfg)
+        plan.tune(28, solver)
+        fd = _dev(torch, f0)
+        en = torch.zeros(50, device="cuda", dtype=torch.float64)
+        plan.run(fd, cfg.dt, 50, None, False, en)
+        torch.cuda.synchronize()
+        hist[solver] = en.cpu().numpy()
+        if solver == 1:       # one step against the oracle: x/2, trapezoid field, v, x/2
+            gd = _dev(torch, f0)
+            plan.step(gd, cfg.dt)
+            a = (cfg.L, cfg.vmin, cfg.vmax)
+            h = oracle.advect_x(f0.astype(np.float64), *a, 0.5 * cfg.dt, cfg.kind, cfg.order)
+            E = oracle.field_trapezoid(oracle.density(h, cfg.vmin, cfg.vmax), cfg.L)
+            h = oracle.advect_v(h, E, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq)
+            h = oracle.advect_x(h, *a, 0.5 * cfg.dt, cfg.kind, cfg.order)
+            _check(gd.cpu().numpy(), h, np.abs(f0).max(), tol=3 * TOL)
+        plan.destroy()
+    kdx = 0.5 * cfg.dx
+    rel = np.abs(hist[1] - hist[0]).max() / hist[0].max()
+    assert rel < 4 * kdx ** 2 / 12 + 1e-4, rel
+    assert rel > 1e-6                                   # and it IS another solver
+
+
+# ------------------------------------------------------------------ direct-stencil path (SURVEY 8(f) NEXT-4)
+@pytest.mark.parametrize("kind,order", ALL_KINDS)
+@pytest.mark.parametrize("Nx,Nv", [(1024, 1024), (2048, 1024), (8192, 1024), (1024, 4096), (16384, 1024)])
+def test_stencil_path_shift_parity(torch, vog, oracle, Nx, Nv, kind, order):
+    """vog_plan_tune(27, 1): the circulant product taken directly (eq (4)) instead of in Fourier space; the
+    same matrix, the same oracle, the same 2e-6.  x in place with shifts of thousands of cells (the landed barrier),
+    v with shift spreads below and above the row buffer's 32; several line groups per CTA."""
+    if Nx * Nv > (1 << 22) and (kind, order) not in ((LAG, 17), (SPL, 3), (LAG, 3)):
+        pytest.skip("large shapes: three interpolators only")
+    f = inputs.uniform_grid(Nx, Nv, seed=inputs.SEED + 201)
+    plan = vog.Plan(Nx, Nv, 4 * math.pi, -6.0, 6.0, kind, order)
+    plan.tune(27, 1)
+    bx = inputs.uniform_shifts(Nv, inputs.SEED + 202, lo=-3000.0, hi=3000.0)
+    bx[:8] = [0.0, 3.0, -5.0, -0.25, 0.999999, 1e-9, 123456.75, -98765.5]
+    fd = _dev(torch, f)
+    plan.shift_x(fd, _dev(torch, bx))
+    _check(fd.cpu().numpy(), oracle.shift_x(f, bx, kind, order), 1.0)
+    for lo, hi in ((-8.0, 8.0), (-40.0, 25.0)):
+        bv = inputs.uniform_shifts(Nx, inputs.SEED + 203, lo=lo, hi=hi)
+        bv[:6] = [0.0, 3.0, -5.0, -0.25, 0.999999, 7.5]
+        fd = _dev(torch, f)
+        plan.shift_v(fd, _dev(torch, bv))
+        _check(fd.cpu().numpy(), oracle.shift_v(f, bv, kind, order), 1.0)
+    plan.destroy()
+
+
+@pytest.mark.parametrize("split", [0, 1])
+@pytest.mark.parametrize("idx,over", [(1, dict(Nx=1024, Nv=1024)), (2, dict(Nx=1024, Nv=2048)), (3, dict(Nx=2048, Nv=1024)),
+                                      (1, dict(Nx=1024, Nv=1024, kind=SPL, order=3))])
+def test_stencil_path_step_parity(torch, vog, oracle, idx, over, split):
+    """Two Strang steps through the direct-stencil kernels (delta-f source included), both split orders."""
+    cfg = inputs.config(idx, split=split, **over)
+    f = inputs.initial_f(cfg)
+    if np.abs(f).max() == 0:
+        f = 1e-3 * inputs.smooth_grid(cfg.Nx, cfg.Nv)
+    plan = vog.Plan.from_config(cfg)
+    plan.tune(27, 1)
+    feq = oracle.Feq.make(cfg.feq)
+    ext = (0.02 * np.sin(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx)).astype(np.float32)
+    fd = _dev(torch, f)
+    for _ in range(2):
+        plan.step(fd, cfg.dt, _dev(torch, ext))
+    Ed = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+    plan.get_field(Ed)
+    fo = f.astype(np.float64)
+    Eo = None
+    for _ in range(2):
+        fo, Eo = oracle.step(fo, cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order, feq, split, ext, Eo)
+    scale = max(np.abs(f).max(), _v_scale(oracle, cfg, f, Eo + ext, cfg.dt))
+    _check(fd.cpu().numpy(), fo, scale, tol=3 * TOL * 2)
+    assert np.abs(Ed.cpu().numpy() - Eo).max() <= 1e-4 * np.abs(Eo).max()
+    plan.destroy()
+
+
 @pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("lo,hi", [(-4.0, 4.0), (-8.0, 8.0), (-20.0, 12.0), (-900.0, 900.0)])
 def test_v_coalesced_landing_any_shift_spread(torch, vog, oracle, lo, hi, variant):

@@ -483,3 +483,60 @@ def test_keen_drive_sign_and_phase(oracle):
     dt = 4 * cfg.dv / float(e[i])                               # four cells at the maximum
     out, _ = oracle.step(f, cfg.L, cfg.vmin, cfg.vmax, dt, LAG, 17, None, inputs.SPLIT_VXV, e, np.zeros(256))
     assert np.argmax(out[:, i]) == np.argmax(prof) + 4
+
+
+# ---------------------------------------------------------------- NEXT-3: trapezoid field solve and diagnostics
+def test_trapezoid_field_on_a_mode_has_the_closed_form_factor(oracle):
+    """rho = 1 + a cos(kx): summing the trapezoid rule in closed form gives E = a sin(kx)/k * (k dx/2)/tan(k dx/2),
+    i.e. the Fourier solve's answer times 1 - (k dx)^2/12 + O((k dx)^4), and the zero-mean
+    modifications leave exactly that."""
+    L = 4 * math.pi
+    for Nx, m in ((32, 1), (64, 3), (256, 5)):
+        dx = L / Nx
+        x = np.arange(Nx) * dx
+        k = 2 * math.pi * m / L
+        E = oracle.field_trapezoid(1.0 + 0.3 * np.cos(k * x), L)
+        fac = (k * dx / 2) / math.tan(k * dx / 2)
+        assert np.abs(E - 0.3 * fac * np.sin(k * x) / k).max() < 1e-13
+        assert abs(E.mean()) < 1e-15
+        assert abs(fac - (1 - (k * dx) ** 2 / 12)) < (k * dx) ** 4 / 100
+        Ef = oracle.poisson(1.0 + 0.3 * np.cos(k * x), L)
+        assert abs(np.abs(E).max() / np.abs(Ef).max() - fac) < 1e-12
+
+
+def test_trapezoid_field_without_zero_mean_keeps_the_systematic_error(oracle):
+    """without the modification rho~ = rho - 1; a density whose mean is 1 + eps (the rounding drift the
+    paper talks about) then leaves a ramp eps x in E, which the zero-mean version removes."""
+    Nx, L, eps = 128, 4 * math.pi, 1e-4
+    x = np.arange(Nx) * L / Nx
+    rho = 1.0 + eps + 0.01 * np.cos(0.5 * x)
+    E0 = oracle.field_trapezoid(rho, L, zero_mean=False, background=1.0)
+    E1 = oracle.field_trapezoid(rho, L, zero_mean=True)
+    ramp = E0 - oracle.field_trapezoid(rho - eps, L, zero_mean=False, background=1.0)
+    assert np.abs(ramp - eps * x).max() < 1e-13
+    assert abs(E1.mean()) < 1e-16
+    assert np.abs(E1 - oracle.field_trapezoid(rho - eps, L, zero_mean=True)).max() < 1e-13   # the mean plays no role
+    # Poisson's equation holds cell by cell for the trapezoid rule: (E_{k+1} - E_k)/dx = mean of rho~ over the cell
+    d = np.diff(E1) / (L / Nx)
+    rt = rho - rho.mean()
+    assert np.abs(d - 0.5 * (rt[:-1] + rt[1:])).max() < 1e-13
+
+
+def test_rho_modes_and_kinetic_energy_closed_forms(oracle):
+    """rho^_0 and |rho^_1| against numpy.fft; the kinetic energy of a Maxwellian is L/2 (second moment 1),
+    the rectangle rule being spectrally accurate for a Gaussian."""
+    rng = np.random.default_rng(3)
+    rho = 1.0 + 0.1 * rng.normal(size=96)
+    r0, r1 = oracle.rho_modes(rho)
+    F = np.fft.fft(rho) / rho.size
+    assert abs(r0 - F[0].real) < 1e-15 and abs(r1 - abs(F[1])) < 1e-15
+    assert abs(oracle.rho_modes(1.0 + 0.25 * np.cos(2 * math.pi * np.arange(64) / 64 + 0.7))[1] - 0.125) < 1e-15
+    cfg = inputs.config(0, Nx=32, Nv=256, vmin=-8.0, vmax=8.0)
+    f = np.tile((np.exp(-cfg.v() ** 2 / 2) / math.sqrt(2 * math.pi))[:, None], (1, 32))
+    assert abs(oracle.kinetic_energy(f, cfg.L, cfg.vmin, cfg.vmax) - 0.5 * cfg.L) < 1e-12
+    # weights: doubling one row's value adds (1/2) dx dv v_j^2 * (row sum)
+    g = f.copy()
+    g[40] *= 2
+    dx, dv = cfg.L / 32, 16.0 / 256
+    assert abs(oracle.kinetic_energy(g, cfg.L, -8, 8) - oracle.kinetic_energy(f, cfg.L, -8, 8)
+               - 0.5 * dx * dv * cfg.v()[40] ** 2 * f[40].sum()) < 1e-15
