@@ -142,7 +142,7 @@ cudaError_t osx7_launch(const OsArgs& a, int geom, int grid, int threads, size_t
 int osx7_occupancy(int geom, int threads, size_t smem);
 cudaError_t osx6_launch(const OsArgs& a, int geom, int grid, int threads, size_t smem, cudaStream_t st);
 int osx6_occupancy(int geom, int threads, size_t smem);
-cudaError_t osv7_launch(const OsArgs& a, int geom, int n_sm, cudaStream_t st);
+cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_sm, cudaStream_t st);
 cudaError_t osv6_launch(const OsArgs& a, int geom, dim3 grid, cudaStream_t st);
 cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st);
 

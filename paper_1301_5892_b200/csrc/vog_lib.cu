@@ -408,13 +408,19 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     pdl_wait();                                   // the slab sums come from the density kernel
     pdl_launch_dependents();
     // rho_i = dv * (sum of the slab sums, in slab order); rho_0 is the reference value
-    double ref = 0.0;
-    for (int y = 0; y < nby; ++y) ref += __ldcg(part + (size_t)y * Nx);
-    ref *= dv;
+    // (all <= 16 slab values of a cell are requested before the first is used: one L2 latency per cell, not nby)
+    auto slab_sum = [&](const int i) {
+        double v[16];
+#pragma unroll
+        for (int y = 0; y < 16; ++y) v[y] = y < nby ? __ldcg(part + (size_t)y * Nx + i) : 0.0;
+        double s = v[0];
+#pragma unroll
+        for (int y = 1; y < 16; ++y) s += v[y];        // (slabs beyond nby add +0.0: the sum is the ordered sum)
+        return s * dv;
+    };
+    const double ref = slab_sum(0);
     for (int i = tid; i < Nx; i += T) {
-        double s = 0.0;
-        for (int y = 0; y < nby; ++y) s += __ldcg(part + (size_t)y * Nx + i);
-        s *= dv;
+        const double s = slab_sum(i);
         rho[i] = s;
         z[i] = make_float2((float)(s - ref), 0.0f);
     }
@@ -491,6 +497,7 @@ struct vog_plan_s {
     vog::PoissonRadix prx;
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int os2x_lpi, os3x_occ, os2v_gpc;      // x: lines per iteration, cached occupancy; v: pairs per CTA (0 = default)
+    vog::OsSetupArgs vsetup;               // v-advection: shift source (E, E_ext, beta, dt) of the pending advection
     int solver;                            // field solve: 0 = Fourier (default), 1 = trapezoid + zero mean, 2 = trapezoid, rho - 1
     double feq_mass, feq_kin;              // dv sum_j f_eq(v_j) and (1/2) L dv sum_j v_j^2 f_eq(v_j) (0 in full-f mode)
     double *partk, *diag;                  // kinetic-energy slab sums [nby_max][Nx]; 5 doubles of scratch
@@ -702,6 +709,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         const int Vx = p->kind == VOG_LAGRANGE ? OS_VL : OS_V;
         const int npx = ((Nx + Vx - 1) / Vx + 1) / 2;
         int l2 = 288 / (16 * npx);
+        if (l2 > 2) l2 = 2;                          // measured (2048, 4096 cells): 2 lines per group, then 1, then 3
         if (l2 < 1) l2 = 1;
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
@@ -920,6 +928,11 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
         s.cs64 = P->os_cs64;
         s.lam = vdir ? P->os_lam_v : P->os_lam_x;
         if (P->method == 1) return st_setup_launch(s, vdir ? P->taps_v : P->taps_x, P->st);
+        if (vdir && P->osv_variant == 0) {         // the default v kernel computes its strips' tables itself (S1 fused)
+            P->vsetup = s;
+            P->launches--;
+            return cudaSuccess;
+        }
         return os_setup_launch(s, P->st);
     }
     SetupArgs s;
@@ -1030,7 +1043,7 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
         int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : (a.np >= 18 ? 9 : (a.np >= 6 ? 3 : a.np));
         if (gpc > a.np) gpc = a.np;
         a.gpc = gpc;
-        return osv7_launch(a, geom, P->n_sm, P->st);
+        return osv7_launch(a, P->vsetup, geom, P->n_sm, P->st);
     }
     if (P->osv_variant == 2) {
         // 16-column strips, one group per CTA, symbol through L1
@@ -1156,7 +1169,7 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
     P->E_of = f;
     int Ta = Nx < 1024 ? Nx : 1024;
     if (P->solver == 0) {
-        int T = Nx / 4;
+        int T = Nx / 2;                            // (the radix passes keep Nx / 4 or Nx / 8 threads busy, the loads all)
         if (T > 1024) T = 1024;
         if (T < 32) T = 32;
         const int tw_in_smem = Nx <= 8192;

@@ -268,19 +268,20 @@ int osx6_occupancy(int geom, int threads, size_t smem)
 }
 
 // three-group v kernel (default): one persistent CTA of 768 threads per SM; a.gpc = pairs per work item
-cudaError_t osv7_launch(const OsArgs& a, int geom, int n_sm, cudaStream_t st)
+cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_sm, cudaStream_t st)
 {
-    const size_t smem = (size_t)OS_LAMW * os2::VW * 8 + 240 * 8 + 3 * ((size_t)os2::VRR * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8);
+    const size_t smem = (size_t)OS_LAMW * os2::VW * 8 + 240 * 8 + 20 * os2::VW * 4 +
+                        3 * ((size_t)os2::VRR * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8);
     const int n_items = (a.Nx / os2::VW) * ((a.np + a.gpc - 1) / a.gpc);
     const int grid = n_items < n_sm ? n_items : n_sm;
     if (geom) {
         cudaError_t e = set_max_smem((const void*)osv7_kernel<OS_VL, OS_HL>, smem);
         if (e != cudaSuccess) return e;
-        return launch_pdl(osv7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(768), smem, st, a);
+        return launch_pdl(osv7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(768), smem, st, a, su);
     }
     cudaError_t e = set_max_smem((const void*)osv7_kernel<OS_V, OS_H>, smem);
     if (e != cudaSuccess) return e;
-    return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a);
+    return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a, su);
 }
 
 // 16-column-strip v kernel, symbol through L1; grid = (Nx / 16, ceil(np / gpc))

@@ -856,7 +856,7 @@ __device__ __forceinline__ void bar_group(const int id) { asm volatile("bar.sync
 }
 
 template <int V, int HLO>
-__global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
+__global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSetupArgs su)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int W = os2::VW, RR = os2::VRR;
@@ -864,8 +864,11 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
     constexpr int GB = RR * W * 4 + OS_LB * W * 8; // bytes per group: raw rows + exchange buffer
     float2* const lamS = reinterpret_cast<float2*>(smem_raw);                     // [OS_LAMW][16]
     float2* const twS = lamS + OS_LAMW * W;                                       // [15][16] e^{-2 pi i t q / 256}
+    float* const afS = reinterpret_cast<float*>(twS + 240);                       // [18][16] symbol coefficients per column
+    int* const bS = reinterpret_cast<int*>(afS + 18 * W);                         // [16] integer shifts
+    float* const sS = reinterpret_cast<float*>(bS + W);                           // [16] source shifts E dt
     const int tid = threadIdx.x, gid = tid >> 8, gt = tid & 255;                  // group, thread of the group
-    unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + 240 * 8 + gid * GB;
+    unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + 240 * 8 + 20 * W * 4 + gid * GB;
     float* const raw = reinterpret_cast<float*>(gbase);                           // [RR][16]
     float2* const exch = reinterpret_cast<float2*>(raw + RR * W);                 // [256][16]
     const int c = gt & 15, h = gt >> 4;                                           // column of the strip, item index
@@ -879,23 +882,92 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a)
     pdl_launch_dependents();
     float2* const own = exch + h * W + c;                                     // position t = h
     constexpr int PS = 16 * W;                                                // float2 between positions 16 apart
-    const size_t ks = (size_t)a.lam_ks;
 
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
         const int strip = item % nstrips, seg = item / nstrips;              // (neighbouring CTAs: neighbouring strips)
         const int c0 = strip * W;
         const int q0 = seg * a.gpc, q1 = min(a.np, q0 + a.gpc);              // pairs of the segment
         __syncthreads();                           // every group is done with the table of the previous item
-        {   // symbol table of the strip: OS_LAMW rows of 128 B
-            const float4* src4 = reinterpret_cast<const float4*>(a.lam + c0);
-            float4* dst4 = reinterpret_cast<float4*>(lamS);
-            for (int i = tid; i < OS_LAMW * 8; i += 768)
-                os2::cp_async16(dst4 + i, src4 + (size_t)(i >> 3) * (ks / 2) + (i & 7));
+        // S1 inside the kernel: the symbol table of the strip is COMPUTED here (no set-up kernel between the field
+        // solve and this one).  Same arithmetic, entry for entry, as os_setup_v_kernel: beta, b, b* and the Everett /
+        // B-spline coefficients in fp64 per column (32 threads: column x half), the 130 entries by fp32 Horner.
+        if (tid < 2 * W) {
+            const int half = tid >> 4, cc = tid & 15, l = c0 + cc;
+            double beta;
+            float sshift = 0.0f;
+            if (su.mode == 1) {
+                double e = (double)su.E[l];
+                if (su.Eext) e += (double)su.Eext[l];
+                beta = -e * su.dt / su.delta;
+                sshift = (float)(su.dt * e);
+            } else {
+                beta = su.beta[l];
+            }
+            const double fl = floor(beta);
+            const double tt0 = beta - fl;
+            int bb;
+            if (fabs(fl) < 9.0e18) {
+                bb = (int)(__double2ll_rn(fl) & (long long)(su.N - 1));
+            } else {
+                double bm = fmod(fl, (double)su.N);
+                if (bm < 0.0) bm += (double)su.N;
+                bb = (int)bm;
+                if (bb >= su.N) bb = 0;
+            }
+            if (half == 0) { bS[cc] = bb; sS[cc] = sshift; }
+            if (!su.spline) {
+                const double tt = half == 0 ? 1.0 - tt0 : tt0;
+                double av = tt;
+                constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
+                                           1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
+                afS[(half * 9) * W + cc] = (float)av;
+#pragma unroll
+                for (int m = 1; m <= 8; ++m) {
+                    av = av * ((double)(m * m) - tt * tt) * rcp[m];
+                    afS[(half * 9 + m) * W + cc] = m <= su.d ? (float)av : 0.0f;
+                }
+            } else if (half == 0) {
+                const double t = tt0, u = 1.0 - t;
+                afS[0 * W + cc] = (float)(u * u * u / 6.0);
+                afS[1 * W + cc] = (float)((4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0);
+                afS[2 * W + cc] = (float)((1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0);
+                afS[3 * W + cc] = (float)(t * t * t / 6.0);
+            }
+        }
+        __syncthreads();
+        for (int idx = tid; idx < OS_LAMW * W; idx += 768) {
+            const int kk = idx >> 4, cc = idx & 15;
+            float2 o;
+            if (kk == 129) o = make_float2(__int_as_float(bS[cc]), sS[cc]);
+            else if (kk == 0) o = make_float2(1.0f / (float)OS_LB, 0.0f);          // lambda_0 = sum of the weights = 1
+            else {
+                const double2 cs = su.cs64[kk];
+                const float cf = (float)cs.x, sn = (float)cs.y;
+                float lr, li;
+                if (su.spline) {
+                    const float Bm1 = afS[cc], B0 = afS[W + cc], B1 = afS[2 * W + cc], B2 = afS[3 * W + cc];
+                    const float c2 = (float)(2.0 * cs.x * cs.x - 1.0), s2 = (float)(2.0 * cs.y * cs.x);
+                    const float gg = 3.0f / (2.0f + cf);
+                    lr = fmaf(B2, c2, fmaf(Bm1 + B1, cf, B0)) * gg;
+                    li = fmaf(B2, s2, (B1 - Bm1) * sn) * gg;
+                } else {
+                    const float sv = (float)(2.0 - 2.0 * cs.x);
+                    float q0 = 0.0f, q1 = 0.0f;
+#pragma unroll
+                    for (int j = 8; j >= 0; --j) {
+                        q0 = fmaf(q0, sv, afS[j * W + cc]);
+                        q1 = fmaf(q1, sv, afS[(9 + j) * W + cc]);
+                    }
+                    lr = fmaf(cf, q1, q0);
+                    li = sn * q1;
+                }
+                o = make_float2(lr * (1.0f / (float)OS_LB), li * (1.0f / (float)OS_LB));
+            }
+            lamS[idx] = o;
         }
         // integer shift (rows) and source shift of this lane's column
-        const float2 e129 = __ldg(a.lam + 129 * ks + c0 + c);
-        const int b = __float_as_int(e129.x);
-        const float ssh = e129.y;
+        const int b = bS[c];
+        const float ssh = sS[c];
         // spread of the shifts over the strip, as signed distances from column 0's (shifts live mod Nv)
         const int b0 = __shfl_sync(0xffffffffu, b, 0, 16);
         const int d = (((b - b0) + (Nv >> 1)) & vmask) - (Nv >> 1);
