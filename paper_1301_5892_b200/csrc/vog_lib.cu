@@ -14,6 +14,14 @@
 
 namespace vog {
 
+// (working builds only, -DVOG_STAMPS: globaltimer stamps of the field kernels' phases)
+#ifdef VOG_STAMPS
+__device__ long long vog_stamps[32];
+#define VOG_STAMP(i) do { if (threadIdx.x == 0) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); vog_stamps[i] = t_; } } while (0)
+#else
+#define VOG_STAMP(i) do { } while (0)
+#endif
+
 // Programmatic dependent launch is a per-plan choice (vog_plan_tune(26, .)); the entry points of the C ABI set it
 // for the calling thread before they launch anything.
 static thread_local bool t_pdl = true;
@@ -200,6 +208,9 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
     const int j0 = blockIdx.y * rows_per_block;
     pdl_wait();                                   // f comes from the advection before; part may still be read
     pdl_launch_dependents();
+#ifdef VOG_STAMPS
+    if (blockIdx.x == 0 && blockIdx.y == 0) VOG_STAMP(8);
+#endif
     double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
     double k0 = 0, k1 = 0, k2 = 0, k3 = 0;
     const float* p = f + (size_t)(j0 + warp * 4 + rl) * Nx + col;
@@ -241,6 +252,9 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
         part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
         if constexpr (KIN) partk[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = k;
     }
+#ifdef VOG_STAMPS
+    if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) VOG_STAMP(9);
+#endif
 }
 
 // ------------------------------------------------------------------------------------------
@@ -355,36 +369,122 @@ struct PoissonRadix { int np; int lr[8]; int off[8]; };   // log2 radix and twid
 
 // One pass over sub-blocks of length B = 1 << lB, radix R, stride S = B / R.  tw = the pass's compact table
 // [(q-1) S + t] = e^{-2 pi i t q / B}: lanes read consecutive entries (no bank conflicts).
-template <int R, bool INV>
-__device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int Nx, const int lB,
-                                             const float2* __restrict__ tw, const int tid, const int T)
+// Twiddles are read with explicit shared-memory loads when TWS (the table is staged in shared memory for Nx <= 8192): a
+// generic pointer that may be shared or global compiles to generic loads, ~4x the latency, and they sat in the
+// dependency chain of every pass (measured: 0.42 us per pass of 512 butterflies).  All loads of a butterfly are
+// issued before its first store.
+template <bool TWS>
+__device__ __forceinline__ float2 poisson_tw(const float2* tw, const int i)
 {
+    if constexpr (TWS) {
+        float2 v;
+        const unsigned a = (unsigned)__cvta_generic_to_shared(tw + i);
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];\n" : "=f"(v.x), "=f"(v.y) : "r"(a));
+        return v;
+    } else {
+        return __ldg(tw + i);
+    }
+}
+
+template <int R, bool INV, bool TWS>
+__device__ __forceinline__ void poisson_pass(float2* __restrict__ z, const int Nx, const int lB,
+                                             const float2* __restrict__ tw, const int tid, const int T,
+                                             const float* __restrict__ iks)
+{
+    // (positions are padded by one float2 per 16, padp(): the last forward / first inverse pass has a stride of R
+    // positions between neighbouring threads, which would put a warp on few bank pairs)
     constexpr int LR = ilog2(R);
     const int lS = lB - LR, S = 1 << lS;
+#pragma unroll 1
     for (int g = tid; g < (Nx >> LR); g += T) {
         const int t = g & (S - 1), base = ((g >> lS) << lB) + t;
-        float2 x[R];
+        float2 x[R], w[R];
+#pragma unroll
+        for (int q = 1; q < R; ++q) w[q] = poisson_tw<TWS>(tw, ((q - 1) << lS) + t);
         if constexpr (!INV) {
 #pragma unroll
-            for (int k = 0; k < R; ++k) x[k] = z[base + (k << lS)];
+            for (int k = 0; k < R; ++k) x[k] = z[padp(base + (k << lS))];
             dft_dif<R, 1>(x);
-            z[base] = x[0];
+            z[padp(base)] = x[0];
 #pragma unroll
-            for (int q = 1; q < R; ++q) z[base + (q << lS)] = cmul(x[brev(q, R)], tw[((q - 1) << lS) + t]);
+            for (int q = 1; q < R; ++q) z[padp(base + (q << lS))] = cmul(x[brev(q, R)], w[q]);
         } else {
-            x[0] = z[base];
+            // iks != NULL (first inverse pass): the spectrum is divided by i k on the way in, (zr + i zi) / (i k) / Nx
+            float2 v[R];
 #pragma unroll
-            for (int q = 1; q < R; ++q) x[brev(q, R)] = cmulc(z[base + (q << lS)], tw[((q - 1) << lS) + t]);
+            for (int q = 0; q < R; ++q) v[q] = z[padp(base + (q << lS))];
+            if (iks) {
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const float ik = iks[base + (q << lS)];
+                    v[q] = make_float2(v[q].y * ik, -v[q].x * ik);
+                }
+            }
+            x[0] = v[0];
+#pragma unroll
+            for (int q = 1; q < R; ++q) x[brev(q, R)] = cmulc(v[q], w[q]);
             idft_dit<R, 1>(x);
 #pragma unroll
-            for (int k = 0; k < R; ++k) z[base + (k << lS)] = x[k];
+            for (int k = 0; k < R; ++k) z[padp(base + (k << lS))] = x[k];
         }
     }
 }
 
-// S9: single-CTA Poisson solve.  rho (fp64, from the density kernel) minus a reference value in fp64
-// (zero mean, = mode 0 dropped); radix-4 (one radix-8 pass for odd log2 Nx) DIF FFT in shared memory (fp32) with all threads
-// busy in every pass; E^_m = rho^_m / (i k_m) with modes 0 and Nx/2 dropped; DIT inverse; E to E_a (and E_b).
+// forward passes, then the inverse passes in reverse order (the first inverse pass divides by i k); ONE radix-4 body
+// per direction in a run-time loop, plus one radix-2 pass when log2 Nx is odd.  Twiddle tables follow one another in
+// pass order: radix R at block size B takes (R - 1) B / R entries.
+template <bool INV, bool TWS>
+__device__ __forceinline__ void poisson_pass_r(const int lr, float2* __restrict__ z, const int Nx, const int lB,
+                                               const float2* __restrict__ tw, const int tid, const int T,
+                                               const float* __restrict__ iks)
+{
+    if (lr == 1) poisson_pass<2, INV, TWS>(z, Nx, lB, tw, tid, T, iks);
+    else if (lr == 2) poisson_pass<4, INV, TWS>(z, Nx, lB, tw, tid, T, iks);
+    else poisson_pass<8, INV, TWS>(z, Nx, lB, tw, tid, T, iks);
+}
+
+// forward passes, then the inverse passes in reverse order (the first inverse pass divides by i k).  Radix 2^LR passes
+// in a run-time loop (one body per direction), preceded by one pass of radix 2^(log2 Nx mod LR) when LR does not divide
+// log2 Nx.  Twiddle tables follow one another in pass order: radix R at block size B takes (R - 1) B / R entries.
+template <bool TWS, int LR>
+__device__ __forceinline__ void poisson_fft(float2* __restrict__ z, const int Nx, const float2* __restrict__ tws,
+                                            const float* __restrict__ iks, const int tid, const int T)
+{
+    constexpr int R = 1 << LR;
+    const int lg = ilog2(Nx), rem = lg % LR;
+    int lB = lg;
+    const float2* tw = tws;
+    if (rem) {
+        poisson_pass_r<false, TWS>(rem, z, Nx, lB, tw, tid, T, nullptr);
+        tw += ((1 << rem) - 1) << (lB - rem);
+        lB -= rem;
+        __syncthreads();
+    }
+#pragma unroll 1
+    for (; lB > 0; lB -= LR) {
+        poisson_pass<R, false, TWS>(z, Nx, lB, tw, tid, T, nullptr);
+        tw += (R - 1) << (lB - LR);
+        __syncthreads();
+    }
+    VOG_STAMP(4);
+#pragma unroll 1
+    for (lB = LR; lB <= lg - rem; lB += LR) {
+        tw -= (R - 1) << (lB - LR);
+        poisson_pass<R, true, TWS>(z, Nx, lB, tw, tid, T, lB == LR ? iks : nullptr);
+        __syncthreads();
+    }
+    if (rem) {
+        poisson_pass_r<true, TWS>(rem, z, Nx, lg, tws, tid, T, nullptr);
+        __syncthreads();
+    }
+}
+
+// S9: single-CTA Poisson solve.  rho (fp64, the density kernel's slab sums added in slab order) minus a
+// reference value in fp64 (zero mean, = mode 0 dropped); DIF FFT in shared memory (fp32) in at most four
+// register-resident passes -- radix 16, preceded by one radix 2, 4 or 8 pass when log2 Nx is not a multiple of 4:
+// 2048 = 8 x 16 x 16 (a single SM runs this kernel, so its time is the number of barrier-separated passes: three
+// fat ones instead of the five thin radix-4 ones of round 1); E^_m = rho^_m / (i k_m) with modes 0 and Nx/2
+// dropped, applied while the first inverse pass loads; DIT inverse; E to E_a (and E_b).
 __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadix rx, int tw_len, int tw_in_smem,
                                                        const float2* __restrict__ tw_g, const float* __restrict__ ikt,
                                                        const double* __restrict__ part, int nby, double dv,
@@ -395,68 +495,57 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     __shared__ double ered[32];
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* z = reinterpret_cast<float2*>(smem_raw);
-    float* iks = reinterpret_cast<float*>(z + Nx);      // 1/(i k) factors
+    float* iks = reinterpret_cast<float*>(z + padded_len(Nx));      // 1/(i k) factors
     float2* twsm = reinterpret_cast<float2*>(iks + Nx); // compact twiddle tables of all passes (if they fit)
-    const float2* __restrict__ tws = tw_in_smem ? twsm : tw_g;
     const int tid = threadIdx.x, T = blockDim.x;
     // Zero mean = mode 0 dropped below.  Before the conversion to fp32 a constant of the size of
     // the mean must still be removed in fp64 (in full-f mode rho ~ 1 carries a 1e-3 perturbation): rho[0]
     // serves as well as the mean (any constant only changes mode 0) and needs no reduction.
+    VOG_STAMP(0);
     for (int i = tid; i < Nx; i += T) iks[i] = __ldg(ikt + i);               // (plan constants: before the wait)
     if (tw_in_smem)
         for (int i = tid; i < tw_len; i += T) twsm[i] = __ldg(tw_g + i);
     pdl_wait();                                   // the slab sums come from the density kernel
     pdl_launch_dependents();
     // rho_i = dv * (sum of the slab sums, in slab order); rho_0 is the reference value
-    // (all <= 16 slab values of a cell are requested before the first is used: one L2 latency per cell, not nby)
-    auto slab_sum = [&](const int i) {
-        double v[16];
+    // rho_i = dv * (sum of the slab sums in a fixed order: slabs 0..7, then slabs 8..15, then the two halves).  The eight
+    // values of a half are requested before the first is used, and the reference cell 0 travels with the thread's
+    // first cell: one L2 round trip for the first 1024 cells, one more per further 1024.
+    auto slab8 = [&](const int i, const int y0) {
+        double v[8];
 #pragma unroll
-        for (int y = 0; y < 16; ++y) v[y] = y < nby ? __ldcg(part + (size_t)y * Nx + i) : 0.0;
+        for (int y = 0; y < 8; ++y) v[y] = y0 + y < nby ? __ldcg(part + (size_t)(y0 + y) * Nx + i) : 0.0;
         double s = v[0];
 #pragma unroll
-        for (int y = 1; y < 16; ++y) s += v[y];        // (slabs beyond nby add +0.0: the sum is the ordered sum)
-        return s * dv;
+        for (int y = 1; y < 8; ++y) s += v[y];
+        return s;
     };
-    const double ref = slab_sum(0);
-    for (int i = tid; i < Nx; i += T) {
-        const double s = slab_sum(i);
-        rho[i] = s;
-        z[i] = make_float2((float)(s - ref), 0.0f);
+    const double ref0 = slab8(0, 0);
+    double s_first = slab8(tid, 0);                // (T <= Nx)
+    double ref = ref0;
+    if (nby > 8) { ref += slab8(0, 8); s_first += slab8(tid, 8); }
+    ref *= dv;
+    s_first *= dv;
+    rho[tid] = s_first;
+    z[padp(tid)] = make_float2((float)(s_first - ref), 0.0f);
+#pragma unroll 1
+    for (int i = tid + T; i < Nx; i += T) {
+        double sv = slab8(i, 0);
+        if (nby > 8) sv += slab8(i, 8);
+        sv *= dv;
+        rho[i] = sv;
+        z[padp(i)] = make_float2((float)(sv - ref), 0.0f);
     }
     __syncthreads();
+    VOG_STAMP(3);
     // forward, decimation in frequency: position ((q0 r1 + q1) r2 + q2).. holds mode q0 + r0 (q1 + r1 (q2 + ..));
     // ikt[pos] = L / (2 pi m Nx) for that mode (0 for modes 0 and Nx/2)
-    int lB = ilog2(Nx);
-    // (the pass loops are unrolled so that rx.lr[p], rx.off[p] are read from the parameter bank; a run-time index
-    // made the compiler copy the struct to local memory: two dependent local loads at the head of every pass)
-#pragma unroll
-    for (int p = 0; p < 8; ++p) {
-        if (p < rx.np) {
-            if (rx.lr[p] == 3) poisson_pass<8, false>(z, Nx, lB, tws + rx.off[p], tid, T);
-            else poisson_pass<4, false>(z, Nx, lB, tws + rx.off[p], tid, T);
-            lB -= rx.lr[p];
-            __syncthreads();
-        }
-    }
-    for (int pos = tid; pos < Nx; pos += T) {
-        const float2 v = z[pos];
-        const float ik = iks[pos];
-        z[pos] = make_float2(v.y * ik, -v.x * ik);         // (zr + i zi) / (i k), times 1/Nx
-    }
-    __syncthreads();
-#pragma unroll
-    for (int p = 7; p >= 0; --p) {
-        if (p < rx.np) {
-            lB += rx.lr[p];
-            if (rx.lr[p] == 3) poisson_pass<8, true>(z, Nx, lB, tws + rx.off[p], tid, T);
-            else poisson_pass<4, true>(z, Nx, lB, tws + rx.off[p], tid, T);
-            __syncthreads();
-        }
-    }
+    if (tw_in_smem) poisson_fft<true, 3>(z, Nx, twsm, iks, tid, T);
+    else poisson_fft<false, 3>(z, Nx, tw_g, iks, tid, T);
+    VOG_STAMP(5);
     double e2 = 0.0;
     for (int i = tid; i < Nx; i += T) {
-        const float e = z[i].x;
+        const float e = z[padp(i)].x;
         E_a[i] = e;
         if (E_b) E_b[i] = e;
         e2 += (double)e * (double)e;
@@ -472,6 +561,7 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
             energy_out[0] = half_dx * s;
         }
     }
+    VOG_STAMP(6);
 }
 
 }  // namespace vog
@@ -747,8 +837,12 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         int lg = ilog2i(Nx);
         P->prx.np = 0;
         for (int i = 0; i < 8; ++i) { P->prx.lr[i] = 0; P->prx.off[i] = 0; }
-        if (lg & 1) { P->prx.lr[P->prx.np++] = 3; lg -= 3; }
-        while (lg > 0) { P->prx.lr[P->prx.np++] = 2; lg -= 2; }
+        // radix 8, preceded by one radix 2 or 4 pass (measured at 2048 with the phases of the kernel time-stamped:
+        // radix 4, 8 and 16 plans are within the run-to-run noise of one another once the twiddles are explicit
+        // shared-memory loads; radix 8 with Nx / 4 threads was the best by a little)
+        const int mr = 3;
+        if (lg % mr) { P->prx.lr[P->prx.np++] = lg % mr; lg -= lg % mr; }      // the odd radix first
+        while (lg > 0) { P->prx.lr[P->prx.np++] = mr; lg -= mr; }
         int Bp = Nx;
         for (int q = 0; q < P->prx.np; ++q) {             // compact twiddles [(j-1) S + t] = e^{-2 pi i t j / B}
             const int R = 1 << P->prx.lr[q], S = Bp / R;
@@ -1169,11 +1263,11 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
     P->E_of = f;
     int Ta = Nx < 1024 ? Nx : 1024;
     if (P->solver == 0) {
-        int T = Nx / 2;                            // (the radix passes keep Nx / 4 or Nx / 8 threads busy, the loads all)
+        int T = Nx / 4;                            // (radix-8 passes keep Nx / 8 threads busy, the loads and stores all)
         if (T > 1024) T = 1024;
         if (T < 32) T = 32;
         const int tw_in_smem = Nx <= 8192;
-        const size_t psmem = (sizeof(float2) + sizeof(float)) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
+        const size_t psmem = sizeof(float2) * (Nx + Nx / 16) + sizeof(float) * Nx + (tw_in_smem ? sizeof(float2) * P->ptw_len : 0);
         e = set_max_smem((const void*)poisson_kernel, psmem);
         if (e != cudaSuccess) return e;
         e = launch_pdl(poisson_kernel, dim3(1), dim3(T), psmem, P->st, Nx, P->prx, P->ptw_len, tw_in_smem,
@@ -1420,5 +1514,9 @@ extern "C" int vog_reset(vog_plan_t P)
     P->recx_valid = false;
     return VOG_OK;
 }
+
+#ifdef VOG_STAMPS
+extern "C" int vog_debug_stamps(long long* out32) { return (int)cudaMemcpyFromSymbol(out32, vog::vog_stamps, sizeof(long long) * 32); }
+#endif
 
 extern "C" long long vog_launch_count(vog_plan_t P) { return P ? P->launches : -1; }
