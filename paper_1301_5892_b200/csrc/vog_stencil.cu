@@ -17,7 +17,7 @@
 //            group's window is in flight in the other slot); a thread computes four consecutive cells at a time from
 //            128-bit shared loads and stores them with one 128-bit store.  In place: a CTA-wide "landed" mbarrier
 //            (as in osx7_kernel) before the first store of a line group; out of place: no synchronisation between warps.
-//   v      : a CTA owns 32 columns x 256 rows; the union of the rows it needs lands coalesced in shared memory
+//   v      : a CTA owns 32 columns x 128 rows; the union of the rows it needs lands coalesced in shared memory
 //            (raw[row][column], conflict free for any per-column shift); a thread computes 16 consecutive rows of its
 //            column from a sliding register window; rows are stored coalesced; the delta-f source is added in
 //            the same pass.  Out of place, like the Fourier v kernels.
@@ -203,13 +203,13 @@ __global__ void __launch_bounds__(512, 1) stx_kernel(const OsArgs a, const float
 // ---------------------------------------------------------------------------------------------
 // v-direction
 namespace st {
-constexpr int VRS = 256;               // rows per CTA
+constexpr int VRS = 128;               // rows per CTA (8 warps x 16 rows; four CTAs per SM interleave load, compute, store)
 constexpr int VR = 16;                 // consecutive rows per thread
 constexpr int VSPREAD = 32;            // spread of the integer shifts of a strip that the row buffer can hold
 }
 
 template <int NT, int JL>
-__global__ void __launch_bounds__(512, 2) stv_kernel(const OsArgs a, const float* __restrict__ taps)
+__global__ void __launch_bounds__(256, 4) stv_kernel(const OsArgs a, const float* __restrict__ taps)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int W = 32, RS = st::VRS, R = st::VR, RMAX = st::VSPREAD;
@@ -243,13 +243,13 @@ __global__ void __launch_bounds__(512, 2) stv_kernel(const OsArgs a, const float
     const int rs = r0 - JL + base;
     if (!gather) {
         const float* const src = a.src + c0;
-        for (int i = tid; i < nrows * 8; i += 512) {
+        for (int i = tid; i < nrows * 8; i += 256) {
             const int r = i >> 3, q4 = (i & 7) * 4;
             os2::cp_async16_cg(raw + r * W + q4, src + (size_t)((rs + r) & vmask) * Nx + q4);
         }
     } else {
         const float* const col = a.src + c0 + lane;
-        for (int r = wid; r < nrows; r += 16) os2::cp_async4(raw + r * W + lane, col + (size_t)((rs + r) & vmask) * Nx);
+        for (int r = wid; r < nrows; r += 8) os2::cp_async4(raw + r * W + lane, col + (size_t)((rs + r) & vmask) * Nx);
     }
     os2::cp_async_wait_all();
     __syncthreads();
@@ -375,7 +375,7 @@ static cudaError_t stv_launch_t(const OsArgs& a, const float* taps, cudaStream_t
     const size_t smem = (size_t)(st::VRS + NT - 1 + st::VSPREAD) * 32 * 4;
     cudaError_t e = set_max_smem((const void*)stv_kernel<NT, JL>, smem);
     if (e != cudaSuccess) return e;
-    return launch_pdl(stv_kernel<NT, JL>, dim3(a.Nx / 32, a.Nv / st::VRS), dim3(512), smem, st, a, taps);
+    return launch_pdl(stv_kernel<NT, JL>, dim3(a.Nx / 32, a.Nv / st::VRS), dim3(256), smem, st, a, taps);
 }
 
 cudaError_t stv_launch(const OsArgs& a, int spline, int d, const float* taps, cudaStream_t st)
