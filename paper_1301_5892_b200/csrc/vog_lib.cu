@@ -953,8 +953,7 @@ static OsxShape osx_shape(const vog_plan_s* P, int lpi)
     o.smem6 = (size_t)lpi * (P->p.Nx + 480) * 4 + (size_t)2 * lpi * OS_LAMW * 8 + (size_t)(o.thr / 16) * (16 * 17 * 8) + 16;
     // warp-private windows (one round only): window slot, exchange scratch (overlapping by its unused last element) and
     // two shift words per pair, two symbol rows per line, one mbarrier per warp + 2
-    o.smem7 = (size_t)(o.thr / 16) * (492 * 4 + (16 * 17 - 1) * 8 + 8) + 8 + (size_t)2 * lpi * OS_LAMW * 8 + (size_t)(o.thr / 32 + 2) * 8 + 8 +
-              (size_t)4 * (((16 - ((o.thr / 16 + 1) / 2) * 492) % 32 + 32) % 32);
+    o.smem7 = (size_t)(o.thr / 16) * (492 * 4 + (16 * 17 - 1) * 8 + 8) + 8 + (size_t)2 * lpi * OS_LAMW * 8 + (size_t)(o.thr / 32 + 2) * 8;
     return o;
 }
 

@@ -163,15 +163,6 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
     const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
     asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(s) : "memory");
 }
-// non-blocking: has the phase with this parity completed?
-__device__ __forceinline__ bool mbar_test(unsigned long long* bar, const unsigned parity)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
-    unsigned ok;
-    asm volatile("{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-                 : "=r"(ok) : "r"(s), "r"(parity) : "memory");
-    return ok != 0;
-}
 // (the suspend-time hint lets the hardware park the warp instead of spinning: in the first version 23 % of the
 // kernel's instructions were this loop)
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, const unsigned parity)
@@ -371,8 +362,6 @@ __global__ void __launch_bounds__(288, 3) osx6_kernel(const OsArgs a)
 namespace os2 {
 constexpr int XWIN = 492;              // floats per window slot = floats copied per window: 3 (alignment) + 15 + 240 + V + 1
 constexpr int XCOPY = XWIN;
-// words of padding between the nA even-pair slots and the odd-pair slots: (nA XWIN + pad) = 16 mod 32
-__host__ __device__ constexpr int xwin_pad(int nA) { return ((16 - nA * XWIN) % 32 + 32) % 32; }
 }
 
 template <int V, int HLO>
@@ -385,18 +374,13 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
     // shared memory (sized to the byte: three CTAs of 18 pairs fill an SM): window slots | symbol rows [2][lpi] | exchange
     // scratch (the unused last pad element of a pair's 16 x 17 block overlaps the next pair's first) | shifts | mbarriers
     const int S = T >> 4;                                                                          // pair slots
-    // the slots of the even pairs first, then (after a pad of a few words) those of the odd pairs, so that the two
-    // windows of a warp lie 16 banks apart: with slots simply one after the other (492 words = 12 mod 32) four banks
-    // of the two half-warps overlapped and 12 % of all shared wavefronts were replays of pass A's loads
-    const int nA = (S + 1) >> 1, padw = os2::xwin_pad(nA);
-    float* const win = reinterpret_cast<float*>(smem_raw) + (hw >> 1) * os2::XWIN + (hw & 1) * (nA * os2::XWIN + padw);
-    float2* const lamS = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + S * os2::XWIN + padw);   // [2][lpi][OS_LAMW]
+    float* const win = reinterpret_cast<float*>(smem_raw) + hw * os2::XWIN;                       // this pair's window
+    float2* const lamS = reinterpret_cast<float2*>(reinterpret_cast<float*>(smem_raw) + S * os2::XWIN);   // [2][lpi][OS_LAMW]
     float2* const scr = lamS + 2 * lpi * OS_LAMW + hw * (os2::XPAIR - 1);
     int* const wsh = reinterpret_cast<int*>(lamS + 2 * lpi * OS_LAMW + S * (os2::XPAIR - 1) + 1) + 2 * hw;   // [S][2]
     unsigned long long* const bars = reinterpret_cast<unsigned long long*>(
         reinterpret_cast<int*>(lamS + 2 * lpi * OS_LAMW + S * (os2::XPAIR - 1) + 1) + 2 * S);
     // bars: [0] landed; [1] symbol rows; [2 + warp] windows of the warp
-    int* const rowseq = reinterpret_cast<int*>(bars + 2 + (T >> 5));       // groups whose NEXT symbol rows were requested
     Tw4 w;
     w.b1 = __ldg(a.tw + t);               // [q-1][t] = e^{-2 pi i t q / 256}
     w.b2 = __ldg(a.tw + 16 + t);
@@ -404,9 +388,8 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
     w.b8 = __ldg(a.tw + 7 * 16 + t);
     // (one barrier per thread: a loop over the barriers in ONE thread made ptxas 12.9 read the uniform register that
     // holds the address of the last barrier before writing it, and the kernel then waited on an uninitialised object)
-    if (tid == 0) *rowseq = 0;
     if (tid <= nwarps + 1) {
-        // [0]: one arrival per warp; [1]: the requester's expect_tx; others: the two half-warp leaders' expect_tx arrivals
+        // [0]: one arrival per warp; [1]: thread 0's expect_tx; others: the two half-warp leaders' expect_tx arrivals
         os2::mbar_init(bars + tid, tid == 0 ? (unsigned)nwarps : (tid == 1 ? 1u : 2u));
         os2::mbar_init_fence();
     }
@@ -440,12 +423,9 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
         const int line = g * lpi + l;
         if (has_pair && g < a.n_groups && line < a.n_lines) os2::cp_async4(wsh, &a.lam[(size_t)line * OS_LAMW + 129].x);
     };
-    // symbol rows of the lines of group g into row buffer (par); one thread.  Requested for group g + G once the landed
-    // barrier of group g has completed: by then every warp has started pass A of group g, i.e. is done with the middle
-    // stage of group g - G, whose rows this overwrites.  WHO requests: the first warp leader that finds the barrier
-    // complete, looking right after its own pass A (non-blocking) and again after its wait before the stores -- with
-    // thread 0 alone requesting after ITS wait, a tenth of all warp samples sat waiting for the rows at the top of the
-    // next group.  A sequence word in shared memory elects the requester (atomicCAS).
+    // thread 0: symbol rows of the lines of group g into row buffer (par).  Called for group g + G right after the
+    // landed barrier of group g: by then every warp has started pass A of group g, i.e. is done with the middle stage
+    // of group g - G, whose rows this overwrites; they arrive long before the first middle stage of group g + G.
     auto issue_rows = [&](const int g, const unsigned par) {
         const int line0 = g * lpi, nl = min(lpi, a.n_lines - line0);
         os2::mbar_expect_tx(bars + 1, (unsigned)nl * 8u * OS_LAMW);
@@ -463,8 +443,7 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
         if (tid == 0) issue_rows(blockIdx.x, 0u);
     }
     unsigned parity = 0;
-    int it = 0;                                    // groups done by this CTA
-    for (int g = blockIdx.x; g < a.n_groups; g += G, ++it) {
+    for (int g = blockIdx.x; g < a.n_groups; g += G) {
         const int gn = g + G;
         const int line = g * lpi + l;
         const bool active = has_pair && line < a.n_lines;
@@ -489,8 +468,6 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
             });
         }
         __syncwarp();
-        if (lane == 0 && gn < a.n_groups && os2::mbar_test(bars, parity) && atomicCAS(rowseq, it, it + 1) == it)
-            issue_rows(gn, parity ^ 1u);
         // (the shared stores above needed every sample: the window slots of this warp are free)
         if (gn < a.n_groups) {
             if (t == 0) {
@@ -514,7 +491,7 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
         }
         __syncwarp();
         os2::mbar_wait(bars, parity);              // every window of this line group is on chip: stores may begin
-        if (lane == 0 && gn < a.n_groups && atomicCAS(rowseq, it, it + 1) == it) issue_rows(gn, parity ^ 1u);
+        if (tid == 0 && gn < a.n_groups) issue_rows(gn, parity ^ 1u);
         // ---- inverse pass A: scratch -> registers -> global
         if (active) {
             float2 x[16];
