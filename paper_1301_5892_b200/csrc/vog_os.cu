@@ -267,21 +267,69 @@ int osx6_occupancy(int geom, int threads, size_t smem)
     return nb;
 }
 
+// Tensor maps of a source grid for osv7_kernel: fp32 [Nv][Nx], boxes of 16 columns x {256, 64, 16, 4, 2} rows.  The
+// encoder is a host-only driver entry point (no kernel, no copy), looked up through the runtime so that the library has
+// no link-time dependency on libcuda; maps are cached per (grid pointer, Nx, Nv): a step alternates between two grids.
+static cudaError_t v_maps(const float* src, int Nx, int Nv, os2::VMaps* out)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static std::mutex mu;
+    static encode_fn encode = nullptr;
+    struct Key {
+        const float* p; int nx, nv;
+        bool operator<(const Key& o) const { return p != o.p ? p < o.p : (nx != o.nx ? nx < o.nx : nv < o.nv); }
+    };
+    static std::map<Key, os2::VMaps> cache;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+        if (e != cudaSuccess) return e;
+        if (qr != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+        encode = (encode_fn)fn;
+    }
+    const Key key{src, Nx, Nv};
+    auto it = cache.find(key);
+    if (it == cache.end()) {
+        if (cache.size() > 64) cache.clear();
+        os2::VMaps m;
+        const cuuint64_t dims[2] = {(cuuint64_t)Nx, (cuuint64_t)Nv};
+        const cuuint64_t strides[1] = {(cuuint64_t)Nx * 4};
+        const cuuint32_t estr[2] = {1, 1};
+        for (int i = 0; i < 5; ++i) {
+            const cuuint32_t box[2] = {(cuuint32_t)os2::VW, (cuuint32_t)(i == 4 ? 2 : 256 >> (2 * i))};
+            const CUresult r = encode(&m.m[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)src, dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+        }
+        it = cache.emplace(key, m).first;
+    }
+    *out = it->second;
+    return cudaSuccess;
+}
+
 // three-group v kernel (default): one persistent CTA of 768 threads per SM; a.gpc = pairs per work item
 cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_sm, cudaStream_t st)
 {
     const size_t smem = (size_t)OS_LAMW * os2::VW * 8 + 240 * 8 + 20 * os2::VW * 4 +
-                        3 * ((size_t)os2::VRR * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8);
+                        3 * ((size_t)os2::VRT * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8) + 3 * 8;
     const int n_items = (a.Nx / os2::VW) * ((a.np + a.gpc - 1) / a.gpc);
     const int grid = n_items < n_sm ? n_items : n_sm;
-    if (geom) {
-        cudaError_t e = set_max_smem((const void*)osv7_kernel<OS_VL, OS_HL>, smem);
-        if (e != cudaSuccess) return e;
-        return launch_pdl(osv7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(768), smem, st, a, su);
-    }
-    cudaError_t e = set_max_smem((const void*)osv7_kernel<OS_V, OS_H>, smem);
+    os2::VMaps maps;
+    cudaError_t e = v_maps(a.src, a.Nx, a.Nv, &maps);
     if (e != cudaSuccess) return e;
-    return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a, su);
+    if (geom) {
+        e = set_max_smem((const void*)osv7_kernel<OS_VL, OS_HL>, smem);
+        if (e != cudaSuccess) return e;
+        return launch_pdl(osv7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(768), smem, st, a, su, maps);
+    }
+    e = set_max_smem((const void*)osv7_kernel<OS_V, OS_H>, smem);
+    if (e != cudaSuccess) return e;
+    return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a, su, maps);
 }
 
 // 16-column-strip v kernel, symbol through L1; grid = (Nx / 16, ceil(np / gpc))

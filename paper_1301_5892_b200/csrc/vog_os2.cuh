@@ -17,6 +17,8 @@
 // (cp.async, 4 bytes: the full integer shift b of P:107 is applied by addressing, no alignment residue) exactly
 // the samples that it transforms in pass A.
 #pragma once
+#include <cuda.h>
+
 #include "vog_fft.cuh"
 #include "vog_internal.h"
 
@@ -853,14 +855,29 @@ __global__ void __launch_bounds__(256, 3) osv6_kernel(const OsArgs a)
 // and has the raw rows of its next pair in flight while it transforms the current one.  Persistent grid.
 namespace os2 {
 __device__ __forceinline__ void bar_group(const int id) { asm volatile("bar.sync %0, 256;\n" ::"r"(id) : "memory"); }
+constexpr int VRT = 520;               // rows of a group's raw buffer in osv7_kernel (even: rows land two by two)
+// tensor maps of the source grid [Nv][Nx] with boxes of 16 columns x {256, 64, 16, 4, 2} rows (host: osv7_launch)
+struct VMaps { CUtensorMap m[5]; };
+__device__ __forceinline__ int vbox_rows(const int i) { return i == 4 ? 2 : 256 >> (2 * i); }
+// box (16 columns from column x, the map's rows from row y) -> shared memory (128-byte aligned), completing on bar
+__device__ __forceinline__ void tensor_g2s(void* smem, const CUtensorMap* map, const int x, const int y,
+                                           unsigned long long* bar)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem), b = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n"
+                 ::"r"(d), "l"(reinterpret_cast<unsigned long long>(map)), "r"(x), "r"(y), "r"(b)
+                 : "memory");
+}
 }
 
 template <int V, int HLO>
-__global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSetupArgs su)
+__global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSetupArgs su,
+                                                      const __grid_constant__ os2::VMaps maps)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr int W = os2::VW, RR = os2::VRR;
-    constexpr int RMAX = RR - OS_LB - V;           // spread of the integer shifts that the raw buffer can hold
+    constexpr int W = os2::VW, RR = os2::VRT;
+    constexpr int RMAX = RR - OS_LB - V - 1;       // spread of the integer shifts that the raw buffer can hold (the
+                                                   // window starts on an even row: up to one row more than needed)
     constexpr int GB = RR * W * 4 + OS_LB * W * 8; // bytes per group: raw rows + exchange buffer
     float2* const lamS = reinterpret_cast<float2*>(smem_raw);                     // [OS_LAMW][16]
     float2* const twS = lamS + OS_LAMW * W;                                       // [15][16] e^{-2 pi i t q / 256}
@@ -871,6 +888,14 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + 240 * 8 + 20 * W * 4 + gid * GB;
     float* const raw = reinterpret_cast<float*>(gbase);                           // [RR][16]
     float2* const exch = reinterpret_cast<float2*>(raw + RR * W);                 // [256][16]
+    // one mbarrier per group: the bytes of the group's raw rows (one expect_tx arrival by the thread that requests them)
+    unsigned long long* const vbar =
+        reinterpret_cast<unsigned long long*>(smem_raw + OS_LAMW * W * 8 + 240 * 8 + 20 * W * 4 + 3 * GB) + gid;
+    unsigned vpar = 0;
+    if (gt == 0) {                                 // (one barrier per thread, see osx7_kernel)
+        os2::mbar_init(vbar, 1u);
+        os2::mbar_init_fence();
+    }
     const int c = gt & 15, h = gt >> 4;                                           // column of the strip, item index
     const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
     const int nstrips = Nx / W, nseg = (a.np + a.gpc - 1) / a.gpc, n_items = nstrips * nseg;
@@ -979,19 +1004,38 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         }
         const int R = dmax - dmin;
         const bool gather = R > RMAX;              // uniform over the CTA (every half-warp sees the same 16 columns)
-        const int db = gather ? 0 : d - dmin;      // this lane's row offset inside the raw window
-        const int base = gather ? b : b0 + dmin;   // first raw row = pair start - HLO + base
+        // The union of the rows the 16 columns need is a box of the grid: 16 columns x (V + 256 + R) rows.  It is
+        // requested by ONE thread of the group as a handful of 2-D tensor copies (cp.async.bulk.tensor, the TMA engine:
+        // boxes of 256, 64, 16, 4 and 2 rows; a second run of boxes when the window wraps around the end of the
+        // columns), counted in bytes on the group's mbarrier.  The per-thread 16-byte cp.async loop this replaces was
+        // 18 % of all instructions the kernel executed (25 instructions of address arithmetic per copy).  A box must
+        // start on a 128-byte boundary of shared memory = an even row of the raw buffer: the window starts on an even
+        // row of the grid (one row early if need be) and holds an even number of rows.
+        const int odd = gather ? 0 : ((b0 + dmin - HLO) & 1);
+        const int db = gather ? 0 : d - dmin + odd;      // this lane's row offset inside the raw window
+        const int base = gather ? b : b0 + dmin - odd;   // first raw row = pair start - HLO + base
         const float* const col = a.src + c0 + c;
         float* const ocol = a.dst + c0 + c;
-        const int nrows = V + OS_LB + (gather ? 0 : R);
+        const int nrows = gather ? V + OS_LB : (V + OS_LB + R + odd + 1) & ~1;
         // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
         auto land = [&](const int p) {
             const int rs = p * (2 * V) - HLO + base;
             if (!gather) {
-                const float* const src = a.src + c0;
-                for (int i = gt; i < nrows * 4; i += 256) {
-                    const int r = i >> 2, q4 = (i & 3) * 4;
-                    os2::cp_async16_cg(raw + r * W + q4, src + (size_t)((rs + r) & vmask) * Nx + q4);
+                if (gt == 0) {
+                    os2::mbar_expect_tx(vbar, (unsigned)nrows * (W * 4u));
+                    int gr = rs & vmask, sr = 0;
+                    for (int seg = 0; seg < 2 && sr < nrows; ++seg) {
+                        int n = min(nrows - sr, Nv - gr);        // (a window past the last row wraps to row 0)
+#pragma unroll 1
+                        for (int i = 0; i < 5; ++i) {
+                            const int hb = os2::vbox_rows(i);
+                            while (n >= hb) {
+                                os2::tensor_g2s(raw + sr * W, &maps.m[i], c0, gr, vbar);
+                                gr += hb; sr += hb; n -= hb;
+                            }
+                        }
+                        gr = 0;
+                    }
                 }
             } else {
                 for (int r = h; r < nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
@@ -1002,7 +1046,8 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         os2::cp_async_wait_all();                  // this thread's chunks of the table (and of the first raw rows)
         __syncthreads();                           // table visible to everybody
         for (int p = p0; p < q1; p += 3) {
-            os2::cp_async_wait_all();
+            if (gather) os2::cp_async_wait_all();
+            else { os2::mbar_wait(vbar, vpar); vpar ^= 1u; }
             os2::bar_group(gid + 1);               // raw rows of pair p visible; exchange buffer of the last pair read
             // ---- pass A (item t = h): samples from the raw rows with this lane's offset
             {
