@@ -315,10 +315,11 @@ static cudaError_t v_maps(const float* src, int Nx, int Nv, os2::VMaps* out)
 // three-group v kernel (default): one persistent CTA of 768 threads per SM; a.gpc = pairs per work item
 cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_sm, cudaStream_t st)
 {
-    const size_t smem = (size_t)OS_LAMW * os2::VW * 8 + 240 * 8 + 20 * os2::VW * 4 +
+    // table | twiddles | three coefficient records | (cos, sin) table | three groups (raw rows + exchange) | mbarriers
+    const size_t smem = (size_t)OS_LAMW * os2::VW * 8 + 240 * 8 + 3 * 20 * os2::VW * 4 + 136 * 16 +
                         3 * ((size_t)os2::VRT * os2::VW * 4 + (size_t)OS_LB * os2::VW * 8) + 3 * 8;
-    const int n_items = (a.Nx / os2::VW) * ((a.np + a.gpc - 1) / a.gpc);
-    const int grid = n_items < n_sm ? n_items : n_sm;
+    const int nstrips = a.Nx / os2::VW;
+    const int grid = nstrips >= n_sm ? n_sm : nstrips * (n_sm / nstrips);     // (see the kernel: pieces of work)
     os2::VMaps maps;
     cudaError_t e = v_maps(a.src, a.Nx, a.Nv, &maps);
     if (e != cudaSuccess) return e;

@@ -879,120 +879,119 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     constexpr int RMAX = RR - OS_LB - V - 1;       // spread of the integer shifts that the raw buffer can hold (the
                                                    // window starts on an even row: up to one row more than needed)
     constexpr int GB = RR * W * 4 + OS_LB * W * 8; // bytes per group: raw rows + exchange buffer
+    constexpr int CF = 20 * W;                     // words of one coefficient record: [18][16] floats, [16] b, [16] E dt
+    constexpr int HEAD = OS_LAMW * W * 8 + 240 * 8 + 3 * CF * 4 + 136 * 16;   // a multiple of 128 bytes
     float2* const lamS = reinterpret_cast<float2*>(smem_raw);                     // [OS_LAMW][16]
     float2* const twS = lamS + OS_LAMW * W;                                       // [15][16] e^{-2 pi i t q / 256}
-    float* const afS = reinterpret_cast<float*>(twS + 240);                       // [18][16] symbol coefficients per column
-    int* const bS = reinterpret_cast<int*>(afS + 18 * W);                         // [16] integer shifts
-    float* const sS = reinterpret_cast<float*>(bS + W);                           // [16] source shifts E dt
+    float* const cfS = reinterpret_cast<float*>(twS + 240);                       // [3] coefficient records (ring)
+    float4* const csS = reinterpret_cast<float4*>(cfS + 3 * CF);                  // [129] (cos, sin, ..) of theta_k
     const int tid = threadIdx.x, gid = tid >> 8, gt = tid & 255;                  // group, thread of the group
-    unsigned char* const gbase = smem_raw + OS_LAMW * W * 8 + 240 * 8 + 20 * W * 4 + gid * GB;
+    unsigned char* const gbase = smem_raw + HEAD + gid * GB;
     float* const raw = reinterpret_cast<float*>(gbase);                           // [RR][16]
     float2* const exch = reinterpret_cast<float2*>(raw + RR * W);                 // [256][16]
     // one mbarrier per group: the bytes of the group's raw rows (one expect_tx arrival by the thread that requests them)
-    unsigned long long* const vbar =
-        reinterpret_cast<unsigned long long*>(smem_raw + OS_LAMW * W * 8 + 240 * 8 + 20 * W * 4 + 3 * GB) + gid;
+    unsigned long long* const vbar = reinterpret_cast<unsigned long long*>(smem_raw + HEAD + 3 * GB) + gid;
     unsigned vpar = 0;
     if (gt == 0) {                                 // (one barrier per thread, see osx7_kernel)
         os2::mbar_init(vbar, 1u);
         os2::mbar_init_fence();
     }
     const int c = gt & 15, h = gt >> 4;                                           // column of the strip, item index
-    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1;
-    const int nstrips = Nx / W, nseg = (a.np + a.gpc - 1) / a.gpc, n_items = nstrips * nseg;
+    const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1, np = a.np;
     // (the FP32 pipe is what this kernel waits for most: the 15 twiddles of an item come from a 1.9 KB table in
     // shared memory, 15 loads per pass, instead of 11 complex products of four register-resident powers)
-    for (int i = tid; i < 240; i += 768) twS[i] = __ldg(a.tw + i);               // (plan constant: before the wait)
+    for (int i = tid; i < 240; i += 768) twS[i] = __ldg(a.tw + i);               // (plan constants: before the wait)
+    for (int k = tid; k < 129; k += 768) {
+        const double2 cs = su.cs64[k];
+        csS[k] = su.spline ? make_float4((float)cs.x, (float)cs.y, (float)(2.0 * cs.x * cs.x - 1.0), (float)(2.0 * cs.y * cs.x))
+                           : make_float4((float)cs.x, (float)cs.y, (float)(2.0 - 2.0 * cs.x), 0.0f);
+    }
     const float2* const twp = twS + h;            // [q-1][t], t = item index of passes A
-    pdl_wait();                                   // the symbol tables and the source grid come from earlier kernels
-    pdl_launch_dependents();
     float2* const own = exch + h * W + c;                                     // position t = h
     constexpr int PS = 16 * W;                                                // float2 between positions 16 apart
 
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const int strip = item % nstrips, seg = item / nstrips;              // (neighbouring CTAs: neighbouring strips)
-        const int c0 = strip * W;
-        const int q0 = seg * a.gpc, q1 = min(a.np, q0 + a.gpc);              // pairs of the segment
-        __syncthreads();                           // every group is done with the table of the previous item
-        // S1 inside the kernel: the symbol table of the strip is COMPUTED here (no set-up kernel between the field
-        // solve and this one).  Same arithmetic, entry for entry, as os_setup_v_kernel: beta, b, b* and the Everett /
-        // B-spline coefficients in fp64 per column (32 threads: column x half), the 130 entries by fp32 Horner.
-        if (tid < 2 * W) {
-            const int half = tid >> 4, cc = tid & 15, l = c0 + cc;
-            double beta;
-            float sshift = 0.0f;
-            if (su.mode == 1) {
-                double e = (double)su.E[l];
-                if (su.Eext) e += (double)su.Eext[l];
-                beta = -e * su.dt / su.delta;
-                sshift = (float)(su.dt * e);
-            } else {
-                beta = su.beta[l];
-            }
-            const double fl = floor(beta);
-            const double tt0 = beta - fl;
-            int bb;
-            if (fabs(fl) < 9.0e18) {
-                bb = (int)(__double2ll_rn(fl) & (long long)(su.N - 1));
-            } else {
-                double bm = fmod(fl, (double)su.N);
-                if (bm < 0.0) bm += (double)su.N;
-                bb = (int)bm;
-                if (bb >= su.N) bb = 0;
-            }
-            if (half == 0) { bS[cc] = bb; sS[cc] = sshift; }
-            if (!su.spline) {
-                const double tt = half == 0 ? 1.0 - tt0 : tt0;
-                double av = tt;
-                constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
-                                           1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
-                afS[(half * 9) * W + cc] = (float)av;
-#pragma unroll
-                for (int m = 1; m <= 8; ++m) {
-                    av = av * ((double)(m * m) - tt * tt) * rcp[m];
-                    afS[(half * 9 + m) * W + cc] = m <= su.d ? (float)av : 0.0f;
-                }
-            } else if (half == 0) {
-                const double t = tt0, u = 1.0 - t;
-                afS[0 * W + cc] = (float)(u * u * u / 6.0);
-                afS[1 * W + cc] = (float)((4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0);
-                afS[2 * W + cc] = (float)((1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0);
-                afS[3 * W + cc] = (float)(t * t * t / 6.0);
-            }
+    // Work of this CTA, in pieces (strip of 16 columns, pairs q0 .. q1-1).  The strips are dealt out round-robin in
+    // whole rounds of gridDim.x strips (neighbouring CTAs work on neighbouring strips at the same time); the strips
+    // left over after the last whole round are cut by PAIRS into gridDim.x equal shares, so every CTA gets the same
+    // number of pairs (+-1) whatever Nx / 16 is (8192: 512 strips on 148 CTAs were 4 rounds for 3.46 rounds of work).
+    const int G = gridDim.x, kb = blockIdx.x, nstrips = Nx / W;
+    const int Rr = nstrips / G, Lt = nstrips - Rr * G;
+    const int tlo = (int)((long long)Lt * np * kb / G), thi = (int)((long long)Lt * np * (kb + 1) / G);
+    auto piece = [&](const int i, int& strip, int& q0, int& q1) -> bool {
+        if (i < Rr) { strip = i * G + kb; q0 = 0; q1 = np; return true; }
+        if (Rr == 0) {
+            // fewer strips than CTAs (grids up to 2048 columns): a share of pairs would straddle two strips and pay two
+            // tables for a handful of pairs; instead every strip gets floor(G / nstrips) CTAs, one segment each
+            const int m = G / nstrips, sidx = kb / nstrips, sg = (np + m - 1) / m;
+            strip = kb % nstrips;
+            q0 = sidx * sg;
+            q1 = min(np, q0 + sg);
+            return i == 0 && sidx < m && q0 < q1;
         }
-        __syncthreads();
-        for (int idx = tid; idx < OS_LAMW * W; idx += 768) {
-            const int kk = idx >> 4, cc = idx & 15;
-            float2 o;
-            if (kk == 129) o = make_float2(__int_as_float(bS[cc]), sS[cc]);
-            else if (kk == 0) o = make_float2(1.0f / (float)OS_LB, 0.0f);          // lambda_0 = sum of the weights = 1
-            else {
-                const double2 cs = su.cs64[kk];
-                const float cf = (float)cs.x, sn = (float)cs.y;
-                float lr, li;
-                if (su.spline) {
-                    const float Bm1 = afS[cc], B0 = afS[W + cc], B1 = afS[2 * W + cc], B2 = afS[3 * W + cc];
-                    const float c2 = (float)(2.0 * cs.x * cs.x - 1.0), s2 = (float)(2.0 * cs.y * cs.x);
-                    const float gg = 3.0f / (2.0f + cf);
-                    lr = fmaf(B2, c2, fmaf(Bm1 + B1, cf, B0)) * gg;
-                    li = fmaf(B2, s2, (B1 - Bm1) * sn) * gg;
-                } else {
-                    const float sv = (float)(2.0 - 2.0 * cs.x);
-                    float q0 = 0.0f, q1 = 0.0f;
-#pragma unroll
-                    for (int j = 8; j >= 0; --j) {
-                        q0 = fmaf(q0, sv, afS[j * W + cc]);
-                        q1 = fmaf(q1, sv, afS[(9 + j) * W + cc]);
-                    }
-                    lr = fmaf(cf, q1, q0);
-                    li = sn * q1;
-                }
-                o = make_float2(lr * (1.0f / (float)OS_LB), li * (1.0f / (float)OS_LB));
-            }
-            lamS[idx] = o;
+        int L = tlo;
+        for (int j = i - Rr;; --j) {
+            if (L >= thi) return false;
+            const int sidx = L / np;
+            q0 = L - sidx * np;
+            q1 = min(np, q0 + thi - L);
+            if (j == 0) { strip = Rr * G + sidx; return true; }
+            L += q1 - q0;
         }
-        // integer shift (rows) and source shift of this lane's column
-        const int b = bS[c];
-        const float ssh = sS[c];
+    };
+    // S1 inside the kernel: the symbol table of a strip is COMPUTED here (no set-up kernel between the field solve and
+    // this one).  Same arithmetic, entry for entry, as os_setup_v_kernel: beta, b, b* and the Everett / B-spline
+    // coefficients in fp64 per column (32 threads: column x half; lane = the thread's index 0..31), then the 130
+    // entries by fp32 Horner.  The fp64 part of piece i + 2 runs in ONE warp while piece i is being transformed.
+    auto coeffs = [&](const int lane32, const int c0, float* const rec) {
+        float* const afS = rec;
+        int* const bS = reinterpret_cast<int*>(rec + 18 * W);
+        float* const sS = rec + 19 * W;
+        const int half = lane32 >> 4, cc = lane32 & 15, l = c0 + cc;
+        double beta;
+        float sshift = 0.0f;
+        if (su.mode == 1) {
+            double e = (double)su.E[l];
+            if (su.Eext) e += (double)su.Eext[l];
+            beta = -e * su.dt / su.delta;
+            sshift = (float)(su.dt * e);
+        } else {
+            beta = su.beta[l];
+        }
+        const double fl = floor(beta);
+        const double tt0 = beta - fl;
+        int bb;
+        if (fabs(fl) < 9.0e18) {
+            bb = (int)(__double2ll_rn(fl) & (long long)(su.N - 1));
+        } else {
+            double bm = fmod(fl, (double)su.N);
+            if (bm < 0.0) bm += (double)su.N;
+            bb = (int)bm;
+            if (bb >= su.N) bb = 0;
+        }
+        if (half == 0) { bS[cc] = bb; sS[cc] = sshift; }
+        if (!su.spline) {
+            const double tt = half == 0 ? 1.0 - tt0 : tt0;
+            double av = tt;
+            constexpr double rcp[9] = {0.0, 1.0 / 6.0, 1.0 / 20.0, 1.0 / 42.0, 1.0 / 72.0, 1.0 / 110.0, 1.0 / 156.0,
+                                       1.0 / 210.0, 1.0 / 272.0};            // 1 / (2m (2m+1))
+            afS[(half * 9) * W + cc] = (float)av;
+#pragma unroll
+            for (int m = 1; m <= 8; ++m) {
+                av = av * ((double)(m * m) - tt * tt) * rcp[m];
+                afS[(half * 9 + m) * W + cc] = m <= su.d ? (float)av : 0.0f;
+            }
+        } else if (half == 0) {
+            const double t = tt0, u = 1.0 - t;
+            afS[0 * W + cc] = (float)(u * u * u / 6.0);
+            afS[1 * W + cc] = (float)((4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0);
+            afS[2 * W + cc] = (float)((1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0);
+            afS[3 * W + cc] = (float)(t * t * t / 6.0);
+        }
+    };
+    // where the raw rows of a piece lie: per-lane offset db, first row base (relative to pair start - HLO), row count
+    struct Geo { int c0, base, nrows, db; bool gather; };
+    auto geometry = [&](const int c0, const float* const rec) -> Geo {
+        const int b = reinterpret_cast<const int*>(rec + 18 * W)[c];
         // spread of the shifts over the strip, as signed distances from column 0's (shifts live mod Nv)
         const int b0 = __shfl_sync(0xffffffffu, b, 0, 16);
         const int d = (((b - b0) + (Nv >> 1)) & vmask) - (Nv >> 1);
@@ -1003,7 +1002,9 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
         }
         const int R = dmax - dmin;
-        const bool gather = R > RMAX;              // uniform over the CTA (every half-warp sees the same 16 columns)
+        Geo g;
+        g.c0 = c0;
+        g.gather = R > RMAX;                       // uniform over the CTA (every half-warp sees the same 16 columns)
         // The union of the rows the 16 columns need is a box of the grid: 16 columns x (V + 256 + R) rows.  It is
         // requested by ONE thread of the group as a handful of 2-D tensor copies (cp.async.bulk.tensor, the TMA engine:
         // boxes of 256, 64, 16, 4 and 2 rows; a second run of boxes when the window wraps around the end of the
@@ -1011,48 +1012,100 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         // 18 % of all instructions the kernel executed (25 instructions of address arithmetic per copy).  A box must
         // start on a 128-byte boundary of shared memory = an even row of the raw buffer: the window starts on an even
         // row of the grid (one row early if need be) and holds an even number of rows.
-        const int odd = gather ? 0 : ((b0 + dmin - HLO) & 1);
-        const int db = gather ? 0 : d - dmin + odd;      // this lane's row offset inside the raw window
-        const int base = gather ? b : b0 + dmin - odd;   // first raw row = pair start - HLO + base
-        const float* const col = a.src + c0 + c;
-        float* const ocol = a.dst + c0 + c;
-        const int nrows = gather ? V + OS_LB : (V + OS_LB + R + odd + 1) & ~1;
-        // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
-        auto land = [&](const int p) {
-            const int rs = p * (2 * V) - HLO + base;
-            if (!gather) {
-                if (gt == 0) {
-                    os2::mbar_expect_tx(vbar, (unsigned)nrows * (W * 4u));
-                    int gr = rs & vmask, sr = 0;
-                    for (int seg = 0; seg < 2 && sr < nrows; ++seg) {
-                        int n = min(nrows - sr, Nv - gr);        // (a window past the last row wraps to row 0)
+        const int odd = g.gather ? 0 : ((b0 + dmin - HLO) & 1);
+        g.db = g.gather ? 0 : d - dmin + odd;      // this lane's row offset inside the raw window
+        g.base = g.gather ? b : b0 + dmin - odd;   // first raw row = pair start - HLO + base
+        g.nrows = g.gather ? V + OS_LB : (V + OS_LB + R + odd + 1) & ~1;
+        return g;
+    };
+    // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
+    auto land = [&](const Geo& g, const int p) {
+        const int rs = p * (2 * V) - HLO + g.base;
+        if (!g.gather) {
+            if (gt == 0) {
+                os2::mbar_expect_tx(vbar, (unsigned)g.nrows * (W * 4u));
+                int gr = rs & vmask, sr = 0;
+                for (int sg = 0; sg < 2 && sr < g.nrows; ++sg) {
+                    int n = min(g.nrows - sr, Nv - gr);          // (a window past the last row wraps to row 0)
 #pragma unroll 1
-                        for (int i = 0; i < 5; ++i) {
-                            const int hb = os2::vbox_rows(i);
-                            while (n >= hb) {
-                                os2::tensor_g2s(raw + sr * W, &maps.m[i], c0, gr, vbar);
-                                gr += hb; sr += hb; n -= hb;
-                            }
+                    for (int i = 0; i < 5; ++i) {
+                        const int hb = os2::vbox_rows(i);
+                        while (n >= hb) {
+                            os2::tensor_g2s(raw + sr * W, &maps.m[i], g.c0, gr, vbar);
+                            gr += hb; sr += hb; n -= hb;
                         }
-                        gr = 0;
                     }
+                    gr = 0;
                 }
-            } else {
-                for (int r = h; r < nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
             }
-        };
+        } else {
+            const float* const col = a.src + g.c0 + c;
+            for (int r = h; r < g.nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
+        }
+    };
+
+    pdl_wait();                                   // the field and the source grid come from earlier kernels
+    pdl_launch_dependents();
+    int strip, q0, q1, nstrip = 0, nq0 = 0, nq1 = 0;
+    bool has = piece(0, strip, q0, q1), nhas = has && piece(1, nstrip, nq0, nq1);
+    if (tid < 2 * W && has) coeffs(tid, strip * W, cfS);
+    if (tid >= 2 * W && tid < 4 * W && nhas) coeffs(tid - 2 * W, nstrip * W, cfS + CF);
+    __syncthreads();
+    bool pref = false;                             // the first window of this group in the current piece is on its way
+    for (int it = 0; has; ++it) {
+        const float* const rec = cfS + (it % 3) * CF;
+        // ---- the strip's table: 130 x 16 entries
+        for (int idx = tid; idx < OS_LAMW * W; idx += 768) {
+            const int kk = idx >> 4, cc = idx & 15;
+            float2 o;
+            if (kk == 129) o = make_float2(rec[18 * W + cc], rec[19 * W + cc]);
+            else if (kk == 0) o = make_float2(1.0f / (float)OS_LB, 0.0f);          // lambda_0 = sum of the weights = 1
+            else {
+                const float4 cs = csS[kk];
+                const float cf = cs.x, sn = cs.y;
+                float lr, li;
+                if (su.spline) {
+                    const float Bm1 = rec[cc], B0 = rec[W + cc], B1 = rec[2 * W + cc], B2 = rec[3 * W + cc];
+                    const float gg = 3.0f / (2.0f + cf);
+                    lr = fmaf(B2, cs.z, fmaf(Bm1 + B1, cf, B0)) * gg;
+                    li = fmaf(B2, cs.w, (B1 - Bm1) * sn) * gg;
+                } else {
+                    const float sv = cs.z;
+                    float h0 = 0.0f, h1 = 0.0f;
+#pragma unroll
+                    for (int j = 8; j >= 0; --j) {
+                        h0 = fmaf(h0, sv, rec[j * W + cc]);
+                        h1 = fmaf(h1, sv, rec[(9 + j) * W + cc]);
+                    }
+                    lr = fmaf(cf, h1, h0);
+                    li = sn * h1;
+                }
+                o = make_float2(lr * (1.0f / (float)OS_LB), li * (1.0f / (float)OS_LB));
+            }
+            lamS[idx] = o;
+        }
+        const Geo g = geometry(strip * W, rec);
+        const float ssh = rec[19 * W + c];
         const int p0 = q0 + gid;
-        if (p0 < q1) land(p0);
-        os2::cp_async_wait_all();                  // this thread's chunks of the table (and of the first raw rows)
+        if (!pref && p0 < q1) land(g, p0);
+        pref = false;
         __syncthreads();                           // table visible to everybody
+        // the piece after next: its fp64 coefficients, in the last warp, while everybody else transforms
+        int fstrip = 0, fq0 = 0, fq1 = 0;
+        const bool fhas = nhas && piece(it + 2, fstrip, fq0, fq1);
+        if (tid >= 768 - 2 * W && fhas) coeffs(tid - (768 - 2 * W), fstrip * W, cfS + ((it + 2) % 3) * CF);
+        Geo gn = g;
+        if (nhas) gn = geometry(nstrip * W, cfS + ((it + 1) % 3) * CF);
+        const int np0 = nq0 + gid;
+        float* const ocol = a.dst + g.c0 + c;
         for (int p = p0; p < q1; p += 3) {
-            if (gather) os2::cp_async_wait_all();
+            if (g.gather) os2::cp_async_wait_all();
             else { os2::mbar_wait(vbar, vpar); vpar ^= 1u; }
             os2::bar_group(gid + 1);               // raw rows of pair p visible; exchange buffer of the last pair read
             // ---- pass A (item t = h): samples from the raw rows with this lane's offset
             {
                 float2 x[16];
-                const float* const rp = raw + (h + db) * W + c;
+                const float* const rp = raw + (h + g.db) * W + c;
 #pragma unroll
                 for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + V) * W]);
                 dft_dif<16, 1>(x);
@@ -1061,7 +1114,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 for (int q = 1; q < 16; ++q) own[q * PS] = cmul(x[brev(q, 16)], twp[(q - 1) * 16]);
             }
             os2::bar_group(gid + 1);               // exchange buffer complete; raw rows all read
-            if (p + 3 < q1) land(p + 3);           // the next window lands behind the middle stage and the inverse pass
+            // the next window lands behind the middle stage and the inverse pass: this piece's, or -- after the group's
+            // last pair of the piece -- the group's first of the NEXT piece (its shifts are known two pieces ahead)
+            if (p + 3 < q1) land(g, p + 3);
+            else if (nhas && np0 < nq1) { land(gn, np0); pref = true; }
             // ---- middle stage (item g = h): positions 16 g + j
             {
                 float2* const sp = exch + h * 16 * W + c;
@@ -1087,6 +1143,9 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 else os2_store_v<V, HLO>(po, (size_t)Nx, r0, Nv, h, false, x);
             }
         }
+        __syncthreads();                           // every group is done with the table of this piece
+        has = nhas; strip = nstrip; q0 = nq0; q1 = nq1;
+        nhas = fhas; nstrip = fstrip; nq0 = fq0; nq1 = fq1;
     }
 }
 
