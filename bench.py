@@ -446,24 +446,37 @@ def small_grids(torch, vog, stream, emit):
     return res
 
 
-def _time_calls(torch, stream, fn, warm, reps):
+def _time_calls(torch, stream, fn, warm, reps, inner=1):
+    """Median and best, in ms per call, of `reps` timed regions of `inner` back-to-back calls each."""
     for _ in range(warm):
         fn()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     times = []
     for _ in range(reps):
         e0.record(stream)
-        fn()
+        for _ in range(inner):
+            fn()
         e1.record(stream)
         stream.synchronize()
-        times.append(e0.elapsed_time(e1))
+        times.append(e0.elapsed_time(e1) / inner)
     return float(np.median(times)), min(times)
+
+
+def _time_kernel(torch, stream, fn, rec):
+    """A kernel-only row: the average launch duration over a timed region of 4 back-to-back launches (what a step
+    sees: the launches are chained by programmatic dependent launch), and beside it the event-to-event time of a
+    single launch (which includes the launch latency and the ramp of an idle GPU)."""
+    r = rec(*_time_calls(torch, stream, fn, 3, 10, inner=4))
+    r["us_single_launch"] = 1e3 * _time_calls(torch, stream, fn, 1, 10)[0]
+    return r
 
 
 def sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle):
     """BASELINE.json config 4: one x- and one v-advection on N x N, f ~ U[0,1), per-line shifts ~ U[-8,8] cells.
-    x / v = the public in-place calls vog_shift_x / vog_shift_v (table setup + kernel); x_kernel_only = vog_advect_x
-    with cached tables; v_out_of_place = vog_shift_v_to; strang_step = vog_step (28 B/cell: 3 advections + density).
+    x / v = the public in-place calls vog_shift_x / vog_shift_v (table setup + kernel), one call per timed region;
+    x_kernel_only = vog_advect_x with cached tables and v_out_of_place = vog_shift_v_to: average launch duration over
+    timed regions of 4 back-to-back launches (us_single_launch beside it); strang_step = vog_step (28 B/cell: 3
+    advections + density), one step per timed region.
     With with_oracle, the oracle's shift_x / shift_v (double, stencil or cyclic solve, all host cores) is timed on the
     same shape next to it for N <= 8192 (best of 3)."""
     orc = None
@@ -489,10 +502,10 @@ def sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle):
 
             row["x"] = rec(*_time_calls(torch, stream, lambda: plan.shift_x(f, bx), 3, 10))
             row["v"] = rec(*_time_calls(torch, stream, lambda: plan.shift_v(f, bx), 3, 10))
-            row["x_kernel_only"] = rec(*_time_calls(torch, stream, lambda: plan.advect_x(f, 0.01), 3, 10))
+            row["x_kernel_only"] = _time_kernel(torch, stream, lambda: plan.advect_x(f, 0.01), rec)
             if N * N * 4 * 3 < 160e9:
                 g = torch.empty_like(f)
-                row["v_out_of_place"] = rec(*_time_calls(torch, stream, lambda: plan.shift_v_to(f, g, bx), 3, 10))
+                row["v_out_of_place"] = _time_kernel(torch, stream, lambda: plan.shift_v_to(f, g, bx), rec)
                 del g
             row["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step(f, 1e-3), 2, 5), 28.0)
             row["strang_step"]["cell_updates_per_s"] = N * N / (row["strang_step"]["us_median"] * 1e-6)
@@ -502,10 +515,10 @@ def sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle):
                 # never instead of it -- the north-star fractions above are the Fourier kernels'
                 plan = vog.Plan(N, N, 1.0, -1.0, 1.0, kind, order, stream=stream)
                 plan.tune(27, 1)
-                st = {"x_kernel_only": rec(*_time_calls(torch, stream, lambda: plan.advect_x(f, 0.01), 3, 10))}
+                st = {"x_kernel_only": _time_kernel(torch, stream, lambda: plan.advect_x(f, 0.01), rec)}
                 if N * N * 4 * 3 < 160e9:
                     g = torch.empty_like(f)
-                    st["v_out_of_place"] = rec(*_time_calls(torch, stream, lambda: plan.shift_v_to(f, g, bx), 3, 10))
+                    st["v_out_of_place"] = _time_kernel(torch, stream, lambda: plan.shift_v_to(f, g, bx), rec)
                     del g
                 st["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step(f, 1e-3), 2, 5), 28.0)
                 row["direct_stencil"] = st
