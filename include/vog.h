@@ -190,6 +190,29 @@ int vog_plan_tune(vog_plan_t plan, int which, int value);
  * needed with VOG_SPLIT_XVX.  Returns VOG_OK, or VOG_EINVAL for NULL. */
 int vog_reset(vog_plan_t plan);
 
+/* Double-precision mode.  The same plan, the same parameters and the same
+ * call sequence with every array in fp64: f_dev holds Nx*Nv DOUBLES in the layout of the fp32 calls, E / E_ext / beta
+ * are Nx (or Nv) doubles in device memory.  The mode keeps its own tables and its own second grid (Nx*Nv doubles,
+ * allocated on the first v-advection; the out-of-place v kernel writes it and the following x-advection reads it back,
+ * so a step makes no copy; the stand-alone v calls copy back), created on the first *_f64 call of the plan; its state
+ * (cached x tables, the field kept for vog_get_field_f64 and the first half step of a VXV step) is separate from the
+ * fp32 calls', with the same rules.  What is computed:
+ *   - the circulant product of eq (4) in its direct form u'_i = sum_j a_j u_(i+b+j): the 2d+2 non-zero
+ *     entries of the row of A for Lagrange 2d+1, and for the cubic spline the row a = m * g with
+ *     g_n = sqrt(3) (sqrt(3) - 2)^|n| cut at |n| <= 30 (the neglected part of the row is < 1e-17), all in fp64;
+ *   - rho by fixed-order fp64 column sums, zero mean, the Fourier solve E^_m = rho^_m / (i k_m) with modes 0 and Nx/2
+ *     dropped (Q12) as two plain DFT sums (exact to rounding; O(Nx^2) operations spread over the GPU);
+ *   - the delta-f source f_eq(v - dt E) - f_eq(v) with expm1 in fp64.
+ * Asynchronous on the plan's stream, same error behaviour as the fp32 calls (VOG_EINVAL for NULL pointers, VOG_ENOMEM
+ * when the tables or the second grid cannot be allocated).  vog_plan_tune codes do not apply to this mode. */
+int vog_shift_x_f64(vog_plan_t plan, double* f_dev, const double* beta_cells_dev);
+int vog_shift_v_f64(vog_plan_t plan, double* f_dev, const double* beta_cells_dev);
+int vog_advect_x_f64(vog_plan_t plan, double* f_dev, double dt);
+int vog_advect_v_f64(vog_plan_t plan, double* f_dev, const double* E_dev, double dt);
+int vog_field_f64(vog_plan_t plan, const double* f_dev, double* E_dev);
+int vog_get_field_f64(vog_plan_t plan, double* E_dev);
+int vog_step_f64(vog_plan_t plan, double* f_dev, double dt, const double* E_ext_dev);
+
 /* Number of kernels the library launched on this plan since creation (for accounting). */
 long long vog_launch_count(vog_plan_t plan);
 

@@ -4,6 +4,8 @@
 
 #include <utility>
 
+#include "../../include/vog.h"
+
 namespace vog {
 
 // ---- Programmatic dependent launch.  The kernels of a Strang step (S1-S9) run back to back on one stream and at
@@ -152,6 +154,19 @@ size_t stx_smem_bytes(int spline, int d, int threads);
 cudaError_t stx_launch(const OsArgs& a, int spline, int d, const float* taps, int grid, int threads, size_t smem, cudaStream_t st);
 int stx_occupancy(int spline, int d, int threads, size_t smem);
 cudaError_t stv_launch(const OsArgs& a, int spline, int d, const float* taps, cudaStream_t st);
+
+// ---- double-precision mode (vog_f64.cu, NEXT-2): its own tables and kernels, created on the first *_f64 call of a plan
+struct F64State;
+int f64_create(F64State** out, const vog_params_t* p, cudaStream_t st, int n_sm);
+void f64_destroy(F64State* S);
+long long f64_launches(const F64State* S);
+bool f64_has_field(const F64State* S);
+cudaError_t f64_shift(F64State* S, double* f, const double* beta, bool vdir);
+cudaError_t f64_advect_x(F64State* S, double* f, double dt);
+cudaError_t f64_advect_v(F64State* S, double* f, const double* E, double dt);
+cudaError_t f64_field(F64State* S, const double* f, double* E_out);
+cudaError_t f64_get_field(F64State* S, double* E);
+cudaError_t f64_step(F64State* S, double* f, double dt, const double* Eext);
 
 // launchers, one family per line length N (defined in vog_advect_inst.cu, compiled once per N)
 typedef cudaError_t (*advect_launch_fn)(const AdvectArgs& a, int sym, bool vdir, int n_tiles, int threads,

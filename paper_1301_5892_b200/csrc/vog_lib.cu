@@ -612,6 +612,7 @@ struct vog_plan_s {
                                 // call on the plan left it (VXV steps may then skip their first field solve); NULL otherwise
     bool recx_valid; double recx_dt;
     long long launches;
+    vog::F64State* f64;         // double-precision mode (NEXT-2), created on the first *_f64 call
     float* f_buf;               // only for vog_run_host
     float* ext_buf;
 };
@@ -740,6 +741,7 @@ static void free_plan(vog_plan_s* P)
     if (!P) return;
     cudaFree(P->taps_x); cudaFree(P->taps_v); cudaFree(P->os_lam_x); cudaFree(P->os_lam_v); cudaFree(P->os_twv); cudaFree(P->os_cs64); cudaFree(P->ikt); cudaFree(P->ptw); cudaFree(P->cg4);
     cudaFree(P->g_buf);
+    vog::f64_destroy(P->f64);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
     cudaFree(P->part); cudaFree(P->partk); cudaFree(P->diag); cudaFree(P->rho); cudaFree(P->E_self);
@@ -1519,4 +1521,50 @@ extern "C" int vog_reset(vog_plan_t P)
 extern "C" int vog_debug_stamps(long long* out32) { return (int)cudaMemcpyFromSymbol(out32, vog::vog_stamps, sizeof(long long) * 32); }
 #endif
 
-extern "C" long long vog_launch_count(vog_plan_t P) { return P ? P->launches : -1; }
+extern "C" long long vog_launch_count(vog_plan_t P) { return P ? P->launches + vog::f64_launches(P->f64) : -1; }
+
+// ---- double-precision mode (NEXT-2; kernels and state in vog_f64.cu)
+static int f64_state(vog_plan_s* P)
+{
+    if (P->f64) return VOG_OK;
+    return vog::f64_create(&P->f64, &P->p, P->st, P->n_sm);
+}
+#define VOG_F64_ENTER(...) \
+    if (!P || __VA_ARGS__) return VOG_EINVAL; \
+    { const int rc = f64_state(P); if (rc != VOG_OK) return rc; }
+
+extern "C" int vog_shift_x_f64(vog_plan_t P, double* f_dev, const double* beta)
+{
+    VOG_F64_ENTER(!f_dev || !beta)
+    return cuda_status(vog::f64_shift(P->f64, f_dev, beta, false));
+}
+extern "C" int vog_shift_v_f64(vog_plan_t P, double* f_dev, const double* beta)
+{
+    VOG_F64_ENTER(!f_dev || !beta)
+    return cuda_status(vog::f64_shift(P->f64, f_dev, beta, true));
+}
+extern "C" int vog_advect_x_f64(vog_plan_t P, double* f_dev, double dt)
+{
+    VOG_F64_ENTER(!f_dev || !std::isfinite(dt))
+    return cuda_status(vog::f64_advect_x(P->f64, f_dev, dt));
+}
+extern "C" int vog_advect_v_f64(vog_plan_t P, double* f_dev, const double* E_dev, double dt)
+{
+    VOG_F64_ENTER(!f_dev || !E_dev || !std::isfinite(dt))
+    return cuda_status(vog::f64_advect_v(P->f64, f_dev, E_dev, dt));
+}
+extern "C" int vog_field_f64(vog_plan_t P, const double* f_dev, double* E_dev)
+{
+    VOG_F64_ENTER(!f_dev || !E_dev)
+    return cuda_status(vog::f64_field(P->f64, f_dev, E_dev));
+}
+extern "C" int vog_get_field_f64(vog_plan_t P, double* E_dev)
+{
+    if (!P || !E_dev || !vog::f64_has_field(P->f64)) return VOG_EINVAL;
+    return cuda_status(vog::f64_get_field(P->f64, E_dev));
+}
+extern "C" int vog_step_f64(vog_plan_t P, double* f_dev, double dt, const double* E_ext_dev)
+{
+    VOG_F64_ENTER(!f_dev || !std::isfinite(dt))
+    return cuda_status(vog::f64_step(P->f64, f_dev, dt, E_ext_dev));
+}

@@ -17,7 +17,9 @@ SPLIT_XVX, SPLIT_VXV = 0, 1
 
 EXPORTS = ("vog_plan", "vog_destroy", "vog_advect_x", "vog_advect_v", "vog_field", "vog_step",
            "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_run", "vog_run_host",
-           "vog_run_host_async", "vog_launch_count", "vog_strerror", "vog_plan_tune", "vog_reset", "vog_diagnostics")
+           "vog_run_host_async", "vog_launch_count", "vog_strerror", "vog_plan_tune", "vog_reset", "vog_diagnostics",
+           "vog_shift_x_f64", "vog_shift_v_f64", "vog_advect_x_f64", "vog_advect_v_f64", "vog_field_f64",
+           "vog_get_field_f64", "vog_step_f64")
 
 
 class vog_feq_t(ctypes.Structure):
@@ -69,6 +71,13 @@ def lib():
         L.vog_plan_tune.argtypes = [vp, ctypes.c_int, ctypes.c_int]
         L.vog_reset.argtypes = [vp]
         L.vog_diagnostics.argtypes = [vp, vp, vp]
+        L.vog_shift_x_f64.argtypes = [vp, vp, vp]
+        L.vog_shift_v_f64.argtypes = [vp, vp, vp]
+        L.vog_advect_x_f64.argtypes = [vp, vp, ctypes.c_double]
+        L.vog_advect_v_f64.argtypes = [vp, vp, vp, ctypes.c_double]
+        L.vog_field_f64.argtypes = [vp, vp, vp]
+        L.vog_get_field_f64.argtypes = [vp, vp]
+        L.vog_step_f64.argtypes = [vp, vp, ctypes.c_double, vp]
         for name in EXPORTS:
             if name not in ("vog_launch_count", "vog_strerror"):
                 getattr(L, name).restype = ctypes.c_int
@@ -153,6 +162,28 @@ class Plan:
 
     def shift_v_to(self, src, dst, beta):
         self._ck(lib().vog_shift_v_to(self._h, _ptr(src), _ptr(dst), _ptr(beta)), "vog_shift_v_to")
+
+    # double-precision mode (include/vog.h, NEXT-2): the same calls on fp64 arrays
+    def shift_x_f64(self, f, beta):
+        self._ck(lib().vog_shift_x_f64(self._h, _ptr(f), _ptr(beta)), "vog_shift_x_f64")
+
+    def shift_v_f64(self, f, beta):
+        self._ck(lib().vog_shift_v_f64(self._h, _ptr(f), _ptr(beta)), "vog_shift_v_f64")
+
+    def advect_x_f64(self, f, dt):
+        self._ck(lib().vog_advect_x_f64(self._h, _ptr(f), float(dt)), "vog_advect_x_f64")
+
+    def advect_v_f64(self, f, E, dt):
+        self._ck(lib().vog_advect_v_f64(self._h, _ptr(f), _ptr(E), float(dt)), "vog_advect_v_f64")
+
+    def field_f64(self, f, E):
+        self._ck(lib().vog_field_f64(self._h, _ptr(f), _ptr(E)), "vog_field_f64")
+
+    def get_field_f64(self, E):
+        self._ck(lib().vog_get_field_f64(self._h, _ptr(E)), "vog_get_field_f64")
+
+    def step_f64(self, f, dt, E_ext=None):
+        self._ck(lib().vog_step_f64(self._h, _ptr(f), float(dt), _ptr(E_ext)), "vog_step_f64")
 
     def run(self, f, dt, nsteps, E_ext_seq=None, merge=False, energy=None):
         self._ck(lib().vog_run(self._h, _ptr(f), float(dt), int(nsteps), _ptr(E_ext_seq), 1 if merge else 0,
