@@ -14,7 +14,7 @@
 #include <cmath>
 #include <new>
 
-#include "vog_internal.h"
+#include "vog_os2.cuh"
 
 namespace vog {
 
@@ -33,11 +33,14 @@ struct F64SetupArgs {
     const double* beta;
 };
 
-// S1 in fp64: integer shift b, taps a_j of the first row of A, and (v direction) the source shift s = E dt
+// S1 in fp64: integer shift b, taps a_j of the first row of A, and (v direction) the source shift s = E dt.
+// One thread per (line, tap): with one thread per line the 2d+2 products of 2d+1 factors ran one after the other in
+// every thread (33 us for 2048 lines, a quarter of the 2048^2 step).
 __global__ void __launch_bounds__(128) f64_setup_kernel(const F64SetupArgs s, double* __restrict__ taps, int* __restrict__ bsh,
                                                         double* __restrict__ ssh)
 {
-    const int l = blockIdx.x * blockDim.x + threadIdx.x;
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int l = (int)(idx / s.NT), k = (int)(idx - (long long)l * s.NT);
     if (l >= s.n_lines) return;
     double beta, sshift = 0.0;
     if (s.mode == 0) {
@@ -52,30 +55,31 @@ __global__ void __launch_bounds__(128) f64_setup_kernel(const F64SetupArgs s, do
     }
     const double fl = floor(beta);
     const double t = beta - fl;                      // b* in [0, 1)
-    int b;
-    if (fabs(fl) < 9.0e18) {                         // N is a power of two: mathematical mod by masking
-        b = (int)(__double2ll_rn(fl) & (long long)(s.N - 1));
-    } else {
-        double bm = fmod(fl, (double)s.N);
-        if (bm < 0.0) bm += (double)s.N;
-        b = (int)bm;
-        if (b >= s.N) b = 0;
-    }
-    bsh[l] = b;
-    if (ssh) ssh[l] = sshift;
     double* const out = taps + (long long)l * s.ls;
+    if (k == 0) {
+        int b;
+        if (fabs(fl) < 9.0e18) {                     // N is a power of two: mathematical mod by masking
+            b = (int)(__double2ll_rn(fl) & (long long)(s.N - 1));
+        } else {
+            double bm = fmod(fl, (double)s.N);
+            if (bm < 0.0) bm += (double)s.N;
+            b = (int)bm;
+            if (b >= s.N) b = 0;
+        }
+        bsh[l] = b;
+        if (ssh) ssh[l] = sshift;
+        if (s.ks == 1) { out[s.NT] = (double)b; out[s.NT + 1] = 0.0; }       // x rows: (taps, b, pad), see f64_x_kernel
+    }
+    const int j = k - s.JL;
+    double a = 0.0;
     if (!s.spline) {
         // Lagrange 2d+1: a_j = prod_{m != j} (b* - m) / (j - m), j = -d .. d+1 (zero outside: the kernels
-        // are compiled for 4, 10 and 18 taps)
-        for (int k = 0; k < s.NT; ++k) {
-            const int j = k - s.JL;
-            double a = 0.0;
-            if (j >= -s.d && j <= s.d + 1) {
-                a = 1.0;
-                for (int m = -s.d; m <= s.d + 1; ++m)
-                    if (m != j) a *= (t - (double)m) / (double)(j - m);
-            }
-            out[k * s.ks] = a;
+        // are compiled for 4, 10 and 18 taps).  The denominator is an integer of at most 17! < 2^53: exact.
+        if (j >= -s.d && j <= s.d + 1) {
+            double num = 1.0, den = 1.0;
+            for (int m = -s.d; m <= s.d + 1; ++m)
+                if (m != j) { num *= t - (double)m; den *= (double)(j - m); }
+            a = num / den;
         }
     } else {
         // cubic spline: a = m * g, m = (B(b*+1), B(b*), B(b*-1), B(b*-2)) at j = -1..2
@@ -83,55 +87,89 @@ __global__ void __launch_bounds__(128) f64_setup_kernel(const F64SetupArgs s, do
         const double mq[4] = {u * u * u / 6.0, (4.0 - 6.0 * t * t + 3.0 * t * t * t) / 6.0,
                               (1.0 + 3.0 * t + 3.0 * t * t - 3.0 * t * t * t) / 6.0, t * t * t / 6.0};
         const double rt3 = 1.7320508075688772935, q = rt3 - 2.0;
-        for (int k = 0; k < s.NT; ++k) {
-            const int j = k - s.JL;
-            double a = 0.0;
-            for (int p = 0; p < 4; ++p) {
-                const int n = j - (p - 1);
-                a += mq[p] * rt3 * pow(q, (double)(n < 0 ? -n : n));
-            }
-            out[k * s.ks] = a;
+        for (int p = 0; p < 4; ++p) {
+            const int n = j - (p - 1);
+            a += mq[p] * rt3 * pow(q, (double)(n < 0 ? -n : n));
         }
     }
+    out[k * s.ks] = a;
 }
 
 // ---------------------------------------------------------------------------------------------
-// x direction: a CTA lands a whole line in shared memory (Nx doubles), so in place needs no further care; a thread
-// computes CP = 4 consecutive cells from a register window (NT + 3 shared loads for 4 NT multiply-adds).
-template <int NT>
-__global__ void __launch_bounds__(512) f64_x_kernel(const double* src, double* dst, const int Nx,
-                                                    const int Nv, const int nt_rt, const int JL,
-                                                    const double* __restrict__ taps, const int* __restrict__ bsh)
+// x direction: a persistent CTA owns whole lines.  One thread lands the NEXT line and its row of taps in shared memory
+// with bulk asynchronous copies (cp.async.bulk, completion counted in bytes on an mbarrier) while the CTA computes the
+// current one from the other buffer (two buffers when 2 Nx doubles fit, one for 16384-cell lines).  The whole line is on
+// chip before its first store: in place needs no further care.
+// Taps row of a line: NT doubles, then the integer shift b as a double, then one unused double (16-byte multiple).
+//
+// Two consecutive cells per thread from 128-bit shared loads: a warp reads 512 contiguous bytes per instruction, the
+// conflict-free minimum of four wavefronts (four cells per thread from 64-bit loads put the lanes 32 bytes apart:
+// eight wavefronts per load, and the kernel ran at the speed of the shared-memory pipe, 2.3 times slower).  be = the
+// even base of the window, M = 1 when the first sample wanted is the odd one of its pair.
+template <int NT, int M>
+__device__ __forceinline__ void f64_x_cells(const double* __restrict__ line, const double* a, double* o, const int be,
+                                            const int tid, const int T, const int Nx)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* const line = reinterpret_cast<double*>(smem_raw);
-    double* const tp = line + Nx;
-    const int tid = threadIdx.x, T = blockDim.x, mask = Nx - 1;
-    const int nt = NT > 0 ? NT : nt_rt;
-    for (int l = blockIdx.x; l < Nv; l += gridDim.x) {
-        __syncthreads();                           // the previous line has been read by everybody
-        const double2* const s2 = reinterpret_cast<const double2*>(src + (size_t)l * Nx);
-        for (int i = tid; i < Nx / 2; i += T) reinterpret_cast<double2*>(line)[i] = s2[i];
-        if (tid < nt) tp[tid] = taps[(size_t)l * nt + tid];
-        __syncthreads();
-        const int b = bsh[l] - JL;
+    constexpr int NL = (NT + 1 + M + 1) / 2;       // 128-bit loads for NT + 1 samples starting at offset M
+    const int mask = Nx - 1;
+    for (int i0 = 2 * tid; i0 < Nx; i0 += 2 * T) {
+        double r[2 * NL];
+#pragma unroll
+        for (int n = 0; n < NL; ++n) {
+            const double2 v = *reinterpret_cast<const double2*>(line + ((i0 + be + 2 * n) & mask));
+            r[2 * n] = v.x;
+            r[2 * n + 1] = v.y;
+        }
+        double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll
+        for (int k = 0; k < NT; ++k) {
+            acc0 = fma(a[k], r[M + k], acc0);
+            acc1 = fma(a[k], r[M + k + 1], acc1);
+        }
+        *reinterpret_cast<double2*>(o + i0) = make_double2(acc0, acc1);
+    }
+}
+
+template <int NT>
+__global__ void __launch_bounds__(1024) f64_x_kernel(const double* src, double* dst, const int Nx, const int Nv,
+                                                     const int nt_rt, const int JL, const int nbuf,
+                                                     const double* __restrict__ taps)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int nt = NT > 0 ? NT : nt_rt, tw = nt + 2;
+    double* const lines = reinterpret_cast<double*>(smem_raw);                     // [nbuf][Nx]
+    double* const tps = lines + (size_t)nbuf * Nx;                                 // [nbuf][tw]
+    unsigned long long* const bars = reinterpret_cast<unsigned long long*>(tps + nbuf * f64::NTMAX + 2 * nbuf);
+    const int tid = threadIdx.x, T = blockDim.x, mask = Nx - 1, G = gridDim.x;
+    if (tid < nbuf) {                              // (one barrier per thread, see osx7_kernel)
+        os2::mbar_init(bars + tid, 1u);
+        os2::mbar_init_fence();
+    }
+    __syncthreads();
+    auto request = [&](const int l, const int buf) {
+        os2::mbar_expect_tx(bars + buf, (unsigned)(Nx * 8 + tw * 8));
+        os2::bulk_g2s(lines + (size_t)buf * Nx, src + (size_t)l * Nx, (unsigned)Nx * 8u, bars + buf);
+        os2::bulk_g2s(tps + buf * (f64::NTMAX + 2), taps + (size_t)l * tw, (unsigned)tw * 8u, bars + buf);
+    };
+    if (tid == 0 && blockIdx.x < Nv) request(blockIdx.x, 0);
+    unsigned ph0 = 0, ph1 = 0;
+    int it = 0;
+    for (int l = blockIdx.x; l < Nv; l += G, ++it) {
+        const int buf = nbuf == 2 ? (it & 1) : 0;
+        if (nbuf == 2 && tid == 0 && l + G < Nv) request(l + G, buf ^ 1);          // (that buffer was released by the
+                                                                                   // barrier that ended iteration it-1)
+        if (buf == 0) { os2::mbar_wait(bars, ph0); ph0 ^= 1u; }
+        else { os2::mbar_wait(bars + 1, ph1); ph1 ^= 1u; }
+        const double* const line = lines + (size_t)buf * Nx;
+        const double* const tp = tps + buf * (f64::NTMAX + 2);
+        const int b = (int)tp[nt] - JL;
         double* const o = dst + (size_t)l * Nx;
         if constexpr (NT > 0) {
             double a[NT];
 #pragma unroll
             for (int k = 0; k < NT; ++k) a[k] = tp[k];
-            for (int i0 = 4 * tid; i0 < Nx; i0 += 4 * T) {
-                double acc[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                for (int n = 0; n < NT + 3; ++n) {
-                    const double v = line[(i0 + b + n) & mask];
-#pragma unroll
-                    for (int c = 0; c < 4; ++c)
-                        if (n - c >= 0 && n - c < NT) acc[c] = fma(a[n - c], v, acc[c]);
-                }
-                reinterpret_cast<double2*>(o + i0)[0] = make_double2(acc[0], acc[1]);
-                reinterpret_cast<double2*>(o + i0)[1] = make_double2(acc[2], acc[3]);
-            }
+            if (b & 1) f64_x_cells<NT, 1>(line, a, o, b - 1, tid, T, Nx);
+            else f64_x_cells<NT, 0>(line, a, o, b, tid, T, Nx);
         } else {
             for (int i = tid; i < Nx; i += T) {
                 double acc = 0.0;
@@ -139,25 +177,29 @@ __global__ void __launch_bounds__(512) f64_x_kernel(const double* src, double* d
                 o[i] = acc;
             }
         }
+        __syncthreads();                           // the line has been read by everybody: its buffer may be refilled
+        if (nbuf == 1 && tid == 0 && l + G < Nv) request(l + G, 0);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // v direction, out of place: a thread owns a column and R = 16 consecutive rows; the rows it needs are read straight
-// from global memory (neighbouring columns with the same integer shift read the same 256-byte row segments; the
-// NT - 1 rows shared with the tile below come from L2).  delta-f source: f_eq,g(v_j) expm1(c_g s (2 (v_j -
+// from global memory (neighbouring columns with the same integer shift read the same 256-byte row segments).  delta-f source: f_eq,g(v_j) expm1(c_g s (2 (v_j -
 // mu_g) - s)) with s = E dt, summed over the Gaussians: f_eq(v - s) - f_eq(v) without the cancellation.
 struct F64Feq { int n; double amp[4], mu[4], c[4]; };
 
 template <int NT>
-__global__ void __launch_bounds__(128) f64_v_kernel(const double* __restrict__ src, double* __restrict__ dst, const int Nx,
+__global__ void __launch_bounds__(256) f64_v_kernel(const double* __restrict__ src, double* __restrict__ dst, const int Nx,
                                                     const int Nv, const int nt_rt, const int JL,
                                                     const double* __restrict__ taps, const int* __restrict__ bsh,
                                                     const double* __restrict__ ssh, const F64Feq fq, const double vmin,
                                                     const double dv)
 {
     constexpr int R = 16;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x, r0 = blockIdx.y * R, mask = Nv - 1;
+    // block = 32 columns x (blockDim.x / 32) warps, warp w takes rows r0 .. r0 + 15 of the block's row range: the
+    // NT - 1 rows a warp shares with the warp below it are hits in L1 (the loads go through the read-only path)
+    const int c = blockIdx.x * 32 + (threadIdx.x & 31), mask = Nv - 1;
+    const int r0 = (blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5)) * R;
     const int nt = NT > 0 ? NT : nt_rt;
     const int b = bsh[c] - JL;
     const double* const col = src + c;
@@ -188,9 +230,12 @@ __global__ void __launch_bounds__(128) f64_v_kernel(const double* __restrict__ s
         for (int r = 0; r < R; ++r) {
             const double v = vmin + (double)(r0 + r) * dv;
             double q = 0.0;
-            for (int g = 0; g < fq.n; ++g) {
-                const double u = v - fq.mu[g];
-                q += fq.amp[g] * exp(-fq.c[g] * u * u) * expm1(fq.c[g] * s * (2.0 * u - s));
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                if (g < fq.n) {
+                    const double u = v - fq.mu[g];
+                    q += fq.amp[g] * exp(-fq.c[g] * u * u) * expm1(fq.c[g] * s * (2.0 * u - s));
+                }
             }
             acc[r] += q;
         }
@@ -251,49 +296,67 @@ __global__ void __launch_bounds__(1024) f64_rho_kernel(const int Nx, const int n
 }
 
 // S9 in fp64, the Fourier solve of P:221 as two plain DFT sums.  tw[q] = (cos, sin)(2 pi q / Nx).
-//   forward, one warp per mode m = 1 .. Nx/2 - 1:  rho^_m = sum_i rt_i e^{-2 i pi m i / Nx};  E^_m = rho^_m / (i k_m),
-//   k_m = 2 pi m / L.  Modes 0 and Nx/2 are dropped (reading Q12).
-__global__ void __launch_bounds__(256) f64_dft_fwd_kernel(const int Nx, const double L, const double* __restrict__ rt,
-                                                          const double2* __restrict__ tw, double2* __restrict__ Ehat)
+//   forward, one CTA of 128 threads per mode m = 1 .. Nx/2 - 1:  rho^_m = sum_i rt_i e^{-2 i pi m i / Nx};
+//   E^_m = rho^_m / (i k_m), k_m = 2 pi m / L.  Modes 0 and Nx/2 are dropped (reading Q12).
+//   Sums in a fixed order (thread-strided partial sums, shuffle tree, the four warps in order): deterministic.
+__device__ __forceinline__ double2 f64_block_sum(double a, double b, double2* red)
 {
-    const int m = 1 + blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31, mask = Nx - 1;
-    if (m >= Nx / 2) return;
-    double sr = 0.0, si = 0.0;
-    for (int i = lane; i < Nx; i += 32) {
-        const double2 w = __ldg(tw + (int)(((long long)m * i) & mask));
-        const double r = rt[i];
-        sr = fma(r, w.x, sr);
-        si = fma(-r, w.y, si);
-    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        sr += __shfl_xor_sync(0xffffffffu, sr, o);
-        si += __shfl_xor_sync(0xffffffffu, si, o);
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
     }
-    if (lane == 0) {
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = make_double2(a, b);
+    __syncthreads();
+    double2 s = red[0];
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { s.x += red[w].x; s.y += red[w].y; }
+    return s;
+}
+
+// The root of a term is the product of two table entries, e^{-2 i pi m i / Nx} with i = i1 + 128 i2: the first factor
+// is the thread's own (loaded once), the second the same for the whole CTA (one broadcast load per term) -- a gather
+// of tw[(m i) mod Nx] per term made these two kernels 18 % of the 8192^2 step.
+__global__ void __launch_bounds__(128) f64_dft_fwd_kernel(const int Nx, const double L, const double* __restrict__ rt,
+                                                          const double2* __restrict__ tw, double2* __restrict__ Ehat)
+{
+    __shared__ double2 red[4];
+    const int m = 1 + blockIdx.x, mask = Nx - 1, T = blockDim.x;
+    const double2 w1 = __ldg(tw + (int)(((long long)m * threadIdx.x) & mask));
+    double sr = 0.0, si = 0.0;
+    for (int i2 = 0; i2 * T < Nx; ++i2) {
+        const double2 w2 = __ldg(tw + (int)(((long long)m * T * i2) & mask));
+        const double wx = w1.x * w2.x - w1.y * w2.y, wy = w1.x * w2.y + w1.y * w2.x;
+        const double r = rt[i2 * T + threadIdx.x];
+        sr = fma(r, wx, sr);
+        si = fma(-r, wy, si);
+    }
+    const double2 s = f64_block_sum(sr, si, red);
+    if (threadIdx.x == 0) {
         const double k = 2.0 * 3.14159265358979323846 * (double)m / L;
-        Ehat[m] = make_double2(si / k, -sr / k);   // (sr + i si) / (i k)
+        Ehat[m] = make_double2(s.y / k, -s.x / k);   // (sr + i si) / (i k)
     }
 }
 
-//   inverse, one warp per cell i:  E_i = (1/Nx) sum_m E^_m e^{+2 i pi m i / Nx} = (2/Nx) sum_{0 < m < Nx/2} Re(..)
-//   (E^_{Nx-m} is the conjugate of E^_m: rho is real).
-__global__ void __launch_bounds__(256) f64_dft_inv_kernel(const int Nx, const double2* __restrict__ Ehat,
+//   inverse, one CTA per cell i:  E_i = (1/Nx) sum_m E^_m e^{+2 i pi m i / Nx} = (2/Nx) sum_{0 < m < Nx/2} Re(..)
+//   (E^_{Nx-m} is the conjugate of E^_m: rho is real); m = m1 + 128 m2 factored the same way.
+__global__ void __launch_bounds__(128) f64_dft_inv_kernel(const int Nx, const double2* __restrict__ Ehat,
                                                           const double2* __restrict__ tw, double* __restrict__ E_a,
                                                           double* __restrict__ E_b)
 {
-    const int i = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31, mask = Nx - 1;
-    if (i >= Nx) return;
+    __shared__ double2 red[4];
+    const int i = blockIdx.x, mask = Nx - 1, T = blockDim.x;
+    const double2 w1 = __ldg(tw + (int)(((long long)threadIdx.x * i) & mask));
     double s = 0.0;
-    for (int m = 1 + lane; m < Nx / 2; m += 32) {
-        const double2 w = __ldg(tw + (int)(((long long)m * i) & mask));
-        const double2 e = Ehat[m];
-        s += e.x * w.x - e.y * w.y;
+    for (int m2 = 0; m2 * T < Nx / 2; ++m2) {
+        const int m = m2 * T + threadIdx.x;
+        const double2 w2 = __ldg(tw + (int)(((long long)m2 * T * i) & mask));
+        const double wx = w1.x * w2.x - w1.y * w2.y, wy = w1.x * w2.y + w1.y * w2.x;
+        const double2 e = m >= 1 ? Ehat[m] : make_double2(0.0, 0.0);
+        s += e.x * wx - e.y * wy;
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (lane == 0) {
-        const double v = 2.0 * s / (double)Nx;
+    const double2 t = f64_block_sum(s, 0.0, red);
+    if (threadIdx.x == 0) {
+        const double v = 2.0 * t.x / (double)Nx;
         E_a[i] = v;
         if (E_b) E_b[i] = v;
     }
@@ -341,14 +404,14 @@ static cudaError_t f64_setup(F64State* S, bool vdir, int mode, double dt, const 
     a.N = vdir ? Nv : Nx;
     a.mode = mode;
     a.spline = S->spline; a.d = S->d; a.NT = S->NT; a.JL = S->JL;
-    a.ls = vdir ? 1 : S->NT;
+    a.ls = vdir ? 1 : S->NT + 2;
     a.ks = vdir ? Nx : 1;
     a.dt = dt;
     a.dv = (S->p.vmax - S->p.vmin) / (double)Nv;
     a.delta = vdir ? a.dv : S->p.L / (double)Nx;
     a.vmin = S->p.vmin;
     a.E = E; a.Eext = Eext; a.beta = beta;
-    f64_setup_kernel<<<(a.n_lines + 127) / 128, 128, 0, S->st>>>(a, vdir ? S->taps_v : S->taps_x, vdir ? S->b_v : S->b_x,
+    f64_setup_kernel<<<(unsigned)(((long long)a.n_lines * a.NT + 127) / 128), 128, 0, S->st>>>(a, vdir ? S->taps_v : S->taps_x, vdir ? S->b_v : S->b_x,
                                                                   vdir ? S->ssh_v : nullptr);
     S->launches++;
     return cudaGetLastError();
@@ -358,18 +421,19 @@ template <int NT>
 static cudaError_t f64_x_launch_t(F64State* S, const double* src, double* dst)
 {
     const int Nx = S->p.Nx, Nv = S->p.Nv;
-    const size_t smem = sizeof(double) * ((size_t)Nx + f64::NTMAX);
+    const int nbuf = Nx <= 8192 ? 2 : 1;
+    const size_t smem = sizeof(double) * ((size_t)nbuf * Nx + nbuf * (f64::NTMAX + 2) + 2 * nbuf) + 16;
     cudaError_t e = set_max_smem((const void*)f64_x_kernel<NT>, smem);
     if (e != cudaSuccess) return e;
-    int threads = NT > 0 ? Nx / 4 : Nx;
-    if (threads > 512) threads = 512;
+    int threads = NT > 0 ? Nx / 2 : Nx;
+    if (threads > 1024) threads = 1024;
     if (threads < 64) threads = 64;
-    int per_sm = (int)((200 * 1024) / (smem + 1024));
+    int per_sm = (int)((220 * 1024) / (smem + 1024));
     if (per_sm > 2048 / threads) per_sm = 2048 / threads;
     if (per_sm < 1) per_sm = 1;
     int grid = S->n_sm * per_sm;
     if (grid > Nv) grid = Nv;
-    f64_x_kernel<NT><<<grid, threads, smem, S->st>>>(src, dst, Nx, Nv, S->NT, S->JL, S->taps_x, S->b_x);
+    f64_x_kernel<NT><<<grid, threads, smem, S->st>>>(src, dst, Nx, Nv, S->NT, S->JL, nbuf, S->taps_x);
     S->launches++;
     return cudaGetLastError();
 }
@@ -389,8 +453,10 @@ static cudaError_t f64_v_launch(F64State* S, const double* src, double* dst, boo
     fq.n = source ? S->p.feq.n : 0;
     for (int g = 0; g < 4; ++g) { fq.amp[g] = S->p.feq.amp[g]; fq.mu[g] = S->p.feq.mu[g]; fq.c[g] = S->p.feq.c[g]; }
     const double dv = (S->p.vmax - S->p.vmin) / (double)Nv;
-    const int threads = Nx < 128 ? Nx : 128;
-    const dim3 grid(Nx / threads, Nv / 16);
+    int warps = Nv / 16;                           // row groups of 16 per block (Nv >= 64: at least 4)
+    if (warps > 8) warps = 8;
+    const int threads = 32 * warps;
+    const dim3 grid(Nx / 32, Nv / (16 * warps));
     if (S->spline) f64_v_kernel<0><<<grid, threads, 0, S->st>>>(src, dst, Nx, Nv, S->NT, S->JL, S->taps_v, S->b_v, S->ssh_v, fq, S->p.vmin, dv);
     else if (S->NT == 4) f64_v_kernel<4><<<grid, threads, 0, S->st>>>(src, dst, Nx, Nv, S->NT, S->JL, S->taps_v, S->b_v, S->ssh_v, fq, S->p.vmin, dv);
     else if (S->NT == 10) f64_v_kernel<10><<<grid, threads, 0, S->st>>>(src, dst, Nx, Nv, S->NT, S->JL, S->taps_v, S->b_v, S->ssh_v, fq, S->p.vmin, dv);
@@ -419,7 +485,7 @@ int f64_create(F64State** out, const vog_params_t* p, cudaStream_t st, int n_sm)
     const size_t Nx = p->Nx, Nv = p->Nv;
     cudaError_t e = cudaSuccess;
     auto alloc = [&](void** q, size_t bytes) { if (e == cudaSuccess) e = cudaMalloc(q, bytes); };
-    alloc((void**)&S->taps_x, sizeof(double) * Nv * S->NT);
+    alloc((void**)&S->taps_x, sizeof(double) * Nv * (S->NT + 2));
     alloc((void**)&S->taps_v, sizeof(double) * Nx * S->NT);
     alloc((void**)&S->ssh_v, sizeof(double) * Nx);
     alloc((void**)&S->b_x, sizeof(int) * Nv);
@@ -495,8 +561,9 @@ cudaError_t f64_field(F64State* S, const double* f, double* E_out)
     while (nby > 1 && Nv / nby < 16) nby >>= 1;
     f64_density_kernel<<<dim3(Nx / 64, nby), 256, 0, S->st>>>(f, Nx, Nv / nby, S->part);
     f64_rho_kernel<<<1, Nx < 1024 ? Nx : 1024, 0, S->st>>>(Nx, nby, dv, S->part, S->rho, S->rt);
-    f64_dft_fwd_kernel<<<(Nx / 2 + 7) / 8, 256, 0, S->st>>>(Nx, S->p.L, S->rt, S->tw, S->Ehat);
-    f64_dft_inv_kernel<<<(Nx + 7) / 8, 256, 0, S->st>>>(Nx, S->Ehat, S->tw, S->E, E_out);
+    const int dft_threads = Nx / 2 < 128 ? Nx / 2 : 128;   // divides Nx / 2
+    f64_dft_fwd_kernel<<<Nx / 2 - 1, dft_threads, 0, S->st>>>(Nx, S->p.L, S->rt, S->tw, S->Ehat);
+    f64_dft_inv_kernel<<<Nx, dft_threads, 0, S->st>>>(Nx, S->Ehat, S->tw, S->E, E_out);
     S->launches += 4;
     S->E_valid = true;
     S->E_of = f;
