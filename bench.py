@@ -273,12 +273,11 @@ def main():
     alg_bytes = 8.0 * cells                      # one read + one write of f per advection
     ach = alg_bytes / (ms_x * 1e-3) / 1e9
     traffic, traffic_src = _traffic()
-    roofline = {"bound": "hbm", "kernel": "x-advection kernel, 2048-cell lines (2 of the step's 3 advections)",
+    roofline = {"bound": "hbm", "kernel": "x-advection kernel, 2048-cell lines (2 of 3 advections)",
                 "achieved": _r(ach, 5), "peak": peak, "unit": "GB/s", "frac": _r(ach / peak), "traffic": traffic,
                 "traffic_source": traffic_src, "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes,
                 "us_per_launch": _r(1e3 * ms_x), "us_v_call": _r(1e3 * ms_v), "us_field": _r(1e3 * ms_f),
-                "note": "16 MiB replica: L2-cold on entry (batch 256 MiB > L2), its writes stay in L2 until "
-                        "later replicas evict them; the HBM-resident figures are target_8192"}
+                "note": "16 MiB replica, L2-cold on entry, its writes stay in L2; HBM-resident sizes: target_8192"}
 
     extras = {}
     if not args.no_extras:
@@ -366,8 +365,8 @@ def main():
     e2e = {"value": _r(world * cells * p_steps / p_s, 5), "unit": UNIT, "h2d_bytes_per_step": 4 * cells,
            "d2h_bytes_per_step": 4 * cells + 4 * cfg.Nx, "steps": p_steps, "replicas_in_flight": NP,
            "serial_value": _r(serial_value, 5),
-           "note": "vog_run_host_async, 3 plans/streams round-robin: pinned host f -> device, 1 Strang step, f and E "
-                   "back to host, every step; serial_value: one replica at a time (vog_run_host, syncs each step)"}
+           "note": "vog_run_host_async on 3 plans/streams: pinned host f -> device, 1 step, f and E back, every step; "
+                   "serial_value: vog_run_host, one replica at a time"}
     plan.destroy()
 
     # ---- small grids (configs 0-1: launch/latency-bound: report steps/s)
@@ -400,7 +399,9 @@ def main():
                                    "v_out_of_place_frac": _r(r.get("v_out_of_place", {}).get("frac_hbm")),
                                    "step_frac_28B": _r(r["strang_step"]["frac_hbm"]),
                                    "direct_stencil_x_v_step": [_r(r.get("direct_stencil", {}).get(k, {}).get("frac_hbm"))
-                                                               for k in ("x_kernel_only", "v_out_of_place", "strang_step")]}
+                                                               for k in ("x_kernel_only", "v_out_of_place", "strang_step")],
+                                   "f64_mode_x_step": [_r(r.get("f64_mode", {}).get(k, {}).get("frac_hbm"))
+                                                       for k in ("x_kernel_only", "strang_step")]}
         roofline["target_8192"] = tgt.get("8192")
         roofline["at_16384"] = tgt.get("16384")
     # ---- oracle on the host cores (rank 0, N=1 only)
@@ -523,6 +524,17 @@ def sweep(torch, vog, stream, peak, sizes, kinds, emit, with_oracle):
                 st["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step(f, 1e-3), 2, 5), 28.0)
                 row["direct_stencil"] = st
                 plan.destroy()
+            if N >= 1024 and N * N * 8 * 3 < 160e9:
+                # double-precision mode (vog_*_f64): 16 B per cell and advection, 56 B per cell and
+                # Strang step (3 advections + the density read)
+                plan = vog.Plan(N, N, 1.0, -1.0, 1.0, kind, order, stream=stream)
+                f64 = f.double()
+                d = {"x_kernel_only": _time_kernel(torch, stream, lambda: plan.advect_x_f64(f64, 0.01),
+                                                   lambda m, b: rec(m, b, 16.0))}
+                d["strang_step"] = rec(*_time_calls(torch, stream, lambda: plan.step_f64(f64, 1e-3), 2, 5), 56.0)
+                row["f64_mode"] = d
+                plan.destroy()
+                del f64
             if fo is not None:
                 ot = {}
                 for name, fn in (("x", orc.shift_x), ("v", orc.shift_v)):
@@ -549,8 +561,8 @@ def cpu_baseline(cfg):
     orc.build()
     val, n, secs = _oracle_step_rate(orc, cfg, 1, 3, 25.0)
     return {"value": _r(val, 5), "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "sample": "best of %d %dx%d Strang steps of one replica after 1 warm-up step (%.1f s of oracle work; "
-                      "double, direct stencils, naive-DFT field)" % (n, cfg.Nx, cfg.Nv, secs)}
+            "sample": "best of %d %dx%d Strang steps of one replica after 1 warm-up (%.1f s of oracle work; fp64)"
+                      % (n, cfg.Nx, cfg.Nv, secs)}
 
 
 if __name__ == "__main__":
