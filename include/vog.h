@@ -29,7 +29,7 @@ extern "C" {
 
 typedef struct vog_plan_s* vog_plan_t; /* opaque, library-owned */
 
-enum { VOG_OK = 0, VOG_EINVAL = -1, VOG_ENOMEM = -2, VOG_ECUDA = -3, VOG_EUNSUPPORTED = -4 };
+enum { VOG_OK = 0, VOG_EINVAL = -1, VOG_ENOMEM = -2, VOG_ECUDA = -3, VOG_EUNSUPPORTED = -4, VOG_ETOOLARGE = -5 };
 enum { VOG_LAGRANGE = 0, VOG_BSPLINE = 1 }; /* order = polynomial degree: Lagrange odd 1..17, B-spline 3 (Q6) */
 enum { VOG_SPLIT_XVX = 0, VOG_SPLIT_VXV = 1 };
 
@@ -212,6 +212,23 @@ int vog_advect_v_f64(vog_plan_t plan, double* f_dev, const double* E_dev, double
 int vog_field_f64(vog_plan_t plan, const double* f_dev, double* E_dev);
 int vog_get_field_f64(vog_plan_t plan, double* E_dev);
 int vog_step_f64(vog_plan_t plan, double* f_dev, double dt, const double* E_ext_dev);
+
+/* The self-consistent field WITHOUT a plan and without any allocation, for callers that cannot call cudaMalloc (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same definition as vog_field (P:157, 172,
+ * 205-211, 221): rho_i = dv sum_j f[j][i] with dv = (vmax - vmin) / Nv, zero mean, E^_m = rho^_m / (i k_m) with modes 0
+ * and Nx/2 dropped; f_dev holds Nx*Nv floats in the layout above, E_dev receives Nx floats (both caller-owned device
+ * memory); enqueued on cuda_stream (a cudaStream_t as void*, NULL = the legacy default stream), asynchronous.  The
+ * density kernel's slab sums and the O(Nx) work arrays of the solve live in a file-scope device array of 416 KB that
+ * every GPU loading the library holds until the process exits; the call makes no cudaMalloc / cudaFree and calls no
+ * allocating library routine.  Limit: Nx <= VOG_NOALLOC_MAX_NX, beyond it VOG_ETOOLARGE (use a plan and vog_field).
+ * Nx, Nv powers of two, Nx >= 64, 64 <= Nv <= 16384, L > 0, vmax > vmin, non-NULL pointers: else VOG_EINVAL.
+ * ALL calls in the process share the one scratch array (per GPU), which keeps the last call's contents; every call
+ * overwrites each word before reading it, so nothing needs clearing, but calls that OVERLAP on the same GPU (different
+ * streams) race on it: keep them on one stream or order them with events.  The sums are plain fp64 DFT sums, O(Nx^2):
+ * meant for the moderate Nx it is limited to, not as a replacement of vog_field. */
+#define VOG_NOALLOC_MAX_NX 4096
+int vog_field_noalloc(const float* f_dev, int Nx, int Nv, double L, double vmin, double vmax, float* E_dev,
+                      void* cuda_stream);
 
 /* Number of kernels the library launched on this plan since creation (for accounting). */
 long long vog_launch_count(vog_plan_t plan);

@@ -732,6 +732,7 @@ extern "C" const char* vog_strerror(int status)
         case VOG_ENOMEM: return "out of device memory";
         case VOG_ECUDA: return "CUDA error";
         case VOG_EUNSUPPORTED: return "unsupported interpolation kind/order";
+        case VOG_ETOOLARGE: return "size beyond the fixed scratch of the allocation-free entry point (VOG_NOALLOC_MAX_NX)";
     }
     return "unknown status";
 }

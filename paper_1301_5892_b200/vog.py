@@ -11,7 +11,8 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvog.so")
 
-OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ETOOLARGE = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_NX = 4096
 LAGRANGE, BSPLINE = 0, 1
 SPLIT_XVX, SPLIT_VXV = 0, 1
 
@@ -19,7 +20,7 @@ EXPORTS = ("vog_plan", "vog_destroy", "vog_advect_x", "vog_advect_v", "vog_field
            "vog_get_field", "vog_shift_x", "vog_shift_v", "vog_shift_v_to", "vog_run", "vog_run_host",
            "vog_run_host_async", "vog_launch_count", "vog_strerror", "vog_plan_tune", "vog_reset", "vog_diagnostics",
            "vog_shift_x_f64", "vog_shift_v_f64", "vog_advect_x_f64", "vog_advect_v_f64", "vog_field_f64",
-           "vog_get_field_f64", "vog_step_f64")
+           "vog_get_field_f64", "vog_step_f64", "vog_field_noalloc")
 
 
 class vog_feq_t(ctypes.Structure):
@@ -78,6 +79,8 @@ def lib():
         L.vog_field_f64.argtypes = [vp, vp, vp]
         L.vog_get_field_f64.argtypes = [vp, vp]
         L.vog_step_f64.argtypes = [vp, vp, ctypes.c_double, vp]
+        L.vog_field_noalloc.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                        ctypes.c_double, vp, vp]
         for name in EXPORTS:
             if name not in ("vog_launch_count", "vog_strerror"):
                 getattr(L, name).restype = ctypes.c_int
@@ -108,6 +111,16 @@ def make_params(Nx, Nv, L, vmin, vmax, kind=LAGRANGE, order=17, feq=(), split=SP
         if g < 4:
             p.feq.amp[g], p.feq.mu[g], p.feq.c[g] = float(amp), float(mu), float(c)
     return p
+
+
+def field_noalloc(f, Nx, Nv, L, vmin, vmax, E, stream=None):
+    """vog_field_noalloc (include/vog.h): the self-consistent field without a plan and without any allocation; scratch in
+    a fixed device array shared by all calls (Nx <= NOALLOC_MAX_NX; overlapping calls race).  Returns nothing; raises
+    VogError (ETOOLARGE beyond the limit)."""
+    sp = None if stream is None else ctypes.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+    rc = lib().vog_field_noalloc(_ptr(f), int(Nx), int(Nv), float(L), float(vmin), float(vmax), _ptr(E), sp)
+    if rc != OK:
+        raise VogError(rc, "vog_field_noalloc")
 
 
 class Plan:
