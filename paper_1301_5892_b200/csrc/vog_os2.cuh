@@ -1,21 +1,20 @@
-// vog_os2.cuh -- overlap-save advection kernels, second generation (line length N >= 1024;
-// SURVEY.md 8(a) S2-S7).  Product code; shares nothing with oracle/.
+// vog_os2.cuh -- overlap-save advection kernels (line length N >= 1024).
+// Product code; shares nothing with oracle/.
 //
-// Same method as vog_os.cuh (the circulant product of P:98-100 taken block-wise in Fourier space, P:131-149:
-// blocks of LB = 256 samples of the rolled line, V = 224 kept, H = 16 discarded on either side), but the
-// real-data trick is different.  The interpolation matrix is REAL, so two blocks A, B of the SAME line share
-// the symbol lambda and can ride one complex transform:  z_n = A_n + i B_n,  Z = FFT_256(z),
-// Z_k *= lambda_k (lambda_{256-k} = conj lambda_k),  z' = IFFT(Z)  =>  A' = Re z', B' = Im z'.
-// Compared with the even/odd packing of vog_os.cuh there is no untangle / re-tangle stage, no "special"
-// mirror item, no divergence, and a work item is ONE radix-16 butterfly (16 complex = 32 registers) in every
-// phase, so the kernels fit 64 registers and run at twice the occupancy:
+// The circulant product of P:98-100 taken block-wise in Fourier space: blocks of LB = 256 samples of the
+// rolled line, V kept, H_lo discarded on the left (geometry (V, H_lo) = (232, 8) for Lagrange plans, (228, 14) for the
+// cubic spline; template parameters).  The interpolation matrix is REAL, so two blocks A, B of the SAME line share the
+// symbol lambda and ride one complex transform:  z_n = A_n + i B_n,  Z = FFT_256(z),  Z_k *= lambda_k
+// (lambda_{256-k} = conj lambda_k),  z' = IFFT(Z)  =>  A' = Re z', B' = Im z'.  A work item is ONE radix-16 butterfly
+// (16 complex = 32 registers) in every phase:
 //   pass A   : item (pair, t):  n = t + 16 k  -> radix 16 over k, times W_256^{t k1}, stored at [k1][t]
 //   middle   : item (pair, g = k1): radix 16 over t -> Z_{g + 16 k2}; times lambda; inverse radix 16
-//   inverse A: item (pair, j): times conj W, inverse radix 16 over k1 -> z'_{j + 16 m}; m = 1..14 are the
-//              kept samples of both blocks (uniform over the threads), stored straight to global memory.
-// Every phase has 16 items per pair, every item touches only its own 16 scratch slots, and a thread lands
-// (cp.async, 4 bytes: the full integer shift b of P:107 is applied by addressing, no alignment residue) exactly
-// the samples that it transforms in pass A.
+//   inverse A: item (pair, j): times conj W, inverse radix 16 over k1 -> z'_{j + 16 m}; the kept samples of both
+//              blocks go straight to global memory.
+// Every phase has 16 items per pair and every item touches only its own 16 scratch slots.  The full integer shift b of
+// P:107 is applied by addressing.  Kernels in this file: osx7_kernel (x, default: per-pair windows landed by bulk
+// copies), osx6_kernel (x, whole lines landed by bulk copies; 16384-cell lines), osv7_kernel (v, default: 16-column
+// strips, three groups per CTA, raw rows by 2-D tensor copies), osv6_kernel / osv4_kernel (v fallbacks).
 #pragma once
 #include <cuda.h>
 
