@@ -180,6 +180,11 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *          zero-mean modifications on rho and on E; 2 = trapezoidal rule without them (rho - 1, P:213;
  *          minus the equilibrium's mass in delta-f mode) -- the variant whose drift the paper shows in Fig. 1.
  *          This one DOES change results: it is the paper's other solver, not a launch shape.
+ *   29     grids up to 256 x 256 only: 1 = vog_run executes the whole run as ONE persistent kernel on a thread-block
+ *          cluster that keeps the grid in shared memory for all nsteps (the circulant products in
+ *          their direct form, the same matrices up to rounding), same sequences, E_ext and energy semantics as the
+ *          launch-per-kernel loop; 0 = that loop (default: vog_run(merge = 0) stays bit-identical to vog_step).
+ *          Ignored while the trapezoid field solver (28) is selected.
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

@@ -54,7 +54,8 @@ def build(force=False, verbose=False):
             (os.path.join(CSRC, "vog_os.cu"), os.path.join(OBJ, "vog_os.o"), []),
             (os.path.join(CSRC, "vog_stencil.cu"), os.path.join(OBJ, "vog_stencil.o"), []),
             (os.path.join(CSRC, "vog_f64.cu"), os.path.join(OBJ, "vog_f64.o"), []),
-            (os.path.join(CSRC, "vog_noalloc.cu"), os.path.join(OBJ, "vog_noalloc.o"), [])]
+            (os.path.join(CSRC, "vog_noalloc.cu"), os.path.join(OBJ, "vog_noalloc.o"), []),
+            (os.path.join(CSRC, "vog_small.cu"), os.path.join(OBJ, "vog_small.o"), [])]
     for n in SIZES:
         jobs.append((os.path.join(CSRC, "vog_advect_inst.cu"), os.path.join(OBJ, "vog_advect_%d.o" % n),
                      ["-DVOG_N=%d" % n]))

@@ -155,6 +155,22 @@ cudaError_t stx_launch(const OsArgs& a, int spline, int d, const float* taps, in
 int stx_occupancy(int spline, int d, int threads, size_t smem);
 cudaError_t stv_launch(const OsArgs& a, int spline, int d, const float* taps, cudaStream_t st);
 
+// ---- one persistent kernel for a whole run of a small grid (vog_small.cu, NEXT-1; Nx, Nv <= 256)
+struct SmallArgs {
+    float* f;                  // [Nv][Nx], in place
+    float* E_out;              // [Nx] self-consistent field of the last field solve (or NULL)
+    const float* E_init;       // VXV: field for the first half step (NULL: solved from f first)
+    const float* E_ext_seq;    // [n_vadv][Nx] or NULL
+    double* energy;            // [n_field] or NULL
+    int Nx, Nv, rpc;           // rpc = rows per CTA = Nv / cluster size
+    int split, merge, nsteps, spline, d, ng;
+    double dt, L, vmin, dv, dx;
+    double amp[4], mu[4], c[4];
+    float cg[4];
+};
+int small_run_cluster(int Nx, int Nv);
+cudaError_t small_run_launch(const SmallArgs& a, cudaStream_t st);
+
 // ---- double-precision mode (vog_f64.cu, NEXT-2): its own tables and kernels, created on the first *_f64 call of a plan
 struct F64State;
 int f64_create(F64State** out, const vog_params_t* p, cudaStream_t st, int n_sm);

@@ -588,6 +588,7 @@ struct vog_plan_s {
     float* g_buf;                  // second grid for the out-of-place v kernel (allocated on first use)
     int os2x_lpi, os3x_occ, os2v_gpc;      // x: lines per iteration, cached occupancy; v: pairs per CTA (0 = default)
     vog::OsSetupArgs vsetup;               // v-advection: shift source (E, E_ext, beta, dt) of the pending advection
+    int small_run;                         // vog_run on grids up to 256 x 256 as one persistent kernel (vog_small.cu): 0 / 1
     int solver;                            // field solve: 0 = Fourier (default), 1 = trapezoid + zero mean, 2 = trapezoid, rho - 1
     double feq_mass, feq_kin;              // dv sum_j f_eq(v_j) and (1/2) L dv sum_j v_j^2 f_eq(v_j) (0 in full-f mode)
     double *partk, *diag;                  // kinetic-energy slab sums [nby_max][Nx]; 5 doubles of scratch
@@ -989,6 +990,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
         case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
         case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
+        case 29: if (value < 0 || value > 1 || P->p.Nx > 256 || P->p.Nv > 256) return VOG_EINVAL; P->small_run = value; break;
         case 28: if (value < 0 || value > 2) return VOG_EINVAL; P->solver = value; P->E_of = nullptr; P->E_valid = false; break;
         case 27: if (value < 0 || value > 1) return VOG_EINVAL; P->method = value; P->recx_valid = false; P->E_of = nullptr; break;
         default: return VOG_EINVAL;
@@ -1415,6 +1417,27 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
     t_pdl = P->pdl != 0;
     const int Nx = P->p.Nx;
     cudaError_t e = cudaSuccess;
+    if (P->small_run && P->solver == 0) {
+        // the whole run as ONE persistent cluster kernel (vog_small.cu; vog_plan_tune(29, 1)): same sequences
+        vog::SmallArgs a;
+        const int Nv = P->p.Nv, C = vog::small_run_cluster(Nx, Nv);
+        a.f = f_dev; a.E_out = P->E_self;
+        a.E_init = (P->p.split == VOG_SPLIT_VXV && P->E_of == f_dev) ? P->E_self : nullptr;
+        a.E_ext_seq = E_ext_seq_dev; a.energy = energy_dev;
+        a.Nx = Nx; a.Nv = Nv; a.rpc = Nv / C;
+        a.split = P->p.split; a.merge = merge; a.nsteps = nsteps;
+        a.spline = P->p.kind == VOG_BSPLINE; a.d = a.spline ? 0 : (P->p.order - 1) / 2; a.ng = P->p.feq.n;
+        a.dt = dt; a.L = P->p.L; a.vmin = P->p.vmin; a.dv = (P->p.vmax - P->p.vmin) / (double)Nv; a.dx = P->p.L / (double)Nx;
+        for (int g = 0; g < 4; ++g) {
+            a.amp[g] = P->p.feq.amp[g]; a.mu[g] = P->p.feq.mu[g]; a.c[g] = P->p.feq.c[g];
+            a.cg[g] = g < a.ng ? (float)P->p.feq.c[g] : 0.0f;
+        }
+        e = vog::small_run_launch(a, P->st);
+        P->launches++;
+        P->E_valid = e == cudaSuccess;
+        P->E_of = (e == cudaSuccess && P->p.split == VOG_SPLIT_VXV) ? f_dev : nullptr;
+        return cuda_status(e);
+    }
     float* g = f_dev;
     if (P->os_v) {
         e = ensure_gbuf(P);
