@@ -421,29 +421,34 @@ def main():
 
 def small_grids(torch, vog, stream, emit):
     """Configs 0 and 1 (64^2 full-f, 256^2 delta-f): Strang steps per second through vog_run (one host call for the
-    whole run, energies on the device), the configs' own step counts."""
+    whole run, energies on the device), the configs' own step counts; first as the launch-per-kernel loop, then as ONE
+    persistent cluster kernel for the whole run (vog_plan_tune(29, 1), csrc/vog_small.cu)."""
     res = {}
     for idx in (0, 1):
         cfg = inputs.config(idx)
-        plan = vog.Plan.from_config(cfg, stream=stream)
         f0 = torch.from_numpy(inputs.initial_f(cfg)).cuda()
         en = torch.empty(cfg.steps, device="cuda", dtype=torch.float64)
-        best = None
-        for rep in range(4):
-            f = f0.clone()
-            stream.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            plan.run(f, cfg.dt, cfg.steps, None, False, en)
-            e1.record(stream)
-            stream.synchronize()
-            t = e0.elapsed_time(e1)
-            if rep > 0:
-                best = t if best is None else min(best, t)
-        plan.destroy()
-        res[cfg.name] = _r(cfg.steps / (best * 1e-3))
-        emit({"small_grid": cfg.name, "steps": cfg.steps, "ms_run": best, "steps_per_s": cfg.steps / (best * 1e-3),
-              "us_per_step": 1e3 * best / cfg.steps})
+        for one_kernel in (0, 1):
+            plan = vog.Plan.from_config(cfg, stream=stream)
+            if one_kernel:
+                plan.tune(29, 1)
+            best = None
+            for rep in range(4):
+                f = f0.clone()
+                stream.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                plan.run(f, cfg.dt, cfg.steps, None, False, en)
+                e1.record(stream)
+                stream.synchronize()
+                t = e0.elapsed_time(e1)
+                if rep > 0:
+                    best = t if best is None else min(best, t)
+            plan.destroy()
+            name = cfg.name + ("_one_kernel" if one_kernel else "")
+            res[name] = _r(cfg.steps / (best * 1e-3))
+            emit({"small_grid": name, "steps": cfg.steps, "ms_run": best, "steps_per_s": cfg.steps / (best * 1e-3),
+                  "us_per_step": 1e3 * best / cfg.steps})
     return res
 
 

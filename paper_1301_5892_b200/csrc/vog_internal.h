@@ -135,6 +135,18 @@ struct OsSetupArgs {
     const double* beta;
     const double2* cs64;       // [OS_LB] (cos, sin)(2 pi j / OS_LB) in fp64
     float2* lam;
+    // field solve fused into the v kernel (osv7_kernel, one piece per CTA; vog_lib.cu field_then_v): fpart != NULL => E
+    // is not read but COMPUTED from the density kernel's slab sums as the circular convolution of rho with the Green's
+    // function of the Fourier solve (green: [N lines] doubles), and written to E_out / rho_out by the strip's first CTA
+    const double* fpart;       // [n_lines] rho of the density kernel (its last blocks add the slabs; NULL: E is given)
+    const double* green;       // [n_lines]
+    int nby;
+    float* E_out;              // [n_lines] self-consistent field (without E_ext)
+    double* rho_out;           // [n_lines]
+    double* energy_out;        // (1/2) dx sum E^2 of this field solve, or NULL
+    double* e_part;            // [n_lines / 16] per-strip sums of E^2 (scratch of the energy reduction)
+    unsigned* ticket;          // arrival counter of the energy reduction (zero between launches)
+    double half_dx;
 };
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st);

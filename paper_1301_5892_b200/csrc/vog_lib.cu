@@ -198,9 +198,12 @@ __global__ void shift_setup_x_kernel(const SetupArgs s)
 template <bool KIN>
 __global__ void __launch_bounds__(256) density_partial_kernel(const float* __restrict__ f, int Nx, int Nv,
                                                               int rows_per_block, double* __restrict__ part,
-                                                              double* __restrict__ partk, double vmin, double dvd)
+                                                              double* __restrict__ partk, double vmin, double dvd,
+                                                              unsigned* __restrict__ tick, double* __restrict__ rho_out,
+                                                              double rho_scale)
 {
     __shared__ double red[8][32];
+    __shared__ unsigned last_s;
     __shared__ double redk[KIN ? 8 : 1][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int xl = lane & 7, rl = lane >> 3;
@@ -251,6 +254,29 @@ __global__ void __launch_bounds__(256) density_partial_kernel(const float* __res
         }
         part[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = s;
         if constexpr (KIN) partk[(size_t)blockIdx.y * Nx + blockIdx.x * 32 + threadIdx.x] = k;
+    }
+    if (tick) {
+        // (fused field solve, field_then_v: the v kernel's CTAs all need all of rho.)  The last block of a column group
+        // to arrive adds the group's slabs in the order of poisson_kernel -- slabs 0..7, slabs 8..15, then the two
+        // halves -- and writes rho_i = dv * sum: the same value whichever block comes last.
+        if (threadIdx.x < 32) {
+            __threadfence();
+            __syncwarp();
+            if (threadIdx.x == 0) last_s = atomicAdd(tick + blockIdx.x, 1u);
+            __syncwarp();
+            if (last_s == gridDim.y - 1u) {
+                __threadfence();
+                const int i = blockIdx.x * 32 + threadIdx.x, nby = (int)gridDim.y;
+                double v[16];
+#pragma unroll
+                for (int y = 0; y < 16; ++y) v[y] = y < nby ? __ldcg(part + (size_t)y * Nx + i) : 0.0;
+                double a = v[0], b = v[8];
+#pragma unroll
+                for (int y = 1; y < 8; ++y) { a += v[y]; b += v[8 + y]; }
+                rho_out[i] = (nby > 8 ? a + b : a) * rho_scale;
+                if (threadIdx.x == 0) tick[blockIdx.x] = 0u;
+            }
+        }
     }
 #ifdef VOG_STAMPS
     if (blockIdx.x == gridDim.x - 1 && blockIdx.y == gridDim.y - 1) VOG_STAMP(9);
@@ -564,6 +590,21 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     VOG_STAMP(6);
 }
 
+// Green's function of the Fourier field solve: E_i = sum_j G_{i-j} rho_j with
+// G_n = (1/Nx) sum_{m != 0, Nx/2} e^{2 pi i m n / Nx} / (i k_m) = L / (pi Nx) sum_{m=1}^{Nx/2-1} sin(2 pi m n / Nx) / m,
+// k_m = 2 pi m / L.  fp64, small terms first; a plan constant (osv7_kernel's fused field solve reads it).
+__global__ void green_kernel(int Nx, double L, double* __restrict__ G)
+{
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= Nx) return;
+    double s = 0.0;
+    for (int m = Nx / 2 - 1; m >= 1; --m) {
+        const int r = (int)(((long long)m * n) & (long long)(Nx - 1));
+        s += sinpi(2.0 * (double)r / (double)Nx) / (double)m;
+    }
+    G[n] = s * L / (3.14159265358979323846 * (double)Nx);
+}
+
 }  // namespace vog
 
 // ==========================================================================================
@@ -604,6 +645,9 @@ struct vog_plan_s {
     double* part;               // density partials [nby][Nx]
     double* rho;                // [Nx]
     float* E_self;              // [Nx] last self-consistent field
+    double* green;              // [Nx] Green's function of the Fourier solve (plans whose v kernel can solve the field itself)
+    double* e_part;             // [Nx / 16] + ticket word: energy reduction of the fused field solve
+    int fuse_field;             // steps: density -> v kernel with the field solve inside (no Poisson launch); 0 / 1
     float *feq_tab, *vmu_tab;   // [ng][Nv]
     int nby, nby_max;           // density: row slabs per column group (tunable up to the allocated nby_max)
     int lognl_x, lognl_v, thr_x, thr_v;
@@ -746,7 +790,7 @@ static void free_plan(vog_plan_s* P)
     vog::f64_destroy(P->f64);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
-    cudaFree(P->part); cudaFree(P->partk); cudaFree(P->diag); cudaFree(P->rho); cudaFree(P->E_self);
+    cudaFree(P->part); cudaFree(P->partk); cudaFree(P->diag); cudaFree(P->rho); cudaFree(P->E_self); cudaFree(P->green); cudaFree(P->e_part);
     cudaFree(P->feq_tab); cudaFree(P->vmu_tab); cudaFree(P->f_buf); cudaFree(P->ext_buf);
     delete P;
 }
@@ -927,6 +971,20 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         if (e == cudaSuccess) e = cudaMemcpyAsync(P->vmu_tab, vt.data(), sizeof(float) * vt.size(), cudaMemcpyHostToDevice, P->st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
     }
+    if (e == cudaSuccess && P->os_v && Nx / 16 <= P->n_sm) {
+        // the default v kernel runs one piece per CTA on this grid: it can solve the field itself (field_then_v)
+        e = cudaMalloc((void**)&P->green, sizeof(double) * Nx);
+        // e_part: [Nx / 16] strip sums of E^2 | 1 word: ticket of the energy reduction | [Nx / 32] tickets of the density kernel
+        if (e == cudaSuccess) e = cudaMalloc((void**)&P->e_part, sizeof(double) * (Nx / 16 + 1) + sizeof(unsigned) * (Nx / 32));
+        if (e == cudaSuccess) e = cudaMemsetAsync(P->e_part, 0, sizeof(double) * (Nx / 16 + 1) + sizeof(unsigned) * (Nx / 32), P->st);
+        if (e == cudaSuccess) {
+            green_kernel<<<(Nx + 127) / 128, 128, 0, P->st>>>(Nx, p->L, P->green);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
+        if (e == cudaSuccess) P->fuse_field = 1;
+        else { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
+    }
     if (e != cudaSuccess) { free_plan(P); cudaGetLastError(); return VOG_ECUDA; }
     *out = P;
     return VOG_OK;
@@ -990,6 +1048,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 24: if (value < 1 || value > P->nby_max || (value & (value - 1)) || Nv / value < 32) return VOG_EINVAL; P->nby = value; break;
         case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
         case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
+        case 30: if (value < 0 || value > 1 || (value == 1 && !P->green)) return VOG_EINVAL; P->fuse_field = value; break;
         case 29: if (value < 0 || value > 1 || P->p.Nx > 256 || P->p.Nv > 256) return VOG_EINVAL; P->small_run = value; break;
         case 28: if (value < 0 || value > 2) return VOG_EINVAL; P->solver = value; P->E_of = nullptr; P->E_valid = false; break;
         case 27: if (value < 0 || value > 1) return VOG_EINVAL; P->method = value; P->recx_valid = false; P->E_of = nullptr; break;
@@ -1013,6 +1072,7 @@ static cudaError_t run_setup(vog_plan_s* P, bool vdir, int mode, double dt, cons
     P->launches++;
     if (vdir ? P->os_v : P->os_x) {
         OsSetupArgs s;
+        std::memset(&s, 0, sizeof(s));
         s.n_lines = vdir ? Nx : Nv;
         s.N = vdir ? Nv : Nx;
         s.mode = mode;
@@ -1258,10 +1318,10 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
     cudaError_t e;
     if (diag_out)
         e = launch_pdl(density_partial_kernel<true>, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part, P->partk,
-                       P->p.vmin, dv);
+                       P->p.vmin, dv, (unsigned*)nullptr, (double*)nullptr, 0.0);
     else
         e = launch_pdl(density_partial_kernel<false>, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part,
-                       (double*)nullptr, 0.0, 0.0);
+                       (double*)nullptr, 0.0, 0.0, (unsigned*)nullptr, (double*)nullptr, 0.0);
     if (e != cudaSuccess) return e;
     P->launches += 2;
     P->E_valid = true;
@@ -1290,6 +1350,43 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
                    P->rho, P->E_self, E_out, dg);
     if (e == cudaSuccess && energy_out)
         e = cudaMemcpyAsync(energy_out, dg, sizeof(double), cudaMemcpyDeviceToDevice, P->st);
+    return e;
+}
+
+// field solve from src, then the v-advection src -> dst over dts with E + E_ext (S8, S9, S1-S7).  On grids whose default
+// v kernel runs one piece per CTA (Nx / 16 <= SMs) the Poisson launch is dropped: the density kernel's slab sums go
+// straight to the v kernel, where every CTA computes E on its own 16 columns as the circular convolution of rho with the
+// Green's function of the same Fourier solve (fp64) and the strip's first CTA publishes rho, E_self and the energy share.
+static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, double dts, const float* Eext,
+                                double* energy_out)
+{
+    const bool fuse = P->fuse_field && P->green && P->os_v && P->method == 0 && P->osv_variant == 0 && P->solver == 0 &&
+                      src != dst;
+    cudaError_t e;
+    if (!fuse) {
+        e = run_field(P, src, nullptr, energy_out);
+        if (e == cudaSuccess) e = run_setup(P, true, 1, dts, P->E_self, Eext, nullptr);
+        if (e == cudaSuccess) e = advect_v(P, src, dst, true);
+        return e;
+    }
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    e = launch_pdl(density_partial_kernel<false>, dim3(Nx / 32, P->nby), dim3(256), 0, P->st, src, Nx, Nv, Nv / P->nby,
+                   P->part, (double*)nullptr, 0.0, 0.0, reinterpret_cast<unsigned*>(P->e_part + Nx / 16 + 1), P->rho, dv);
+    if (e != cudaSuccess) return e;
+    P->launches++;
+    P->E_valid = true;
+    P->E_of = src;
+    e = run_setup(P, true, 1, dts, P->E_self, Eext, nullptr);          // (records the shift source; no launch)
+    if (e != cudaSuccess) return e;
+    OsSetupArgs& su = P->vsetup;
+    su.fpart = P->rho; su.green = P->green; su.nby = P->nby;
+    su.E_out = P->E_self; su.rho_out = nullptr;
+    su.energy_out = energy_out; su.e_part = P->e_part;
+    su.ticket = reinterpret_cast<unsigned*>(P->e_part + Nx / 16);
+    su.half_dx = 0.5 * P->p.L / (double)Nx;
+    e = run_osv(P, src, dst, true);
+    su.fpart = nullptr;
     return e;
 }
 
@@ -1389,9 +1486,7 @@ extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ex
     if (P->p.split == VOG_SPLIT_XVX) {
         e = ensure_recx(P, 0.5 * dt);
         if (e == cudaSuccess) e = advect_x(P, f_dev, f_dev);
-        if (e == cudaSuccess) e = run_field(P, f_dev, nullptr);
-        if (e == cudaSuccess) e = run_setup(P, true, 1, dt, P->E_self, E_ext_dev, nullptr);
-        if (e == cudaSuccess) e = advect_v(P, f_dev, g, true);
+        if (e == cudaSuccess) e = field_then_v(P, f_dev, g, dt, E_ext_dev, nullptr);
         if (e == cudaSuccess) e = advect_x(P, g, f_dev);
         P->E_of = nullptr;                        // E_self is the field at the half step, not of the final state
     } else {
@@ -1401,9 +1496,7 @@ extern "C" int vog_step(vog_plan_t P, float* f_dev, double dt, const float* E_ex
         if (e == cudaSuccess) e = advect_v(P, f_dev, g, true);
         if (e == cudaSuccess) e = ensure_recx(P, dt);
         if (e == cudaSuccess) e = advect_x(P, g, g);
-        if (e == cudaSuccess) e = run_field(P, g, nullptr);
-        if (e == cudaSuccess) e = run_setup(P, true, 1, 0.5 * dt, P->E_self, E_ext_dev, nullptr);
-        if (e == cudaSuccess) e = advect_v(P, g, f_dev, true);
+        if (e == cudaSuccess) e = field_then_v(P, g, f_dev, 0.5 * dt, E_ext_dev, nullptr);
         P->E_of = e == cudaSuccess ? f_dev : nullptr;      // rho, hence E, is invariant under the v-advection
     }
     return cuda_status(e);
@@ -1453,9 +1546,7 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
         e = ensure_recx(P, 0.5 * dt);
         if (ok()) e = advect_x(P, f_dev, f_dev);
         for (int s = 0; s < nsteps && ok(); ++s) {
-            e = run_field(P, f_dev, nullptr, en());
-            if (ok()) e = run_setup(P, true, 1, dt, P->E_self, ext(), nullptr);
-            if (ok()) e = advect_v(P, f_dev, g, true);
+            e = field_then_v(P, f_dev, g, dt, ext(), en());
             const bool last = s == nsteps - 1;
             if (ok()) e = ensure_recx(P, (merge && !last) ? dt : 0.5 * dt);
             if (ok()) e = advect_x(P, g, f_dev);
@@ -1479,14 +1570,12 @@ extern "C" int vog_run(vog_plan_t P, float* f_dev, double dt, int nsteps, const 
         for (int s = 0; s < nsteps && ok(); ++s) {
             if (flip_x) { e = advect_x(P, cur, oth); std::swap(cur, oth); flip_x = false; }
             else e = advect_x(P, cur, cur);
-            if (ok()) e = run_field(P, cur, nullptr, en());
             const bool last = s == nsteps - 1;
             if (!ok()) break;
-            if (merge && !last) vadv(dt);
-            else {
-                vadv(0.5 * dt);
-                if (ok() && !last) vadv(0.5 * dt);
-            }
+            // (field solve + the v-advection that follows it; unmerged, the second v(dt/2) reuses E_self)
+            e = field_then_v(P, cur, oth, (merge && !last) ? dt : 0.5 * dt, ext(), en());
+            std::swap(cur, oth);
+            if (ok() && !(merge && !last) && !last) vadv(0.5 * dt);
         }
         P->E_of = ok() ? f_dev : nullptr;
     }

@@ -908,6 +908,16 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     const float2* const twp = twS + h;            // [q-1][t], t = item index of passes A
     float2* const own = exch + h * W + c;                                     // position t = h
     constexpr int PS = 16 * W;                                                // float2 between positions 16 apart
+    // Field solve fused into this kernel (su.fpart != NULL; grids of at most gridDim.x strips, one piece per CTA): the
+    // exchange buffers of the three groups are free until the first pass A and hold, in this order, rho (Nx doubles),
+    // the Green's function of the Fourier solve (Nx doubles, a plan constant: loaded before the wait) and the partial
+    // sums of the convolution.
+    __shared__ float fusedE[W];
+    double* const fRho = reinterpret_cast<double*>(smem_raw + HEAD + RR * W * 4);
+    double* const fGreen = reinterpret_cast<double*>(smem_raw + HEAD + GB + RR * W * 4);
+    double* const fSum = reinterpret_cast<double*>(smem_raw + HEAD + 2 * GB + RR * W * 4);
+    if (su.fpart)
+        for (int i = tid; i < Nx; i += 768) fGreen[i] = __ldg(su.green + i);
 
     // Work of this CTA, in pieces (strip of 16 columns, pairs q0 .. q1-1).  The strips are dealt out round-robin in
     // whole rounds of gridDim.x strips (neighbouring CTAs work on neighbouring strips at the same time); the strips
@@ -949,7 +959,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         double beta;
         float sshift = 0.0f;
         if (su.mode == 1) {
-            double e = (double)su.E[l];
+            double e = su.fpart ? (double)fusedE[cc] : (double)su.E[l];
             if (su.Eext) e += (double)su.Eext[l];
             beta = -e * su.dt / su.delta;
             sshift = (float)(su.dt * e);
@@ -1047,6 +1057,62 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     pdl_launch_dependents();
     int strip, q0, q1, nstrip = 0, nq0 = 0, nq1 = 0;
     bool has = piece(0, strip, q0, q1), nhas = has && piece(1, nstrip, nq0, nq1);
+    if (su.fpart) {
+        // S9 for the 16 columns of this strip.  rho_i (the density kernel's last blocks wrote it: dv * the slab sums in
+        // the order of poisson_kernel) minus rho_0 (any constant only changes mode 0, which is dropped: P:205-211);
+        // E_i = sum_j G_{i-j} rho_j with G = the inverse transform of 1 / (i k_m), modes 0 and Nx/2 dropped:
+        // the Fourier solve written as the circular convolution it is, in fp64, fixed order.
+        const int xmask = Nx - 1, c0f = strip * W;
+        const bool writer = has && q0 == 0;        // the strip's first segment publishes E and the energy share
+        {
+            const double ref = __ldcg(su.fpart);
+            double r[3];                           // (Nx <= 16 gridDim.x <= 2368: three cells per thread, one round trip)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) r[k] = tid + 768 * k < Nx ? __ldcg(su.fpart + tid + 768 * k) : 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+                if (tid + 768 * k < Nx) fRho[tid + 768 * k] = r[k] - ref;
+            for (int i = tid + 2304; i < Nx; i += 768) fRho[i] = __ldcg(su.fpart + i) - ref;
+        }
+        __syncthreads();
+        {
+            const int cc = tid & 15, part = tid >> 4;          // 48 interleaved shares of the sum over j
+            double acc = 0.0;
+#pragma unroll 4
+            for (int j = part; j < Nx; j += 48) acc = fma(fGreen[(c0f + cc - j) & xmask], fRho[j], acc);
+            acc += __shfl_xor_sync(0xffffffffu, acc, 16);      // shares 2 w and 2 w + 1 of warp w
+            if ((tid & 16) == 0) fSum[(tid >> 5) * W + cc] = acc;
+        }
+        __syncthreads();
+        if (tid < W) {
+            double sv = 0.0;
+#pragma unroll
+            for (int q = 0; q < 24; ++q) sv += fSum[q * W + tid];
+            const float ef = (float)sv;
+            fusedE[tid] = ef;
+            if (writer) {
+                su.E_out[c0f + tid] = ef;
+                if (su.energy_out) {   // (1/2) dx sum_i E_i^2: strip sums in strip order by the last strip to arrive
+                    double e2 = (double)ef * (double)ef;
+#pragma unroll
+                    for (int o = 8; o > 0; o >>= 1) e2 += __shfl_xor_sync(0xffffu, e2, o);
+                    if (tid == 0) {
+                        su.e_part[strip] = e2;
+                        __threadfence();
+                        const unsigned n = atomicAdd(su.ticket, 1u);
+                        if (n == (unsigned)nstrips - 1u) {
+                            __threadfence();
+                            double tot = 0.0;
+                            for (int q = 0; q < nstrips; ++q) tot += __ldcg(su.e_part + q);
+                            su.energy_out[0] = su.half_dx * tot;
+                            *su.ticket = 0u;
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
     if (tid < 2 * W && has) coeffs(tid, strip * W, cfS);
     if (tid >= 2 * W && tid < 4 * W && nhas) coeffs(tid - 2 * W, nstrip * W, cfS + CF);
     __syncthreads();
