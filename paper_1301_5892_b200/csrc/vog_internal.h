@@ -147,6 +147,7 @@ struct OsSetupArgs {
     double* e_part;            // [n_lines / 16] per-strip sums of E^2 (scratch of the energy reduction)
     unsigned* ticket;          // arrival counter of the energy reduction (zero between launches)
     double half_dx;
+    int spec;                  // osv7_kernel: request every group's first window before the field is known (shifts < 16 rows)
 };
 
 cudaError_t os_setup_launch(const OsSetupArgs& s, cudaStream_t st);

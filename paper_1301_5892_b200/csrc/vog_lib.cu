@@ -648,6 +648,8 @@ struct vog_plan_s {
     double* green;              // [Nx] Green's function of the Fourier solve (plans whose v kernel can solve the field itself)
     double* e_part;             // [Nx / 16] + ticket word: energy reduction of the fused field solve
     int fuse_field;             // steps: density -> v kernel with the field solve inside (no Poisson launch); 0 / 1
+    int v_spec;                 // v kernel: first windows requested before the shifts are known (default 1)
+    bool v_behind_field;        // ... set by field_then_v around its v launch
     float *feq_tab, *vmu_tab;   // [ng][Nv]
     int nby, nby_max;           // density: row slabs per column group (tunable up to the allocated nby_max)
     int lognl_x, lognl_v, thr_x, thr_v;
@@ -841,6 +843,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     default_x_tile(Nx, Nv, &P->x_lpi_log, &P->x_thr);
     P->os_x = Nx >= 1024;
     P->os_v = Nv >= 1024;
+    P->v_spec = 1;
     {
         // pair kernels: 16 items per pair and phase; lines per iteration so that one round of <= 320 threads
         // covers the items (8192: 18 pairs = 288 items; 2048: 3 lines x 5 pairs = 240)
@@ -1049,6 +1052,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 25: if (value < 0 || value > 1 || (value == 1 && P->p.kind != VOG_LAGRANGE)) return VOG_EINVAL; P->os_geom = value; P->os3x_occ = 0; break;
         case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
         case 30: if (value < 0 || value > 1 || (value == 1 && !P->green)) return VOG_EINVAL; P->fuse_field = value; break;
+        case 31: if (value < 0 || value > 1) return VOG_EINVAL; P->v_spec = value; break;
         case 29: if (value < 0 || value > 1 || P->p.Nx > 256 || P->p.Nv > 256) return VOG_EINVAL; P->small_run = value; break;
         case 28: if (value < 0 || value > 2) return VOG_EINVAL; P->solver = value; P->E_of = nullptr; P->E_valid = false; break;
         case 27: if (value < 0 || value > 1) return VOG_EINVAL; P->method = value; P->recx_valid = false; P->E_of = nullptr; break;
@@ -1202,6 +1206,9 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
         int gpc = P->os2v_gpc > 0 ? P->os2v_gpc : (a.np >= 18 ? 9 : (a.np >= 6 ? 3 : a.np));
         if (gpc > a.np) gpc = a.np;
         a.gpc = gpc;
+        // (the first windows may be requested before the kernel's wait only when the kernel in front of it on the
+        // stream is not the one that writes src: true behind a field solve, whose kernels only read the grid)
+        P->vsetup.spec = P->v_spec && P->v_behind_field;
         return osv7_launch(a, P->vsetup, geom, P->n_sm, P->st);
     }
     if (P->osv_variant == 2) {
@@ -1366,7 +1373,9 @@ static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, dou
     if (!fuse) {
         e = run_field(P, src, nullptr, energy_out);
         if (e == cudaSuccess) e = run_setup(P, true, 1, dts, P->E_self, Eext, nullptr);
+        P->v_behind_field = true;
         if (e == cudaSuccess) e = advect_v(P, src, dst, true);
+        P->v_behind_field = false;
         return e;
     }
     const int Nx = P->p.Nx, Nv = P->p.Nv;
@@ -1385,7 +1394,9 @@ static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, dou
     su.energy_out = energy_out; su.e_part = P->e_part;
     su.ticket = reinterpret_cast<unsigned*>(P->e_part + Nx / 16);
     su.half_dx = 0.5 * P->p.L / (double)Nx;
+    P->v_behind_field = true;
     e = run_osv(P, src, dst, true);
+    P->v_behind_field = false;
     su.fpart = nullptr;
     return e;
 }

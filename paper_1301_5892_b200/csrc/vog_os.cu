@@ -360,3 +360,8 @@ cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_
 }
 
 }  // namespace vog
+
+#ifdef VOG_STAMPS
+extern "C" int vog_debug_os_stamps(long long* out64) { return (int)cudaMemcpyFromSymbol(out64, vog::os_stamps, sizeof(long long) * 64); }
+extern "C" int vog_debug_os_blk(long long* out4096) { return (int)cudaMemcpyFromSymbol(out4096, vog::os_blk, sizeof(long long) * 4096); }
+#endif

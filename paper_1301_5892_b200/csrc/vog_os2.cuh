@@ -23,6 +23,17 @@
 
 namespace vog {
 
+// (working builds only, -DVOG_STAMPS: globaltimer stamps of the phases of CTA 0, read with vog_debug_os_stamps)
+#ifdef VOG_STAMPS
+__device__ long long os_stamps[64];
+#define OS_STAMP(i) do { if (blockIdx.x == 0 && threadIdx.x == 0) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); os_stamps[i] = t_; } } while (0)
+__device__ long long os_blk[4 * 1024];
+#define OS_BLK(i) do { if (threadIdx.x == 0 && blockIdx.x < 1024) { long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); os_blk[4 * blockIdx.x + (i)] = t_; } } while (0)
+#else
+#define OS_STAMP(i) do { } while (0)
+#define OS_BLK(i) do { } while (0)
+#endif
+
 namespace os2 {
 
 __device__ __forceinline__ void cp_async4(void* smem, const void* gmem)
@@ -530,7 +541,7 @@ __global__ void __launch_bounds__(288, 3) osx7_kernel(const OsArgs a)
 // has 512 floats of padding: rows >= Nv are read but never stored; rows < 0 (m = 0 of the first pair) are clamped.
 template <int V, int HLO, int W = 32>
 __device__ __forceinline__ void osv2_source(float2* x, const OsArgs& a, const float4* __restrict__ RS, const int lane,
-                                            const int r0, const float ssh)
+                                            const int r0, const float ssh, const float2* __restrict__ RV = nullptr)
 {
     constexpr int M0 = KeptM<V, HLO, 0>::none ? 1 : 0;       // first and last sample rows that hold kept samples
     constexpr int M1 = KeptM<V, HLO, 15>::none ? 14 : 15;
@@ -546,7 +557,10 @@ __device__ __forceinline__ void osv2_source(float2* x, const OsArgs& a, const fl
             Rr = make_float4(expf(hh), expm1f(hh), expf(-hh), expm1f(-hh));
         }
         const float ea8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128), a.dvf, u0) - ssh));
-        const float eb8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128 + V), a.dvf, u0) - ssh));
+        // (block B lies V rows further: e^{X + g V} - 1 = (e^X - 1) e^{g V} + (e^{g V} - 1), RV = (e^{g V}, expm1(g V)) per lane)
+        float eb8;
+        if (RV) { const float2 rv = RV[g * W + lane]; eb8 = fmaf(ea8, rv.x, rv.y); }
+        else eb8 = expm1f(cgs * (2.0f * fmaf((float)(r0 + 128 + V), a.dvf, u0) - ssh));
         float ea = ea8, eb = eb8;
 #pragma unroll
         for (int m = 8; m <= M1; ++m) {
@@ -913,11 +927,14 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     // the Green's function of the Fourier solve (Nx doubles, a plan constant: loaded before the wait) and the partial
     // sums of the convolution.
     __shared__ float fusedE[W];
-    double* const fRho = reinterpret_cast<double*>(smem_raw + HEAD + RR * W * 4);
-    double* const fGreen = reinterpret_cast<double*>(smem_raw + HEAD + GB + RR * W * 4);
+    __shared__ float4 srcRS[4 * W];               // delta-f source: (e^h, expm1 h, e^-h, expm1 -h), h = 16 rows, per (Gaussian, column)
+    __shared__ float2 srcRV[4 * W];               // ... and (e^{g V}, expm1(g V)): block B from block A
+    float* const fRho = reinterpret_cast<float*>(smem_raw + HEAD + RR * W * 4);
+    float* const fGreen = reinterpret_cast<float*>(smem_raw + HEAD + GB + RR * W * 4);
     double* const fSum = reinterpret_cast<double*>(smem_raw + HEAD + 2 * GB + RR * W * 4);
     if (su.fpart)
-        for (int i = tid; i < Nx; i += 768) fGreen[i] = __ldg(su.green + i);
+        for (int i = tid; i < Nx; i += 768) fGreen[i] = (float)__ldg(su.green + i);
+    if (tid < 5) asm volatile("prefetch.tensormap [%0];\n" ::"l"(reinterpret_cast<unsigned long long>(&maps.m[tid])) : "memory");
 
     // Work of this CTA, in pieces (strip of 16 columns, pairs q0 .. q1-1).  The strips are dealt out round-robin in
     // whole rounds of gridDim.x strips (neighbouring CTAs work on neighbouring strips at the same time); the strips
@@ -1053,15 +1070,34 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         }
     };
 
-    pdl_wait();                                   // the field and the source grid come from earlier kernels
-    pdl_launch_dependents();
+    OS_STAMP(0);
+    OS_BLK(0);
     int strip, q0, q1, nstrip = 0, nq0 = 0, nq1 = 0;
     bool has = piece(0, strip, q0, q1), nhas = has && piece(1, nstrip, nq0, nq1);
+    // Speculative first window.  The source grid is final before this CTA exists: this kernel's predecessor in the
+    // stream (density or Poisson kernel) lets its dependents start only after its own wait on the kernel that wrote
+    // the grid, so only E / rho need the wait below.  Each group requests, for its first pair, the rows that serve every
+    // integer shift in [-SPEC, SPEC) -- the whole raw buffer -- while the field is still being solved; if the shifts
+    // turn out larger (or spread too far) the window is requested again once they are known.
+    constexpr int SPEC = (RR - OS_LB - V) / 2;     // 16 (Lagrange geometry) / 18 rows
+    bool spec = false;
+    if (su.spec && has && q0 + gid < q1) {
+        Geo gs;
+        gs.c0 = strip * W; gs.base = -SPEC; gs.nrows = RR; gs.db = 0; gs.gather = false;
+        land(gs, q0 + gid);
+        spec = true;
+    }
+    pdl_wait();                                   // the field (or rho) comes from the kernel before
+    pdl_launch_dependents();
+    OS_STAMP(1);
+    OS_BLK(1);
     if (su.fpart) {
         // S9 for the 16 columns of this strip.  rho_i (the density kernel's last blocks wrote it: dv * the slab sums in
-        // the order of poisson_kernel) minus rho_0 (any constant only changes mode 0, which is dropped: P:205-211);
-        // E_i = sum_j G_{i-j} rho_j with G = the inverse transform of 1 / (i k_m), modes 0 and Nx/2 dropped:
-        // the Fourier solve written as the circular convolution it is, in fp64, fixed order.
+        // the order of poisson_kernel) minus rho_0 (any constant only changes mode 0, which is dropped: P:205-211),
+        // rounded to fp32 like poisson_kernel's input; E_i = sum_j G_{i-j} rho_j with G = the inverse transform of
+        // 1 / (i k_m), modes 0 and Nx/2 dropped: the Fourier solve written as the circular convolution it is.
+        // 48 shares of <= 43 products per column in fp32 (the fp64 pipe took 2.6 us for these 33 k multiply-adds), the
+        // shares added in fp64 in a fixed order.
         const int xmask = Nx - 1, c0f = strip * W;
         const bool writer = has && q0 == 0;        // the strip's first segment publishes E and the energy share
         {
@@ -1071,25 +1107,53 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             for (int k = 0; k < 3; ++k) r[k] = tid + 768 * k < Nx ? __ldcg(su.fpart + tid + 768 * k) : 0.0;
 #pragma unroll
             for (int k = 0; k < 3; ++k)
-                if (tid + 768 * k < Nx) fRho[tid + 768 * k] = r[k] - ref;
-            for (int i = tid + 2304; i < Nx; i += 768) fRho[i] = __ldcg(su.fpart + i) - ref;
+                if (tid + 768 * k < Nx) fRho[tid + 768 * k] = (float)(r[k] - ref);
+            for (int i = tid + 2304; i < Nx; i += 768) fRho[i] = (float)(__ldcg(su.fpart + i) - ref);
+            if (tid < 192) fRho[Nx + tid] = 0.0f;  // (the last chunks of the sum over j run past Nx)
         }
         __syncthreads();
+        OS_STAMP(40);
         {
-            const int cc = tid & 15, part = tid >> 4;          // 48 interleaved shares of the sum over j
-            double acc = 0.0;
+            // thread = (quad of columns cq, chunk of JC consecutive cells j): per cell one value of rho, one new value of G
+            // (a rolling window of four) and four multiply-adds in fp32; the 8 chunks of a warp are folded by shuffles,
+            // the 24 warps meet in shared memory; sums across threads in fp64, fixed order.
+            const int cq = tid & 3, jp = tid >> 2, JC = (Nx + 191) / 192, j0 = jp * JC;
+            const int gb = c0f + 4 * cq + 3 - j0;                      // index of G for column 4 cq + 3 at cell j0
+            float g0 = fGreen[gb & xmask], g1 = fGreen[(gb - 1) & xmask], g2 = fGreen[(gb - 2) & xmask], g3;
+            float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;        // columns 4 cq + 3, + 2, + 1, + 0
 #pragma unroll 4
-            for (int j = part; j < Nx; j += 48) acc = fma(fGreen[(c0f + cc - j) & xmask], fRho[j], acc);
-            acc += __shfl_xor_sync(0xffffffffu, acc, 16);      // shares 2 w and 2 w + 1 of warp w
-            if ((tid & 16) == 0) fSum[(tid >> 5) * W + cc] = acc;
+            for (int i = 0; i < JC; ++i) {
+                g3 = fGreen[(gb - 3 - i) & xmask];
+                const float rj = fRho[j0 + i];
+                a0 = fmaf(g0, rj, a0); a1 = fmaf(g1, rj, a1); a2 = fmaf(g2, rj, a2); a3 = fmaf(g3, rj, a3);
+                g0 = g1; g1 = g2; g2 = g3;
+            }
+            double d0 = (double)a0, d1 = (double)a1, d2 = (double)a2, d3 = (double)a3;
+#pragma unroll
+            for (int o = 16; o >= 4; o >>= 1) {
+                d0 += __shfl_xor_sync(0xffffffffu, d0, o); d1 += __shfl_xor_sync(0xffffffffu, d1, o);
+                d2 += __shfl_xor_sync(0xffffffffu, d2, o); d3 += __shfl_xor_sync(0xffffffffu, d3, o);
+            }
+            if ((tid & 28) == 0) {                 // lanes 0..3 of the warp: quad cq
+                double* const o = fSum + (tid >> 5) * W + 4 * cq;
+                o[3] = d0; o[2] = d1; o[1] = d2; o[0] = d3;
+            }
+        }
+        __syncthreads();
+        OS_STAMP(41);
+        if (tid < 4 * W) {
+            // 24 warp sums per column: four threads add six each, then the four meet by shuffles
+            const int cc = tid >> 2, part = tid & 3;
+            double sv = 0.0;
+#pragma unroll
+            for (int q = 0; q < 6; ++q) sv += fSum[(6 * part + q) * W + cc];
+            sv += __shfl_xor_sync(0xffffffffu, sv, 1);
+            sv += __shfl_xor_sync(0xffffffffu, sv, 2);
+            if (part == 0) fusedE[cc] = (float)sv;
         }
         __syncthreads();
         if (tid < W) {
-            double sv = 0.0;
-#pragma unroll
-            for (int q = 0; q < 24; ++q) sv += fSum[q * W + tid];
-            const float ef = (float)sv;
-            fusedE[tid] = ef;
+            const float ef = fusedE[tid];
             if (writer) {
                 su.E_out[c0f + tid] = ef;
                 if (su.energy_out) {   // (1/2) dx sum_i E_i^2: strip sums in strip order by the last strip to arrive
@@ -1113,12 +1177,44 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         }
         __syncthreads();
     }
+    OS_STAMP(2);
     if (tid < 2 * W && has) coeffs(tid, strip * W, cfS);
     if (tid >= 2 * W && tid < 4 * W && nhas) coeffs(tid - 2 * W, nstrip * W, cfS + CF);
     __syncthreads();
+    OS_STAMP(3);
     bool pref = false;                             // the first window of this group in the current piece is on its way
     for (int it = 0; has; ++it) {
         const float* const rec = cfS + (it % 3) * CF;
+        // the group's first window of the piece is requested first: it lands while the table is computed
+        const Geo g = geometry(strip * W, rec);
+        const float ssh = rec[19 * W + c];
+        const int p0 = q0 + gid;
+        int db_first = g.db;                       // row offset of this lane in the window of the group's first pair
+        if (spec) {
+            // does the speculative window hold the rows of every column?  first row needed by this lane, relative to
+            // the window's first row: (base + db) - (-SPEC), base as a signed shift
+            const int sb = (((g.base + (Nv >> 1)) & vmask) - (Nv >> 1)) + SPEC;
+            const bool fits = !g.gather && sb >= 0 && sb + (g.nrows - (V + OS_LB)) <= RR - (V + OS_LB);
+            if (fits) db_first = sb + g.db;
+            else {                                 // (uniform over the CTA: every half-warp sees the same 16 columns)
+                os2::mbar_wait(vbar, vpar); vpar ^= 1u;
+                os2::bar_group(gid + 1);           // (nobody of the group may still be waiting when the barrier is re-armed)
+                land(g, p0);
+            }
+            spec = false;
+        } else if (!pref && p0 < q1) land(g, p0);
+        pref = false;
+        if (tid < 6 * a.ng * W) {
+            // delta-f source constants of (Gaussian gg, column cc): same expressions as osv2_source without a table,
+            // one transcendental per thread (two warps computing all six per entry were the slowest of this phase)
+            const int which = tid / (a.ng * W), i = tid - which * (a.ng * W), cc = i & (W - 1), gg = i >> 4;
+            const float cgs = a.cg4[gg] * rec[19 * W + cc];
+            const float hh = 32.0f * cgs * a.dvf, hv = 2.0f * (float)V * cgs * a.dvf;
+            const float arg = which < 2 ? hh : (which < 4 ? -hh : hv);
+            const float val = (which & 1) ? expm1f(arg) : expf(arg);
+            if (which < 4) reinterpret_cast<float*>(srcRS)[4 * i + which] = val;
+            else reinterpret_cast<float*>(srcRV)[2 * i + (which - 4)] = val;
+        }
         // ---- the strip's table: 130 x 16 entries
         for (int idx = tid; idx < OS_LAMW * W; idx += 768) {
             const int kk = idx >> 4, cc = idx & 15;
@@ -1149,12 +1245,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             }
             lamS[idx] = o;
         }
-        const Geo g = geometry(strip * W, rec);
-        const float ssh = rec[19 * W + c];
-        const int p0 = q0 + gid;
-        if (!pref && p0 < q1) land(g, p0);
-        pref = false;
+        OS_STAMP(42);
         __syncthreads();                           // table visible to everybody
+        OS_STAMP(4);
+        if (it == 0) OS_BLK(2);
         // the piece after next: its fp64 coefficients, in the last warp, while everybody else transforms
         int fstrip = 0, fq0 = 0, fq1 = 0;
         const bool fhas = nhas && piece(it + 2, fstrip, fq0, fq1);
@@ -1166,11 +1260,13 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         for (int p = p0; p < q1; p += 3) {
             if (g.gather) os2::cp_async_wait_all();
             else { os2::mbar_wait(vbar, vpar); vpar ^= 1u; }
+            OS_STAMP(5 + 4 * ((p - p0) / 3));
             os2::bar_group(gid + 1);               // raw rows of pair p visible; exchange buffer of the last pair read
             // ---- pass A (item t = h): samples from the raw rows with this lane's offset
             {
                 float2 x[16];
-                const float* const rp = raw + (h + g.db) * W + c;
+                const float* const rp = raw + (h + db_first) * W + c;
+                db_first = g.db;
 #pragma unroll
                 for (int k = 0; k < 16; ++k) x[k] = make_float2(rp[16 * k * W], rp[(16 * k + V) * W]);
                 dft_dif<16, 1>(x);
@@ -1179,6 +1275,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 for (int q = 1; q < 16; ++q) own[q * PS] = cmul(x[brev(q, 16)], twp[(q - 1) * 16]);
             }
             os2::bar_group(gid + 1);               // exchange buffer complete; raw rows all read
+            OS_STAMP(6 + 4 * ((p - p0) / 3));
             // the next window lands behind the middle stage and the inverse pass: this piece's, or -- after the group's
             // last pair of the piece -- the group's first of the NEXT piece (its shifts are known two pieces ahead)
             if (p + 3 < q1) land(g, p + 3);
@@ -1194,6 +1291,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 for (int j = 0; j < 16; ++j) sp[j * W] = x[j];
             }
             os2::bar_group(gid + 1);
+            OS_STAMP(7 + 4 * ((p - p0) / 3));
             // ---- inverse pass A (item j = h): kept samples -> rows of the destination
             {
                 float2 x[16];
@@ -1202,13 +1300,16 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 for (int q = 1; q < 16; ++q) x[brev(q, 16)] = cmulc(own[q * PS], twp[(q - 1) * 16]);
                 idft_dit<16, 1>(x);
                 const int r0 = p * (2 * V) + h - HLO;          // row of sample n = t = h of block A
-                if (a.ng > 0) osv2_source<V, HLO, W>(x, a, nullptr, c, r0, ssh);
+                if (a.ng > 0) osv2_source<V, HLO, W>(x, a, srcRS, c, r0, ssh, srcRV);
                 float* const po = ocol + (ptrdiff_t)r0 * Nx;
                 if ((p + 1) * (2 * V) <= Nv) os2_store_v_full<V, HLO>(po, (size_t)Nx, h, x);
                 else os2_store_v<V, HLO>(po, (size_t)Nx, r0, Nv, h, false, x);
             }
+            OS_STAMP(8 + 4 * ((p - p0) / 3));
         }
         __syncthreads();                           // every group is done with the table of this piece
+        OS_STAMP(30);
+        OS_BLK(3);
         has = nhas; strip = nstrip; q0 = nq0; q1 = nq1;
         nhas = fhas; nstrip = fstrip; nq0 = fq0; nq1 = fq1;
     }
