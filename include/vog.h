@@ -194,6 +194,8 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   31     v kernel (Nv >= 1024): 1 (default) = every group requests the rows of its first pair of blocks BEFORE the
  *          field / the shifts are known -- the raw buffer's whole 520 rows, which serve any integer shift in [-16, 16)
  *          -- and requests them again if the shifts turn out larger; 0 = after the shifts are known.
+ *   33     density kernel launched with (1) or without (0) the programmatic-dependent-launch attribute of code 26
+ *          (default: with it below 4096 x 4096 cells, without it from there on).
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

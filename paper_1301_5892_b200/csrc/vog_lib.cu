@@ -649,6 +649,7 @@ struct vog_plan_s {
     double* e_part;             // [Nx / 16] + ticket word: energy reduction of the fused field solve
     int fuse_field;             // steps: density -> v kernel with the field solve inside (no Poisson launch); 0 / 1
     int v_spec;                 // v kernel: first windows requested before the shifts are known (default 1)
+    int density_pdl;            // density kernel launched with the programmatic-dependent-launch attribute (0 / 1)
     bool v_behind_field;        // ... set by field_then_v around its v launch
     float *feq_tab, *vmu_tab;   // [ng][Nv]
     int nby, nby_max;           // density: row slabs per column group (tunable up to the allocated nby_max)
@@ -844,6 +845,10 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     P->os_x = Nx >= 1024;
     P->os_v = Nv >= 1024;
     P->v_spec = 1;
+    // (measured: behind an x kernel of a grid of 4096^2 cells or more the density kernel's 512 long-running blocks do
+    // worse when they trickle onto the SMs as the x kernel drains -- 8192^2 step 484 us with the attribute, 451 us
+    // without; on the 2048^2 grid the early start wins: 51.6 against 54.7 us)
+    P->density_pdl = (long long)Nx * Nv < 4096LL * 4096LL ? 1 : 0;
     {
         // pair kernels: 16 items per pair and phase; lines per iteration so that one round of <= 320 threads
         // covers the items (8192: 18 pairs = 288 items; 2048: 3 lines x 5 pairs = 240)
@@ -1053,6 +1058,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 26: if (value < 0 || value > 1) return VOG_EINVAL; P->pdl = value; break;
         case 30: if (value < 0 || value > 1 || (value == 1 && !P->green)) return VOG_EINVAL; P->fuse_field = value; break;
         case 31: if (value < 0 || value > 1) return VOG_EINVAL; P->v_spec = value; break;
+        case 33: if (value < 0 || value > 1) return VOG_EINVAL; P->density_pdl = value; break;
         case 29: if (value < 0 || value > 1 || P->p.Nx > 256 || P->p.Nv > 256) return VOG_EINVAL; P->small_run = value; break;
         case 28: if (value < 0 || value > 2) return VOG_EINVAL; P->solver = value; P->E_of = nullptr; P->E_valid = false; break;
         case 27: if (value < 0 || value > 1) return VOG_EINVAL; P->method = value; P->recx_valid = false; P->E_of = nullptr; break;
@@ -1323,12 +1329,15 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
     const double dv = (P->p.vmax - P->p.vmin) / (double)Nv, dx = P->p.L / (double)Nx;
     dim3 grid(Nx / 32, P->nby);
     cudaError_t e;
+    const bool pdl_was = t_pdl;
+    t_pdl = pdl_was && P->density_pdl;
     if (diag_out)
         e = launch_pdl(density_partial_kernel<true>, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part, P->partk,
                        P->p.vmin, dv, (unsigned*)nullptr, (double*)nullptr, 0.0);
     else
         e = launch_pdl(density_partial_kernel<false>, grid, dim3(256), 0, P->st, f, Nx, Nv, Nv / P->nby, P->part,
                        (double*)nullptr, 0.0, 0.0, (unsigned*)nullptr, (double*)nullptr, 0.0);
+    t_pdl = pdl_was;
     if (e != cudaSuccess) return e;
     P->launches += 2;
     P->E_valid = true;
@@ -1380,8 +1389,11 @@ static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, dou
     }
     const int Nx = P->p.Nx, Nv = P->p.Nv;
     const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    const bool pdl_was = t_pdl;
+    t_pdl = pdl_was && P->density_pdl;
     e = launch_pdl(density_partial_kernel<false>, dim3(Nx / 32, P->nby), dim3(256), 0, P->st, src, Nx, Nv, Nv / P->nby,
                    P->part, (double*)nullptr, 0.0, 0.0, reinterpret_cast<unsigned*>(P->e_part + Nx / 16 + 1), P->rho, dv);
+    t_pdl = pdl_was;
     if (e != cudaSuccess) return e;
     P->launches++;
     P->E_valid = true;
