@@ -185,12 +185,14 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *          their direct form, the same matrices up to rounding), same sequences, E_ext and energy semantics as the
  *          launch-per-kernel loop; 0 = that loop (default: vog_run(merge = 0) stays bit-identical to vog_step).
  *          Ignored while the trapezoid field solver (28) is selected.
- *   30     grids with Nv >= 1024 and Nx / 16 <= the number of SMs (Nx <= 2048 on a B200) only: 1 (default there) = in
+ *   30     grids with Nv >= 1024 and Nx / 16 <= the number of SMs (Nx <= 2048 on a B200), or Nx >= 4096: 1 (default there) = in
  *          vog_step / vog_run the field solve that precedes a v-advection runs INSIDE the v kernel: the density kernel's
  *          last blocks write rho, every CTA of the v kernel computes E on its own 16 columns as the circular convolution
  *          of rho with the Green's function of the same Fourier solve (fp64) and the strip's first CTA publishes
  *          E (vog_get_field) and the energy share; a step is then 4 launches (x, density, v, x).  0 = density, Poisson
  *          kernel, v kernel (5 launches).  Same E up to rounding (the convolution is the more accurate of the two).
+ *          On grids of 8192 columns or more, 1 (default) = the same convolution as a kernel of its own (one CTA per 64
+ *          columns) in the place of the single-CTA Poisson kernel.
  *   31     v kernel (Nv >= 1024): 1 (default) = every group requests the rows of its first pair of blocks BEFORE the
  *          field / the shifts are known -- the raw buffer's whole 520 rows, which serve any integer shift in [-16, 16)
  *          -- and requests them again if the shifts turn out larger; 0 = after the shifts are known.

@@ -590,19 +590,101 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
     VOG_STAMP(6);
 }
 
-// Green's function of the Fourier field solve: E_i = sum_j G_{i-j} rho_j with
-// G_n = (1/Nx) sum_{m != 0, Nx/2} e^{2 pi i m n / Nx} / (i k_m) = L / (pi Nx) sum_{m=1}^{Nx/2-1} sin(2 pi m n / Nx) / m,
-// k_m = 2 pi m / L.  fp64, small terms first; a plan constant (osv7_kernel's fused field solve reads it).
-__global__ void green_kernel(int Nx, double L, double* __restrict__ G)
+// ------------------------------------------------------------------------------------------
+// S9 in x space (steps on grids of 8192 columns or more; the 2048-column grids do the same inside the v kernel, see
+// osv7_kernel).  The Fourier solve of P:221 is a circular convolution, E_i = sum_j G_{i-j} rho_j, with the Green's function
+// G_n = (1/Nx) sum_{m != 0, Nx/2} e^{2 pi i m n / Nx} / (i k_m), k_m = 2 pi m / L (a plan constant, computed on the host
+// in fp64: green_host).  One CTA of 1024 threads per 64 columns instead of ONE CTA for the whole solve (poisson_kernel
+// takes 20 us at Nx = 8192: a single SM, ten barrier-separated passes): thread = (8 columns, a chunk of Nx / 128
+// consecutive cells j) with a rolling window of G in registers -- one value of rho, one new value of G and eight
+// multiply-adds per cell, fp32 (<= 128 products per partial sum); the partial sums meet in fp64 in a fixed order.
+// rho comes from the density kernel's last blocks (ticket), minus rho_0, rounded to fp32 like poisson_kernel's input.
+// Shared arrays are padded by one word per 32 (chunk starts are multiples of 32 cells apart).
+__global__ void __launch_bounds__(1024) green_field_kernel(int Nx, const double* __restrict__ green,
+                                                           const double* __restrict__ rho, float* __restrict__ E_a,
+                                                           double* __restrict__ energy_out, double* __restrict__ e_part,
+                                                           unsigned* __restrict__ ticket, double half_dx)
 {
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= Nx) return;
-    double s = 0.0;
-    for (int m = Nx / 2 - 1; m >= 1; --m) {
-        const int r = (int)(((long long)m * n) & (long long)(Nx - 1));
-        s += sinpi(2.0 * (double)r / (double)Nx) / (double)m;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double eS[8];
+    const int PN = Nx + (Nx >> 5);
+    float* const gS = reinterpret_cast<float*>(smem_raw);
+    float* const rS = gS + PN;
+    double* const sumS = reinterpret_cast<double*>(rS + PN);              // [32 warps][64 columns]
+    const int tid = threadIdx.x, xmask = Nx - 1;
+    for (int i = tid; i < Nx; i += 1024) gS[i + (i >> 5)] = (float)__ldg(green + i);      // (plan constant: before the wait)
+    if (blockIdx.x == 0) VOG_STAMP(10);
+    pdl_wait();                                   // rho comes from the density kernel
+    pdl_launch_dependents();
+    if (blockIdx.x == 0) VOG_STAMP(11);
+    const double ref = __ldcg(rho);
+    for (int i = tid; i < Nx; i += 1024) rS[i + (i >> 5)] = (float)(__ldcg(rho + i) - ref);
+    __syncthreads();
+    if (blockIdx.x == 0) VOG_STAMP(12);
+    const int oct = tid & 7, jp = tid >> 3, JC = Nx >> 7, j0 = jp * JC;
+    const int gb = (int)blockIdx.x * 64 + 8 * oct + 7 - j0;               // index of G for column c0 + 7 at cell j0
+    float w[8], acc[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = 0.0f;                             // acc[k]: column 64 blockIdx.x + 8 oct + 7 - k
+#pragma unroll
+    for (int k = 0; k < 7; ++k) { const int gi = (gb - k) & xmask; w[k] = gS[gi + (gi >> 5)]; }
+#pragma unroll 8
+    for (int i = 0; i < JC; ++i) {
+        const int gi = (gb - 7 - i) & xmask, j = j0 + i;
+        w[7] = gS[gi + (gi >> 5)];
+        const float rj = rS[j + (j >> 5)];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc[k] = fmaf(w[k], rj, acc[k]);
+#pragma unroll
+        for (int k = 0; k < 7; ++k) w[k] = w[k + 1];
     }
-    G[n] = s * L / (3.14159265358979323846 * (double)Nx);
+    if (blockIdx.x == 0) VOG_STAMP(13);
+    // the four chunks of a warp by shuffles, the 32 warps through shared memory
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        double d = (double)acc[k];
+        d += __shfl_xor_sync(0xffffffffu, d, 8);
+        d += __shfl_xor_sync(0xffffffffu, d, 16);
+        if ((tid & 31) < 8) sumS[(tid >> 5) * 64 + 8 * oct + 7 - k] = d;
+    }
+    __syncthreads();
+    if (blockIdx.x == 0) VOG_STAMP(14);
+    double e2 = 0.0;
+    if (tid < 256) {
+        const int col = tid >> 2, part = tid & 3;
+        double sv = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) sv += sumS[(8 * part + q) * 64 + col];
+        sv += __shfl_xor_sync(0xffffffffu, sv, 1);
+        sv += __shfl_xor_sync(0xffffffffu, sv, 2);
+        if (part == 0) {
+            const float ef = (float)sv;
+            E_a[blockIdx.x * 64 + col] = ef;
+            e2 = (double)ef * (double)ef;
+        }
+    }
+    if (blockIdx.x == 0) VOG_STAMP(15);
+    if (energy_out) {   // (1/2) dx sum_i E_i^2: CTA sums in CTA order by the last CTA to arrive
+        if (tid < 256) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) e2 += __shfl_xor_sync(0xffffffffu, e2, o);
+            if ((tid & 31) == 0) eS[tid >> 5] = e2;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            double tot = 0.0;
+            for (int q = 0; q < 8; ++q) tot += eS[q];
+            e_part[blockIdx.x] = tot;
+            __threadfence();
+            if (atomicAdd(ticket, 1u) == gridDim.x - 1u) {
+                __threadfence();
+                tot = 0.0;
+                for (int q = 0; q < (int)gridDim.x; ++q) tot += __ldcg(e_part + q);
+                energy_out[0] = half_dx * tot;
+                *ticket = 0u;
+            }
+        }
+    }
 }
 
 }  // namespace vog
@@ -668,6 +750,42 @@ struct vog_plan_s {
 using namespace vog;
 
 static int ilog2i(int n) { int l = 0; while ((1 << l) < n) ++l; return l; }
+
+// Green's function of the Fourier field solve on the host: G_n = (1/N) sum_{m != 0, N/2} e^{2 pi i m n / N} / (i k_m),
+// k_m = 2 pi m / L with m counted from -N/2: the inverse transform of the solver's own factors, by a plain radix-2
+// transform in fp64 (N <= 16384 is a power of two).  Real by symmetry.
+static void green_host(int N, double L, std::vector<double>& G)
+{
+    const long double PI = 3.14159265358979323846264338327950288L;
+    std::vector<double> re(N, 0.0), im(N, 0.0);
+    for (int m = 1; m < N; ++m) {
+        if (2 * m == N) continue;
+        const int ms = m < N / 2 ? m : m - N;
+        im[m] = (double)(-(long double)L / (2.0L * PI * (long double)ms * (long double)N));      // 1 / (i k) = -i / k
+    }
+    const int lg = ilog2i(N);
+    for (int i = 0; i < N; ++i) {                  // bit reversal
+        int r = 0;
+        for (int b = 0; b < lg; ++b) r |= ((i >> b) & 1) << (lg - 1 - b);
+        if (r > i) { std::swap(re[i], re[r]); std::swap(im[i], im[r]); }
+    }
+    for (int len = 2; len <= N; len <<= 1) {       // decimation in time, e^{+2 pi i / len}
+        const int half = len / 2;
+        std::vector<double> wr(half), wi(half);
+        for (int k = 0; k < half; ++k) {
+            const long double a = 2.0L * PI * (long double)k / (long double)len;
+            wr[k] = (double)cosl(a); wi[k] = (double)sinl(a);
+        }
+        for (int i0 = 0; i0 < N; i0 += len)
+            for (int k = 0; k < half; ++k) {
+                const int p = i0 + k, q = p + half;
+                const double tr = re[q] * wr[k] - im[q] * wi[k], ti = re[q] * wi[k] + im[q] * wr[k];
+                re[q] = re[p] - tr; im[q] = im[p] - ti;
+                re[p] += tr; im[p] += ti;
+            }
+    }
+    G.assign(re.begin(), re.end());
+}
 static bool pow2_in_range(int n) { return n >= 64 && n <= 16384 && (n & (n - 1)) == 0; }
 
 static void fill_roots(std::vector<float2>& h, int N)
@@ -979,16 +1097,16 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         if (e == cudaSuccess) e = cudaMemcpyAsync(P->vmu_tab, vt.data(), sizeof(float) * vt.size(), cudaMemcpyHostToDevice, P->st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
     }
-    if (e == cudaSuccess && P->os_v && Nx / 16 <= P->n_sm) {
-        // the default v kernel runs one piece per CTA on this grid: it can solve the field itself (field_then_v)
+    if (e == cudaSuccess && ((P->os_v && Nx / 16 <= P->n_sm) || Nx >= 4096)) {
+        // steps solve the field in x space (field_then_v): inside the v kernel where it runs one piece per CTA, by
+        // green_field_kernel on grids of 4096 columns or more
         e = cudaMalloc((void**)&P->green, sizeof(double) * Nx);
         // e_part: [Nx / 16] strip sums of E^2 | 1 word: ticket of the energy reduction | [Nx / 32] tickets of the density kernel
         if (e == cudaSuccess) e = cudaMalloc((void**)&P->e_part, sizeof(double) * (Nx / 16 + 1) + sizeof(unsigned) * (Nx / 32));
         if (e == cudaSuccess) e = cudaMemsetAsync(P->e_part, 0, sizeof(double) * (Nx / 16 + 1) + sizeof(unsigned) * (Nx / 32), P->st);
-        if (e == cudaSuccess) {
-            green_kernel<<<(Nx + 127) / 128, 128, 0, P->st>>>(Nx, p->L, P->green);
-            e = cudaGetLastError();
-        }
+        std::vector<double> gh;
+        green_host(Nx, p->L, gh);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(P->green, gh.data(), sizeof(double) * Nx, cudaMemcpyHostToDevice, P->st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(P->st);
         if (e == cudaSuccess) P->fuse_field = 1;
         else { free_plan(P); cudaGetLastError(); return e == cudaErrorMemoryAllocation ? VOG_ENOMEM : VOG_ECUDA; }
@@ -1376,9 +1494,35 @@ static cudaError_t run_field(vog_plan_s* P, const float* f, float* E_out, double
 static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, double dts, const float* Eext,
                                 double* energy_out)
 {
-    const bool fuse = P->fuse_field && P->green && P->os_v && P->method == 0 && P->osv_variant == 0 && P->solver == 0 &&
-                      src != dst;
+    const int Nx = P->p.Nx, Nv = P->p.Nv;
+    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
+    const bool xspace = P->fuse_field && P->green && P->solver == 0;
+    const bool fuse = xspace && Nx / 16 <= P->n_sm && P->os_v && P->method == 0 && P->osv_variant == 0 && src != dst;
     cudaError_t e;
+    if (xspace && !fuse && Nx >= 8192) {       // (at 4096 columns it only ties with the Poisson kernel: measured)
+        // density (its last blocks write rho) -> green_field_kernel (E_self, energy) -> v-advection
+        const bool pdl_was = t_pdl;
+        t_pdl = pdl_was && P->density_pdl;
+        e = launch_pdl(density_partial_kernel<false>, dim3(Nx / 32, P->nby), dim3(256), 0, P->st, src, Nx, Nv, Nv / P->nby,
+                       P->part, (double*)nullptr, 0.0, 0.0, reinterpret_cast<unsigned*>(P->e_part + Nx / 16 + 1), P->rho, dv);
+        t_pdl = pdl_was;
+        if (e != cudaSuccess) return e;
+        const size_t gsmem = sizeof(float) * 2 * (size_t)(Nx + Nx / 32) + sizeof(double) * 32 * 64;
+        e = set_max_smem((const void*)green_field_kernel, gsmem);
+        if (e != cudaSuccess) return e;
+        e = launch_pdl(green_field_kernel, dim3(Nx / 64), dim3(1024), gsmem, P->st, Nx, (const double*)P->green,
+                       (const double*)P->rho, P->E_self, energy_out, P->e_part,
+                       reinterpret_cast<unsigned*>(P->e_part + Nx / 16), 0.5 * P->p.L / (double)Nx);
+        if (e != cudaSuccess) return e;
+        P->launches += 2;
+        P->E_valid = true;
+        P->E_of = src;
+        e = run_setup(P, true, 1, dts, P->E_self, Eext, nullptr);
+        P->v_behind_field = true;
+        if (e == cudaSuccess) e = advect_v(P, src, dst, true);
+        P->v_behind_field = false;
+        return e;
+    }
     if (!fuse) {
         e = run_field(P, src, nullptr, energy_out);
         if (e == cudaSuccess) e = run_setup(P, true, 1, dts, P->E_self, Eext, nullptr);
@@ -1387,8 +1531,6 @@ static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, dou
         P->v_behind_field = false;
         return e;
     }
-    const int Nx = P->p.Nx, Nv = P->p.Nv;
-    const double dv = (P->p.vmax - P->p.vmin) / (double)Nv;
     const bool pdl_was = t_pdl;
     t_pdl = pdl_was && P->density_pdl;
     e = launch_pdl(density_partial_kernel<false>, dim3(Nx / 32, P->nby), dim3(256), 0, P->st, src, Nx, Nv, Nv / P->nby,

@@ -1,7 +1,9 @@
 """GPU parity of the field solve fused into the v kernel (csrc/vog_os2.cuh osv7_kernel, csrc/vog_lib.cu field_then_v;
 vog_plan_tune(30, 0/1)): on grids whose v kernel runs one piece per CTA (Nv >= 1024, Nx / 16 <= SMs) a step launches
 x, density, v, x -- no Poisson kernel; every v CTA computes E on its own 16 columns as the circular convolution of rho
-with the Green's function of the Fourier solve (E^_m = rho^_m / (i k_m), modes 0 and Nx/2 dropped).
+with the Green's function of the Fourier solve (E^_m = rho^_m / (i k_m), modes 0 and Nx/2 dropped).  On grids of
+8192 columns or more the same convolution is a kernel of its own (green_field_kernel, one CTA per 64 columns) in the
+single-CTA Poisson kernel's place.
 
 Checked here: the step and its field against the oracle (same tolerances as the unfused tests), against the unfused
 launch sequence, the electric energies of vog_run against the oracle's, both split orders, merged half steps,
@@ -56,7 +58,8 @@ def _steps(torch, vog, cfg, f, ext, n, fuse):
 
 @pytest.mark.parametrize("split", [0, 1])
 @pytest.mark.parametrize("idx,over", [(1, dict(Nx=1024, Nv=1024)), (2, dict(Nx=2048, Nv=1024)), (2, dict(Nx=256, Nv=2048)),
-                                      (1, dict(Nx=64, Nv=4096, kind=1, order=3)), (0, dict(Nx=2048, Nv=2048))])
+                                      (1, dict(Nx=64, Nv=4096, kind=1, order=3)), (0, dict(Nx=2048, Nv=2048)),
+                                      (1, dict(Nx=4096, Nv=1024)), (2, dict(Nx=8192, Nv=256)), (1, dict(Nx=16384, Nv=128))])
 def test_fused_field_step_against_oracle_and_unfused(torch, vog, oracle, idx, over, split):
     cfg = inputs.config(idx, split=split, **over)
     f = inputs.initial_f(cfg)
@@ -64,8 +67,9 @@ def test_fused_field_step_against_oracle_and_unfused(torch, vog, oracle, idx, ov
     n = 2
     f1, E1, l1 = _steps(torch, vog, cfg, f, ext, n, True)
     f0, E0, l0 = _steps(torch, vog, cfg, f, ext, n, False)
-    # one launch fewer per fused field solve (XVX: one per step; VXV: the first step's opening solve stays unfused)
-    assert l0 - l1 == n
+    # one launch fewer per fused field solve (XVX: one per step; VXV: the first step's opening solve stays unfused);
+    # from 8192 columns on the x-space solve is a kernel of its own (green_field_kernel in the Poisson kernel's place)
+    assert l0 - l1 == (n if cfg.Nx <= 2048 else 0)
     feq = oracle.Feq.make(cfg.feq)
     fo, Eo = f.astype(np.float64), None
     for _ in range(n):
@@ -98,12 +102,13 @@ def test_fused_field_is_the_fourier_solve(torch, vog, oracle):
     plan.destroy()
 
 
+@pytest.mark.parametrize("Nx,Nv", [(1024, 1024), (8192, 256)])
 @pytest.mark.parametrize("merge", [False, True])
 @pytest.mark.parametrize("split", [0, 1])
-def test_fused_field_run_energies(torch, vog, oracle, split, merge):
+def test_fused_field_run_energies(torch, vog, oracle, split, merge, Nx, Nv):
     """vog_run with an energy per field solve: the fused reduction (strip sums added in strip order by the last strip
-    to arrive) against the unfused kernel's and, unmerged, against the oracle's steps."""
-    cfg = inputs.config(1, Nx=1024, Nv=1024, split=split)
+    to arrive; CTA sums in green_field_kernel) against the unfused kernel's and, unmerged, against the oracle's steps."""
+    cfg = inputs.config(1, Nx=Nx, Nv=Nv, split=split)
     f = inputs.initial_f(cfg)
     n = 3
     outs = []
@@ -136,7 +141,7 @@ def test_fused_field_repeats_bit_for_bit_and_is_off_where_it_cannot_run(torch, v
     a = _steps(torch, vog, cfg, f, None, 3, True)
     b = _steps(torch, vog, cfg, f, None, 3, True)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
-    plan = vog.Plan(4096, 1024, 1.0, -1.0, 1.0)          # 256 strips > SMs: several pieces per CTA, no Green's function
+    plan = vog.Plan(1024, 256, 1.0, -1.0, 1.0)           # whole-line v kernel, fewer than 4096 columns: no Green's function
     with pytest.raises(vog.VogError):
         plan.tune(30, 1)
     plan.destroy()
