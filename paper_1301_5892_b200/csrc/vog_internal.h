@@ -123,6 +123,9 @@ struct OsArgs {
     unsigned inv_np;       // x: ceil(2^16 / np)
     int n_lines;           // x: number of lines (the last line group may be ragged)
     int lam_ks;            // v: row stride of the transposed symbol table [k][column] in float2 (Nx + 16)
+    int inplace;           // v (osv7_kernel): dst == src, whole strips per CTA, stored in place where the shifts allow it
+    float* dst2;           // ... second grid for the strips whose shifts do not
+    int* strip_flags;      // ... [Nx / 16] 1 = the strip went to dst2 (cleared by the copy-back kernel)
 };
 
 struct OsSetupArgs {
@@ -158,6 +161,7 @@ int osx7_occupancy(int geom, int threads, size_t smem);
 cudaError_t osx6_launch(const OsArgs& a, int geom, int grid, int threads, size_t smem, cudaStream_t st);
 int osx6_occupancy(int geom, int threads, size_t smem);
 cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_sm, cudaStream_t st);
+cudaError_t strip_copy_launch(float* dst, const float* src, int* strip_flags, int Nx, int Nv, cudaStream_t st);
 cudaError_t osv6_launch(const OsArgs& a, int geom, dim3 grid, cudaStream_t st);
 cudaError_t osv4_launch(const OsArgs& a, int geom, dim3 grid, int threads, size_t smem, cudaStream_t st);
 

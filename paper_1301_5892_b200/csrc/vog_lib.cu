@@ -731,8 +731,11 @@ struct vog_plan_s {
     double* e_part;             // [Nx / 16] + ticket word: energy reduction of the fused field solve
     int fuse_field;             // steps: density -> v kernel with the field solve inside (no Poisson launch); 0 / 1
     int v_spec;                 // v kernel: first windows requested before the shifts are known (default 1)
+    int v_inplace;              // vog_advect_v / vog_shift_v: the v kernel stores in place where the shifts allow it (default 1)
+    int* strip_flags;           // [Nx / 16] strips of the last in-place v-advection that went to the second grid
     int density_pdl;            // density kernel launched with the programmatic-dependent-launch attribute (0 / 1)
     bool v_behind_field;        // ... set by field_then_v around its v launch
+    bool v_inplace_now;         // set by advect_v_inplace around its v launch
     float *feq_tab, *vmu_tab;   // [ng][Nv]
     int nby, nby_max;           // density: row slabs per column group (tunable up to the allocated nby_max)
     int lognl_x, lognl_v, thr_x, thr_v;
@@ -911,7 +914,7 @@ static void free_plan(vog_plan_s* P)
     vog::f64_destroy(P->f64);
     cudaFree(P->xtwA); cudaFree(P->xtwB); cudaFree(P->xcs); cudaFree(P->xrec);
     cudaFree(P->tw_x); cudaFree(P->tw_v); cudaFree(P->rec_x); cudaFree(P->rec_v);
-    cudaFree(P->part); cudaFree(P->partk); cudaFree(P->diag); cudaFree(P->rho); cudaFree(P->E_self); cudaFree(P->green); cudaFree(P->e_part);
+    cudaFree(P->part); cudaFree(P->partk); cudaFree(P->diag); cudaFree(P->rho); cudaFree(P->E_self); cudaFree(P->green); cudaFree(P->e_part); cudaFree(P->strip_flags);
     cudaFree(P->feq_tab); cudaFree(P->vmu_tab); cudaFree(P->f_buf); cudaFree(P->ext_buf);
     delete P;
 }
@@ -963,6 +966,7 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     P->os_x = Nx >= 1024;
     P->os_v = Nv >= 1024;
     P->v_spec = 1;
+    P->v_inplace = 1;
     // (measured: behind an x kernel of a grid of 4096^2 cells or more the density kernel's 512 long-running blocks do
     // worse when they trickle onto the SMs as the x kernel drains -- 8192^2 step 484 us with the attribute, 451 us
     // without; on the 2048^2 grid the early start wins: 51.6 against 54.7 us)
@@ -1059,6 +1063,8 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
     alloc((void**)&P->partk, sizeof(double) * P->nby_max * Nx);
     alloc((void**)&P->diag, sizeof(double) * 8);
     alloc((void**)&P->rho, sizeof(double) * Nx);
+    alloc((void**)&P->strip_flags, sizeof(int) * (Nx / 16 + 1));
+    if (e == cudaSuccess) e = cudaMemsetAsync(P->strip_flags, 0, sizeof(int) * (Nx / 16 + 1), P->st);
     alloc((void**)&P->E_self, sizeof(float) * Nx);
     alloc((void**)&P->feq_tab, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512));   // + padding read (not used) by osv2_kernel
     if (e == cudaSuccess) e = cudaMemsetAsync(P->feq_tab, 0, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512), P->st);
@@ -1177,6 +1183,7 @@ extern "C" int vog_plan_tune(vog_plan_t P, int which, int value)
         case 30: if (value < 0 || value > 1 || (value == 1 && !P->green)) return VOG_EINVAL; P->fuse_field = value; break;
         case 31: if (value < 0 || value > 1) return VOG_EINVAL; P->v_spec = value; break;
         case 33: if (value < 0 || value > 1) return VOG_EINVAL; P->density_pdl = value; break;
+        case 34: if (value < 0 || value > 1) return VOG_EINVAL; P->v_inplace = value; break;
         case 29: if (value < 0 || value > 1 || P->p.Nx > 256 || P->p.Nv > 256) return VOG_EINVAL; P->small_run = value; break;
         case 28: if (value < 0 || value > 2) return VOG_EINVAL; P->solver = value; P->E_of = nullptr; P->E_valid = false; break;
         case 27: if (value < 0 || value > 1) return VOG_EINVAL; P->method = value; P->recx_valid = false; P->E_of = nullptr; break;
@@ -1333,6 +1340,8 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
         // (the first windows may be requested before the kernel's wait only when the kernel in front of it on the
         // stream is not the one that writes src: true behind a field solve, whose kernels only read the grid)
         P->vsetup.spec = P->v_spec && P->v_behind_field;
+        a.inplace = P->v_inplace_now ? 1 : 0;
+        a.dst2 = P->g_buf; a.strip_flags = P->strip_flags;
         return osv7_launch(a, P->vsetup, geom, P->n_sm, P->st);
     }
     if (P->osv_variant == 2) {
@@ -1435,6 +1444,15 @@ static cudaError_t advect_v_inplace(vog_plan_s* P, float* f, bool source)
 {
     if (!P->os_v) return run_advect_line(P, f, true, source);
     cudaError_t e = ensure_gbuf(P);
+    if (e == cudaSuccess && P->method == 0 && P->osv_variant == 0 && P->v_inplace) {
+        // whole strips per CTA, stored in place where the integer shifts stay inside the kernel's saved halo (<= 24 rows);
+        // the other strips go through the second grid and are copied back by a second, otherwise empty, launch
+        P->v_inplace_now = true;
+        e = run_osv(P, f, f, source);
+        P->v_inplace_now = false;
+        if (e == cudaSuccess) { e = strip_copy_launch(f, P->g_buf, P->strip_flags, P->p.Nx, P->p.Nv, P->st); P->launches++; }
+        return e;
+    }
     if (e == cudaSuccess) e = P->method == 1 ? run_stv(P, f, P->g_buf, source) : run_osv(P, f, P->g_buf, source);
     if (e == cudaSuccess) e = copy_grid(P, f, P->g_buf);
     return e;

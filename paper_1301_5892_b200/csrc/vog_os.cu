@@ -333,6 +333,30 @@ cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_
     return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a, su, maps);
 }
 
+// In-place v-advection, second launch: the strips that osv7_kernel could not store in place (integer shifts beyond its
+// saved halo) lie in the second grid; copy them back and clear their flags.  One CTA per strip: 64-byte row segments,
+// four threads per row.  A launch in which no strip is flagged reads Nx / 16 words and ends.
+__global__ void __launch_bounds__(256) strip_copy_kernel(float* __restrict__ dst, const float* __restrict__ src,
+                                                         int* __restrict__ strip_flags, int Nx, int Nv)
+{
+    pdl_wait();                                   // flags and the second grid come from the v kernel
+    pdl_launch_dependents();
+    const int strip = blockIdx.x;
+    if (strip_flags[strip] == 0) return;          // (uniform over the CTA)
+    const size_t off = (size_t)strip * os2::VW + (threadIdx.x & 3) * 4;
+    for (int r = threadIdx.x >> 2; r < Nv; r += 64) {
+        const float4 v = *reinterpret_cast<const float4*>(src + (size_t)r * Nx + off);
+        *reinterpret_cast<float4*>(dst + (size_t)r * Nx + off) = v;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) strip_flags[strip] = 0;
+}
+
+cudaError_t strip_copy_launch(float* dst, const float* src, int* strip_flags, int Nx, int Nv, cudaStream_t st)
+{
+    return launch_pdl(strip_copy_kernel, dim3(Nx / os2::VW), dim3(256), 0, st, dst, src, strip_flags, Nx, Nv);
+}
+
 // 16-column-strip v kernel, symbol through L1; grid = (Nx / 16, ceil(np / gpc))
 cudaError_t osv6_launch(const OsArgs& a, int geom, dim3 grid, cudaStream_t st)
 {

@@ -926,6 +926,15 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     // exchange buffers of the three groups are free until the first pass A and hold, in this order, rho (Nx doubles),
     // the Green's function of the Fourier solve (Nx doubles, a plan constant: loaded before the wait) and the partial
     // sums of the convolution.
+    // In-place mode (a.inplace: dst == src, whole strips per CTA; vog_advect_v / vog_shift_v).  A strip's pairs are
+    // stored in place as long as every window that still needs the overwritten rows is already on chip: the store of
+    // pair p waits until the windows of pairs p - 1 and p + 1 have landed (landedS: last pair landed per group), and the
+    // strip's first IPH rows, which the LAST pair's window reads again after the wrap, are kept in saveS.  That holds
+    // for integer shifts up to IPB rows; a strip with larger shifts is written to the second grid a.dst2 instead and
+    // flagged for the copy-back kernel (vog_os.cu strip_copy_kernel).
+    constexpr int IPH = 40, IPB = 24;
+    __shared__ float saveS[IPH * W];
+    __shared__ volatile int landedS[3];
     __shared__ float fusedE[W];
     __shared__ float4 srcRS[4 * W];               // delta-f source: (e^h, expm1 h, e^-h, expm1 -h), h = 16 rows, per (Gaussian, column)
     __shared__ float2 srcRV[4 * W];               // ... and (e^{g V}, expm1(g V)): block B from block A
@@ -944,6 +953,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     const int Rr = nstrips / G, Lt = nstrips - Rr * G;
     const int tlo = (int)((long long)Lt * np * kb / G), thi = (int)((long long)Lt * np * (kb + 1) / G);
     auto piece = [&](const int i, int& strip, int& q0, int& q1) -> bool {
+        if (a.inplace) { strip = i * G + kb; q0 = 0; q1 = np; return strip < nstrips; }
         if (i < Rr) { strip = i * G + kb; q0 = 0; q1 = np; return true; }
         if (Rr == 0) {
             // fewer strips than CTAs (grids up to 2048 columns): a share of pairs would straddle two strips and pay two
@@ -1045,12 +1055,14 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         return g;
     };
     // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
-    auto land = [&](const Geo& g, const int p) {
+    auto land = [&](const Geo& g, const int p, const bool use_save = false) {
         const int rs = p * (2 * V) - HLO + g.base;
         if (!g.gather) {
+            const int gr0 = rs & vmask, n1 = min(g.nrows, Nv - gr0);       // rows before the wrap to row 0
+            const int ns = use_save ? min(g.nrows - n1, IPH) : 0;          // wrapped rows taken from the save area
             if (gt == 0) {
-                os2::mbar_expect_tx(vbar, (unsigned)g.nrows * (W * 4u));
-                int gr = rs & vmask, sr = 0;
+                os2::mbar_expect_tx(vbar, (unsigned)(g.nrows - ns) * (W * 4u));
+                int gr = gr0, sr = 0;
                 for (int sg = 0; sg < 2 && sr < g.nrows; ++sg) {
                     int n = min(g.nrows - sr, Nv - gr);          // (a window past the last row wraps to row 0)
 #pragma unroll 1
@@ -1061,9 +1073,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                             gr += hb; sr += hb; n -= hb;
                         }
                     }
-                    gr = 0;
+                    gr = ns; sr += ns;
                 }
             }
+            for (int i = gt; i < ns * W; i += 256) raw[n1 * W + i] = saveS[i];
         } else {
             const float* const col = a.src + g.c0 + c;
             for (int r = h; r < g.nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
@@ -1189,6 +1202,14 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         const Geo g = geometry(strip * W, rec);
         const float ssh = rec[19 * W + c];
         const int p0 = q0 + gid;
+        bool ipok = false;
+        if (a.inplace) {
+            const int sb = ((g.base + (Nv >> 1)) & vmask) - (Nv >> 1);     // first window row as a signed shift
+            ipok = !g.gather && sb >= -4 * IPB && sb + (g.nrows - (V + OS_LB)) <= IPB;
+            for (int i = tid; i < IPH * W; i += 768) saveS[i] = __ldcg(a.src + (size_t)(i >> 4) * Nx + g.c0 + (i & (W - 1)));
+            if (tid < 3) landedS[tid] = -1;
+            if (tid == 0 && !ipok) a.strip_flags[strip] = 1;
+        }
         int db_first = g.db;                       // row offset of this lane in the window of the group's first pair
         if (spec) {
             // does the speculative window hold the rows of every column?  first row needed by this lane, relative to
@@ -1256,10 +1277,11 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         Geo gn = g;
         if (nhas) gn = geometry(nstrip * W, cfS + ((it + 1) % 3) * CF);
         const int np0 = nq0 + gid;
-        float* const ocol = a.dst + g.c0 + c;
+        float* const ocol = ((a.inplace && !ipok) ? a.dst2 : a.dst) + g.c0 + c;
         for (int p = p0; p < q1; p += 3) {
             if (g.gather) os2::cp_async_wait_all();
             else { os2::mbar_wait(vbar, vpar); vpar ^= 1u; }
+            if (ipok && gt == 0) landedS[gid] = p;
             OS_STAMP(5 + 4 * ((p - p0) / 3));
             os2::bar_group(gid + 1);               // raw rows of pair p visible; exchange buffer of the last pair read
             // ---- pass A (item t = h): samples from the raw rows with this lane's offset
@@ -1278,7 +1300,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             OS_STAMP(6 + 4 * ((p - p0) / 3));
             // the next window lands behind the middle stage and the inverse pass: this piece's, or -- after the group's
             // last pair of the piece -- the group's first of the NEXT piece (its shifts are known two pieces ahead)
-            if (p + 3 < q1) land(g, p + 3);
+            if (p + 3 < q1) land(g, p + 3, ipok);
             else if (nhas && np0 < nq1) { land(gn, np0); pref = true; }
             // ---- middle stage (item g = h): positions 16 g + j
             {
@@ -1289,6 +1311,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 os2::mid16<W>(x, lamS + c, h);
 #pragma unroll
                 for (int j = 0; j < 16; ++j) sp[j * W] = x[j];
+            }
+            if (ipok && gt == 0) {                 // in place: the neighbours' windows must be on chip before these rows change
+                if (p + 1 < q1) while (landedS[(gid + 1) % 3] < p + 1) { }
+                if (p > q0) while (landedS[(gid + 2) % 3] < p - 1) { }
             }
             os2::bar_group(gid + 1);
             OS_STAMP(7 + 4 * ((p - p0) / 3));
