@@ -169,8 +169,8 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *   25     block geometry of the overlap-save kernels: 1 = 232 kept samples, 8 + 16 discarded (Lagrange
  *          plans only, their default), 0 = 224 kept, 16 + 16 discarded (the cubic spline's);
  *   26     programmatic dependent launch of the plan's kernels: 1 = each kernel may be staged on the SMs while its
- *          predecessor in the stream drains and waits for it on the device (default up to 8192 x 8192), 0 = plain
- *          stream order.  Results are bit-identical either way.
+ *          predecessor in the stream drains and waits for it on the device (default), 0 = plain stream order.
+ *          Results are bit-identical either way.
  *   27     how the circulant product of lines >= 1024 cells is taken: 0 = in Fourier space (default: FFT, symbol,
  *          inverse FFT, P:131-149 -- the path BASELINE.json names), 1 = directly, u'_i = sum_j a_j u_(i+b+j) with the
  *          2d+2 non-zero entries of the row of A (eq (4); the spline's row cut at |j| <= 14 like the

@@ -983,8 +983,9 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
         P->os2x_lpi = l2; P->os3x_occ = 0; P->os2v_gpc = 0;
     }
-    // measured (profiles/r1i_pdl_setup.md): 512^2 step -20 %, 2048^2 -15 %, 8192^2 +-0, 16384^2 +1.3 %
-    P->pdl = (long long)Nx * Nv <= (1ll << 26) ? 1 : 0;
+    // measured (profiles/r1i_pdl_setup.md): 512^2 step -20 %, 2048^2 -15 %, 8192^2 +-0; the +1.3 % at 16384^2 of round 1
+    // was the density kernel (launched without the attribute on large grids since, see density_pdl): now -0.5..-4 %
+    P->pdl = 1;
     P->x_nbuf = 1;   // measured: 4 single-buffered CTAs/SM beat 3 double-buffered ones (L1 keeps the twiddles)
     default_tile(Nv, Nx, true, &P->lognl_v, &P->thr_v);
     cudaError_t e = cudaSuccess;
