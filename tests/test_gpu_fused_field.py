@@ -145,3 +145,52 @@ def test_fused_field_repeats_bit_for_bit_and_is_off_where_it_cannot_run(torch, v
     with pytest.raises(vog.VogError):
         plan.tune(30, 1)
     plan.destroy()
+
+
+@pytest.mark.parametrize("which", [31, 33])
+@pytest.mark.parametrize("idx,over", [(1, dict(Nx=2048, Nv=2048)), (2, dict(Nx=1024, Nv=2048)), (1, dict(Nx=8192, Nv=1024))])
+def test_launch_shape_switches_do_not_change_a_bit(torch, vog, which, idx, over):
+    """vog_plan_tune(31, .) (first windows of the v kernel requested before / after the shifts are known) and (33, .)
+    (density kernel with / without the dependent-launch attribute) only change WHEN things are requested: 3 steps with an
+    external field must come out bit for bit the same, field included."""
+    cfg = inputs.config(idx, **over)
+    f = inputs.initial_f(cfg)
+    ext = (0.3 * np.cos(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx)).astype(np.float32)
+    outs = []
+    for value in (0, 1):
+        plan = vog.Plan.from_config(cfg)
+        plan.tune(which, value)
+        fd = _dev(torch, f)
+        ed = _dev(torch, ext)
+        for _ in range(3):
+            plan.step(fd, cfg.dt, ed)
+        E = torch.empty(cfg.Nx, device="cuda", dtype=torch.float32)
+        plan.get_field(E)
+        torch.cuda.synchronize()
+        outs.append((fd.cpu().numpy(), E.cpu().numpy()))
+        plan.destroy()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+def test_speculative_window_is_redone_when_the_shifts_are_large(torch, vog, oracle):
+    """A strong external field gives integer shifts far beyond the +-16 rows the speculative window covers: the v kernel
+    must drop it and request the right rows (parity with the oracle's step, and the same bits as without speculation)."""
+    cfg = inputs.config(1, Nx=1024, Nv=2048)
+    f = inputs.initial_f(cfg)
+    dv = (cfg.vmax - cfg.vmin) / cfg.Nv
+    ext = (60.0 * dv / cfg.dt * np.sin(2 * math.pi * np.arange(cfg.Nx) / cfg.Nx)).astype(np.float32)   # up to 60 rows
+    outs = []
+    for spec in (1, 0):
+        plan = vog.Plan.from_config(cfg)
+        plan.tune(31, spec)
+        fd = _dev(torch, f)
+        plan.step(fd, cfg.dt, _dev(torch, ext))
+        torch.cuda.synchronize()
+        outs.append(fd.cpu().numpy())
+        plan.destroy()
+    assert np.array_equal(outs[0], outs[1])
+    fo, _ = oracle.step(f.astype(np.float64), cfg.L, cfg.vmin, cfg.vmax, cfg.dt, cfg.kind, cfg.order,
+                        oracle.Feq.make(cfg.feq), cfg.split, ext.astype(np.float64))
+    # (the delta-f source of a 60-row shift is of order one: reading Q21b, the scale is that of the update)
+    scale = max(float(np.abs(f).max()), float(np.abs(fo).max()))
+    assert np.abs(outs[0] - fo).max() <= 3 * TOL * scale
