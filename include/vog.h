@@ -198,10 +198,11 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *          -- and requests them again if the shifts turn out larger; 0 = after the shifts are known.
  *   33     density kernel launched with (1) or without (0) the programmatic-dependent-launch attribute of code 26
  *          (default: with it below 4096 x 4096 cells, without it from there on).
- *   34     vog_advect_v / vog_shift_v with Nv >= 1024: 1 (default) = the v kernel works on whole 16-column strips and
- *          stores them IN PLACE wherever a strip's integer shifts are at most 24 rows (a store waits until the windows
- *          that still need the rows are on chip); strips with larger shifts go through the plan's second grid and are
- *          copied back by a second launch.  0 = every strip through the second grid and a copy of the whole grid.
+ *   34     vog_advect_v / vog_shift_v with Nv >= 1024: 1 (default) = the v kernel stores IN PLACE wherever a strip's
+ *          integer shifts are at most 24 rows (a store waits until the windows that still need the rows are on chip; the
+ *          rows on either side of a piece of work are saved first); strips with larger shifts go through the plan's
+ *          second grid and are copied back by a second launch.  0 = every strip through the second grid and a copy of
+ *          the whole grid.
  * VOG_EINVAL for an unknown code or a shape that does not fit (shared memory, grid). */
 int vog_plan_tune(vog_plan_t plan, int which, int value);
 

@@ -926,15 +926,22 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     // exchange buffers of the three groups are free until the first pass A and hold, in this order, rho (Nx doubles),
     // the Green's function of the Fourier solve (Nx doubles, a plan constant: loaded before the wait) and the partial
     // sums of the convolution.
-    // In-place mode (a.inplace: dst == src, whole strips per CTA; vog_advect_v / vog_shift_v).  A strip's pairs are
+    // In-place mode (a.inplace: dst == src; vog_advect_v / vog_shift_v).  A strip's pairs are
     // stored in place as long as every window that still needs the overwritten rows is already on chip: the store of
     // pair p waits until the windows of pairs p - 1 and p + 1 have landed (landedS: last pair landed per group), and the
     // strip's first IPH rows, which the LAST pair's window reads again after the wrap, are kept in saveS.  That holds
     // for integer shifts up to IPB rows; a strip with larger shifts is written to the second grid a.dst2 instead and
     // flagged for the copy-back kernel (vog_os.cu strip_copy_kernel).
+    // Pieces that are not whole strips (the balanced shares of the strips left over, or several CTAs per strip on narrow
+    // grids) border on rows that ANOTHER CTA stores: every CTA first copies the IPH rows on either side of its pieces
+    // into a.halo (global scratch) and arrives on a.ipsync; nobody starts such a piece before all have arrived, and a
+    // piece's first / last window takes the rows beyond its own range from there.
     constexpr int IPH = 40, IPB = 24;
     __shared__ float saveS[IPH * W];
     __shared__ volatile int landedS[3];
+    const float* hlo = nullptr;                    // rows [Lw - IPH, Lw) below the current piece (original values)
+    const float* hup = saveS;                      // rows [Uw, Uw + IPH) above it (whole strips: the strip's first rows)
+    int Lw = 0, Uw = Nv;                           // first row of the piece, first row behind it (unwrapped)
     __shared__ float fusedE[W];
     __shared__ float4 srcRS[4 * W];               // delta-f source: (e^h, expm1 h, e^-h, expm1 -h), h = 16 rows, per (Gaussian, column)
     __shared__ float2 srcRV[4 * W];               // ... and (e^{g V}, expm1(g V)): block B from block A
@@ -953,7 +960,6 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     const int Rr = nstrips / G, Lt = nstrips - Rr * G;
     const int tlo = (int)((long long)Lt * np * kb / G), thi = (int)((long long)Lt * np * (kb + 1) / G);
     auto piece = [&](const int i, int& strip, int& q0, int& q1) -> bool {
-        if (a.inplace) { strip = i * G + kb; q0 = 0; q1 = np; return strip < nstrips; }
         if (i < Rr) { strip = i * G + kb; q0 = 0; q1 = np; return true; }
         if (Rr == 0) {
             // fewer strips than CTAs (grids up to 2048 columns): a share of pairs would straddle two strips and pay two
@@ -1055,28 +1061,41 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         return g;
     };
     // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
-    auto land = [&](const Geo& g, const int p, const bool use_save = false) {
+    // mode (in place only): 1 = the rows below the piece come from hlo, 2 = the rows behind it from hup
+    auto land = [&](const Geo& g, const int p, const int mode = 0) {
         const int rs = p * (2 * V) - HLO + g.base;
         if (!g.gather) {
-            const int gr0 = rs & vmask, n1 = min(g.nrows, Nv - gr0);       // rows before the wrap to row 0
-            const int ns = use_save ? min(g.nrows - n1, IPH) : 0;          // wrapped rows taken from the save area
+            // unwrapped first row of the window (the shift as a signed number), rows from the two halos
+            const int urs = p * (2 * V) - HLO + (((g.base + (Nv >> 1)) & vmask) - (Nv >> 1));
+            const int nA = (mode & 1) ? min(max(Lw - urs, 0), g.nrows) : 0;
+            const int over = urs + g.nrows - Uw;
+            const int nC = (mode & 2) ? min(max(over, 0), IPH) : 0;
             if (gt == 0) {
-                os2::mbar_expect_tx(vbar, (unsigned)(g.nrows - ns) * (W * 4u));
-                int gr = gr0, sr = 0;
-                for (int sg = 0; sg < 2 && sr < g.nrows; ++sg) {
-                    int n = min(g.nrows - sr, Nv - gr);          // (a window past the last row wraps to row 0)
+                os2::mbar_expect_tx(vbar, (unsigned)(g.nrows - nA - nC) * (W * 4u));
+                // global rows: [urs + nA, e1) and, behind the upper halo, [Uw + nC, urs + nrows) (rows that only feed
+                // discarded samples); each run wraps at the last row of the grid
+                const int e1 = nC > 0 ? Uw : urs + g.nrows;
+                for (int run = 0; run < 2; ++run) {
+                    int ur = run == 0 ? urs + nA : Uw + nC;
+                    const int ue = run == 0 ? e1 : urs + g.nrows;
+                    if (run == 1 && nC == 0) break;
+                    while (ur < ue) {
+                        int gr = ur & vmask, sr = ur - urs;
+                        int n = min(ue - ur, Nv - gr);               // (a window past the last row wraps to row 0)
+                        ur += n;
 #pragma unroll 1
-                    for (int i = 0; i < 5; ++i) {
-                        const int hb = os2::vbox_rows(i);
-                        while (n >= hb) {
-                            os2::tensor_g2s(raw + sr * W, &maps.m[i], g.c0, gr, vbar);
-                            gr += hb; sr += hb; n -= hb;
+                        for (int i = 0; i < 5; ++i) {
+                            const int hb = os2::vbox_rows(i);
+                            while (n >= hb) {
+                                os2::tensor_g2s(raw + sr * W, &maps.m[i], g.c0, gr, vbar);
+                                gr += hb; sr += hb; n -= hb;
+                            }
                         }
                     }
-                    gr = ns; sr += ns;
                 }
             }
-            for (int i = gt; i < ns * W; i += 256) raw[n1 * W + i] = saveS[i];
+            for (int i = gt; i < nA * W; i += 256) raw[i] = hlo[(IPH - nA) * W + i];
+            for (int i = gt; i < nC * W; i += 256) raw[(Uw - urs) * W + i] = hup[i];
         } else {
             const float* const col = a.src + g.c0 + c;
             for (int r = h; r < g.nrows; r += 16) os2::cp_async4(raw + r * W + c, col + (size_t)((rs + r) & vmask) * Nx);
@@ -1104,6 +1123,23 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     pdl_launch_dependents();
     OS_STAMP(1);
     OS_BLK(1);
+    if (a.inplace) {
+        int s0, qa, qb, li = 0;
+        for (int i = 0; li < 4 && piece(i, s0, qa, qb); ++i) {
+            if (qa == 0 && qb == np) continue;
+            float* const hs = a.halo + (size_t)(kb * 4 + li) * (2 * IPH * W);
+            const int lw = qa * (2 * V), uw = qb < np ? qb * (2 * V) : Nv;
+            for (int j = tid; j < 2 * IPH * W; j += 768) {
+                const int side = j >= IPH * W, r = (j - side * IPH * W) >> 4, cc = j & (W - 1);
+                const int row = (side ? uw + r : lw - IPH + r) & vmask;
+                hs[j] = __ldcg(a.src + (size_t)row * Nx + s0 * W + cc);
+            }
+            ++li;
+        }
+        __syncthreads();
+        if (tid == 0) { __threadfence(); atomicAdd(a.ipsync, 1u); }
+    }
+    int li_cur = 0;                                // pieces of this CTA that were not whole strips, so far
     if (su.fpart) {
         // S9 for the 16 columns of this strip.  rho_i (the density kernel's last blocks wrote it: dv * the slab sums in
         // the order of poisson_kernel) minus rho_0 (any constant only changes mode 0, which is dropped: P:205-211),
@@ -1203,13 +1239,32 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         const float ssh = rec[19 * W + c];
         const int p0 = q0 + gid;
         bool ipok = false;
+        const bool whole = q0 == 0 && q1 == np;
         if (a.inplace) {
             const int sb = ((g.base + (Nv >> 1)) & vmask) - (Nv >> 1);     // first window row as a signed shift
-            ipok = !g.gather && sb >= -4 * IPB && sb + (g.nrows - (V + OS_LB)) <= IPB;
-            for (int i = tid; i < IPH * W; i += 768) saveS[i] = __ldcg(a.src + (size_t)(i >> 4) * Nx + g.c0 + (i & (W - 1)));
+            ipok = !g.gather && sb >= (whole ? -4 * IPB : 8 - IPH) && sb + (g.nrows - (V + OS_LB)) <= IPB;
+            Lw = q0 * (2 * V);
+            Uw = q1 < np ? q1 * (2 * V) : Nv;
+            if (whole) {
+                hup = saveS;
+            } else {
+                hlo = a.halo + (size_t)(kb * 4 + min(li_cur, 3)) * (2 * IPH * W);
+                hup = hlo + IPH * W;
+                ++li_cur;
+                // every CTA has saved its halos before anybody stores into a strip that is shared between CTAs
+                if (tid == 0) while (*reinterpret_cast<volatile unsigned*>(a.ipsync) < gridDim.x) { }
+                __syncthreads();
+            }
             if (tid < 3) landedS[tid] = -1;
             if (tid == 0 && !ipok) a.strip_flags[strip] = 1;
         }
+        // which halos the window of pair p takes (in place): whole strips only the wrap behind the last row, and only for
+        // windows requested after the strip's first stores; other pieces both sides, always
+        auto lmode = [&](const int p) -> int {
+            if (!ipok) return 0;
+            if (whole) return p >= q0 + 3 ? 2 : 0;
+            return (p == q0 ? 1 : 0) | (p == q1 - 1 ? 2 : 0);
+        };
         int db_first = g.db;                       // row offset of this lane in the window of the group's first pair
         if (spec) {
             // does the speculative window hold the rows of every column?  first row needed by this lane, relative to
@@ -1223,8 +1278,11 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 land(g, p0);
             }
             spec = false;
-        } else if (!pref && p0 < q1) land(g, p0);
+        } else if (!pref && p0 < q1) land(g, p0, lmode(p0));
         pref = false;
+        if (a.inplace && whole)                    // (behind the first requests: the table barrier below orders it before any store)
+            for (int i = tid; i < IPH * W; i += 768)
+                saveS[i] = __ldcg(a.src + (size_t)(i >> 4) * Nx + g.c0 + (i & (W - 1)));
         if (tid < 6 * a.ng * W) {
             // delta-f source constants of (Gaussian gg, column cc): same expressions as osv2_source without a table,
             // one transcendental per thread (two warps computing all six per entry were the slowest of this phase)
@@ -1300,8 +1358,8 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             OS_STAMP(6 + 4 * ((p - p0) / 3));
             // the next window lands behind the middle stage and the inverse pass: this piece's, or -- after the group's
             // last pair of the piece -- the group's first of the NEXT piece (its shifts are known two pieces ahead)
-            if (p + 3 < q1) land(g, p + 3, ipok);
-            else if (nhas && np0 < nq1) { land(gn, np0); pref = true; }
+            if (p + 3 < q1) land(g, p + 3, lmode(p + 3));
+            else if (nhas && np0 < nq1 && !(a.inplace && !(nq0 == 0 && nq1 == np))) { land(gn, np0); pref = true; }
             // ---- middle stage (item g = h): positions 16 g + j
             {
                 float2* const sp = exch + h * 16 * W + c;
@@ -1313,6 +1371,8 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 for (int j = 0; j < 16; ++j) sp[j * W] = x[j];
             }
             if (ipok && gt == 0) {                 // in place: the neighbours' windows must be on chip before these rows change
+                // (publishing a group's window in flight as soon as its barrier completes, instead of when the group
+                // gets to it, was measured: 144 -> 149 us at 8192^2, the polling costs more than the wait)
                 if (p + 1 < q1) while (landedS[(gid + 1) % 3] < p + 1) { }
                 if (p > q0) while (landedS[(gid + 2) % 3] < p - 1) { }
             }
@@ -1338,6 +1398,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         OS_BLK(3);
         has = nhas; strip = nstrip; q0 = nq0; q1 = nq1;
         nhas = fhas; nstrip = fstrip; nq0 = fq0; nq1 = fq1;
+    }
+    if (a.inplace && tid == 0) {                   // the last CTA of the launch to finish re-arms the two counters
+        __threadfence();
+        if (atomicAdd(a.ipsync + 1, 1u) == gridDim.x - 1u) { a.ipsync[0] = 0u; a.ipsync[1] = 0u; }
     }
 }
 

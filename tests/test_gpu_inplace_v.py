@@ -2,8 +2,10 @@
 its whole-strip mode, csrc/vog_os.cu strip_copy_kernel; vog_plan_tune(34, 0/1)).
 
 A strip whose integer shifts are at most 24 rows is stored in place: the store of a pair of blocks waits until the
-windows of its neighbours are on chip, and the strip's first rows, which the last window reads again after the wrap,
-are kept in shared memory.  Other strips go through the plan's second grid and are copied back.  The arithmetic per pair
+windows of its neighbours are on chip, the strip's first rows, which the last window reads again after the wrap, are
+kept in shared memory, and the rows on either side of a piece of work that is not a whole strip are saved in a global
+scratch before any CTA starts such a piece (shapes below: 4096 x 1024 has left-over strips cut into shares, 512 x 8192
+four CTAs per strip).  Other strips go through the plan's second grid and are copied back.  The arithmetic per pair
 of blocks is that of the out-of-place kernel, so the result must be BIT-IDENTICAL to vog_shift_v_to on the same input,
 whatever the mix of strips (up to rounding in a column's last pair of blocks, see _same); against the oracle it is checked at the
 usual 2e-6 of max|f| (BASELINE.json north_star).
