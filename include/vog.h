@@ -191,7 +191,7 @@ int vog_run_host_async(vog_plan_t plan, float* f_host, double dt, int nsteps,
  *          of rho with the Green's function of the same Fourier solve (fp64) and the strip's first CTA publishes
  *          E (vog_get_field) and the energy share; a step is then 4 launches (x, density, v, x).  0 = density, Poisson
  *          kernel, v kernel (5 launches).  Same E up to rounding (the convolution is the more accurate of the two).
- *          On grids of 8192 columns or more, 1 (default) = the same convolution as a kernel of its own (one CTA per 64
+ *          On grids of 4096 columns or more, 1 (default) = the same convolution as a kernel of its own (one CTA per 64
  *          columns) in the place of the single-CTA Poisson kernel.
  *   31     v kernel (Nv >= 1024): 1 (default) = every group requests the rows of its first pair of blocks BEFORE the
  *          field / the shifts are known -- the raw buffer's whole 520 rows, which serve any integer shift in [-16, 16)

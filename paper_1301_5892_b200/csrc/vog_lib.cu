@@ -591,7 +591,7 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
 }
 
 // ------------------------------------------------------------------------------------------
-// S9 in x space (steps on grids of 8192 columns or more; the 2048-column grids do the same inside the v kernel, see
+// S9 in x space (steps on grids of 4096 columns or more; the 2048-column grids do the same inside the v kernel, see
 // osv7_kernel).  The Fourier solve of P:221 is a circular convolution, E_i = sum_j G_{i-j} rho_j, with the Green's function
 // G_n = (1/Nx) sum_{m != 0, Nx/2} e^{2 pi i m n / Nx} / (i k_m), k_m = 2 pi m / L (a plan constant, computed on the host
 // in fp64: green_host).  One CTA of 1024 threads per 64 columns instead of ONE CTA for the whole solve (poisson_kernel
@@ -599,7 +599,6 @@ __global__ void __launch_bounds__(1024) poisson_kernel(int Nx, const PoissonRadi
 // consecutive cells j) with a rolling window of G in registers -- one value of rho, one new value of G and eight
 // multiply-adds per cell, fp32 (<= 128 products per partial sum); the partial sums meet in fp64 in a fixed order.
 // rho comes from the density kernel's last blocks (ticket), minus rho_0, rounded to fp32 like poisson_kernel's input.
-// Shared arrays are padded by one word per 32 (chunk starts are multiples of 32 cells apart).
 __global__ void __launch_bounds__(1024) green_field_kernel(int Nx, const double* __restrict__ green,
                                                            const double* __restrict__ rho, float* __restrict__ E_a,
                                                            double* __restrict__ energy_out, double* __restrict__ e_part,
@@ -607,36 +606,51 @@ __global__ void __launch_bounds__(1024) green_field_kernel(int Nx, const double*
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double eS[8];
-    const int PN = Nx + (Nx >> 5);
+    // G padded by one word per 8 (index x + (x >> 3)): the 32 lanes of a warp -- 8 octets of columns x 4 chunks -- read
+    // G at distances 8 oct - JC jp, which this padding spreads over 32 different banks at Nx = 4096 and 8192 (two
+    // wavefronts remain at 16384); rho chunk by chunk with one word between chunks (chunk jp at jp (JC + 1)).
+    const int JC = Nx >> 7, PG = Nx + (Nx >> 3), PR = Nx + 128;
     float* const gS = reinterpret_cast<float*>(smem_raw);
-    float* const rS = gS + PN;
-    double* const sumS = reinterpret_cast<double*>(rS + PN);              // [32 warps][64 columns]
+    float* const rS = gS + PG;
+    double* const sumS = reinterpret_cast<double*>(rS + PR);              // [32 warps][64 columns]
     const int tid = threadIdx.x, xmask = Nx - 1;
-    for (int i = tid; i < Nx; i += 1024) gS[i + (i >> 5)] = (float)__ldg(green + i);      // (plan constant: before the wait)
+    for (int i = tid; i < Nx; i += 1024) gS[i + (i >> 3)] = (float)__ldg(green + i);      // (plan constant: before the wait)
     if (blockIdx.x == 0) VOG_STAMP(10);
     pdl_wait();                                   // rho comes from the density kernel
     pdl_launch_dependents();
     if (blockIdx.x == 0) VOG_STAMP(11);
     const double ref = __ldcg(rho);
-    for (int i = tid; i < Nx; i += 1024) rS[i + (i >> 5)] = (float)(__ldcg(rho + i) - ref);
+    const int jsh = 31 - __clz(JC);
+    for (int i = tid; i < Nx; i += 1024) rS[i + (i >> jsh)] = (float)(__ldcg(rho + i) - ref);
     __syncthreads();
     if (blockIdx.x == 0) VOG_STAMP(12);
-    const int oct = tid & 7, jp = tid >> 3, JC = Nx >> 7, j0 = jp * JC;
+    const int oct = tid & 7, jp = tid >> 3, j0 = jp * JC;
     const int gb = (int)blockIdx.x * 64 + 8 * oct + 7 - j0;               // index of G for column c0 + 7 at cell j0
+    const float* const rp = rS + jp * (JC + 1);
     float w[8], acc[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) acc[k] = 0.0f;                             // acc[k]: column 64 blockIdx.x + 8 oct + 7 - k
 #pragma unroll
-    for (int k = 0; k < 7; ++k) { const int gi = (gb - k) & xmask; w[k] = gS[gi + (gi >> 5)]; }
-#pragma unroll 8
-    for (int i = 0; i < JC; ++i) {
-        const int gi = (gb - 7 - i) & xmask, j = j0 + i;
-        w[7] = gS[gi + (gi >> 5)];
-        const float rj = rS[j + (j >> 5)];
+    for (int k = 0; k < 7; ++k) { const int gi = (gb - k) & xmask; w[k] = gS[gi + (gi >> 3)]; }
+    // cells in groups of eight: G indices gb - 7 - i run from a multiple of 8 downwards, so the first lies in one padded
+    // group of 8 and the other seven, contiguous, in the group below: two address computations per 8 cells
+#pragma unroll 1
+    for (int i0 = 0; i0 < JC; i0 += 8) {
+        const int g0 = (gb - 7 - i0) & xmask, g1 = (g0 - 1) & xmask;
+        const float* const q1 = gS + g1 + (g1 >> 3);
+        float gv[8];
+        gv[0] = gS[g0 + (g0 >> 3)];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) acc[k] = fmaf(w[k], rj, acc[k]);
+        for (int m = 1; m < 8; ++m) gv[m] = q1[1 - m];
 #pragma unroll
-        for (int k = 0; k < 7; ++k) w[k] = w[k + 1];
+        for (int m = 0; m < 8; ++m) {
+            w[7] = gv[m];
+            const float rj = rp[i0 + m];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) acc[k] = fmaf(w[k], rj, acc[k]);
+#pragma unroll
+            for (int k = 0; k < 7; ++k) w[k] = w[k + 1];
+        }
     }
     if (blockIdx.x == 0) VOG_STAMP(13);
     // the four chunks of a warp by shuffles, the 32 warps through shared memory
@@ -1532,7 +1546,7 @@ static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, dou
     const bool xspace = P->fuse_field && P->green && P->solver == 0;
     const bool fuse = xspace && Nx / 16 <= P->n_sm && P->os_v && P->method == 0 && P->osv_variant == 0 && src != dst;
     cudaError_t e;
-    if (xspace && !fuse && Nx >= 8192) {       // (at 4096 columns it only ties with the Poisson kernel: measured)
+    if (xspace && !fuse && Nx >= 4096) {
         // density (its last blocks write rho) -> green_field_kernel (E_self, energy) -> v-advection
         const bool pdl_was = t_pdl;
         t_pdl = pdl_was && P->density_pdl;
@@ -1540,7 +1554,7 @@ static cudaError_t field_then_v(vog_plan_s* P, const float* src, float* dst, dou
                        P->part, (double*)nullptr, 0.0, 0.0, reinterpret_cast<unsigned*>(P->e_part + Nx / 16 + 1), P->rho, dv);
         t_pdl = pdl_was;
         if (e != cudaSuccess) return e;
-        const size_t gsmem = sizeof(float) * 2 * (size_t)(Nx + Nx / 32) + sizeof(double) * 32 * 64;
+        const size_t gsmem = sizeof(float) * ((size_t)Nx + Nx / 8 + Nx + 128) + sizeof(double) * 32 * 64;
         e = set_max_smem((const void*)green_field_kernel, gsmem);
         if (e != cudaSuccess) return e;
         e = launch_pdl(green_field_kernel, dim3(Nx / 64), dim3(1024), gsmem, P->st, Nx, (const double*)P->green,

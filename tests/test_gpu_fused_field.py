@@ -2,7 +2,7 @@
 vog_plan_tune(30, 0/1)): on grids whose v kernel runs one piece per CTA (Nv >= 1024, Nx / 16 <= SMs) a step launches
 x, density, v, x -- no Poisson kernel; every v CTA computes E on its own 16 columns as the circular convolution of rho
 with the Green's function of the Fourier solve (E^_m = rho^_m / (i k_m), modes 0 and Nx/2 dropped).  On grids of
-8192 columns or more the same convolution is a kernel of its own (green_field_kernel, one CTA per 64 columns) in the
+4096 columns or more the same convolution is a kernel of its own (green_field_kernel, one CTA per 64 columns) in the
 single-CTA Poisson kernel's place.
 
 Checked here: the step and its field against the oracle (same tolerances as the unfused tests), against the unfused
@@ -68,7 +68,7 @@ def test_fused_field_step_against_oracle_and_unfused(torch, vog, oracle, idx, ov
     f1, E1, l1 = _steps(torch, vog, cfg, f, ext, n, True)
     f0, E0, l0 = _steps(torch, vog, cfg, f, ext, n, False)
     # one launch fewer per fused field solve (XVX: one per step; VXV: the first step's opening solve stays unfused);
-    # from 8192 columns on the x-space solve is a kernel of its own (green_field_kernel in the Poisson kernel's place)
+    # from 4096 columns on the x-space solve is a kernel of its own (green_field_kernel in the Poisson kernel's place)
     assert l0 - l1 == (n if cfg.Nx <= 2048 else 0)
     feq = oracle.Feq.make(cfg.feq)
     fo, Eo = f.astype(np.float64), None
