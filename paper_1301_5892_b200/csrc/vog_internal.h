@@ -127,7 +127,6 @@ struct OsArgs {
     float* dst2;           // ... second grid for the strips whose shifts do not
     int* strip_flags;      // ... [Nx / 16] 1 = the strip went to dst2 (cleared by the copy-back kernel)
     float* halo;           // ... [CTAs][4][2][40][16] rows on either side of the pieces that are not whole strips
-    unsigned* ipsync;      // ... [2] "halos saved" and "CTA done" counters (zero between launches)
 };
 
 struct OsSetupArgs {

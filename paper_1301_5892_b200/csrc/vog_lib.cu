@@ -747,8 +747,7 @@ struct vog_plan_s {
     int v_spec;                 // v kernel: first windows requested before the shifts are known (default 1)
     int v_inplace;              // vog_advect_v / vog_shift_v: the v kernel stores in place where the shifts allow it (default 1)
     int* strip_flags;           // [Nx / 16] strips of the last in-place v-advection that went to the second grid
-    float* ip_halo;             // [n_sm][4][2][40][16] boundary rows of the in-place v kernel's pieces; then 2 counters
-    size_t ip_halo_floats;
+    float* ip_halo;             // [n_sm][4][2][40][16] boundary rows of the in-place v kernel's pieces
     int density_pdl;            // density kernel launched with the programmatic-dependent-launch attribute (0 / 1)
     bool v_behind_field;        // ... set by field_then_v around its v launch
     bool v_inplace_now;         // set by advect_v_inplace around its v launch
@@ -1088,10 +1087,9 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
         if (nsm <= 0) nsm = 148;
-        const size_t hb = sizeof(float) * (size_t)nsm * 4 * 2 * 40 * 16 + 2 * sizeof(unsigned);
+        const size_t hb = sizeof(float) * (size_t)nsm * 4 * 2 * 40 * 16;
         alloc((void**)&P->ip_halo, hb);
         if (e == cudaSuccess) e = cudaMemsetAsync(P->ip_halo, 0, hb, P->st);
-        P->ip_halo_floats = (size_t)nsm * 4 * 2 * 40 * 16;
     }
     alloc((void**)&P->E_self, sizeof(float) * Nx);
     alloc((void**)&P->feq_tab, sizeof(float) * ((size_t)(ng ? ng : 1) * Nv + 512));   // + padding read (not used) by osv2_kernel
@@ -1370,7 +1368,7 @@ static cudaError_t run_osv(vog_plan_s* P, const float* src, float* dst, bool sou
         P->vsetup.spec = P->v_spec && P->v_behind_field;
         a.inplace = P->v_inplace_now ? 1 : 0;
         a.dst2 = P->g_buf; a.strip_flags = P->strip_flags;
-        a.halo = P->ip_halo; a.ipsync = reinterpret_cast<unsigned*>(P->ip_halo + P->ip_halo_floats);
+        a.halo = P->ip_halo;
         return osv7_launch(a, P->vsetup, geom, P->n_sm, P->st);
     }
     if (P->osv_variant == 2) {

@@ -323,6 +323,11 @@ cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_
     os2::VMaps maps;
     cudaError_t e = v_maps(a.src, a.Nx, a.Nv, &maps);
     if (e != cudaSuccess) return e;
+    if (a.inplace && (nstrips % grid != 0 || (nstrips < grid && grid / nstrips > 1))) {
+        // in place with pieces that are not whole strips: their boundary rows are saved by a launch of their own
+        e = launch_pdl(osv7_halo_kernel, dim3(grid), dim3(256), 0, st, a, 2 * (geom ? OS_VL : OS_V));
+        if (e != cudaSuccess) return e;
+    }
     if (geom) {
         e = set_max_smem((const void*)osv7_kernel<OS_VL, OS_HL>, smem);
         if (e != cudaSuccess) return e;

@@ -883,6 +883,61 @@ __device__ __forceinline__ void tensor_g2s(void* smem, const CUtensorMap* map, c
 }
 }
 
+// Work of CTA kb of G in osv7_kernel, piece i: (strip of 16 columns, pairs q0 .. q1-1); false = no such piece.  The
+// strips are dealt out round-robin in whole rounds of G strips (neighbouring CTAs work on neighbouring strips at the same
+// time); the strips left over after the last whole round are cut by PAIRS into G equal shares, so every CTA gets the
+// same number of pairs (+-1) whatever Nx / 16 is (8192: 512 strips on 148 CTAs were 4 rounds for 3.46 rounds of work).
+__device__ __forceinline__ bool osv7_piece(const int i, const int G, const int kb, const int nstrips, const int np,
+                                           int& strip, int& q0, int& q1)
+{
+    const int Rr = nstrips / G, Lt = nstrips - Rr * G;
+    if (i < Rr) { strip = i * G + kb; q0 = 0; q1 = np; return true; }
+    if (Rr == 0) {
+        // fewer strips than CTAs (grids up to 2048 columns): a share of pairs would straddle two strips and pay two
+        // tables for a handful of pairs; instead every strip gets floor(G / nstrips) CTAs, one segment each
+        const int m = G / nstrips, sidx = kb / nstrips, sg = (np + m - 1) / m;
+        strip = kb % nstrips;
+        q0 = sidx * sg;
+        q1 = min(np, q0 + sg);
+        return i == 0 && sidx < m && q0 < q1;
+    }
+    const int tlo = (int)((long long)Lt * np * kb / G), thi = (int)((long long)Lt * np * (kb + 1) / G);
+    int L = tlo;
+    for (int j = i - Rr;; --j) {
+        if (L >= thi) return false;
+        const int sidx = L / np;
+        q0 = L - sidx * np;
+        q1 = min(np, q0 + thi - L);
+        if (j == 0) { strip = Rr * G + sidx; return true; }
+        L += q1 - q0;
+    }
+}
+
+namespace os2 { constexpr int IPH = 40; }       // rows kept on either side of a piece of the in-place v kernel
+
+// In-place v-advection, first launch (only when the v kernel's pieces are not all whole strips): the rows on either side
+// of every such piece, which ANOTHER CTA of osv7_kernel will store, copied to a.halo [CTA][4][2][IPH][16] while the grid
+// is still untouched.  Same grid as osv7_kernel (CTA kb saves for CTA kb of that launch), 256 threads.
+static __global__ void __launch_bounds__(256) osv7_halo_kernel(const OsArgs a, const int V2)
+{
+    constexpr int W = os2::VW, IPH = os2::IPH;
+    pdl_wait();                                   // the grid comes from the kernel before
+    pdl_launch_dependents();
+    const int G = gridDim.x, kb = blockIdx.x, np = a.np, vmask = a.Nv - 1;
+    int s0, qa, qb, li = 0;
+    for (int i = 0; li < 4 && osv7_piece(i, G, kb, a.Nx / W, np, s0, qa, qb); ++i) {
+        if (qa == 0 && qb == np) continue;
+        float* const hs = a.halo + (size_t)(kb * 4 + li) * (2 * IPH * W);
+        const int lw = qa * V2, uw = qb < np ? qb * V2 : a.Nv;
+        for (int j = threadIdx.x; j < 2 * IPH * W; j += 256) {
+            const int side = j >= IPH * W, r = (j - side * IPH * W) >> 4, cc = j & (W - 1);
+            const int row = (side ? uw + r : lw - IPH + r) & vmask;
+            hs[j] = __ldcg(a.src + (size_t)row * a.Nx + s0 * W + cc);
+        }
+        ++li;
+    }
+}
+
 template <int V, int HLO>
 __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSetupArgs su,
                                                       const __grid_constant__ os2::VMaps maps)
@@ -933,10 +988,11 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     // for integer shifts up to IPB rows; a strip with larger shifts is written to the second grid a.dst2 instead and
     // flagged for the copy-back kernel (vog_os.cu strip_copy_kernel).
     // Pieces that are not whole strips (the balanced shares of the strips left over, or several CTAs per strip on narrow
-    // grids) border on rows that ANOTHER CTA stores: every CTA first copies the IPH rows on either side of its pieces
-    // into a.halo (global scratch) and arrives on a.ipsync; nobody starts such a piece before all have arrived, and a
-    // piece's first / last window takes the rows beyond its own range from there.
-    constexpr int IPH = 40, IPB = 24;
+    // grids) border on rows that ANOTHER CTA stores: a launch of osv7_halo_kernel in front of this one has copied the
+    // IPH rows on either side of every such piece into a.halo (global scratch), and a piece's first / last window takes
+    // the rows beyond its own range from there.  (A counter inside this kernel, on which every CTA arrives after saving
+    // its own halos, did the same in one launch -- and deadlocks when two such grids share the GPU.)
+    constexpr int IPH = os2::IPH, IPB = 24;
     __shared__ float saveS[IPH * W];
     __shared__ volatile int landedS[3];
     const float* hlo = nullptr;                    // rows [Lw - IPH, Lw) below the current piece (original values)
@@ -952,33 +1008,9 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         for (int i = tid; i < Nx; i += 768) fGreen[i] = (float)__ldg(su.green + i);
     if (tid < 5) asm volatile("prefetch.tensormap [%0];\n" ::"l"(reinterpret_cast<unsigned long long>(&maps.m[tid])) : "memory");
 
-    // Work of this CTA, in pieces (strip of 16 columns, pairs q0 .. q1-1).  The strips are dealt out round-robin in
-    // whole rounds of gridDim.x strips (neighbouring CTAs work on neighbouring strips at the same time); the strips
-    // left over after the last whole round are cut by PAIRS into gridDim.x equal shares, so every CTA gets the same
-    // number of pairs (+-1) whatever Nx / 16 is (8192: 512 strips on 148 CTAs were 4 rounds for 3.46 rounds of work).
     const int G = gridDim.x, kb = blockIdx.x, nstrips = Nx / W;
-    const int Rr = nstrips / G, Lt = nstrips - Rr * G;
-    const int tlo = (int)((long long)Lt * np * kb / G), thi = (int)((long long)Lt * np * (kb + 1) / G);
     auto piece = [&](const int i, int& strip, int& q0, int& q1) -> bool {
-        if (i < Rr) { strip = i * G + kb; q0 = 0; q1 = np; return true; }
-        if (Rr == 0) {
-            // fewer strips than CTAs (grids up to 2048 columns): a share of pairs would straddle two strips and pay two
-            // tables for a handful of pairs; instead every strip gets floor(G / nstrips) CTAs, one segment each
-            const int m = G / nstrips, sidx = kb / nstrips, sg = (np + m - 1) / m;
-            strip = kb % nstrips;
-            q0 = sidx * sg;
-            q1 = min(np, q0 + sg);
-            return i == 0 && sidx < m && q0 < q1;
-        }
-        int L = tlo;
-        for (int j = i - Rr;; --j) {
-            if (L >= thi) return false;
-            const int sidx = L / np;
-            q0 = L - sidx * np;
-            q1 = min(np, q0 + thi - L);
-            if (j == 0) { strip = Rr * G + sidx; return true; }
-            L += q1 - q0;
-        }
+        return osv7_piece(i, G, kb, nstrips, np, strip, q0, q1);
     };
     // S1 inside the kernel: the symbol table of a strip is COMPUTED here (no set-up kernel between the field solve and
     // this one).  Same arithmetic, entry for entry, as os_setup_v_kernel: beta, b, b* and the Everett / B-spline
@@ -1123,22 +1155,6 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     pdl_launch_dependents();
     OS_STAMP(1);
     OS_BLK(1);
-    if (a.inplace) {
-        int s0, qa, qb, li = 0;
-        for (int i = 0; li < 4 && piece(i, s0, qa, qb); ++i) {
-            if (qa == 0 && qb == np) continue;
-            float* const hs = a.halo + (size_t)(kb * 4 + li) * (2 * IPH * W);
-            const int lw = qa * (2 * V), uw = qb < np ? qb * (2 * V) : Nv;
-            for (int j = tid; j < 2 * IPH * W; j += 768) {
-                const int side = j >= IPH * W, r = (j - side * IPH * W) >> 4, cc = j & (W - 1);
-                const int row = (side ? uw + r : lw - IPH + r) & vmask;
-                hs[j] = __ldcg(a.src + (size_t)row * Nx + s0 * W + cc);
-            }
-            ++li;
-        }
-        __syncthreads();
-        if (tid == 0) { __threadfence(); atomicAdd(a.ipsync, 1u); }
-    }
     int li_cur = 0;                                // pieces of this CTA that were not whole strips, so far
     if (su.fpart) {
         // S9 for the 16 columns of this strip.  rho_i (the density kernel's last blocks wrote it: dv * the slab sums in
@@ -1251,9 +1267,6 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 hlo = a.halo + (size_t)(kb * 4 + min(li_cur, 3)) * (2 * IPH * W);
                 hup = hlo + IPH * W;
                 ++li_cur;
-                // every CTA has saved its halos before anybody stores into a strip that is shared between CTAs
-                if (tid == 0) while (*reinterpret_cast<volatile unsigned*>(a.ipsync) < gridDim.x) { }
-                __syncthreads();
             }
             if (tid < 3) landedS[tid] = -1;
             if (tid == 0 && !ipok) a.strip_flags[strip] = 1;
@@ -1398,10 +1411,6 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         OS_BLK(3);
         has = nhas; strip = nstrip; q0 = nq0; q1 = nq1;
         nhas = fhas; nstrip = fstrip; nq0 = fq0; nq1 = fq1;
-    }
-    if (a.inplace && tid == 0) {                   // the last CTA of the launch to finish re-arms the two counters
-        __threadfence();
-        if (atomicAdd(a.ipsync + 1, 1u) == gridDim.x - 1u) { a.ipsync[0] = 0u; a.ipsync[1] = 0u; }
     }
 }
 

@@ -123,3 +123,32 @@ def test_inplace_advect_v_with_source_matches_the_step_kernel(torch, vog, oracle
     scale = max(float(np.abs(f).max()), 1e-2)
     assert np.abs(fd.cpu().numpy() - ref).max() <= TOL * scale
     plan.destroy()
+
+
+@pytest.mark.timeout(300)
+def test_inplace_v_on_several_streams_at_once(torch, vog):
+    """In-place calls of three plans on three streams share the GPU: no CTA may wait for another CTA of its grid to
+    become resident (an earlier version synchronised the halo saving through a counter inside the kernel and would hang
+    here: each grid holds SMs the other grids' remaining CTAs need).  Results as for one stream."""
+    Nx, Nv = 4096, 4096
+    rng = np.random.default_rng(9)
+    beta = _dev(torch, rng.uniform(-8.0, 8.0, Nx))
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    plans = [vog.Plan(Nx, Nv, 1.0, -1.0, 1.0, 0, 17, stream=s) for s in streams]
+    f0 = torch.rand((Nv, Nx), device="cuda")
+    ref = torch.empty_like(f0)
+    plans[0].shift_v_to(f0, ref, beta)
+    torch.cuda.synchronize()
+    fs = [f0.clone() for _ in plans]
+    torch.cuda.synchronize()
+    for p_, f_ in zip(plans, fs):
+        p_.shift_v(f_, beta)
+    torch.cuda.synchronize()
+    for f_ in fs:
+        assert _same(torch, f_, ref, Nv, 0)
+    for rep in range(10):                        # and again, back to back on all three
+        for p_, f_ in zip(plans, fs):
+            p_.shift_v(f_, beta)
+    torch.cuda.synchronize()
+    for p_ in plans:
+        p_.destroy()
