@@ -108,9 +108,11 @@ def test_inplace_v_against_the_oracle(torch, vog, oracle, kind):
     plan.destroy()
 
 
-def test_inplace_advect_v_with_source_matches_the_step_kernel(torch, vog, oracle):
-    """vog_advect_v (delta-f source included) in place on the bench grid against the oracle's advect_v."""
-    cfg = inputs.metric_config()
+@pytest.mark.parametrize("shape", [None, (4096, 1024), (512, 4096)])
+def test_inplace_advect_v_with_source_matches_the_step_kernel(torch, vog, oracle, shape):
+    """vog_advect_v (delta-f source included) in place against the oracle's advect_v: the bench grid (whole strips), a
+    grid with left-over strips cut into shares and one with several CTAs per strip."""
+    cfg = inputs.metric_config() if shape is None else inputs.config(1, Nx=shape[0], Nv=shape[1])
     f = inputs.initial_f(cfg)
     rng = np.random.default_rng(2)
     E = (0.3 * np.sin(2 * np.pi * np.arange(cfg.Nx) / cfg.Nx) + 0.05 * rng.standard_normal(cfg.Nx)).astype(np.float32)
