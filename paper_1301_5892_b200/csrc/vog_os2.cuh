@@ -1296,10 +1296,12 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         if (a.inplace && whole)                    // (behind the first requests: the table barrier below orders it before any store)
             for (int i = tid; i < IPH * W; i += 768)
                 saveS[i] = __ldcg(a.src + (size_t)(i >> 4) * Nx + g.c0 + (i & (W - 1)));
-        if (tid < 6 * a.ng * W) {
+        if (tid >= 768 - 6 * a.ng * W) {
             // delta-f source constants of (Gaussian gg, column cc): same expressions as osv2_source without a table,
-            // one transcendental per thread (two warps computing all six per entry were the slowest of this phase)
-            const int which = tid / (a.ng * W), i = tid - which * (a.ng * W), cc = i & (W - 1), gg = i >> 4;
+            // one transcendental per thread (two warps computing all six per entry were the slowest of this phase), in
+            // the CTA's last threads, which have two table entries below instead of three
+            const int ti = tid - (768 - 6 * a.ng * W);
+            const int which = ti / (a.ng * W), i = ti - which * (a.ng * W), cc = i & (W - 1), gg = i >> 4;
             const float cgs = a.cg4[gg] * rec[19 * W + cc];
             const float hh = 32.0f * cgs * a.dvf, hv = 2.0f * (float)V * cgs * a.dvf;
             const float arg = which < 2 ? hh : (which < 4 ? -hh : hv);
@@ -1307,35 +1309,42 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             if (which < 4) reinterpret_cast<float*>(srcRS)[4 * i + which] = val;
             else reinterpret_cast<float*>(srcRV)[2 * i + (which - 4)] = val;
         }
-        // ---- the strip's table: 130 x 16 entries
-        for (int idx = tid; idx < OS_LAMW * W; idx += 768) {
-            const int kk = idx >> 4, cc = idx & 15;
-            float2 o;
-            if (kk == 129) o = make_float2(rec[18 * W + cc], rec[19 * W + cc]);
-            else if (kk == 0) o = make_float2(1.0f / (float)OS_LB, 0.0f);          // lambda_0 = sum of the weights = 1
-            else {
-                const float4 cs = csS[kk];
-                const float cf = cs.x, sn = cs.y;
-                float lr, li;
-                if (su.spline) {
-                    const float Bm1 = rec[cc], B0 = rec[W + cc], B1 = rec[2 * W + cc], B2 = rec[3 * W + cc];
-                    const float gg = 3.0f / (2.0f + cf);
-                    lr = fmaf(B2, cs.z, fmaf(Bm1 + B1, cf, B0)) * gg;
-                    li = fmaf(B2, cs.w, (B1 - Bm1) * sn) * gg;
-                } else {
-                    const float sv = cs.z;
-                    float h0 = 0.0f, h1 = 0.0f;
+        // ---- the strip's table: 130 x 16 entries.  A thread's entries all belong to column tid & 15 (768 is a multiple
+        // of 16): its 18 coefficients are read once.
+        {
+            const int cc = tid & 15;
+            float cfr[18];
 #pragma unroll
-                    for (int j = 8; j >= 0; --j) {
-                        h0 = fmaf(h0, sv, rec[j * W + cc]);
-                        h1 = fmaf(h1, sv, rec[(9 + j) * W + cc]);
+            for (int j = 0; j < 18; ++j) cfr[j] = rec[j * W + cc];
+#pragma unroll 1
+            for (int kk = tid >> 4; kk < OS_LAMW; kk += 48) {
+                float2 o;
+                if (kk == 129) o = make_float2(rec[18 * W + cc], rec[19 * W + cc]);
+                else if (kk == 0) o = make_float2(1.0f / (float)OS_LB, 0.0f);          // lambda_0 = sum of the weights = 1
+                else {
+                    const float4 cs = csS[kk];
+                    const float cf = cs.x, sn = cs.y;
+                    float lr, li;
+                    if (su.spline) {
+                        const float Bm1 = cfr[0], B0 = cfr[1], B1 = cfr[2], B2 = cfr[3];
+                        const float gg = 3.0f / (2.0f + cf);
+                        lr = fmaf(B2, cs.z, fmaf(Bm1 + B1, cf, B0)) * gg;
+                        li = fmaf(B2, cs.w, (B1 - Bm1) * sn) * gg;
+                    } else {
+                        const float sv = cs.z;
+                        float h0 = 0.0f, h1 = 0.0f;
+#pragma unroll
+                        for (int j = 8; j >= 0; --j) {
+                            h0 = fmaf(h0, sv, cfr[j]);
+                            h1 = fmaf(h1, sv, cfr[9 + j]);
+                        }
+                        lr = fmaf(cf, h1, h0);
+                        li = sn * h1;
                     }
-                    lr = fmaf(cf, h1, h0);
-                    li = sn * h1;
+                    o = make_float2(lr * (1.0f / (float)OS_LB), li * (1.0f / (float)OS_LB));
                 }
-                o = make_float2(lr * (1.0f / (float)OS_LB), li * (1.0f / (float)OS_LB));
+                lamS[kk * W + cc] = o;
             }
-            lamS[idx] = o;
         }
         OS_STAMP(42);
         __syncthreads();                           // table visible to everybody
