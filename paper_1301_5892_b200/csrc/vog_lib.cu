@@ -997,6 +997,10 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
         P->os2x_lpi = l2; P->os3x_occ = 0; P->os2v_gpc = 0;
+        // lines of 1024 / 2048 cells: the whole-line kernel (osx6_kernel).  Alone it is as fast as the per-pair-window
+        // kernel (12.3 us at 2048^2), in the chain of a step it is 0.55 us per step faster at both sizes (measured on
+        // the metric grid: 46.44 -> 45.85 us); from 4096 cells on the window kernel wins (141.7 against 144.0 us).
+        P->osx_variant = Nx <= 2048 ? 1 : 0;
     }
     // measured (profiles/r1i_pdl_setup.md): 512^2 step -20 %, 2048^2 -15 %, 8192^2 +-0; the +1.3 % at 16384^2 of round 1
     // was the density kernel (launched without the attribute on large grids since, see density_pdl): now -0.5..-4 %
