@@ -997,10 +997,12 @@ extern "C" int vog_plan(vog_plan_t* out, const vog_params_t* p, void* cuda_strea
         while (l2 > 1 && (Nv + l2 - 1) / l2 < P->n_sm * 3) --l2;
         P->os_geom = p->kind == VOG_LAGRANGE ? 1 : 0;
         P->os2x_lpi = l2; P->os3x_occ = 0; P->os2v_gpc = 0;
-        // lines of 1024 / 2048 cells: the whole-line kernel (osx6_kernel).  Alone it is as fast as the per-pair-window
-        // kernel (12.3 us at 2048^2), in the chain of a step it is 0.55 us per step faster at both sizes (measured on
-        // the metric grid: 46.44 -> 45.85 us); from 4096 cells on the window kernel wins (141.7 against 144.0 us).
-        P->osx_variant = Nx <= 2048 ? 1 : 0;
+        // Which x kernel (measured at the end of round 2, same box, vog_plan_tune(21, .)): lines of 1024 / 2048 cells: the
+        // whole-line kernel osx6_kernel -- alone as fast as the per-pair-window kernel osx7_kernel (12.3 us at 2048^2),
+        // in the chain of a step 0.55 us per step faster (46.44 -> 45.85 us); 4096 cells: osx7_kernel (step 134.7
+        // against 136.2 us); 8192 cells: osx6_kernel again (116.5 against 121.7 us per launch, step 432 against 441 us);
+        // 16384 cells need two rounds per line, which only osx6_kernel does.
+        P->osx_variant = Nx == 4096 ? 0 : 1;
     }
     // measured (profiles/r1i_pdl_setup.md): 512^2 step -20 %, 2048^2 -15 %, 8192^2 +-0; the +1.3 % at 16384^2 of round 1
     // was the density kernel (launched without the attribute on large grids since, see density_pdl): now -0.5..-4 %
