@@ -1258,7 +1258,8 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         const bool whole = q0 == 0 && q1 == np;
         if (a.inplace) {
             const int sb = ((g.base + (Nv >> 1)) & vmask) - (Nv >> 1);     // first window row as a signed shift
-            ipok = !g.gather && sb >= (whole ? -4 * IPB : 8 - IPH) && sb + (g.nrows - (V + OS_LB)) <= IPB;
+            // (a piece's first window starts HLO - sb rows below the piece: at most the IPH rows of the lower halo)
+            ipok = !g.gather && sb >= (whole ? -4 * IPB : HLO - IPH) && sb + (g.nrows - (V + OS_LB)) <= IPB;
             Lw = q0 * (2 * V);
             Uw = q1 < np ? q1 * (2 * V) : Nv;
             if (whole) {

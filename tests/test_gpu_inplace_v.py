@@ -60,6 +60,12 @@ def _betas(Nx, kind, seed):
         return rng.uniform(-30.0, 30.0, Nx)
     if kind == "negative":         # large negative shifts stay in place (only the wrap after the last row is bounded)
         return rng.uniform(-90.0, 5.0, Nx)
+    if kind == "lowedge":          # strips whose first window just fits / just misses the rows kept below a piece
+        b = np.empty(Nx)
+        for s0 in range(0, Nx, 16):
+            lo = [-33.5, -31.5, -27.5, -25.5, -23.5, -19.5][(s0 // 16) % 6]
+            b[s0:s0 + 16] = lo + rng.uniform(0.0, 6.0, 16)
+        return b
     if kind == "mixed":            # some strips far outside (second grid), some with a wide spread (per-lane landing)
         b = rng.uniform(-6.0, 6.0, Nx)
         b[Nx // 8:Nx // 4] += 300.0
@@ -69,7 +75,7 @@ def _betas(Nx, kind, seed):
     raise ValueError(kind)
 
 
-@pytest.mark.parametrize("kind", ["small", "edge", "negative", "mixed"])
+@pytest.mark.parametrize("kind", ["small", "edge", "lowedge", "negative", "mixed"])
 @pytest.mark.parametrize("Nx,Nv,ikind,order", [(2048, 2048, 0, 17), (4096, 1024, 0, 9), (1024, 4096, 1, 3), (512, 8192, 0, 3)])
 def test_inplace_v_is_bit_identical_to_out_of_place(torch, vog, Nx, Nv, ikind, order, kind):
     rng = np.random.default_rng(5)
