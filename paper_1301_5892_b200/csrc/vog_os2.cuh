@@ -995,9 +995,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     constexpr int IPH = os2::IPH, IPB = 24;
     __shared__ float saveS[IPH * W];
     __shared__ volatile int landedS[3];
-    const float* hlo = nullptr;                    // rows [Lw - IPH, Lw) below the current piece (original values)
-    const float* hup = saveS;                      // rows [Uw, Uw + IPH) above it (whole strips: the strip's first rows)
-    int Lw = 0, Uw = Nv;                           // first row of the piece, first row behind it (unwrapped)
+    // the rows around a piece: lo = rows [Lw - IPH, Lw) below it, up = rows [Uw, Uw + IPH) behind it (original values;
+    // whole strips: up = the strip's first rows in saveS); Lw = first row of the piece, Uw = first row behind it (unwrapped)
+    struct Halo { const float* lo; const float* up; int Lw, Uw; };
+    Halo hcur = {nullptr, saveS, 0, Nv};
     __shared__ float fusedE[W];
     __shared__ float4 srcRS[4 * W];               // delta-f source: (e^h, expm1 h, e^-h, expm1 -h), h = 16 rows, per (Gaussian, column)
     __shared__ float2 srcRV[4 * W];               // ... and (e^{g V}, expm1(g V)): block B from block A
@@ -1094,7 +1095,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     };
     // request the raw rows of pair p: the union of the rows, unshifted (or, in the fallback, every lane its own rows)
     // mode (in place only): 1 = the rows below the piece come from hlo, 2 = the rows behind it from hup
-    auto land = [&](const Geo& g, const int p, const int mode = 0) {
+    auto land = [&](const Geo& g, const int p, const int mode, const Halo& hl) {
+        const float* const hlo = hl.lo;
+        const float* const hup = hl.up;
+        const int Lw = hl.Lw, Uw = hl.Uw;
         const int rs = p * (2 * V) - HLO + g.base;
         if (!g.gather) {
             // unwrapped first row of the window (the shift as a signed number), rows from the two halos
@@ -1148,7 +1152,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     if (su.spec && has && q0 + gid < q1) {
         Geo gs;
         gs.c0 = strip * W; gs.base = -SPEC; gs.nrows = RR; gs.db = 0; gs.gather = false;
-        land(gs, q0 + gid);
+        land(gs, q0 + gid, 0, hcur);
         spec = true;
     }
     pdl_wait();                                   // the field (or rho) comes from the kernel before
@@ -1260,13 +1264,14 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             const int sb = ((g.base + (Nv >> 1)) & vmask) - (Nv >> 1);     // first window row as a signed shift
             // (a piece's first window starts HLO - sb rows below the piece: at most the IPH rows of the lower halo)
             ipok = !g.gather && sb >= (whole ? -4 * IPB : HLO - IPH) && sb + (g.nrows - (V + OS_LB)) <= IPB;
-            Lw = q0 * (2 * V);
-            Uw = q1 < np ? q1 * (2 * V) : Nv;
+            hcur.Lw = q0 * (2 * V);
+            hcur.Uw = q1 < np ? q1 * (2 * V) : Nv;
             if (whole) {
-                hup = saveS;
+                hcur.lo = nullptr;
+                hcur.up = saveS;
             } else {
-                hlo = a.halo + (size_t)(kb * 4 + min(li_cur, 3)) * (2 * IPH * W);
-                hup = hlo + IPH * W;
+                hcur.lo = a.halo + (size_t)(kb * 4 + min(li_cur, 3)) * (2 * IPH * W);
+                hcur.up = hcur.lo + IPH * W;
                 ++li_cur;
             }
             if (tid < 3) landedS[tid] = -1;
@@ -1289,10 +1294,10 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             else {                                 // (uniform over the CTA: every half-warp sees the same 16 columns)
                 os2::mbar_wait(vbar, vpar); vpar ^= 1u;
                 os2::bar_group(gid + 1);           // (nobody of the group may still be waiting when the barrier is re-armed)
-                land(g, p0);
+                land(g, p0, 0, hcur);
             }
             spec = false;
-        } else if (!pref && p0 < q1) land(g, p0, lmode(p0));
+        } else if (!pref && p0 < q1) land(g, p0, lmode(p0), hcur);
         pref = false;
         if (a.inplace && whole)                    // (behind the first requests: the table barrier below orders it before any store)
             for (int i = tid; i < IPH * W; i += 768)
@@ -1381,8 +1386,25 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             OS_STAMP(6 + 4 * ((p - p0) / 3));
             // the next window lands behind the middle stage and the inverse pass: this piece's, or -- after the group's
             // last pair of the piece -- the group's first of the NEXT piece (its shifts are known two pieces ahead)
-            if (p + 3 < q1) land(g, p + 3, lmode(p + 3));
-            else if (nhas && np0 < nq1 && !(a.inplace && !(nq0 == 0 && nq1 == np))) { land(gn, np0); pref = true; }
+            if (p + 3 < q1) land(g, p + 3, lmode(p + 3), hcur);
+            else if (nhas && np0 < nq1) {
+                // the group's first window of the NEXT piece.  In place, a piece that is not a whole strip takes the rows
+                // beyond its range from its halo slot (saved before this kernel started), if its shifts allow in-place
+                // storing at all -- the same test as at the top of the piece, on the next piece's geometry.
+                int nmode = 0;
+                Halo hn = hcur;
+                if (a.inplace && !(nq0 == 0 && nq1 == np)) {
+                    const int sbn = ((gn.base + (Nv >> 1)) & vmask) - (Nv >> 1);
+                    const bool okn = !gn.gather && sbn >= HLO - IPH && sbn + (gn.nrows - (V + OS_LB)) <= IPB;
+                    hn.lo = a.halo + (size_t)(kb * 4 + min(li_cur, 3)) * (2 * IPH * W);
+                    hn.up = hn.lo + IPH * W;
+                    hn.Lw = nq0 * (2 * V);
+                    hn.Uw = nq1 < np ? nq1 * (2 * V) : Nv;
+                    if (okn) nmode = (np0 == nq0 ? 1 : 0) | (np0 == nq1 - 1 ? 2 : 0);
+                }
+                land(gn, np0, nmode, hn);
+                pref = true;
+            }
             // ---- middle stage (item g = h): positions 16 g + j
             {
                 float2* const sp = exch + h * 16 * W + c;
