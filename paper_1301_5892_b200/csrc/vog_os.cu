@@ -328,14 +328,20 @@ cudaError_t osv7_launch(const OsArgs& a, const OsSetupArgs& su, int geom, int n_
         e = launch_pdl(osv7_halo_kernel, dim3(grid), dim3(256), 0, st, a, 2 * (geom ? OS_VL : OS_V));
         if (e != cudaSuccess) return e;
     }
+#define VOG_OSV7_LAUNCH(VV, HH, IPF)                                                                     \
+    do {                                                                                                 \
+        e = set_max_smem((const void*)osv7_kernel<VV, HH, IPF>, smem);                                   \
+        if (e != cudaSuccess) return e;                                                                  \
+        return launch_pdl(osv7_kernel<VV, HH, IPF>, dim3(grid), dim3(768), smem, st, a, su, maps);       \
+    } while (0)
+    const bool flag_at_run_time = a.inplace || a.Nx <= 2048;       // (see the kernel's template comment)
     if (geom) {
-        e = set_max_smem((const void*)osv7_kernel<OS_VL, OS_HL>, smem);
-        if (e != cudaSuccess) return e;
-        return launch_pdl(osv7_kernel<OS_VL, OS_HL>, dim3(grid), dim3(768), smem, st, a, su, maps);
+        if (flag_at_run_time) VOG_OSV7_LAUNCH(OS_VL, OS_HL, 2);
+        VOG_OSV7_LAUNCH(OS_VL, OS_HL, 0);
     }
-    e = set_max_smem((const void*)osv7_kernel<OS_V, OS_H>, smem);
-    if (e != cudaSuccess) return e;
-    return launch_pdl(osv7_kernel<OS_V, OS_H>, dim3(grid), dim3(768), smem, st, a, su, maps);
+    if (flag_at_run_time) VOG_OSV7_LAUNCH(OS_V, OS_H, 2);
+    VOG_OSV7_LAUNCH(OS_V, OS_H, 0);
+#undef VOG_OSV7_LAUNCH
 }
 
 // In-place v-advection, second launch: the strips that osv7_kernel could not store in place (integer shifts beyond its

@@ -938,7 +938,12 @@ static __global__ void __launch_bounds__(256) osv7_halo_kernel(const OsArgs a, c
     }
 }
 
-template <int V, int HLO>
+// IPM = 0: out of place only, the in-place bookkeeping compiled out (grids of 4096 columns or more: with the run-time
+// flag the out-of-place kernel was 2.3 % slower at 8192^2 than before the mode existed, 131.4 against 128.5 us; this
+// instance takes 127.4 us); IPM = 2: a.inplace decides at run time (in-place calls, and the grids up to 2048 columns,
+// where the compile-time instance made the 2048^2 step 2.1 us SLOWER: 46.15 -> 48.27 us, same box -- code generation
+// of the prologue, not the flag).
+template <int V, int HLO, int IPM = 2>
 __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSetupArgs su,
                                                       const __grid_constant__ os2::VMaps maps)
 {
@@ -966,6 +971,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
     }
     const int c = gt & 15, h = gt >> 4;                                           // column of the strip, item index
     const int Nx = a.Nx, Nv = a.Nv, vmask = Nv - 1, np = a.np;
+    const bool IP = IPM == 2 ? a.inplace != 0 : false;
     // (the FP32 pipe is what this kernel waits for most: the 15 twiddles of an item come from a 1.9 KB table in
     // shared memory, 15 loads per pass, instead of 11 complex products of four register-resident powers)
     for (int i = tid; i < 240; i += 768) twS[i] = __ldg(a.tw + i);               // (plan constants: before the wait)
@@ -1260,7 +1266,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         const int p0 = q0 + gid;
         bool ipok = false;
         const bool whole = q0 == 0 && q1 == np;
-        if (a.inplace) {
+        if (IP) {
             const int sb = ((g.base + (Nv >> 1)) & vmask) - (Nv >> 1);     // first window row as a signed shift
             // (a piece's first window starts HLO - sb rows below the piece: at most the IPH rows of the lower halo)
             ipok = !g.gather && sb >= (whole ? -4 * IPB : HLO - IPH) && sb + (g.nrows - (V + OS_LB)) <= IPB;
@@ -1280,7 +1286,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         // which halos the window of pair p takes (in place): whole strips only the wrap behind the last row, and only for
         // windows requested after the strip's first stores; other pieces both sides, always
         auto lmode = [&](const int p) -> int {
-            if (!ipok) return 0;
+            if (!IP || !ipok) return 0;
             if (whole) return p >= q0 + 3 ? 2 : 0;
             return (p == q0 ? 1 : 0) | (p == q1 - 1 ? 2 : 0);
         };
@@ -1299,7 +1305,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
             spec = false;
         } else if (!pref && p0 < q1) land(g, p0, lmode(p0), hcur);
         pref = false;
-        if (a.inplace && whole)                    // (behind the first requests: the table barrier below orders it before any store)
+        if (IP && whole)                           // (behind the first requests: the table barrier below orders it before any store)
             for (int i = tid; i < IPH * W; i += 768)
                 saveS[i] = __ldcg(a.src + (size_t)(i >> 4) * Nx + g.c0 + (i & (W - 1)));
         if (tid >= 768 - 6 * a.ng * W) {
@@ -1363,11 +1369,11 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
         Geo gn = g;
         if (nhas) gn = geometry(nstrip * W, cfS + ((it + 1) % 3) * CF);
         const int np0 = nq0 + gid;
-        float* const ocol = ((a.inplace && !ipok) ? a.dst2 : a.dst) + g.c0 + c;
+        float* const ocol = ((IP && !ipok) ? a.dst2 : a.dst) + g.c0 + c;
         for (int p = p0; p < q1; p += 3) {
             if (g.gather) os2::cp_async_wait_all();
             else { os2::mbar_wait(vbar, vpar); vpar ^= 1u; }
-            if (ipok && gt == 0) landedS[gid] = p;
+            if (IP && ipok && gt == 0) landedS[gid] = p;
             OS_STAMP(5 + 4 * ((p - p0) / 3));
             os2::bar_group(gid + 1);               // raw rows of pair p visible; exchange buffer of the last pair read
             // ---- pass A (item t = h): samples from the raw rows with this lane's offset
@@ -1393,7 +1399,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
                 // storing at all -- the same test as at the top of the piece, on the next piece's geometry.
                 int nmode = 0;
                 Halo hn = hcur;
-                if (a.inplace && !(nq0 == 0 && nq1 == np)) {
+                if (IP && !(nq0 == 0 && nq1 == np)) {
                     const int sbn = ((gn.base + (Nv >> 1)) & vmask) - (Nv >> 1);
                     const bool okn = !gn.gather && sbn >= HLO - IPH && sbn + (gn.nrows - (V + OS_LB)) <= IPB;
                     hn.lo = a.halo + (size_t)(kb * 4 + min(li_cur, 3)) * (2 * IPH * W);
@@ -1415,7 +1421,7 @@ __global__ void __launch_bounds__(768, 1) osv7_kernel(const OsArgs a, const OsSe
 #pragma unroll
                 for (int j = 0; j < 16; ++j) sp[j * W] = x[j];
             }
-            if (ipok && gt == 0) {                 // in place: the neighbours' windows must be on chip before these rows change
+            if (IP && ipok && gt == 0) {           // in place: the neighbours' windows must be on chip before these rows change
                 // (publishing a group's window in flight as soon as its barrier completes, instead of when the group
                 // gets to it, was measured: 144 -> 149 us at 8192^2, the polling costs more than the wait)
                 if (p + 1 < q1) while (landedS[(gid + 1) % 3] < p + 1) { }
