@@ -245,11 +245,13 @@ __device__ __forceinline__ void os2_store_x_full(float* __restrict__ o, const in
     }
 }
 
-template <int V, int HLO>
+// LPI = 2: two lines per group as a compile-time constant AND one round with every thread busy (32 np == blockDim.x: the
+// host checks it); LPI = 0: everything at run time (one line per group at 8192 cells, two rounds per group at 16384).
+template <int V, int HLO, int LPI = 0>
 __global__ void __launch_bounds__(288, 3) osx6_kernel(const OsArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int lpi = a.lpi, np = a.np, nitem = lpi * np * 16;
+    const int lpi = LPI ? LPI : a.lpi, np = a.np, nitem = LPI ? (int)blockDim.x : lpi * np * 16;
     const int tid = threadIdx.x, T = blockDim.x, t = tid & 15;
     const int N = a.N, mask = N - 1, LS = N + os2::XPAD;
     float* const lines = reinterpret_cast<float*>(smem_raw);                       // lpi lines of LS floats
@@ -295,9 +297,10 @@ __global__ void __launch_bounds__(288, 3) osx6_kernel(const OsArgs a)
 #pragma unroll 1
         for (int it0 = 0; it0 < nitem; it0 += T) {                      // rounds (one when the group fits the CTA)
             const int it = it0 + tid;
-            const bool active = it < nitem;
+            const bool active = LPI ? true : it < nitem;
             const int pr = it >> 4;
-            const int l = (int)(((unsigned)pr * a.inv_np) >> 16), pp = pr - l * np;   // line of the group, pair of the line
+            const int l = LPI == 2 ? (pr >= np ? 1 : 0) : (int)(((unsigned)pr * a.inv_np) >> 16);
+            const int pp = pr - l * np;                                               // line of the group, pair of the line
             const float2* const lamL = lamG + l * OS_LAMW;
             // ---- pass A from the line in shared memory
             if (active) {
