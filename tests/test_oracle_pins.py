@@ -265,6 +265,27 @@ def test_field_equals_fft_solve(oracle):
     assert abs(oracle.electric_energy(expect, L) - 0.5 * (L / Nx) * (expect ** 2).sum()) < 1e-15
 
 
+def test_field_is_the_circular_convolution_with_its_green_function(oracle):
+    """the Fourier solve is linear and translation invariant, so E = G (*) rho with G = the field of a unit point
+    density; G is real, odd about cell 0 (1/(ik) is odd and imaginary), has zero mean, and its closed form is
+    G_n = L/(pi Nx) sum_{m=1}^{Nx/2-1} sin(2 pi m n / Nx)/m (modes 0 and Nx/2 dropped, reading Q12).  The GPU path's
+    x-space field solve (csrc: field_then_v) computes exactly this convolution; here the ORACLE is held to it."""
+    rng = np.random.default_rng(21)
+    Nx, L = 96, 5.0
+    delta = np.zeros(Nx)
+    delta[0] = 1.0
+    G = oracle.poisson(delta, L)
+    n = np.arange(Nx)
+    closed = np.array([sum(math.sin(2 * math.pi * m * k / Nx) / m for m in range(1, Nx // 2)) for k in n]) * L / (math.pi * Nx)
+    assert np.abs(G - closed).max() < 1e-13
+    assert abs(G[0]) < 1e-15 and np.abs(G[1:] + G[:0:-1]).max() < 1e-14 and abs(G.mean()) < 1e-15
+    rho = rng.random(Nx)
+    conv = np.array([sum(G[(i - j) % Nx] * rho[j] for j in range(Nx)) for i in range(Nx)])
+    assert np.abs(oracle.poisson(rho, L) - conv).max() < 1e-13
+    # translation: shifting rho by 7 cells shifts E by 7 cells
+    assert np.abs(oracle.poisson(np.roll(rho, 7), L) - np.roll(oracle.poisson(rho, L), 7)).max() < 1e-13
+
+
 def test_delta_f_source_is_plain_difference(oracle):
     """P:197 with zero delta-f: the update is f_eq(v - dt E) - f_eq(v)."""
     cfg = inputs.config(1, Nx=16, Nv=32)
